@@ -1,0 +1,478 @@
+"""Synthetic DDC phantoms: geometry, fields, COO generator, fluence draws.
+
+Readings of BASELINE.json `configs` that the text leaves open:
+
+D1 geometry   Grid centred on the isocentre, voxel centre ((ix-(nx-1)/2)h, ...);
+              z is the rotation axis; the body is an elliptic cylinder for all z;
+              rows of D are the in-body voxels only, compact index in x-fastest
+              raster order.  Parallel beam: travel direction b=(cos t, sin t, 0),
+              lateral axis e_l=(-sin t, cos t, 0).  Collimator 0: leaves travel
+              along e_l, leaf rows are stacked along z.  Collimator 90 (second
+              arc of config 3): leaves travel along z, rows stacked along e_l.
+D2 field      config 0: the stated 8x8 rectangle.  Others: ragged field - per
+              leaf row the contiguous span from the leftmost to the rightmost
+              beamlet whose square meets the union of the projected target
+              discs, plus one margin beamlet each side; rows that see no target
+              hold 0 beamlets.  Columns: angle-major, leaf row, left->right.
+D3 r, depth   r = distance from the voxel centre to the beamlet's central ray;
+              depth = distance along b from where the ray THROUGH THE VOXEL
+              CENTRE enters the body ellipse to the voxel.
+D4 value      exp(-mu depth) exp(-r^2/(2 sigma^2)) + 1e-3 u, u in [0,1) from a
+              counter-based hash of (seed, voxel, beamlet); FP64, rounded once
+              to FP32; kept iff r <= cutoff and value >= 1e-4.
+D5 config 3   body semi-axes 140 x 110 mm (the config names none).
+D6 seeds      seed_ddc = 150301721 + cfg, seed_geom = 1503 + cfg,
+              seed_x = 1721*1000 + eval_index.
+D7 objective  target T=70 w+=w-=1; OAR T=30 w+=0.2 w-=0; body T=50 w+=0.05 w-=0.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+from typing import List, Optional, Sequence, Tuple
+
+import torch
+
+_M32 = 0xFFFFFFFF
+
+
+# --------------------------------------------------------------------------
+# counter-based hash -> uniform [0,1)   (same bits for python ints and tensors)
+# --------------------------------------------------------------------------
+def _mix32_int(h: int) -> int:
+    h &= _M32
+    h ^= h >> 16
+    h = (h * 0x85EBCA6B) & _M32
+    h ^= h >> 13
+    h = (h * 0xC2B2AE35) & _M32
+    h ^= h >> 16
+    return h
+
+
+def _mix32_t(h: torch.Tensor) -> torch.Tensor:
+    # int64 tensors; products wrap mod 2^64 and the mask keeps the exact low 32 bits
+    h = h & _M32
+    h = h ^ (h >> 16)
+    h = (h * 0x85EBCA6B) & _M32
+    h = h ^ (h >> 13)
+    h = (h * 0xC2B2AE35) & _M32
+    h = h ^ (h >> 16)
+    return h
+
+
+def hash_u32_int(seed: int, a: int, b: int) -> int:
+    h = _mix32_int((seed & _M32) ^ 0x9E3779B9)
+    h = _mix32_int(h ^ (a & _M32))
+    h = _mix32_int((h + (((b & _M32) * 0x9E3779B1) & _M32)) & _M32)
+    return h
+
+
+def hash_uniform_int(seed: int, a: int, b: int) -> float:
+    return hash_u32_int(seed, a, b) / 4294967296.0
+
+
+def hash_uniform(seed: int, a: torch.Tensor, b: torch.Tensor) -> torch.Tensor:
+    """u in [0,1) (float64) from (seed, a, b); a, b integer tensors (broadcastable)."""
+    a = a.to(torch.int64)
+    b = b.to(torch.int64)
+    h0 = _mix32_int((seed & _M32) ^ 0x9E3779B9)
+    h = _mix32_t(a ^ h0)  # a < 2^32 so (h0 ^ a) stays within 32 bits after the mask in _mix32_t
+    h = _mix32_t((h + ((b * 0x9E3779B1) & _M32)) & _M32)
+    return h.to(torch.float64) / 4294967296.0
+
+
+# --------------------------------------------------------------------------
+# specification
+# --------------------------------------------------------------------------
+@dataclass(frozen=True)
+class Sphere:
+    cx: float
+    cy: float
+    cz: float
+    r: float
+
+
+@dataclass(frozen=True)
+class ZCylinder:
+    """Cylinder with axis parallel to z (the rectum of config 2)."""
+    cx: float
+    cy: float
+    r: float
+    z0: float
+    z1: float
+
+
+@dataclass(frozen=True)
+class Arc:
+    n_angles: int
+    start_deg: float
+    step_deg: float
+    collimator90: bool
+    n_rows: int           # leaf rows per control point (potential grid)
+    n_cols: int           # potential beamlet columns per leaf row
+
+
+@dataclass
+class PhantomSpec:
+    name: str
+    cfg: int
+    grid: Tuple[int, int, int]
+    h: float
+    body: Tuple[float, float]
+    targets: List[Sphere]
+    oars: list
+    arcs: List[Arc]
+    w: float
+    sigma: float
+    cutoff: float
+    mu: float = 0.005
+    noise: float = 1e-3
+    drop: float = 1e-4
+    ragged: bool = True
+    seed_ddc: int = 0
+    # objective (D7): per structure (T, w_over, w_under); id 0 = body
+    T_target: float = 70.0
+    T_oar: float = 30.0
+    T_body: float = 50.0
+    w_target: Tuple[float, float] = (1.0, 1.0)
+    w_oar: Tuple[float, float] = (0.2, 0.0)
+    w_body: Tuple[float, float] = (0.05, 0.0)
+
+    @property
+    def n_angles(self) -> int:
+        return sum(a.n_angles for a in self.arcs)
+
+
+@dataclass
+class Phantom:
+    spec: PhantomSpec
+    n_voxels: int
+    n_beamlets: int
+    n_angles: int
+    n_rows_total: int
+    # COO triplets (device of generation): int32, int32, float32
+    coo_voxel: torch.Tensor
+    coo_beamlet: torch.Tensor
+    coo_val: torch.Tensor
+    # host int32 offsets
+    angle_col_offset: torch.Tensor      # [n_angles+1]
+    angle_row_offset: torch.Tensor      # [n_angles+1]
+    leafrow_col_offset: torch.Tensor    # [n_rows_total+1]
+    # per-voxel structure id (uint8, host) and per-structure parameters (float32, host)
+    voxel_struct: torch.Tensor
+    struct_T: torch.Tensor
+    struct_w_over: torch.Tensor
+    struct_w_under: torch.Tensor
+    angles_generated: Sequence[int] = field(default_factory=list)
+
+    @property
+    def nnz(self) -> int:
+        return int(self.coo_val.numel())
+
+    def stats(self) -> dict:
+        nb, nv = max(self.n_beamlets, 1), max(self.n_voxels, 1)
+        return {
+            "name": self.spec.name, "n_voxels": self.n_voxels, "n_beamlets": self.n_beamlets,
+            "n_angles": self.n_angles, "n_leaf_rows": self.n_rows_total, "nnz": self.nnz,
+            "nnz_per_beamlet": self.nnz / nb, "nnz_per_voxel": self.nnz / nv,
+            "bytes_per_layout": 8 * self.nnz,
+        }
+
+
+# --------------------------------------------------------------------------
+# the five configs of BASELINE.json
+# --------------------------------------------------------------------------
+CONFIG_NAMES = {
+    0: "cfg0-tiny-phantom",
+    1: "cfg1-hn-like-one-arc",
+    2: "cfg2-prostate-like",
+    3: "cfg3-large-hn-two-arcs",
+}
+
+
+def _place_spheres(seed: int, tag: int, radii: Sequence[float], body: Tuple[float, float],
+                   z_half: float, keep_out: Sequence[Sphere], gap: float) -> List[Sphere]:
+    """Seeded rejection sampling of sphere centres inside the body ellipse (shrunk by r),
+    |z| <= z_half - r, at distance >= r + r' + gap from every sphere in keep_out and from
+    the ones placed before."""
+    placed: List[Sphere] = []
+    for k, r in enumerate(radii):
+        t = 0
+        while True:
+            ux = hash_uniform_int(seed, tag * 1000 + k, 3 * t + 0)
+            uy = hash_uniform_int(seed, tag * 1000 + k, 3 * t + 1)
+            uz = hash_uniform_int(seed, tag * 1000 + k, 3 * t + 2)
+            t += 1
+            if t > 100000:
+                raise RuntimeError("sphere placement failed")
+            ax, ay = body[0] - r - 2.0, body[1] - r - 2.0
+            cx, cy = (2 * ux - 1) * ax, (2 * uy - 1) * ay
+            if (cx / ax) ** 2 + (cy / ay) ** 2 > 1.0:
+                continue
+            cz = (2 * uz - 1) * (z_half - r)
+            ok = True
+            for s in list(keep_out) + placed:
+                if math.dist((cx, cy, cz), (s.cx, s.cy, s.cz)) < r + s.r + gap:
+                    ok = False
+                    break
+            if ok:
+                placed.append(Sphere(cx, cy, cz, r))
+                break
+    return placed
+
+
+def config_spec(cfg: int, scale: float = 1.0) -> PhantomSpec:
+    """PhantomSpec of BASELINE.json configs[cfg].
+
+    `scale` (config 4, the roofline sweep: "scale voxel size and beamlet size") multiplies
+    the voxel size h and DIVIDES the grid counts, and multiplies the beamlet width w, sigma
+    and cutoff, keeping the anatomy in mm fixed; scale > 1 gives fewer nnz.
+    """
+    seed_geom = 1503 + cfg
+    if cfg == 0:
+        spec = PhantomSpec(
+            name=CONFIG_NAMES[0], cfg=0, grid=(24, 24, 8), h=5.0, body=(55.0, 45.0),
+            targets=[Sphere(0.0, 0.0, 0.0, 20.0)], oars=[Sphere(30.0, 0.0, 0.0, 10.0)],
+            arcs=[Arc(8, 0.0, 45.0, False, 8, 8)], w=5.0, sigma=2.5, cutoff=15.0, ragged=False)
+    elif cfg == 1:
+        body = (90.0, 75.0)
+        targets = _place_spheres(seed_geom, 1, [35.0, 20.0], body, 100.0, [], 5.0)
+        radii = [10.0 + 5.0 * hash_uniform_int(seed_geom, 77, k) for k in range(4)]
+        oars = _place_spheres(seed_geom, 2, radii, body, 100.0, targets, 0.0)
+        spec = PhantomSpec(
+            name=CONFIG_NAMES[1], cfg=1, grid=(200, 200, 128), h=2.5, body=body,
+            targets=targets, oars=oars, arcs=[Arc(180, 0.0, 2.0, False, 40, 40)],
+            w=5.0, sigma=2.5, cutoff=15.0)
+    elif cfg == 2:
+        spec = PhantomSpec(
+            name=CONFIG_NAMES[2], cfg=2, grid=(160, 120, 96), h=3.0, body=(180.0, 120.0),
+            targets=[Sphere(0.0, 0.0, 0.0, 25.0)],
+            oars=[ZCylinder(0.0, -39.0, 12.0, -40.0, 40.0), Sphere(0.0, 57.0, 0.0, 30.0)],
+            arcs=[Arc(180, 0.0, 2.0, False, 12, 40)], w=5.0, sigma=2.5, cutoff=15.0)
+    elif cfg == 3:
+        body = (140.0, 110.0)
+        targets = _place_spheres(seed_geom, 1, [40.0, 30.0, 20.0], body, 180.0, [], 5.0)
+        radii = [10.0 + 10.0 * hash_uniform_int(seed_geom, 77, k) for k in range(6)]
+        oars = _place_spheres(seed_geom, 2, radii, body, 180.0, targets, 0.0)
+        spec = PhantomSpec(
+            name=CONFIG_NAMES[3], cfg=3, grid=(256, 256, 160), h=2.5, body=body,
+            targets=targets, oars=oars,
+            arcs=[Arc(180, 0.0, 2.0, False, 160, 128), Arc(180, 0.0, 2.0, True, 128, 160)],
+            w=2.5, sigma=1.25, cutoff=10.0)
+    else:
+        raise ValueError("config 4 is config_spec(1, scale=s); configs are 0..3")
+    spec.seed_ddc = 150301721 + cfg
+    if scale != 1.0:
+        nx, ny, nz = spec.grid
+        spec.grid = (max(4, round(nx / scale)), max(4, round(ny / scale)), max(2, round(nz / scale)))
+        spec.h *= scale
+        spec.w *= scale
+        spec.sigma *= scale
+        spec.cutoff *= scale
+        spec.arcs = [Arc(a.n_angles, a.start_deg, a.step_deg, a.collimator90,
+                         max(1, math.ceil(a.n_rows / scale)), max(1, math.ceil(a.n_cols / scale)))
+                     for a in spec.arcs]
+        spec.name = f"{spec.name}-scale{scale:g}"
+    return spec
+
+
+# --------------------------------------------------------------------------
+# geometry helpers
+# --------------------------------------------------------------------------
+def _angle_table(spec: PhantomSpec):
+    """[(theta_rad, arc)] for every control point, arc-major."""
+    out = []
+    for arc in spec.arcs:
+        for k in range(arc.n_angles):
+            out.append((math.radians(arc.start_deg + k * arc.step_deg), arc))
+    return out
+
+
+def _axes(theta: float, arc: Arc):
+    """(e_col, e_row): unit vectors of leaf travel (columns) and of leaf-row stacking."""
+    e_l = (-math.sin(theta), math.cos(theta), 0.0)
+    e_z = (0.0, 0.0, 1.0)
+    return (e_z, e_l) if arc.collimator90 else (e_l, e_z)
+
+
+def _voxels(spec: PhantomSpec, device):
+    """In-body voxel centres (float64, mm) in x-fastest raster order, and structure ids."""
+    nx, ny, nz = spec.grid
+    h = spec.h
+    xs = (torch.arange(nx, dtype=torch.float64, device=device) - (nx - 1) / 2.0) * h
+    ys = (torch.arange(ny, dtype=torch.float64, device=device) - (ny - 1) / 2.0) * h
+    zs = (torch.arange(nz, dtype=torch.float64, device=device) - (nz - 1) / 2.0) * h
+    Z, Y, X = torch.meshgrid(zs, ys, xs, indexing="ij")          # x fastest when flattened
+    inside = ((X / spec.body[0]) ** 2 + (Y / spec.body[1]) ** 2) <= 1.0
+    X, Y, Z = X[inside], Y[inside], Z[inside]
+    # structure ids: 0 body, 1..nT targets, nT+1.. OARs; precedence target > OAR > body (C9)
+    sid = torch.zeros(X.shape, dtype=torch.uint8, device=device)
+    nT = len(spec.targets)
+    for k, s in reversed(list(enumerate(spec.oars))):
+        if isinstance(s, Sphere):
+            m = (X - s.cx) ** 2 + (Y - s.cy) ** 2 + (Z - s.cz) ** 2 <= s.r ** 2
+        else:
+            m = ((X - s.cx) ** 2 + (Y - s.cy) ** 2 <= s.r ** 2) & (Z >= s.z0) & (Z <= s.z1)
+        sid[m] = nT + 1 + k
+    for k, s in reversed(list(enumerate(spec.targets))):
+        m = (X - s.cx) ** 2 + (Y - s.cy) ** 2 + (Z - s.cz) ** 2 <= s.r ** 2
+        sid[m] = 1 + k
+    return X, Y, Z, sid
+
+
+def _fields(spec: PhantomSpec):
+    """Per control point and leaf row: first/last potential column kept (cmin > cmax = empty).
+    Returns (cmin list of int64 tensors, cmax list, angle_col_offset, angle_row_offset,
+    leafrow_col_offset) - all host."""
+    table = _angle_table(spec)
+    cmins, cmaxs = [], []
+    row_counts = []
+    w = spec.w
+    for theta, arc in table:
+        NR, NC = arc.n_rows, arc.n_cols
+        if not spec.ragged:
+            cmin = torch.zeros(NR, dtype=torch.int64)
+            cmax = torch.full((NR,), NC - 1, dtype=torch.int64)
+        else:
+            e_c, e_r = _axes(theta, arc)
+            uc = (torch.arange(NC, dtype=torch.float64) - (NC - 1) / 2.0) * w     # column centres
+            vr = (torch.arange(NR, dtype=torch.float64) - (NR - 1) / 2.0) * w     # row centres
+            meets = torch.zeros((NR, NC), dtype=torch.bool)
+            for s in spec.targets:
+                pc = s.cx * e_c[0] + s.cy * e_c[1] + s.cz * e_c[2]
+                pr = s.cx * e_r[0] + s.cy * e_r[1] + s.cz * e_r[2]
+                dx = torch.clamp((uc - pc).abs() - w / 2.0, min=0.0)[None, :]
+                dy = torch.clamp((vr - pr).abs() - w / 2.0, min=0.0)[:, None]
+                meets |= (dx * dx + dy * dy) <= s.r ** 2
+            any_row = meets.any(dim=1)
+            idx = torch.arange(NC, dtype=torch.int64)[None, :].expand(NR, NC)
+            first = torch.where(meets, idx, torch.full_like(idx, NC)).min(dim=1).values
+            last = torch.where(meets, idx, torch.full_like(idx, -1)).max(dim=1).values
+            cmin = torch.clamp(first - 1, min=0)
+            cmax = torch.clamp(last + 1, max=NC - 1)
+            cmin = torch.where(any_row, cmin, torch.ones_like(cmin))
+            cmax = torch.where(any_row, cmax, torch.zeros_like(cmax))       # empty: cmin=1 > cmax=0
+        cmins.append(cmin)
+        cmaxs.append(cmax)
+        row_counts.append(NR)
+    lens = torch.cat([torch.clamp(cx - cn + 1, min=0) for cn, cx in zip(cmins, cmaxs)])
+    leafrow_col_offset = torch.zeros(lens.numel() + 1, dtype=torch.int64)
+    leafrow_col_offset[1:] = torch.cumsum(lens, 0)
+    angle_row_offset = torch.zeros(len(table) + 1, dtype=torch.int64)
+    angle_row_offset[1:] = torch.cumsum(torch.tensor(row_counts, dtype=torch.int64), 0)
+    angle_col_offset = leafrow_col_offset[angle_row_offset]
+    return cmins, cmaxs, angle_col_offset, angle_row_offset, leafrow_col_offset
+
+
+# --------------------------------------------------------------------------
+# the generator
+# --------------------------------------------------------------------------
+def _angle_entries(spec, theta, arc, cmin, cmax, row_base, leafrow_col_offset_dev,
+                   X, Y, Z, vox_chunk):
+    """COO entries of one control point: (voxel int64, beamlet int64, value float64)."""
+    dev = X.device
+    w, NR, NC = spec.w, arc.n_rows, arc.n_cols
+    k = int(math.ceil(spec.cutoff / w))
+    e_c, e_r = _axes(theta, arc)
+    ct, st = math.cos(theta), math.sin(theta)
+    a, b = spec.body
+    cmin_d, cmax_d = cmin.to(dev), cmax.to(dev)
+    nonempty = (cmax >= cmin)
+    if not bool(nonempty.any()):
+        z = torch.zeros(0, dtype=torch.int64, device=dev)
+        return z, z, torch.zeros(0, dtype=torch.float64, device=dev)
+    rows_ne = torch.nonzero(nonempty).flatten()
+    r_lo, r_hi = int(rows_ne.min()) - k, int(rows_ne.max()) + k
+    c_lo, c_hi = int(cmin[nonempty].min()) - k, int(cmax[nonempty].max()) + k
+
+    pc = X * e_c[0] + Y * e_c[1] + Z * e_c[2]              # position along leaf travel
+    pr = X * e_r[0] + Y * e_r[1] + Z * e_r[2]              # position across leaf rows
+    ic0 = torch.round(pc / w + (NC - 1) / 2.0).to(torch.int64)
+    ir0 = torch.round(pr / w + (NR - 1) / 2.0).to(torch.int64)
+    sel = torch.nonzero((ir0 >= r_lo) & (ir0 <= r_hi) & (ic0 >= c_lo) & (ic0 <= c_hi)).flatten()
+    if sel.numel() == 0:
+        z = torch.zeros(0, dtype=torch.int64, device=dev)
+        return z, z, torch.zeros(0, dtype=torch.float64, device=dev)
+    # depth (D3): ray through the voxel centre, P + s b, enters the ellipse at s_in < 0
+    A = (ct / a) ** 2 + (st / b) ** 2
+    off = torch.arange(-k, k + 1, dtype=torch.int64, device=dev)
+    dR = off.repeat_interleave(2 * k + 1)[None, :]         # window offsets, [1, K]
+    dC = off.repeat(2 * k + 1)[None, :]
+    vs, bs, vals = [], [], []
+    for s0 in range(0, sel.numel(), vox_chunk):
+        v = sel[s0:s0 + vox_chunk]
+        x, y = X[v], Y[v]
+        B = x * ct / a ** 2 + y * st / b ** 2
+        C = (x / a) ** 2 + (y / b) ** 2 - 1.0
+        depth = (B + torch.sqrt(torch.clamp(B * B - A * C, min=0.0))) / A   # = -s_in >= 0
+        r = ir0[v][:, None] + dR
+        c = ic0[v][:, None] + dC
+        ok = (r >= 0) & (r < NR)
+        rc = torch.clamp(r, 0, NR - 1)
+        ok &= (c >= cmin_d[rc]) & (c <= cmax_d[rc])
+        du = pc[v][:, None] - (c.to(torch.float64) - (NC - 1) / 2.0) * w
+        dv = pr[v][:, None] - (r.to(torch.float64) - (NR - 1) / 2.0) * w
+        rr = du * du + dv * dv
+        ok &= rr <= spec.cutoff ** 2
+        iv, ik = torch.nonzero(ok, as_tuple=True)
+        if iv.numel() == 0:
+            continue
+        vox = v[iv]
+        rsel, csel = r[iv, ik], c[iv, ik]
+        beam = leafrow_col_offset_dev[row_base + rsel] + (csel - cmin_d[rsel])
+        val = torch.exp(-spec.mu * depth[iv]) * torch.exp(-rr[iv, ik] / (2.0 * spec.sigma ** 2))
+        val = val + spec.noise * hash_uniform(spec.seed_ddc, vox, beam)
+        keep = val >= spec.drop
+        vs.append(vox[keep])
+        bs.append(beam[keep])
+        vals.append(val[keep])
+    if not vs:
+        z = torch.zeros(0, dtype=torch.int64, device=dev)
+        return z, z, torch.zeros(0, dtype=torch.float64, device=dev)
+    return torch.cat(vs), torch.cat(bs), torch.cat(vals)
+
+
+def generate(spec: PhantomSpec, device="cpu", angles: Optional[Sequence[int]] = None,
+             vox_chunk: int = 1 << 18) -> Phantom:
+    """Generate the COO triplets of D for `spec` on `device`.
+
+    `angles`: generate only these control points (global indices; the column numbering,
+    offsets and n_beamlets stay those of the full matrix) - the angle blocks D_a of
+    PAPER.md L119.  Default: all."""
+    device = torch.device(device)
+    X, Y, Z, sid = _voxels(spec, device)
+    cmins, cmaxs, aco, aro, lco = _fields(spec)
+    lco_dev = lco.to(device)
+    table = _angle_table(spec)
+    todo = list(range(len(table))) if angles is None else list(angles)
+    vs, bs, vals = [], [], []
+    for a_idx in todo:
+        theta, arc = table[a_idx]
+        v, b, val = _angle_entries(spec, theta, arc, cmins[a_idx], cmaxs[a_idx], int(aro[a_idx]),
+                                   lco_dev, X, Y, Z, vox_chunk)
+        vs.append(v.to(torch.int32))
+        bs.append(b.to(torch.int32))
+        vals.append(val.to(torch.float32))                  # the single rounding to FP32 (D4)
+    cat = (lambda xs, dt: torch.cat(xs) if xs else torch.zeros(0, dtype=dt, device=device))
+    nT, nO = len(spec.targets), len(spec.oars)
+    T = [spec.T_body] + [spec.T_target] * nT + [spec.T_oar] * nO
+    wo = [spec.w_body[0]] + [spec.w_target[0]] * nT + [spec.w_oar[0]] * nO
+    wu = [spec.w_body[1]] + [spec.w_target[1]] * nT + [spec.w_oar[1]] * nO
+    return Phantom(
+        spec=spec, n_voxels=int(X.numel()), n_beamlets=int(lco[-1]), n_angles=len(table),
+        n_rows_total=int(lco.numel() - 1),
+        coo_voxel=cat(vs, torch.int32), coo_beamlet=cat(bs, torch.int32), coo_val=cat(vals, torch.float32),
+        angle_col_offset=aco.to(torch.int32), angle_row_offset=aro.to(torch.int32),
+        leafrow_col_offset=lco.to(torch.int32),
+        voxel_struct=sid.cpu(), struct_T=torch.tensor(T, dtype=torch.float32),
+        struct_w_over=torch.tensor(wo, dtype=torch.float32),
+        struct_w_under=torch.tensor(wu, dtype=torch.float32),
+        angles_generated=todo)
+
+
+def draw_x(n_beamlets: int, eval_index: int, device="cpu", scale: float = 1.0) -> torch.Tensor:
+    """Fluence vector x ~ seeded Uniform[0,1) (FP32), seed_x = 1721*1000 + eval_index (D6).
+    `scale` multiplies it (C13: config 0 needs x*8, x*16 to reach the overdose branches)."""
+    j = torch.arange(n_beamlets, dtype=torch.int64, device=device)
+    u = hash_uniform(1721 * 1000 + eval_index, j, torch.zeros_like(j))
+    return (u * scale).to(torch.float32)
