@@ -1,0 +1,329 @@
+#!/usr/bin/env python
+"""bench.py - price evaluations per second of the VMAT beamlet-price path on B200.
+
+One "step" = one whole price evaluation (d = D x -> F, g -> p = D^T g -> leaf-row openings -> best
+control point) on a fresh fluence vector x, through the C ABI
+(`vmat_price_eval`).  Inputs are synthetic (synth/), shaped like BASELINE.json `configs`.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config {0,1,2,3}] [--scale S] [--impl reference]
+
+Prints ONE JSON line (rank 0).  Multi-GPU: the path does not need a second GPU (BASELINE.json
+north_star), so N > 1 runs N independent replicas, one process per GPU ("replicas only", weak scaling).
+`--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded angle-block sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+import synth
+
+METRIC = "beamlet-price evaluations/sec"
+UNIT = "evals/s"
+
+
+# ----------------------------------------------------------------------------- helpers
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy bandwidth)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx, self.proc, self.lines = gpu_index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.idx), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [t.strip() for t in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def phantom_arrays_host(ph):
+    return dict(vox=ph.coo_voxel.cpu().numpy(), beam=ph.coo_beamlet.cpu().numpy(), val=ph.coo_val.cpu().numpy(),
+                n_v=ph.n_voxels, n_b=ph.n_beamlets, sid=ph.voxel_struct.numpy(), T=ph.struct_T.numpy(),
+                wo=ph.struct_w_over.numpy(), wu=ph.struct_w_under.numpy(), lco=ph.leafrow_col_offset.numpy(),
+                aro=ph.angle_row_offset.numpy())
+
+
+# ----------------------------------------------------------------------------- the CPU oracle, timed
+def oracle_rate(spec, gen_device, budget_s: float, reps: int):
+    """Times the oracle (one whole price evaluation, O1-O5) on an angle-block sample of `spec`
+    (D = [D_1 ... D_A]; the evaluation is additive over angle blocks) sized to about
+    `budget_s` seconds of single-thread CPU work.  Returns (evals/s extrapolated to the full matrix,
+    description, per-rep seconds, nnz_sample, nnz_full_estimate)."""
+    import oracle
+    n_a = spec.n_angles
+    # calibrate on one control point
+    probe = synth.generate(spec, device=gen_device, angles=[n_a // 3])
+    A = phantom_arrays_host(probe)
+    x = synth.draw_x(probe.n_beamlets, 0).numpy()
+    t0 = time.perf_counter()
+    oracle.price_eval(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], x, A["sid"], A["T"], A["wo"], A["wu"],
+                      A["lco"], A["aro"])
+    t1 = time.perf_counter() - t0
+    k = int(max(1, min(n_a, budget_s / max(t1, 1e-4))))
+    angles = sorted(set(int(round(i * n_a / k)) % n_a for i in range(k)))
+    smp = synth.generate(spec, device=gen_device, angles=angles)
+    A = phantom_arrays_host(smp)
+    times = []
+    for r in range(reps):
+        x = synth.draw_x(smp.n_beamlets, r).numpy()
+        t0 = time.perf_counter()
+        oracle.price_eval(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], x, A["sid"], A["T"], A["wo"],
+                          A["wu"], A["lco"], A["aro"])
+        times.append(time.perf_counter() - t0)
+    frac = len(angles) / n_a
+    t_full = float(np.median(times)) / frac                 # the evaluation is additive over angle blocks
+    desc = (f"{len(angles)} of {n_a} control points of {spec.name} (every {n_a / len(angles):.1f}th angle block, "
+            f"{smp.nnz} nnz), whole evaluation O1-O5 per rep, {reps} reps, median; evals/s extrapolated by "
+            f"angle-block additivity (x{1 / frac:.1f})")
+    return 1.0 / t_full, desc, times, smp.nnz, smp.nnz / frac
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    spec = synth.config_spec(args.config, args.scale)
+    gen_dev = "cuda:0" if torch.cuda.is_available() else "cpu"
+    total_budget = 150.0                                     # seconds for the whole --steps/--warmup run
+    per_step = min(15.0, total_budget / max(1, args.steps + args.warmup))
+    # warm-up reps are part of `reps`; only the last `steps` are reported
+    value, desc, times, nnz_s, nnz_full = oracle_rate(spec, gen_dev, per_step, args.steps + args.warmup)
+    timed = times[args.warmup:] if len(times) > args.warmup else times
+    frac = nnz_s / nnz_full
+    t_full = float(np.median(timed)) / frac
+    value = 1.0 / t_full
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_full, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": spec.name, "nnz_full_estimate": int(nnz_full), "sample_nnz": int(nnz_s)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------- the CUDA path, timed
+def run_ours(args):
+    import paper_1503_01721_b200 as vm
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device - the product path has no CPU fallback "
+                         "(use --impl reference for the oracle)")
+    vm.load_library()
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+    use_dist = world > 1
+    if use_dist:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    spec = synth.config_spec(args.config, args.scale)
+    t0 = time.time()
+    ph = synth.generate(spec, device=dev)
+    torch.cuda.synchronize()
+    t_gen = time.time() - t0
+    t0 = time.time()
+    h = vm.vmat_ddc_create(ph.n_voxels, ph.n_beamlets, ph.coo_voxel, ph.coo_beamlet, ph.coo_val,
+                           ph.angle_col_offset, ph.angle_row_offset, ph.leafrow_col_offset, device=dev)
+    t_ingest = time.time() - t0
+    stats = ph.stats()
+    ph.coo_voxel = ph.coo_beamlet = ph.coo_val = None      # the handle holds its own layouts
+    torch.cuda.empty_cache()
+    obj = vm.Objective(ph.voxel_struct.to(dev), ph.struct_T.to(dev), ph.struct_w_over.to(dev),
+                       ph.struct_w_under.to(dev))
+    out = h.alloc_outputs()
+    K, W = args.steps, args.warmup
+    n_b, n_v, nnz = h.n_beamlets, h.n_voxels, h.nnz
+    n_rows, n_a = h.n_leaf_rows, h.n_angles
+    # x re-drawn for every evaluation (configs[4]); each rank draws its own sequence
+    xs = [synth.draw_x(n_b, rank * 100000 + k, device=dev) for k in range(K + W)]
+
+    def barrier():
+        if use_dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: K evaluations between two events, per-kernel events inside
+    for k in range(W):
+        vm.vmat_price_eval(h, xs[k], obj, out)
+    ev_k = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
+    for evs in ev_k:
+        for e in evs:
+            e.record()                                       # creates the underlying cudaEvent_t handles
+    start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    launches = 0
+    start.record()
+    for k in range(K):
+        h.set_profile_events(ev_k[k])
+        vm.vmat_price_eval(h, xs[W + k], obj, out)
+        launches += vm.last_launch_count()
+    stop.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    h.set_profile_events(None)
+    elapsed_ms = start.elapsed_time(stop)
+    t_dose = np.array([e[0].elapsed_time(e[1]) for e in ev_k])
+    t_price = np.array([e[2].elapsed_time(e[3]) for e in ev_k])
+    best_last = int(out.best_angle.item())
+    F_last = float(out.F.item())
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    xh = [x.cpu().pin_memory() for x in xs]
+    Fh = torch.empty(1, dtype=torch.float64).pin_memory()
+    Lh = torch.empty(n_rows, dtype=torch.int32).pin_memory()
+    Rh = torch.empty(n_rows, dtype=torch.int32).pin_memory()
+    rph = torch.empty(n_rows, dtype=torch.float64).pin_memory()
+    aph = torch.empty(n_a, dtype=torch.float64).pin_memory()
+    bh = torch.empty(1, dtype=torch.int32).pin_memory()
+    for k in range(min(W, 3)):
+        vm.vmat_price_eval_host(h, xh[k], obj, Fh, Lh, Rh, rph, aph, bh)
+    barrier()
+    s2, e2 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s2.record()
+    for k in range(K):
+        vm.vmat_price_eval_host(h, xh[W + k], obj, Fh, Lh, Rh, rph, aph, bh)
+    e2.record()
+    barrier()
+    e2e_ms = s2.elapsed_time(e2)
+    h2d = 4 * n_b
+    d2h = 4 * n_rows * 2 + 8 * n_rows + 8 * n_a + 4 + 8
+
+    # ---- max over ranks
+    if use_dist:
+        t = torch.tensor([elapsed_ms, e2e_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        elapsed_ms, e2e_ms = float(t[0]), float(t[1])
+
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        # algorithmic bytes per launch
+        B_dose = 8 * nnz + 8 * (n_v + 1) + 4 * n_b + 4 * n_v + (1 * n_v + 4 * n_v)      # + struct id, g (fused A2)
+        B_price = 8 * nnz + 8 * (n_b + 1) + 4 * n_v + 4 * n_b + 4 * (n_rows + 1) + 16 * n_rows
+        B_eval = B_dose + B_price
+        k_dose = {"name": "k_dose<fused objective>", "ms": float(t_dose.mean()), "ms_min": float(t_dose.min()),
+                  "bytes": B_dose, "gbs": B_dose / (t_dose.mean() * 1e-3) / 1e9}
+        k_price = {"name": "k_price_select", "ms": float(t_price.mean()), "ms_min": float(t_price.min()),
+                   "bytes": B_price, "gbs": B_price / (t_price.mean() * 1e-3) / 1e9}
+        dom = k_price if k_price["ms"] >= k_dose["ms"] else k_dose
+        ms_per_step = elapsed_ms / K
+        value = world * K / (elapsed_ms * 1e-3)
+        eval_gbs = B_eval / (ms_per_step * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": spec.name, "n_voxels": n_v, "n_beamlets": n_b, "nnz": nnz, "n_angles": n_a,
+                       "n_leaf_rows": n_rows, "bytes_per_layout": 8 * nnz,
+                       "parallelism": "replicas only" if world > 1 else "1 gpu",
+                       "l2": f"inputs larger than L2: {B_eval / 1e9:.2f} GB streamed per step vs 126 MB L2"
+                             if B_eval > 4 * 126e6 else "L2-resident: matrix fits the 126 MB L2, no HBM fraction claimed",
+                       "x": "re-drawn per step, seeded Uniform[0,1)", "gen_s": round(t_gen, 2),
+                       "ingest_s": round(t_ingest, 2)},
+            "hbm_gbs": eval_gbs, "hbm_frac_of_8TBs": eval_gbs / 8000.0, "hbm_frac_of_measured": eval_gbs / peak,
+            "clocks": clocks,
+            "e2e": {"value": world * K / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / K},
+            "gpu_launches": launches,
+            "roofline": {"bound": "hbm", "kernel": dom["name"], "achieved": dom["gbs"], "peak": peak,
+                         "unit": "GB/s", "frac": dom["gbs"] / peak, "frac_of_8TBs": dom["gbs"] / 8000.0,
+                         "peak_source": peak_src, "traffic": None, "algorithmic_bytes": dom["bytes"],
+                         "ms": dom["ms"]},
+            "kernels": [k_dose, k_price],
+            "result_check": {"F_last": F_last, "best_angle_last": best_last},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            v, desc, _, _, _ = oracle_rate(spec, dev, 12.0, 3)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc}
+        print(json.dumps(line))
+    h.close()
+    if use_dist:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (default 3: the largest DDC)")
+    ap.add_argument("--scale", type=float, default=1.0, help="config 4 sweep: coarsen voxels/beamlets by this factor")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

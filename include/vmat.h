@@ -1,0 +1,166 @@
+/*
+ * vmat.h - C ABI of libvmat: the beamlet-price step of the pricing problem of the
+ * column-generation VMAT optimiser of arXiv 1503.01721, on one NVIDIA B200 (sm_100a).
+ *
+ *   x --> d = D x --> (F, g = dF/dd) --> p = D^T g --> per control point, per MLC leaf row,
+ *                                                      the minimum-price contiguous opening
+ *
+ * Citations are lines of /root/reference/PAPER.md ("L43" = line 43) with the section or
+ * equation they fall in; "C1".."C14" are the readings listed in DESIGN.md.
+ *
+ * Conventions for every call
+ *   - `dev` pointers are CUDA device memory of the current device, `host` pointers are host
+ *     memory.  The library never allocates or frees a vector it is handed: the caller owns
+ *     every argument before and after the call.  The handle owns only the two matrix layouts
+ *     and its scratch.
+ *   - Compute calls enqueue work on `stream` (a cudaStream_t passed as void*, NULL = the legacy
+ *     default stream) and return without synchronising.  Scalars (F, best_angle) land in device
+ *     memory.  One evaluation may be in flight per handle at a time (the handle holds scratch).
+ *   - Return value: VMAT_OK (0) or a negative vmat_status; no exception or abort crosses the
+ *     ABI; on failure the outputs are unspecified and *out handles are left untouched.
+ *     vmat_last_error() gives a thread-local message for the last failure.
+ *   - Results are deterministic run to run: canonical storage order, fixed reduction order,
+ *     no floating-point atomics anywhere.
+ *   - Values are FP32, indices int32, nnz and row pointers int64 (Table 2,
+ *     L198-L202: 12 B/nnz COO, 8 B/nnz CSR).
+ */
+#ifndef VMAT_H
+#define VMAT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum vmat_status {
+    VMAT_OK = 0,
+    VMAT_ERR_INVALID_ARG = -1,   /* NULL pointer, negative size, non-monotone offsets, ...        */
+    VMAT_ERR_INDEX_RANGE = -2,   /* a COO voxel / beamlet index outside [0,n)                     */
+    VMAT_ERR_DUPLICATE   = -3,   /* the same (voxel, beamlet) pair twice (C14)                    */
+    VMAT_ERR_OOM         = -4,   /* device or host allocation failed                              */
+    VMAT_ERR_CUDA        = -5,   /* any other CUDA runtime error (message in vmat_last_error)     */
+    VMAT_ERR_NONFINITE   = -6    /* a COO value is NaN or +-Inf                                   */
+} vmat_status;
+
+/* Opaque handle: owns CSR(D) (voxel rows, for D x), CSR(D^T) (beamlet rows, for D^T g; the
+ * paper's GPU format, L121), the offset tables and scratch. */
+typedef struct vmat_ddc vmat_ddc;
+
+typedef struct vmat_ddc_info {
+    int64_t n_voxels, n_beamlets, nnz, n_angles, n_leaf_rows;
+    int64_t bytes_csr_d;        /* 8*nnz + 8*(n_voxels+1)   (values + indices + int64 row pointers) */
+    int64_t bytes_csr_dt;       /* 8*nnz + 8*(n_beamlets+1)                                         */
+    int64_t bytes_device_total; /* everything the handle holds on the device                        */
+    int64_t n_dose_blocks;      /* row blocks (= CTAs) of the dose kernel                           */
+    int64_t max_leaf_row_len;   /* longest leaf row, in beamlets                                    */
+    int64_t max_voxel_row_nnz, max_beamlet_row_nnz;
+} vmat_ddc_info;
+
+/* A0 ingest / layout build (D arrives as COO - values, voxel (row) index,
+ * beamlet (column) index, equal length, any order - and is converted to CSR "at the
+ * initialization stage").  Builds both layouts on the device, rows in canonical order (sorted by
+ * the secondary index).
+ *   coo_*               host OR device pointers, length nnz (detected with cudaPointerGetAttributes);
+ *                       the caller may free them when the call returns.
+ *   angle_col_offset    host [n_angles+1]: beamlets of control point a are columns [off[a], off[a+1])
+ *                       (the angle blocks D = [D_1 ... D_A] of L119); off[0] = 0, off[n_angles] = n_beamlets.
+ *   angle_row_offset    host [n_angles+1]: MLC leaf rows of control point a.
+ *   leafrow_col_offset  host [n_leaf_rows+1], n_leaf_rows = angle_row_offset[n_angles]: beamlets of a
+ *                       leaf row, left to right; leaf rows do not straddle control points.
+ * Synchronous (returns after the build finished).  Validates index ranges, finiteness, duplicates
+ * and offset tables.  Empty rows, empty columns and nnz = 0 are legal. */
+int vmat_ddc_create(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int64_t nnz,
+                    const int32_t *coo_voxel, const int32_t *coo_beamlet, const float *coo_val,
+                    int32_t n_angles, const int32_t *angle_col_offset, const int32_t *angle_row_offset,
+                    const int32_t *leafrow_col_offset, void *stream);
+
+/* Frees the layouts and scratch.  NULL is a no-op. */
+int vmat_ddc_destroy(vmat_ddc *h);
+
+int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info /* host, out */);
+
+/* Test/debug: copies one layout to host arrays.  which = 0: CSR(D) (rows = voxels, idx = beamlets),
+ * which = 1: CSR(D^T) (rows = beamlets, idx = voxels).  ptr [rows+1], idx/val [nnz]. Synchronous. */
+int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx, float *val /* host, out */);
+
+/* A1 forward dose d = D x, d_i = sum_j D_ij x_j ("repeated forward dose
+ * calculation", L27).  x dev [n_beamlets] in, d dev [n_voxels] out. */
+int vmat_dose(const vmat_ddc *h, const float *x, float *d, void *stream);
+
+/* A2 objective and gradient (Eq. (1); Eq. (4)):
+ *   F   = sum_i w_over[s_i] max(0, d_i - T[s_i])^2 + w_under[s_i] max(0, T[s_i] - d_i)^2
+ *   g_i = dF/dd_i = 2 w_over[s_i] max(0, d_i - T[s_i]) - 2 w_under[s_i] max(0, T[s_i] - d_i)
+ * with s_i = voxel_struct[i] (C9).  Sign: the paper's g is -grad F and its price pi is maximised;
+ * here g = +grad F, p = -pi is minimised - identical selections (C1).  w_over = omega+ (overdose),
+ * w_under = omega- (C10).
+ *   d dev [n_voxels] in; voxel_struct dev u8 [n_voxels]; T, w_over, w_under dev [n_struct], n_struct <= 256;
+ *   g dev [n_voxels] out; F dev double [1] out (FP64 sum in a fixed order). */
+int vmat_objective_grad(const vmat_ddc *h, const float *d, const uint8_t *voxel_struct, int32_t n_struct,
+                        const float *T, const float *w_over, const float *w_under,
+                        float *g, double *F, void *stream);
+
+/* A3 beamlet prices p = D^T g, p_j = sum_i D_ij g_i (Eq. (3); "Pi = D^T g", L121; one warp per
+ * beamlet row as in L127).  g dev [n_voxels] in, p dev [n_beamlets] out. */
+int vmat_price(const vmat_ddc *h, const float *g, float *p, void *stream);
+
+/* A4 + A5 aperture selection without interdigitation (L133): for every MLC leaf row the contiguous
+ * opening [L,R) (beamlet columns within the row, 0 <= L <= R <= n_row; C8) minimising the summed
+ * price, the closed opening (value 0, L = R = 0) included (C4); then per control point the sum of its
+ * rows' best prices, and the control point with the smallest sum.
+ * Arithmetic (C5, C6): S_0 = 0, S_{c+1} = S_c + (double)p[j0+c] left to right in FP64; candidates all
+ * 0 <= L <= R <= n with V = S_R - S_L; the result is the smallest candidate in the order (V, L, R).
+ *   p dev [n_beamlets] in; angle_mask dev u8 [n_angles] or NULL (1 = occupied control point: its rows
+ *   stay closed, angle_price = +inf; C7);
+ *   L, R dev int32 [n_leaf_rows]; row_price dev double [n_leaf_rows]; angle_price dev double [n_angles]
+ *   (sum in row order, FP64); best_angle dev int32 [1]: smallest control point attaining the minimum
+ *   among unoccupied ones, or -1 when that minimum is >= 0 (no improving aperture, L56). */
+int vmat_select_apertures(const vmat_ddc *h, const float *p, const uint8_t *angle_mask,
+                          int32_t *L, int32_t *R, double *row_price, double *angle_price,
+                          int32_t *best_angle, void *stream);
+
+/* One whole price evaluation A1 -> A5 with the fused kernels: (dose + objective/gradient) then
+ * (price + row opening) then aperture price.  Same arguments and outputs as the four calls above;
+ * every output vector is written (d, g, p included). */
+int vmat_price_eval(const vmat_ddc *h, const float *x,
+                    const uint8_t *voxel_struct, int32_t n_struct,
+                    const float *T, const float *w_over, const float *w_under,
+                    const uint8_t *angle_mask,
+                    float *d, float *g, double *F, float *p,
+                    int32_t *L, int32_t *R, double *row_price, double *angle_price,
+                    int32_t *best_angle, void *stream);
+
+/* End-to-end variant with HOST buffers: copies x (host, ideally pinned, [n_beamlets]) to the device,
+ * runs vmat_price_eval on device scratch owned by the handle, copies F, L, R, row_price, angle_price
+ * and best_angle back to the host arrays, and synchronises the stream before returning.
+ * The objective tables (voxel_struct, T, w_over, w_under, angle_mask) are device pointers as above. */
+int vmat_price_eval_host(vmat_ddc *h, const float *x_host,
+                         const uint8_t *voxel_struct, int32_t n_struct,
+                         const float *T, const float *w_over, const float *w_under,
+                         const uint8_t *angle_mask,
+                         double *F_host, int32_t *L_host, int32_t *R_host, double *row_price_host,
+                         double *angle_price_host, int32_t *best_angle_host, void *stream);
+
+/* Aperture dose vector DA(A_k) = sum_{j in A_k} D_:j (Eq. (5)) of the aperture given by the
+ * openings [L,R) of the leaf rows of control point `angle`: DA = D 1_A, on the device (the paper did
+ * this on the CPU from COO, L137).  L, R dev int32 [n_leaf_rows] (as written by the selection);
+ * x_scratch dev [n_beamlets] (overwritten with the indicator); DA dev [n_voxels] out. */
+int vmat_aperture_dose(const vmat_ddc *h, int32_t angle, const int32_t *L, const int32_t *R,
+                       float *x_scratch, float *DA, void *stream);
+
+/* Profiling hook for bench.py's roofline: four CUDA events (cudaEvent_t passed as void*, any may be NULL)
+ * that every following vmat_price_eval / vmat_price_eval_host on this handle records on its stream:
+ * ev[0] just before and ev[1] just after the dose(+objective) kernel, ev[2] just before and ev[3] just
+ * after the price(+row opening) kernel.  Pass NULL for `ev` to clear.  The events stay owned by the caller. */
+int vmat_ddc_set_profile_events(vmat_ddc *h, void *const *ev /* host [4] or NULL */);
+
+/* Thread-local, static storage; never NULL. */
+const char *vmat_last_error(void);
+
+/* Number of kernels the last compute call on this thread launched (bench.py's gpu_launches). */
+int vmat_last_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VMAT_H */

@@ -1,0 +1,275 @@
+"""paper_1503_01721_b200 - thin Python binding of libvmat (include/vmat.h).
+
+The beamlet-price step of the column-generation VMAT optimiser of arXiv 1503.01721 on one
+B200: d = D x -> (F, g) -> p = D^T g -> per-leaf-row minimum-price opening -> best control
+point.  Every step runs in the CUDA kernels of `csrc/`; this module only marshals arguments
+(torch tensors provide device memory and the stream).  There is no CPU fallback: if
+`libvmat.so` is missing or cannot be loaded, the first call raises.
+
+Function names mirror the C ABI: vmat_ddc_create, vmat_dose, vmat_objective_grad,
+vmat_price, vmat_select_apertures, vmat_price_eval, vmat_price_eval_host, vmat_aperture_dose.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libvmat.so")
+_lib = None
+
+VMAT_OK = 0
+STATUS_NAMES = {0: "VMAT_OK", -1: "VMAT_ERR_INVALID_ARG", -2: "VMAT_ERR_INDEX_RANGE", -3: "VMAT_ERR_DUPLICATE",
+                -4: "VMAT_ERR_OOM", -5: "VMAT_ERR_CUDA", -6: "VMAT_ERR_NONFINITE"}
+
+EXPORTS = [
+    "vmat_ddc_create", "vmat_ddc_destroy", "vmat_ddc_info_get", "vmat_ddc_export_csr", "vmat_dose",
+    "vmat_objective_grad", "vmat_price", "vmat_select_apertures", "vmat_price_eval", "vmat_price_eval_host",
+    "vmat_aperture_dose", "vmat_ddc_set_profile_events", "vmat_last_error", "vmat_last_launch_count",
+]
+
+
+class VmatError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {message}")
+        self.status = status
+
+
+class _Info(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int64) for n in (
+        "n_voxels", "n_beamlets", "nnz", "n_angles", "n_leaf_rows", "bytes_csr_d", "bytes_csr_dt",
+        "bytes_device_total", "n_dose_blocks", "max_leaf_row_len", "max_voxel_row_nnz", "max_beamlet_row_nnz")]
+
+
+def load_library():
+    """Load libvmat.so (built in-tree by `python -m paper_1503_01721_b200.build`).  Raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} not found: build it with `python -m paper_1503_01721_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+    lib.vmat_ddc_create.argtypes = [ctypes.POINTER(vp), i32, i32, i64, vp, vp, vp, i32, vp, vp, vp, vp]
+    lib.vmat_ddc_destroy.argtypes = [vp]
+    lib.vmat_ddc_info_get.argtypes = [vp, ctypes.POINTER(_Info)]
+    lib.vmat_ddc_export_csr.argtypes = [vp, ctypes.c_int, vp, vp, vp]
+    lib.vmat_dose.argtypes = [vp, vp, vp, vp]
+    lib.vmat_objective_grad.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp]
+    lib.vmat_price.argtypes = [vp, vp, vp, vp]
+    lib.vmat_select_apertures.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.vmat_price_eval.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.vmat_price_eval_host.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.vmat_aperture_dose.argtypes = [vp, i32, vp, vp, vp, vp, vp]
+    lib.vmat_ddc_set_profile_events.argtypes = [vp, vp]
+    lib.vmat_last_error.restype = ctypes.c_char_p
+    lib.vmat_last_launch_count.restype = ctypes.c_int
+    for name in EXPORTS:
+        if name not in ("vmat_last_error",):
+            getattr(lib, name).restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def _check(rc: int):
+    if rc != VMAT_OK:
+        raise VmatError(rc, load_library().vmat_last_error().decode())
+
+
+def _ptr(t: Optional[torch.Tensor], dtype=None, device_type=None, n=None):
+    if t is None:
+        return None
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"expected {dtype}, got {t.dtype}")
+    if device_type is not None and t.device.type != device_type:
+        raise ValueError(f"expected a {device_type} tensor, got {t.device}")
+    if not t.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    if n is not None and t.numel() < n:
+        raise ValueError(f"tensor too small: {t.numel()} < {n}")
+    return t.data_ptr()
+
+
+def _stream():
+    return torch.cuda.current_stream().cuda_stream
+
+
+@dataclass
+class Objective:
+    """Per-voxel structure ids and per-structure {T, w_over, w_under} on the device (Eq. (1))."""
+    voxel_struct: torch.Tensor   # uint8 [n_voxels]
+    T: torch.Tensor              # float32 [n_struct]
+    w_over: torch.Tensor
+    w_under: torch.Tensor
+
+    @property
+    def n_struct(self) -> int:
+        return int(self.T.numel())
+
+
+@dataclass
+class PriceEvalOut:
+    d: torch.Tensor
+    g: torch.Tensor
+    F: torch.Tensor            # float64 [1]
+    p: torch.Tensor
+    L: torch.Tensor            # int32 [n_leaf_rows]
+    R: torch.Tensor
+    row_price: torch.Tensor    # float64 [n_leaf_rows]
+    angle_price: torch.Tensor  # float64 [n_angles]
+    best_angle: torch.Tensor   # int32 [1]
+
+
+class DDC:
+    """Owns a vmat_ddc handle (both CSR layouts on the device)."""
+
+    def __init__(self, handle: int, device: torch.device):
+        self._h = ctypes.c_void_p(handle)
+        self.device = device
+        info = _Info()
+        _check(load_library().vmat_ddc_info_get(self._h, ctypes.byref(info)))
+        self.info = {n: int(getattr(info, n)) for n, _ in _Info._fields_}
+        self.n_voxels, self.n_beamlets = self.info["n_voxels"], self.info["n_beamlets"]
+        self.n_angles, self.n_leaf_rows, self.nnz = self.info["n_angles"], self.info["n_leaf_rows"], self.info["nnz"]
+
+    def close(self):
+        if self._h is not None and self._h.value:
+            load_library().vmat_ddc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def alloc_outputs(self) -> PriceEvalOut:
+        dev, f32, f64, i32 = self.device, torch.float32, torch.float64, torch.int32
+        return PriceEvalOut(
+            d=torch.empty(self.n_voxels, dtype=f32, device=dev), g=torch.empty(self.n_voxels, dtype=f32, device=dev),
+            F=torch.empty(1, dtype=f64, device=dev), p=torch.empty(self.n_beamlets, dtype=f32, device=dev),
+            L=torch.empty(self.n_leaf_rows, dtype=i32, device=dev), R=torch.empty(self.n_leaf_rows, dtype=i32, device=dev),
+            row_price=torch.empty(self.n_leaf_rows, dtype=f64, device=dev),
+            angle_price=torch.empty(self.n_angles, dtype=f64, device=dev),
+            best_angle=torch.empty(1, dtype=i32, device=dev))
+
+    def set_profile_events(self, events=None):
+        """events: four torch.cuda.Event(enable_timing=True) (already recorded once, so their handles exist)
+        or None to clear; see vmat_ddc_set_profile_events."""
+        if events is None:
+            _check(load_library().vmat_ddc_set_profile_events(self._h, None))
+            return
+        arr = (ctypes.c_void_p * 4)(*[e.cuda_event for e in events])
+        _check(load_library().vmat_ddc_set_profile_events(self._h, arr))
+
+    def export_csr(self, which: int):
+        """(ptr int64 [rows+1], idx int32 [nnz], val float32 [nnz]) of CSR(D) (0) or CSR(D^T) (1), on the host."""
+        rows = self.n_voxels if which == 0 else self.n_beamlets
+        ptr = torch.empty(rows + 1, dtype=torch.int64)
+        idx = torch.empty(self.nnz, dtype=torch.int32)
+        val = torch.empty(self.nnz, dtype=torch.float32)
+        _check(load_library().vmat_ddc_export_csr(self._h, which, ptr.data_ptr(), idx.data_ptr(), val.data_ptr()))
+        return ptr, idx, val
+
+
+def vmat_ddc_create(n_voxels: int, n_beamlets: int, coo_voxel: torch.Tensor, coo_beamlet: torch.Tensor,
+                    coo_val: torch.Tensor, angle_col_offset: torch.Tensor, angle_row_offset: torch.Tensor,
+                    leafrow_col_offset: torch.Tensor, device=None) -> DDC:
+    """A0: build both layouts from COO triplets (host or device tensors)."""
+    lib = load_library()
+    if not torch.cuda.is_available():
+        raise RuntimeError("vmat_ddc_create needs a CUDA device (there is no CPU fallback)")
+    dev = torch.device(device if device is not None else (coo_val.device if coo_val.is_cuda else "cuda:0"))
+    nnz = int(coo_val.numel())
+    if coo_voxel.numel() != nnz or coo_beamlet.numel() != nnz:
+        raise ValueError("the three COO vectors must have equal length (PAPER.md L115)")
+    offs = [t.to(torch.int32).cpu().contiguous() for t in (angle_col_offset, angle_row_offset, leafrow_col_offset)]
+    n_angles = offs[0].numel() - 1
+    if offs[1].numel() != n_angles + 1:
+        raise ValueError("angle_row_offset must have n_angles+1 entries")
+    if offs[2].numel() != int(offs[1][-1]) + 1:
+        raise ValueError("leafrow_col_offset must have n_leaf_rows+1 entries")
+    out = ctypes.c_void_p()
+    with torch.cuda.device(dev):
+        rc = lib.vmat_ddc_create(ctypes.byref(out), n_voxels, n_beamlets, nnz,
+                                 _ptr(coo_voxel, torch.int32), _ptr(coo_beamlet, torch.int32),
+                                 _ptr(coo_val, torch.float32), n_angles,
+                                 offs[0].data_ptr(), offs[1].data_ptr(), offs[2].data_ptr(), _stream())
+    _check(rc)
+    return DDC(out.value, dev)
+
+
+def vmat_dose(h: DDC, x: torch.Tensor, d: torch.Tensor):
+    """A1: d = D x."""
+    _check(load_library().vmat_dose(h._h, _ptr(x, torch.float32, "cuda", h.n_beamlets),
+                                    _ptr(d, torch.float32, "cuda", h.n_voxels), _stream()))
+
+
+def vmat_objective_grad(h: DDC, d: torch.Tensor, obj: Objective, g: torch.Tensor, F: torch.Tensor):
+    """A2: F and g = dF/dd (Eq. (1), Eq. (4))."""
+    _check(load_library().vmat_objective_grad(
+        h._h, _ptr(d, torch.float32, "cuda", h.n_voxels), _ptr(obj.voxel_struct, torch.uint8, "cuda", h.n_voxels),
+        obj.n_struct, _ptr(obj.T, torch.float32, "cuda"), _ptr(obj.w_over, torch.float32, "cuda"),
+        _ptr(obj.w_under, torch.float32, "cuda"), _ptr(g, torch.float32, "cuda", h.n_voxels),
+        _ptr(F, torch.float64, "cuda", 1), _stream()))
+
+
+def vmat_price(h: DDC, g: torch.Tensor, p: torch.Tensor):
+    """A3: p = D^T g (Eq. (3))."""
+    _check(load_library().vmat_price(h._h, _ptr(g, torch.float32, "cuda", h.n_voxels),
+                                     _ptr(p, torch.float32, "cuda", h.n_beamlets), _stream()))
+
+
+def vmat_select_apertures(h: DDC, p: torch.Tensor, angle_mask: Optional[torch.Tensor], L, R, row_price,
+                          angle_price, best_angle):
+    """A4 + A5: best opening per leaf row, aperture price per control point, best control point (L133)."""
+    _check(load_library().vmat_select_apertures(
+        h._h, _ptr(p, torch.float32, "cuda", h.n_beamlets), _ptr(angle_mask, torch.uint8, "cuda", h.n_angles),
+        _ptr(L, torch.int32, "cuda", h.n_leaf_rows), _ptr(R, torch.int32, "cuda", h.n_leaf_rows),
+        _ptr(row_price, torch.float64, "cuda", h.n_leaf_rows), _ptr(angle_price, torch.float64, "cuda", h.n_angles),
+        _ptr(best_angle, torch.int32, "cuda", 1), _stream()))
+
+
+def vmat_price_eval(h: DDC, x: torch.Tensor, obj: Objective, out: PriceEvalOut,
+                    angle_mask: Optional[torch.Tensor] = None):
+    """One whole price evaluation A1 -> A5 with the fused kernels; outputs are written into `out`."""
+    _check(load_library().vmat_price_eval(
+        h._h, _ptr(x, torch.float32, "cuda", h.n_beamlets), _ptr(obj.voxel_struct, torch.uint8, "cuda", h.n_voxels),
+        obj.n_struct, _ptr(obj.T, torch.float32, "cuda"), _ptr(obj.w_over, torch.float32, "cuda"),
+        _ptr(obj.w_under, torch.float32, "cuda"), _ptr(angle_mask, torch.uint8, "cuda", h.n_angles),
+        _ptr(out.d, torch.float32, "cuda", h.n_voxels), _ptr(out.g, torch.float32, "cuda", h.n_voxels),
+        _ptr(out.F, torch.float64, "cuda", 1), _ptr(out.p, torch.float32, "cuda", h.n_beamlets),
+        _ptr(out.L, torch.int32, "cuda", h.n_leaf_rows), _ptr(out.R, torch.int32, "cuda", h.n_leaf_rows),
+        _ptr(out.row_price, torch.float64, "cuda", h.n_leaf_rows),
+        _ptr(out.angle_price, torch.float64, "cuda", h.n_angles), _ptr(out.best_angle, torch.int32, "cuda", 1),
+        _stream()))
+
+
+def vmat_price_eval_host(h: DDC, x_host: torch.Tensor, obj: Objective, F_host, L_host, R_host, row_price_host,
+                         angle_price_host, best_angle_host, angle_mask: Optional[torch.Tensor] = None):
+    """End-to-end call with HOST buffers (x in, F/L/R/prices/best out); synchronises before returning."""
+    _check(load_library().vmat_price_eval_host(
+        h._h, _ptr(x_host, torch.float32, "cpu", h.n_beamlets), _ptr(obj.voxel_struct, torch.uint8, "cuda", h.n_voxels),
+        obj.n_struct, _ptr(obj.T, torch.float32, "cuda"), _ptr(obj.w_over, torch.float32, "cuda"),
+        _ptr(obj.w_under, torch.float32, "cuda"), _ptr(angle_mask, torch.uint8, "cuda", h.n_angles),
+        _ptr(F_host, torch.float64, "cpu", 1), _ptr(L_host, torch.int32, "cpu", h.n_leaf_rows),
+        _ptr(R_host, torch.int32, "cpu", h.n_leaf_rows), _ptr(row_price_host, torch.float64, "cpu", h.n_leaf_rows),
+        _ptr(angle_price_host, torch.float64, "cpu", h.n_angles), _ptr(best_angle_host, torch.int32, "cpu", 1),
+        _stream()))
+
+
+def vmat_aperture_dose(h: DDC, angle: int, L: torch.Tensor, R: torch.Tensor, x_scratch: torch.Tensor,
+                       DA: torch.Tensor):
+    """NEXT-1: DA(A_k) = sum_{j in A_k} D_:j (Eq. (5)) for the openings [L,R) of control point `angle`."""
+    _check(load_library().vmat_aperture_dose(
+        h._h, int(angle), _ptr(L, torch.int32, "cuda", h.n_leaf_rows), _ptr(R, torch.int32, "cuda", h.n_leaf_rows),
+        _ptr(x_scratch, torch.float32, "cuda", h.n_beamlets), _ptr(DA, torch.float32, "cuda", h.n_voxels), _stream()))
+
+
+def last_launch_count() -> int:
+    return int(load_library().vmat_last_launch_count())

@@ -1,0 +1,295 @@
+// api.cu - the extern "C" boundary of libvmat (include/vmat.h): argument checks, handle lifetime,
+// and the sequencing of the kernels on the caller's stream.  No arithmetic lives here.
+#include "common.cuh"
+#include <stdarg.h>
+#include <string.h>
+#include <new>
+#include <vector>
+
+static thread_local char g_err[512] = "";
+thread_local int g_vmat_launches = 0;
+
+void vmat_set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+#define REQUIRE(cond, msg)                                            \
+    do {                                                              \
+        if (!(cond)) { vmat_set_error("%s: %s", __func__, msg); return VMAT_ERR_INVALID_ARG; } \
+    } while (0)
+#define TRY(x) do { int rc_ = (x); if (rc_ != VMAT_OK) return rc_; } while (0)
+
+template <typename T>
+static int upload(T **dst, const T *src, int64_t n, int64_t *bytes)
+{
+    const size_t b = (size_t)(n > 0 ? n : 1) * sizeof(T);
+    VMAT_CUDA(cudaMalloc((void **)dst, b));
+    *bytes += (int64_t)b;
+    if (n > 0) VMAT_CUDA(cudaMemcpy(*dst, src, (size_t)n * sizeof(T), cudaMemcpyHostToDevice));
+    return VMAT_OK;
+}
+
+// PDL-free, graph-free sequencing: plain launches on the caller's stream.
+__global__ void k_aperture_indicator(int n_beamlets, float *__restrict__ x, int row0, int row1,
+                                     const int32_t *__restrict__ leafrow_col_offset,
+                                     const int32_t *__restrict__ L, const int32_t *__restrict__ R)
+{
+    // x = indicator of the aperture (Eq. (5): the beamlets within the chosen openings)
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n_beamlets) return;
+    float v = 0.f;
+    if (j >= leafrow_col_offset[row0] && j < leafrow_col_offset[row1]) {
+        int lo = row0, hi = row1;                       // leaf row of beamlet j: last row with offset <= j
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (leafrow_col_offset[mid] <= j) lo = mid; else hi = mid;
+        }
+        const int c = j - leafrow_col_offset[lo];
+        v = (c >= L[lo] && c < R[lo]) ? 1.f : 0.f;
+    }
+    x[j] = v;
+}
+
+extern "C" {
+
+const char *vmat_last_error(void) { return g_err; }
+int vmat_last_launch_count(void) { return g_vmat_launches; }
+
+int vmat_ddc_destroy(vmat_ddc *h)
+{
+    if (!h) return VMAT_OK;
+    void *ptrs[] = {h->D.ptr, h->D.idx, h->D.val, h->Dt.ptr, h->Dt.idx, h->Dt.val, h->angle_col_offset,
+                    h->angle_row_offset, h->leafrow_col_offset, h->leafrow_angle, h->blk_row, h->F_partial,
+                    h->F_partial_obj, h->S_scratch, h->e2e_x, h->e2e_d, h->e2e_g, h->e2e_p, h->e2e_L, h->e2e_R,
+                    h->e2e_best, h->e2e_row_price, h->e2e_angle_price, h->e2e_F};
+    for (void *p : ptrs)
+        if (p) cudaFree(p);
+    delete h;
+    return VMAT_OK;
+}
+
+int vmat_ddc_create(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int64_t nnz,
+                    const int32_t *coo_voxel, const int32_t *coo_beamlet, const float *coo_val,
+                    int32_t n_angles, const int32_t *angle_col_offset, const int32_t *angle_row_offset,
+                    const int32_t *leafrow_col_offset, void *stream)
+{
+    REQUIRE(out != nullptr, "out is NULL");
+    REQUIRE(n_voxels >= 0 && n_beamlets >= 0 && nnz >= 0 && n_angles >= 0, "negative size");
+    REQUIRE(nnz == 0 || (coo_voxel && coo_beamlet && coo_val), "COO pointer is NULL");
+    REQUIRE(nnz == 0 || (n_voxels > 0 && n_beamlets > 0), "nnz > 0 with an empty dimension");
+    REQUIRE(angle_col_offset && angle_row_offset && leafrow_col_offset, "offset table is NULL");
+    REQUIRE(angle_col_offset[0] == 0 && angle_row_offset[0] == 0 && leafrow_col_offset[0] == 0,
+            "offset tables must start at 0");
+    for (int a = 0; a < n_angles; ++a) {
+        REQUIRE(angle_col_offset[a + 1] >= angle_col_offset[a], "angle_col_offset not monotone");
+        REQUIRE(angle_row_offset[a + 1] >= angle_row_offset[a], "angle_row_offset not monotone");
+    }
+    REQUIRE(angle_col_offset[n_angles] == n_beamlets, "angle_col_offset must end at n_beamlets");
+    const int32_t n_rows = angle_row_offset[n_angles];
+    int32_t max_len = 0;
+    for (int r = 0; r < n_rows; ++r) {
+        REQUIRE(leafrow_col_offset[r + 1] >= leafrow_col_offset[r], "leafrow_col_offset not monotone");
+        max_len = leafrow_col_offset[r + 1] - leafrow_col_offset[r] > max_len
+                      ? leafrow_col_offset[r + 1] - leafrow_col_offset[r] : max_len;
+    }
+    REQUIRE(leafrow_col_offset[n_rows] == n_beamlets, "leafrow_col_offset must end at n_beamlets");
+    std::vector<int32_t> row_angle((size_t)(n_rows > 0 ? n_rows : 1), 0);
+    for (int a = 0; a < n_angles; ++a) {                 // leaf rows must not straddle control points
+        REQUIRE(leafrow_col_offset[angle_row_offset[a]] == angle_col_offset[a],
+                "leaf rows straddle a control point boundary");
+        for (int r = angle_row_offset[a]; r < angle_row_offset[a + 1]; ++r) row_angle[r] = a;
+    }
+
+    vmat_ddc *h = new (std::nothrow) vmat_ddc();
+    if (!h) { vmat_set_error("vmat_ddc_create: host allocation failed"); return VMAT_ERR_OOM; }
+    h->n_voxels = n_voxels; h->n_beamlets = n_beamlets; h->nnz = nnz;
+    h->n_angles = n_angles; h->n_leaf_rows = n_rows; h->max_leaf_row_len = max_len;
+    cudaGetDevice(&h->device);
+    h->h_angle_row_offset.assign(angle_row_offset, angle_row_offset + n_angles + 1);
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = vmat_build_layouts(h, coo_voxel, coo_beamlet, coo_val, st);
+    if (rc == VMAT_OK) rc = upload(&h->angle_col_offset, angle_col_offset, (int64_t)n_angles + 1, &h->bytes_device);
+    if (rc == VMAT_OK) rc = upload(&h->angle_row_offset, angle_row_offset, (int64_t)n_angles + 1, &h->bytes_device);
+    if (rc == VMAT_OK) rc = upload(&h->leafrow_col_offset, leafrow_col_offset, (int64_t)n_rows + 1, &h->bytes_device);
+    if (rc == VMAT_OK) rc = upload(&h->leafrow_angle, row_angle.data(), (int64_t)n_rows, &h->bytes_device);
+    if (rc == VMAT_OK && max_len > SELECT_MAX_ROW) {
+        const size_t b = ((size_t)n_beamlets + (size_t)n_rows + 1) * sizeof(double);
+        cudaError_t e = cudaMalloc((void **)&h->S_scratch, b);
+        if (e != cudaSuccess) { vmat_set_error("vmat_ddc_create: cudaMalloc(S_scratch) failed"); rc = VMAT_ERR_OOM; }
+        h->bytes_device += (int64_t)b;
+    }
+    if (rc == VMAT_OK) {
+        cudaError_t e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) { vmat_set_error("vmat_ddc_create: %s", cudaGetErrorString(e)); rc = VMAT_ERR_CUDA; }
+    }
+    if (rc != VMAT_OK) { vmat_ddc_destroy(h); cudaGetLastError(); return rc; }
+    *out = h;
+    return VMAT_OK;
+}
+
+int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info)
+{
+    REQUIRE(h && info, "NULL argument");
+    info->n_voxels = h->n_voxels; info->n_beamlets = h->n_beamlets; info->nnz = h->nnz;
+    info->n_angles = h->n_angles; info->n_leaf_rows = h->n_leaf_rows;
+    info->bytes_csr_d = 8 * h->nnz + 8 * ((int64_t)h->n_voxels + 1);
+    info->bytes_csr_dt = 8 * h->nnz + 8 * ((int64_t)h->n_beamlets + 1);
+    info->bytes_device_total = h->bytes_device;
+    info->n_dose_blocks = h->n_blocks;
+    info->max_leaf_row_len = h->max_leaf_row_len;
+    info->max_voxel_row_nnz = h->max_voxel_row_nnz;
+    info->max_beamlet_row_nnz = h->max_beamlet_row_nnz;
+    return VMAT_OK;
+}
+
+int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx, float *val)
+{
+    REQUIRE(h && ptr && (h->nnz == 0 || (idx && val)), "NULL argument");
+    REQUIRE(which == 0 || which == 1, "which must be 0 (D) or 1 (D^T)");
+    const CsrLayout &A = which == 0 ? h->D : h->Dt;
+    VMAT_CUDA(cudaDeviceSynchronize());
+    VMAT_CUDA(cudaMemcpy(ptr, A.ptr, ((size_t)A.n_rows + 1) * 8, cudaMemcpyDeviceToHost));
+    if (h->nnz > 0) {
+        VMAT_CUDA(cudaMemcpy(idx, A.idx, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost));
+        VMAT_CUDA(cudaMemcpy(val, A.val, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost));
+    }
+    return VMAT_OK;
+}
+
+int vmat_dose(const vmat_ddc *h, const float *x, float *d, void *stream)
+{
+    REQUIRE(h && (x || h->n_beamlets == 0) && (d || h->n_voxels == 0), "NULL argument");
+    g_vmat_launches = 0;
+    return vmat_launch_dose(h, x, d, false, nullptr, 0, nullptr, nullptr, nullptr, nullptr, nullptr,
+                            (cudaStream_t)stream);
+}
+
+int vmat_objective_grad(const vmat_ddc *h, const float *d, const uint8_t *voxel_struct, int32_t n_struct,
+                        const float *T, const float *w_over, const float *w_under,
+                        float *g, double *F, void *stream)
+{
+    REQUIRE(h && F && T && w_over && w_under, "NULL argument");
+    REQUIRE(h->n_voxels == 0 || (d && voxel_struct && g), "NULL argument");
+    REQUIRE(n_struct >= 1 && n_struct <= 256, "n_struct must be in 1..256");
+    g_vmat_launches = 0;
+    return vmat_launch_objective(h, d, voxel_struct, n_struct, T, w_over, w_under, g, F, (cudaStream_t)stream);
+}
+
+int vmat_price(const vmat_ddc *h, const float *g, float *p, void *stream)
+{
+    REQUIRE(h && (g || h->n_voxels == 0) && (p || h->n_beamlets == 0), "NULL argument");
+    g_vmat_launches = 0;
+    return vmat_launch_price(h, g, p, (cudaStream_t)stream);
+}
+
+int vmat_select_apertures(const vmat_ddc *h, const float *p, const uint8_t *angle_mask,
+                          int32_t *L, int32_t *R, double *row_price, double *angle_price,
+                          int32_t *best_angle, void *stream)
+{
+    REQUIRE(h && best_angle, "NULL argument");
+    REQUIRE(h->n_beamlets == 0 || p, "p is NULL");
+    REQUIRE(h->n_leaf_rows == 0 || (L && R && row_price), "NULL output");
+    REQUIRE(h->n_angles == 0 || angle_price, "angle_price is NULL");
+    g_vmat_launches = 0;
+    TRY(vmat_launch_select(h, p, angle_mask, L, R, row_price, (cudaStream_t)stream));
+    return vmat_launch_angle_price(h, row_price, angle_mask, angle_price, best_angle, (cudaStream_t)stream);
+}
+
+int vmat_price_eval(const vmat_ddc *h, const float *x,
+                    const uint8_t *voxel_struct, int32_t n_struct,
+                    const float *T, const float *w_over, const float *w_under,
+                    const uint8_t *angle_mask,
+                    float *d, float *g, double *F, float *p,
+                    int32_t *L, int32_t *R, double *row_price, double *angle_price,
+                    int32_t *best_angle, void *stream)
+{
+    REQUIRE(h && F && best_angle && T && w_over && w_under, "NULL argument");
+    REQUIRE(h->n_voxels == 0 || (d && g && voxel_struct), "NULL voxel vector");
+    REQUIRE(h->n_beamlets == 0 || (x && p), "NULL beamlet vector");
+    REQUIRE(h->n_leaf_rows == 0 || (L && R && row_price), "NULL leaf-row output");
+    REQUIRE(h->n_angles == 0 || angle_price, "angle_price is NULL");
+    REQUIRE(n_struct >= 1 && n_struct <= 256, "n_struct must be in 1..256");
+    cudaStream_t st = (cudaStream_t)stream;
+    g_vmat_launches = 0;
+    TRY(vmat_launch_dose(h, x, d, true, voxel_struct, n_struct, T, w_over, w_under, g, F, st));
+    if (h->prof_ev[2]) VMAT_CUDA(cudaEventRecord(h->prof_ev[2], st));
+    if (h->max_leaf_row_len <= SELECT_MAX_ROW) {
+        TRY(vmat_launch_price_select(h, g, angle_mask, p, L, R, row_price, st));
+    } else {
+        TRY(vmat_launch_price(h, g, p, st));
+        TRY(vmat_launch_select(h, p, angle_mask, L, R, row_price, st));
+    }
+    if (h->prof_ev[3]) VMAT_CUDA(cudaEventRecord(h->prof_ev[3], st));
+    return vmat_launch_angle_price(h, row_price, angle_mask, angle_price, best_angle, st);
+}
+
+int vmat_ddc_set_profile_events(vmat_ddc *h, void *const *ev)
+{
+    REQUIRE(h != nullptr, "handle is NULL");
+    for (int i = 0; i < 4; ++i) h->prof_ev[i] = ev ? (cudaEvent_t)ev[i] : nullptr;
+    return VMAT_OK;
+}
+
+int vmat_price_eval_host(vmat_ddc *h, const float *x_host,
+                         const uint8_t *voxel_struct, int32_t n_struct,
+                         const float *T, const float *w_over, const float *w_under,
+                         const uint8_t *angle_mask,
+                         double *F_host, int32_t *L_host, int32_t *R_host, double *row_price_host,
+                         double *angle_price_host, int32_t *best_angle_host, void *stream)
+{
+    REQUIRE(h && F_host && best_angle_host, "NULL argument");
+    REQUIRE(h->n_beamlets == 0 || x_host, "x_host is NULL");
+    REQUIRE(h->n_leaf_rows == 0 || (L_host && R_host && row_price_host), "NULL leaf-row output");
+    REQUIRE(h->n_angles == 0 || angle_price_host, "angle_price_host is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!h->e2e_F) {                                      // device scratch, allocated once
+        const size_t nv = h->n_voxels > 0 ? h->n_voxels : 1, nb = h->n_beamlets > 0 ? h->n_beamlets : 1;
+        const size_t nr = h->n_leaf_rows > 0 ? h->n_leaf_rows : 1, na = h->n_angles > 0 ? h->n_angles : 1;
+        VMAT_CUDA(cudaMalloc((void **)&h->e2e_x, nb * 4));
+        VMAT_CUDA(cudaMalloc((void **)&h->e2e_p, nb * 4));
+        VMAT_CUDA(cudaMalloc((void **)&h->e2e_d, nv * 4));
+        VMAT_CUDA(cudaMalloc((void **)&h->e2e_g, nv * 4));
+        VMAT_CUDA(cudaMalloc((void **)&h->e2e_L, nr * 4));
+        VMAT_CUDA(cudaMalloc((void **)&h->e2e_R, nr * 4));
+        VMAT_CUDA(cudaMalloc((void **)&h->e2e_row_price, nr * 8));
+        VMAT_CUDA(cudaMalloc((void **)&h->e2e_angle_price, na * 8));
+        VMAT_CUDA(cudaMalloc((void **)&h->e2e_best, 4));
+        VMAT_CUDA(cudaMalloc((void **)&h->e2e_F, 8));
+        h->bytes_device += (int64_t)(8 * nb + 8 * nv + 16 * nr + 8 * na + 12);
+    }
+    if (h->n_beamlets > 0)
+        VMAT_CUDA(cudaMemcpyAsync(h->e2e_x, x_host, (size_t)h->n_beamlets * 4, cudaMemcpyHostToDevice, st));
+    TRY(vmat_price_eval(h, h->e2e_x, voxel_struct, n_struct, T, w_over, w_under, angle_mask, h->e2e_d, h->e2e_g,
+                        h->e2e_F, h->e2e_p, h->e2e_L, h->e2e_R, h->e2e_row_price, h->e2e_angle_price, h->e2e_best, st));
+    if (h->n_leaf_rows > 0) {
+        VMAT_CUDA(cudaMemcpyAsync(L_host, h->e2e_L, (size_t)h->n_leaf_rows * 4, cudaMemcpyDeviceToHost, st));
+        VMAT_CUDA(cudaMemcpyAsync(R_host, h->e2e_R, (size_t)h->n_leaf_rows * 4, cudaMemcpyDeviceToHost, st));
+        VMAT_CUDA(cudaMemcpyAsync(row_price_host, h->e2e_row_price, (size_t)h->n_leaf_rows * 8, cudaMemcpyDeviceToHost, st));
+    }
+    if (h->n_angles > 0)
+        VMAT_CUDA(cudaMemcpyAsync(angle_price_host, h->e2e_angle_price, (size_t)h->n_angles * 8, cudaMemcpyDeviceToHost, st));
+    VMAT_CUDA(cudaMemcpyAsync(best_angle_host, h->e2e_best, 4, cudaMemcpyDeviceToHost, st));
+    VMAT_CUDA(cudaMemcpyAsync(F_host, h->e2e_F, 8, cudaMemcpyDeviceToHost, st));
+    VMAT_CUDA(cudaStreamSynchronize(st));
+    return VMAT_OK;
+}
+
+int vmat_aperture_dose(const vmat_ddc *h, int32_t angle, const int32_t *L, const int32_t *R,
+                       float *x_scratch, float *DA, void *stream)
+{
+    REQUIRE(h && L && R && x_scratch && DA, "NULL argument");
+    REQUIRE(angle >= 0 && angle < h->n_angles, "angle out of range");
+    cudaStream_t st = (cudaStream_t)stream;
+    g_vmat_launches = 0;
+    const int32_t aro[2] = {h->h_angle_row_offset[angle], h->h_angle_row_offset[angle + 1]};
+    k_aperture_indicator<<<(h->n_beamlets + 255) / 256, 256, 0, st>>>(h->n_beamlets, x_scratch, aro[0], aro[1],
+                                                                      h->leafrow_col_offset, L, R);
+    VMAT_LAUNCH_CHECK();
+    return vmat_launch_dose(h, x_scratch, DA, false, nullptr, 0, nullptr, nullptr, nullptr, nullptr, nullptr, st);
+}
+
+}  // extern "C"

@@ -1,0 +1,118 @@
+// common.cuh - handle layout, error plumbing and load helpers shared by the libvmat kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <vector>
+#include "../../include/vmat.h"
+
+// ------------------------------------------------------------------ error plumbing
+void vmat_set_error(const char *fmt, ...);
+extern thread_local int g_vmat_launches;
+
+#define VMAT_CUDA(call)                                                                     \
+    do {                                                                                    \
+        cudaError_t e_ = (call);                                                            \
+        if (e_ != cudaSuccess) {                                                            \
+            vmat_set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            return (e_ == cudaErrorMemoryAllocation) ? VMAT_ERR_OOM : VMAT_ERR_CUDA;        \
+        }                                                                                   \
+    } while (0)
+
+#define VMAT_LAUNCH_CHECK()                                                                 \
+    do {                                                                                    \
+        ++g_vmat_launches;                                                                  \
+        cudaError_t e_ = cudaGetLastError();                                                \
+        if (e_ != cudaSuccess) {                                                            \
+            vmat_set_error("%s:%d: kernel launch -> %s", __FILE__, __LINE__, cudaGetErrorString(e_)); \
+            return VMAT_ERR_CUDA;                                                           \
+        }                                                                                   \
+    } while (0)
+
+// ------------------------------------------------------------------ one CSR layout on the device
+struct CsrLayout {
+    int32_t n_rows = 0;
+    int64_t nnz = 0;
+    int64_t *ptr = nullptr;   // [n_rows+1]
+    int32_t *idx = nullptr;   // [nnz (+pad)]  secondary index, ascending within a row
+    float   *val = nullptr;   // [nnz (+pad)]
+};
+
+// ------------------------------------------------------------------ the handle
+struct vmat_ddc {
+    int32_t n_voxels = 0, n_beamlets = 0, n_angles = 0, n_leaf_rows = 0;
+    int64_t nnz = 0;
+    CsrLayout D;    // rows = voxels,   idx = beamlet   (for d = D x)
+    CsrLayout Dt;   // rows = beamlets, idx = voxel     (for p = D^T g; the paper's format, L121)
+    // offset tables (device)
+    int32_t *angle_col_offset = nullptr;    // [n_angles+1]
+    int32_t *angle_row_offset = nullptr;    // [n_angles+1]
+    int32_t *leafrow_col_offset = nullptr;  // [n_leaf_rows+1]
+    int32_t *leafrow_angle = nullptr;       // [n_leaf_rows] control point of each leaf row
+    // dose kernel work list: row block b covers voxel rows [blk_row[b], blk_row[b+1])
+    int32_t *blk_row = nullptr;             // [n_blocks+1]
+    int32_t n_blocks = 0;
+    double *F_partial = nullptr;            // [n_blocks] per-block objective partials
+    int32_t n_obj_blocks = 0;               // blocks of the standalone objective kernel
+    double *F_partial_obj = nullptr;        // [n_obj_blocks]
+    double *S_scratch = nullptr;            // prefix-sum scratch for leaf rows longer than SELECT_MAX_ROW
+    std::vector<int32_t> h_angle_row_offset; // host copy
+    int32_t max_leaf_row_len = 0;
+    int64_t max_voxel_row_nnz = 0, max_beamlet_row_nnz = 0;
+    int64_t bytes_device = 0;
+    int device = 0;
+    cudaEvent_t prof_ev[4] = {nullptr, nullptr, nullptr, nullptr};   // vmat_ddc_set_profile_events
+    // scratch for the end-to-end host call (allocated on first use)
+    float *e2e_x = nullptr, *e2e_d = nullptr, *e2e_g = nullptr, *e2e_p = nullptr;
+    int32_t *e2e_L = nullptr, *e2e_R = nullptr, *e2e_best = nullptr;
+    double *e2e_row_price = nullptr, *e2e_angle_price = nullptr, *e2e_F = nullptr;
+};
+
+// ------------------------------------------------------------------ tuning constants
+// Dose kernel (CSR-stream): one CTA per row block; products staged in shared memory.
+constexpr int DOSE_THREADS = 256;
+constexpr int DOSE_BLOCK_NNZ = 4096;        // products per block held in smem (16 KB)
+constexpr int DOSE_MAX_ROWS = 1024;         // rows per block (bounds runs of empty rows)
+// Price kernel (CSR-vector, one warp per beamlet row, L127).
+constexpr int PRICE_THREADS = 256;
+constexpr int PRICE_WARPS = PRICE_THREADS / 32;
+constexpr int SELECT_MAX_ROW = 2048;        // longest leaf row the fused price+select kernel takes
+
+// ------------------------------------------------------------------ load helpers
+// Matrix streams are read exactly once per evaluation.  sm_100 has 256-bit global loads
+// (SASS LDG.E.256); they carry the L2::evict_first priority, and L1::no_allocate keeps the
+// stream out of L1, so the 16-64 GB of matrix data do not wash the gathered vector (x or g,
+// <= a few MB) out of the caches.  The address must be 32-byte aligned.
+struct Vec8 { uint32_t w[8]; };
+__device__ __forceinline__ Vec8 ld_stream_256(const void *p)
+{
+    Vec8 r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::evict_first.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r.w[0]), "=r"(r.w[1]), "=r"(r.w[2]), "=r"(r.w[3]),
+                   "=r"(r.w[4]), "=r"(r.w[5]), "=r"(r.w[6]), "=r"(r.w[7]) : "l"(p));
+    return r;
+}
+// Gathered vector (x or g): read-only path, allocated in L1 with evict-last priority.
+__device__ __forceinline__ float ld_gather(const float *p)
+{
+    float r;
+    asm volatile("ld.global.nc.L1::evict_last.f32 %0, [%1];" : "=f"(r) : "l"(p));
+    return r;
+}
+
+// ------------------------------------------------------------------ internal entry points
+int vmat_build_layouts(vmat_ddc *h, const int32_t *coo_voxel, const int32_t *coo_beamlet,
+                       const float *coo_val, cudaStream_t st);
+int vmat_launch_dose(const vmat_ddc *h, const float *x, float *d, bool fuse,
+                     const uint8_t *voxel_struct, int32_t n_struct, const float *T, const float *w_over,
+                     const float *w_under, float *g, double *F, cudaStream_t st);
+int vmat_launch_objective(const vmat_ddc *h, const float *d, const uint8_t *voxel_struct, int32_t n_struct,
+                          const float *T, const float *w_over, const float *w_under, float *g, double *F,
+                          cudaStream_t st);
+int vmat_launch_price(const vmat_ddc *h, const float *g, float *p, cudaStream_t st);
+int vmat_launch_select(const vmat_ddc *h, const float *p, const uint8_t *angle_mask, int32_t *L, int32_t *R,
+                       double *row_price, cudaStream_t st);
+int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *angle_mask, float *p,
+                             int32_t *L, int32_t *R, double *row_price, cudaStream_t st);
+int vmat_launch_angle_price(const vmat_ddc *h, const double *row_price, const uint8_t *angle_mask,
+                            double *angle_price, int32_t *best_angle, cudaStream_t st);

@@ -1,0 +1,216 @@
+// dose.cu - A1 forward dose d = D x through the voxel-row CSR, with the
+// objective / gradient (Eq. (1), Eq. (4)) fused into the row epilogue (A2).
+//
+// Voxel rows are ragged (0 ... ~18 k non-zeros, mean 10^2-10^3), so rows are not mapped to warps
+// one by one.  The ingest step cuts the row range into blocks of <= DOSE_BLOCK_NNZ non-zeros
+// (a row longer than that is a block of its own); one CTA per block:
+//   several rows : the whole CTA streams the block's contiguous (val, idx) range with 256-bit loads,
+//                  multiplies by the gathered x and parks the products in shared memory; then groups
+//                  of G lanes (G sized to the block's mean row length) reduce one row each with
+//                  shuffles.  Streaming is perfectly coalesced whatever the row lengths are.
+//   one row      : all threads accumulate the row in registers; one block reduction.
+// Everything is FP32 with a fixed summation order; the objective partials are FP64, one per block,
+// summed afterwards in a fixed order (no atomics).
+#include "spmv.cuh"
+
+struct ObjTables {              // per-structure parameters staged in shared memory
+    float T[256], wo[256], wu[256];
+};
+
+// g_i and the voxel's term of F for dose v (Eq. (1); sign and factor 2: C1, C2)
+__device__ __forceinline__ float voxel_grad(float v, float T, float wo, float wu, double &f)
+{
+    const float over = fmaxf(v - T, 0.f);
+    const float under = fmaxf(T - v, 0.f);
+    f += (double)wo * ((double)over * (double)over) + (double)wu * ((double)under * (double)under);
+    return 2.f * wo * over - 2.f * wu * under;
+}
+
+// deterministic block sum of doubles; result valid in thread 0
+template <int NT>
+__device__ __forceinline__ double block_sum_double(double v, double *red /* [NT/32] */)
+{
+    v = warp_sum(v);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) red[w] = v;
+    __syncthreads();
+    double s = 0.0;
+    if (threadIdx.x == 0)
+        for (int i = 0; i < NT / 32; ++i) s += red[i];
+    return s;
+}
+
+template <bool FUSE>
+__global__ void __launch_bounds__(DOSE_THREADS)
+k_dose(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const float *__restrict__ val,
+       const int32_t *__restrict__ blk_row, const float *__restrict__ x, float *__restrict__ d,
+       const uint8_t *__restrict__ vstruct, int n_struct, const float *__restrict__ T,
+       const float *__restrict__ w_over, const float *__restrict__ w_under, float *__restrict__ g,
+       double *__restrict__ F_partial)
+{
+    __shared__ __align__(32) float prod[DOSE_BLOCK_NNZ + 8];
+    __shared__ float red_f[DOSE_THREADS / 32];
+    __shared__ double red_d[DOSE_THREADS / 32];
+    __shared__ ObjTables tab;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (FUSE) {
+        for (int i = tid; i < n_struct; i += DOSE_THREADS) {
+            tab.T[i] = T[i];
+            tab.wo[i] = w_over[i];
+            tab.wu[i] = w_under[i];
+        }
+        __syncthreads();
+    }
+    const int r0 = blk_row[blockIdx.x], r1 = blk_row[blockIdx.x + 1];
+    const int nr = r1 - r0;
+    const int64_t s = ptr[r0], e = ptr[r1];
+    double fsum = 0.0;
+
+    if (nr == 1) {
+        // ---- one row: register accumulation by the whole CTA
+        float acc = strided_row_dot<DOSE_THREADS>(val, idx, s, e, x, tid);
+        acc = warp_sum(acc);
+        if (lane == 0) red_f[warp] = acc;
+        __syncthreads();
+        if (tid == 0) {
+            float tot = 0.f;
+#pragma unroll
+            for (int i = 0; i < DOSE_THREADS / 32; ++i) tot += red_f[i];
+            d[r0] = tot;
+            if (FUSE) {
+                const int sid = vstruct[r0];
+                g[r0] = voxel_grad(tot, tab.T[sid], tab.wo[sid], tab.wu[sid], fsum);
+            }
+        }
+    } else {
+        // ---- several rows: stream products into shared memory ...
+        const int64_t a = s & ~int64_t(7);
+        for (int64_t k = a + (int64_t)tid * 8; k < e; k += (int64_t)DOSE_THREADS * 16) {
+            const int64_t k2 = k + (int64_t)DOSE_THREADS * 8;
+            const bool has2 = k2 < e;
+            Vec8 v0 = ld_stream_256(val + k);
+            Vec8 c0 = ld_stream_256(idx + k);
+            Vec8 v1, c1;
+            if (has2) {
+                v1 = ld_stream_256(val + k2);
+                c1 = ld_stream_256(idx + k2);
+            }
+            float q[8];
+#pragma unroll
+            for (int t = 0; t < 8; ++t) q[t] = __uint_as_float(v0.w[t]) * ld_gather(x + c0.w[t]);
+            float4 *dst = reinterpret_cast<float4 *>(prod + (k - a));
+            dst[0] = make_float4(q[0], q[1], q[2], q[3]);
+            dst[1] = make_float4(q[4], q[5], q[6], q[7]);
+            if (has2) {
+#pragma unroll
+                for (int t = 0; t < 8; ++t) q[t] = __uint_as_float(v1.w[t]) * ld_gather(x + c1.w[t]);
+                dst = reinterpret_cast<float4 *>(prod + (k2 - a));
+                dst[0] = make_float4(q[0], q[1], q[2], q[3]);
+                dst[1] = make_float4(q[4], q[5], q[6], q[7]);
+            }
+        }
+        __syncthreads();
+        // ... then G lanes per row, G = power of two near (mean row length)/4, 1..32
+        const int mean = (int)((e - s) / nr);
+        int G = 1;
+        while (G < 32 && G * 4 < mean) G <<= 1;
+        const int grp = tid / G, gl = tid % G, n_grp = DOSE_THREADS / G;
+        const int n_iter = (nr + n_grp - 1) / n_grp;            // uniform trip count: shuffles stay converged
+        for (int it = 0; it < n_iter; ++it) {
+            const int r = r0 + grp + it * n_grp;
+            float acc = 0.f;
+            if (r < r1) {
+                const int b = (int)(ptr[r] - a), f = (int)(ptr[r + 1] - a);
+                for (int k = b + gl; k < f; k += G) acc += prod[k];
+            }
+            for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+            if (r < r1 && gl == 0) {
+                d[r] = acc;
+                if (FUSE) {
+                    const int sid = vstruct[r];
+                    g[r] = voxel_grad(acc, tab.T[sid], tab.wo[sid], tab.wu[sid], fsum);
+                }
+            }
+        }
+    }
+    if (FUSE) {
+        const double tot = block_sum_double<DOSE_THREADS>(fsum, red_d);
+        if (tid == 0) F_partial[blockIdx.x] = tot;
+    }
+}
+
+// Standalone A2 (vmat_objective_grad): one thread per voxel, FP64 partial per block.
+constexpr int OBJ_THREADS = 256;
+__global__ void __launch_bounds__(OBJ_THREADS)
+k_objective(int n_voxels, const float *__restrict__ d, const uint8_t *__restrict__ vstruct, int n_struct,
+            const float *__restrict__ T, const float *__restrict__ w_over, const float *__restrict__ w_under,
+            float *__restrict__ g, double *__restrict__ F_partial)
+{
+    __shared__ ObjTables tab;
+    __shared__ double red_d[OBJ_THREADS / 32];
+    for (int i = threadIdx.x; i < n_struct; i += OBJ_THREADS) {
+        tab.T[i] = T[i];
+        tab.wo[i] = w_over[i];
+        tab.wu[i] = w_under[i];
+    }
+    __syncthreads();
+    const int i = blockIdx.x * OBJ_THREADS + threadIdx.x;
+    double f = 0.0;
+    if (i < n_voxels) {
+        const int sid = vstruct[i];
+        g[i] = voxel_grad(d[i], tab.T[sid], tab.wo[sid], tab.wu[sid], f);
+    }
+    const double tot = block_sum_double<OBJ_THREADS>(f, red_d);
+    if (threadIdx.x == 0) F_partial[blockIdx.x] = tot;
+}
+
+// F = sum of the per-block partials, fixed order: thread t sums part[t], part[t+1024], ...; then a tree.
+constexpr int SUM_THREADS = 1024;
+__global__ void __launch_bounds__(SUM_THREADS)
+k_sum_partials(const double *__restrict__ part, int n, double *__restrict__ out)
+{
+    __shared__ double red_d[SUM_THREADS / 32];
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n; i += SUM_THREADS) s += part[i];
+    const double tot = block_sum_double<SUM_THREADS>(s, red_d);
+    if (threadIdx.x == 0) out[0] = tot;
+}
+
+int vmat_launch_dose(const vmat_ddc *h, const float *x, float *d, bool fuse,
+                     const uint8_t *voxel_struct, int32_t n_struct, const float *T, const float *w_over,
+                     const float *w_under, float *g, double *F, cudaStream_t st)
+{
+    if (fuse && h->prof_ev[0]) VMAT_CUDA(cudaEventRecord(h->prof_ev[0], st));
+    if (h->n_blocks > 0) {
+        if (fuse)
+            k_dose<true><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.ptr, h->D.idx, h->D.val, h->blk_row, x, d,
+                                                               voxel_struct, n_struct, T, w_over, w_under, g,
+                                                               h->F_partial);
+        else
+            k_dose<false><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.ptr, h->D.idx, h->D.val, h->blk_row, x, d,
+                                                                nullptr, 0, nullptr, nullptr, nullptr, nullptr,
+                                                                nullptr);
+        VMAT_LAUNCH_CHECK();
+    }
+    if (fuse && h->prof_ev[1]) VMAT_CUDA(cudaEventRecord(h->prof_ev[1], st));
+    if (fuse) {
+        k_sum_partials<<<1, SUM_THREADS, 0, st>>>(h->F_partial, h->n_blocks, F);
+        VMAT_LAUNCH_CHECK();
+    }
+    return VMAT_OK;
+}
+
+int vmat_launch_objective(const vmat_ddc *h, const float *d, const uint8_t *voxel_struct, int32_t n_struct,
+                          const float *T, const float *w_over, const float *w_under, float *g, double *F,
+                          cudaStream_t st)
+{
+    if (h->n_obj_blocks > 0) {
+        k_objective<<<h->n_obj_blocks, OBJ_THREADS, 0, st>>>(h->n_voxels, d, voxel_struct, n_struct, T, w_over,
+                                                             w_under, g, h->F_partial_obj);
+        VMAT_LAUNCH_CHECK();
+    }
+    k_sum_partials<<<1, SUM_THREADS, 0, st>>>(h->F_partial_obj, h->n_obj_blocks, F);
+    VMAT_LAUNCH_CHECK();
+    return VMAT_OK;
+}

@@ -1,0 +1,219 @@
+// price.cu - A3 beamlet prices p = D^T g (Eq. (3), "Pi = D^T g" L121) through the
+// beamlet-row CSR, A4 per-leaf-row best opening and A5 aperture price / best control point (L133).
+//
+// Beamlet rows are long and even (a radius-`cutoff` cylinder through the body: 10^3-10^4 non-zeros),
+// so the paper's mapping holds on sm_100a: one warp per beamlet row (L127), here with 256-bit loads
+// and 128 B per lane in flight.  In the fused kernel a CTA owns one MLC leaf row: its warps price the
+// row's beamlets, the prices stay in shared memory, and the CTA then selects the row's opening - the
+// selection never re-reads p from HBM and costs no launch.
+//
+// Selection arithmetic (readings C4-C6, C8): S_0 = 0, S_{c+1} = S_c + (double)p_c left to
+// right in FP64; candidates all 0 <= L <= R <= n with V = S_R - S_L; result = smallest (V, L, R).
+// All pairs are enumerated - the definition itself, n <= ~10^2 - so the leaf positions are
+// bit-identical to the exhaustive CPU definition for the same FP32 p.
+#include "spmv.cuh"
+
+struct Opening {
+    double V;
+    int L, R;
+};
+__device__ __forceinline__ bool opening_less(const Opening &a, const Opening &b)
+{
+    if (a.V != b.V) return a.V < b.V;
+    if (a.L != b.L) return a.L < b.L;
+    return a.R < b.R;
+}
+
+// Best opening of one leaf row whose n FP32 prices are sp[0..n).  S: n+1 doubles of scratch.
+// Executed by all NT threads of the CTA; the result is returned in thread 0.
+template <int NT>
+__device__ __forceinline__ Opening select_row(const float *sp, int n, double *S, Opening *red /* [NT/32] */)
+{
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        S[0] = 0.0;
+        for (int c = 0; c < n; ++c) {
+            s = s + (double)sp[c];                 // strictly left to right
+            S[c + 1] = s;
+        }
+    }
+    __syncthreads();
+    Opening best = {0.0, 0, 0};                    // the closed opening (C4)
+    for (int L = threadIdx.x; L <= n; L += NT) {
+        const double SL = S[L];
+        for (int R = L; R <= n; ++R) {
+            const double V = S[R] - SL;
+            if (V < best.V) { best.V = V; best.L = L; best.R = R; }   // visited in (L,R) order: strict < keeps the first
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        Opening other;
+        other.V = __shfl_xor_sync(0xffffffffu, best.V, o);
+        other.L = __shfl_xor_sync(0xffffffffu, best.L, o);
+        other.R = __shfl_xor_sync(0xffffffffu, best.R, o);
+        if (opening_less(other, best)) best = other;
+    }
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = best;
+    __syncthreads();
+    if (threadIdx.x == 0)
+        for (int i = 1; i < NT / 32; ++i)
+            if (opening_less(red[i], best)) best = red[i];
+    return best;
+}
+
+// ---------------------------------------------------------------- A3 alone: one warp per beamlet row
+__global__ void __launch_bounds__(PRICE_THREADS)
+k_price(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const float *__restrict__ val,
+        int n_rows, const float *__restrict__ g, float *__restrict__ p)
+{
+    const int lane = threadIdx.x & 31;
+    const int row = blockIdx.x * PRICE_WARPS + (threadIdx.x >> 5);
+    if (row >= n_rows) return;
+    float acc = strided_row_dot<32>(val, idx, ptr[row], ptr[row + 1], g, lane);
+    acc = warp_sum(acc);
+    if (lane == 0) p[row] = acc;
+}
+
+// ---------------------------------------------------------------- A3 + A4 fused: one CTA per leaf row
+__global__ void __launch_bounds__(PRICE_THREADS)
+k_price_select(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const float *__restrict__ val,
+               const float *__restrict__ g, const int32_t *__restrict__ leafrow_col_offset,
+               const int32_t *__restrict__ leafrow_angle, const uint8_t *__restrict__ angle_mask,
+               float *__restrict__ p, int32_t *__restrict__ Lout, int32_t *__restrict__ Rout,
+               double *__restrict__ row_price)
+{
+    __shared__ double S[SELECT_MAX_ROW + 1];
+    __shared__ float sp[SELECT_MAX_ROW];
+    __shared__ Opening red[PRICE_WARPS];
+    const int r = blockIdx.x;
+    const int j0 = leafrow_col_offset[r];
+    const int n = leafrow_col_offset[r + 1] - j0;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int c = warp; c < n; c += PRICE_WARPS) {
+        const int row = j0 + c;
+        float acc = strided_row_dot<32>(val, idx, ptr[row], ptr[row + 1], g, lane);
+        acc = warp_sum(acc);
+        if (lane == 0) {
+            p[row] = acc;
+            sp[c] = acc;
+        }
+    }
+    __syncthreads();
+    const bool occupied = angle_mask != nullptr && angle_mask[leafrow_angle[r]] != 0;    // C7
+    Opening best = select_row<PRICE_THREADS>(sp, occupied ? 0 : n, S, red);
+    if (threadIdx.x == 0) {
+        Lout[r] = best.L;
+        Rout[r] = best.R;
+        row_price[r] = best.V;
+    }
+}
+
+// ---------------------------------------------------------------- A4 alone (vmat_select_apertures)
+// S_glob: global scratch of n_beamlets + n_leaf_rows doubles, used only by rows longer than
+// SELECT_MAX_ROW (NULL when no such row exists).
+__global__ void __launch_bounds__(PRICE_THREADS)
+k_select(const float *__restrict__ p, const int32_t *__restrict__ leafrow_col_offset,
+         const int32_t *__restrict__ leafrow_angle, const uint8_t *__restrict__ angle_mask,
+         double *__restrict__ S_glob, int32_t *__restrict__ Lout, int32_t *__restrict__ Rout,
+         double *__restrict__ row_price)
+{
+    __shared__ double S[SELECT_MAX_ROW + 1];
+    __shared__ float sp[SELECT_MAX_ROW];
+    __shared__ Opening red[PRICE_WARPS];
+    const int r = blockIdx.x;
+    const int j0 = leafrow_col_offset[r];
+    int n = leafrow_col_offset[r + 1] - j0;
+    if (angle_mask != nullptr && angle_mask[leafrow_angle[r]] != 0) n = 0;               // C7
+    Opening best;
+    if (n <= SELECT_MAX_ROW) {
+        for (int c = threadIdx.x; c < n; c += PRICE_THREADS) sp[c] = p[j0 + c];
+        __syncthreads();
+        best = select_row<PRICE_THREADS>(sp, n, S, red);
+    } else {
+        best = select_row<PRICE_THREADS>(p + j0, n, S_glob + j0 + r, red);
+    }
+    if (threadIdx.x == 0) {
+        Lout[r] = best.L;
+        Rout[r] = best.R;
+        row_price[r] = best.V;
+    }
+}
+
+// ---------------------------------------------------------------- A5: aperture price per control point, best one
+constexpr int ANGLE_THREADS = 256;
+__global__ void __launch_bounds__(ANGLE_THREADS)
+k_angle_price(int n_angles, const int32_t *__restrict__ angle_row_offset, const double *__restrict__ row_price,
+              const uint8_t *__restrict__ angle_mask, double *__restrict__ angle_price,
+              int32_t *__restrict__ best_angle)
+{
+    __shared__ double bv[ANGLE_THREADS / 32];
+    __shared__ int bi[ANGLE_THREADS / 32];
+    double best = 0.0;           // only a strictly negative price improves F (L56)
+    int besta = -1;
+    for (int a = threadIdx.x; a < n_angles; a += ANGLE_THREADS) {
+        double s;
+        if (angle_mask != nullptr && angle_mask[a] != 0) {
+            s = __longlong_as_double(0x7ff0000000000000LL);          // +inf: occupied (C7)
+        } else {
+            s = 0.0;
+            for (int r = angle_row_offset[a]; r < angle_row_offset[a + 1]; ++r) s += row_price[r];   // row order
+        }
+        angle_price[a] = s;
+        if (s < best) { best = s; besta = a; }                       // ascending a: strict < keeps the smallest a
+    }
+    // reduce (value, index): smaller value wins, ties -> smaller index; -1 means "none"
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+        const int oa = __shfl_xor_sync(0xffffffffu, besta, o);
+        if (oa >= 0 && (besta < 0 || ov < best || (ov == best && oa < besta))) { best = ov; besta = oa; }
+    }
+    if ((threadIdx.x & 31) == 0) { bv[threadIdx.x >> 5] = best; bi[threadIdx.x >> 5] = besta; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int i = 1; i < ANGLE_THREADS / 32; ++i)
+            if (bi[i] >= 0 && (besta < 0 || bv[i] < best || (bv[i] == best && bi[i] < besta))) { best = bv[i]; besta = bi[i]; }
+        best_angle[0] = besta;
+    }
+}
+
+// ---------------------------------------------------------------- launchers
+int vmat_launch_price(const vmat_ddc *h, const float *g, float *p, cudaStream_t st)
+{
+    if (h->n_beamlets == 0) return VMAT_OK;
+    const int grid = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
+    k_price<<<grid, PRICE_THREADS, 0, st>>>(h->Dt.ptr, h->Dt.idx, h->Dt.val, h->n_beamlets, g, p);
+    VMAT_LAUNCH_CHECK();
+    return VMAT_OK;
+}
+
+int vmat_launch_select(const vmat_ddc *h, const float *p, const uint8_t *angle_mask, int32_t *L, int32_t *R,
+                       double *row_price, cudaStream_t st)
+{
+    if (h->n_leaf_rows == 0) return VMAT_OK;
+    k_select<<<h->n_leaf_rows, PRICE_THREADS, 0, st>>>(p, h->leafrow_col_offset, h->leafrow_angle, angle_mask,
+                                                       h->S_scratch, L, R, row_price);
+    VMAT_LAUNCH_CHECK();
+    return VMAT_OK;
+}
+
+int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *angle_mask, float *p,
+                             int32_t *L, int32_t *R, double *row_price, cudaStream_t st)
+{
+    if (h->n_leaf_rows == 0) return VMAT_OK;
+    k_price_select<<<h->n_leaf_rows, PRICE_THREADS, 0, st>>>(h->Dt.ptr, h->Dt.idx, h->Dt.val, g,
+                                                             h->leafrow_col_offset, h->leafrow_angle, angle_mask,
+                                                             p, L, R, row_price);
+    VMAT_LAUNCH_CHECK();
+    return VMAT_OK;
+}
+
+int vmat_launch_angle_price(const vmat_ddc *h, const double *row_price, const uint8_t *angle_mask,
+                            double *angle_price, int32_t *best_angle, cudaStream_t st)
+{
+    k_angle_price<<<1, ANGLE_THREADS, 0, st>>>(h->n_angles, h->angle_row_offset, row_price, angle_mask,
+                                               angle_price, best_angle);
+    VMAT_LAUNCH_CHECK();
+    return VMAT_OK;
+}

@@ -1,0 +1,172 @@
+"""GPU parity on edge-case matrices and on the larger BASELINE.json configs."""
+import time
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from conftest import as_np
+from helpers import (assert_vec_close, check_selection_protocol, ddc_from_arrays, obj_to_device, oracle_eval,
+                     REL_L2)
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+@pytest.fixture(scope="module")
+def vm():
+    import paper_1503_01721_b200 as vm
+    vm.load_library()
+    return vm
+
+
+def _random_problem(rng, n_v, n_b, rows_spec, row_lens, n_struct=4):
+    """Random sparse D with prescribed per-voxel row lengths; leaf rows from `rows_spec` (list of lengths
+    per angle)."""
+    vox, beam = [], []
+    for i, ln in enumerate(row_lens):
+        if ln > 0:
+            vox.append(np.full(ln, i, np.int32))
+            beam.append(np.sort(rng.choice(n_b, ln, replace=False)).astype(np.int32))
+    vox = np.concatenate(vox) if vox else np.zeros(0, np.int32)
+    beam = np.concatenate(beam) if beam else np.zeros(0, np.int32)
+    val = (rng.random(vox.size) + 0.01).astype(np.float32)
+    perm = rng.permutation(vox.size)
+    lens = np.concatenate(rows_spec) if rows_spec else np.zeros(0, np.int64)
+    assert lens.sum() == n_b
+    lco = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+    aro = np.concatenate([[0], np.cumsum([len(r) for r in rows_spec])]).astype(np.int32)
+    aco = lco[aro]
+    return dict(vox=vox[perm], beam=beam[perm], val=val[perm], n_v=n_v, n_b=n_b,
+                sid=rng.integers(0, n_struct, n_v).astype(np.uint8),
+                T=np.array([5.0, 20.0, 8.0, 12.0], np.float32)[:n_struct],
+                wo=np.array([0.05, 1.0, 0.2, 0.7], np.float32)[:n_struct],
+                wu=np.array([0.0, 1.0, 0.0, 0.3], np.float32)[:n_struct], lco=lco, aro=aro, aco=aco)
+
+
+def _run_and_check(vm, A, x, mask=None, expect_no_diff=True):
+    h = ddc_from_arrays(A, DEV)
+    out = h.alloc_outputs()
+    m = None if mask is None else torch.from_numpy(mask).to(DEV)
+    vm.vmat_price_eval(h, torch.from_numpy(x).to(DEV), obj_to_device(A, DEV), out, m)
+    torch.cuda.synchronize()
+    ev = oracle_eval(A, x, mask)
+    assert_vec_close("d", out.d.cpu().numpy(), ev.d)
+    assert_vec_close("g", out.g.cpu().numpy(), ev.g)
+    assert_vec_close("p", out.p.cpu().numpy(), ev.p)
+    assert abs(out.F.item() - ev.F) <= REL_L2 * abs(ev.F) + 1e-300
+    n_diff = check_selection_protocol(A, out, ev, mask)
+    if expect_no_diff:
+        assert n_diff == 0
+    # the unfused calls give the same bits as the fused ones for d and p
+    d2 = torch.empty_like(out.d); p2 = torch.empty_like(out.p)
+    vm.vmat_dose(h, torch.from_numpy(x).to(DEV), d2)
+    vm.vmat_price(h, out.g, p2)
+    assert torch.equal(d2, out.d) and torch.equal(p2, out.p)
+    info = h.info
+    h.close()
+    return out, ev, info
+
+
+def test_empty_matrix(vm):
+    """nnz = 0 is legal: d = 0, g = -2 w- T on under-dose structures, p = 0, everything closed."""
+    rng = np.random.default_rng(0)
+    A = _random_problem(rng, 50, 12, [np.array([4, 0, 2]), np.array([6])], np.zeros(50, int))
+    out, ev, _ = _run_and_check(vm, A, np.ones(12, np.float32))
+    assert (out.d == 0).all() and (out.p == 0).all() and (out.L == 0).all() and (out.R == 0).all()
+    assert int(out.best_angle.item()) == -1
+
+
+def test_ragged_rows_spanning_every_kernel_path(vm):
+    """Voxel rows of 0, 1, 7, 8, 9 ... entries, rows longer than one dose block (4096), one longer than the
+    shared-memory sort (24576); leaf rows of length 0, 1 and 2100 (> the fused kernel's 2048 limit)."""
+    rng = np.random.default_rng(1)
+    n_v, n_b = 3000, 30000
+    lens = rng.integers(0, 40, n_v)
+    lens[rng.random(n_v) < 0.3] = 0
+    lens[[5, 6, 7, 8]] = [1, 7, 8, 9]
+    lens[100] = 4096; lens[101] = 4097; lens[102] = 5000; lens[1500] = 26000; lens[2999] = 12345
+    rows = [np.array([2100, 0, 1, 899]), np.array([0, 0]), np.array([5000, 3000, 1, 1, 1, 997]),
+            np.array([18000]), np.array([], int)]
+    A = _random_problem(rng, n_v, n_b, rows, lens)
+    x = (rng.random(n_b) * 0.02).astype(np.float32)
+    out, ev, info = _run_and_check(vm, A, x)
+    assert info["max_voxel_row_nnz"] == 26000 and info["max_leaf_row_len"] == 18000
+    assert (ev.g > 0).any() and (ev.g < 0).any() and (ev.R > ev.L).any()
+
+
+def test_short_leaf_rows_fused_path_and_masks(vm):
+    rng = np.random.default_rng(2)
+    n_v, n_b = 20000, 4000
+    lens = rng.integers(0, 300, n_v)
+    rows = [rng.multinomial(500, np.ones(10) / 10) for _ in range(8)]
+    A = _random_problem(rng, n_v, n_b, rows, lens)
+    x = (rng.random(n_b) * 0.30).astype(np.float32)       # near balance: mixed-sign prices
+    mask = np.zeros(8, np.uint8); mask[[1, 6]] = 1
+    out, ev, info = _run_and_check(vm, A, x, mask)
+    assert info["max_leaf_row_len"] <= 2048
+    assert (ev.g > 0).any() and (ev.g < 0).any() and (ev.R > ev.L).any() and (ev.p_f32 > 0).any()
+
+
+def test_exact_ties_in_prices(vm):
+    """Integer-valued data: prices are exact small integers, so equal-sum openings tie exactly (C5)."""
+    rng = np.random.default_rng(3)
+    n_v, n_b = 400, 240
+    lens = rng.integers(0, 6, n_v)
+    rows = [np.array([8] * 10) for _ in range(3)]
+    A = _random_problem(rng, n_v, n_b, rows, lens, n_struct=2)
+    A["val"] = rng.integers(1, 3, A["val"].size).astype(np.float32)
+    A["T"] = np.array([3.0, 2.0], np.float32); A["wo"] = np.array([0.5, 1.0], np.float32)
+    A["wu"] = np.array([0.0, 1.0], np.float32)
+    x = rng.integers(0, 2, n_b).astype(np.float32)
+    out, ev, _ = _run_and_check(vm, A, x)
+    assert np.array_equal(out.p.cpu().numpy().astype(np.float64), ev.p)          # exact integers on both sides
+    assert np.array_equal(out.L.cpu().numpy(), ev.L) and np.array_equal(out.R.cpu().numpy(), ev.R)
+
+
+# ------------------------------------------------------------------ the configs
+def _phantom_on_gpu(cfg, scale=1.0, angles=None):
+    spec = synth.config_spec(cfg, scale)
+    t = time.time()
+    ph = synth.generate(spec, device=DEV, angles=angles)
+    torch.cuda.synchronize()
+    print(f"\n[{spec.name}] generated on GPU in {time.time() - t:.1f}s: {ph.stats()}")
+    return ph
+
+
+def _full_parity(vm, ph, scales):
+    import paper_1503_01721_b200 as vmod
+    A = as_np(ph)
+    h = vmod.vmat_ddc_create(ph.n_voxels, ph.n_beamlets, ph.coo_voxel, ph.coo_beamlet, ph.coo_val,
+                             ph.angle_col_offset, ph.angle_row_offset, ph.leafrow_col_offset, device=DEV)
+    obj = obj_to_device(A, DEV)
+    out = h.alloc_outputs()
+    for k, sc in enumerate(scales):
+        x = synth.draw_x(ph.n_beamlets, 100 + k, scale=sc)
+        vmod.vmat_price_eval(h, x.to(DEV), obj, out)
+        torch.cuda.synchronize()
+        ev = oracle_eval(A, x.numpy())
+        assert_vec_close("d", out.d.cpu().numpy(), ev.d)
+        assert_vec_close("g", out.g.cpu().numpy(), ev.g)
+        assert_vec_close("p", out.p.cpu().numpy(), ev.p)
+        assert abs(out.F.item() - ev.F) <= REL_L2 * abs(ev.F)
+        n_diff = check_selection_protocol(A, out, ev)
+        print(f"  x*{sc}: F={ev.F:.6e} open rows={(ev.R > ev.L).sum()} best={ev.best_angle} "
+              f"rows differing from the pure-FP64 path={n_diff}")
+        assert n_diff <= max(1, A["lco"].size // 1000)
+    h.close()
+
+
+def test_config1_scaled_down(vm):
+    """Config 1 at 2.5x coarser voxels/beamlets (~1e6 nnz): several dose blocks, ragged leaf rows."""
+    _full_parity(vm, _phantom_on_gpu(1, scale=2.5), [1.0, 0.7])
+
+
+def test_config1_full(vm):
+    _full_parity(vm, _phantom_on_gpu(1), [1.0, 0.6])
+
+
+def test_config2_full(vm):
+    _full_parity(vm, _phantom_on_gpu(2), [1.0])

@@ -1,0 +1,225 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's: rel L2 <= 1e-5 and |delta| <= 1e-4 max|ref|
+for FP32 vectors and F; leaf positions bit-exact under the protocol of DESIGN.md reading C6."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from conftest import as_np
+from helpers import (assert_vec_close, check_selection_protocol, ddc_from_arrays, obj_to_device, oracle_eval,
+                     REL_L2)
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+@pytest.fixture(scope="module")
+def vm():
+    import paper_1503_01721_b200 as vm
+    vm.load_library()
+    return vm
+
+
+@pytest.fixture(scope="module")
+def A0(cfg0):
+    return as_np(cfg0)
+
+
+@pytest.fixture(scope="module")
+def h0(vm, A0):
+    h = ddc_from_arrays(A0, DEV)
+    yield h
+    h.close()
+
+
+def _x(n_b, k, scale=1.0):
+    return synth.draw_x(n_b, k, scale=scale)
+
+
+def _eval_gpu(vm, h, A, x, mask=None):
+    obj = obj_to_device(A, DEV)
+    out = h.alloc_outputs()
+    m = None if mask is None else torch.from_numpy(np.asarray(mask, np.uint8)).to(DEV)
+    vm.vmat_price_eval(h, x.to(DEV), obj, out, m)
+    torch.cuda.synchronize()
+    return out
+
+
+def _check_eval(A, out, ev, mask=None):
+    assert_vec_close("d", out.d.cpu().numpy(), ev.d)
+    assert_vec_close("g", out.g.cpu().numpy(), ev.g)
+    assert_vec_close("p", out.p.cpu().numpy(), ev.p)
+    assert abs(out.F.item() - ev.F) <= REL_L2 * abs(ev.F) + 1e-300
+    return check_selection_protocol(A, out, ev, mask)
+
+
+# ------------------------------------------------------------------ A0 ingest / layout
+def test_layouts_round_trip_config0(vm, A0, h0):
+    """Both layouts expand back to exactly the input triplets; rows are in canonical order (P7, P9)."""
+    key_in = np.sort(A0["vox"].astype(np.int64) * A0["n_b"] + A0["beam"])
+    order = np.lexsort((A0["beam"], A0["vox"]))
+    for which, rows in ((0, A0["n_v"]), (1, A0["n_b"])):
+        ptr, idx, val = [t.numpy() for t in h0.export_csr(which)]
+        assert ptr[0] == 0 and ptr[-1] == A0["vox"].size and (np.diff(ptr) >= 0).all()
+        row = np.repeat(np.arange(rows), np.diff(ptr))
+        v, b = (row, idx) if which == 0 else (idx, row)
+        assert np.array_equal(np.sort(v.astype(np.int64) * A0["n_b"] + b), key_in)
+        inner = np.diff(idx.astype(np.int64))
+        same_row = np.diff(row) == 0
+        assert (inner[same_row] > 0).all()                       # strictly ascending secondary index
+        if which == 0:
+            assert np.array_equal(val, A0["val"][order])
+    info = h0.info
+    assert info["bytes_csr_d"] == 8 * info["nnz"] + 8 * (info["n_voxels"] + 1)       # 8 B/nnz
+    assert info["bytes_csr_dt"] == 8 * info["nnz"] + 8 * (info["n_beamlets"] + 1)
+
+
+def test_ingest_host_and_device_coo_and_shuffle_give_identical_layouts(vm, A0, h0):
+    perm = np.random.default_rng(3).permutation(A0["vox"].size)
+    B = dict(A0, vox=A0["vox"][perm], beam=A0["beam"][perm], val=A0["val"][perm])
+    ref = [t.numpy() for w in (0, 1) for t in h0.export_csr(w)]
+    for on_dev in (True, False):
+        h = ddc_from_arrays(B, DEV, coo_on_device=on_dev)
+        got = [t.numpy() for w in (0, 1) for t in h.export_csr(w)]
+        for a, b in zip(ref, got):
+            assert np.array_equal(a, b)
+        h.close()
+
+
+def test_ingest_rejects_bad_input(vm, A0):
+    def create(vox, beam, val, n_v=A0["n_v"], n_b=A0["n_b"]):
+        return ddc_from_arrays(dict(A0, vox=vox, beam=beam, val=val, n_v=n_v, n_b=n_b), DEV)
+    vox, beam, val = A0["vox"].copy(), A0["beam"].copy(), A0["val"].copy()
+    bad = vox.copy(); bad[17] = A0["n_v"]
+    with pytest.raises(vm.VmatError) as e:
+        create(bad, beam, val)
+    assert e.value.status == -2
+    bad = beam.copy(); bad[5] = -1
+    with pytest.raises(vm.VmatError) as e:
+        create(vox, bad, val)
+    assert e.value.status == -2
+    badv = val.copy(); badv[100] = np.nan
+    with pytest.raises(vm.VmatError) as e:
+        create(vox, beam, badv)
+    assert e.value.status == -6
+    with pytest.raises(vm.VmatError) as e:                       # duplicate (voxel, beamlet) pair (C14)
+        create(np.append(vox, vox[7]), np.append(beam, beam[7]), np.append(val, val[7]))
+    assert e.value.status == -3
+    lco = A0["lco"].copy(); lco[3] = lco[2] - 1
+    with pytest.raises(vm.VmatError) as e:
+        ddc_from_arrays(dict(A0, lco=lco), DEV)
+    assert e.value.status == -1
+
+
+# ------------------------------------------------------------------ per-call parity, config 0
+@pytest.mark.parametrize("scale", [1.0, 8.0, 14.0, 16.0, 20.0])
+def test_each_call_alone_config0(vm, A0, h0, scale):
+    """Every C-ABI call on its own, fed the oracle's (FP32-rounded) input of that step."""
+    x = _x(A0["n_b"], 21, scale)
+    ev = oracle_eval(A0, x.numpy())
+    obj = obj_to_device(A0, DEV)
+    out = h0.alloc_outputs()
+    # A1
+    vm.vmat_dose(h0, x.to(DEV), out.d)
+    assert_vec_close("d", out.d.cpu().numpy(), ev.d)
+    # A2 on the oracle's d rounded to FP32
+    d32 = ev.d.astype(np.float32)
+    F_ref, g_ref = oracle.objective_grad(d32.astype(np.float64), A0["sid"], A0["T"], A0["wo"], A0["wu"])
+    vm.vmat_objective_grad(h0, torch.from_numpy(d32).to(DEV), obj, out.g, out.F)
+    assert_vec_close("g", out.g.cpu().numpy(), g_ref)
+    assert abs(out.F.item() - F_ref) <= REL_L2 * abs(F_ref)
+    # A3 on the oracle's g rounded to FP32
+    g32 = ev.g.astype(np.float32)
+    p_ref = oracle.price(A0["vox"], A0["beam"], A0["val"], A0["n_b"], g32.astype(np.float64))
+    vm.vmat_price(h0, torch.from_numpy(g32).to(DEV), out.p)
+    assert_vec_close("p", out.p.cpu().numpy(), p_ref)
+    # A4 + A5 on the oracle's p rounded to FP32: bit-exact (C6 (i))
+    vm.vmat_select_apertures(h0, torch.from_numpy(ev.p_f32).to(DEV), None, out.L, out.R, out.row_price,
+                             out.angle_price, out.best_angle)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.L.cpu().numpy(), ev.L) and np.array_equal(out.R.cpu().numpy(), ev.R)
+    assert np.array_equal(out.row_price.cpu().numpy(), ev.row_price)
+    assert np.array_equal(out.angle_price.cpu().numpy(), ev.angle_price)
+    assert int(out.best_angle.item()) == ev.best_angle
+
+
+@pytest.mark.parametrize("scale", [0.0, 1.0, 8.0, 14.0, 16.0, 20.0])
+def test_price_eval_fused_config0(vm, A0, h0, scale):
+    x = _x(A0["n_b"], 22, scale)
+    ev = oracle_eval(A0, x.numpy())
+    out = _eval_gpu(vm, h0, A0, x)
+    n_diff = _check_eval(A0, out, ev)
+    assert n_diff == 0
+    if scale == 0.0:                                   # the paper's first iteration (L56): closed form
+        assert (out.d == 0).all() and int(out.best_angle.item()) == ev.best_angle >= 0
+
+
+def test_angle_mask(vm, A0, h0):
+    x = _x(A0["n_b"], 23, 14.0)
+    mask = np.zeros(A0["aro"].size - 1, np.uint8)
+    ev0 = oracle_eval(A0, x.numpy())
+    mask[ev0.best_angle] = 1                              # occupy the best control point (C7)
+    mask[0] = 1
+    ev = oracle_eval(A0, x.numpy(), mask)
+    out = _eval_gpu(vm, h0, A0, x, mask)
+    _check_eval(A0, out, ev, mask)
+    assert int(out.best_angle.item()) == ev.best_angle != ev0.best_angle
+    assert torch.isinf(out.angle_price[0]) and out.angle_price[0] > 0
+    # unfused call, same mask
+    o2 = h0.alloc_outputs()
+    vm.vmat_select_apertures(h0, out.p, torch.from_numpy(mask).to(DEV), o2.L, o2.R, o2.row_price, o2.angle_price,
+                             o2.best_angle)
+    for a, b in ((o2.L, out.L), (o2.R, out.R), (o2.row_price, out.row_price), (o2.angle_price, out.angle_price),
+                 (o2.best_angle, out.best_angle)):
+        assert torch.equal(a, b)
+
+
+def test_determinism_and_shuffle_invariance(vm, A0, h0):
+    """Two runs are bit-identical, and so is a handle built from shuffled triplets (P9)."""
+    x = _x(A0["n_b"], 24, 14.0)
+    o1 = _eval_gpu(vm, h0, A0, x)
+    o2 = _eval_gpu(vm, h0, A0, x)
+    perm = np.random.default_rng(5).permutation(A0["vox"].size)
+    hB = ddc_from_arrays(dict(A0, vox=A0["vox"][perm], beam=A0["beam"][perm], val=A0["val"][perm]), DEV)
+    o3 = _eval_gpu(vm, hB, A0, x)
+    hB.close()
+    for f in ("d", "g", "F", "p", "L", "R", "row_price", "angle_price", "best_angle"):
+        assert torch.equal(getattr(o1, f), getattr(o2, f)), f
+        assert torch.equal(getattr(o1, f), getattr(o3, f)), f
+
+
+def test_host_buffer_call_matches_device_call(vm, A0, h0):
+    x = _x(A0["n_b"], 25, 14.0)
+    out = _eval_gpu(vm, h0, A0, x)
+    obj = obj_to_device(A0, DEV)
+    xh = x.pin_memory()
+    F = torch.empty(1, dtype=torch.float64).pin_memory()
+    L = torch.empty(h0.n_leaf_rows, dtype=torch.int32).pin_memory()
+    R = torch.empty(h0.n_leaf_rows, dtype=torch.int32).pin_memory()
+    rp = torch.empty(h0.n_leaf_rows, dtype=torch.float64).pin_memory()
+    ap = torch.empty(h0.n_angles, dtype=torch.float64).pin_memory()
+    best = torch.empty(1, dtype=torch.int32).pin_memory()
+    vm.vmat_price_eval_host(h0, xh, obj, F, L, R, rp, ap, best)
+    assert F.item() == out.F.item() and best.item() == out.best_angle.item()
+    assert torch.equal(L, out.L.cpu()) and torch.equal(R, out.R.cpu())
+    assert torch.equal(rp, out.row_price.cpu()) and torch.equal(ap, out.angle_price.cpu())
+
+
+def test_aperture_dose(vm, A0, h0):
+    """NEXT-1, Eq. (5): DA = sum of the columns of the beamlets inside the chosen aperture."""
+    x = _x(A0["n_b"], 26, 14.0)
+    out = _eval_gpu(vm, h0, A0, x)
+    a = int(out.best_angle.item())
+    assert a >= 0
+    DA = torch.empty(h0.n_voxels, dtype=torch.float32, device=DEV)
+    xs = torch.empty(h0.n_beamlets, dtype=torch.float32, device=DEV)
+    vm.vmat_aperture_dose(h0, a, out.L, out.R, xs, DA)
+    ind = np.zeros(A0["n_b"], np.float32)
+    L, R = out.L.cpu().numpy(), out.R.cpu().numpy()
+    for r in range(A0["aro"][a], A0["aro"][a + 1]):
+        ind[A0["lco"][r] + L[r]:A0["lco"][r] + R[r]] = 1.0
+    assert ind.sum() > 0
+    assert np.array_equal(xs.cpu().numpy(), ind)
+    assert_vec_close("DA", DA.cpu().numpy(), oracle.dose(A0["vox"], A0["beam"], A0["val"], A0["n_v"], ind))
