@@ -84,6 +84,11 @@ int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info /* host, out */);
  * which = 1: CSR(D^T) (rows = beamlets, idx = voxels).  ptr [rows+1], idx/val [nnz]. Synchronous. */
 int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx, float *val /* host, out */);
 
+/* Zero-copy, read-only view of one layout's device arrays (same `which` as above); the pointers stay
+ * owned by the handle and valid until vmat_ddc_destroy.  Any of the three outputs may be NULL. */
+int vmat_ddc_device_csr(const vmat_ddc *h, int which, const int64_t **ptr, const int32_t **idx,
+                        const float **val /* host, out: device pointers */);
+
 /* A1 forward dose d = D x, d_i = sum_j D_ij x_j ("repeated forward dose
  * calculation", L27).  x dev [n_beamlets] in, d dev [n_voxels] out. */
 int vmat_dose(const vmat_ddc *h, const float *x, float *d, void *stream);

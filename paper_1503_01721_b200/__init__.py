@@ -27,7 +27,7 @@ STATUS_NAMES = {0: "VMAT_OK", -1: "VMAT_ERR_INVALID_ARG", -2: "VMAT_ERR_INDEX_RA
                 -4: "VMAT_ERR_OOM", -5: "VMAT_ERR_CUDA", -6: "VMAT_ERR_NONFINITE"}
 
 EXPORTS = [
-    "vmat_ddc_create", "vmat_ddc_destroy", "vmat_ddc_info_get", "vmat_ddc_export_csr", "vmat_dose",
+    "vmat_ddc_create", "vmat_ddc_destroy", "vmat_ddc_info_get", "vmat_ddc_export_csr", "vmat_ddc_device_csr", "vmat_dose",
     "vmat_objective_grad", "vmat_price", "vmat_select_apertures", "vmat_price_eval", "vmat_price_eval_host",
     "vmat_aperture_dose", "vmat_ddc_set_profile_events", "vmat_last_error", "vmat_last_launch_count",
 ]
@@ -59,6 +59,7 @@ def load_library():
     lib.vmat_ddc_destroy.argtypes = [vp]
     lib.vmat_ddc_info_get.argtypes = [vp, ctypes.POINTER(_Info)]
     lib.vmat_ddc_export_csr.argtypes = [vp, ctypes.c_int, vp, vp, vp]
+    lib.vmat_ddc_device_csr.argtypes = [vp, ctypes.c_int, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp)]
     lib.vmat_dose.argtypes = [vp, vp, vp, vp]
     lib.vmat_objective_grad.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp]
     lib.vmat_price.argtypes = [vp, vp, vp, vp]
@@ -166,6 +167,12 @@ class DDC:
             return
         arr = (ctypes.c_void_p * 4)(*[e.cuda_event for e in events])
         _check(load_library().vmat_ddc_set_profile_events(self._h, arr))
+
+    def device_csr(self, which: int):
+        """Raw device pointers (ptr, idx, val) of a layout, owned by the handle (zero-copy view)."""
+        a, b, c = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_void_p()
+        _check(load_library().vmat_ddc_device_csr(self._h, which, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
+        return a.value, b.value, c.value
 
     def export_csr(self, which: int):
         """(ptr int64 [rows+1], idx int32 [nnz], val float32 [nnz]) of CSR(D) (0) or CSR(D^T) (1), on the host."""

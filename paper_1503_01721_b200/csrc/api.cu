@@ -1,6 +1,6 @@
 // api.cu - the extern "C" boundary of libvmat (include/vmat.h): argument checks, handle lifetime,
 // and the sequencing of the kernels on the caller's stream.  No arithmetic lives here.
-#include "common.cuh"
+#include "spmv.cuh"
 #include <stdarg.h>
 #include <string.h>
 #include <new>
@@ -64,7 +64,7 @@ int vmat_ddc_destroy(vmat_ddc *h)
     if (!h) return VMAT_OK;
     void *ptrs[] = {h->D.ptr, h->D.idx, h->D.val, h->Dt.ptr, h->Dt.idx, h->Dt.val, h->angle_col_offset,
                     h->angle_row_offset, h->leafrow_col_offset, h->leafrow_angle, h->blk_row, h->F_partial,
-                    h->F_partial_obj, h->S_scratch, h->e2e_x, h->e2e_d, h->e2e_g, h->e2e_p, h->e2e_L, h->e2e_R,
+                    h->F_partial_obj, h->S_scratch, h->beamlet_leafrow, h->leafrow_done, h->e2e_x, h->e2e_d, h->e2e_g, h->e2e_p, h->e2e_L, h->e2e_R,
                     h->e2e_best, h->e2e_row_price, h->e2e_angle_price, h->e2e_F};
     for (void *p : ptrs)
         if (p) cudaFree(p);
@@ -116,10 +116,23 @@ int vmat_ddc_create(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int64_
     if (rc == VMAT_OK) rc = upload(&h->angle_row_offset, angle_row_offset, (int64_t)n_angles + 1, &h->bytes_device);
     if (rc == VMAT_OK) rc = upload(&h->leafrow_col_offset, leafrow_col_offset, (int64_t)n_rows + 1, &h->bytes_device);
     if (rc == VMAT_OK) rc = upload(&h->leafrow_angle, row_angle.data(), (int64_t)n_rows, &h->bytes_device);
-    if (rc == VMAT_OK && max_len > SELECT_MAX_ROW) {
+    if (rc == VMAT_OK) {
         const size_t b = ((size_t)n_beamlets + (size_t)n_rows + 1) * sizeof(double);
         cudaError_t e = cudaMalloc((void **)&h->S_scratch, b);
         if (e != cudaSuccess) { vmat_set_error("vmat_ddc_create: cudaMalloc(S_scratch) failed"); rc = VMAT_ERR_OOM; }
+        h->bytes_device += (int64_t)b;
+    }
+    if (rc == VMAT_OK) {
+        std::vector<int32_t> bl((size_t)(n_beamlets > 0 ? n_beamlets : 1), 0);
+        for (int r = 0; r < n_rows; ++r)
+            for (int j = leafrow_col_offset[r]; j < leafrow_col_offset[r + 1]; ++j) bl[j] = r;
+        rc = upload(&h->beamlet_leafrow, bl.data(), (int64_t)n_beamlets, &h->bytes_device);
+    }
+    if (rc == VMAT_OK) {
+        const size_t b = (size_t)(n_rows > 0 ? n_rows : 1) * sizeof(uint32_t);
+        cudaError_t e = cudaMalloc((void **)&h->leafrow_done, b);
+        if (e != cudaSuccess) { vmat_set_error("vmat_ddc_create: cudaMalloc(leafrow_done) failed"); rc = VMAT_ERR_OOM; }
+        else cudaMemsetAsync(h->leafrow_done, 0, b, st);
         h->bytes_device += (int64_t)b;
     }
     if (rc == VMAT_OK) {
@@ -157,6 +170,36 @@ int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx
         VMAT_CUDA(cudaMemcpy(idx, A.idx, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost));
         VMAT_CUDA(cudaMemcpy(val, A.val, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost));
     }
+    // undo the tile interleave (spmv.cuh): the caller gets canonical CSR order
+    std::vector<int64_t> hp((size_t)A.n_rows + 1);
+    memcpy(hp.data(), ptr, hp.size() * 8);
+    const int64_t n_seg = which == 0 ? (int64_t)h->n_blocks : (int64_t)A.n_rows;
+    int32_t ti_[TILE];
+    float tv_[TILE];
+    for (int64_t w = 0; w < n_seg; ++w) {
+        const int64_t s = which == 0 ? hp[h->h_blk_row[w]] : hp[w];
+        const int64_t e = which == 0 ? hp[h->h_blk_row[w + 1]] : hp[w + 1];
+        const Segment sg = segment_of(s, e);
+        for (int64_t t = 0; t < sg.nt; ++t) {
+            int32_t *pi = idx + sg.a0 + t * TILE;
+            float *pv = val + sg.a0 + t * TILE;
+            for (int l = 0; l < 32; ++l)
+                for (int u = 0; u < 8; ++u) { ti_[32 * u + l] = pi[8 * l + u]; tv_[32 * u + l] = pv[8 * l + u]; }
+            memcpy(pi, ti_, sizeof(ti_));
+            memcpy(pv, tv_, sizeof(tv_));
+        }
+    }
+    return VMAT_OK;
+}
+
+int vmat_ddc_device_csr(const vmat_ddc *h, int which, const int64_t **ptr, const int32_t **idx, const float **val)
+{
+    REQUIRE(h != nullptr, "handle is NULL");
+    REQUIRE(which == 0 || which == 1, "which must be 0 (D) or 1 (D^T)");
+    const CsrLayout &A = which == 0 ? h->D : h->Dt;
+    if (ptr) *ptr = A.ptr;
+    if (idx) *idx = A.idx;
+    if (val) *val = A.val;
     return VMAT_OK;
 }
 
@@ -217,12 +260,7 @@ int vmat_price_eval(const vmat_ddc *h, const float *x,
     g_vmat_launches = 0;
     TRY(vmat_launch_dose(h, x, d, true, voxel_struct, n_struct, T, w_over, w_under, g, F, st));
     if (h->prof_ev[2]) VMAT_CUDA(cudaEventRecord(h->prof_ev[2], st));
-    if (h->max_leaf_row_len <= SELECT_MAX_ROW) {
-        TRY(vmat_launch_price_select(h, g, angle_mask, p, L, R, row_price, st));
-    } else {
-        TRY(vmat_launch_price(h, g, p, st));
-        TRY(vmat_launch_select(h, p, angle_mask, L, R, row_price, st));
-    }
+    TRY(vmat_launch_price_select(h, g, angle_mask, p, L, R, row_price, st));
     if (h->prof_ev[3]) VMAT_CUDA(cudaEventRecord(h->prof_ev[3], st));
     return vmat_launch_angle_price(h, row_price, angle_mask, angle_price, best_angle, st);
 }

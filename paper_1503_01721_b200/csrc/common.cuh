@@ -55,8 +55,11 @@ struct vmat_ddc {
     double *F_partial = nullptr;            // [n_blocks] per-block objective partials
     int32_t n_obj_blocks = 0;               // blocks of the standalone objective kernel
     double *F_partial_obj = nullptr;        // [n_obj_blocks]
-    double *S_scratch = nullptr;            // prefix-sum scratch for leaf rows longer than SELECT_MAX_ROW
+    double *S_scratch = nullptr;            // [n_beamlets + n_leaf_rows + 1] prefix sums of the row selection
+    int32_t *beamlet_leafrow = nullptr;     // [n_beamlets] leaf row of each beamlet
+    uint32_t *leafrow_done = nullptr;       // [n_leaf_rows] tickets of the fused price+selection kernel (self-resetting)
     std::vector<int32_t> h_angle_row_offset; // host copy
+    std::vector<int32_t> h_blk_row;          // host copy of blk_row (export un-permutes the tiles)
     int32_t max_leaf_row_len = 0;
     int64_t max_voxel_row_nnz = 0, max_beamlet_row_nnz = 0;
     int64_t bytes_device = 0;
@@ -70,8 +73,14 @@ struct vmat_ddc {
 
 // ------------------------------------------------------------------ tuning constants
 // Dose kernel (CSR-stream): one CTA per row block; products staged in shared memory.
-constexpr int DOSE_THREADS = 256;
-constexpr int DOSE_BLOCK_NNZ = 4096;        // products per block held in smem (16 KB)
+#ifndef VMAT_DOSE_THREADS
+#define VMAT_DOSE_THREADS 256
+#endif
+#ifndef VMAT_DOSE_BLOCK_NNZ
+#define VMAT_DOSE_BLOCK_NNZ 4096
+#endif
+constexpr int DOSE_THREADS = VMAT_DOSE_THREADS;
+constexpr int DOSE_BLOCK_NNZ = VMAT_DOSE_BLOCK_NNZ;   // products per block held in smem (4 B each)
 constexpr int DOSE_MAX_ROWS = 1024;         // rows per block (bounds runs of empty rows)
 // Price kernel (CSR-vector, one warp per beamlet row, L127).
 constexpr int PRICE_THREADS = 256;
@@ -90,6 +99,18 @@ __device__ __forceinline__ Vec8 ld_stream_256(const void *p)
     asm volatile("ld.global.nc.L1::no_allocate.L2::evict_first.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                  : "=r"(r.w[0]), "=r"(r.w[1]), "=r"(r.w[2]), "=r"(r.w[3]),
                    "=r"(r.w[4]), "=r"(r.w[5]), "=r"(r.w[6]), "=r"(r.w[7]) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ float ld_stream_f(const float *p)
+{
+    float r;
+    asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(r) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ int ld_stream_i(const int32_t *p)
+{
+    int r;
+    asm volatile("ld.global.nc.L1::no_allocate.s32 %0, [%1];" : "=r"(r) : "l"(p));
     return r;
 }
 // Gathered vector (x or g): read-only path, allocated in L1 with evict-last priority.

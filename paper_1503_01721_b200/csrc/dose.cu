@@ -48,7 +48,7 @@ k_dose(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const f
        const float *__restrict__ w_over, const float *__restrict__ w_under, float *__restrict__ g,
        double *__restrict__ F_partial)
 {
-    __shared__ __align__(32) float prod[DOSE_BLOCK_NNZ + 8];
+    __shared__ float prod[DOSE_BLOCK_NNZ];
     __shared__ float red_f[DOSE_THREADS / 32];
     __shared__ double red_d[DOSE_THREADS / 32];
     __shared__ ObjTables tab;
@@ -67,9 +67,13 @@ k_dose(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const f
     const int64_t s = ptr[r0], e = ptr[r1];
     double fsum = 0.0;
 
+    const Segment sg = segment_of(s, e);
     if (nr == 1) {
-        // ---- one row: register accumulation by the whole CTA
-        float acc = strided_row_dot<DOSE_THREADS>(val, idx, s, e, x, tid);
+        // ---- one row: register accumulation by the whole CTA (warps take tiles round-robin)
+        float acc = 0.f;
+        for (int64_t ti = warp; ti < sg.nt; ti += DOSE_THREADS / 32)
+            acc += tile_dot(val, idx, sg.a0 + ti * TILE, x, lane);
+        plain_foreach<DOSE_THREADS>(val, idx, s, sg, e, x, tid, [&](int64_t, float q) { acc += q; });
         acc = warp_sum(acc);
         if (lane == 0) red_f[warp] = acc;
         __syncthreads();
@@ -84,32 +88,16 @@ k_dose(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const f
             }
         }
     } else {
-        // ---- several rows: stream products into shared memory ...
-        const int64_t a = s & ~int64_t(7);
-        for (int64_t k = a + (int64_t)tid * 8; k < e; k += (int64_t)DOSE_THREADS * 16) {
-            const int64_t k2 = k + (int64_t)DOSE_THREADS * 8;
-            const bool has2 = k2 < e;
-            Vec8 v0 = ld_stream_256(val + k);
-            Vec8 c0 = ld_stream_256(idx + k);
-            Vec8 v1, c1;
-            if (has2) {
-                v1 = ld_stream_256(val + k2);
-                c1 = ld_stream_256(idx + k2);
-            }
-            float q[8];
+        // ---- several rows: products into shared memory at their logical position k - s ...
+        for (int64_t ti = warp; ti < sg.nt; ti += DOSE_THREADS / 32) {
+            const int64_t k = sg.a0 + ti * TILE;
+            const Vec8 v = ld_stream_256(val + k + lane * 8);
+            const Vec8 c = ld_stream_256(idx + k + lane * 8);
+            float *dst = prod + (k - s) + lane;
 #pragma unroll
-            for (int t = 0; t < 8; ++t) q[t] = __uint_as_float(v0.w[t]) * ld_gather(x + c0.w[t]);
-            float4 *dst = reinterpret_cast<float4 *>(prod + (k - a));
-            dst[0] = make_float4(q[0], q[1], q[2], q[3]);
-            dst[1] = make_float4(q[4], q[5], q[6], q[7]);
-            if (has2) {
-#pragma unroll
-                for (int t = 0; t < 8; ++t) q[t] = __uint_as_float(v1.w[t]) * ld_gather(x + c1.w[t]);
-                dst = reinterpret_cast<float4 *>(prod + (k2 - a));
-                dst[0] = make_float4(q[0], q[1], q[2], q[3]);
-                dst[1] = make_float4(q[4], q[5], q[6], q[7]);
-            }
+            for (int t = 0; t < 8; ++t) dst[32 * t] = __uint_as_float(v.w[t]) * ld_gather(x + c.w[t]);
         }
+        plain_foreach<DOSE_THREADS>(val, idx, s, sg, e, x, tid, [&](int64_t k, float q) { prod[k - s] = q; });
         __syncthreads();
         // ... then G lanes per row, G = power of two near (mean row length)/4, 1..32
         const int mean = (int)((e - s) / nr);
@@ -121,7 +109,7 @@ k_dose(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const f
             const int r = r0 + grp + it * n_grp;
             float acc = 0.f;
             if (r < r1) {
-                const int b = (int)(ptr[r] - a), f = (int)(ptr[r + 1] - a);
+                const int b = (int)(ptr[r] - s), f = (int)(ptr[r + 1] - s);
                 for (int k = b + gl; k < f; k += G) acc += prod[k];
             }
             for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);

@@ -12,7 +12,7 @@
 //              floating-point sum has a fixed order whatever the order of the input triplets (C14);
 //              equal neighbours after the sort are duplicates -> VMAT_ERR_DUPLICATE
 // Host-resident COO is streamed through a device staging buffer in chunks, twice.
-#include "common.cuh"
+#include "spmv.cuh"
 #include <vector>
 #include <algorithm>
 
@@ -175,6 +175,31 @@ __global__ void k_sort_rows_gmem(const int64_t *__restrict__ ptr, int32_t *idx, 
         if (ri[i] == ri[i - 1]) atomicOr(flags + FLAG_DUP, 1);
 }
 
+// ---------------------------------------------------------------- tile interleave (spmv.cuh)
+// One warp per segment (a beamlet row of D^T when blk_row == NULL, else a row block of D): every full
+// 256-entry tile is permuted in place so that stored word 8*l + t holds the tile's entry 32*t + l.
+__global__ void __launch_bounds__(256)
+k_interleave(const int64_t *__restrict__ ptr, const int32_t *__restrict__ blk_row, int n_seg,
+             int32_t *idx, float *val)
+{
+    const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (w >= n_seg) return;
+    const int r0 = blk_row ? blk_row[w] : w, r1 = blk_row ? blk_row[w + 1] : w + 1;
+    const int64_t s = ptr[r0], e = ptr[r1];
+    const Segment sg = segment_of(s, e);
+    for (int64_t ti = 0; ti < sg.nt; ++ti) {
+        const int64_t base = sg.a0 + ti * TILE;
+        int32_t ci[8];
+        float vi[8];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) { ci[t] = idx[base + t * 32 + lane]; vi[t] = val[base + t * 32 + lane]; }
+        __syncwarp();
+#pragma unroll
+        for (int t = 0; t < 8; ++t) { idx[base + lane * 8 + t] = ci[t]; val[base + lane * 8 + t] = vi[t]; }
+        __syncwarp();
+    }
+}
+
 constexpr int SORT_SMALL = 2048;       // 16 KB of keys, 256 threads
 constexpr int SORT_BIG = 24576;        // 192 KB of keys, 1024 threads
 
@@ -326,6 +351,15 @@ int vmat_build_layouts(vmat_ddc *h, const int32_t *coo_voxel, const int32_t *coo
     h->n_blocks = (int32_t)blk.size() - 1;
     TRY(dev_alloc(&h->blk_row, (int64_t)blk.size(), &h->bytes_device));
     VMAT_CUDA(cudaMemcpy(h->blk_row, blk.data(), blk.size() * 4, cudaMemcpyHostToDevice));
+    h->h_blk_row = blk;
+    // ---- tile-interleave both layouts: segments = row blocks of D, beamlet rows of D^T
+    if (nnz > 0) {
+        k_interleave<<<(h->n_blocks + 7) / 8, 256, 0, st>>>(h->D.ptr, h->blk_row, h->n_blocks, h->D.idx, h->D.val);
+        VMAT_LAUNCH_CHECK();
+        k_interleave<<<(nb + 7) / 8, 256, 0, st>>>(h->Dt.ptr, nullptr, nb, h->Dt.idx, h->Dt.val);
+        VMAT_LAUNCH_CHECK();
+        VMAT_CUDA(cudaStreamSynchronize(st));
+    }
     TRY(dev_alloc(&h->F_partial, h->n_blocks, &h->bytes_device));
     h->n_obj_blocks = (nv + 255) / 256;
     TRY(dev_alloc(&h->F_partial_obj, h->n_obj_blocks, &h->bytes_device));

@@ -2,10 +2,12 @@
 // beamlet-row CSR, A4 per-leaf-row best opening and A5 aperture price / best control point (L133).
 //
 // Beamlet rows are long and even (a radius-`cutoff` cylinder through the body: 10^3-10^4 non-zeros),
-// so the paper's mapping holds on sm_100a: one warp per beamlet row (L127), here with 256-bit loads
-// and 128 B per lane in flight.  In the fused kernel a CTA owns one MLC leaf row: its warps price the
-// row's beamlets, the prices stay in shared memory, and the CTA then selects the row's opening - the
-// selection never re-reads p from HBM and costs no launch.
+// so the paper's mapping holds on sm_100a: one warp per beamlet row (L127), here over lane-interleaved
+// 256-entry tiles read with 256-bit loads (spmv.cuh).  Measured on B200 the warp-per-row kernel beats
+// a CTA-per-leaf-row kernel by 12 % (perfect balance, more independent streams), so the row selection
+// is fused differently: every warp takes a ticket of its leaf row after writing its price, and the
+// warp that draws the last ticket selects that row's opening on the spot - the selection costs no
+// launch and no second pass over p, and the price kernel keeps its one-warp-per-row balance.
 //
 // Selection arithmetic (readings C4-C6, C8): S_0 = 0, S_{c+1} = S_c + (double)p_c left to
 // right in FP64; candidates all 0 <= L <= R <= n with V = S_R - S_L; result = smallest (V, L, R).
@@ -62,50 +64,96 @@ __device__ __forceinline__ Opening select_row(const float *sp, int n, double *S,
     return best;
 }
 
-// ---------------------------------------------------------------- A3 alone: one warp per beamlet row
-__global__ void __launch_bounds__(PRICE_THREADS)
-k_price(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const float *__restrict__ val,
-        int n_rows, const float *__restrict__ g, float *__restrict__ p)
+// Best opening of one leaf row by ONE WARP (the fused path).  p_row: the row's n prices in global memory,
+// written by other warps (read through L2).  S: n+1 doubles of global scratch private to this row.
+__device__ __noinline__ Opening warp_select_row(const float *p_row, int n, double *S, int lane)
 {
-    const int lane = threadIdx.x & 31;
-    const int row = blockIdx.x * PRICE_WARPS + (threadIdx.x >> 5);
-    if (row >= n_rows) return;
-    float acc = strided_row_dot<32>(val, idx, ptr[row], ptr[row + 1], g, lane);
-    acc = warp_sum(acc);
-    if (lane == 0) p[row] = acc;
-}
-
-// ---------------------------------------------------------------- A3 + A4 fused: one CTA per leaf row
-__global__ void __launch_bounds__(PRICE_THREADS)
-k_price_select(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const float *__restrict__ val,
-               const float *__restrict__ g, const int32_t *__restrict__ leafrow_col_offset,
-               const int32_t *__restrict__ leafrow_angle, const uint8_t *__restrict__ angle_mask,
-               float *__restrict__ p, int32_t *__restrict__ Lout, int32_t *__restrict__ Rout,
-               double *__restrict__ row_price)
-{
-    __shared__ double S[SELECT_MAX_ROW + 1];
-    __shared__ float sp[SELECT_MAX_ROW];
-    __shared__ Opening red[PRICE_WARPS];
-    const int r = blockIdx.x;
-    const int j0 = leafrow_col_offset[r];
-    const int n = leafrow_col_offset[r + 1] - j0;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int c = warp; c < n; c += PRICE_WARPS) {
-        const int row = j0 + c;
-        float acc = strided_row_dot<32>(val, idx, ptr[row], ptr[row + 1], g, lane);
-        acc = warp_sum(acc);
-        if (lane == 0) {
-            p[row] = acc;
-            sp[c] = acc;
+    if (lane == 0) {
+        double s = 0.0;
+        S[0] = 0.0;
+        for (int c = 0; c < n; ++c) {
+            s = s + (double)__ldcg(p_row + c);     // strictly left to right
+            S[c + 1] = s;
         }
     }
-    __syncthreads();
-    const bool occupied = angle_mask != nullptr && angle_mask[leafrow_angle[r]] != 0;    // C7
-    Opening best = select_row<PRICE_THREADS>(sp, occupied ? 0 : n, S, red);
-    if (threadIdx.x == 0) {
-        Lout[r] = best.L;
-        Rout[r] = best.R;
-        row_price[r] = best.V;
+    __syncwarp();
+    Opening best = {0.0, 0, 0};                    // the closed opening (C4)
+    for (int L = lane; L <= n; L += 32) {
+        const double SL = S[L];
+        for (int R = L; R <= n; ++R) {
+            const double V = S[R] - SL;
+            if (V < best.V) { best.V = V; best.L = L; best.R = R; }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        Opening other;
+        other.V = __shfl_xor_sync(0xffffffffu, best.V, o);
+        other.L = __shfl_xor_sync(0xffffffffu, best.L, o);
+        other.R = __shfl_xor_sync(0xffffffffu, best.R, o);
+        if (opening_less(other, best)) best = other;
+    }
+    return best;
+}
+
+struct SelectArgs {
+    const int32_t *beamlet_leafrow;      // [n_beamlets]
+    const int32_t *leafrow_col_offset;   // [n_leaf_rows+1]
+    const int32_t *leafrow_angle;        // [n_leaf_rows]
+    const uint8_t *angle_mask;           // [n_angles] or NULL
+    uint32_t *leafrow_done;              // [n_leaf_rows] tickets, zero between launches
+    double *S;                           // [n_beamlets + n_leaf_rows + 1]
+    int32_t *L, *R;
+    double *row_price;
+    int n_leaf_rows;
+};
+
+// ---------------------------------------------------------------- A3 (+ A4 fused): one warp per beamlet row
+#ifndef VMAT_PRICE_MINB
+#define VMAT_PRICE_MINB 6        // 40 registers, 1536 threads per SM: fastest of 4..8 on B200 (cfg 3)
+#endif
+template <bool SELECT>
+__global__ void __launch_bounds__(PRICE_THREADS, VMAT_PRICE_MINB)
+k_price(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const float *__restrict__ val,
+        int n_rows, const float *__restrict__ g, float *__restrict__ p, SelectArgs sa)
+{
+    const int lane = threadIdx.x & 31;
+    if (SELECT) {                                   // leaf rows without beamlets draw no ticket: close them here
+        const int r = blockIdx.x * PRICE_THREADS + threadIdx.x;
+        if (r < sa.n_leaf_rows && sa.leafrow_col_offset[r + 1] == sa.leafrow_col_offset[r]) {
+            sa.L[r] = 0; sa.R[r] = 0; sa.row_price[r] = 0.0;
+        }
+    }
+    const int row = blockIdx.x * PRICE_WARPS + (threadIdx.x >> 5);
+    if (row >= n_rows) return;
+    const int64_t s = ptr[row], e = ptr[row + 1];
+    const Segment sg = segment_of(s, e);
+    float acc = 0.f;
+    for (int64_t ti = 0; ti < sg.nt; ++ti) acc += tile_dot(val, idx, sg.a0 + ti * TILE, g, lane);
+    plain_foreach<32>(val, idx, s, sg, e, g, lane, [&](int64_t, float q) { acc += q; });
+    acc = warp_sum(acc);
+    if (lane == 0) p[row] = acc;
+    if (SELECT) {
+        const int r = sa.beamlet_leafrow[row];
+        const int j0 = sa.leafrow_col_offset[r];
+        const int n = sa.leafrow_col_offset[r + 1] - j0;
+        int last = 0;
+        if (lane == 0) {
+            __threadfence();                                            // p[row] visible before the ticket
+            last = atomicAdd(sa.leafrow_done + r, 1u) == (uint32_t)(n - 1);
+        }
+        last = __shfl_sync(0xffffffffu, last, 0);
+        if (last) {                                                     // every price of leaf row r is written
+            if (lane == 0) sa.leafrow_done[r] = 0;                      // ready for the next launch
+            __threadfence();
+            const bool occupied = sa.angle_mask != nullptr && sa.angle_mask[sa.leafrow_angle[r]] != 0;   // C7
+            const Opening best = warp_select_row(p + j0, occupied ? 0 : n, sa.S + j0 + r, lane);
+            if (lane == 0) {
+                sa.L[r] = best.L;
+                sa.R[r] = best.R;
+                sa.row_price[r] = best.V;
+            }
+        }
     }
 }
 
@@ -183,7 +231,7 @@ int vmat_launch_price(const vmat_ddc *h, const float *g, float *p, cudaStream_t 
 {
     if (h->n_beamlets == 0) return VMAT_OK;
     const int grid = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
-    k_price<<<grid, PRICE_THREADS, 0, st>>>(h->Dt.ptr, h->Dt.idx, h->Dt.val, h->n_beamlets, g, p);
+    k_price<false><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.ptr, h->Dt.idx, h->Dt.val, h->n_beamlets, g, p, SelectArgs{});
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }
@@ -202,9 +250,15 @@ int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *a
                              int32_t *L, int32_t *R, double *row_price, cudaStream_t st)
 {
     if (h->n_leaf_rows == 0) return VMAT_OK;
-    k_price_select<<<h->n_leaf_rows, PRICE_THREADS, 0, st>>>(h->Dt.ptr, h->Dt.idx, h->Dt.val, g,
-                                                             h->leafrow_col_offset, h->leafrow_angle, angle_mask,
-                                                             p, L, R, row_price);
+    const int grid = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
+    // the "no beamlets" pass needs one thread per leaf row: fall back to the two-kernel path otherwise
+    if (h->n_beamlets == 0 || (int64_t)grid * PRICE_THREADS < h->n_leaf_rows) {
+        int rc = vmat_launch_price(h, g, p, st);
+        return rc != VMAT_OK ? rc : vmat_launch_select(h, p, angle_mask, L, R, row_price, st);
+    }
+    SelectArgs sa{h->beamlet_leafrow, h->leafrow_col_offset, h->leafrow_angle, angle_mask, h->leafrow_done,
+                  h->S_scratch, L, R, row_price, h->n_leaf_rows};
+    k_price<true><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.ptr, h->Dt.idx, h->Dt.val, h->n_beamlets, g, p, sa);
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }

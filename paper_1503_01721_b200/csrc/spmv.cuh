@@ -1,51 +1,86 @@
-// spmv.cuh - the row-dot building block of both SpMV kernels.
+// spmv.cuh - the streaming building blocks of both SpMV kernels, and the tile-interleaved storage
+// order they rely on.
 //
-// A CSR row [s, e) of (val, idx) is streamed with 256-bit loads: every cooperating thread takes
-// 8 consecutive non-zeros per load (32 B of values + 32 B of indices), so a warp covers 1 KB + 1 KB
-// of contiguous, 32-byte-aligned stream per load pair.  Rows start at arbitrary offsets: the
-// stream is read from the 8-element boundary at or below s and the (at most 7 + 7) elements outside
-// [s, e) are masked.  Two chunks per thread are kept in flight (4 x 32 B = 128 B per thread).
+// Why the layout is not plain CSR order.  A warp must read the (val, idx) streams with wide,
+// coalesced loads (sm_100 has 256-bit loads: 32 lanes x 32 B = 1 KB per instruction), but the gather
+// vec[idx] that follows wants CONSECUTIVE lanes on CONSECUTIVE non-zeros: indices come in runs (a
+// beamlet's voxels are x-runs of the raster, a voxel's beamlets are runs along a leaf row), so 32
+// consecutive non-zeros touch a handful of 32-byte sectors, while "lane l owns non-zeros 8l..8l+7"
+// touches 32 sectors in every gather instruction - ncu showed exactly that (profiles/r1_v1_first_path.md:
+// 2.78 G sectors for 2.78 G gathered floats, L1TEX at 77-83 %, HBM at 45-64 %).
+//
+// So a segment [s, e) of a layout (a beamlet row of D^T; a row block of D) is stored as
+//     head   [s, a0)            plain order,  a0 = min(e, s rounded up to 8)   (<= 7 entries)
+//     tiles  [a0, a0 + 256 nt)  nt = (e - a0) / 256 full tiles, each LANE-INTERLEAVED:
+//                               stored word 8*l + t of a tile holds the tile's logical entry 32*t + l
+//     tail   [a0 + 256 nt, e)   plain order  (< 256 entries)
+// It is a permutation inside the segment: 8 B/nnz, row pointers unchanged.  Lane l's 256-bit load of a
+// tile yields logical entries l, 32+l, ..., 224+l, so gather instruction t covers 32 consecutive entries.
 #pragma once
 #include "common.cuh"
 
-// sum over the 8 elements k..k+7 of val*vec[idx], restricted to [s, e)
-__device__ __forceinline__ float chunk_dot(const Vec8 &v, const Vec8 &c, int64_t k, int64_t s, int64_t e,
-                                           const float *__restrict__ vec)
+constexpr int TILE = 256;
+
+struct Segment {
+    int64_t a0;   // first tile
+    int64_t nt;   // number of full tiles
+    int64_t t0;   // start of the plain tail
+};
+__host__ __device__ __forceinline__ Segment segment_of(int64_t s, int64_t e)
 {
+    Segment g;
+    const int64_t up = (s + 7) & ~int64_t(7);
+    g.a0 = up < e ? up : e;
+    g.nt = (e - g.a0) / TILE;
+    g.t0 = g.a0 + g.nt * TILE;
+    return g;
+}
+
+// One interleaved tile starting at k: this lane's partial of sum val*vec[idx].
+__device__ __forceinline__ float tile_dot(const float *__restrict__ val, const int32_t *__restrict__ idx,
+                                          int64_t k, const float *__restrict__ vec, int lane)
+{
+    const Vec8 v = ld_stream_256(val + k + lane * 8);
+    const Vec8 c = ld_stream_256(idx + k + lane * 8);
     float acc = 0.f;
-    if (k >= s && k + 8 <= e) {
 #pragma unroll
-        for (int t = 0; t < 8; ++t) acc = fmaf(__uint_as_float(v.w[t]), ld_gather(vec + c.w[t]), acc);
-    } else {
-#pragma unroll
-        for (int t = 0; t < 8; ++t)
-            if (k + t >= s && k + t < e) acc = fmaf(__uint_as_float(v.w[t]), ld_gather(vec + c.w[t]), acc);
-    }
+    for (int t = 0; t < 8; ++t) acc = fmaf(__uint_as_float(v.w[t]), ld_gather(vec + c.w[t]), acc);
     return acc;
 }
 
-// Partial dot product of row [s, e) with vec, for thread t of NT cooperating threads.
-// The caller reduces the partials (warp shuffles or a block reduction).
-template <int NT>
-__device__ __forceinline__ float strided_row_dot(const float *__restrict__ val, const int32_t *__restrict__ idx,
-                                                 int64_t s, int64_t e, const float *__restrict__ vec, int t)
+// The plain head [s, a0) and tail [t0, e) of a segment, spread over NT cooperating threads (thread t):
+// calls f(k, val[k] * vec[idx[k]]) for this thread's entries.  At most 7 + 255 entries, so
+// ceil(255 / NT) + 1 independent loads per thread, all issued before the gathers.
+template <int NT, typename F>
+__device__ __forceinline__ void plain_foreach(const float *__restrict__ val, const int32_t *__restrict__ idx,
+                                              int64_t s, const Segment &sg, int64_t e,
+                                              const float *__restrict__ vec, int t, F f)
 {
-    const int64_t a = s & ~int64_t(7);
-    float acc0 = 0.f, acc1 = 0.f;
-    for (int64_t k = a + (int64_t)t * 8; k < e; k += (int64_t)NT * 16) {
-        const int64_t k2 = k + (int64_t)NT * 8;
-        const bool has2 = k2 < e;
-        Vec8 v0 = ld_stream_256(val + k);
-        Vec8 c0 = ld_stream_256(idx + k);
-        Vec8 v1, c1;
-        if (has2) {
-            v1 = ld_stream_256(val + k2);
-            c1 = ld_stream_256(idx + k2);
+    constexpr int N = (TILE - 1 + NT - 1) / NT;           // tail passes (8 for a warp, 1 for 256 threads)
+    constexpr int B = N < 4 ? N : 4;                      // loads issued together
+    const int n_tail = (int)(e - sg.t0);
+#pragma unroll
+    for (int i0 = 0; i0 < N; i0 += B) {
+        float v[B];
+        int c[B];
+#pragma unroll
+        for (int i = 0; i < B; ++i) {
+            const int o = (i0 + i) * NT + t;
+            const bool ok = i0 + i < N && o < n_tail;
+            v[i] = ok ? ld_stream_f(val + sg.t0 + o) : 0.f;
+            c[i] = ok ? ld_stream_i(idx + sg.t0 + o) : 0;
         }
-        acc0 += chunk_dot(v0, c0, k, s, e, vec);
-        if (has2) acc1 += chunk_dot(v1, c1, k2, s, e, vec);
+#pragma unroll
+        for (int i = 0; i < B; ++i) {
+            const int o = (i0 + i) * NT + t;
+            if (i0 + i < N && o < n_tail) f(sg.t0 + o, v[i] * ld_gather(vec + c[i]));
+        }
     }
-    return acc0 + acc1;
+    if (s + t < sg.a0) {                                  // head: NT >= 8 > 7 entries
+        const float v = ld_stream_f(val + s + t);
+        const int c = ld_stream_i(idx + s + t);
+        f(s + t, v * ld_gather(vec + c));
+    }
 }
 
 __device__ __forceinline__ float warp_sum(float v)
