@@ -52,7 +52,7 @@ typedef struct vmat_ddc_info {
     int64_t bytes_csr_d;        /* 8*nnz + 8*(n_voxels+1)   (values + indices + int64 row pointers) */
     int64_t bytes_csr_dt;       /* 8*nnz + 8*(n_beamlets+1)                                         */
     int64_t bytes_device_total; /* everything the handle holds on the device                        */
-    int64_t n_dose_blocks;      /* row blocks (= CTAs) of the dose kernel                           */
+    int64_t n_dose_blocks;      /* segments (one warp each) of the dose kernel                      */
     int64_t max_leaf_row_len;   /* longest leaf row, in beamlets                                    */
     int64_t max_voxel_row_nnz, max_beamlet_row_nnz;
 } vmat_ddc_info;

@@ -63,7 +63,7 @@ int vmat_ddc_destroy(vmat_ddc *h)
 {
     if (!h) return VMAT_OK;
     void *ptrs[] = {h->D.ptr, h->D.idx, h->D.val, h->Dt.ptr, h->Dt.idx, h->Dt.val, h->angle_col_offset,
-                    h->angle_row_offset, h->leafrow_col_offset, h->leafrow_angle, h->blk_row, h->F_partial,
+                    h->angle_row_offset, h->leafrow_col_offset, h->leafrow_angle, h->seg_row, h->F_partial,
                     h->F_partial_obj, h->S_scratch, h->beamlet_leafrow, h->leafrow_done, h->e2e_x, h->e2e_d, h->e2e_g, h->e2e_p, h->e2e_L, h->e2e_R,
                     h->e2e_best, h->e2e_row_price, h->e2e_angle_price, h->e2e_F};
     for (void *p : ptrs)
@@ -152,7 +152,7 @@ int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info)
     info->bytes_csr_d = 8 * h->nnz + 8 * ((int64_t)h->n_voxels + 1);
     info->bytes_csr_dt = 8 * h->nnz + 8 * ((int64_t)h->n_beamlets + 1);
     info->bytes_device_total = h->bytes_device;
-    info->n_dose_blocks = h->n_blocks;
+    info->n_dose_blocks = h->n_seg;
     info->max_leaf_row_len = h->max_leaf_row_len;
     info->max_voxel_row_nnz = h->max_voxel_row_nnz;
     info->max_beamlet_row_nnz = h->max_beamlet_row_nnz;
@@ -173,12 +173,12 @@ int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx
     // undo the tile interleave (spmv.cuh): the caller gets canonical CSR order
     std::vector<int64_t> hp((size_t)A.n_rows + 1);
     memcpy(hp.data(), ptr, hp.size() * 8);
-    const int64_t n_seg = which == 0 ? (int64_t)h->n_blocks : (int64_t)A.n_rows;
+    const int64_t n_seg = which == 0 ? (int64_t)h->n_seg : (int64_t)A.n_rows;
     int32_t ti_[TILE];
     float tv_[TILE];
     for (int64_t w = 0; w < n_seg; ++w) {
-        const int64_t s = which == 0 ? hp[h->h_blk_row[w]] : hp[w];
-        const int64_t e = which == 0 ? hp[h->h_blk_row[w + 1]] : hp[w + 1];
+        const int64_t s = which == 0 ? hp[h->h_seg_row[w]] : hp[w];
+        const int64_t e = which == 0 ? hp[h->h_seg_row[w + 1]] : hp[w + 1];
         const Segment sg = segment_of(s, e);
         for (int64_t t = 0; t < sg.nt; ++t) {
             int32_t *pi = idx + sg.a0 + t * TILE;

@@ -49,17 +49,18 @@ struct vmat_ddc {
     int32_t *angle_row_offset = nullptr;    // [n_angles+1]
     int32_t *leafrow_col_offset = nullptr;  // [n_leaf_rows+1]
     int32_t *leafrow_angle = nullptr;       // [n_leaf_rows] control point of each leaf row
-    // dose kernel work list: row block b covers voxel rows [blk_row[b], blk_row[b+1])
-    int32_t *blk_row = nullptr;             // [n_blocks+1]
-    int32_t n_blocks = 0;
-    double *F_partial = nullptr;            // [n_blocks] per-block objective partials
+    // dose kernel work list: segment i (one warp) covers voxel rows [seg_row[i], seg_row[i+1])
+    int32_t *seg_row = nullptr;             // [n_seg+1]
+    int32_t n_seg = 0;
+    int32_t n_blocks = 0;                   // CTAs of the dose kernel = ceil(n_seg / warps per CTA)
+    double *F_partial = nullptr;            // [n_blocks] per-CTA objective partials
     int32_t n_obj_blocks = 0;               // blocks of the standalone objective kernel
     double *F_partial_obj = nullptr;        // [n_obj_blocks]
     double *S_scratch = nullptr;            // [n_beamlets + n_leaf_rows + 1] prefix sums of the row selection
     int32_t *beamlet_leafrow = nullptr;     // [n_beamlets] leaf row of each beamlet
     uint32_t *leafrow_done = nullptr;       // [n_leaf_rows] tickets of the fused price+selection kernel (self-resetting)
     std::vector<int32_t> h_angle_row_offset; // host copy
-    std::vector<int32_t> h_blk_row;          // host copy of blk_row (export un-permutes the tiles)
+    std::vector<int32_t> h_seg_row;          // host copy of seg_row (export un-permutes the tiles)
     int32_t max_leaf_row_len = 0;
     int64_t max_voxel_row_nnz = 0, max_beamlet_row_nnz = 0;
     int64_t bytes_device = 0;
@@ -76,12 +77,15 @@ struct vmat_ddc {
 #ifndef VMAT_DOSE_THREADS
 #define VMAT_DOSE_THREADS 256
 #endif
-#ifndef VMAT_DOSE_BLOCK_NNZ
-#define VMAT_DOSE_BLOCK_NNZ 4096
+#ifndef VMAT_DOSE_SEG_NNZ
+#define VMAT_DOSE_SEG_NNZ 512
+#endif
+#ifndef VMAT_DOSE_MINB
+#define VMAT_DOSE_MINB 6
 #endif
 constexpr int DOSE_THREADS = VMAT_DOSE_THREADS;
-constexpr int DOSE_BLOCK_NNZ = VMAT_DOSE_BLOCK_NNZ;   // products per block held in smem (4 B each)
-constexpr int DOSE_MAX_ROWS = 1024;         // rows per block (bounds runs of empty rows)
+constexpr int DOSE_SEG_NNZ = VMAT_DOSE_SEG_NNZ;   // a warp's group of short rows holds at most this many non-zeros
+constexpr int DOSE_MAX_ROWS = 256;                // rows per segment (bounds runs of empty rows)
 // Price kernel (CSR-vector, one warp per beamlet row, L127).
 constexpr int PRICE_THREADS = 256;
 constexpr int PRICE_WARPS = PRICE_THREADS / 32;

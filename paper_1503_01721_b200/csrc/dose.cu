@@ -1,21 +1,18 @@
 // dose.cu - A1 forward dose d = D x through the voxel-row CSR, with the
 // objective / gradient (Eq. (1), Eq. (4)) fused into the row epilogue (A2).
 //
-// Voxel rows are ragged (0 ... ~18 k non-zeros, mean 10^2-10^3), so rows are not mapped to warps
-// one by one.  The ingest step cuts the row range into blocks of <= DOSE_BLOCK_NNZ non-zeros
-// (a row longer than that is a block of its own); one CTA per block:
-//   several rows : the whole CTA streams the block's contiguous (val, idx) range with 256-bit loads,
-//                  multiplies by the gathered x and parks the products in shared memory; then groups
-//                  of G lanes (G sized to the block's mean row length) reduce one row each with
-//                  shuffles.  Streaming is perfectly coalesced whatever the row lengths are.
-//   one row      : all threads accumulate the row in registers; one block reduction.
-// Everything is FP32 with a fixed summation order; the objective partials are FP64, one per block,
-// summed afterwards in a fixed order (no atomics).
+// Voxel rows are ragged (0 ... ~18 k non-zeros, mean 10^2-10^3).  The ingest step cuts the row range
+// into SEGMENTS, each owned by one warp (8 consecutive segments per CTA, so neighbouring voxels - which
+// see nearly the same beamlets - share the x sectors cached in L1):
+//   long row   (> DOSE_SEG_NNZ non-zeros)  a segment of its own: the warp streams the row's interleaved
+//              tiles with 256-bit loads and accumulates in registers, as the price kernel does;
+//   short rows (consecutive rows, <= DOSE_SEG_NNZ non-zeros together)  the warp streams the contiguous
+//              range once, parks the products in its private slice of shared memory, then groups of
+//              G lanes (G sized to the segment's mean row length) reduce one row each with shuffles.
+// No block-wide barrier sits in the hot path (the first version, one CTA per 4096-entry block, lost
+// 21 % of its issue slots to barrier stalls - profiles/).  Everything is FP32 with a fixed summation
+// order; the objective partials are FP64, one per CTA, summed afterwards in a fixed order (no atomics).
 #include "spmv.cuh"
-
-struct ObjTables {              // per-structure parameters staged in shared memory
-    float T[256], wo[256], wu[256];
-};
 
 // g_i and the voxel's term of F for dose v (Eq. (1); sign and factor 2: C1, C2)
 __device__ __forceinline__ float voxel_grad(float v, float T, float wo, float wu, double &f)
@@ -41,90 +38,73 @@ __device__ __forceinline__ double block_sum_double(double v, double *red /* [NT/
 }
 
 template <bool FUSE>
-__global__ void __launch_bounds__(DOSE_THREADS)
+__global__ void __launch_bounds__(DOSE_THREADS, VMAT_DOSE_MINB)
 k_dose(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const float *__restrict__ val,
-       const int32_t *__restrict__ blk_row, const float *__restrict__ x, float *__restrict__ d,
-       const uint8_t *__restrict__ vstruct, int n_struct, const float *__restrict__ T,
+       const int32_t *__restrict__ seg_row, int n_seg, const float *__restrict__ x, float *__restrict__ d,
+       const uint8_t *__restrict__ vstruct, const float *__restrict__ T,
        const float *__restrict__ w_over, const float *__restrict__ w_under, float *__restrict__ g,
        double *__restrict__ F_partial)
 {
-    __shared__ float prod[DOSE_BLOCK_NNZ];
-    __shared__ float red_f[DOSE_THREADS / 32];
+    __shared__ float prod[DOSE_THREADS / 32][DOSE_SEG_NNZ];
     __shared__ double red_d[DOSE_THREADS / 32];
-    __shared__ ObjTables tab;
-
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (FUSE) {
-        for (int i = tid; i < n_struct; i += DOSE_THREADS) {
-            tab.T[i] = T[i];
-            tab.wo[i] = w_over[i];
-            tab.wu[i] = w_under[i];
-        }
-        __syncthreads();
-    }
-    const int r0 = blk_row[blockIdx.x], r1 = blk_row[blockIdx.x + 1];
-    const int nr = r1 - r0;
-    const int64_t s = ptr[r0], e = ptr[r1];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sgi = blockIdx.x * (DOSE_THREADS / 32) + warp;
     double fsum = 0.0;
-
-    const Segment sg = segment_of(s, e);
-    if (nr == 1) {
-        // ---- one row: register accumulation by the whole CTA (warps take tiles round-robin)
-        float acc = 0.f;
-        for (int64_t ti = warp; ti < sg.nt; ti += DOSE_THREADS / 32)
-            acc += tile_dot(val, idx, sg.a0 + ti * TILE, x, lane);
-        plain_foreach<DOSE_THREADS>(val, idx, s, sg, e, x, tid, [&](int64_t, float q) { acc += q; });
-        acc = warp_sum(acc);
-        if (lane == 0) red_f[warp] = acc;
-        __syncthreads();
-        if (tid == 0) {
-            float tot = 0.f;
-#pragma unroll
-            for (int i = 0; i < DOSE_THREADS / 32; ++i) tot += red_f[i];
-            d[r0] = tot;
-            if (FUSE) {
-                const int sid = vstruct[r0];
-                g[r0] = voxel_grad(tot, tab.T[sid], tab.wo[sid], tab.wu[sid], fsum);
-            }
+    auto epilogue = [&](int r, float v) {          // d, and the fused A2: g and the voxel's term of F
+        d[r] = v;
+        if (FUSE) {
+            const int sid = vstruct[r];
+            g[r] = voxel_grad(v, __ldg(T + sid), __ldg(w_over + sid), __ldg(w_under + sid), fsum);
         }
-    } else {
-        // ---- several rows: products into shared memory at their logical position k - s ...
-        for (int64_t ti = warp; ti < sg.nt; ti += DOSE_THREADS / 32) {
-            const int64_t k = sg.a0 + ti * TILE;
-            const Vec8 v = ld_stream_256(val + k + lane * 8);
-            const Vec8 c = ld_stream_256(idx + k + lane * 8);
-            float *dst = prod + (k - s) + lane;
-#pragma unroll
-            for (int t = 0; t < 8; ++t) dst[32 * t] = __uint_as_float(v.w[t]) * ld_gather(x + c.w[t]);
-        }
-        plain_foreach<DOSE_THREADS>(val, idx, s, sg, e, x, tid, [&](int64_t k, float q) { prod[k - s] = q; });
-        __syncthreads();
-        // ... then G lanes per row, G = power of two near (mean row length)/4, 1..32
-        const int mean = (int)((e - s) / nr);
-        int G = 1;
-        while (G < 32 && G * 4 < mean) G <<= 1;
-        const int grp = tid / G, gl = tid % G, n_grp = DOSE_THREADS / G;
-        const int n_iter = (nr + n_grp - 1) / n_grp;            // uniform trip count: shuffles stay converged
-        for (int it = 0; it < n_iter; ++it) {
-            const int r = r0 + grp + it * n_grp;
+    };
+    if (sgi < n_seg) {
+        const int r0 = seg_row[sgi], r1 = seg_row[sgi + 1];
+        const int nr = r1 - r0;
+        const int64_t s = ptr[r0], e = ptr[r1];
+        const Segment sg = segment_of(s, e);
+        if (nr == 1) {
+            // ---- one row: register accumulation
             float acc = 0.f;
-            if (r < r1) {
-                const int b = (int)(ptr[r] - s), f = (int)(ptr[r + 1] - s);
-                for (int k = b + gl; k < f; k += G) acc += prod[k];
+#pragma unroll 1
+            for (int64_t ti = 0; ti < sg.nt; ++ti) acc += tile_dot(val, idx, sg.a0 + ti * TILE, x, lane);
+            plain_foreach<32>(val, idx, s, sg, e, x, lane, [&](int64_t, float q) { acc += q; });
+            acc = warp_sum(acc);
+            if (lane == 0) epilogue(r0, acc);
+        } else {
+            // ---- several short rows: products into this warp's slice at their logical position k - s ...
+            float *wp = prod[warp];
+#pragma unroll 1
+            for (int64_t ti = 0; ti < sg.nt; ++ti) {
+                const int64_t k = sg.a0 + ti * TILE;
+                const Vec8 v = ld_stream_256(val + k + lane * 8);
+                const Vec8 c = ld_stream_256(idx + k + lane * 8);
+                float *dst = wp + (k - s) + lane;
+#pragma unroll
+                for (int t = 0; t < 8; ++t) dst[32 * t] = __uint_as_float(v.w[t]) * ld_gather(x + c.w[t]);
             }
-            for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-            if (r < r1 && gl == 0) {
-                d[r] = acc;
-                if (FUSE) {
-                    const int sid = vstruct[r];
-                    g[r] = voxel_grad(acc, tab.T[sid], tab.wo[sid], tab.wu[sid], fsum);
+            plain_foreach<32>(val, idx, s, sg, e, x, lane, [&](int64_t k, float q) { wp[k - s] = q; });
+            __syncwarp();
+            // ... then G lanes per row, G = power of two near (mean row length)/4, 1..32
+            const int mean = (int)((e - s) / nr);
+            int G = 1;
+            while (G < 32 && G * 4 < mean) G <<= 1;
+            const int grp = lane / G, gl = lane % G, n_grp = 32 / G;
+            const int n_iter = (nr + n_grp - 1) / n_grp;        // uniform trip count: shuffles stay converged
+            for (int it = 0; it < n_iter; ++it) {
+                const int r = r0 + grp + it * n_grp;
+                float acc = 0.f;
+                if (r < r1) {
+                    const int b = (int)(ptr[r] - s), f = (int)(ptr[r + 1] - s);
+                    for (int k = b + gl; k < f; k += G) acc += wp[k];
                 }
+                for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+                if (r < r1 && gl == 0) epilogue(r, acc);
             }
         }
     }
     if (FUSE) {
         const double tot = block_sum_double<DOSE_THREADS>(fsum, red_d);
-        if (tid == 0) F_partial[blockIdx.x] = tot;
+        if (threadIdx.x == 0) F_partial[blockIdx.x] = tot;
     }
 }
 
@@ -135,19 +115,12 @@ k_objective(int n_voxels, const float *__restrict__ d, const uint8_t *__restrict
             const float *__restrict__ T, const float *__restrict__ w_over, const float *__restrict__ w_under,
             float *__restrict__ g, double *__restrict__ F_partial)
 {
-    __shared__ ObjTables tab;
     __shared__ double red_d[OBJ_THREADS / 32];
-    for (int i = threadIdx.x; i < n_struct; i += OBJ_THREADS) {
-        tab.T[i] = T[i];
-        tab.wo[i] = w_over[i];
-        tab.wu[i] = w_under[i];
-    }
-    __syncthreads();
     const int i = blockIdx.x * OBJ_THREADS + threadIdx.x;
     double f = 0.0;
     if (i < n_voxels) {
         const int sid = vstruct[i];
-        g[i] = voxel_grad(d[i], tab.T[sid], tab.wo[sid], tab.wu[sid], f);
+        g[i] = voxel_grad(d[i], __ldg(T + sid), __ldg(w_over + sid), __ldg(w_under + sid), f);
     }
     const double tot = block_sum_double<OBJ_THREADS>(f, red_d);
     if (threadIdx.x == 0) F_partial[blockIdx.x] = tot;
@@ -172,13 +145,11 @@ int vmat_launch_dose(const vmat_ddc *h, const float *x, float *d, bool fuse,
     if (fuse && h->prof_ev[0]) VMAT_CUDA(cudaEventRecord(h->prof_ev[0], st));
     if (h->n_blocks > 0) {
         if (fuse)
-            k_dose<true><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.ptr, h->D.idx, h->D.val, h->blk_row, x, d,
-                                                               voxel_struct, n_struct, T, w_over, w_under, g,
-                                                               h->F_partial);
+            k_dose<true><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.ptr, h->D.idx, h->D.val, h->seg_row, h->n_seg, x, d,
+                                                               voxel_struct, T, w_over, w_under, g, h->F_partial);
         else
-            k_dose<false><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.ptr, h->D.idx, h->D.val, h->blk_row, x, d,
-                                                                nullptr, 0, nullptr, nullptr, nullptr, nullptr,
-                                                                nullptr);
+            k_dose<false><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.ptr, h->D.idx, h->D.val, h->seg_row, h->n_seg, x, d,
+                                                                nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
         VMAT_LAUNCH_CHECK();
     }
     if (fuse && h->prof_ev[1]) VMAT_CUDA(cudaEventRecord(h->prof_ev[1], st));

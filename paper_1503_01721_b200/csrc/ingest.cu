@@ -176,15 +176,15 @@ __global__ void k_sort_rows_gmem(const int64_t *__restrict__ ptr, int32_t *idx, 
 }
 
 // ---------------------------------------------------------------- tile interleave (spmv.cuh)
-// One warp per segment (a beamlet row of D^T when blk_row == NULL, else a row block of D): every full
+// One warp per segment (a beamlet row of D^T when seg_row == NULL, else a dose segment of D): every full
 // 256-entry tile is permuted in place so that stored word 8*l + t holds the tile's entry 32*t + l.
 __global__ void __launch_bounds__(256)
-k_interleave(const int64_t *__restrict__ ptr, const int32_t *__restrict__ blk_row, int n_seg,
+k_interleave(const int64_t *__restrict__ ptr, const int32_t *__restrict__ seg_row, int n_seg,
              int32_t *idx, float *val)
 {
     const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (w >= n_seg) return;
-    const int r0 = blk_row ? blk_row[w] : w, r1 = blk_row ? blk_row[w + 1] : w + 1;
+    const int r0 = seg_row ? seg_row[w] : w, r1 = seg_row ? seg_row[w + 1] : w + 1;
     const int64_t s = ptr[r0], e = ptr[r1];
     const Segment sg = segment_of(s, e);
     for (int64_t ti = 0; ti < sg.nt; ++ti) {
@@ -336,25 +336,27 @@ int vmat_build_layouts(vmat_ddc *h, const int32_t *coo_voxel, const int32_t *coo
     VMAT_CUDA(cudaStreamSynchronize(st));
     if (hf[FLAG_DUP]) { vmat_set_error("vmat_ddc_create: duplicate (voxel, beamlet) pair"); return VMAT_ERR_DUPLICATE; }
 
-    // ---- dose kernel row blocks (host, from the voxel row pointers)
+    // ---- dose kernel segments (host, from the voxel row pointers): a long row alone, or consecutive
+    //      short rows with at most DOSE_SEG_NNZ non-zeros together
     std::vector<int64_t> hptr((size_t)nv + 1);
     VMAT_CUDA(cudaMemcpy(hptr.data(), h->D.ptr, ((size_t)nv + 1) * 8, cudaMemcpyDeviceToHost));
-    std::vector<int32_t> blk;
-    blk.push_back(0);
+    std::vector<int32_t> seg;
+    seg.push_back(0);
     int32_t r = 0;
     while (r < nv) {
-        int32_t r1 = r + 1;                                   // a block always takes at least one row
-        while (r1 < nv && r1 - r < DOSE_MAX_ROWS && hptr[r1 + 1] - hptr[r] <= DOSE_BLOCK_NNZ) ++r1;
-        blk.push_back(r1);
+        int32_t r1 = r + 1;                                   // a segment always takes at least one row
+        while (r1 < nv && r1 - r < DOSE_MAX_ROWS && hptr[r1 + 1] - hptr[r] <= DOSE_SEG_NNZ) ++r1;
+        seg.push_back(r1);
         r = r1;
     }
-    h->n_blocks = (int32_t)blk.size() - 1;
-    TRY(dev_alloc(&h->blk_row, (int64_t)blk.size(), &h->bytes_device));
-    VMAT_CUDA(cudaMemcpy(h->blk_row, blk.data(), blk.size() * 4, cudaMemcpyHostToDevice));
-    h->h_blk_row = blk;
-    // ---- tile-interleave both layouts: segments = row blocks of D, beamlet rows of D^T
+    h->n_seg = (int32_t)seg.size() - 1;
+    h->n_blocks = (h->n_seg + DOSE_THREADS / 32 - 1) / (DOSE_THREADS / 32);
+    TRY(dev_alloc(&h->seg_row, (int64_t)seg.size(), &h->bytes_device));
+    VMAT_CUDA(cudaMemcpy(h->seg_row, seg.data(), seg.size() * 4, cudaMemcpyHostToDevice));
+    h->h_seg_row = seg;
+    // ---- tile-interleave both layouts: segments = dose segments of D, beamlet rows of D^T
     if (nnz > 0) {
-        k_interleave<<<(h->n_blocks + 7) / 8, 256, 0, st>>>(h->D.ptr, h->blk_row, h->n_blocks, h->D.idx, h->D.val);
+        k_interleave<<<(h->n_seg + 7) / 8, 256, 0, st>>>(h->D.ptr, h->seg_row, h->n_seg, h->D.idx, h->D.val);
         VMAT_LAUNCH_CHECK();
         k_interleave<<<(nb + 7) / 8, 256, 0, st>>>(h->Dt.ptr, nullptr, nb, h->Dt.idx, h->Dt.val);
         VMAT_LAUNCH_CHECK();

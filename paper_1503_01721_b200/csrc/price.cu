@@ -129,6 +129,7 @@ k_price(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const 
     const int64_t s = ptr[row], e = ptr[row + 1];
     const Segment sg = segment_of(s, e);
     float acc = 0.f;
+#pragma unroll 1
     for (int64_t ti = 0; ti < sg.nt; ++ti) acc += tile_dot(val, idx, sg.a0 + ti * TILE, g, lane);
     plain_foreach<32>(val, idx, s, sg, e, g, lane, [&](int64_t, float q) { acc += q; });
     acc = warp_sum(acc);
