@@ -3,6 +3,7 @@
 #include "spmv.cuh"
 #include <stdarg.h>
 #include <string.h>
+#include <stdlib.h>
 #include <new>
 #include <vector>
 
@@ -260,7 +261,13 @@ int vmat_price_eval(const vmat_ddc *h, const float *x,
     g_vmat_launches = 0;
     TRY(vmat_launch_dose(h, x, d, true, voxel_struct, n_struct, T, w_over, w_under, g, F, st));
     if (h->prof_ev[2]) VMAT_CUDA(cudaEventRecord(h->prof_ev[2], st));
-    TRY(vmat_launch_price_select(h, g, angle_mask, p, L, R, row_price, st));
+    static const bool unfused = getenv("VMAT_UNFUSED_SELECT") != nullptr;   // measurement knob: A3 and A4 as two kernels
+    if (unfused) {
+        TRY(vmat_launch_price(h, g, p, st));
+        TRY(vmat_launch_select(h, p, angle_mask, L, R, row_price, st));
+    } else {
+        TRY(vmat_launch_price_select(h, g, angle_mask, p, L, R, row_price, st));
+    }
     if (h->prof_ev[3]) VMAT_CUDA(cudaEventRecord(h->prof_ev[3], st));
     return vmat_launch_angle_price(h, row_price, angle_mask, angle_price, best_angle, st);
 }

@@ -5,9 +5,9 @@
 // so the paper's mapping holds on sm_100a: one warp per beamlet row (L127), here over lane-interleaved
 // 256-entry tiles read with 256-bit loads (spmv.cuh).  Measured on B200 the warp-per-row kernel beats
 // a CTA-per-leaf-row kernel by 12 % (perfect balance, more independent streams), so the row selection
-// is fused differently: every warp takes a ticket of its leaf row after writing its price, and the
-// warp that draws the last ticket selects that row's opening on the spot - the selection costs no
-// launch and no second pass over p, and the price kernel keeps its one-warp-per-row balance.
+// is fused differently: every CTA (8 consecutive beamlet rows) hands in tickets for the leaf rows it
+// priced, and the CTA whose ticket completes a leaf row selects that row's opening on the spot - the
+// selection costs no launch and no second pass over p, and the price kernel keeps its balance.
 //
 // Selection arithmetic (readings C4-C6, C8): S_0 = 0, S_{c+1} = S_c + (double)p_c left to
 // right in FP64; candidates all 0 <= L <= R <= n with V = S_R - S_L; result = smallest (V, L, R).
@@ -124,29 +124,50 @@ k_price(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const 
             sa.L[r] = 0; sa.R[r] = 0; sa.row_price[r] = 0.0;
         }
     }
-    const int row = blockIdx.x * PRICE_WARPS + (threadIdx.x >> 5);
-    if (row >= n_rows) return;
-    const int64_t s = ptr[row], e = ptr[row + 1];
-    const Segment sg = segment_of(s, e);
-    float acc = 0.f;
+    const int warp = threadIdx.x >> 5;
+    const int row = blockIdx.x * PRICE_WARPS + warp;
+    if (row < n_rows) {
+        const int64_t s = ptr[row], e = ptr[row + 1];
+        const Segment sg = segment_of(s, e);
+        float acc = 0.f;
 #pragma unroll 1
-    for (int64_t ti = 0; ti < sg.nt; ++ti) acc += tile_dot(val, idx, sg.a0 + ti * TILE, g, lane);
-    plain_foreach<32>(val, idx, s, sg, e, g, lane, [&](int64_t, float q) { acc += q; });
-    acc = warp_sum(acc);
-    if (lane == 0) p[row] = acc;
+        for (int64_t ti = 0; ti < sg.nt; ++ti) acc += tile_dot(val, idx, sg.a0 + ti * TILE, g, lane);
+        plain_foreach<32>(val, idx, s, sg, e, g, lane, [&](int64_t, float q) { acc += q; });
+        acc = warp_sum(acc);
+        if (lane == 0) p[row] = acc;
+    }
     if (SELECT) {
-        const int r = sa.beamlet_leafrow[row];
-        const int j0 = sa.leafrow_col_offset[r];
-        const int n = sa.leafrow_col_offset[r + 1] - j0;
-        int last = 0;
-        if (lane == 0) {
-            __threadfence();                                            // p[row] visible before the ticket
-            last = atomicAdd(sa.leafrow_done + r, 1u) == (uint32_t)(n - 1);
+        // One ticket per CTA and leaf row: the CTA's 8 consecutive beamlet rows lie in a few leaf rows.
+        // Thread 0 adds, for each of them, the number of its rows this CTA priced; the CTA whose add
+        // completes a leaf row selects that row's opening (warp w takes the w-th completed row).
+        __shared__ int done_rows[PRICE_WARPS];
+        __shared__ int n_done;
+        __syncthreads();                                                // the CTA's prices are written
+        if (threadIdx.x == 0) {
+            __threadfence();                                            // ... and visible before the tickets
+            int nd = 0;
+            const int row0 = blockIdx.x * PRICE_WARPS;
+            const int row1 = min(row0 + PRICE_WARPS, n_rows);
+            int c = row0;
+            while (c < row1) {
+                const int r = sa.beamlet_leafrow[c];
+                const int j1 = sa.leafrow_col_offset[r + 1];
+                const int cnt = min(row1, j1) - c;                      // rows of leaf row r priced here
+                const int n = j1 - sa.leafrow_col_offset[r];
+                if (atomicAdd(sa.leafrow_done + r, (uint32_t)cnt) + cnt == (uint32_t)n) {
+                    sa.leafrow_done[r] = 0;                             // ready for the next launch
+                    done_rows[nd++] = r;
+                }
+                c += cnt;
+            }
+            if (nd > 0) __threadfence();
+            n_done = nd;
         }
-        last = __shfl_sync(0xffffffffu, last, 0);
-        if (last) {                                                     // every price of leaf row r is written
-            if (lane == 0) sa.leafrow_done[r] = 0;                      // ready for the next launch
-            __threadfence();
+        __syncthreads();
+        if (warp < n_done) {                                            // every price of leaf row r is written
+            const int r = done_rows[warp];
+            const int j0 = sa.leafrow_col_offset[r];
+            const int n = sa.leafrow_col_offset[r + 1] - j0;
             const bool occupied = sa.angle_mask != nullptr && sa.angle_mask[sa.leafrow_angle[r]] != 0;   // C7
             const Opening best = warp_select_row(p + j0, occupied ? 0 : n, sa.S + j0 + r, lane);
             if (lane == 0) {
