@@ -94,6 +94,25 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def rank_eval_index(rank: int, k: int) -> int:
+    """Fluence draw index of step k on `rank`: every replica prices its own sequence of x vectors."""
+    return rank * 100000 + k
+
+
+def reduce_max(values, dist, device):
+    """Max over ranks of per-rank device times (dist = torch.distributed or None for one rank)."""
+    if dist is None:
+        return [float(v) for v in values]
+    t = torch.tensor(values, dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def aggregate(world: int, steps: int, elapsed_ms: float) -> dict:
+    """Whole-job throughput: all ranks' evaluations over the slowest rank's time."""
+    return {"value": world * steps / (elapsed_ms * 1e-3), "ms_per_step": elapsed_ms / steps}
+
+
 def phantom_arrays_host(ph):
     return dict(vox=ph.coo_voxel.cpu().numpy(), beam=ph.coo_beamlet.cpu().numpy(), val=ph.coo_val.cpu().numpy(),
                 n_v=ph.n_voxels, n_b=ph.n_beamlets, sid=ph.voxel_struct.numpy(), T=ph.struct_T.numpy(),
@@ -102,7 +121,7 @@ def phantom_arrays_host(ph):
 
 
 # ----------------------------------------------------------------------------- the CPU oracle, timed
-def oracle_rate(spec, gen_device, budget_s: float, reps: int):
+def oracle_rate(spec, gen_device, budget_s: float, reps: int, reps_auto: bool = False):
     """Times the oracle (one whole price evaluation, O1-O5) on an angle-block sample of `spec`
     (D = [D_1 ... D_A]; the evaluation is additive over angle blocks) sized to about
     `budget_s` seconds of single-thread CPU work.  Returns (evals/s extrapolated to the full matrix,
@@ -117,12 +136,14 @@ def oracle_rate(spec, gen_device, budget_s: float, reps: int):
     oracle.price_eval(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], x, A["sid"], A["T"], A["wo"], A["wu"],
                       A["lco"], A["aro"])
     t1 = time.perf_counter() - t0
-    k = int(max(1, min(n_a, budget_s / max(t1, 1e-4))))
+    k = int(max(1, min(n_a, budget_s / max(t1, 1e-4), 4e8 / max(probe.nnz, 1))))   # <= ~4e8 nnz (5 GB of host COO)
     angles = sorted(set(int(round(i * n_a / k)) % n_a for i in range(k)))
     smp = synth.generate(spec, device=gen_device, angles=angles)
     A = phantom_arrays_host(smp)
     times = []
     for r in range(reps):
+        if r >= 3 and reps_auto and sum(times) > budget_s:
+            break
         x = synth.draw_x(smp.n_beamlets, r).numpy()
         t0 = time.perf_counter()
         oracle.price_eval(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], x, A["sid"], A["T"], A["wo"],
@@ -131,7 +152,7 @@ def oracle_rate(spec, gen_device, budget_s: float, reps: int):
     frac = len(angles) / n_a
     t_full = float(np.median(times)) / frac                 # the evaluation is additive over angle blocks
     desc = (f"{len(angles)} of {n_a} control points of {spec.name} (every {n_a / len(angles):.1f}th angle block, "
-            f"{smp.nnz} nnz), whole evaluation O1-O5 per rep, {reps} reps, median; evals/s extrapolated by "
+            f"{smp.nnz} nnz), whole evaluation O1-O5 per rep, {len(times)} reps, median; evals/s extrapolated by "
             f"angle-block additivity (x{1 / frac:.1f})")
     return 1.0 / t_full, desc, times, smp.nnz, smp.nnz / frac
 
@@ -199,7 +220,7 @@ def run_ours(args):
     n_b, n_v, nnz = h.n_beamlets, h.n_voxels, h.nnz
     n_rows, n_a = h.n_leaf_rows, h.n_angles
     # x re-drawn for every evaluation (configs[4]); each rank draws its own sequence
-    xs = [synth.draw_x(n_b, rank * 100000 + k, device=dev) for k in range(K + W)]
+    xs = [synth.draw_x(n_b, rank_eval_index(rank, k), device=dev) for k in range(K + W)]
 
     def barrier():
         if use_dist:
@@ -257,10 +278,7 @@ def run_ours(args):
     d2h = 4 * n_rows * 2 + 8 * n_rows + 8 * n_a + 4 + 8
 
     # ---- max over ranks
-    if use_dist:
-        t = torch.tensor([elapsed_ms, e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        elapsed_ms, e2e_ms = float(t[0]), float(t[1])
+    elapsed_ms, e2e_ms = reduce_max([elapsed_ms, e2e_ms], dist if use_dist else None, dev)
 
     if rank == 0:
         peak, peak_src = measured_peaks()
@@ -273,8 +291,8 @@ def run_ours(args):
         k_price = {"name": "k_price_select", "ms": float(t_price.mean()), "ms_min": float(t_price.min()),
                    "bytes": B_price, "gbs": B_price / (t_price.mean() * 1e-3) / 1e9}
         dom = k_price if k_price["ms"] >= k_dose["ms"] else k_dose
-        ms_per_step = elapsed_ms / K
-        value = world * K / (elapsed_ms * 1e-3)
+        agg = aggregate(world, K, elapsed_ms)
+        ms_per_step, value = agg["ms_per_step"], agg["value"]
         eval_gbs = B_eval / (ms_per_step * 1e-3) / 1e9
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -289,7 +307,7 @@ def run_ours(args):
                        "ingest_s": round(t_ingest, 2)},
             "hbm_gbs": eval_gbs, "hbm_frac_of_8TBs": eval_gbs / 8000.0, "hbm_frac_of_measured": eval_gbs / peak,
             "clocks": clocks,
-            "e2e": {"value": world * K / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+            "e2e": {"value": aggregate(world, K, e2e_ms)["value"], "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / K},
             "gpu_launches": launches,
             "roofline": {"bound": "hbm", "kernel": dom["name"], "achieved": dom["gbs"], "peak": peak,
@@ -300,7 +318,7 @@ def run_ours(args):
             "result_check": {"F_last": F_last, "best_angle_last": best_last},
         }
         if not args.no_cpu_baseline and world == 1:
-            v, desc, _, _, _ = oracle_rate(spec, dev, 12.0, 3)
+            v, desc, _, _, _ = oracle_rate(spec, dev, 12.0, 40, reps_auto=True)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc}
         print(json.dumps(line))
     h.close()

@@ -170,3 +170,71 @@ def test_config1_full(vm):
 
 def test_config2_full(vm):
     _full_parity(vm, _phantom_on_gpu(2), [1.0])
+
+
+def test_config3_full_size_sampled(vm):
+    """Config 3 at full size (2.8e9 nnz, the workload and launch configuration bench.py times):
+    sampled outputs the oracle computes one by one, the whole selection, and properties that hold at any size."""
+    import paper_1503_01721_b200 as vmod
+    ph = _phantom_on_gpu(3)
+    n_v, n_b = ph.n_voxels, ph.n_beamlets
+    h = vmod.vmat_ddc_create(n_v, n_b, ph.coo_voxel, ph.coo_beamlet, ph.coo_val, ph.angle_col_offset,
+                             ph.angle_row_offset, ph.leafrow_col_offset, device=DEV)
+    A = dict(sid=ph.voxel_struct.numpy(), T=ph.struct_T.numpy(), wo=ph.struct_w_over.numpy(),
+             wu=ph.struct_w_under.numpy(), lco=ph.leafrow_col_offset.numpy(), aro=ph.angle_row_offset.numpy())
+    obj = obj_to_device(A, DEV)
+    out = h.alloc_outputs()
+    x = synth.draw_x(n_b, 7, scale=0.55)                       # near balance: mixed-sign prices
+    vmod.vmat_price_eval(h, x.to(DEV), obj, out)
+    torch.cuda.synchronize()
+    d, g, p = out.d.cpu().numpy(), out.g.cpu().numpy(), out.p.cpu().numpy()
+    assert h.info["nnz"] == ph.nnz > 2 ** 31                   # 64-bit offsets are exercised
+
+    # -- sampled voxel rows (A1): longest row, empty rows, random rows
+    rng = np.random.default_rng(33)
+    cnt_v = torch.bincount(ph.coo_voxel.long(), minlength=n_v)
+    sv = np.unique(np.concatenate([rng.choice(n_v, 48, replace=False), [int(cnt_v.argmax())],
+                                   torch.nonzero(cnt_v == 0).flatten()[:4].cpu().numpy(), [0, n_v - 1]]))
+    m = torch.isin(ph.coo_voxel, torch.from_numpy(sv).to(DEV, torch.int32))
+    d_ref = oracle.dose(ph.coo_voxel[m].cpu().numpy(), ph.coo_beamlet[m].cpu().numpy(), ph.coo_val[m].cpu().numpy(),
+                        n_v, x.numpy())[sv]
+    del m
+    dmax = float(np.abs(d).max())
+    assert np.abs(d[sv] - d_ref).max() <= 1e-4 * dmax
+    assert np.linalg.norm(d[sv] - d_ref) <= REL_L2 * np.linalg.norm(d_ref)
+    print(f"  sampled d: {sv.size} rows, longest {int(cnt_v.max())} nnz, rel L2 err "
+          f"{np.linalg.norm(d[sv] - d_ref) / np.linalg.norm(d_ref):.2e}")
+
+    # -- A2 on the GPU's own d, every voxel (elementwise; F is a plain sum)
+    F_ref, g_ref = oracle.objective_grad(d.astype(np.float64), A["sid"], A["T"], A["wo"], A["wu"])
+    assert_vec_close("g", g, g_ref)
+    assert abs(out.F.item() - F_ref) <= REL_L2 * F_ref
+    assert (g > 0).any() and (g < 0).any()
+
+    # -- sampled beamlet rows (A3) on the GPU's own g
+    cnt_b = torch.bincount(ph.coo_beamlet.long(), minlength=n_b)
+    sb = np.unique(np.concatenate([rng.choice(n_b, 48, replace=False), [int(cnt_b.argmax()), 0, n_b - 1]]))
+    m = torch.isin(ph.coo_beamlet, torch.from_numpy(sb).to(DEV, torch.int32))
+    p_ref = oracle.price(ph.coo_voxel[m].cpu().numpy(), ph.coo_beamlet[m].cpu().numpy(), ph.coo_val[m].cpu().numpy(),
+                         n_b, g.astype(np.float64))[sb]
+    del m
+    assert np.abs(p[sb] - p_ref).max() <= 1e-4 * float(np.abs(p).max())
+    assert np.linalg.norm(p[sb] - p_ref) <= REL_L2 * np.linalg.norm(p_ref)
+
+    # -- adjoint identity on the GPU's vectors: <D x, g> = <x, D^T g>
+    lhs = float(np.dot(d.astype(np.float64), g.astype(np.float64)))
+    rhs = float(np.dot(x.numpy().astype(np.float64), p.astype(np.float64)))
+    scale = float(np.dot(np.abs(d).astype(np.float64), np.abs(g).astype(np.float64)))
+    assert abs(lhs - rhs) <= 1e-5 * scale
+
+    # -- A4 + A5 in full: the oracle's exhaustive selection on the GPU's FP32 p, bit for bit (C6 (ii))
+    L, R, rp = oracle.select_rows(p, A["lco"])
+    ap, best = oracle.angle_price(rp, A["aro"])
+    assert np.array_equal(out.L.cpu().numpy(), L) and np.array_equal(out.R.cpu().numpy(), R)
+    assert np.array_equal(out.row_price.cpu().numpy(), rp) and np.array_equal(out.angle_price.cpu().numpy(), ap)
+    assert int(out.best_angle.item()) == best
+    n_open = int((R > L).sum())
+    n_partial = int(((R - L) < np.diff(A["lco"])).sum())
+    print(f"  selection: {n_open} open rows of {L.size}, {n_partial} not fully open, best control point {best}")
+    assert n_open > 0 and n_partial > 0
+    h.close()
