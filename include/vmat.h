@@ -81,7 +81,9 @@ int vmat_ddc_destroy(vmat_ddc *h);
 int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info /* host, out */);
 
 /* Test/debug: copies one layout to host arrays.  which = 0: CSR(D) (rows = voxels, idx = beamlets),
- * which = 1: CSR(D^T) (rows = beamlets, idx = voxels).  ptr [rows+1], idx/val [nnz]. Synchronous. */
+ * which = 1: CSR(D^T) (rows = beamlets, idx = voxels).  ptr [rows+1], idx/val [nnz] in canonical CSR order
+ * (the tile interleave of the device layout is undone); idx = val = NULL copies the row pointers only.
+ * Synchronous. */
 int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx, float *val /* host, out */);
 
 /* Zero-copy, read-only view of one layout's device arrays (same `which` as above); the pointers stay

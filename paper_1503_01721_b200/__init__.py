@@ -174,6 +174,13 @@ class DDC:
         _check(load_library().vmat_ddc_device_csr(self._h, which, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
         return a.value, b.value, c.value
 
+    def export_ptr(self, which: int) -> torch.Tensor:
+        """Row pointers (int64 [rows+1], host) of CSR(D) (0) or CSR(D^T) (1)."""
+        rows = self.n_voxels if which == 0 else self.n_beamlets
+        ptr = torch.empty(rows + 1, dtype=torch.int64)
+        _check(load_library().vmat_ddc_export_csr(self._h, which, ptr.data_ptr(), None, None))
+        return ptr
+
     def export_csr(self, which: int):
         """(ptr int64 [rows+1], idx int32 [nnz], val float32 [nnz]) of CSR(D) (0) or CSR(D^T) (1), on the host."""
         rows = self.n_voxels if which == 0 else self.n_beamlets

@@ -162,15 +162,14 @@ int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info)
 
 int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx, float *val)
 {
-    REQUIRE(h && ptr && (h->nnz == 0 || (idx && val)), "NULL argument");
+    REQUIRE(h && ptr && ((idx == nullptr) == (val == nullptr)), "NULL argument");
     REQUIRE(which == 0 || which == 1, "which must be 0 (D) or 1 (D^T)");
     const CsrLayout &A = which == 0 ? h->D : h->Dt;
     VMAT_CUDA(cudaDeviceSynchronize());
     VMAT_CUDA(cudaMemcpy(ptr, A.ptr, ((size_t)A.n_rows + 1) * 8, cudaMemcpyDeviceToHost));
-    if (h->nnz > 0) {
-        VMAT_CUDA(cudaMemcpy(idx, A.idx, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost));
-        VMAT_CUDA(cudaMemcpy(val, A.val, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost));
-    }
+    if (idx == nullptr || h->nnz == 0) return VMAT_OK;       // row pointers only
+    VMAT_CUDA(cudaMemcpy(idx, A.idx, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost));
+    VMAT_CUDA(cudaMemcpy(val, A.val, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost));
     // undo the tile interleave (spmv.cuh): the caller gets canonical CSR order
     std::vector<int64_t> hp((size_t)A.n_rows + 1);
     memcpy(hp.data(), ptr, hp.size() * 8);

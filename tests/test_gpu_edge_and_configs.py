@@ -172,6 +172,17 @@ def test_config2_full(vm):
     _full_parity(vm, _phantom_on_gpu(2), [1.0])
 
 
+def _entries_with_key(key, n, sample):
+    """Positions of the COO entries whose `key` (int32 tensor on the GPU) is in `sample` - chunked lookup table."""
+    flag = torch.zeros(n, dtype=torch.bool, device=key.device)
+    flag[torch.from_numpy(sample).to(key.device, torch.int64)] = True
+    pos = []
+    CH = 1 << 28
+    for c0 in range(0, key.numel(), CH):
+        pos.append(torch.nonzero(flag[key[c0:c0 + CH].long()]).flatten() + c0)
+    return torch.cat(pos)
+
+
 def test_config3_full_size_sampled(vm):
     """Config 3 at full size (2.8e9 nnz, the workload and launch configuration bench.py times):
     sampled outputs the oracle computes one by one, the whole selection, and properties that hold at any size."""
@@ -184,18 +195,23 @@ def test_config3_full_size_sampled(vm):
              wu=ph.struct_w_under.numpy(), lco=ph.leafrow_col_offset.numpy(), aro=ph.angle_row_offset.numpy())
     obj = obj_to_device(A, DEV)
     out = h.alloc_outputs()
-    x = synth.draw_x(n_b, 7, scale=0.55)                       # near balance: mixed-sign prices
-    vmod.vmat_price_eval(h, x.to(DEV), obj, out)
-    torch.cuda.synchronize()
+    for scale in (0.55, 0.5, 0.47, 0.44, 0.41, 0.38):          # near balance: mixed-sign gradient and prices
+        x = synth.draw_x(n_b, 7, scale=scale)
+        vmod.vmat_price_eval(h, x.to(DEV), obj, out)
+        torch.cuda.synchronize()
+        if bool((out.p > 0).any()) and bool((out.p < 0).any()) and bool((out.g < 0).any()):
+            break
+    print(f"  x scale {scale}")
     d, g, p = out.d.cpu().numpy(), out.g.cpu().numpy(), out.p.cpu().numpy()
     assert h.info["nnz"] == ph.nnz > 2 ** 31                   # 64-bit offsets are exercised
 
     # -- sampled voxel rows (A1): longest row, empty rows, random rows
     rng = np.random.default_rng(33)
-    cnt_v = torch.bincount(ph.coo_voxel.long(), minlength=n_v)
+    ptrD = h.export_ptr(0)
+    cnt_v = (ptrD[1:] - ptrD[:-1]).to(DEV)
     sv = np.unique(np.concatenate([rng.choice(n_v, 48, replace=False), [int(cnt_v.argmax())],
                                    torch.nonzero(cnt_v == 0).flatten()[:4].cpu().numpy(), [0, n_v - 1]]))
-    m = torch.isin(ph.coo_voxel, torch.from_numpy(sv).to(DEV, torch.int32))
+    m = _entries_with_key(ph.coo_voxel, n_v, sv)
     d_ref = oracle.dose(ph.coo_voxel[m].cpu().numpy(), ph.coo_beamlet[m].cpu().numpy(), ph.coo_val[m].cpu().numpy(),
                         n_v, x.numpy())[sv]
     del m
@@ -212,9 +228,10 @@ def test_config3_full_size_sampled(vm):
     assert (g > 0).any() and (g < 0).any()
 
     # -- sampled beamlet rows (A3) on the GPU's own g
-    cnt_b = torch.bincount(ph.coo_beamlet.long(), minlength=n_b)
+    ptrT = h.export_ptr(1)
+    cnt_b = (ptrT[1:] - ptrT[:-1]).to(DEV)
     sb = np.unique(np.concatenate([rng.choice(n_b, 48, replace=False), [int(cnt_b.argmax()), 0, n_b - 1]]))
-    m = torch.isin(ph.coo_beamlet, torch.from_numpy(sb).to(DEV, torch.int32))
+    m = _entries_with_key(ph.coo_beamlet, n_b, sb)
     p_ref = oracle.price(ph.coo_voxel[m].cpu().numpy(), ph.coo_beamlet[m].cpu().numpy(), ph.coo_val[m].cpu().numpy(),
                          n_b, g.astype(np.float64))[sb]
     del m
