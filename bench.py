@@ -94,6 +94,28 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def ncu_traffic(kernel_prefix: str, cfg: int, scale: float):
+    """dram bytes (read + write) per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/r1_ncu_full_cfg3_v4.csv, config 3 only); None for other workloads."""
+    if cfg != 3 or scale != 1.0:
+        return None
+    try:
+        import csv
+        rows = list(csv.reader(open(os.path.join(ROOT, "profiles", "r1_ncu_full_cfg3_v4.csv"))))
+        hdr, units = rows[0], rows[1]
+        mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+        for r in rows[2:]:
+            if kernel_prefix in r[hdr.index("Kernel Name")]:
+                tot = 0.0
+                for col in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                    i = hdr.index(col)
+                    tot += float(r[i]) * mult[units[i]]
+                return tot
+    except Exception:
+        return None
+    return None
+
+
 def rank_eval_index(rank: int, k: int) -> int:
     """Fluence draw index of step k on `rank`: every replica prices its own sequence of x vectors."""
     return rank * 100000 + k
@@ -286,9 +308,9 @@ def run_ours(args):
         B_dose = 8 * nnz + 8 * (n_v + 1) + 4 * n_b + 4 * n_v + (1 * n_v + 4 * n_v)      # + struct id, g (fused A2)
         B_price = 8 * nnz + 8 * (n_b + 1) + 4 * n_v + 4 * n_b + 4 * (n_rows + 1) + 16 * n_rows
         B_eval = B_dose + B_price
-        k_dose = {"name": "k_dose<fused objective>", "ms": float(t_dose.mean()), "ms_min": float(t_dose.min()),
+        k_dose = {"name": "k_dose<true> (dose + fused objective/gradient)", "ncu": "k_dose<1>", "ms": float(t_dose.mean()), "ms_min": float(t_dose.min()),
                   "bytes": B_dose, "gbs": B_dose / (t_dose.mean() * 1e-3) / 1e9}
-        k_price = {"name": "k_price_select", "ms": float(t_price.mean()), "ms_min": float(t_price.min()),
+        k_price = {"name": "k_price<true> (price + fused leaf-row selection)", "ncu": "k_price<1>", "ms": float(t_price.mean()), "ms_min": float(t_price.min()),
                    "bytes": B_price, "gbs": B_price / (t_price.mean() * 1e-3) / 1e9}
         dom = k_price if k_price["ms"] >= k_dose["ms"] else k_dose
         agg = aggregate(world, K, elapsed_ms)
@@ -312,7 +334,8 @@ def run_ours(args):
             "gpu_launches": launches,
             "roofline": {"bound": "hbm", "kernel": dom["name"], "achieved": dom["gbs"], "peak": peak,
                          "unit": "GB/s", "frac": dom["gbs"] / peak, "frac_of_8TBs": dom["gbs"] / 8000.0,
-                         "peak_source": peak_src, "traffic": None, "algorithmic_bytes": dom["bytes"],
+                         "peak_source": peak_src, "traffic": ncu_traffic(dom["ncu"], args.config, args.scale),
+                         "traffic_source": "profiles/r1_ncu_full_cfg3_v4.csv (ncu --set full, one launch)", "algorithmic_bytes": dom["bytes"],
                          "ms": dom["ms"]},
             "kernels": [k_dose, k_price],
             "result_check": {"F_last": F_last, "best_angle_last": best_last},

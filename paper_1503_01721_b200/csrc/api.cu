@@ -130,8 +130,9 @@ int vmat_ddc_create(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int64_
         rc = upload(&h->beamlet_leafrow, bl.data(), (int64_t)n_beamlets, &h->bytes_device);
     }
     if (rc == VMAT_OK) {
-        const size_t b = (size_t)(n_rows > 0 ? n_rows : 1) * sizeof(uint32_t);
+        const size_t b = (size_t)(n_rows + 1) * sizeof(uint32_t);          // + 1: the aperture-price ticket
         cudaError_t e = cudaMalloc((void **)&h->leafrow_done, b);
+        h->angle_ticket = h->leafrow_done + n_rows;
         if (e != cudaSuccess) { vmat_set_error("vmat_ddc_create: cudaMalloc(leafrow_done) failed"); rc = VMAT_ERR_OOM; }
         else cudaMemsetAsync(h->leafrow_done, 0, b, st);
         h->bytes_device += (int64_t)b;

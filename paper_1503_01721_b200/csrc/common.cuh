@@ -58,6 +58,7 @@ struct vmat_ddc {
     double *F_partial_obj = nullptr;        // [n_obj_blocks]
     double *S_scratch = nullptr;            // [n_beamlets + n_leaf_rows + 1] prefix sums of the row selection
     int32_t *beamlet_leafrow = nullptr;     // [n_beamlets] leaf row of each beamlet
+    uint32_t *angle_ticket = nullptr;       // [1] ticket of the aperture-price kernel (self-resetting)
     uint32_t *leafrow_done = nullptr;       // [n_leaf_rows] tickets of the fused price+selection kernel (self-resetting)
     std::vector<int32_t> h_angle_row_offset; // host copy
     std::vector<int32_t> h_seg_row;          // host copy of seg_row (export un-permutes the tiles)
@@ -75,19 +76,22 @@ struct vmat_ddc {
 // ------------------------------------------------------------------ tuning constants
 // Dose kernel (CSR-stream): one CTA per row block; products staged in shared memory.
 #ifndef VMAT_DOSE_THREADS
-#define VMAT_DOSE_THREADS 256
+#define VMAT_DOSE_THREADS 128
 #endif
 #ifndef VMAT_DOSE_SEG_NNZ
 #define VMAT_DOSE_SEG_NNZ 512
 #endif
 #ifndef VMAT_DOSE_MINB
-#define VMAT_DOSE_MINB 6
+#define VMAT_DOSE_MINB 12
 #endif
 constexpr int DOSE_THREADS = VMAT_DOSE_THREADS;
 constexpr int DOSE_SEG_NNZ = VMAT_DOSE_SEG_NNZ;   // a warp's group of short rows holds at most this many non-zeros
 constexpr int DOSE_MAX_ROWS = 256;                // rows per segment (bounds runs of empty rows)
 // Price kernel (CSR-vector, one warp per beamlet row, L127).
-constexpr int PRICE_THREADS = 256;
+#ifndef VMAT_PRICE_THREADS
+#define VMAT_PRICE_THREADS 256
+#endif
+constexpr int PRICE_THREADS = VMAT_PRICE_THREADS;
 constexpr int PRICE_WARPS = PRICE_THREADS / 32;
 constexpr int SELECT_MAX_ROW = 2048;        // longest leaf row the fused price+select kernel takes
 

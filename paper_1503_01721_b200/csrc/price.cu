@@ -211,35 +211,57 @@ k_select(const float *__restrict__ p, const int32_t *__restrict__ leafrow_col_of
 }
 
 // ---------------------------------------------------------------- A5: aperture price per control point, best one
+// One warp per control point: the FP64 sum of its rows' prices IN ROW ORDER (lanes load 32 prices at a
+// time, every lane then adds them one by one - the same additions in the same order as the definition).
+// The CTA that draws the last ticket picks the best control point.
 constexpr int ANGLE_THREADS = 256;
 __global__ void __launch_bounds__(ANGLE_THREADS)
 k_angle_price(int n_angles, const int32_t *__restrict__ angle_row_offset, const double *__restrict__ row_price,
               const uint8_t *__restrict__ angle_mask, double *__restrict__ angle_price,
-              int32_t *__restrict__ best_angle)
+              int32_t *__restrict__ best_angle, uint32_t *__restrict__ ticket)
 {
     __shared__ double bv[ANGLE_THREADS / 32];
     __shared__ int bi[ANGLE_THREADS / 32];
-    double best = 0.0;           // only a strictly negative price improves F (L56)
-    int besta = -1;
-    for (int a = threadIdx.x; a < n_angles; a += ANGLE_THREADS) {
+    __shared__ int is_last;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int a = blockIdx.x * (ANGLE_THREADS / 32) + warp;
+    if (a < n_angles) {
         double s;
         if (angle_mask != nullptr && angle_mask[a] != 0) {
             s = __longlong_as_double(0x7ff0000000000000LL);          // +inf: occupied (C7)
         } else {
             s = 0.0;
-            for (int r = angle_row_offset[a]; r < angle_row_offset[a + 1]; ++r) s += row_price[r];   // row order
+            const int r1 = angle_row_offset[a + 1];
+            for (int base = angle_row_offset[a]; base < r1; base += 32) {
+                const double v = base + lane < r1 ? row_price[base + lane] : 0.0;
+                const int m = min(32, r1 - base);
+                for (int i = 0; i < m; ++i) s += __shfl_sync(0xffffffffu, v, i);   // row order
+            }
         }
-        angle_price[a] = s;
-        if (s < best) { best = s; besta = a; }                       // ascending a: strict < keeps the smallest a
+        if (lane == 0) angle_price[a] = s;
     }
-    // reduce (value, index): smaller value wins, ties -> smaller index; -1 means "none"
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        is_last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+        if (is_last) { *ticket = 0; __threadfence(); }
+    }
+    __syncthreads();
+    if (!is_last) return;
+    // arg-min over the unoccupied control points: smaller price wins, ties -> smaller index; -1 = none < 0 (L56)
+    double best = 0.0;
+    int besta = -1;
+    for (int k = threadIdx.x; k < n_angles; k += ANGLE_THREADS) {
+        const double v = __ldcg(angle_price + k);
+        if (v < best) { best = v; besta = k; }                       // ascending k: strict < keeps the smallest k
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         const double ov = __shfl_xor_sync(0xffffffffu, best, o);
         const int oa = __shfl_xor_sync(0xffffffffu, besta, o);
         if (oa >= 0 && (besta < 0 || ov < best || (ov == best && oa < besta))) { best = ov; besta = oa; }
     }
-    if ((threadIdx.x & 31) == 0) { bv[threadIdx.x >> 5] = best; bi[threadIdx.x >> 5] = besta; }
+    if (lane == 0) { bv[warp] = best; bi[warp] = besta; }
     __syncthreads();
     if (threadIdx.x == 0) {
         for (int i = 1; i < ANGLE_THREADS / 32; ++i)
@@ -288,8 +310,9 @@ int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *a
 int vmat_launch_angle_price(const vmat_ddc *h, const double *row_price, const uint8_t *angle_mask,
                             double *angle_price, int32_t *best_angle, cudaStream_t st)
 {
-    k_angle_price<<<1, ANGLE_THREADS, 0, st>>>(h->n_angles, h->angle_row_offset, row_price, angle_mask,
-                                               angle_price, best_angle);
+    const int grid = h->n_angles > 0 ? (h->n_angles + ANGLE_THREADS / 32 - 1) / (ANGLE_THREADS / 32) : 1;
+    k_angle_price<<<grid, ANGLE_THREADS, 0, st>>>(h->n_angles, h->angle_row_offset, row_price, angle_mask,
+                                                  angle_price, best_angle, h->angle_ticket);
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }
