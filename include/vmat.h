@@ -21,8 +21,10 @@
  *     vmat_last_error() gives a thread-local message for the last failure.
  *   - Results are deterministic run to run: canonical storage order, fixed reduction order,
  *     no floating-point atomics anywhere.
- *   - Values are FP32, indices int32, nnz and row pointers int64 (Table 2,
- *     L198-L202: 12 B/nnz COO, 8 B/nnz CSR).
+ *   - Values are FP32, indices int32, nnz and row pointers int64 at the boundary (Table 2,
+ *     L198-L202: 12 B/nnz COO, 8 B/nnz CSR).  Inside the handle a layout stores its secondary indices
+ *     either as int32 (8 B per entry, the paper's format) or as a u16 offset from a per-32-entry base
+ *     (6.125 B per entry); see vmat_ddc_create_ex.
  */
 #ifndef VMAT_H
 #define VMAT_H
@@ -49,12 +51,17 @@ typedef struct vmat_ddc vmat_ddc;
 
 typedef struct vmat_ddc_info {
     int64_t n_voxels, n_beamlets, nnz, n_angles, n_leaf_rows;
-    int64_t bytes_csr_d;        /* 8*nnz + 8*(n_voxels+1)   (values + indices + int64 row pointers) */
-    int64_t bytes_csr_dt;       /* 8*nnz + 8*(n_beamlets+1)                                         */
-    int64_t bytes_device_total; /* everything the handle holds on the device                        */
-    int64_t n_dose_blocks;      /* segments (one warp each) of the dose kernel                      */
-    int64_t max_leaf_row_len;   /* longest leaf row, in beamlets                                    */
+    int64_t bytes_csr_d;        /* 8*nnz + 8*(n_voxels+1): plain CSR(D) in the paper's format (Table 2)  */
+    int64_t bytes_csr_dt;       /* 8*nnz + 8*(n_beamlets+1)                                             */
+    int64_t bytes_device_total; /* everything the handle holds on the device                            */
+    int64_t n_dose_blocks;      /* segments (one warp each) of the dose kernel                          */
+    int64_t max_leaf_row_len;   /* longest leaf row, in beamlets                                        */
     int64_t max_voxel_row_nnz, max_beamlet_row_nnz;
+    int64_t index_bits_d, index_bits_dt;     /* 16 or 32: index encoding chosen for each layout          */
+    int64_t padded_d, padded_dt;             /* stored entries incl. pads (multiples of 32), >= nnz      */
+    int64_t bytes_stream_d;     /* bytes vmat_dose streams per call: values + indices (+ bases) of the
+                                   padded entries + int64 row starts + the int32 segment table           */
+    int64_t bytes_stream_dt;    /* bytes vmat_price streams per call: the same for D^T (no segment table) */
 } vmat_ddc_info;
 
 /* A0 ingest / layout build (D arrives as COO - values, voxel (row) index,
@@ -75,6 +82,21 @@ int vmat_ddc_create(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int64_
                     int32_t n_angles, const int32_t *angle_col_offset, const int32_t *angle_row_offset,
                     const int32_t *leafrow_col_offset, void *stream);
 
+/* Same, with the index encoding of the two layouts chosen by the caller:
+ *   index_bits = 32  int32 secondary indices, 8 B per stored entry (the paper's CSR, Table 2);
+ *   index_bits = 16  u16 offsets from one int32 base per group of 32 stored entries, 6.125 B per entry; a
+ *                    group whose indices would span more than 65535 is closed early and padded, so any
+ *                    matrix can be stored;
+ *   index_bits = 0   per layout, 16 if that is at least 5 % smaller than 32, else 32 (what
+ *                    vmat_ddc_create does).
+ * Results are deterministic for a given setting.  Across settings they are bit-identical whenever no group
+ * had to be closed early (always when the layout's secondary dimension is <= 65536); otherwise the pads
+ * shift entries between the lanes' partial sums and the FP32 results differ by summation order only. */
+int vmat_ddc_create_ex(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int64_t nnz,
+                       const int32_t *coo_voxel, const int32_t *coo_beamlet, const float *coo_val,
+                       int32_t n_angles, const int32_t *angle_col_offset, const int32_t *angle_row_offset,
+                       const int32_t *leafrow_col_offset, int32_t index_bits, void *stream);
+
 /* Frees the layouts and scratch.  NULL is a no-op. */
 int vmat_ddc_destroy(vmat_ddc *h);
 
@@ -82,14 +104,9 @@ int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info /* host, out */);
 
 /* Test/debug: copies one layout to host arrays.  which = 0: CSR(D) (rows = voxels, idx = beamlets),
  * which = 1: CSR(D^T) (rows = beamlets, idx = voxels).  ptr [rows+1], idx/val [nnz] in canonical CSR order
- * (the tile interleave of the device layout is undone); idx = val = NULL copies the row pointers only.
+ * (the grouping, padding, tile interleave and index encoding of the device layout are undone); idx = val = NULL copies the row pointers only.
  * Synchronous. */
 int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx, float *val /* host, out */);
-
-/* Zero-copy, read-only view of one layout's device arrays (same `which` as above); the pointers stay
- * owned by the handle and valid until vmat_ddc_destroy.  Any of the three outputs may be NULL. */
-int vmat_ddc_device_csr(const vmat_ddc *h, int which, const int64_t **ptr, const int32_t **idx,
-                        const float **val /* host, out: device pointers */);
 
 /* A1 forward dose d = D x, d_i = sum_j D_ij x_j ("repeated forward dose
  * calculation", L27).  x dev [n_beamlets] in, d dev [n_voxels] out. */

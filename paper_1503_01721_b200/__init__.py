@@ -27,7 +27,7 @@ STATUS_NAMES = {0: "VMAT_OK", -1: "VMAT_ERR_INVALID_ARG", -2: "VMAT_ERR_INDEX_RA
                 -4: "VMAT_ERR_OOM", -5: "VMAT_ERR_CUDA", -6: "VMAT_ERR_NONFINITE"}
 
 EXPORTS = [
-    "vmat_ddc_create", "vmat_ddc_destroy", "vmat_ddc_info_get", "vmat_ddc_export_csr", "vmat_ddc_device_csr", "vmat_dose",
+    "vmat_ddc_create", "vmat_ddc_create_ex", "vmat_ddc_destroy", "vmat_ddc_info_get", "vmat_ddc_export_csr", "vmat_dose",
     "vmat_objective_grad", "vmat_price", "vmat_select_apertures", "vmat_price_eval", "vmat_price_eval_host",
     "vmat_aperture_dose", "vmat_ddc_set_profile_events", "vmat_last_error", "vmat_last_launch_count",
 ]
@@ -42,7 +42,8 @@ class VmatError(RuntimeError):
 class _Info(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int64) for n in (
         "n_voxels", "n_beamlets", "nnz", "n_angles", "n_leaf_rows", "bytes_csr_d", "bytes_csr_dt",
-        "bytes_device_total", "n_dose_blocks", "max_leaf_row_len", "max_voxel_row_nnz", "max_beamlet_row_nnz")]
+        "bytes_device_total", "n_dose_blocks", "max_leaf_row_len", "max_voxel_row_nnz", "max_beamlet_row_nnz",
+        "index_bits_d", "index_bits_dt", "padded_d", "padded_dt", "bytes_stream_d", "bytes_stream_dt")]
 
 
 def load_library():
@@ -59,7 +60,7 @@ def load_library():
     lib.vmat_ddc_destroy.argtypes = [vp]
     lib.vmat_ddc_info_get.argtypes = [vp, ctypes.POINTER(_Info)]
     lib.vmat_ddc_export_csr.argtypes = [vp, ctypes.c_int, vp, vp, vp]
-    lib.vmat_ddc_device_csr.argtypes = [vp, ctypes.c_int, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(vp)]
+    lib.vmat_ddc_create_ex.argtypes = [ctypes.POINTER(vp), i32, i32, i64, vp, vp, vp, i32, vp, vp, vp, i32, vp]
     lib.vmat_dose.argtypes = [vp, vp, vp, vp]
     lib.vmat_objective_grad.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp]
     lib.vmat_price.argtypes = [vp, vp, vp, vp]
@@ -168,12 +169,6 @@ class DDC:
         arr = (ctypes.c_void_p * 4)(*[e.cuda_event for e in events])
         _check(load_library().vmat_ddc_set_profile_events(self._h, arr))
 
-    def device_csr(self, which: int):
-        """Raw device pointers (ptr, idx, val) of a layout, owned by the handle (zero-copy view)."""
-        a, b, c = ctypes.c_void_p(), ctypes.c_void_p(), ctypes.c_void_p()
-        _check(load_library().vmat_ddc_device_csr(self._h, which, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
-        return a.value, b.value, c.value
-
     def export_ptr(self, which: int) -> torch.Tensor:
         """Row pointers (int64 [rows+1], host) of CSR(D) (0) or CSR(D^T) (1)."""
         rows = self.n_voxels if which == 0 else self.n_beamlets
@@ -193,8 +188,9 @@ class DDC:
 
 def vmat_ddc_create(n_voxels: int, n_beamlets: int, coo_voxel: torch.Tensor, coo_beamlet: torch.Tensor,
                     coo_val: torch.Tensor, angle_col_offset: torch.Tensor, angle_row_offset: torch.Tensor,
-                    leafrow_col_offset: torch.Tensor, device=None) -> DDC:
-    """A0: build both layouts from COO triplets (host or device tensors)."""
+                    leafrow_col_offset: torch.Tensor, device=None, index_bits: int = 0) -> DDC:
+    """A0: build both layouts from COO triplets (host or device tensors).
+    index_bits = 0 calls vmat_ddc_create (encoding chosen per layout); 16 or 32 call vmat_ddc_create_ex."""
     lib = load_library()
     if not torch.cuda.is_available():
         raise RuntimeError("vmat_ddc_create needs a CUDA device (there is no CPU fallback)")
@@ -210,10 +206,13 @@ def vmat_ddc_create(n_voxels: int, n_beamlets: int, coo_voxel: torch.Tensor, coo
         raise ValueError("leafrow_col_offset must have n_leaf_rows+1 entries")
     out = ctypes.c_void_p()
     with torch.cuda.device(dev):
-        rc = lib.vmat_ddc_create(ctypes.byref(out), n_voxels, n_beamlets, nnz,
-                                 _ptr(coo_voxel, torch.int32), _ptr(coo_beamlet, torch.int32),
-                                 _ptr(coo_val, torch.float32), n_angles,
-                                 offs[0].data_ptr(), offs[1].data_ptr(), offs[2].data_ptr(), _stream())
+        args = (ctypes.byref(out), n_voxels, n_beamlets, nnz,
+                _ptr(coo_voxel, torch.int32), _ptr(coo_beamlet, torch.int32), _ptr(coo_val, torch.float32),
+                n_angles, offs[0].data_ptr(), offs[1].data_ptr(), offs[2].data_ptr())
+        if index_bits == 0:
+            rc = lib.vmat_ddc_create(*args, _stream())
+        else:
+            rc = lib.vmat_ddc_create_ex(*args, int(index_bits), _stream())
     _check(rc)
     return DDC(out.value, dev)
 

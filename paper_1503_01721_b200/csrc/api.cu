@@ -63,7 +63,8 @@ int vmat_last_launch_count(void) { return g_vmat_launches; }
 int vmat_ddc_destroy(vmat_ddc *h)
 {
     if (!h) return VMAT_OK;
-    void *ptrs[] = {h->D.ptr, h->D.idx, h->D.val, h->Dt.ptr, h->Dt.idx, h->Dt.val, h->angle_col_offset,
+    void *ptrs[] = {h->D.ptr, h->D.pptr, h->D.val, h->D.sec, h->D.base, h->Dt.ptr, h->Dt.pptr, h->Dt.val, h->Dt.sec,
+                    h->Dt.base, h->angle_col_offset,
                     h->angle_row_offset, h->leafrow_col_offset, h->leafrow_angle, h->seg_row, h->F_partial,
                     h->F_partial_obj, h->S_scratch, h->beamlet_leafrow, h->leafrow_done, h->e2e_x, h->e2e_d, h->e2e_g, h->e2e_p, h->e2e_L, h->e2e_R,
                     h->e2e_best, h->e2e_row_price, h->e2e_angle_price, h->e2e_F};
@@ -78,7 +79,17 @@ int vmat_ddc_create(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int64_
                     int32_t n_angles, const int32_t *angle_col_offset, const int32_t *angle_row_offset,
                     const int32_t *leafrow_col_offset, void *stream)
 {
+    return vmat_ddc_create_ex(out, n_voxels, n_beamlets, nnz, coo_voxel, coo_beamlet, coo_val, n_angles,
+                              angle_col_offset, angle_row_offset, leafrow_col_offset, 0, stream);
+}
+
+int vmat_ddc_create_ex(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int64_t nnz,
+                       const int32_t *coo_voxel, const int32_t *coo_beamlet, const float *coo_val,
+                       int32_t n_angles, const int32_t *angle_col_offset, const int32_t *angle_row_offset,
+                       const int32_t *leafrow_col_offset, int32_t index_bits, void *stream)
+{
     REQUIRE(out != nullptr, "out is NULL");
+    REQUIRE(index_bits == 0 || index_bits == 16 || index_bits == 32, "index_bits must be 0 (auto), 16 or 32");
     REQUIRE(n_voxels >= 0 && n_beamlets >= 0 && nnz >= 0 && n_angles >= 0, "negative size");
     REQUIRE(nnz == 0 || (coo_voxel && coo_beamlet && coo_val), "COO pointer is NULL");
     REQUIRE(nnz == 0 || (n_voxels > 0 && n_beamlets > 0), "nnz > 0 with an empty dimension");
@@ -112,7 +123,7 @@ int vmat_ddc_create(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int64_
     cudaGetDevice(&h->device);
     h->h_angle_row_offset.assign(angle_row_offset, angle_row_offset + n_angles + 1);
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = vmat_build_layouts(h, coo_voxel, coo_beamlet, coo_val, st);
+    int rc = vmat_build_layouts(h, coo_voxel, coo_beamlet, coo_val, index_bits, st);
     if (rc == VMAT_OK) rc = upload(&h->angle_col_offset, angle_col_offset, (int64_t)n_angles + 1, &h->bytes_device);
     if (rc == VMAT_OK) rc = upload(&h->angle_row_offset, angle_row_offset, (int64_t)n_angles + 1, &h->bytes_device);
     if (rc == VMAT_OK) rc = upload(&h->leafrow_col_offset, leafrow_col_offset, (int64_t)n_rows + 1, &h->bytes_device);
@@ -158,6 +169,10 @@ int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info)
     info->max_leaf_row_len = h->max_leaf_row_len;
     info->max_voxel_row_nnz = h->max_voxel_row_nnz;
     info->max_beamlet_row_nnz = h->max_beamlet_row_nnz;
+    info->index_bits_d = h->D.index_bits; info->index_bits_dt = h->Dt.index_bits;
+    info->padded_d = h->D.P; info->padded_dt = h->Dt.P;
+    info->bytes_stream_d = h->D.bytes() + 4 * ((int64_t)h->n_seg + 1);      // + the segment table
+    info->bytes_stream_dt = h->Dt.bytes();
     return VMAT_OK;
 }
 
@@ -165,42 +180,43 @@ int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx
 {
     REQUIRE(h && ptr && ((idx == nullptr) == (val == nullptr)), "NULL argument");
     REQUIRE(which == 0 || which == 1, "which must be 0 (D) or 1 (D^T)");
-    const CsrLayout &A = which == 0 ? h->D : h->Dt;
+    const PackedLayout &A = which == 0 ? h->D : h->Dt;
     VMAT_CUDA(cudaDeviceSynchronize());
     VMAT_CUDA(cudaMemcpy(ptr, A.ptr, ((size_t)A.n_rows + 1) * 8, cudaMemcpyDeviceToHost));
     if (idx == nullptr || h->nnz == 0) return VMAT_OK;       // row pointers only
-    VMAT_CUDA(cudaMemcpy(idx, A.idx, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost));
-    VMAT_CUDA(cudaMemcpy(val, A.val, (size_t)h->nnz * 4, cudaMemcpyDeviceToHost));
-    // undo the tile interleave (spmv.cuh): the caller gets canonical CSR order
-    std::vector<int64_t> hp((size_t)A.n_rows + 1);
-    memcpy(hp.data(), ptr, hp.size() * 8);
+    // Unpack the grouped layout (spmv.cuh) on the host: undo the tile interleave, add the group bases,
+    // drop the pads.  Within a row the real entries ascend strictly and a pad repeats the index before it.
+    const bool narrow = A.index_bits == 16;
+    std::vector<int64_t> pp((size_t)A.n_rows + 1);
+    std::vector<float> pv((size_t)A.P);
+    std::vector<int32_t> pi32(narrow ? 0 : (size_t)A.P), pbase(narrow ? (size_t)(A.P / GROUP) : 0);
+    std::vector<uint16_t> pi16(narrow ? (size_t)A.P : 0);
+    VMAT_CUDA(cudaMemcpy(pp.data(), A.pptr, pp.size() * 8, cudaMemcpyDeviceToHost));
+    VMAT_CUDA(cudaMemcpy(pv.data(), A.val, pv.size() * 4, cudaMemcpyDeviceToHost));
+    if (narrow) {
+        VMAT_CUDA(cudaMemcpy(pi16.data(), A.sec, pi16.size() * 2, cudaMemcpyDeviceToHost));
+        VMAT_CUDA(cudaMemcpy(pbase.data(), A.base, pbase.size() * 4, cudaMemcpyDeviceToHost));
+    } else {
+        VMAT_CUDA(cudaMemcpy(pi32.data(), A.sec, pi32.size() * 4, cudaMemcpyDeviceToHost));
+    }
     const int64_t n_seg = which == 0 ? (int64_t)h->n_seg : (int64_t)A.n_rows;
-    int32_t ti_[TILE];
-    float tv_[TILE];
     for (int64_t w = 0; w < n_seg; ++w) {
-        const int64_t s = which == 0 ? hp[h->h_seg_row[w]] : hp[w];
-        const int64_t e = which == 0 ? hp[h->h_seg_row[w + 1]] : hp[w + 1];
-        const Segment sg = segment_of(s, e);
-        for (int64_t t = 0; t < sg.nt; ++t) {
-            int32_t *pi = idx + sg.a0 + t * TILE;
-            float *pv = val + sg.a0 + t * TILE;
-            for (int l = 0; l < 32; ++l)
-                for (int u = 0; u < 8; ++u) { ti_[32 * u + l] = pi[8 * l + u]; tv_[32 * u + l] = pv[8 * l + u]; }
-            memcpy(pi, ti_, sizeof(ti_));
-            memcpy(pv, tv_, sizeof(tv_));
+        const int32_t r0 = which == 0 ? h->h_seg_row[w] : (int32_t)w;
+        const int32_t r1 = which == 0 ? h->h_seg_row[w + 1] : (int32_t)w + 1;
+        const int64_t S = pp[r0], G = (pp[r1] - S) / GROUP;
+        for (int32_t r = r0; r < r1; ++r) {
+            int64_t o = ptr[r];
+            int32_t prev = -1;
+            for (int64_t q = pp[r]; q < pp[r + 1]; ++q) {
+                const int64_t sp = stored_pos(S, G, q);
+                const int32_t c = narrow ? pbase[q >> 5] + (int32_t)pi16[sp] : pi32[sp];
+                if (c <= prev) continue;                              // a pad
+                if (o >= ptr[r + 1]) { vmat_set_error("vmat_ddc_export_csr: layout inconsistent (row %d)", r); return VMAT_ERR_CUDA; }
+                idx[o] = c; val[o] = pv[sp]; prev = c; ++o;
+            }
+            if (o != ptr[r + 1]) { vmat_set_error("vmat_ddc_export_csr: layout inconsistent (row %d)", r); return VMAT_ERR_CUDA; }
         }
     }
-    return VMAT_OK;
-}
-
-int vmat_ddc_device_csr(const vmat_ddc *h, int which, const int64_t **ptr, const int32_t **idx, const float **val)
-{
-    REQUIRE(h != nullptr, "handle is NULL");
-    REQUIRE(which == 0 || which == 1, "which must be 0 (D) or 1 (D^T)");
-    const CsrLayout &A = which == 0 ? h->D : h->Dt;
-    if (ptr) *ptr = A.ptr;
-    if (idx) *idx = A.idx;
-    if (val) *val = A.val;
     return VMAT_OK;
 }
 

@@ -29,21 +29,43 @@ extern thread_local int g_vmat_launches;
         }                                                                                   \
     } while (0)
 
-// ------------------------------------------------------------------ one CSR layout on the device
-struct CsrLayout {
+// ------------------------------------------------------------------ one matrix layout on the device
+// A layout is a PADDED, GROUPED CSR (spmv.cuh): the rows are cut into segments (one warp each), every
+// segment starts at a multiple of 32 padded positions and is a whole number of 32-entry groups.
+//   narrow (index_bits 16): val f32[P], off u16[P], base i32[P/32]: secondary index = base[group] + off
+//   wide   (index_bits 32): val f32[P], idx i32[P]                 (the paper's 8 B/nnz format, Table 2)
+// ptr holds the canonical (unpadded) row pointers, pptr the padded position of each row's first entry.
+struct PackedLayout {
     int32_t n_rows = 0;
-    int64_t nnz = 0;
-    int64_t *ptr = nullptr;   // [n_rows+1]
-    int32_t *idx = nullptr;   // [nnz (+pad)]  secondary index, ascending within a row
-    float   *val = nullptr;   // [nnz (+pad)]
+    int64_t nnz = 0;          // real entries
+    int64_t P = 0;            // padded entries (multiple of 32)
+    int index_bits = 32;      // 16 or 32
+    int64_t *ptr = nullptr;   // [n_rows+1] canonical row pointers
+    int64_t *pptr = nullptr;  // [n_rows+1] padded row starts; pptr[n_rows] = P
+    float *val = nullptr;     // [P (+pad)]
+    void *sec = nullptr;      // narrow: uint16_t off[P (+pad)];  wide: int32_t idx[P (+pad)]
+    int32_t *base = nullptr;  // narrow: [P/32 (+pad)];           wide: unused (NULL)
+    int64_t bytes() const     // device bytes of the streams a product reads (values + indices + padded row starts)
+    {
+        return index_bits == 16 ? 6 * P + 4 * (P / 32) + 8 * ((int64_t)n_rows + 1)
+                                : 8 * P + 8 * ((int64_t)n_rows + 1);
+    }
 };
+
+// Device view handed to the kernels.
+struct MatView {
+    const float *val;
+    const void *sec;
+    const int32_t *base;
+};
+static inline MatView view_of(const PackedLayout &A) { return MatView{A.val, A.sec, A.base}; }
 
 // ------------------------------------------------------------------ the handle
 struct vmat_ddc {
     int32_t n_voxels = 0, n_beamlets = 0, n_angles = 0, n_leaf_rows = 0;
     int64_t nnz = 0;
-    CsrLayout D;    // rows = voxels,   idx = beamlet   (for d = D x)
-    CsrLayout Dt;   // rows = beamlets, idx = voxel     (for p = D^T g; the paper's format, L121)
+    PackedLayout D;    // rows = voxels,   secondary index = beamlet   (for d = D x)
+    PackedLayout Dt;   // rows = beamlets, secondary index = voxel     (for p = D^T g; the paper's format, L121)
     // offset tables (device)
     int32_t *angle_col_offset = nullptr;    // [n_angles+1]
     int32_t *angle_row_offset = nullptr;    // [n_angles+1]
@@ -61,7 +83,7 @@ struct vmat_ddc {
     uint32_t *angle_ticket = nullptr;       // [1] ticket of the aperture-price kernel (self-resetting)
     uint32_t *leafrow_done = nullptr;       // [n_leaf_rows] tickets of the fused price+selection kernel (self-resetting)
     std::vector<int32_t> h_angle_row_offset; // host copy
-    std::vector<int32_t> h_seg_row;          // host copy of seg_row (export un-permutes the tiles)
+    std::vector<int32_t> h_seg_row;          // host copy of seg_row (export undoes the tile interleave)
     int32_t max_leaf_row_len = 0;
     int64_t max_voxel_row_nnz = 0, max_beamlet_row_nnz = 0;
     int64_t bytes_device = 0;
@@ -74,7 +96,7 @@ struct vmat_ddc {
 };
 
 // ------------------------------------------------------------------ tuning constants
-// Dose kernel (CSR-stream): one CTA per row block; products staged in shared memory.
+// Dose kernel: one warp per segment (a long voxel row, or a run of short rows parked in shared memory).
 #ifndef VMAT_DOSE_THREADS
 #define VMAT_DOSE_THREADS 128
 #endif
@@ -85,7 +107,7 @@ struct vmat_ddc {
 #define VMAT_DOSE_MINB 12
 #endif
 constexpr int DOSE_THREADS = VMAT_DOSE_THREADS;
-constexpr int DOSE_SEG_NNZ = VMAT_DOSE_SEG_NNZ;   // a warp's group of short rows holds at most this many non-zeros
+constexpr int DOSE_SEG_NNZ = VMAT_DOSE_SEG_NNZ;   // a warp's run of short rows holds at most this many padded entries
 constexpr int DOSE_MAX_ROWS = 256;                // rows per segment (bounds runs of empty rows)
 // Price kernel (CSR-vector, one warp per beamlet row, L127).
 #ifndef VMAT_PRICE_THREADS
@@ -109,6 +131,24 @@ __device__ __forceinline__ Vec8 ld_stream_256(const void *p)
                    "=r"(r.w[4]), "=r"(r.w[5]), "=r"(r.w[6]), "=r"(r.w[7]) : "l"(p));
     return r;
 }
+// 128-bit stream load (eight u16 offsets).  The .L2::evict_first qualifier exists only for .v8.b32, so the
+// same priority is given through a cache-hint policy.
+struct Vec4 { uint32_t w[4]; };
+__device__ __forceinline__ Vec4 ld_stream_128(const void *p)
+{
+    Vec4 r;
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.b32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(r.w[0]), "=r"(r.w[1]), "=r"(r.w[2]), "=r"(r.w[3]) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ int ld_stream_u16(const uint16_t *p)
+{
+    unsigned short r;
+    asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(r) : "l"(p));
+    return (int)r;
+}
 __device__ __forceinline__ float ld_stream_f(const float *p)
 {
     float r;
@@ -131,7 +171,7 @@ __device__ __forceinline__ float ld_gather(const float *p)
 
 // ------------------------------------------------------------------ internal entry points
 int vmat_build_layouts(vmat_ddc *h, const int32_t *coo_voxel, const int32_t *coo_beamlet,
-                       const float *coo_val, cudaStream_t st);
+                       const float *coo_val, int index_bits, cudaStream_t st);
 int vmat_launch_dose(const vmat_ddc *h, const float *x, float *d, bool fuse,
                      const uint8_t *voxel_struct, int32_t n_struct, const float *T, const float *w_over,
                      const float *w_under, float *g, double *F, cudaStream_t st);

@@ -2,13 +2,14 @@
 // objective / gradient (Eq. (1), Eq. (4)) fused into the row epilogue (A2).
 //
 // Voxel rows are ragged (0 ... ~18 k non-zeros, mean 10^2-10^3).  The ingest step cuts the row range
-// into SEGMENTS, each owned by one warp (8 consecutive segments per CTA, so neighbouring voxels - which
+// into SEGMENTS, each owned by one warp (consecutive segments per CTA, so neighbouring voxels - which
 // see nearly the same beamlets - share the x sectors cached in L1):
-//   long row   (> DOSE_SEG_NNZ non-zeros)  a segment of its own: the warp streams the row's interleaved
-//              tiles with 256-bit loads and accumulates in registers, as the price kernel does;
-//   short rows (consecutive rows, <= DOSE_SEG_NNZ non-zeros together)  the warp streams the contiguous
+//   long row   (> DOSE_SEG_NNZ padded entries)  a segment of its own: the warp streams the row's
+//              interleaved tiles with 256-bit loads and accumulates in registers, as the price kernel does;
+//   short rows (consecutive rows, <= DOSE_SEG_NNZ padded entries together)  the warp streams the contiguous
 //              range once, parks the products in its private slice of shared memory, then groups of
-//              G lanes (G sized to the segment's mean row length) reduce one row each with shuffles.
+//              G lanes (G sized to the segment's mean row length) reduce one row each with shuffles
+//              (pads hold 0 and belong to the row before them, so they change no sum).
 // No block-wide barrier sits in the hot path (the first version, one CTA per 4096-entry block, lost
 // 21 % of its issue slots to barrier stalls - profiles/).  Everything is FP32 with a fixed summation
 // order; the objective partials are FP64, one per CTA, summed afterwards in a fixed order (no atomics).
@@ -37,10 +38,10 @@ __device__ __forceinline__ double block_sum_double(double v, double *red /* [NT/
     return s;
 }
 
-template <bool FUSE>
+template <bool FUSE, bool NARROW>
 __global__ void __launch_bounds__(DOSE_THREADS, VMAT_DOSE_MINB)
-k_dose(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const float *__restrict__ val,
-       const int32_t *__restrict__ seg_row, int n_seg, const float *__restrict__ x, float *__restrict__ d,
+k_dose(const int64_t *__restrict__ pptr, const MatView A, const int32_t *__restrict__ seg_row, int n_seg,
+       const float *__restrict__ x, float *__restrict__ d,
        const uint8_t *__restrict__ vstruct, const float *__restrict__ T,
        const float *__restrict__ w_over, const float *__restrict__ w_under, float *__restrict__ g,
        double *__restrict__ F_partial)
@@ -60,29 +61,28 @@ k_dose(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const f
     if (sgi < n_seg) {
         const int r0 = seg_row[sgi], r1 = seg_row[sgi + 1];
         const int nr = r1 - r0;
-        const int64_t s = ptr[r0], e = ptr[r1];
-        const Segment sg = segment_of(s, e);
+        const int64_t s = pptr[r0], e = pptr[r1];               // padded positions, multiples of 32
         if (nr == 1) {
             // ---- one row: register accumulation
-            float acc = 0.f;
-#pragma unroll 1
-            for (int64_t ti = 0; ti < sg.nt; ++ti) acc += tile_dot(val, idx, sg.a0 + ti * TILE, x, lane);
-            plain_foreach<32>(val, idx, s, sg, e, x, lane, [&](int64_t, float q) { acc += q; });
-            acc = warp_sum(acc);
+            const float acc = warp_sum(segment_dot<NARROW>(A, s, e, x, lane));
             if (lane == 0) epilogue(r0, acc);
         } else {
-            // ---- several short rows: products into this warp's slice at their logical position k - s ...
+            // ---- several short rows: products into this warp's slice at their padded position k - s ...
             float *wp = prod[warp];
+            const int nt = (int)((e - s) >> 8);
 #pragma unroll 1
-            for (int64_t ti = 0; ti < sg.nt; ++ti) {
-                const int64_t k = sg.a0 + ti * TILE;
-                const Vec8 v = ld_stream_256(val + k + lane * 8);
-                const Vec8 c = ld_stream_256(idx + k + lane * 8);
-                float *dst = wp + (k - s) + lane;
+            for (int ti = 0; ti < nt; ++ti) {
+                const int64_t k = s + (int64_t)ti * TILE;
+                const Vec8 v = ld_stream_256(A.val + k + lane * 8);
+                int c[8];
+                tile_indices<NARROW>(A, k, lane, c);
+                float *dst = wp + ti * TILE + lane;
 #pragma unroll
-                for (int t = 0; t < 8; ++t) dst[32 * t] = __uint_as_float(v.w[t]) * ld_gather(x + c.w[t]);
+                for (int t = 0; t < 8; ++t) dst[32 * t] = __uint_as_float(v.w[t]) * ld_gather(x + c[t]);
             }
-            plain_foreach<32>(val, idx, s, sg, e, x, lane, [&](int64_t k, float q) { wp[k - s] = q; });
+            const int64_t k0 = s + (int64_t)nt * TILE;
+            float *dst = wp + nt * TILE + lane;
+            tail_foreach<NARROW>(A, k0, (int)((e - k0) >> 5), x, lane, [&](int t, float q) { dst[32 * t] = q; });
             __syncwarp();
             // ... then G lanes per row, G = power of two near (mean row length)/4, 1..32
             const int mean = (int)((e - s) / nr);
@@ -94,7 +94,7 @@ k_dose(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const f
                 const int r = r0 + grp + it * n_grp;
                 float acc = 0.f;
                 if (r < r1) {
-                    const int b = (int)(ptr[r] - s), f = (int)(ptr[r + 1] - s);
+                    const int b = (int)(pptr[r] - s), f = (int)(pptr[r + 1] - s);
                     for (int k = b + gl; k < f; k += G) acc += wp[k];
                 }
                 for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
@@ -144,12 +144,15 @@ int vmat_launch_dose(const vmat_ddc *h, const float *x, float *d, bool fuse,
 {
     if (fuse && h->prof_ev[0]) VMAT_CUDA(cudaEventRecord(h->prof_ev[0], st));
     if (h->n_blocks > 0) {
-        if (fuse)
-            k_dose<true><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.ptr, h->D.idx, h->D.val, h->seg_row, h->n_seg, x, d,
-                                                               voxel_struct, T, w_over, w_under, g, h->F_partial);
-        else
-            k_dose<false><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.ptr, h->D.idx, h->D.val, h->seg_row, h->n_seg, x, d,
-                                                                nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+        const MatView A = view_of(h->D);
+        const bool narrow = h->D.index_bits == 16;
+#define VMAT_DOSE_LAUNCH(FUSE_, NARROW_, ...)                                                           \
+        k_dose<FUSE_, NARROW_><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.pptr, A, h->seg_row, h->n_seg, x, d, __VA_ARGS__)
+        if (fuse && narrow)       VMAT_DOSE_LAUNCH(true, true, voxel_struct, T, w_over, w_under, g, h->F_partial);
+        else if (fuse)            VMAT_DOSE_LAUNCH(true, false, voxel_struct, T, w_over, w_under, g, h->F_partial);
+        else if (narrow)          VMAT_DOSE_LAUNCH(false, true, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+        else                      VMAT_DOSE_LAUNCH(false, false, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+#undef VMAT_DOSE_LAUNCH
         VMAT_LAUNCH_CHECK();
     }
     if (fuse && h->prof_ev[1]) VMAT_CUDA(cudaEventRecord(h->prof_ev[1], st));

@@ -11,10 +11,14 @@
 //              up to 24 k entries, in place in global memory beyond) -> canonical order, so every later
 //              floating-point sum has a fixed order whatever the order of the input triplets (C14);
 //              equal neighbours after the sort are duplicates -> VMAT_ERR_DUPLICATE
+//   pack       the canonical CSR arrays are cut into segments and 32-entry groups and copied into the
+//              final padded, tile-interleaved arrays (spmv.cuh), with u16 offsets + a base per group where
+//              that is smaller than int32 indices; the canonical arrays are freed
 // Host-resident COO is streamed through a device staging buffer in chunks, twice.
 #include "spmv.cuh"
 #include <vector>
 #include <algorithm>
+#include <climits>
 
 enum { FLAG_RANGE = 0, FLAG_NONFINITE = 1, FLAG_DUP = 2, N_FLAGS = 4 };
 
@@ -175,35 +179,77 @@ __global__ void k_sort_rows_gmem(const int64_t *__restrict__ ptr, int32_t *idx, 
         if (ri[i] == ri[i - 1]) atomicOr(flags + FLAG_DUP, 1);
 }
 
-// ---------------------------------------------------------------- tile interleave (spmv.cuh)
-// One warp per segment (a beamlet row of D^T when seg_row == NULL, else a dose segment of D): every full
-// 256-entry tile is permuted in place so that stored word 8*l + t holds the tile's entry 32*t + l.
+// ---------------------------------------------------------------- pack: canonical CSR -> grouped, padded layout
+// One warp per segment (rows [seg_row[w], seg_row[w+1]); seg_row == NULL: segment w = row w).  The warp
+// walks the segment's canonical entries and forms groups greedily: a group takes the next entries while it
+// holds fewer than 32 and the span max - min of its secondary indices stays <= span_limit (65535 for u16
+// offsets; INT32_MAX for the wide format, where only the segment's last group is short).  Greedy prefixes
+// give the fewest groups any such partition can have, in particular never more than packing each row alone.
+//   WRITE = false: n_groups[w] = number of groups of the segment.
+//   WRITE = true : gstart[w] = first group of the segment (exclusive scan of n_groups); writes the values,
+//                  offsets + bases (narrow) or indices (wide) at their tile-interleaved position, pads
+//                  (value 0, index of the entry before) and the padded row starts pptr.
+template <bool WRITE>
 __global__ void __launch_bounds__(256)
-k_interleave(const int64_t *__restrict__ ptr, const int32_t *__restrict__ seg_row, int n_seg,
-             int32_t *idx, float *val)
+k_pack(const int64_t *__restrict__ ptr, const int32_t *__restrict__ cidx, const float *__restrict__ cval,
+       const int32_t *__restrict__ seg_row, int n_seg, int64_t span_limit, bool narrow,
+       uint32_t *__restrict__ n_groups, const int64_t *__restrict__ gstart,
+       float *__restrict__ val, void *__restrict__ sec, int32_t *__restrict__ base, int64_t *__restrict__ pptr)
 {
     const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (w >= n_seg) return;
     const int r0 = seg_row ? seg_row[w] : w, r1 = seg_row ? seg_row[w + 1] : w + 1;
     const int64_t s = ptr[r0], e = ptr[r1];
-    const Segment sg = segment_of(s, e);
-    for (int64_t ti = 0; ti < sg.nt; ++ti) {
-        const int64_t base = sg.a0 + ti * TILE;
-        int32_t ci[8];
-        float vi[8];
+    int64_t S = 0, G = 0;
+    if (WRITE) { S = gstart[w] * GROUP; G = gstart[w + 1] - gstart[w]; }
+    int64_t k = s, gl = 0;
+    while (k < e) {
+        const bool valid = k + lane < e;
+        const int c = valid ? cidx[k + lane] : 0;
+        int mn = valid ? c : INT32_MAX, mx = valid ? c : INT32_MIN;
 #pragma unroll
-        for (int t = 0; t < 8; ++t) { ci[t] = idx[base + t * 32 + lane]; vi[t] = val[base + t * 32 + lane]; }
-        __syncwarp();
-#pragma unroll
-        for (int t = 0; t < 8; ++t) { idx[base + lane * 8 + t] = ci[t]; val[base + lane * 8 + t] = vi[t]; }
-        __syncwarp();
+        for (int o = 1; o < 32; o <<= 1) {                       // inclusive prefix min / max
+            const int a = __shfl_up_sync(0xffffffffu, mn, o), b = __shfl_up_sync(0xffffffffu, mx, o);
+            if (lane >= o) { mn = min(mn, a); mx = max(mx, b); }
+        }
+        const bool ok = valid && (int64_t)mx - (int64_t)mn <= span_limit;
+        const int n_take = __popc(__ballot_sync(0xffffffffu, ok));       // a prefix of the lanes, >= 1
+        if (WRITE) {
+            const int b = __shfl_sync(0xffffffffu, mn, n_take - 1);       // the group's minimum index
+            const int c_last = __shfl_sync(0xffffffffu, c, n_take - 1);
+            const bool real = lane < n_take;
+            const int ci = real ? c : c_last;                             // pad: index of the entry before it
+            const float vi = real ? cval[k + lane] : 0.f;
+            const int64_t pos = stored_pos(S, G, S + gl * GROUP + lane);
+            val[pos] = vi;
+            if (narrow) {
+                ((uint16_t *)sec)[pos] = (uint16_t)(ci - b);
+                if (lane == 0) base[gstart[w] + gl] = b;
+            } else {
+                ((int32_t *)sec)[pos] = ci;
+            }
+            for (int r = r0 + lane; r < r1; r += 32) {                    // rows whose first entry is in this group
+                const int64_t pr = ptr[r];
+                if (pr >= k && pr < k + n_take) pptr[r] = S + gl * GROUP + (pr - k);
+            }
+        }
+        k += n_take;
+        ++gl;
+    }
+    if (WRITE) {
+        for (int r = r0 + lane; r < r1; r += 32)                          // empty rows at the segment's end
+            if (ptr[r] == e) pptr[r] = S + G * GROUP;
+    } else if (lane == 0) {
+        n_groups[w] = (uint32_t)gl;
     }
 }
 
 constexpr int SORT_SMALL = 2048;       // 16 KB of keys, 256 threads
 constexpr int SORT_BIG = 24576;        // 192 KB of keys, 1024 threads
 
-static int sort_layout(const CsrLayout &A, int64_t max_len, int *flags, cudaStream_t st)
+struct CanonCsr { int32_t n_rows; int64_t *ptr; int32_t *idx; float *val; };
+
+static int sort_layout(const CanonCsr &A, int64_t max_len, int *flags, cudaStream_t st)
 {
     if (A.n_rows == 0 || max_len <= 1) return VMAT_OK;
     k_sort_rows_smem<<<A.n_rows, 256, SORT_SMALL * 8, st>>>(A.ptr, A.idx, A.val, 1, SORT_SMALL, flags);
@@ -238,39 +284,158 @@ static int dev_alloc(T **p, int64_t n, int64_t *bytes)
 
 #define TRY(x) do { int rc_ = (x); if (rc_ != VMAT_OK) return rc_; } while (0)
 
+// frees device scratch on every exit path
+struct DevGuard {
+    std::vector<void **> p;
+    ~DevGuard() { for (void **q : p) if (*q) { cudaFree(*q); *q = nullptr; } }
+    void add(void **q) { p.push_back(q); }
+};
+
+// ---------------------------------------------------------------- segments + groups of one layout
+struct PackPlan {
+    bool narrow = false;
+    std::vector<int32_t> seg;          // segment -> first row, [n_seg+1] (empty when every row is a segment)
+    int32_t n_seg = 0;
+    int32_t *d_seg = nullptr;          // device copy of seg (NULL when every row is a segment)
+    int64_t *d_gstart = nullptr;       // [n_seg+1] first group of each segment
+    int64_t P = 0;                     // padded entries
+    void release() { if (d_seg) cudaFree(d_seg); if (d_gstart) cudaFree(d_gstart); d_seg = nullptr; d_gstart = nullptr; }
+};
+
+// Plans the layout of the canonical CSR C in the given format.  group_short: voxel rows (D) - consecutive
+// short rows share a warp; otherwise every row is its own segment (beamlet rows of D^T).
+static int plan_layout(const CanonCsr &C, bool narrow, bool group_short, PackPlan *pl, cudaStream_t st)
+{
+    const int32_t n_rows = C.n_rows;
+    const int64_t span = narrow ? 65535 : (int64_t)INT32_MAX;
+    uint32_t *d_cnt = nullptr;
+    unsigned long long *d_max = nullptr;
+    DevGuard guard;
+    guard.add((void **)&d_cnt); guard.add((void **)&d_max);
+    int64_t dummy = 0;
+    TRY(dev_alloc(&d_cnt, n_rows, &dummy));
+    TRY(dev_alloc(&d_max, 1, &dummy));
+    pl->narrow = narrow;
+    const int grid_rows = (n_rows + 7) / 8;
+    if (n_rows > 0) {                                            // groups of every row packed alone
+        k_pack<false><<<grid_rows, 256, 0, st>>>(C.ptr, C.idx, C.val, nullptr, n_rows, span, narrow, d_cnt, nullptr,
+                                                 nullptr, nullptr, nullptr, nullptr);
+        VMAT_LAUNCH_CHECK();
+    }
+    pl->n_seg = n_rows;
+    if (group_short) {
+        // dose-kernel segments: a row of more than DOSE_SEG_NNZ padded entries alone, else consecutive rows
+        // with at most DOSE_SEG_NNZ padded entries together (packed together they never need more groups)
+        std::vector<uint32_t> c((size_t)std::max(n_rows, 1));
+        VMAT_CUDA(cudaMemcpyAsync(c.data(), d_cnt, (size_t)n_rows * 4, cudaMemcpyDeviceToHost, st));
+        VMAT_CUDA(cudaStreamSynchronize(st));
+        const uint32_t SEG_GROUPS = DOSE_SEG_NNZ / GROUP;
+        pl->seg.clear();
+        pl->seg.push_back(0);
+        int32_t r = 0;
+        while (r < n_rows) {
+            int32_t q = r + 1;                                   // a segment always takes at least one row
+            uint64_t tot = c[r];
+            while (q < n_rows && q - r < DOSE_MAX_ROWS && tot + c[q] <= SEG_GROUPS) tot += c[q++];
+            pl->seg.push_back(q);
+            r = q;
+        }
+        pl->n_seg = (int32_t)pl->seg.size() - 1;
+        TRY(dev_alloc(&pl->d_seg, (int64_t)pl->seg.size(), &dummy));
+        VMAT_CUDA(cudaMemcpyAsync(pl->d_seg, pl->seg.data(), pl->seg.size() * 4, cudaMemcpyHostToDevice, st));
+        if (pl->n_seg > 0) {
+            k_pack<false><<<(pl->n_seg + 7) / 8, 256, 0, st>>>(C.ptr, C.idx, C.val, pl->d_seg, pl->n_seg, span, narrow,
+                                                               d_cnt, nullptr, nullptr, nullptr, nullptr, nullptr);
+            VMAT_LAUNCH_CHECK();
+        }
+    }
+    TRY(dev_alloc(&pl->d_gstart, (int64_t)pl->n_seg + 1, &dummy));
+    k_scan<<<1, SCAN_THREADS, 0, st>>>(d_cnt, pl->n_seg, pl->d_gstart, d_max);
+    VMAT_LAUNCH_CHECK();
+    int64_t total = 0;
+    VMAT_CUDA(cudaMemcpyAsync(&total, pl->d_gstart + pl->n_seg, 8, cudaMemcpyDeviceToHost, st));
+    VMAT_CUDA(cudaStreamSynchronize(st));
+    pl->P = total * GROUP;
+    return VMAT_OK;
+}
+
+// Chooses the format (index_bits: 16, 32, or 0 = the smaller one), allocates the final arrays of layout A
+// and fills them from the canonical CSR C.  A.ptr is C.ptr (kept); A.pptr must be allocated.
+static int pack_layout(vmat_ddc *h, PackedLayout &A, const CanonCsr &C, int32_t n_cols, bool group_short,
+                       int index_bits, PackPlan *chosen, cudaStream_t st)
+{
+    PackPlan narrow_pl, wide_pl;
+    struct Rel { PackPlan &a, &b; ~Rel() { a.release(); b.release(); } } rel{narrow_pl, wide_pl};
+    bool use_narrow;
+    if (index_bits == 16 || (index_bits == 0 && n_cols <= 65536)) {          // every span fits: no early closes
+        TRY(plan_layout(C, true, group_short, &narrow_pl, st));
+        use_narrow = true;
+    } else if (index_bits == 32) {
+        TRY(plan_layout(C, false, group_short, &wide_pl, st));
+        use_narrow = false;
+    } else {
+        TRY(plan_layout(C, true, group_short, &narrow_pl, st));
+        TRY(plan_layout(C, false, group_short, &wide_pl, st));
+        // bytes per padded entry: 6.125 narrow, 8 wide; narrow must save at least 5 %
+        use_narrow = 6.125 * (double)narrow_pl.P <= 0.95 * 8.0 * (double)wide_pl.P;
+    }
+    PackPlan &pl = use_narrow ? narrow_pl : wide_pl;
+    A.P = pl.P;
+    A.index_bits = use_narrow ? 16 : 32;
+    const int64_t SLACK = 64;
+    TRY(dev_alloc(&A.val, A.P + SLACK, &h->bytes_device));
+    if (use_narrow) {
+        uint16_t *off = nullptr;
+        TRY(dev_alloc(&off, A.P + SLACK, &h->bytes_device));
+        A.sec = off;
+        TRY(dev_alloc(&A.base, A.P / GROUP + SLACK, &h->bytes_device));
+    } else {
+        int32_t *idx = nullptr;
+        TRY(dev_alloc(&idx, A.P + SLACK, &h->bytes_device));
+        A.sec = idx;
+    }
+    if (pl.n_seg > 0) {
+        k_pack<true><<<(pl.n_seg + 7) / 8, 256, 0, st>>>(C.ptr, C.idx, C.val, pl.d_seg, pl.n_seg,
+                                                         use_narrow ? 65535 : (int64_t)INT32_MAX, use_narrow, nullptr,
+                                                         pl.d_gstart, A.val, A.sec, A.base, A.pptr);
+        VMAT_LAUNCH_CHECK();
+    }
+    VMAT_CUDA(cudaMemcpyAsync(A.pptr + A.n_rows, &A.P, 8, cudaMemcpyHostToDevice, st));
+    VMAT_CUDA(cudaStreamSynchronize(st));
+    if (chosen) {                                               // hand the segment table to the caller
+        chosen->seg = pl.seg; chosen->n_seg = pl.n_seg; chosen->d_seg = pl.d_seg; pl.d_seg = nullptr;
+    }
+    return VMAT_OK;
+}
+
 int vmat_build_layouts(vmat_ddc *h, const int32_t *coo_voxel, const int32_t *coo_beamlet,
-                       const float *coo_val, cudaStream_t st)
+                       const float *coo_val, int index_bits, cudaStream_t st)
 {
     const int64_t nnz = h->nnz;
     const int32_t nv = h->n_voxels, nb = h->n_beamlets;
-    const int64_t PAD = 16;                                  // 256-bit loads may read up to 7 entries past a row
     h->D.n_rows = nv; h->D.nnz = nnz;
     h->Dt.n_rows = nb; h->Dt.nnz = nnz;
     TRY(dev_alloc(&h->D.ptr, (int64_t)nv + 1, &h->bytes_device));
     TRY(dev_alloc(&h->Dt.ptr, (int64_t)nb + 1, &h->bytes_device));
-    TRY(dev_alloc(&h->D.idx, nnz + PAD, &h->bytes_device));
-    TRY(dev_alloc(&h->D.val, nnz + PAD, &h->bytes_device));
-    TRY(dev_alloc(&h->Dt.idx, nnz + PAD, &h->bytes_device));
-    TRY(dev_alloc(&h->Dt.val, nnz + PAD, &h->bytes_device));
-    VMAT_CUDA(cudaMemsetAsync(h->D.idx + nnz, 0, PAD * 4, st));
-    VMAT_CUDA(cudaMemsetAsync(h->D.val + nnz, 0, PAD * 4, st));
-    VMAT_CUDA(cudaMemsetAsync(h->Dt.idx + nnz, 0, PAD * 4, st));
-    VMAT_CUDA(cudaMemsetAsync(h->Dt.val + nnz, 0, PAD * 4, st));
+    TRY(dev_alloc(&h->D.pptr, (int64_t)nv + 1, &h->bytes_device));
+    TRY(dev_alloc(&h->Dt.pptr, (int64_t)nb + 1, &h->bytes_device));
 
-    // scratch (freed before returning)
+    // scratch (freed before returning): the canonical CSR arrays of both layouts, counters, staging
+    CanonCsr cD{nv, h->D.ptr, nullptr, nullptr}, cT{nb, h->Dt.ptr, nullptr, nullptr};
     uint32_t *cntV = nullptr, *cntB = nullptr;
     int *flags = nullptr;
     unsigned long long *maxes = nullptr;
     int32_t *stg_v = nullptr, *stg_b = nullptr;
     float *stg_a = nullptr;
     int64_t scratch_bytes = 0;
-    struct Guard {
-        void **p[7]; int n = 0;
-        ~Guard() { for (int i = 0; i < n; ++i) if (*p[i]) cudaFree(*p[i]); }
-        void add(void **q) { p[n++] = q; }
-    } guard;
+    DevGuard guard;
+    guard.add((void **)&cD.idx); guard.add((void **)&cD.val); guard.add((void **)&cT.idx); guard.add((void **)&cT.val);
     guard.add((void **)&cntV); guard.add((void **)&cntB); guard.add((void **)&flags); guard.add((void **)&maxes);
     guard.add((void **)&stg_v); guard.add((void **)&stg_b); guard.add((void **)&stg_a);
+    TRY(dev_alloc(&cD.idx, nnz, &scratch_bytes));
+    TRY(dev_alloc(&cD.val, nnz, &scratch_bytes));
+    TRY(dev_alloc(&cT.idx, nnz, &scratch_bytes));
+    TRY(dev_alloc(&cT.val, nnz, &scratch_bytes));
     TRY(dev_alloc(&cntV, nv, &scratch_bytes));
     TRY(dev_alloc(&cntB, nb, &scratch_bytes));
     TRY(dev_alloc(&flags, N_FLAGS, &scratch_bytes));
@@ -306,8 +471,8 @@ int vmat_build_layouts(vmat_ddc *h, const int32_t *coo_voxel, const int32_t *coo
             if (pass == 0)
                 k_count<<<grid_for(n), ING_THREADS, 0, st>>>(v, b, a, n, nv, nb, cntV, cntB, flags);
             else
-                k_scatter<<<grid_for(n), ING_THREADS, 0, st>>>(v, b, a, n, h->D.ptr, h->Dt.ptr, cntV, cntB,
-                                                               h->D.idx, h->D.val, h->Dt.idx, h->Dt.val);
+                k_scatter<<<grid_for(n), ING_THREADS, 0, st>>>(v, b, a, n, cD.ptr, cT.ptr, cntV, cntB,
+                                                               cD.idx, cD.val, cT.idx, cT.val);
             VMAT_LAUNCH_CHECK();
         }
         if (pass == 0) {
@@ -316,9 +481,9 @@ int vmat_build_layouts(vmat_ddc *h, const int32_t *coo_voxel, const int32_t *coo
             VMAT_CUDA(cudaStreamSynchronize(st));
             if (hf[FLAG_RANGE]) { vmat_set_error("vmat_ddc_create: COO index out of range"); return VMAT_ERR_INDEX_RANGE; }
             if (hf[FLAG_NONFINITE]) { vmat_set_error("vmat_ddc_create: non-finite COO value"); return VMAT_ERR_NONFINITE; }
-            k_scan<<<1, SCAN_THREADS, 0, st>>>(cntV, nv, h->D.ptr, maxes + 0);
+            k_scan<<<1, SCAN_THREADS, 0, st>>>(cntV, nv, cD.ptr, maxes + 0);
             VMAT_LAUNCH_CHECK();
-            k_scan<<<1, SCAN_THREADS, 0, st>>>(cntB, nb, h->Dt.ptr, maxes + 1);
+            k_scan<<<1, SCAN_THREADS, 0, st>>>(cntB, nb, cT.ptr, maxes + 1);
             VMAT_LAUNCH_CHECK();
             VMAT_CUDA(cudaMemsetAsync(cntV, 0, (size_t)std::max(nv, 1) * 4, st));
             VMAT_CUDA(cudaMemsetAsync(cntB, 0, (size_t)std::max(nb, 1) * 4, st));
@@ -329,39 +494,24 @@ int vmat_build_layouts(vmat_ddc *h, const int32_t *coo_voxel, const int32_t *coo
     VMAT_CUDA(cudaStreamSynchronize(st));
     h->max_voxel_row_nnz = (int64_t)hmax[0];
     h->max_beamlet_row_nnz = (int64_t)hmax[1];
-    TRY(sort_layout(h->D, h->max_voxel_row_nnz, flags, st));
-    TRY(sort_layout(h->Dt, h->max_beamlet_row_nnz, flags, st));
+    TRY(sort_layout(cD, h->max_voxel_row_nnz, flags, st));
+    TRY(sort_layout(cT, h->max_beamlet_row_nnz, flags, st));
     int hf[N_FLAGS];
     VMAT_CUDA(cudaMemcpyAsync(hf, flags, sizeof(hf), cudaMemcpyDeviceToHost, st));
     VMAT_CUDA(cudaStreamSynchronize(st));
     if (hf[FLAG_DUP]) { vmat_set_error("vmat_ddc_create: duplicate (voxel, beamlet) pair"); return VMAT_ERR_DUPLICATE; }
 
-    // ---- dose kernel segments (host, from the voxel row pointers): a long row alone, or consecutive
-    //      short rows with at most DOSE_SEG_NNZ non-zeros together
-    std::vector<int64_t> hptr((size_t)nv + 1);
-    VMAT_CUDA(cudaMemcpy(hptr.data(), h->D.ptr, ((size_t)nv + 1) * 8, cudaMemcpyDeviceToHost));
-    std::vector<int32_t> seg;
-    seg.push_back(0);
-    int32_t r = 0;
-    while (r < nv) {
-        int32_t r1 = r + 1;                                   // a segment always takes at least one row
-        while (r1 < nv && r1 - r < DOSE_MAX_ROWS && hptr[r1 + 1] - hptr[r] <= DOSE_SEG_NNZ) ++r1;
-        seg.push_back(r1);
-        r = r1;
-    }
-    h->n_seg = (int32_t)seg.size() - 1;
+    // ---- pack D (voxel rows; dose-kernel segments), free its canonical arrays, then D^T (one segment per row)
+    PackPlan segD;
+    TRY(pack_layout(h, h->D, cD, nb, true, index_bits, &segD, st));
+    cudaFree(cD.idx); cD.idx = nullptr;
+    cudaFree(cD.val); cD.val = nullptr;
+    h->seg_row = segD.d_seg;                                    // owned by the handle from here on
+    h->bytes_device += (int64_t)segD.seg.size() * 4;
+    h->n_seg = segD.n_seg;
     h->n_blocks = (h->n_seg + DOSE_THREADS / 32 - 1) / (DOSE_THREADS / 32);
-    TRY(dev_alloc(&h->seg_row, (int64_t)seg.size(), &h->bytes_device));
-    VMAT_CUDA(cudaMemcpy(h->seg_row, seg.data(), seg.size() * 4, cudaMemcpyHostToDevice));
-    h->h_seg_row = seg;
-    // ---- tile-interleave both layouts: segments = dose segments of D, beamlet rows of D^T
-    if (nnz > 0) {
-        k_interleave<<<(h->n_seg + 7) / 8, 256, 0, st>>>(h->D.ptr, h->seg_row, h->n_seg, h->D.idx, h->D.val);
-        VMAT_LAUNCH_CHECK();
-        k_interleave<<<(nb + 7) / 8, 256, 0, st>>>(h->Dt.ptr, nullptr, nb, h->Dt.idx, h->Dt.val);
-        VMAT_LAUNCH_CHECK();
-        VMAT_CUDA(cudaStreamSynchronize(st));
-    }
+    h->h_seg_row = segD.seg;
+    TRY(pack_layout(h, h->Dt, cT, nv, false, index_bits, nullptr, st));
     TRY(dev_alloc(&h->F_partial, h->n_blocks, &h->bytes_device));
     h->n_obj_blocks = (nv + 255) / 256;
     TRY(dev_alloc(&h->F_partial_obj, h->n_obj_blocks, &h->bytes_device));

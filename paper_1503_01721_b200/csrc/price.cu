@@ -3,7 +3,7 @@
 //
 // Beamlet rows are long and even (a radius-`cutoff` cylinder through the body: 10^3-10^4 non-zeros),
 // so the paper's mapping holds on sm_100a: one warp per beamlet row (L127), here over lane-interleaved
-// 256-entry tiles read with 256-bit loads (spmv.cuh).  Measured on B200 the warp-per-row kernel beats
+// 256-entry tiles read with 256-bit loads, with u16 index offsets where the layout allows (spmv.cuh).  Measured on B200 the warp-per-row kernel beats
 // a CTA-per-leaf-row kernel by 12 % (perfect balance, more independent streams), so the row selection
 // is fused differently: every CTA (8 consecutive beamlet rows) hands in tickets for the leaf rows it
 // priced, and the CTA whose ticket completes a leaf row selects that row's opening on the spot - the
@@ -112,10 +112,10 @@ struct SelectArgs {
 #ifndef VMAT_PRICE_MINB
 #define VMAT_PRICE_MINB 6        // 40 registers, 1536 threads per SM: fastest of 4..8 on B200 (cfg 3)
 #endif
-template <bool SELECT>
+template <bool SELECT, bool NARROW>
 __global__ void __launch_bounds__(PRICE_THREADS, VMAT_PRICE_MINB)
-k_price(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const float *__restrict__ val,
-        int n_rows, const float *__restrict__ g, float *__restrict__ p, SelectArgs sa)
+k_price(const int64_t *__restrict__ pptr, const MatView A, int n_rows, const float *__restrict__ g,
+        float *__restrict__ p, SelectArgs sa)
 {
     const int lane = threadIdx.x & 31;
     if (SELECT) {                                   // leaf rows without beamlets draw no ticket: close them here
@@ -127,13 +127,7 @@ k_price(const int64_t *__restrict__ ptr, const int32_t *__restrict__ idx, const 
     const int warp = threadIdx.x >> 5;
     const int row = blockIdx.x * PRICE_WARPS + warp;
     if (row < n_rows) {
-        const int64_t s = ptr[row], e = ptr[row + 1];
-        const Segment sg = segment_of(s, e);
-        float acc = 0.f;
-#pragma unroll 1
-        for (int64_t ti = 0; ti < sg.nt; ++ti) acc += tile_dot(val, idx, sg.a0 + ti * TILE, g, lane);
-        plain_foreach<32>(val, idx, s, sg, e, g, lane, [&](int64_t, float q) { acc += q; });
-        acc = warp_sum(acc);
+        const float acc = warp_sum(segment_dot<NARROW>(A, pptr[row], pptr[row + 1], g, lane));
         if (lane == 0) p[row] = acc;
     }
     if (SELECT) {
@@ -275,7 +269,10 @@ int vmat_launch_price(const vmat_ddc *h, const float *g, float *p, cudaStream_t 
 {
     if (h->n_beamlets == 0) return VMAT_OK;
     const int grid = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
-    k_price<false><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.ptr, h->Dt.idx, h->Dt.val, h->n_beamlets, g, p, SelectArgs{});
+    if (h->Dt.index_bits == 16)
+        k_price<false, true><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, view_of(h->Dt), h->n_beamlets, g, p, SelectArgs{});
+    else
+        k_price<false, false><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, view_of(h->Dt), h->n_beamlets, g, p, SelectArgs{});
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }
@@ -302,7 +299,10 @@ int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *a
     }
     SelectArgs sa{h->beamlet_leafrow, h->leafrow_col_offset, h->leafrow_angle, angle_mask, h->leafrow_done,
                   h->S_scratch, L, R, row_price, h->n_leaf_rows};
-    k_price<true><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.ptr, h->Dt.idx, h->Dt.val, h->n_beamlets, g, p, sa);
+    if (h->Dt.index_bits == 16)
+        k_price<true, true><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, view_of(h->Dt), h->n_beamlets, g, p, sa);
+    else
+        k_price<true, false><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, view_of(h->Dt), h->n_beamlets, g, p, sa);
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }

@@ -64,10 +64,10 @@ def obj_to_device(A, dev):
                      torch.from_numpy(A["wo"]).to(dev), torch.from_numpy(A["wu"]).to(dev))
 
 
-def ddc_from_arrays(A, dev, coo_on_device=True):
+def ddc_from_arrays(A, dev, coo_on_device=True, index_bits=0):
     import paper_1503_01721_b200 as vm
     conv = (lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)) if coo_on_device else \
         (lambda a: torch.from_numpy(np.ascontiguousarray(a)))
     return vm.vmat_ddc_create(A["n_v"], A["n_b"], conv(A["vox"]), conv(A["beam"]), conv(A["val"]),
                               torch.from_numpy(A["aco"]), torch.from_numpy(A["aro"]), torch.from_numpy(A["lco"]),
-                              device=dev)
+                              device=dev, index_bits=index_bits)

@@ -47,27 +47,51 @@ def _random_problem(rng, n_v, n_b, rows_spec, row_lens, n_struct=4):
 
 
 def _run_and_check(vm, A, x, mask=None, expect_no_diff=True):
-    h = ddc_from_arrays(A, DEV)
-    out = h.alloc_outputs()
-    m = None if mask is None else torch.from_numpy(mask).to(DEV)
-    vm.vmat_price_eval(h, torch.from_numpy(x).to(DEV), obj_to_device(A, DEV), out, m)
-    torch.cuda.synchronize()
+    """Whole evaluation against the oracle, once per index encoding (int32 indices; u16 offsets + group
+    bases; the automatic choice).  Returns the outputs / info of the automatic choice."""
     ev = oracle_eval(A, x, mask)
-    assert_vec_close("d", out.d.cpu().numpy(), ev.d)
-    assert_vec_close("g", out.g.cpu().numpy(), ev.g)
-    assert_vec_close("p", out.p.cpu().numpy(), ev.p)
-    assert abs(out.F.item() - ev.F) <= REL_L2 * abs(ev.F) + 1e-300
-    n_diff = check_selection_protocol(A, out, ev, mask)
-    if expect_no_diff:
-        assert n_diff == 0
-    # the unfused calls give the same bits as the fused ones for d and p
-    d2 = torch.empty_like(out.d); p2 = torch.empty_like(out.p)
-    vm.vmat_dose(h, torch.from_numpy(x).to(DEV), d2)
-    vm.vmat_price(h, out.g, p2)
-    assert torch.equal(d2, out.d) and torch.equal(p2, out.p)
-    info = h.info
-    h.close()
-    return out, ev, info
+    outs, infos = {}, {}
+    for bits in (32, 16, 0):
+        h = ddc_from_arrays(A, DEV, index_bits=bits)
+        out = h.alloc_outputs()
+        m = None if mask is None else torch.from_numpy(mask).to(DEV)
+        vm.vmat_price_eval(h, torch.from_numpy(x).to(DEV), obj_to_device(A, DEV), out, m)
+        torch.cuda.synchronize()
+        assert_vec_close("d", out.d.cpu().numpy(), ev.d)
+        assert_vec_close("g", out.g.cpu().numpy(), ev.g)
+        assert_vec_close("p", out.p.cpu().numpy(), ev.p)
+        assert abs(out.F.item() - ev.F) <= REL_L2 * abs(ev.F) + 1e-300
+        n_diff = check_selection_protocol(A, out, ev, mask)
+        if expect_no_diff:
+            assert n_diff == 0
+        # the unfused calls give the same bits as the fused ones for d and p
+        d2 = torch.empty_like(out.d); p2 = torch.empty_like(out.p)
+        vm.vmat_dose(h, torch.from_numpy(x).to(DEV), d2)
+        vm.vmat_price(h, out.g, p2)
+        assert torch.equal(d2, out.d) and torch.equal(p2, out.p)
+        info = h.info
+        if bits:
+            assert info["index_bits_d"] == info["index_bits_dt"] == bits
+        for lay, rows in (("d", "n_voxels"), ("dt", "n_beamlets")):          # storage closed forms (spmv.cuh)
+            P, b = info[f"padded_{lay}"], info[f"index_bits_{lay}"]
+            assert P % 32 == 0 and P >= info["nnz"]
+            per_entry = 6 * P + 4 * (P // 32) if b == 16 else 8 * P
+            seg_table = 4 * (info["n_dose_blocks"] + 1) if lay == "d" else 0
+            assert info[f"bytes_stream_{lay}"] == per_entry + 8 * (info[rows] + 1) + seg_table
+        # the layouts unpack to the same canonical CSR whatever the encoding
+        csr = [t.numpy() for w in (0, 1) for t in h.export_csr(w)]
+        if outs:
+            for a, b in zip(csr, first_csr):
+                assert np.array_equal(a, b)
+        else:
+            first_csr = csr
+        outs[bits], infos[bits] = out, info
+        h.close()
+    # no group closed early (same padded size) => the encodings give the same bits everywhere
+    if infos[16]["padded_d"] == infos[32]["padded_d"] and infos[16]["padded_dt"] == infos[32]["padded_dt"]:
+        for f in ("d", "g", "F", "p", "L", "R", "row_price", "angle_price", "best_angle"):
+            assert torch.equal(getattr(outs[16], f), getattr(outs[32], f)), f
+    return outs[0], ev, infos[0]
 
 
 def test_empty_matrix(vm):
@@ -124,6 +148,53 @@ def test_exact_ties_in_prices(vm):
     out, ev, _ = _run_and_check(vm, A, x)
     assert np.array_equal(out.p.cpu().numpy().astype(np.float64), ev.p)          # exact integers on both sides
     assert np.array_equal(out.L.cpu().numpy(), ev.L) and np.array_equal(out.R.cpu().numpy(), ev.R)
+
+
+def test_index_spans_beyond_16_bits(vm):
+    """Secondary indices scattered over > 65536 columns / rows: the u16 encoding has to close groups early
+    (pads inside rows), and for D the automatic choice falls back to int32 indices; every encoding matches
+    the oracle."""
+    rng = np.random.default_rng(4)
+    n_v, n_b = 150000, 200000
+    lens = np.zeros(n_v, int)
+    hot = rng.choice(n_v, 2500, replace=False)
+    lens[hot] = rng.integers(1, 120, hot.size)
+    lens[hot[:3]] = [700, 1500, 9000]                      # long rows: register path with pads inside tiles
+    rows = [rng.multinomial(n_b // 4, np.ones(50) / 50) for _ in range(4)]
+    A = _random_problem(rng, n_v, n_b, rows, lens)
+    x = (rng.random(n_b) * 0.35).astype(np.float32)
+    out, ev, info = _run_and_check(vm, A, x)
+    assert info["index_bits_d"] == 32                                       # padding would outweigh the saving
+    h16 = ddc_from_arrays(A, DEV, index_bits=16)
+    assert h16.info["padded_d"] > 1.2 * info["padded_d"]                    # groups were closed early
+    h16.close()
+    assert (ev.g > 0).any() and (ev.g < 0).any() and (ev.R > ev.L).any()
+
+
+def test_narrow_encoding_is_chosen_when_smaller(vm):
+    """Clustered indices over > 65536 columns (runs, as in a DDC matrix): u16 offsets fit, 6.125 B per entry."""
+    rng = np.random.default_rng(5)
+    n_v, n_b = 90000, 100000
+    vox, beam = [], []
+    for i in rng.choice(n_v, 4000, replace=False):
+        for start in rng.choice(n_b - 40, rng.integers(1, 6), replace=False):   # a few runs of consecutive beamlets
+            ln = int(rng.integers(3, 30))
+            vox.append(np.full(ln, i, np.int32)); beam.append(np.arange(start, start + ln, dtype=np.int32))
+    vox, beam = np.concatenate(vox), np.concatenate(beam)
+    key = np.unique(vox.astype(np.int64) * n_b + beam)                     # overlapping runs: drop duplicates
+    vox, beam = (key // n_b).astype(np.int32), (key % n_b).astype(np.int32)
+    perm = rng.permutation(vox.size)
+    rows = [rng.multinomial(n_b // 5, np.ones(40) / 40) for _ in range(5)]
+    lens = np.concatenate(rows)
+    lco = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+    aro = np.concatenate([[0], np.cumsum([len(r) for r in rows])]).astype(np.int32)
+    A = dict(vox=vox[perm], beam=beam[perm], val=(rng.random(vox.size) + 0.01).astype(np.float32)[perm], n_v=n_v,
+             n_b=n_b, sid=rng.integers(0, 3, n_v).astype(np.uint8), T=np.array([5.0, 20.0, 8.0], np.float32),
+             wo=np.array([0.05, 1.0, 0.2], np.float32), wu=np.array([0.0, 1.0, 0.0], np.float32), lco=lco, aro=aro,
+             aco=lco[aro])
+    x = (rng.random(n_b) * 2.0).astype(np.float32)
+    out, ev, info = _run_and_check(vm, A, x)
+    assert info["index_bits_dt"] == 16 or info["index_bits_d"] == 16
 
 
 # ------------------------------------------------------------------ the configs

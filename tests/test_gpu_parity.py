@@ -76,6 +76,31 @@ def test_layouts_round_trip_config0(vm, A0, h0):
     assert info["bytes_csr_dt"] == 8 * info["nnz"] + 8 * (info["n_beamlets"] + 1)
 
 
+@pytest.mark.parametrize("bits", [16, 32])
+def test_index_encodings_unpack_to_the_same_csr_and_give_the_same_bits(vm, A0, h0, bits):
+    """int32 indices (the paper's 8 B/nnz, Table 2) and u16 offsets + one base per 32 entries (6.125 B) hold
+    the same entries in the same order: same canonical CSR, and - config 0 needs no early-closed group -
+    bit-identical outputs."""
+    h = ddc_from_arrays(A0, DEV, index_bits=bits)
+    info = h.info
+    assert info["index_bits_d"] == info["index_bits_dt"] == bits
+    for lay, rows in (("d", "n_voxels"), ("dt", "n_beamlets")):
+        P = info[f"padded_{lay}"]
+        assert P % 32 == 0 and info["nnz"] <= P
+        per_entry = 6 * P + 4 * (P // 32) if bits == 16 else 8 * P
+        seg_table = 4 * (info["n_dose_blocks"] + 1) if lay == "d" else 0
+        assert info[f"bytes_stream_{lay}"] == per_entry + 8 * (info[rows] + 1) + seg_table
+    assert info["padded_dt"] - info["nnz"] <= 31 * info["n_beamlets"]                  # < one group of pads per row
+    for w in (0, 1):
+        for a, b in zip(h.export_csr(w), h0.export_csr(w)):
+            assert torch.equal(a, b)
+    x = _x(A0["n_b"], 27, 14.0)
+    o1, o2 = _eval_gpu(vm, h, A0, x), _eval_gpu(vm, h0, A0, x)
+    for f in ("d", "g", "F", "p", "L", "R", "row_price", "angle_price", "best_angle"):
+        assert torch.equal(getattr(o1, f), getattr(o2, f)), f
+    h.close()
+
+
 def test_ingest_host_and_device_coo_and_shuffle_give_identical_layouts(vm, A0, h0):
     perm = np.random.default_rng(3).permutation(A0["vox"].size)
     B = dict(A0, vox=A0["vox"][perm], beam=A0["beam"][perm], val=A0["val"][perm])
