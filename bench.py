@@ -94,14 +94,19 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def ncu_traffic(kernel_prefix: str, cfg: int, scale: float):
+def ncu_capture_file(index_bits: int) -> str:
+    """The committed ncu --set full capture of config 3 for the layout in use (u16 offsets: v5, int32: v4)."""
+    return "r1_ncu_full_cfg3_v5.csv" if index_bits == 16 else "r1_ncu_full_cfg3_v4.csv"
+
+
+def ncu_traffic(kernel_prefix: str, cfg: int, scale: float, index_bits: int):
     """dram bytes (read + write) per launch of the dominant kernel from the committed ncu --set full capture
-    (profiles/r1_ncu_full_cfg3_v4.csv, config 3 only); None for other workloads."""
+    (profiles/r1_ncu_full_cfg3_v{4,5}.csv, config 3 only); None for other workloads."""
     if cfg != 3 or scale != 1.0:
         return None
     try:
         import csv
-        rows = list(csv.reader(open(os.path.join(ROOT, "profiles", "r1_ncu_full_cfg3_v4.csv"))))
+        rows = [r for r in csv.reader(open(os.path.join(ROOT, "profiles", ncu_capture_file(index_bits)))) if len(r) > 3]
         hdr, units = rows[0], rows[1]
         mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
         for r in rows[2:]:
@@ -317,11 +322,11 @@ def run_ours(args):
         B_price_8B = 8 * nnz + 8 * (n_b + 1) + vec_price
         B_eval = B_dose + B_price
         B_eval_8B = B_dose_8B + B_price_8B
-        k_dose = {"name": "k_dose<true> (dose + fused objective/gradient)", "ncu": "k_dose<1>", "ms": float(t_dose.mean()), "ms_min": float(t_dose.min()),
+        k_dose = {"name": "k_dose<true> (dose + fused objective/gradient)", "ncu": "k_dose<1", "ms": float(t_dose.mean()), "ms_min": float(t_dose.min()),
                   "bytes": B_dose, "gbs": B_dose / (t_dose.mean() * 1e-3) / 1e9,
                   "gbs_8B_csr_equiv": B_dose_8B / (t_dose.mean() * 1e-3) / 1e9, "index_bits": info["index_bits_d"],
                   "padded_over_nnz": info["padded_d"] / max(nnz, 1)}
-        k_price = {"name": "k_price<true> (price + fused leaf-row selection)", "ncu": "k_price<1>", "ms": float(t_price.mean()), "ms_min": float(t_price.min()),
+        k_price = {"name": "k_price<true> (price + fused leaf-row selection)", "ncu": "k_price<1", "ms": float(t_price.mean()), "ms_min": float(t_price.min()),
                    "bytes": B_price, "gbs": B_price / (t_price.mean() * 1e-3) / 1e9,
                    "gbs_8B_csr_equiv": B_price_8B / (t_price.mean() * 1e-3) / 1e9, "index_bits": info["index_bits_dt"],
                    "padded_over_nnz": info["padded_dt"] / max(nnz, 1)}
@@ -349,8 +354,8 @@ def run_ours(args):
             "gpu_launches": launches,
             "roofline": {"bound": "hbm", "kernel": dom["name"], "achieved": dom["gbs"], "peak": peak,
                          "unit": "GB/s", "frac": dom["gbs"] / peak, "frac_of_8TBs": dom["gbs"] / 8000.0,
-                         "peak_source": peak_src, "traffic": ncu_traffic(dom["ncu"], args.config, args.scale),
-                         "traffic_source": "profiles/r1_ncu_full_cfg3_v4.csv (ncu --set full, one launch)", "algorithmic_bytes": dom["bytes"],
+                         "peak_source": peak_src, "traffic": ncu_traffic(dom["ncu"], args.config, args.scale, dom["index_bits"]),
+                         "traffic_source": f"profiles/{ncu_capture_file(dom['index_bits'])} (ncu --set full, one launch)", "algorithmic_bytes": dom["bytes"],
                          "ms": dom["ms"]},
             "kernels": [k_dose, k_price],
             "result_check": {"F_last": F_last, "best_angle_last": best_last},
