@@ -325,11 +325,13 @@ def run_ours(args):
         k_dose = {"name": "k_dose<true> (dose + fused objective/gradient)", "ncu": "k_dose<1", "ms": float(t_dose.mean()), "ms_min": float(t_dose.min()),
                   "bytes": B_dose, "gbs": B_dose / (t_dose.mean() * 1e-3) / 1e9,
                   "gbs_8B_csr_equiv": B_dose_8B / (t_dose.mean() * 1e-3) / 1e9, "index_bits": info["index_bits_d"],
-                  "padded_over_nnz": info["padded_d"] / max(nnz, 1)}
+                  "padded_over_nnz": info["padded_d"] / max(nnz, 1),
+                  "tiles_one_base_frac": info["tiles_uniform_d"] / max(info["tiles_d"], 1)}
         k_price = {"name": "k_price<true> (price + fused leaf-row selection)", "ncu": "k_price<1", "ms": float(t_price.mean()), "ms_min": float(t_price.min()),
                    "bytes": B_price, "gbs": B_price / (t_price.mean() * 1e-3) / 1e9,
                    "gbs_8B_csr_equiv": B_price_8B / (t_price.mean() * 1e-3) / 1e9, "index_bits": info["index_bits_dt"],
-                   "padded_over_nnz": info["padded_dt"] / max(nnz, 1)}
+                   "padded_over_nnz": info["padded_dt"] / max(nnz, 1),
+                   "tiles_one_base_frac": info["tiles_uniform_dt"] / max(info["tiles_dt"], 1)}
         dom = k_price if k_price["ms"] >= k_dose["ms"] else k_dose
         agg = aggregate(world, K, elapsed_ms)
         ms_per_step, value = agg["ms_per_step"], agg["value"]

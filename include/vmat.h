@@ -62,6 +62,8 @@ typedef struct vmat_ddc_info {
     int64_t bytes_stream_d;     /* bytes vmat_dose streams per call: values + indices (+ bases) of the
                                    padded entries + int64 row starts + the int32 segment table           */
     int64_t bytes_stream_dt;    /* bytes vmat_price streams per call: the same for D^T (no segment table) */
+    int64_t tiles_d, tiles_uniform_d;        /* u16 layouts: 256-entry tiles, and those stored with ONE base     */
+    int64_t tiles_dt, tiles_uniform_dt;      /* (span <= 65535) instead of one per 32-entry group; 0 for int32   */
 } vmat_ddc_info;
 
 /* A0 ingest / layout build (D arrives as COO - values, voxel (row) index,

@@ -19,7 +19,7 @@ from typing import Optional
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libvmat.so")
+LIB_PATH = os.environ.get("VMAT_LIB", os.path.join(_HERE, "libvmat.so"))     # VMAT_LIB: load another build of libvmat
 _lib = None
 
 VMAT_OK = 0
@@ -43,7 +43,8 @@ class _Info(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int64) for n in (
         "n_voxels", "n_beamlets", "nnz", "n_angles", "n_leaf_rows", "bytes_csr_d", "bytes_csr_dt",
         "bytes_device_total", "n_dose_blocks", "max_leaf_row_len", "max_voxel_row_nnz", "max_beamlet_row_nnz",
-        "index_bits_d", "index_bits_dt", "padded_d", "padded_dt", "bytes_stream_d", "bytes_stream_dt")]
+        "index_bits_d", "index_bits_dt", "padded_d", "padded_dt", "bytes_stream_d", "bytes_stream_dt",
+        "tiles_d", "tiles_uniform_d", "tiles_dt", "tiles_uniform_dt")]
 
 
 def load_library():

@@ -173,6 +173,8 @@ int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info)
     info->padded_d = h->D.P; info->padded_dt = h->Dt.P;
     info->bytes_stream_d = h->D.bytes() + 4 * ((int64_t)h->n_seg + 1);      // + the segment table
     info->bytes_stream_dt = h->Dt.bytes();
+    info->tiles_d = h->D.n_tiles; info->tiles_uniform_d = h->D.n_tiles_uniform;
+    info->tiles_dt = h->Dt.n_tiles; info->tiles_uniform_dt = h->Dt.n_tiles_uniform;
     return VMAT_OK;
 }
 
@@ -209,7 +211,7 @@ int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx
             int32_t prev = -1;
             for (int64_t q = pp[r]; q < pp[r + 1]; ++q) {
                 const int64_t sp = stored_pos(S, G, q);
-                const int32_t c = narrow ? pbase[q >> 5] + (int32_t)pi16[sp] : pi32[sp];
+                const int32_t c = narrow ? base_index(pbase[q >> 5]) + (int32_t)pi16[sp] : pi32[sp];
                 if (c <= prev) continue;                              // a pad
                 if (o >= ptr[r + 1]) { vmat_set_error("vmat_ddc_export_csr: layout inconsistent (row %d)", r); return VMAT_ERR_CUDA; }
                 idx[o] = c; val[o] = pv[sp]; prev = c; ++o;

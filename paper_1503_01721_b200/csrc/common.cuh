@@ -40,6 +40,7 @@ struct PackedLayout {
     int64_t nnz = 0;          // real entries
     int64_t P = 0;            // padded entries (multiple of 32)
     int index_bits = 32;      // 16 or 32
+    int64_t n_tiles = 0, n_tiles_uniform = 0;   // narrow: full tiles, and those with one base for all 8 groups
     int64_t *ptr = nullptr;   // [n_rows+1] canonical row pointers
     int64_t *pptr = nullptr;  // [n_rows+1] padded row starts; pptr[n_rows] = P
     float *val = nullptr;     // [P (+pad)]
@@ -59,6 +60,11 @@ struct MatView {
     const int32_t *base;
 };
 static inline MatView view_of(const PackedLayout &A) { return MatView{A.val, A.sec, A.base}; }
+// kernel variant for a layout (spmv.cuh: FMT_WIDE 0, FMT_NARROW 1, FMT_NARROW_1BASE 2)
+static inline int fmt_of(const PackedLayout &A)
+{
+    return A.index_bits != 16 ? 0 : (A.n_tiles_uniform == A.n_tiles ? 2 : 1);
+}
 
 // ------------------------------------------------------------------ the handle
 struct vmat_ddc {
@@ -105,6 +111,14 @@ struct vmat_ddc {
 #endif
 #ifndef VMAT_DOSE_MINB
 #define VMAT_DOSE_MINB 12
+#endif
+// Software pipelining of the tile loop (next tile's stream loads in flight while this tile gathers): measured on
+// B200, +9 % for the price kernel at 6 CTAs/SM; the dose kernel (12 CTAs of 4 warps) has no registers for it.
+#ifndef VMAT_PRICE_PIPELINE
+#define VMAT_PRICE_PIPELINE true
+#endif
+#ifndef VMAT_DOSE_PIPELINE
+#define VMAT_DOSE_PIPELINE false
 #endif
 constexpr int DOSE_THREADS = VMAT_DOSE_THREADS;
 constexpr int DOSE_SEG_NNZ = VMAT_DOSE_SEG_NNZ;   // a warp's run of short rows holds at most this many padded entries

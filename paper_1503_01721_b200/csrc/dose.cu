@@ -38,7 +38,7 @@ __device__ __forceinline__ double block_sum_double(double v, double *red /* [NT/
     return s;
 }
 
-template <bool FUSE, bool NARROW>
+template <bool FUSE, int FMT>
 __global__ void __launch_bounds__(DOSE_THREADS, VMAT_DOSE_MINB)
 k_dose(const int64_t *__restrict__ pptr, const MatView A, const int32_t *__restrict__ seg_row, int n_seg,
        const float *__restrict__ x, float *__restrict__ d,
@@ -64,25 +64,26 @@ k_dose(const int64_t *__restrict__ pptr, const MatView A, const int32_t *__restr
         const int64_t s = pptr[r0], e = pptr[r1];               // padded positions, multiples of 32
         if (nr == 1) {
             // ---- one row: register accumulation
-            const float acc = warp_sum(segment_dot<NARROW>(A, s, e, x, lane));
+            const float acc = warp_sum(segment_dot<FMT, VMAT_DOSE_PIPELINE>(A, s, e, x, lane));
             if (lane == 0) epilogue(r0, acc);
         } else {
             // ---- several short rows: products into this warp's slice at their padded position k - s ...
             float *wp = prod[warp];
             const int nt = (int)((e - s) >> 8);
+            TileCursor<FMT> tc(A, s, lane);
 #pragma unroll 1
-            for (int ti = 0; ti < nt; ++ti) {
-                const int64_t k = s + (int64_t)ti * TILE;
-                const Vec8 v = ld_stream_256(A.val + k + lane * 8);
+            for (int ti = 0; ti < nt; ++ti, tc.advance()) {
+                TileRegs<FMT> tr;
+                tile_load<FMT>(tc, tr);
                 int c[8];
-                tile_indices<NARROW>(A, k, lane, c);
+                tile_indices<FMT>(tc, tr, lane, c);
                 float *dst = wp + ti * TILE + lane;
 #pragma unroll
-                for (int t = 0; t < 8; ++t) dst[32 * t] = __uint_as_float(v.w[t]) * ld_gather(x + c[t]);
+                for (int t = 0; t < 8; ++t) dst[32 * t] = __uint_as_float(tr.v.w[t]) * ld_gather(x + c[t]);
             }
             const int64_t k0 = s + (int64_t)nt * TILE;
             float *dst = wp + nt * TILE + lane;
-            tail_foreach<NARROW>(A, k0, (int)((e - k0) >> 5), x, lane, [&](int t, float q) { dst[32 * t] = q; });
+            tail_foreach<FMT>(A, k0, (int)((e - k0) >> 5), x, lane, [&](int t, float q) { dst[32 * t] = q; });
             __syncwarp();
             // ... then G lanes per row, G = power of two near (mean row length)/4, 1..32
             const int mean = (int)((e - s) / nr);
@@ -145,14 +146,21 @@ int vmat_launch_dose(const vmat_ddc *h, const float *x, float *d, bool fuse,
     if (fuse && h->prof_ev[0]) VMAT_CUDA(cudaEventRecord(h->prof_ev[0], st));
     if (h->n_blocks > 0) {
         const MatView A = view_of(h->D);
-        const bool narrow = h->D.index_bits == 16;
-#define VMAT_DOSE_LAUNCH(FUSE_, NARROW_, ...)                                                           \
-        k_dose<FUSE_, NARROW_><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.pptr, A, h->seg_row, h->n_seg, x, d, __VA_ARGS__)
-        if (fuse && narrow)       VMAT_DOSE_LAUNCH(true, true, voxel_struct, T, w_over, w_under, g, h->F_partial);
-        else if (fuse)            VMAT_DOSE_LAUNCH(true, false, voxel_struct, T, w_over, w_under, g, h->F_partial);
-        else if (narrow)          VMAT_DOSE_LAUNCH(false, true, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
-        else                      VMAT_DOSE_LAUNCH(false, false, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr);
+#define VMAT_DOSE_LAUNCH(FUSE_, FMT_, ...)                                                              \
+        k_dose<FUSE_, FMT_><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.pptr, A, h->seg_row, h->n_seg, x, d, __VA_ARGS__)
+#define VMAT_DOSE_ARGS_FUSED voxel_struct, T, w_over, w_under, g, h->F_partial
+#define VMAT_DOSE_ARGS_PLAIN nullptr, nullptr, nullptr, nullptr, nullptr, nullptr
+        switch (fmt_of(h->D) + (fuse ? 3 : 0)) {
+        case 0: VMAT_DOSE_LAUNCH(false, FMT_WIDE, VMAT_DOSE_ARGS_PLAIN); break;
+        case 1: VMAT_DOSE_LAUNCH(false, FMT_NARROW, VMAT_DOSE_ARGS_PLAIN); break;
+        case 2: VMAT_DOSE_LAUNCH(false, FMT_NARROW_1BASE, VMAT_DOSE_ARGS_PLAIN); break;
+        case 3: VMAT_DOSE_LAUNCH(true, FMT_WIDE, VMAT_DOSE_ARGS_FUSED); break;
+        case 4: VMAT_DOSE_LAUNCH(true, FMT_NARROW, VMAT_DOSE_ARGS_FUSED); break;
+        default: VMAT_DOSE_LAUNCH(true, FMT_NARROW_1BASE, VMAT_DOSE_ARGS_FUSED); break;
+        }
 #undef VMAT_DOSE_LAUNCH
+#undef VMAT_DOSE_ARGS_FUSED
+#undef VMAT_DOSE_ARGS_PLAIN
         VMAT_LAUNCH_CHECK();
     }
     if (fuse && h->prof_ev[1]) VMAT_CUDA(cudaEventRecord(h->prof_ev[1], st));

@@ -244,6 +244,45 @@ k_pack(const int64_t *__restrict__ ptr, const int32_t *__restrict__ cidx, const 
     }
 }
 
+// Narrow layouts, after the pack: every full tile whose 256 indices span <= 65535 gets ONE base (its minimum)
+// for all 8 groups, flagged in bit 31 of the tile's first base word (spmv.cuh: the kernels then read one
+// broadcast word per tile instead of shuffling 8 bases around).  One warp per segment.
+__global__ void __launch_bounds__(256)
+k_tile_base(const int64_t *__restrict__ pptr, const int32_t *__restrict__ seg_row, int n_seg,
+            uint16_t *__restrict__ off, int32_t *__restrict__ base, unsigned long long *__restrict__ n_tiles /* [2]: all, uniform */)
+{
+    const int w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (w >= n_seg) return;
+    const int r0 = seg_row ? seg_row[w] : w, r1 = seg_row ? seg_row[w + 1] : w + 1;
+    const int64_t s = pptr[r0], e = pptr[r1];
+    const int nt = (int)((e - s) >> 8);
+    int n_uniform = 0;
+    for (int ti = 0; ti < nt; ++ti) {
+        const int64_t k = s + (int64_t)ti * TILE;
+        int c[8], mn = INT32_MAX, mx = INT32_MIN;
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {                              // stored word 8*lane + t = entry `lane` of group t
+            c[t] = base[(k >> 5) + t] + (int)off[k + 8 * lane + t];
+            mn = min(mn, c[t]); mx = max(mx, c[t]);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+            mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        }
+        if ((int64_t)mx - (int64_t)mn > 65535) continue;           // warp-uniform
+#pragma unroll
+        for (int t = 0; t < 8; ++t) off[k + 8 * lane + t] = (uint16_t)(c[t] - mn);
+        __syncwarp();
+        if (lane < 8) base[(k >> 5) + lane] = lane == 0 ? (mn | TILE_UNIFORM_BIT) : mn;
+        ++n_uniform;
+    }
+    if (lane == 0 && nt > 0) {
+        atomicAdd(n_tiles + 0, (unsigned long long)nt);
+        atomicAdd(n_tiles + 1, (unsigned long long)n_uniform);
+    }
+}
+
 constexpr int SORT_SMALL = 2048;       // 16 KB of keys, 256 threads
 constexpr int SORT_BIG = 24576;        // 192 KB of keys, 1024 threads
 
@@ -401,6 +440,20 @@ static int pack_layout(vmat_ddc *h, PackedLayout &A, const CanonCsr &C, int32_t 
         VMAT_LAUNCH_CHECK();
     }
     VMAT_CUDA(cudaMemcpyAsync(A.pptr + A.n_rows, &A.P, 8, cudaMemcpyHostToDevice, st));
+    if (use_narrow && pl.n_seg > 0) {
+        unsigned long long *d_nt = nullptr, h_nt[2] = {0, 0};
+        DevGuard g2;
+        g2.add((void **)&d_nt);
+        int64_t dummy = 0;
+        TRY(dev_alloc(&d_nt, 2, &dummy));
+        VMAT_CUDA(cudaMemsetAsync(d_nt, 0, 16, st));
+        k_tile_base<<<(pl.n_seg + 7) / 8, 256, 0, st>>>(A.pptr, pl.d_seg, pl.n_seg, (uint16_t *)A.sec, A.base, d_nt);
+        VMAT_LAUNCH_CHECK();
+        VMAT_CUDA(cudaMemcpyAsync(h_nt, d_nt, 16, cudaMemcpyDeviceToHost, st));
+        VMAT_CUDA(cudaStreamSynchronize(st));
+        A.n_tiles = (int64_t)h_nt[0];
+        A.n_tiles_uniform = (int64_t)h_nt[1];
+    }
     VMAT_CUDA(cudaStreamSynchronize(st));
     if (chosen) {                                               // hand the segment table to the caller
         chosen->seg = pl.seg; chosen->n_seg = pl.n_seg; chosen->d_seg = pl.d_seg; pl.d_seg = nullptr;

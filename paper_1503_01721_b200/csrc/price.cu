@@ -112,7 +112,7 @@ struct SelectArgs {
 #ifndef VMAT_PRICE_MINB
 #define VMAT_PRICE_MINB 6        // 40 registers, 1536 threads per SM: fastest of 4..8 on B200 (cfg 3)
 #endif
-template <bool SELECT, bool NARROW>
+template <bool SELECT, int FMT>
 __global__ void __launch_bounds__(PRICE_THREADS, VMAT_PRICE_MINB)
 k_price(const int64_t *__restrict__ pptr, const MatView A, int n_rows, const float *__restrict__ g,
         float *__restrict__ p, SelectArgs sa)
@@ -127,7 +127,7 @@ k_price(const int64_t *__restrict__ pptr, const MatView A, int n_rows, const flo
     const int warp = threadIdx.x >> 5;
     const int row = blockIdx.x * PRICE_WARPS + warp;
     if (row < n_rows) {
-        const float acc = warp_sum(segment_dot<NARROW>(A, pptr[row], pptr[row + 1], g, lane));
+        const float acc = warp_sum(segment_dot<FMT, VMAT_PRICE_PIPELINE>(A, pptr[row], pptr[row + 1], g, lane));
         if (lane == 0) p[row] = acc;
     }
     if (SELECT) {
@@ -265,14 +265,22 @@ k_angle_price(int n_angles, const int32_t *__restrict__ angle_row_offset, const 
 }
 
 // ---------------------------------------------------------------- launchers
+template <bool SELECT>
+static void launch_k_price(const vmat_ddc *h, int grid, const float *g, float *p, const SelectArgs &sa, cudaStream_t st)
+{
+    const MatView A = view_of(h->Dt);
+    switch (fmt_of(h->Dt)) {
+    case 0: k_price<SELECT, FMT_WIDE><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
+    case 1: k_price<SELECT, FMT_NARROW><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
+    default: k_price<SELECT, FMT_NARROW_1BASE><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
+    }
+}
+
 int vmat_launch_price(const vmat_ddc *h, const float *g, float *p, cudaStream_t st)
 {
     if (h->n_beamlets == 0) return VMAT_OK;
     const int grid = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
-    if (h->Dt.index_bits == 16)
-        k_price<false, true><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, view_of(h->Dt), h->n_beamlets, g, p, SelectArgs{});
-    else
-        k_price<false, false><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, view_of(h->Dt), h->n_beamlets, g, p, SelectArgs{});
+    launch_k_price<false>(h, grid, g, p, SelectArgs{}, st);
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }
@@ -299,10 +307,7 @@ int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *a
     }
     SelectArgs sa{h->beamlet_leafrow, h->leafrow_col_offset, h->leafrow_angle, angle_mask, h->leafrow_done,
                   h->S_scratch, L, R, row_price, h->n_leaf_rows};
-    if (h->Dt.index_bits == 16)
-        k_price<true, true><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, view_of(h->Dt), h->n_beamlets, g, p, sa);
-    else
-        k_price<true, false><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, view_of(h->Dt), h->n_beamlets, g, p, sa);
+    launch_k_price<true>(h, grid, g, p, sa, st);
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }

@@ -29,6 +29,10 @@
 
 constexpr int GROUP = 32;
 constexpr int TILE = 256;
+// Kernel variants by index format: int32 indices; u16 offsets with the per-tile check of the base flag; u16
+// offsets of a layout in which EVERY full tile has one base (no check, no shuffle path compiled in).
+enum { FMT_WIDE = 0, FMT_NARROW = 1, FMT_NARROW_1BASE = 2 };
+
 
 // Stored position of padded logical position q of a segment that starts at S and holds G groups.
 __host__ __device__ __forceinline__ int64_t stored_pos(int64_t S, int64_t G, int64_t q)
@@ -37,50 +41,99 @@ __host__ __device__ __forceinline__ int64_t stored_pos(int64_t S, int64_t G, int
     return gl < (G & ~int64_t(7)) ? S + ((gl >> 3) << 8) + 8 * slot + (gl & 7) : q;
 }
 
-// Secondary indices of this lane's 8 entries of the tile at padded position k (entry `lane` of groups 0..7).
-template <bool NARROW>
-__device__ __forceinline__ void tile_indices(const MatView &A, int64_t k, int lane, int (&c)[8])
+// Base word of a group: the group's base index; bit 31 of the FIRST group of a full tile set = all 8 groups of
+// the tile share this base (written by the ingest step whenever the tile's indices span <= 65535, which is
+// the rule for these matrices): the warp then needs one broadcast load per tile instead of one base per group.
+constexpr int TILE_UNIFORM_BIT = int(0x80000000u);
+__host__ __device__ __forceinline__ int base_index(int word) { return word & 0x7fffffff; }
+
+// Per-lane stream pointers into a segment's interleaved tiles; advance() steps to the next tile.
+template <int FMT>
+struct TileCursor {
+    const float *v;          // this lane's 8 values of the tile
+    const char *i;           // this lane's 8 offsets (u16) or indices (i32)
+    const int32_t *b;        // the tile's 8 base words (narrow only)
+    __device__ __forceinline__ TileCursor(const MatView &A, int64_t s, int lane)
+        : v(A.val + s + lane * 8), i((const char *)A.sec + (s + lane * 8) * (FMT != FMT_WIDE ? 2 : 4)),
+          b(FMT != FMT_WIDE ? A.base + (s >> 5) : nullptr) {}
+    __device__ __forceinline__ void advance()
+    {
+        v += TILE;
+        i += TILE * (FMT != FMT_WIDE ? 2 : 4);
+        if (FMT != FMT_WIDE) b += TILE / GROUP;
+    }
+};
+
+// This lane's share of one tile's streams, in registers: loading and using are separate steps so that a loop
+// can have the next tile's loads in flight while it gathers for the current one.
+template <int FMT>
+struct TileRegs {
+    Vec8 v;                  // 8 values
+    Vec8 o;                  // wide: 8 int32 indices; narrow: o.w[0..3] = 8 u16 offsets, o.w[4] = the tile's base word
+};
+template <int FMT>
+__device__ __forceinline__ void tile_load(const TileCursor<FMT> &tc, TileRegs<FMT> &r)
 {
-    if (NARROW) {
-        const Vec4 o = ld_stream_128((const uint16_t *)A.sec + k + lane * 8);
-        const int b = ld_stream_i(A.base + (k >> 5) + (lane & 7));        // the tile's 8 bases, one 32-byte line
-#pragma unroll
-        for (int t = 0; t < 8; ++t) {
-            const int bt = __shfl_sync(0xffffffffu, b, t);
-            c[t] = bt + (int)((t & 1) ? (o.w[t >> 1] >> 16) : (o.w[t >> 1] & 0xffffu));
-        }
+    r.v = ld_stream_256(tc.v);
+    if (FMT != FMT_WIDE) {
+        const Vec4 o = ld_stream_128(tc.i);
+        r.o.w[0] = o.w[0]; r.o.w[1] = o.w[1]; r.o.w[2] = o.w[2]; r.o.w[3] = o.w[3];
+        r.o.w[4] = (uint32_t)ld_stream_i(tc.b);                             // broadcast: one 128-byte wavefront
     } else {
-        const Vec8 o = ld_stream_256((const int32_t *)A.sec + k + lane * 8);
-#pragma unroll
-        for (int t = 0; t < 8; ++t) c[t] = (int)o.w[t];
+        r.o = ld_stream_256(tc.i);
     }
 }
 
-// One interleaved tile at padded position k: this lane's partial of sum val*vec[idx].
-template <bool NARROW>
-__device__ __forceinline__ float tile_dot(const MatView &A, int64_t k, const float *__restrict__ vec, int lane)
+// Secondary indices of this lane's 8 entries of the tile (entry `lane` of groups 0..7).
+template <int FMT>
+__device__ __forceinline__ void tile_indices(const TileCursor<FMT> &tc, const TileRegs<FMT> &r, int lane, int (&c)[8])
 {
-    const Vec8 v = ld_stream_256(A.val + k + lane * 8);
+    if (FMT != FMT_WIDE) {
+        const int b0 = (int)r.o.w[4];
+        if (FMT == FMT_NARROW_1BASE || b0 < 0) {                            // warp-uniform branch
+            const int bb = base_index(b0);
+#pragma unroll
+            for (int t = 0; t < 8; ++t)
+                c[t] = bb + (int)((t & 1) ? (r.o.w[t >> 1] >> 16) : (r.o.w[t >> 1] & 0xffffu));
+        } else {                                                            // one base per group, by shuffles
+            const int b = ld_stream_i(tc.b + (lane & 7));
+#pragma unroll
+            for (int t = 0; t < 8; ++t) {
+                const int bt = __shfl_sync(0xffffffffu, b, t);
+                c[t] = bt + (int)((t & 1) ? (r.o.w[t >> 1] >> 16) : (r.o.w[t >> 1] & 0xffffu));
+            }
+        }
+    } else {
+#pragma unroll
+        for (int t = 0; t < 8; ++t) c[t] = (int)r.o.w[t];
+    }
+}
+
+// One interleaved tile: this lane's partial of sum val*vec[idx].
+template <int FMT>
+__device__ __forceinline__ float tile_dot(const TileCursor<FMT> &tc, const TileRegs<FMT> &r,
+                                          const float *__restrict__ vec, int lane)
+{
     int c[8];
-    tile_indices<NARROW>(A, k, lane, c);
+    tile_indices<FMT>(tc, r, lane, c);
     float acc = 0.f;
 #pragma unroll
-    for (int t = 0; t < 8; ++t) acc = fmaf(__uint_as_float(v.w[t]), ld_gather(vec + c[t]), acc);
+    for (int t = 0; t < 8; ++t) acc = fmaf(__uint_as_float(r.v.w[t]), ld_gather(vec + c[t]), acc);
     return acc;
 }
 
 // Entry `lane` of the plain-order group at padded position kg: value and secondary index.
-template <bool NARROW>
+template <int FMT>
 __device__ __forceinline__ void group_entry(const MatView &A, int64_t kg, int lane, float &v, int &c)
 {
     v = ld_stream_f(A.val + kg + lane);
-    if (NARROW) c = ld_stream_i(A.base + (kg >> 5)) + ld_stream_u16((const uint16_t *)A.sec + kg + lane);
+    if (FMT != FMT_WIDE) c = base_index(ld_stream_i(A.base + (kg >> 5))) + ld_stream_u16((const uint16_t *)A.sec + kg + lane);
     else        c = ld_stream_i((const int32_t *)A.sec + kg + lane);
 }
 
 // The ngt (0..7) plain-order groups after the last full tile, starting at padded position k0:
 // calls f(t, product) for this lane's entry of group t.  Four groups' loads are issued together.
-template <bool NARROW, typename F>
+template <int FMT, typename F>
 __device__ __forceinline__ void tail_foreach(const MatView &A, int64_t k0, int ngt, const float *__restrict__ vec,
                                              int lane, F f)
 {
@@ -92,7 +145,7 @@ __device__ __forceinline__ void tail_foreach(const MatView &A, int64_t k0, int n
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             v[i] = 0.f; c[i] = 0;
-            if (t0 + i < ngt) group_entry<NARROW>(A, k0 + 32 * (t0 + i), lane, v[i], c[i]);
+            if (t0 + i < ngt) group_entry<FMT>(A, k0 + 32 * (t0 + i), lane, v[i], c[i]);
         }
 #pragma unroll
         for (int i = 0; i < 4; ++i)
@@ -101,16 +154,40 @@ __device__ __forceinline__ void tail_foreach(const MatView &A, int64_t k0, int n
 }
 
 // A whole segment [s, e) (padded positions, multiples of 32) as one dot product: this lane's partial.
-template <bool NARROW>
+// PIPELINE: the next tile's stream loads are issued before this tile's gathers (13 more live registers).
+template <int FMT, bool PIPELINE>
 __device__ __forceinline__ float segment_dot(const MatView &A, int64_t s, int64_t e, const float *__restrict__ vec,
                                              int lane)
 {
     const int nt = (int)((e - s) >> 8);
     float acc = 0.f;
+    TileCursor<FMT> tc(A, s, lane);
+    if (PIPELINE) {
+        if (nt > 0) {
+            TileRegs<FMT> cur;
+            tile_load<FMT>(tc, cur);
 #pragma unroll 1
-    for (int ti = 0; ti < nt; ++ti) acc += tile_dot<NARROW>(A, s + (int64_t)ti * TILE, vec, lane);
+            for (int ti = 1; ti < nt; ++ti) {
+                TileCursor<FMT> tn = tc;
+                tn.advance();
+                TileRegs<FMT> nxt;
+                tile_load<FMT>(tn, nxt);
+                acc += tile_dot<FMT>(tc, cur, vec, lane);
+                cur = nxt;
+                tc = tn;
+            }
+            acc += tile_dot<FMT>(tc, cur, vec, lane);
+        }
+    } else {
+#pragma unroll 1
+        for (int ti = 0; ti < nt; ++ti, tc.advance()) {
+            TileRegs<FMT> r;
+            tile_load<FMT>(tc, r);
+            acc += tile_dot<FMT>(tc, r, vec, lane);
+        }
+    }
     const int64_t k0 = s + (int64_t)nt * TILE;
-    tail_foreach<NARROW>(A, k0, (int)((e - k0) >> 5), vec, lane, [&](int, float q) { acc += q; });
+    tail_foreach<FMT>(A, k0, (int)((e - k0) >> 5), vec, lane, [&](int, float q) { acc += q; });
     return acc;
 }
 

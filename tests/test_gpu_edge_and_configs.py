@@ -167,6 +167,8 @@ def test_index_spans_beyond_16_bits(vm):
     assert info["index_bits_d"] == 32                                       # padding would outweigh the saving
     h16 = ddc_from_arrays(A, DEV, index_bits=16)
     assert h16.info["padded_d"] > 1.2 * info["padded_d"]                    # groups were closed early
+    # both tile kinds occur: one base per tile (span <= 65535: the 9000-entry row) and one base per group
+    assert 0 < h16.info["tiles_uniform_d"] < h16.info["tiles_d"]
     h16.close()
     assert (ev.g > 0).any() and (ev.g < 0).any() and (ev.R > ev.L).any()
 
