@@ -95,13 +95,13 @@ class ClockSampler:
 
 
 def ncu_capture_file(index_bits: int) -> str:
-    """The committed ncu --set full capture of config 3 for the layout in use (u16 offsets: v5, int32: v4)."""
-    return "r1_ncu_full_cfg3_v5.csv" if index_bits == 16 else "r1_ncu_full_cfg3_v4.csv"
+    """The committed ncu --set full capture of config 3 for the layout in use (u16 offsets: v6, int32: v4)."""
+    return "r1_ncu_full_cfg3_v6.csv" if index_bits == 16 else "r1_ncu_full_cfg3_v4.csv"
 
 
 def ncu_traffic(kernel_prefix: str, cfg: int, scale: float, index_bits: int):
     """dram bytes (read + write) per launch of the dominant kernel from the committed ncu --set full capture
-    (profiles/r1_ncu_full_cfg3_v{4,5}.csv, config 3 only); None for other workloads."""
+    (profiles/r1_ncu_full_cfg3_v{4,6}.csv, config 3 only); None for other workloads."""
     if cfg != 3 or scale != 1.0:
         return None
     try:
