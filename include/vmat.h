@@ -174,6 +174,45 @@ int vmat_price_eval_host(vmat_ddc *h, const float *x_host,
 int vmat_aperture_dose(const vmat_ddc *h, int32_t angle, const int32_t *L, const int32_t *R,
                        float *x_scratch, float *DA, void *stream);
 
+/* ------------------------------------------------------------------------------------------------------
+ * NEXT-2: the master problem (MP), Eq. (6)-(10) L70-L101 and the four BB steps of L139.
+ * With the apertures chosen so far and their dose vectors DA(A_k) (Eq. (5)), find fluence rates
+ * y_k in [y_lo_k, y_hi_k] (Eq. (6): R^L/S^U_k and R^U/S^L_k, supplied by the caller) minimising F(z),
+ * z = sum_k DA(A_k) y_k, by the Barzilai-Borwein iteration: step sizes Eq. (7) and Eq. (8) alternately,
+ * subspace step rule Eq. (9)/(10), three stopping rules (L101).  Readings C15-C20 of DESIGN.md:
+ * g_A = +dF/dy and y <- y - delta g_A; a variable at its lower (upper) bound with g_A > 0 (< 0) is held and
+ * its gradient entry zeroed; y is clipped into the box after every update; first step = exact line minimiser
+ * of the current quadratic piece; iteration 1, 3, .. use Eq. (7), 2, 4, .. Eq. (8), the previous delta is kept
+ * when <s,t> <= 0; z is recomputed as DA y every iteration.
+ * The handle owns a dense voxel-major copy of the aperture dose vectors (float [n_voxels][max_apertures],
+ * max_apertures <= 384) and the FP64 iteration state; y persists between solves (warm start, as in the
+ * column-generation loop L56).  All sums are FP64 in a fixed order: results are deterministic. */
+typedef struct vmat_mp vmat_mp;
+int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void *stream);
+int vmat_mp_destroy(vmat_mp *h);
+/* Forgets every aperture (the storage is kept). */
+int vmat_mp_reset(vmat_mp *h);
+/* Appends aperture k = current count: DA dev float [n_voxels] (e.g. from vmat_aperture_dose), its starting
+ * fluence rate y0 (clipped into the box) and bounds.  Synchronises the stream. */
+int vmat_mp_add_aperture(vmat_mp *h, const float *DA, double y0, double y_lo, double y_hi, void *stream);
+/* Overwrites the fluence rates of the current apertures (y_host host double [count]); clipped by the solve. */
+int vmat_mp_set_fluence(vmat_mp *h, const double *y_host, void *stream);
+int vmat_mp_size(const vmat_mp *h, int32_t *n_apertures, int32_t *max_apertures /* host, out, may be NULL */);
+/* Runs the BB iteration from the handle's current y until a stopping rule fires (tested at the top of every
+ * iteration, in this order):  reason 1 "stationary": every entry of g_A is 0 after the subspace rule;
+ * 2 "objective": it >= 5 and |F(j) - F(j-1)| <= eps_F |F(j-1)| for the five latest j;  3 "step": it >= 1 and
+ * max_k |y_k(it) - y_k(it-1)| <= eps_y;  4: it == max_iter.  The iterate at which the rule fired is returned.
+ *   voxel_struct, T, w_over, w_under: the objective, as for vmat_objective_grad (device pointers);
+ *   z dev float [n_voxels] out or NULL: the dose z = DA y of the returned iterate;
+ *   y_host double [count], F_host, n_iter_host, reason_host: host, out, each may be NULL.
+ * Synchronous: the stream is synchronised every 8 iterations to read the stop flag. */
+int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, const float *T, const float *w_over,
+                  const float *w_under, int32_t max_iter, double eps_F, double eps_y, float *z, double *y_host,
+                  double *F_host, int32_t *n_iter_host, int32_t *reason_host, void *stream);
+/* Trace of the last solve: F_hist host double [n_iter + 1] (objective at iterate 0 .. n_iter), delta_hist host
+ * double [n_iter] (step size used to leave iterate it); either may be NULL. */
+int vmat_mp_history(const vmat_mp *h, double *F_hist, double *delta_hist);
+
 /* Profiling hook for bench.py's roofline: four CUDA events (cudaEvent_t passed as void*, any may be NULL)
  * that every following vmat_price_eval / vmat_price_eval_host on this handle records on its stream:
  * ev[0] just before and ev[1] just after the dose(+objective) kernel, ev[2] just before and ev[3] just

@@ -30,6 +30,8 @@ EXPORTS = [
     "vmat_ddc_create", "vmat_ddc_create_ex", "vmat_ddc_destroy", "vmat_ddc_info_get", "vmat_ddc_export_csr", "vmat_dose",
     "vmat_objective_grad", "vmat_price", "vmat_select_apertures", "vmat_price_eval", "vmat_price_eval_host",
     "vmat_aperture_dose", "vmat_ddc_set_profile_events", "vmat_last_error", "vmat_last_launch_count",
+    "vmat_mp_create", "vmat_mp_destroy", "vmat_mp_reset", "vmat_mp_add_aperture", "vmat_mp_set_fluence", "vmat_mp_size",
+    "vmat_mp_solve", "vmat_mp_history",
 ]
 
 
@@ -70,6 +72,15 @@ def load_library():
     lib.vmat_price_eval_host.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_aperture_dose.argtypes = [vp, i32, vp, vp, vp, vp, vp]
     lib.vmat_ddc_set_profile_events.argtypes = [vp, vp]
+    f64 = ctypes.c_double
+    lib.vmat_mp_create.argtypes = [ctypes.POINTER(vp), i32, i32, vp]
+    lib.vmat_mp_destroy.argtypes = [vp]
+    lib.vmat_mp_reset.argtypes = [vp]
+    lib.vmat_mp_add_aperture.argtypes = [vp, vp, f64, f64, f64, vp]
+    lib.vmat_mp_set_fluence.argtypes = [vp, vp, vp]
+    lib.vmat_mp_size.argtypes = [vp, vp, vp]
+    lib.vmat_mp_solve.argtypes = [vp, vp, i32, vp, vp, vp, i32, f64, f64, vp, vp, vp, vp, vp, vp]
+    lib.vmat_mp_history.argtypes = [vp, vp, vp]
     lib.vmat_last_error.restype = ctypes.c_char_p
     lib.vmat_last_launch_count.restype = ctypes.c_int
     for name in EXPORTS:
@@ -283,6 +294,79 @@ def vmat_aperture_dose(h: DDC, angle: int, L: torch.Tensor, R: torch.Tensor, x_s
     _check(load_library().vmat_aperture_dose(
         h._h, int(angle), _ptr(L, torch.int32, "cuda", h.n_leaf_rows), _ptr(R, torch.int32, "cuda", h.n_leaf_rows),
         _ptr(x_scratch, torch.float32, "cuda", h.n_beamlets), _ptr(DA, torch.float32, "cuda", h.n_voxels), _stream()))
+
+
+MP_STOP_REASONS = {1: "stationary", 2: "objective", 3: "step", 4: "max_iter"}
+
+
+@dataclass
+class MPSolution:
+    y: torch.Tensor            # float64 [n_apertures], host
+    F: float
+    n_iter: int
+    reason: int                # 1 stationary, 2 objective, 3 step, 4 max_iter
+
+
+class MasterProblem:
+    """Owns a vmat_mp handle: the aperture dose vectors chosen so far and the BB iteration state (NEXT-2;
+    PAPER.md Eq. (6)-(10))."""
+
+    def __init__(self, n_voxels: int, max_apertures: int, device="cuda:0"):
+        if not torch.cuda.is_available():
+            raise RuntimeError("vmat_mp_create needs a CUDA device (there is no CPU fallback)")
+        self.device = torch.device(device)
+        self.n_voxels = int(n_voxels)
+        out = ctypes.c_void_p()
+        with torch.cuda.device(self.device):
+            _check(load_library().vmat_mp_create(ctypes.byref(out), self.n_voxels, int(max_apertures), _stream()))
+        self._h = out
+
+    def close(self):
+        if self._h is not None and self._h.value:
+            load_library().vmat_mp_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def n_apertures(self) -> int:
+        n = ctypes.c_int32()
+        _check(load_library().vmat_mp_size(self._h, ctypes.byref(n), None))
+        return int(n.value)
+
+    def reset(self):
+        _check(load_library().vmat_mp_reset(self._h))
+
+    def add_aperture(self, DA: torch.Tensor, y0: float, y_lo: float, y_hi: float):
+        _check(load_library().vmat_mp_add_aperture(self._h, _ptr(DA, torch.float32, "cuda", self.n_voxels),
+                                                   float(y0), float(y_lo), float(y_hi), _stream()))
+
+    def set_fluence(self, y: torch.Tensor):
+        _check(load_library().vmat_mp_set_fluence(self._h, _ptr(y, torch.float64, "cpu", self.n_apertures), _stream()))
+
+    def solve(self, obj: Objective, max_iter: int = 200, eps_F: float = 1e-6, eps_y: float = 1e-9,
+              z: Optional[torch.Tensor] = None) -> MPSolution:
+        y = torch.empty(self.n_apertures, dtype=torch.float64)
+        F, n_iter, reason = ctypes.c_double(), ctypes.c_int32(), ctypes.c_int32()
+        _check(load_library().vmat_mp_solve(
+            self._h, _ptr(obj.voxel_struct, torch.uint8, "cuda", self.n_voxels), obj.n_struct,
+            _ptr(obj.T, torch.float32, "cuda"), _ptr(obj.w_over, torch.float32, "cuda"),
+            _ptr(obj.w_under, torch.float32, "cuda"), int(max_iter), float(eps_F), float(eps_y),
+            _ptr(z, torch.float32, "cuda", self.n_voxels), y.data_ptr(), ctypes.addressof(F),
+            ctypes.addressof(n_iter), ctypes.addressof(reason), _stream()))
+        self._last_n_iter = int(n_iter.value)
+        return MPSolution(y, float(F.value), int(n_iter.value), int(reason.value))
+
+    def history(self):
+        """(F_hist float64 [n_iter+1], delta_hist float64 [n_iter]) of the last solve, on the host."""
+        Fh = torch.empty(self._last_n_iter + 1, dtype=torch.float64)
+        dh = torch.empty(self._last_n_iter, dtype=torch.float64)
+        _check(load_library().vmat_mp_history(self._h, Fh.data_ptr(), dh.data_ptr() if dh.numel() else None))
+        return Fh, dh
 
 
 def last_launch_count() -> int:

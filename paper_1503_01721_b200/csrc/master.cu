@@ -1,0 +1,443 @@
+// master.cu - NEXT-2: the master problem (MP) of the column-generation loop, Eq. (6)-(10) L70-L101
+// and the four BB steps of L139: fluence rates y_k in [lo_k, hi_k] of the apertures chosen so far that minimise
+// F(z), z = sum_k DA(A_k) y_k, by the Barzilai-Borwein iteration with the subspace step rule.
+// Readings C15-C20: DESIGN.md section 2.
+//
+// Storage: DA is dense, VOXEL-MAJOR, float [n_voxels][m_cap] (the paper's aperture dose vectors are "dense-ish",
+// <= 0.15 % of the DDC matrix, L264).  One BB iteration then needs ONE pass over DA: a group of G lanes owns a
+// voxel row, its lanes hold the row's entries in registers, the row dot gives z_i (step 4 of L139), the
+// voxel's gradient follows (Eq. (1)), and every lane adds DA_ik * dF/dz_i to its own entries of the aperture
+// gradient g_A (step 1) - no second read, no atomics.  HBM-bound: 4 m n_voxels bytes per iteration.
+// All sums are FP64 in a fixed order (FP32 storage of DA, T, weights): deterministic, and a trajectory differs
+// from the FP64 oracle's by summation order only.
+#include "common.cuh"
+#include <new>
+#include <vector>
+
+constexpr int MP_THREADS = 256;
+constexpr int MP_WARPS = MP_THREADS / 32;
+constexpr int MP_MAX_NC = 12;                 // up to 12 x 32 = 384 apertures
+constexpr int MP_HIST = 6;                    // objective values the "last five changes" rule looks at
+
+struct MpState {                              // device-resident scalars of one solve
+    int it;                                   // iteration counter
+    int reason;                               // 0 running, 1 stationary, 2 objective, 3 step, 4 max_iter (C19)
+    int max_iter;
+    double eps_F, eps_y;
+    double delta;                             // last step size
+    double F;                                 // objective at the current iterate
+    double Fh[MP_HIST];                       // F(it), F(it-1), ...
+};
+
+struct vmat_mp {
+    int32_t n_voxels = 0, m_cap = 0, m = 0;
+    int n_cta = 0, device = 0;
+    float *DA = nullptr;                      // [n_voxels][m_cap]
+    double *y = nullptr, *y_prev = nullptr, *g = nullptr, *g_prev = nullptr, *lo = nullptr, *hi = nullptr;   // [m_cap]
+    double *gpart = nullptr;                  // [n_cta][m_cap]
+    double *spart = nullptr;                  // [n_cta][2]: F partial, curvature partial
+    MpState *st = nullptr;
+    double *F_hist = nullptr, *delta_hist = nullptr;   // [hist_cap + 1]
+    int32_t hist_cap = 0;
+    int32_t last_n_iter = 0;
+};
+
+__device__ __forceinline__ double shfl_xor_d(double v, int o) { return __shfl_xor_sync(0xffffffffu, v, o); }
+
+// deterministic block sum of doubles (MP_THREADS threads); result valid in every thread
+__device__ __forceinline__ double mp_block_sum(double v, double *red /* [MP_WARPS + 1] */)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += shfl_xor_d(v, o);
+    __syncthreads();                                         // red may still be read from the previous call
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int i = 0; i < MP_WARPS; ++i) s += red[i];
+        red[MP_WARPS] = s;
+    }
+    __syncthreads();
+    return red[MP_WARPS];
+}
+
+__global__ void k_mp_set_column(int n_voxels, int m_cap, int k, const float *__restrict__ col, float *__restrict__ DA)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_voxels) DA[(size_t)i * m_cap + k] = col[i];
+}
+
+__global__ void k_mp_clip(int m, double *__restrict__ y, const double *__restrict__ lo, const double *__restrict__ hi)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < m) y[k] = fmin(fmax(y[k], lo[k]), hi[k]);
+}
+
+// ---------------------------------------------------------------- the pass over DA
+// CURV = false: z = DA y, F, dF/dz, partials of g_A = DA^T dF/dz            (steps 4 and 1 of L139)
+// CURV = true : z = DA y, q = DA g, partials of sum_i w_i q_i^2              (first step size, C17)
+// G lanes per voxel row (G = 32 when m >= 32, else the power of two >= m), NC chunks of G entries per row.
+template <int NC, bool CURV>
+__global__ void __launch_bounds__(MP_THREADS)
+k_mp_pass(int n_voxels, int m, int m_cap, int G, const float *__restrict__ DA,
+          const double *__restrict__ y, const double *__restrict__ gvec,
+          const uint8_t *__restrict__ vstruct, const float *__restrict__ T, const float *__restrict__ w_over,
+          const float *__restrict__ w_under, float *__restrict__ z_out,
+          double *__restrict__ gpart, double *__restrict__ spart, const MpState *__restrict__ st)
+{
+    if (st->reason != 0) return;                              // the solve has stopped: nothing to do
+    __shared__ double red[MP_WARPS][MP_MAX_NC * 32];
+    __shared__ double red_s[MP_WARPS + 1];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int gl = lane % G, sub = lane / G, rows_per_warp = 32 / G;
+    double yk[NC], acc[NC];
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        const int k = c * G + gl;
+        yk[c] = k < m ? y[k] : 0.0;
+        acc[c] = CURV ? (k < m ? gvec[k] : 0.0) : 0.0;        // CURV: acc holds g_A's entries (read only)
+    }
+    double ssum = 0.0;
+    const int n_warps = gridDim.x * MP_WARPS;
+    const int n_iter = (n_voxels + n_warps * rows_per_warp - 1) / (n_warps * rows_per_warp);   // uniform trip count
+    for (int itr = 0; itr < n_iter; ++itr) {
+        const int i = (itr * n_warps + blockIdx.x * MP_WARPS + warp) * rows_per_warp + sub;
+        const bool live = i < n_voxels;
+        float a[NC];
+        double zi = 0.0, qi = 0.0;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const int k = c * G + gl;
+            a[c] = (live && k < m) ? __ldg(DA + (size_t)i * m_cap + k) : 0.f;
+            zi = fma((double)a[c], yk[c], zi);
+            if (CURV) qi = fma((double)a[c], acc[c], qi);
+        }
+        for (int o = G >> 1; o > 0; o >>= 1) {               // row sums over the group's G lanes
+            zi += shfl_xor_d(zi, o);
+            if (CURV) qi += shfl_xor_d(qi, o);
+        }
+        if (live) {
+            const int sid = vstruct[i];
+            const double Ti = (double)__ldg(T + sid), wo = (double)__ldg(w_over + sid), wu = (double)__ldg(w_under + sid);
+            if (!CURV) {
+                const double over = fmax(zi - Ti, 0.0), under = fmax(Ti - zi, 0.0);
+                const double gz = 2.0 * wo * over - 2.0 * wu * under;                    // Eq. (1), sign C1
+                if (gl == 0) {
+                    ssum += wo * over * over + wu * under * under;
+                    if (z_out) z_out[i] = (float)zi;
+                }
+#pragma unroll
+                for (int c = 0; c < NC; ++c) acc[c] = fma((double)a[c], gz, acc[c]);     // g_A += DA_i: * dF/dz_i
+            } else if (gl == 0) {
+                const double w = zi > Ti ? wo : (zi < Ti ? wu : 0.0);                    // C17
+                ssum += w * qi * qi;
+            }
+        }
+    }
+    // ---- CTA partials in a fixed order: lanes with the same gl (rows handled side by side), then the warps
+    if (!CURV) {
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            double v = acc[c];
+            for (int o = G; o < 32; o <<= 1) v += shfl_xor_d(v, o);
+            if (sub == 0) red[warp][c * G + gl] = v;
+        }
+        __syncthreads();
+        for (int k = threadIdx.x; k < NC * G; k += MP_THREADS) {
+            double s = 0.0;
+            for (int w = 0; w < MP_WARPS; ++w) s += red[w][k];
+            if (k < m) gpart[(size_t)blockIdx.x * m_cap + k] = s;
+        }
+    }
+    const double tot = mp_block_sum(ssum, red_s);
+    if (threadIdx.x == 0) spart[2 * blockIdx.x + (CURV ? 1 : 0)] = tot;
+}
+
+// ---------------------------------------------------------------- the step: one CTA
+// PHASE 0: after the first gradient pass (it = 0): finish g_A, subspace rule, stopping rules; no update.
+// PHASE 1: after the curvature pass: delta_0 (C17), update.
+// PHASE 2: after a gradient pass, it >= 1: finish g_A, subspace rule, stopping rules, Eq. (7)/(8), update.
+template <int PHASE>
+__global__ void __launch_bounds__(MP_THREADS)
+k_mp_step(int m, int m_cap, int n_cta, double *__restrict__ y, double *__restrict__ y_prev, double *__restrict__ g,
+          double *__restrict__ g_prev, const double *__restrict__ lo, const double *__restrict__ hi,
+          const double *__restrict__ gpart, const double *__restrict__ spart, MpState *__restrict__ st,
+          double *__restrict__ F_hist, double *__restrict__ delta_hist)
+{
+    if (st->reason != 0) return;
+    __shared__ double red_s[MP_WARPS + 1];
+    __shared__ int s_flag;
+    const int it = st->it;
+    if (PHASE != 1) {
+        // ---- g_A = sum of the CTA partials (fixed order), subspace rule Eq. (9)/(10) with the sign of C15
+        int nonzero = 0;
+        double dy_max = 0.0;
+        for (int k = threadIdx.x; k < m; k += MP_THREADS) {
+            double s = 0.0;
+            for (int c = 0; c < n_cta; ++c) s += gpart[(size_t)c * m_cap + k];
+            const double yk = y[k];
+            if ((yk <= lo[k] && s > 0.0) || (yk >= hi[k] && s < 0.0)) s = 0.0;
+            g[k] = s;
+            nonzero |= s != 0.0;
+            if (it >= 1) dy_max = fmax(dy_max, fabs(yk - y_prev[k]));
+        }
+        double fs = 0.0;
+        for (int c = threadIdx.x; c < n_cta; c += MP_THREADS) fs += spart[2 * c];
+        const double F = mp_block_sum(fs, red_s);
+        if (threadIdx.x == 0) s_flag = 0;
+        __syncthreads();
+        if (nonzero) atomicOr(&s_flag, 1);
+        // max over the block of dy_max (exact, order-free)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) dy_max = fmax(dy_max, shfl_xor_d(dy_max, o));
+        __shared__ double red_m[MP_WARPS];
+        if ((threadIdx.x & 31) == 0) red_m[threadIdx.x >> 5] = dy_max;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int i = 0; i < MP_WARPS; ++i) dy_max = fmax(dy_max, red_m[i]);
+            for (int j = MP_HIST - 1; j > 0; --j) st->Fh[j] = st->Fh[j - 1];
+            st->Fh[0] = F;
+            st->F = F;
+            F_hist[it] = F;
+            // ---- stopping rules, in the order of C19
+            int reason = 0;
+            if (!s_flag) reason = 1;
+            else {
+                bool flat = it >= 5;
+                for (int j = 0; flat && j < 5; ++j)
+                    flat = fabs(st->Fh[j] - st->Fh[j + 1]) <= st->eps_F * fabs(st->Fh[j + 1]);
+                if (flat) reason = 2;
+                else if (it >= 1 && dy_max <= st->eps_y) reason = 3;
+                else if (it >= st->max_iter) reason = 4;
+            }
+            st->reason = reason;
+            s_flag = reason;
+        }
+        __syncthreads();
+        if (s_flag != 0 || PHASE == 0) return;
+    }
+    // ---- step size
+    double delta;
+    if (PHASE == 1) {
+        double cs = 0.0, gg = 0.0;
+        for (int c = threadIdx.x; c < n_cta; c += MP_THREADS) cs += spart[2 * c + 1];
+        for (int k = threadIdx.x; k < m; k += MP_THREADS) gg += g[k] * g[k];
+        const double den = 2.0 * mp_block_sum(cs, red_s);
+        const double num = mp_block_sum(gg, red_s);
+        delta = den > 0.0 ? num / den : 1.0;                                             // C17
+    } else {
+        double ss = 0.0, sv = 0.0, tt = 0.0;
+        for (int k = threadIdx.x; k < m; k += MP_THREADS) {
+            const double s = y[k] - y_prev[k], t = g[k] - g_prev[k];
+            ss += s * s; sv += s * t; tt += t * t;
+        }
+        ss = mp_block_sum(ss, red_s);
+        sv = mp_block_sum(sv, red_s);
+        tt = mp_block_sum(tt, red_s);
+        delta = st->delta;                                                               // kept when <s,t> <= 0 (C18)
+        if (sv > 0.0 && tt > 0.0) delta = (it & 1) ? ss / sv : sv / tt;                  // Eq. (7) odd, Eq. (8) even
+    }
+    // ---- update within the box (step 3; C16)
+    for (int k = threadIdx.x; k < m; k += MP_THREADS) {
+        const double yk = y[k], gk = g[k];
+        y_prev[k] = yk;
+        g_prev[k] = gk;
+        y[k] = fmin(fmax(yk - delta * gk, lo[k]), hi[k]);
+    }
+    if (threadIdx.x == 0) {
+        st->delta = delta;
+        delta_hist[it] = delta;
+        st->it = it + 1;
+    }
+}
+
+// ---------------------------------------------------------------- host side
+template <bool CURV>
+static void mp_launch_pass(const vmat_mp *h, const uint8_t *vs, const float *T, const float *wo, const float *wu,
+                           float *z, cudaStream_t s)
+{
+    const int m = h->m;
+    int G = 32;
+    if (m < 32) { G = 1; while (G < m) G <<= 1; }
+    const int nc = (m + G - 1) / G;
+#define MP_PASS(NC_)                                                                                          \
+    k_mp_pass<NC_, CURV><<<h->n_cta, MP_THREADS, 0, s>>>(h->n_voxels, m, h->m_cap, G, h->DA, h->y, h->g, vs, T, wo, \
+                                                          wu, z, h->gpart, h->spart, h->st)
+    if (nc <= 1) MP_PASS(1);
+    else if (nc <= 2) MP_PASS(2);
+    else if (nc <= 4) MP_PASS(4);
+    else if (nc <= 8) MP_PASS(8);
+    else MP_PASS(12);
+#undef MP_PASS
+}
+
+template <int PHASE>
+static void mp_launch_step(const vmat_mp *h, cudaStream_t s)
+{
+    k_mp_step<PHASE><<<1, MP_THREADS, 0, s>>>(h->m, h->m_cap, h->n_cta, h->y, h->y_prev, h->g, h->g_prev, h->lo, h->hi,
+                                              h->gpart, h->spart, h->st, h->F_hist, h->delta_hist);
+}
+
+#define REQUIRE(cond, msg)                                            \
+    do {                                                              \
+        if (!(cond)) { vmat_set_error("%s: %s", __func__, msg); return VMAT_ERR_INVALID_ARG; } \
+    } while (0)
+
+extern "C" {
+
+int vmat_mp_destroy(vmat_mp *h)
+{
+    if (!h) return VMAT_OK;
+    void *ptrs[] = {h->DA, h->y, h->y_prev, h->g, h->g_prev, h->lo, h->hi, h->gpart, h->spart, h->st, h->F_hist,
+                    h->delta_hist};
+    for (void *p : ptrs)
+        if (p) cudaFree(p);
+    delete h;
+    return VMAT_OK;
+}
+
+int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void *stream)
+{
+    REQUIRE(out != nullptr, "out is NULL");
+    REQUIRE(n_voxels >= 0, "negative n_voxels");
+    REQUIRE(max_apertures >= 1 && max_apertures <= MP_MAX_NC * 32, "max_apertures must be in 1..384");
+    vmat_mp *h = new (std::nothrow) vmat_mp();
+    if (!h) { vmat_set_error("vmat_mp_create: host allocation failed"); return VMAT_ERR_OOM; }
+    h->n_voxels = n_voxels;
+    h->m_cap = (max_apertures + 7) / 8 * 8;                  // rows start on 32-byte boundaries
+    cudaGetDevice(&h->device);
+    int n_sm = 1;
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, h->device);
+    h->n_cta = n_sm * 4;                                     // fixed for the handle: fixes every summation order
+    cudaStream_t s = (cudaStream_t)stream;
+    auto alloc = [&](void **p, size_t bytes) { return cudaMalloc(p, bytes > 0 ? bytes : 1) == cudaSuccess; };
+    const size_t mc = (size_t)h->m_cap;
+    bool ok = alloc((void **)&h->DA, (size_t)n_voxels * mc * 4) && alloc((void **)&h->y, mc * 8) &&
+              alloc((void **)&h->y_prev, mc * 8) && alloc((void **)&h->g, mc * 8) && alloc((void **)&h->g_prev, mc * 8) &&
+              alloc((void **)&h->lo, mc * 8) && alloc((void **)&h->hi, mc * 8) &&
+              alloc((void **)&h->gpart, (size_t)h->n_cta * mc * 8) && alloc((void **)&h->spart, (size_t)h->n_cta * 16) &&
+              alloc((void **)&h->st, sizeof(MpState));
+    if (!ok) {
+        cudaGetLastError();
+        vmat_mp_destroy(h);
+        vmat_set_error("vmat_mp_create: device allocation failed (%lld voxels x %d apertures)", (long long)n_voxels, h->m_cap);
+        return VMAT_ERR_OOM;
+    }
+    cudaMemsetAsync(h->DA, 0, (size_t)n_voxels * mc * 4, s);
+    cudaMemsetAsync(h->y, 0, mc * 8, s);
+    cudaMemsetAsync(h->spart, 0, (size_t)h->n_cta * 16, s);
+    VMAT_CUDA(cudaStreamSynchronize(s));
+    *out = h;
+    return VMAT_OK;
+}
+
+int vmat_mp_reset(vmat_mp *h)
+{
+    REQUIRE(h != nullptr, "handle is NULL");
+    h->m = 0;
+    return VMAT_OK;
+}
+
+int vmat_mp_add_aperture(vmat_mp *h, const float *DA, double y0, double y_lo, double y_hi, void *stream)
+{
+    REQUIRE(h != nullptr, "handle is NULL");
+    REQUIRE(DA != nullptr || h->n_voxels == 0, "DA is NULL");
+    REQUIRE(h->m < h->m_cap, "the handle is full (max_apertures)");
+    REQUIRE(y_lo <= y_hi, "y_lo > y_hi");
+    cudaStream_t s = (cudaStream_t)stream;
+    g_vmat_launches = 0;
+    const int k = h->m;
+    if (h->n_voxels > 0) {
+        k_mp_set_column<<<(h->n_voxels + 255) / 256, 256, 0, s>>>(h->n_voxels, h->m_cap, k, DA, h->DA);
+        VMAT_LAUNCH_CHECK();
+    }
+    const double v[3] = {y0 < y_lo ? y_lo : (y0 > y_hi ? y_hi : y0), y_lo, y_hi};
+    VMAT_CUDA(cudaMemcpyAsync(h->y + k, &v[0], 8, cudaMemcpyHostToDevice, s));
+    VMAT_CUDA(cudaMemcpyAsync(h->lo + k, &v[1], 8, cudaMemcpyHostToDevice, s));
+    VMAT_CUDA(cudaMemcpyAsync(h->hi + k, &v[2], 8, cudaMemcpyHostToDevice, s));
+    VMAT_CUDA(cudaStreamSynchronize(s));                     // v lives on this stack frame
+    h->m = k + 1;
+    return VMAT_OK;
+}
+
+int vmat_mp_set_fluence(vmat_mp *h, const double *y_host, void *stream)
+{
+    REQUIRE(h && y_host, "NULL argument");
+    if (h->m > 0) {
+        VMAT_CUDA(cudaMemcpyAsync(h->y, y_host, (size_t)h->m * 8, cudaMemcpyHostToDevice, (cudaStream_t)stream));
+        VMAT_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    }
+    return VMAT_OK;
+}
+
+int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, const float *T, const float *w_over,
+                  const float *w_under, int32_t max_iter, double eps_F, double eps_y, float *z, double *y_host,
+                  double *F_host, int32_t *n_iter_host, int32_t *reason_host, void *stream)
+{
+    REQUIRE(h && T && w_over && w_under, "NULL argument");
+    REQUIRE(h->n_voxels == 0 || voxel_struct, "voxel_struct is NULL");
+    REQUIRE(n_struct >= 1 && n_struct <= 256, "n_struct must be in 1..256");
+    REQUIRE(h->m >= 1, "no aperture has been added");
+    REQUIRE(max_iter >= 0 && max_iter <= (1 << 24), "max_iter out of range");
+    REQUIRE(eps_F >= 0.0 && eps_y >= 0.0, "negative tolerance");
+    cudaStream_t s = (cudaStream_t)stream;
+    g_vmat_launches = 0;
+    if (max_iter + 1 > h->hist_cap) {
+        if (h->F_hist) cudaFree(h->F_hist);
+        if (h->delta_hist) cudaFree(h->delta_hist);
+        h->F_hist = h->delta_hist = nullptr;
+        h->hist_cap = 0;
+        VMAT_CUDA(cudaMalloc((void **)&h->F_hist, ((size_t)max_iter + 1) * 8));
+        VMAT_CUDA(cudaMalloc((void **)&h->delta_hist, ((size_t)max_iter + 1) * 8));
+        h->hist_cap = max_iter + 1;
+    }
+    MpState init = {};
+    init.max_iter = max_iter; init.eps_F = eps_F; init.eps_y = eps_y;
+    VMAT_CUDA(cudaMemcpyAsync(h->st, &init, sizeof(init), cudaMemcpyHostToDevice, s));
+    k_mp_clip<<<(h->m + 127) / 128, 128, 0, s>>>(h->m, h->y, h->lo, h->hi);          // the start must be feasible (C16)
+    VMAT_LAUNCH_CHECK();
+    // iteration 0: gradient pass, step A, curvature pass, step B
+    mp_launch_pass<false>(h, voxel_struct, T, w_over, w_under, z, s); VMAT_LAUNCH_CHECK();
+    mp_launch_step<0>(h, s); VMAT_LAUNCH_CHECK();
+    mp_launch_pass<true>(h, voxel_struct, T, w_over, w_under, nullptr, s); VMAT_LAUNCH_CHECK();
+    mp_launch_step<1>(h, s); VMAT_LAUNCH_CHECK();
+    MpState cur;
+    const int BATCH = 8;                                     // iterations enqueued between two looks at the stop flag
+    for (;;) {
+        VMAT_CUDA(cudaMemcpyAsync(&cur, h->st, sizeof(cur), cudaMemcpyDeviceToHost, s));
+        VMAT_CUDA(cudaStreamSynchronize(s));
+        if (cur.reason != 0) break;
+        for (int b = 0; b < BATCH; ++b) {                    // kernels after the stop are no-ops (they read the flag)
+            mp_launch_pass<false>(h, voxel_struct, T, w_over, w_under, z, s); VMAT_LAUNCH_CHECK();
+            mp_launch_step<2>(h, s); VMAT_LAUNCH_CHECK();
+        }
+    }
+    h->last_n_iter = cur.it;
+    if (y_host) VMAT_CUDA(cudaMemcpyAsync(y_host, h->y, (size_t)h->m * 8, cudaMemcpyDeviceToHost, s));
+    VMAT_CUDA(cudaStreamSynchronize(s));
+    if (F_host) *F_host = cur.F;
+    if (n_iter_host) *n_iter_host = cur.it;
+    if (reason_host) *reason_host = cur.reason;
+    return VMAT_OK;
+}
+
+int vmat_mp_history(const vmat_mp *h, double *F_hist, double *delta_hist)
+{
+    REQUIRE(h != nullptr, "handle is NULL");
+    REQUIRE(h->F_hist != nullptr, "no solve has run");
+    VMAT_CUDA(cudaDeviceSynchronize());
+    if (F_hist) VMAT_CUDA(cudaMemcpy(F_hist, h->F_hist, ((size_t)h->last_n_iter + 1) * 8, cudaMemcpyDeviceToHost));
+    if (delta_hist && h->last_n_iter > 0)
+        VMAT_CUDA(cudaMemcpy(delta_hist, h->delta_hist, (size_t)h->last_n_iter * 8, cudaMemcpyDeviceToHost));
+    return VMAT_OK;
+}
+
+int vmat_mp_size(const vmat_mp *h, int32_t *n_apertures, int32_t *max_apertures)
+{
+    REQUIRE(h != nullptr, "handle is NULL");
+    if (n_apertures) *n_apertures = h->m;
+    if (max_apertures) *max_apertures = h->m_cap;
+    return VMAT_OK;
+}
+
+}  // extern "C"

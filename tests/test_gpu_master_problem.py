@@ -1,0 +1,229 @@
+"""GPU parity of the master problem (vmat_mp_*, NEXT-2) against oracle/master_problem.py.
+
+The method is an iteration, so parity is checked (a) on the trace: objective value and step size of every
+iteration, (b) on the returned iterate (y, z, F, iteration count, stopping rule).  The CUDA path sums in FP64 in
+its own fixed order, so it differs from the FP64 oracle by summation order only: the tolerances are 1e-9
+relative on the trace and on y (BB amplifies rounding differences over hundreds of iterations), 1e-5 / 1e-4 on
+the FP32 dose z (`north_star`'s vector tolerance).
+"""
+import numpy as np
+import pytest
+import torch
+
+import synth
+from conftest import as_np
+from helpers import assert_vec_close, ddc_from_arrays, obj_to_device
+from oracle import master_problem as omp
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+TRACE_RTOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def vm():
+    import paper_1503_01721_b200 as vm
+    vm.load_library()
+    return vm
+
+
+def _random_mp(rng, n_v, m, n_struct=4, density=0.6):
+    DA = (rng.random((n_v, m)) * (rng.random((n_v, m)) < density)).astype(np.float32)
+    sid = rng.integers(0, n_struct, n_v).astype(np.uint8)
+    T = np.array([30.0, 70.0, 20.0, 50.0], np.float32)[:n_struct]
+    wo = np.array([0.2, 1.0, 0.05, 0.7], np.float32)[:n_struct]
+    wu = np.array([0.0, 1.0, 0.0, 0.3], np.float32)[:n_struct]
+    return DA, sid, T, wo, wu
+
+
+def _solve_both(vm, DA, sid, T, wo, wu, y0, lo, hi, max_iter, eps_F, eps_y, m_cap=None):
+    n_v, m = DA.shape
+    ref = omp.solve(DA.astype(np.float64), y0, lo, hi, T[sid].astype(np.float64), wo[sid].astype(np.float64),
+                    wu[sid].astype(np.float64), max_iter=max_iter, eps_F=eps_F, eps_y=eps_y)
+    mp = vm.MasterProblem(n_v, m_cap or m, DEV)
+    for k in range(m):
+        mp.add_aperture(torch.from_numpy(np.ascontiguousarray(DA[:, k])).to(DEV), y0[k], lo[k], hi[k])
+    obj = vm.Objective(torch.from_numpy(sid).to(DEV), torch.from_numpy(T).to(DEV), torch.from_numpy(wo).to(DEV),
+                       torch.from_numpy(wu).to(DEV))
+    z = torch.empty(n_v, dtype=torch.float32, device=DEV)
+    sol = mp.solve(obj, max_iter=max_iter, eps_F=eps_F, eps_y=eps_y, z=z)
+    Fh, dh = mp.history()
+    return ref, sol, z.cpu().numpy(), Fh.numpy(), dh.numpy(), mp, obj
+
+
+def _check(ref, sol, z, Fh, dh, trace_rtol=TRACE_RTOL):
+    assert sol.n_iter == ref.n_iter and sol.reason == ref.reason
+    assert np.allclose(Fh, np.array(ref.F_hist), rtol=trace_rtol, atol=0.0)
+    assert np.allclose(dh, np.array(ref.delta_hist), rtol=trace_rtol, atol=0.0)
+    scale = max(1.0, float(np.abs(ref.y).max()))
+    assert np.abs(sol.y.numpy() - ref.y).max() <= trace_rtol * scale
+    assert abs(sol.F - ref.F) <= trace_rtol * abs(ref.F)
+    assert_vec_close("z", z, ref.z)
+
+
+@pytest.mark.parametrize("n_v,m", [(1, 1), (37, 1), (1000, 3), (5000, 8), (3001, 31), (4000, 32), (2500, 33),
+                                   (2000, 100), (1500, 257), (700, 384)])
+def test_trace_and_solution_match_the_oracle(vm, n_v, m):
+    """Every group size (G = 1 .. 32), every chunk count (1, 2, 4, 8, 12) and ragged voxel counts."""
+    rng = np.random.default_rng(1000 + n_v + m)
+    DA, sid, T, wo, wu = _random_mp(rng, n_v, m)
+    lo, hi = np.zeros(m), np.full(m, 40.0)
+    y0 = rng.uniform(0.0, 1.0, m)
+    # 12 iterations: far from the rounding floor, where "F has stopped changing" would depend on summation order
+    ref, sol, z, Fh, dh, mp, _ = _solve_both(vm, DA, sid, T, wo, wu, y0, lo, hi, max_iter=12, eps_F=0.0, eps_y=0.0)
+    _check(ref, sol, z, Fh, dh)
+    assert ref.n_iter == 12 or ref.reason == 1
+    mp.close()
+
+
+def test_each_stopping_rule(vm):
+    rng = np.random.default_rng(5)
+    DA, sid, T, wo, wu = _random_mp(rng, 3000, 12)
+    lo, hi, y0 = np.zeros(12), np.full(12, 1e6), np.zeros(12)
+    for kw, reason in ((dict(max_iter=7, eps_F=0.0, eps_y=0.0), 4), (dict(max_iter=5000, eps_F=1e-5, eps_y=0.0), 2),
+                       (dict(max_iter=5000, eps_F=0.0, eps_y=1e-4), 3), (dict(max_iter=0, eps_F=0.0, eps_y=0.0), 4)):
+        ref, sol, z, Fh, dh, mp, _ = _solve_both(vm, DA, sid, T, wo, wu, y0, lo, hi, **kw)
+        assert ref.reason == reason
+        _check(ref, sol, z, Fh, dh, trace_rtol=1e-8)
+        mp.close()
+    # nothing to gain (no under-dose penalty anywhere, everything at its lower bound): stationary at iteration 0
+    ref, sol, z, Fh, dh, mp, _ = _solve_both(vm, DA, sid, T, wo, wu * 0, y0, lo, hi, max_iter=10, eps_F=0.0, eps_y=0.0)
+    assert ref.reason == 1 and ref.n_iter == 0
+    _check(ref, sol, z, Fh, dh)
+    mp.close()
+
+
+def test_active_bounds_and_convergence_to_the_kkt_point(vm):
+    """Upper and lower bounds bind (Eq. (9)/(10)); run to convergence and compare with the oracle's optimum."""
+    rng = np.random.default_rng(9)
+    DA, sid, T, wo, wu = _random_mp(rng, 4000, 10)
+    lo = np.full(10, 0.5)
+    hi = np.array([3.0, 3.0, 3.0, 1e3, 1e3, 1e3, 1e3, 1e3, 1e3, 1e3])
+    y0 = np.full(10, 0.5)
+    ref, sol, z, Fh, dh, mp, obj = _solve_both(vm, DA, sid, T, wo, wu, y0, lo, hi, max_iter=3000, eps_F=0.0, eps_y=1e-11)
+    assert ref.reason in (1, 2, 3)
+    y = sol.y.numpy()
+    assert np.all(y >= lo) and np.all(y <= hi) and ((y <= lo) | (y >= hi)).sum() >= 1
+    assert abs(sol.F - ref.F) <= 1e-9 * ref.F
+    assert np.abs(y - ref.y).max() <= 1e-6 * np.abs(ref.y).max()
+    assert_vec_close("z", z, ref.z)
+    # warm start (L56: the next outer iteration starts from this solution): solving again stops at once
+    sol2 = mp.solve(obj, max_iter=50, eps_F=0.0, eps_y=1e-9)
+    assert sol2.n_iter <= 3 and abs(sol2.F - sol.F) <= 1e-9 * sol.F
+    mp.close()
+
+
+def test_determinism_capacity_and_reset(vm):
+    """Two solves give identical bits; spare capacity (m_cap > m) does not change a bit; reset() starts over."""
+    rng = np.random.default_rng(21)
+    DA, sid, T, wo, wu = _random_mp(rng, 2222, 9)
+    lo, hi, y0 = np.zeros(9), np.full(9, 100.0), np.full(9, 0.25)
+    outs = []
+    for cap in (9, 9, 200):
+        ref, sol, z, Fh, dh, mp, obj = _solve_both(vm, DA, sid, T, wo, wu, y0, lo, hi, max_iter=25, eps_F=0.0,
+                                                   eps_y=0.0, m_cap=cap)
+        outs.append((sol.y.numpy().copy(), z.copy(), Fh.copy(), dh.copy()))
+        if cap == 200:
+            mp.reset()
+            assert mp.n_apertures == 0
+            mp.add_aperture(torch.from_numpy(np.ascontiguousarray(DA[:, 0])).to(DEV), 0.0, 0.0, 100.0)
+            one = mp.solve(obj, max_iter=10, eps_F=0.0, eps_y=0.0)
+            ref1 = omp.solve(DA[:, :1].astype(np.float64), [0.0], [0.0], [100.0], T[sid].astype(np.float64),
+                             wo[sid].astype(np.float64), wu[sid].astype(np.float64), max_iter=10, eps_F=0.0, eps_y=0.0)
+            assert abs(one.y[0].item() - ref1.y[0]) <= 1e-9 * max(1.0, abs(ref1.y[0]))
+        mp.close()
+    for a, b in zip(outs[0], outs[1]):
+        assert np.array_equal(a, b)
+    for a, b in zip(outs[0], outs[2]):
+        assert np.array_equal(a, b)
+
+
+def test_argument_errors(vm):
+    mp = vm.MasterProblem(10, 2, DEV)
+    obj = vm.Objective(torch.zeros(10, dtype=torch.uint8, device=DEV), torch.ones(1, device=DEV),
+                       torch.ones(1, device=DEV), torch.ones(1, device=DEV))
+    with pytest.raises(vm.VmatError, match="no aperture"):
+        mp.solve(obj)
+    col = torch.ones(10, device=DEV)
+    with pytest.raises(vm.VmatError, match="y_lo > y_hi"):
+        mp.add_aperture(col, 0.0, 2.0, 1.0)
+    for _ in range(8):                                       # capacity is rounded up to a multiple of 8
+        mp.add_aperture(col, 0.0, 0.0, 1.0)
+    with pytest.raises(vm.VmatError, match="full"):
+        mp.add_aperture(col, 0.0, 0.0, 1.0)
+    mp.close()
+    with pytest.raises(vm.VmatError):
+        vm.MasterProblem(10, 385, DEV)
+
+
+def test_column_generation_on_config0(vm, cfg0):
+    """The paper's loop (L56) on the tiny phantom, every step on the GPU: start z = 0, no apertures; price all
+    beamlets at the unoccupied control points, select the best aperture, compute its dose vector (Eq. (5)),
+    add it, solve the MP, repeat.  The oracle runs the same loop on its own (FP64, from COO; it never sees a GPU
+    value); at every outer iteration: same control point, same openings, fluence rates / dose / objective within
+    the FP32 tolerances; F decreases monotonically over the outer iterations."""
+    import oracle
+    A = as_np(cfg0)
+    h = ddc_from_arrays(A, DEV)
+    obj = obj_to_device(A, DEV)
+    n_v, n_b, n_a = A["n_v"], A["n_b"], len(A["aro"]) - 1
+    Tv, wov, wuv = (A[k][A["sid"]].astype(np.float64) for k in ("T", "wo", "wu"))
+    mp = vm.MasterProblem(n_v, n_a, DEV)
+    out = h.alloc_outputs()
+    z = torch.zeros(n_v, dtype=torch.float32, device=DEV)
+    mask = torch.zeros(n_a, dtype=torch.uint8, device=DEV)
+    xs = torch.empty(n_b, dtype=torch.float32, device=DEV)
+    DAk = torch.empty(n_v, dtype=torch.float32, device=DEV)
+    # oracle side
+    o_z = np.zeros(n_v)
+    o_mask = np.zeros(n_a, np.uint8)
+    o_cols, o_y, F_outer = [], np.zeros(0), []
+    y_hi = 50.0
+    for outer in range(n_a):
+        vm.vmat_objective_grad(h, z, obj, out.g, out.F)
+        vm.vmat_price(h, out.g, out.p)
+        vm.vmat_select_apertures(h, out.p, mask, out.L, out.R, out.row_price, out.angle_price, out.best_angle)
+        best = int(out.best_angle.item())
+        # oracle: the same pricing step from its own dose
+        oF, og = oracle.objective_grad(o_z, A["sid"], A["T"], A["wo"], A["wu"])
+        op = oracle.price(A["vox"], A["beam"], A["val"], n_b, og)
+        oL, oR, orp = oracle.select_rows(op.astype(np.float32), A["lco"])
+        for a in np.nonzero(o_mask)[0]:
+            sl = slice(A["aro"][a], A["aro"][a + 1])
+            oL[sl] = 0; oR[sl] = 0; orp[sl] = 0.0
+        oap, obest = oracle.angle_price(orp, A["aro"], o_mask)
+        assert best == obest
+        if best < 0:
+            break
+        rows = slice(A["aro"][best], A["aro"][best + 1])
+        assert np.array_equal(out.L.cpu().numpy()[rows], oL[rows]) and np.array_equal(out.R.cpu().numpy()[rows], oR[rows])
+        vm.vmat_aperture_dose(h, best, out.L, out.R, xs, DAk)
+        mp.add_aperture(DAk, 0.0, 0.0, y_hi)
+        mask[best] = 1
+        sol = mp.solve(obj, max_iter=300, eps_F=1e-10, eps_y=1e-12, z=z)
+        # oracle: Eq. (5) from COO, then its own MP from its own warm start
+        ind = np.zeros(n_b)
+        for r in range(A["aro"][best], A["aro"][best + 1]):
+            j0 = A["lco"][r]
+            ind[j0 + oL[r]: j0 + oR[r]] = 1.0
+        col = oracle.dose(A["vox"], A["beam"], A["val"], n_v, ind.astype(np.float32))
+        assert_vec_close("DA", DAk.cpu().numpy(), col)
+        o_cols.append(col)                                       # the oracle chain never sees a GPU value
+        o_mask[best] = 1
+        m = len(o_cols)
+        ref = omp.solve(np.stack(o_cols, 1), np.concatenate([o_y, [0.0]]), np.zeros(m), np.full(m, y_hi), Tv, wov, wuv,
+                        max_iter=300, eps_F=1e-10, eps_y=1e-12)
+        o_y, o_z = ref.y, ref.z
+        # the GPU's MP runs on FP32 aperture dose vectors (2^-24 relative rounding of DA), the oracle's on FP64
+        # ones: the two converged solutions agree to the FP32 tolerances of `north_star`
+        assert sol.reason in (1, 2, 3) and ref.reason in (1, 2, 3)
+        assert np.abs(sol.y.numpy() - ref.y).max() <= 1e-4 * max(1.0, np.abs(ref.y).max())
+        assert abs(sol.F - ref.F) <= 1e-5 * ref.F
+        assert_vec_close("z", z.cpu().numpy(), ref.z)
+        F_outer.append(sol.F)
+    assert len(F_outer) >= 3
+    assert all(b <= a * (1 + 1e-12) for a, b in zip(F_outer, F_outer[1:]))
+    F0, _ = oracle.objective_grad(np.zeros(n_v), A["sid"], A["T"], A["wo"], A["wu"])
+    assert F_outer[-1] < 0.2 * F0                                 # the plan covers the target
+    mp.close()
+    h.close()
