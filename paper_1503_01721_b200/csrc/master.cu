@@ -16,6 +16,8 @@
 
 constexpr int MP_THREADS = 256;
 constexpr int MP_WARPS = MP_THREADS / 32;
+constexpr int MP_STEP_THREADS = 1024;         // the one-CTA step kernel
+constexpr int MP_STEP_WARPS = MP_STEP_THREADS / 32;
 constexpr int MP_MAX_NC = 12;                 // up to 12 x 32 = 384 apertures
 constexpr int MP_HIST = 6;                    // objective values the "last five changes" rule looks at
 
@@ -34,7 +36,7 @@ struct vmat_mp {
     int n_cta = 0, device = 0;
     float *DA = nullptr;                      // [n_voxels][m_cap]
     double *y = nullptr, *y_prev = nullptr, *g = nullptr, *g_prev = nullptr, *lo = nullptr, *hi = nullptr;   // [m_cap]
-    double *gpart = nullptr;                  // [n_cta][m_cap]
+    double *gpart = nullptr;                  // [m_cap][n_cta] per-CTA partials of g_A
     double *spart = nullptr;                  // [n_cta][2]: F partial, curvature partial
     MpState *st = nullptr;
     double *F_hist = nullptr, *delta_hist = nullptr;   // [hist_cap + 1]
@@ -44,8 +46,9 @@ struct vmat_mp {
 
 __device__ __forceinline__ double shfl_xor_d(double v, int o) { return __shfl_xor_sync(0xffffffffu, v, o); }
 
-// deterministic block sum of doubles (MP_THREADS threads); result valid in every thread
-__device__ __forceinline__ double mp_block_sum(double v, double *red /* [MP_WARPS + 1] */)
+// deterministic block sum of doubles (NW warps); result valid in every thread
+template <int NW = MP_WARPS>
+__device__ __forceinline__ double mp_block_sum(double v, double *red /* [NW + 1] */)
 {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += shfl_xor_d(v, o);
@@ -54,11 +57,11 @@ __device__ __forceinline__ double mp_block_sum(double v, double *red /* [MP_WARP
     __syncthreads();
     if (threadIdx.x == 0) {
         double s = 0.0;
-        for (int i = 0; i < MP_WARPS; ++i) s += red[i];
-        red[MP_WARPS] = s;
+        for (int i = 0; i < NW; ++i) s += red[i];
+        red[NW] = s;
     }
     __syncthreads();
-    return red[MP_WARPS];
+    return red[NW];
 }
 
 __global__ void k_mp_set_column(int n_voxels, int m_cap, int k, const float *__restrict__ col, float *__restrict__ DA)
@@ -76,77 +79,141 @@ __global__ void k_mp_clip(int m, double *__restrict__ y, const double *__restric
 // ---------------------------------------------------------------- the pass over DA
 // CURV = false: z = DA y, F, dF/dz, partials of g_A = DA^T dF/dz            (steps 4 and 1 of L139)
 // CURV = true : z = DA y, q = DA g, partials of sum_i w_i q_i^2              (first step size, C17)
-// G lanes per voxel row (G = 32 when m >= 32, else the power of two >= m), NC chunks of G entries per row.
-template <int NC, bool CURV>
+//
+// Persistent CTAs walk over tiles of RT voxel rows.  A tile is brought into shared memory with 16-byte
+// cp.async copies (every load of the tile in flight at once, no register staging), stored with a row stride of
+// m32 = m rounded up to 32 floats.  Phase Z: TPR = 256 / RT threads per row add up the row dot product; thread
+// (row, part) visits column (TPR (j + row) + part) mod m32 at step j, so the 32 lanes of a warp hit 32
+// different banks and no shuffle is needed beyond the TPR partial sums.  The objective is evaluated once per row.
+// Phase G: thread t owns column t mod KT of every RG-th row (KT = min(m32, 256), RG = 256 / KT) and adds
+// DA_ik dF/dz_i to its FP64 accumulator, which it keeps over all its tiles.  The first version of this pass (a
+// group of lanes per row, FP64 shuffle tree per row) issued 118-161 warp instructions per row and ran at
+// 0.7-1.3 TB/s (issue-bound at m = 32, latency-bound at m = 128).
+constexpr int MP_TILE_FLOATS = 16384;          // 64 KB of shared memory per tile
+
+__device__ __forceinline__ void cp_async_16(void *smem, const void *gmem)
+{
+    const uint32_t sa = (uint32_t)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all()
+{
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+}
+
+template <bool CURV>
 __global__ void __launch_bounds__(MP_THREADS)
-k_mp_pass(int n_voxels, int m, int m_cap, int G, const float *__restrict__ DA,
+k_mp_pass(int n_voxels, int m, int m_cap, int RT, const float *__restrict__ DA,
           const double *__restrict__ y, const double *__restrict__ gvec,
-          const uint8_t *__restrict__ vstruct, const float *__restrict__ T, const float *__restrict__ w_over,
-          const float *__restrict__ w_under, float *__restrict__ z_out,
+          const uint8_t *__restrict__ vstruct, int n_struct, const float *__restrict__ T,
+          const float *__restrict__ w_over, const float *__restrict__ w_under, float *__restrict__ z_out,
           double *__restrict__ gpart, double *__restrict__ spart, const MpState *__restrict__ st)
 {
     if (st->reason != 0) return;                              // the solve has stopped: nothing to do
-    __shared__ double red[MP_WARPS][MP_MAX_NC * 32];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int m32 = (m + 31) & ~31, m4 = (m + 3) >> 2;        // row stride in floats; 16-byte chunks per row
+    float *tile = (float *)smem_raw;                          // [RT][m32]
+    double *y_s = (double *)(tile + (size_t)RT * m32);        // [m32] fluence rates (0 beyond m)
+    double *v_s = y_s + m32;                                  // [m32] CURV: g_A;  else unused
+    double *gz_s = v_s + m32;                                 // [RT] dF/dz of the tile's rows
     __shared__ double red_s[MP_WARPS + 1];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int gl = lane % G, sub = lane / G, rows_per_warp = 32 / G;
-    double yk[NC], acc[NC];
-#pragma unroll
-    for (int c = 0; c < NC; ++c) {
-        const int k = c * G + gl;
-        yk[c] = k < m ? y[k] : 0.0;
-        acc[c] = CURV ? (k < m ? gvec[k] : 0.0) : 0.0;        // CURV: acc holds g_A's entries (read only)
+    __shared__ float sT[256], sWo[256], sWu[256];             // the objective's tables
+    for (int t = threadIdx.x; t < n_struct; t += MP_THREADS) { sT[t] = T[t]; sWo[t] = w_over[t]; sWu[t] = w_under[t]; }
+    for (int k = threadIdx.x; k < m32; k += MP_THREADS) {
+        y_s[k] = k < m ? y[k] : 0.0;
+        v_s[k] = (CURV && k < m) ? gvec[k] : 0.0;
     }
+    for (int e = threadIdx.x; e < RT * m32; e += MP_THREADS) tile[e] = 0.f;     // the pad columns stay 0
+    __syncthreads();
+    const int nq = m32 >> 2;                                  // 16-byte chunks per stored row (a multiple of 8)
+    const int TPR = MP_THREADS / RT;                          // threads per row in phase Z: 1, 2, 4 or 8
+    const int zrow = threadIdx.x / TPR, zpart = threadIdx.x % TPR;
+    const int RG = MP_THREADS / nq;                           // phase G: thread = (row group, chunk of 4 columns)
+    const int gq = threadIdx.x % nq, grg = threadIdx.x / nq;
+    const int c_r = MP_THREADS / m4, c_q = MP_THREADS % m4;   // the copy loop steps (row, chunk) by 256 chunks
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};                     // g_A partials of columns 4 gq .. 4 gq + 3
     double ssum = 0.0;
-    const int n_warps = gridDim.x * MP_WARPS;
-    const int n_iter = (n_voxels + n_warps * rows_per_warp - 1) / (n_warps * rows_per_warp);   // uniform trip count
-    for (int itr = 0; itr < n_iter; ++itr) {
-        const int i = (itr * n_warps + blockIdx.x * MP_WARPS + warp) * rows_per_warp + sub;
-        const bool live = i < n_voxels;
-        float a[NC];
-        double zi = 0.0, qi = 0.0;
-#pragma unroll
-        for (int c = 0; c < NC; ++c) {
-            const int k = c * G + gl;
-            a[c] = (live && k < m) ? __ldg(DA + (size_t)i * m_cap + k) : 0.f;
-            zi = fma((double)a[c], yk[c], zi);
-            if (CURV) qi = fma((double)a[c], acc[c], qi);
+    const int n_tiles = (n_voxels + RT - 1) / RT;
+    for (int tix = blockIdx.x; tix < n_tiles; tix += gridDim.x) {
+        const int row0 = tix * RT;
+        // ---- the tile: RT x m4 chunks of 16 bytes, all in flight at once
+        for (int r = threadIdx.x / m4, q = threadIdx.x % m4; r < RT;) {
+            float *dst = tile + (size_t)r * m32 + 4 * q;
+            if (row0 + r < n_voxels) cp_async_16(dst, DA + (size_t)(row0 + r) * m_cap + 4 * q);
+            else *(float4 *)dst = make_float4(0.f, 0.f, 0.f, 0.f);
+            r += c_r; q += c_q;
+            if (q >= m4) { q -= m4; ++r; }
         }
-        for (int o = G >> 1; o > 0; o >>= 1) {               // row sums over the group's G lanes
-            zi += shfl_xor_d(zi, o);
-            if (CURV) qi += shfl_xor_d(qi, o);
-        }
-        if (live) {
-            const int sid = vstruct[i];
-            const double Ti = (double)__ldg(T + sid), wo = (double)__ldg(w_over + sid), wu = (double)__ldg(w_under + sid);
-            if (!CURV) {
-                const double over = fmax(zi - Ti, 0.0), under = fmax(Ti - zi, 0.0);
-                const double gz = 2.0 * wo * over - 2.0 * wu * under;                    // Eq. (1), sign C1
-                if (gl == 0) {
-                    ssum += wo * over * over + wu * under * under;
-                    if (z_out) z_out[i] = (float)zi;
+        cp_async_wait_all();
+        __syncthreads();
+        // ---- phase Z: row dot products, 4 columns per step; thread (row, part) starts at chunk TPR row + part, so
+        //      the 8 lanes of a quarter warp read 8 different bank groups
+        {
+            const float4 *trow = (const float4 *)(tile + (size_t)zrow * m32);
+            const double2 *y2 = (const double2 *)y_s, *v2 = (const double2 *)v_s;
+            double zi = 0.0, qi = 0.0;
+            int cq = (TPR * zrow + zpart) % nq;
+            const int nj = nq / TPR;
+#pragma unroll 2
+            for (int j = 0; j < nj; ++j) {
+                const float4 a = trow[cq];
+                const double2 ya = y2[2 * cq], yb = y2[2 * cq + 1];
+                const double a0 = (double)a.x, a1 = (double)a.y, a2 = (double)a.z, a3 = (double)a.w;
+                zi = fma(a0, ya.x, zi); zi = fma(a1, ya.y, zi); zi = fma(a2, yb.x, zi); zi = fma(a3, yb.y, zi);
+                if (CURV) {
+                    const double2 va = v2[2 * cq], vb = v2[2 * cq + 1];
+                    qi = fma(a0, va.x, qi); qi = fma(a1, va.y, qi); qi = fma(a2, vb.x, qi); qi = fma(a3, vb.y, qi);
                 }
-#pragma unroll
-                for (int c = 0; c < NC; ++c) acc[c] = fma((double)a[c], gz, acc[c]);     // g_A += DA_i: * dF/dz_i
-            } else if (gl == 0) {
-                const double w = zi > Ti ? wo : (zi < Ti ? wu : 0.0);                    // C17
-                ssum += w * qi * qi;
+                cq += TPR;
+                if (cq >= nq) cq -= nq;
+            }
+            for (int o = 1; o < TPR; o <<= 1) {               // the row's TPR parts sit in neighbouring lanes
+                zi += shfl_xor_d(zi, o);
+                if (CURV) qi += shfl_xor_d(qi, o);
+            }
+            const int i = row0 + zrow;
+            if (zpart == 0) {
+                double gz = 0.0;
+                if (i < n_voxels) {
+                    const int sid = vstruct[i];
+                    const double Ti = (double)sT[sid], wo = (double)sWo[sid], wu = (double)sWu[sid];
+                    if (!CURV) {
+                        const double over = fmax(zi - Ti, 0.0), under = fmax(Ti - zi, 0.0);
+                        gz = 2.0 * wo * over - 2.0 * wu * under;                         // Eq. (1), sign C1
+                        ssum += wo * over * over + wu * under * under;
+                        if (z_out) z_out[i] = (float)zi;
+                    } else {
+                        const double w = zi > Ti ? wo : (zi < Ti ? wu : 0.0);            // C17
+                        ssum += w * qi * qi;
+                    }
+                }
+                gz_s[zrow] = gz;
             }
         }
+        __syncthreads();
+        // ---- phase G: g_A += DA_i: * dF/dz_i; a thread owns 4 columns of every RG-th row
+        if (!CURV && grg < RG) {                               // (256 is no multiple of nq = 24, 40, ...: a few threads idle)
+            for (int r = grg; r < RT; r += RG) {
+                const double gz = gz_s[r];
+                const float4 a = ((const float4 *)(tile + (size_t)r * m32))[gq];
+                acc[0] = fma((double)a.x, gz, acc[0]); acc[1] = fma((double)a.y, gz, acc[1]);
+                acc[2] = fma((double)a.z, gz, acc[2]); acc[3] = fma((double)a.w, gz, acc[3]);
+            }
+        }
+        __syncthreads();                                      // the tile is overwritten next
     }
-    // ---- CTA partials in a fixed order: lanes with the same gl (rows handled side by side), then the warps
+    // ---- CTA partials in a fixed order: the RG row groups of every column
     if (!CURV) {
+        double *red = (double *)tile;                         // [RG][m32] doubles <= 8 KB; the tile is free now
+        if (grg < RG) {
 #pragma unroll
-        for (int c = 0; c < NC; ++c) {
-            double v = acc[c];
-            for (int o = G; o < 32; o <<= 1) v += shfl_xor_d(v, o);
-            if (sub == 0) red[warp][c * G + gl] = v;
+            for (int j = 0; j < 4; ++j) red[(size_t)grg * m32 + 4 * gq + j] = acc[j];
         }
         __syncthreads();
-        for (int k = threadIdx.x; k < NC * G; k += MP_THREADS) {
-            double s = 0.0;
-            for (int w = 0; w < MP_WARPS; ++w) s += red[w][k];
-            if (k < m) gpart[(size_t)blockIdx.x * m_cap + k] = s;
+        for (int k = threadIdx.x; k < m; k += MP_THREADS) {
+            double sacc = 0.0;
+            for (int g2 = 0; g2 < RG; ++g2) sacc += red[(size_t)g2 * m32 + k];
+            gpart[(size_t)k * gridDim.x + blockIdx.x] = sacc;                             // [m_cap][n_cta]
         }
     }
     const double tot = mp_block_sum(ssum, red_s);
@@ -158,43 +225,48 @@ k_mp_pass(int n_voxels, int m, int m_cap, int G, const float *__restrict__ DA,
 // PHASE 1: after the curvature pass: delta_0 (C17), update.
 // PHASE 2: after a gradient pass, it >= 1: finish g_A, subspace rule, stopping rules, Eq. (7)/(8), update.
 template <int PHASE>
-__global__ void __launch_bounds__(MP_THREADS)
+__global__ void __launch_bounds__(MP_STEP_THREADS)
 k_mp_step(int m, int m_cap, int n_cta, double *__restrict__ y, double *__restrict__ y_prev, double *__restrict__ g,
           double *__restrict__ g_prev, const double *__restrict__ lo, const double *__restrict__ hi,
           const double *__restrict__ gpart, const double *__restrict__ spart, MpState *__restrict__ st,
           double *__restrict__ F_hist, double *__restrict__ delta_hist)
 {
     if (st->reason != 0) return;
-    __shared__ double red_s[MP_WARPS + 1];
+    __shared__ double red_s[MP_STEP_WARPS + 1];
     __shared__ int s_flag;
     const int it = st->it;
     if (PHASE != 1) {
         // ---- g_A = sum of the CTA partials (fixed order), subspace rule Eq. (9)/(10) with the sign of C15
         int nonzero = 0;
         double dy_max = 0.0;
-        for (int k = threadIdx.x; k < m; k += MP_THREADS) {
+        // one warp per aperture: lane l adds partials l, l+32, ... in that order, then a fixed shuffle tree
+        for (int k = threadIdx.x >> 5; k < m; k += MP_STEP_WARPS) {
+            const double *col = gpart + (size_t)k * n_cta;
             double s = 0.0;
-            for (int c = 0; c < n_cta; ++c) s += gpart[(size_t)c * m_cap + k];
+#pragma unroll 4
+            for (int c = threadIdx.x & 31; c < n_cta; c += 32) s += col[c];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) s += shfl_xor_d(s, o);
             const double yk = y[k];
             if ((yk <= lo[k] && s > 0.0) || (yk >= hi[k] && s < 0.0)) s = 0.0;
-            g[k] = s;
+            if ((threadIdx.x & 31) == 0) g[k] = s;
             nonzero |= s != 0.0;
             if (it >= 1) dy_max = fmax(dy_max, fabs(yk - y_prev[k]));
         }
         double fs = 0.0;
-        for (int c = threadIdx.x; c < n_cta; c += MP_THREADS) fs += spart[2 * c];
-        const double F = mp_block_sum(fs, red_s);
+        for (int c = threadIdx.x; c < n_cta; c += MP_STEP_THREADS) fs += spart[2 * c];
+        const double F = mp_block_sum<MP_STEP_WARPS>(fs, red_s);
         if (threadIdx.x == 0) s_flag = 0;
         __syncthreads();
         if (nonzero) atomicOr(&s_flag, 1);
         // max over the block of dy_max (exact, order-free)
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) dy_max = fmax(dy_max, shfl_xor_d(dy_max, o));
-        __shared__ double red_m[MP_WARPS];
+        __shared__ double red_m[MP_STEP_WARPS];
         if ((threadIdx.x & 31) == 0) red_m[threadIdx.x >> 5] = dy_max;
         __syncthreads();
         if (threadIdx.x == 0) {
-            for (int i = 0; i < MP_WARPS; ++i) dy_max = fmax(dy_max, red_m[i]);
+            for (int i = 0; i < MP_STEP_WARPS; ++i) dy_max = fmax(dy_max, red_m[i]);
             for (int j = MP_HIST - 1; j > 0; --j) st->Fh[j] = st->Fh[j - 1];
             st->Fh[0] = F;
             st->F = F;
@@ -214,31 +286,31 @@ k_mp_step(int m, int m_cap, int n_cta, double *__restrict__ y, double *__restric
             s_flag = reason;
         }
         __syncthreads();
-        if (s_flag != 0 || PHASE == 0) return;
+        if (s_flag != 0 || PHASE == 0) return;           // (the barrier above also publishes g to the whole CTA)
     }
     // ---- step size
     double delta;
     if (PHASE == 1) {
         double cs = 0.0, gg = 0.0;
-        for (int c = threadIdx.x; c < n_cta; c += MP_THREADS) cs += spart[2 * c + 1];
-        for (int k = threadIdx.x; k < m; k += MP_THREADS) gg += g[k] * g[k];
-        const double den = 2.0 * mp_block_sum(cs, red_s);
-        const double num = mp_block_sum(gg, red_s);
+        for (int c = threadIdx.x; c < n_cta; c += MP_STEP_THREADS) cs += spart[2 * c + 1];
+        for (int k = threadIdx.x; k < m; k += MP_STEP_THREADS) gg += g[k] * g[k];
+        const double den = 2.0 * mp_block_sum<MP_STEP_WARPS>(cs, red_s);
+        const double num = mp_block_sum<MP_STEP_WARPS>(gg, red_s);
         delta = den > 0.0 ? num / den : 1.0;                                             // C17
     } else {
         double ss = 0.0, sv = 0.0, tt = 0.0;
-        for (int k = threadIdx.x; k < m; k += MP_THREADS) {
+        for (int k = threadIdx.x; k < m; k += MP_STEP_THREADS) {
             const double s = y[k] - y_prev[k], t = g[k] - g_prev[k];
             ss += s * s; sv += s * t; tt += t * t;
         }
-        ss = mp_block_sum(ss, red_s);
-        sv = mp_block_sum(sv, red_s);
-        tt = mp_block_sum(tt, red_s);
+        ss = mp_block_sum<MP_STEP_WARPS>(ss, red_s);
+        sv = mp_block_sum<MP_STEP_WARPS>(sv, red_s);
+        tt = mp_block_sum<MP_STEP_WARPS>(tt, red_s);
         delta = st->delta;                                                               // kept when <s,t> <= 0 (C18)
         if (sv > 0.0 && tt > 0.0) delta = (it & 1) ? ss / sv : sv / tt;                  // Eq. (7) odd, Eq. (8) even
     }
     // ---- update within the box (step 3; C16)
-    for (int k = threadIdx.x; k < m; k += MP_THREADS) {
+    for (int k = threadIdx.x; k < m; k += MP_STEP_THREADS) {
         const double yk = y[k], gk = g[k];
         y_prev[k] = yk;
         g_prev[k] = gk;
@@ -252,29 +324,32 @@ k_mp_step(int m, int m_cap, int n_cta, double *__restrict__ y, double *__restric
 }
 
 // ---------------------------------------------------------------- host side
-template <bool CURV>
-static void mp_launch_pass(const vmat_mp *h, const uint8_t *vs, const float *T, const float *wo, const float *wu,
-                           float *z, cudaStream_t s)
+static int mp_tile_rows(int m)
 {
-    const int m = h->m;
-    int G = 32;
-    if (m < 32) { G = 1; while (G < m) G <<= 1; }
-    const int nc = (m + G - 1) / G;
-#define MP_PASS(NC_)                                                                                          \
-    k_mp_pass<NC_, CURV><<<h->n_cta, MP_THREADS, 0, s>>>(h->n_voxels, m, h->m_cap, G, h->DA, h->y, h->g, vs, T, wo, \
-                                                          wu, z, h->gpart, h->spart, h->st)
-    if (nc <= 1) MP_PASS(1);
-    else if (nc <= 2) MP_PASS(2);
-    else if (nc <= 4) MP_PASS(4);
-    else if (nc <= 8) MP_PASS(8);
-    else MP_PASS(12);
-#undef MP_PASS
+    const int m32 = (m + 31) & ~31;
+    int rt = MP_THREADS;                                     // 256, 128, 64 or 32 rows so that RT * m32 <= 16384 floats
+    while (rt > 32 && rt * m32 > MP_TILE_FLOATS) rt >>= 1;
+    return rt;
+}
+static size_t mp_pass_smem(int m)
+{
+    const int m32 = (m + 31) & ~31, rt = mp_tile_rows(m);
+    return (size_t)rt * m32 * 4 + (size_t)m32 * 16 + (size_t)rt * 8;
+}
+
+template <bool CURV>
+static void mp_launch_pass(const vmat_mp *h, const uint8_t *vs, int n_struct, const float *T, const float *wo,
+                           const float *wu, float *z, cudaStream_t s)
+{
+    k_mp_pass<CURV><<<h->n_cta, MP_THREADS, mp_pass_smem(h->m), s>>>(h->n_voxels, h->m, h->m_cap, mp_tile_rows(h->m),
+                                                                     h->DA, h->y, h->g, vs, n_struct, T, wo, wu, z,
+                                                                     h->gpart, h->spart, h->st);
 }
 
 template <int PHASE>
 static void mp_launch_step(const vmat_mp *h, cudaStream_t s)
 {
-    k_mp_step<PHASE><<<1, MP_THREADS, 0, s>>>(h->m, h->m_cap, h->n_cta, h->y, h->y_prev, h->g, h->g_prev, h->lo, h->hi,
+    k_mp_step<PHASE><<<1, MP_STEP_THREADS, 0, s>>>(h->m, h->m_cap, h->n_cta, h->y, h->y_prev, h->g, h->g_prev, h->lo, h->hi,
                                               h->gpart, h->spart, h->st, h->F_hist, h->delta_hist);
 }
 
@@ -308,7 +383,11 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
     cudaGetDevice(&h->device);
     int n_sm = 1;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, h->device);
-    h->n_cta = n_sm * 4;                                     // fixed for the handle: fixes every summation order
+    h->n_cta = n_sm * 3;                                     // fixed for the handle: fixes every summation order
+    size_t smem_max = 0;
+    for (int mm = 32; mm <= MP_MAX_NC * 32; mm += 32) smem_max = mp_pass_smem(mm) > smem_max ? mp_pass_smem(mm) : smem_max;
+    cudaFuncSetAttribute(k_mp_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+    cudaFuncSetAttribute(k_mp_pass<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
     cudaStream_t s = (cudaStream_t)stream;
     auto alloc = [&](void **p, size_t bytes) { return cudaMalloc(p, bytes > 0 ? bytes : 1) == cudaSuccess; };
     const size_t mc = (size_t)h->m_cap;
@@ -397,9 +476,9 @@ int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, con
     k_mp_clip<<<(h->m + 127) / 128, 128, 0, s>>>(h->m, h->y, h->lo, h->hi);          // the start must be feasible (C16)
     VMAT_LAUNCH_CHECK();
     // iteration 0: gradient pass, step A, curvature pass, step B
-    mp_launch_pass<false>(h, voxel_struct, T, w_over, w_under, z, s); VMAT_LAUNCH_CHECK();
+    mp_launch_pass<false>(h, voxel_struct, n_struct, T, w_over, w_under, z, s); VMAT_LAUNCH_CHECK();
     mp_launch_step<0>(h, s); VMAT_LAUNCH_CHECK();
-    mp_launch_pass<true>(h, voxel_struct, T, w_over, w_under, nullptr, s); VMAT_LAUNCH_CHECK();
+    mp_launch_pass<true>(h, voxel_struct, n_struct, T, w_over, w_under, nullptr, s); VMAT_LAUNCH_CHECK();
     mp_launch_step<1>(h, s); VMAT_LAUNCH_CHECK();
     MpState cur;
     const int BATCH = 8;                                     // iterations enqueued between two looks at the stop flag
@@ -408,7 +487,7 @@ int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, con
         VMAT_CUDA(cudaStreamSynchronize(s));
         if (cur.reason != 0) break;
         for (int b = 0; b < BATCH; ++b) {                    // kernels after the stop are no-ops (they read the flag)
-            mp_launch_pass<false>(h, voxel_struct, T, w_over, w_under, z, s); VMAT_LAUNCH_CHECK();
+            mp_launch_pass<false>(h, voxel_struct, n_struct, T, w_over, w_under, z, s); VMAT_LAUNCH_CHECK();
             mp_launch_step<2>(h, s); VMAT_LAUNCH_CHECK();
         }
     }
