@@ -211,6 +211,52 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+# ----------------------------------------------------------------------------- NEXT-2: the master problem, timed
+def bench_master_problem(vm, h, obj, out, dev, m: int) -> dict:
+    """BB iterations of the master problem (vmat_mp_solve, Eq. (6)-(10)) on `m` apertures of the bench
+    phantom: one aperture at each of m evenly spaced control points, every leaf row opened over a seeded random
+    contiguous range, dose vectors by vmat_aperture_dose (Eq. (5)).  One iteration = one pass over the dense
+    voxel-major aperture dose matrix (4 m n_voxels bytes) + the one-CTA step kernel; the time per iteration is
+    the whole synchronous solve (host looks at the stop flag every 8 iterations) divided by its iterations."""
+    n_v, n_a, n_rows = h.n_voxels, h.n_angles, h.n_leaf_rows
+    m = max(1, min(m, n_a, 384))
+    ph_lco = h.leafrow_col_offset_host
+    g = torch.Generator().manual_seed(20150301)
+    lens = (ph_lco[1:] - ph_lco[:-1]).to(torch.float64)
+    a = torch.rand(n_rows, generator=g, dtype=torch.float64)
+    b = torch.rand(n_rows, generator=g, dtype=torch.float64)
+    L = (torch.minimum(a, b) * lens).floor().to(torch.int32).to(dev)
+    R = (torch.maximum(a, b) * lens).ceil().to(torch.int32).to(dev)
+    mp = vm.MasterProblem(n_v, m, dev)
+    xs = torch.empty(h.n_beamlets, dtype=torch.float32, device=dev)
+    DA = torch.empty(n_v, dtype=torch.float32, device=dev)
+    t0 = time.time()
+    for k in range(m):
+        vm.vmat_aperture_dose(h, (k * n_a) // m, L, R, xs, DA)
+        mp.add_aperture(DA, 0.0, 0.0, 50.0)
+    torch.cuda.synchronize()
+    t_build = time.time() - t0
+    z = torch.empty(n_v, dtype=torch.float32, device=dev)
+    mp.solve(obj, max_iter=16, eps_F=0.0, eps_y=0.0, z=z)                    # warm-up
+    mp.set_fluence(torch.zeros(m, dtype=torch.float64))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    sol = mp.solve(obj, max_iter=96, eps_F=0.0, eps_y=0.0, z=z)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    Fh, _ = mp.history()
+    n_it = max(sol.n_iter, 1)
+    bytes_it = 4 * m * n_v
+    res = {"apertures": m, "iterations": sol.n_iter, "stop_reason": sol.reason, "us_per_iteration": 1e3 * ms / n_it,
+           "algorithmic_bytes_per_iteration": bytes_it, "gbs": bytes_it / (ms / n_it * 1e-3) / 1e9,
+           "F_start": float(Fh[0]), "F_end": sol.F, "dtype": "f32 storage, f64 sums", "build_s": round(t_build, 2),
+           "workload": f"{m} apertures (random contiguous openings, one per control point), {n_v} voxels"}
+    mp.close()
+    return res
+
+
 # ----------------------------------------------------------------------------- the CUDA path, timed
 def run_ours(args):
     import paper_1503_01721_b200 as vm
@@ -239,6 +285,7 @@ def run_ours(args):
                            index_bits=args.index_bits)
     t_ingest = time.time() - t0
     stats = ph.stats()
+    h.leafrow_col_offset_host = ph.leafrow_col_offset.to(torch.int64).cpu()
     ph.coo_voxel = ph.coo_beamlet = ph.coo_val = None      # the handle holds its own layouts
     torch.cuda.empty_cache()
     obj = vm.Objective(ph.voxel_struct.to(dev), ph.struct_T.to(dev), ph.struct_w_over.to(dev),
@@ -305,6 +352,11 @@ def run_ours(args):
     h2d = 4 * n_b
     d2h = 4 * n_rows * 2 + 8 * n_rows + 8 * n_a + 4 + 8
 
+    # ---- NEXT-2: the master problem on the same phantom, rank 0 at N = 1 only
+    mp_line = None
+    if world == 1 and not args.no_mp:
+        mp_line = bench_master_problem(vm, h, obj, out, dev, args.mp_apertures)
+
     # ---- max over ranks
     elapsed_ms, e2e_ms = reduce_max([elapsed_ms, e2e_ms], dist if use_dist else None, dev)
 
@@ -362,6 +414,9 @@ def run_ours(args):
             "kernels": [k_dose, k_price],
             "result_check": {"F_last": F_last, "best_angle_last": best_last},
         }
+        if mp_line is not None:
+            mp_line["frac_of_measured"] = mp_line["gbs"] / peak
+            line["master_problem"] = mp_line
         if not args.no_cpu_baseline and world == 1:
             v, desc, _, _, _ = oracle_rate(spec, dev, 12.0, 40, reps_auto=True)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc}
@@ -382,6 +437,8 @@ def main():
     ap.add_argument("--index-bits", type=int, default=0, choices=[0, 16, 32],
                     help="index encoding of the layouts (vmat_ddc_create_ex): 0 = chosen per layout")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-mp", action="store_true", help="skip the master-problem measurement")
+    ap.add_argument("--mp-apertures", type=int, default=128)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -89,7 +89,13 @@ __global__ void k_mp_clip(int m, double *__restrict__ y, const double *__restric
 // DA_ik dF/dz_i to its FP64 accumulator, which it keeps over all its tiles.  The first version of this pass (a
 // group of lanes per row, FP64 shuffle tree per row) issued 118-161 warp instructions per row and ran at
 // 0.7-1.3 TB/s (issue-bound at m = 32, latency-bound at m = 128).
-constexpr int MP_TILE_FLOATS = 16384;          // 64 KB of shared memory per tile
+#ifndef VMAT_MP_TILE_FLOATS
+#define VMAT_MP_TILE_FLOATS 16384
+#endif
+#ifndef VMAT_MP_CTAS_PER_SM
+#define VMAT_MP_CTAS_PER_SM 3
+#endif
+constexpr int MP_TILE_FLOATS = VMAT_MP_TILE_FLOATS;   // shared memory per tile, in floats
 
 __device__ __forceinline__ void cp_async_16(void *smem, const void *gmem)
 {
@@ -383,7 +389,7 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
     cudaGetDevice(&h->device);
     int n_sm = 1;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, h->device);
-    h->n_cta = n_sm * 3;                                     // fixed for the handle: fixes every summation order
+    h->n_cta = n_sm * VMAT_MP_CTAS_PER_SM;                                     // fixed for the handle: fixes every summation order
     size_t smem_max = 0;
     for (int mm = 32; mm <= MP_MAX_NC * 32; mm += 32) smem_max = mp_pass_smem(mm) > smem_max ? mp_pass_smem(mm) : smem_max;
     cudaFuncSetAttribute(k_mp_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
