@@ -213,6 +213,24 @@ int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, con
  * double [n_iter] (step size used to leave iterate it); either may be NULL. */
 int vmat_mp_history(const vmat_mp *h, double *F_hist, double *delta_hist);
 
+/* The column-generation loop (Figure 1(a)): start with z = 0 and no apertures; repeat { PP1: g =
+ * dF/dz, p = D^T g;  PP2: best opening per leaf row of the unoccupied control points, best control point; stop if
+ * none has a negative price;  Eq. (5): its aperture dose vector;  MP: fluence rates of all apertures so far (BB,
+ * warm-started, the new aperture at 0 clipped into [y_lo, y_hi]) } until max_apertures.  Every step runs on the
+ * device; `mp` is reset first and holds the apertures afterwards (capacity >= max_apertures).  Neighbour
+ * compatibility of apertures (L50-L54, L66) is not modelled (C7, C21): every aperture gets the bounds [y_lo, y_hi].
+ *   z dev float [n_voxels] out: final dose;  L, R dev int32 [n_leaf_rows] out: openings of the chosen control
+ *   points, 0 elsewhere;  host outputs (each but n_apertures_host may be NULL): n_apertures_host [1];
+ *   angles_host int32 [max_apertures] (control point of aperture k, in the order chosen);  y_host double
+ *   [max_apertures];  F_hist_host double [max_apertures + 1] (F(0), then F after every master problem);
+ *   aperture_price_host double [max_apertures] (price of aperture k when chosen, < 0);  mp_iters_host int32
+ *   [max_apertures];  stop_host [1]: 0 = no improving aperture left, 1 = max_apertures reached.  Synchronous. */
+int vmat_column_generation(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_struct, int32_t n_struct, const float *T,
+                           const float *w_over, const float *w_under, int32_t max_apertures, double y_lo, double y_hi,
+                           int32_t mp_max_iter, double eps_F, double eps_y, float *z, int32_t *L, int32_t *R,
+                           int32_t *n_apertures_host, int32_t *angles_host, double *y_host, double *F_hist_host,
+                           double *aperture_price_host, int32_t *mp_iters_host, int32_t *stop_host, void *stream);
+
 /* Profiling hook for bench.py's roofline: four CUDA events (cudaEvent_t passed as void*, any may be NULL)
  * that every following vmat_price_eval / vmat_price_eval_host on this handle records on its stream:
  * ev[0] just before and ev[1] just after the dose(+objective) kernel, ev[2] just before and ev[3] just

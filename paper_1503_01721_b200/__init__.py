@@ -31,7 +31,7 @@ EXPORTS = [
     "vmat_objective_grad", "vmat_price", "vmat_select_apertures", "vmat_price_eval", "vmat_price_eval_host",
     "vmat_aperture_dose", "vmat_ddc_set_profile_events", "vmat_last_error", "vmat_last_launch_count",
     "vmat_mp_create", "vmat_mp_destroy", "vmat_mp_reset", "vmat_mp_add_aperture", "vmat_mp_set_fluence", "vmat_mp_size",
-    "vmat_mp_solve", "vmat_mp_history",
+    "vmat_mp_solve", "vmat_mp_history", "vmat_column_generation",
 ]
 
 
@@ -81,6 +81,8 @@ def load_library():
     lib.vmat_mp_size.argtypes = [vp, vp, vp]
     lib.vmat_mp_solve.argtypes = [vp, vp, i32, vp, vp, vp, i32, f64, f64, vp, vp, vp, vp, vp, vp]
     lib.vmat_mp_history.argtypes = [vp, vp, vp]
+    lib.vmat_column_generation.argtypes = [vp, vp, vp, i32, vp, vp, vp, i32, f64, f64, i32, f64, f64, vp, vp, vp,
+                                           vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_last_error.restype = ctypes.c_char_p
     lib.vmat_last_launch_count.restype = ctypes.c_int
     for name in EXPORTS:
@@ -367,6 +369,45 @@ class MasterProblem:
         dh = torch.empty(self._last_n_iter, dtype=torch.float64)
         _check(load_library().vmat_mp_history(self._h, Fh.data_ptr(), dh.data_ptr() if dh.numel() else None))
         return Fh, dh
+
+
+@dataclass
+class CGPlan:
+    angles: torch.Tensor           # int32 [n_apertures], host: control point of aperture k in the order chosen
+    y: torch.Tensor                # float64 [n_apertures], host
+    F_hist: torch.Tensor           # float64 [n_apertures + 1], host
+    aperture_price: torch.Tensor   # float64 [n_apertures], host
+    mp_iters: torch.Tensor         # int32 [n_apertures], host
+    stop: str                      # "no improving aperture" | "max_apertures"
+    z: torch.Tensor                # float32 [n_voxels], device
+    L: torch.Tensor                # int32 [n_leaf_rows], device
+    R: torch.Tensor
+
+
+def vmat_column_generation(h: DDC, mp: MasterProblem, obj: Objective, max_apertures: int, y_lo: float, y_hi: float,
+                           mp_max_iter: int = 300, eps_F: float = 1e-10, eps_y: float = 1e-12) -> CGPlan:
+    """The column-generation loop on the device; see vmat_column_generation in include/vmat.h."""
+    dev = h.device
+    z = torch.empty(h.n_voxels, dtype=torch.float32, device=dev)
+    L = torch.empty(h.n_leaf_rows, dtype=torch.int32, device=dev)
+    R = torch.empty(h.n_leaf_rows, dtype=torch.int32, device=dev)
+    n = ctypes.c_int32()
+    stop = ctypes.c_int32()
+    cap = max(int(max_apertures), 1)
+    angles = torch.zeros(cap, dtype=torch.int32)
+    y = torch.zeros(cap, dtype=torch.float64)
+    Fh = torch.zeros(cap + 1, dtype=torch.float64)
+    ap = torch.zeros(cap, dtype=torch.float64)
+    its = torch.zeros(cap, dtype=torch.int32)
+    _check(load_library().vmat_column_generation(
+        h._h, mp._h, _ptr(obj.voxel_struct, torch.uint8, "cuda", h.n_voxels), obj.n_struct,
+        _ptr(obj.T, torch.float32, "cuda"), _ptr(obj.w_over, torch.float32, "cuda"),
+        _ptr(obj.w_under, torch.float32, "cuda"), int(max_apertures), float(y_lo), float(y_hi), int(mp_max_iter),
+        float(eps_F), float(eps_y), z.data_ptr(), L.data_ptr(), R.data_ptr(), ctypes.addressof(n), angles.data_ptr(),
+        y.data_ptr(), Fh.data_ptr(), ap.data_ptr(), its.data_ptr(), ctypes.addressof(stop), _stream()))
+    k = int(n.value)
+    return CGPlan(angles[:k], y[:k], Fh[:k + 1], ap[:k], its[:k],
+                  "max_apertures" if stop.value == 1 else "no improving aperture", z, L, R)
 
 
 def last_launch_count() -> int:

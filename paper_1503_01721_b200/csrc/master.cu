@@ -517,6 +517,99 @@ int vmat_mp_history(const vmat_mp *h, double *F_hist, double *delta_hist)
     return VMAT_OK;
 }
 
+// The column-generation loop of PAPER.md L56 / Figure 1(a), every step on the device; the host only reads the
+// chosen control point (4 bytes) per outer iteration and the master problem's stop flag.
+int vmat_column_generation(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_struct, int32_t n_struct, const float *T,
+                           const float *w_over, const float *w_under, int32_t max_apertures, double y_lo, double y_hi,
+                           int32_t mp_max_iter, double eps_F, double eps_y, float *z, int32_t *L, int32_t *R,
+                           int32_t *n_apertures_host, int32_t *angles_host, double *y_host, double *F_hist_host,
+                           double *aperture_price_host, int32_t *mp_iters_host, int32_t *stop_host, void *stream)
+{
+    REQUIRE(h && mp && T && w_over && w_under && n_apertures_host, "NULL argument");
+    REQUIRE(h->n_voxels == mp->n_voxels, "the DDC handle and the master problem differ in n_voxels");
+    REQUIRE(h->n_voxels == 0 || (voxel_struct && z), "NULL voxel vector");
+    REQUIRE(h->n_leaf_rows == 0 || (L && R), "NULL leaf-row output");
+    REQUIRE(max_apertures >= 0 && max_apertures <= mp->m_cap, "max_apertures exceeds the master problem's capacity");
+    REQUIRE(n_struct >= 1 && n_struct <= 256, "n_struct must be in 1..256");
+    REQUIRE(y_lo <= y_hi, "y_lo > y_hi");
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t nv = (size_t)(h->n_voxels > 0 ? h->n_voxels : 1), nb = (size_t)(h->n_beamlets > 0 ? h->n_beamlets : 1);
+    const size_t nr = (size_t)(h->n_leaf_rows > 0 ? h->n_leaf_rows : 1), na = (size_t)(h->n_angles > 0 ? h->n_angles : 1);
+    // scratch of the pricing step, freed on every exit path
+    struct Scratch {
+        float *g = nullptr, *p = nullptr, *xs = nullptr, *DA = nullptr;
+        int32_t *Lw = nullptr, *Rw = nullptr, *best = nullptr;
+        double *row_price = nullptr, *angle_price = nullptr, *F = nullptr;
+        uint8_t *mask = nullptr;
+        ~Scratch() { for (void *q : {(void *)g, (void *)p, (void *)xs, (void *)DA, (void *)Lw, (void *)Rw, (void *)best,
+                                     (void *)row_price, (void *)angle_price, (void *)F, (void *)mask}) if (q) cudaFree(q); }
+    } w;
+    VMAT_CUDA(cudaMalloc((void **)&w.g, nv * 4)); VMAT_CUDA(cudaMalloc((void **)&w.DA, nv * 4));
+    VMAT_CUDA(cudaMalloc((void **)&w.p, nb * 4)); VMAT_CUDA(cudaMalloc((void **)&w.xs, nb * 4));
+    VMAT_CUDA(cudaMalloc((void **)&w.Lw, nr * 4)); VMAT_CUDA(cudaMalloc((void **)&w.Rw, nr * 4));
+    VMAT_CUDA(cudaMalloc((void **)&w.row_price, nr * 8)); VMAT_CUDA(cudaMalloc((void **)&w.angle_price, na * 8));
+    VMAT_CUDA(cudaMalloc((void **)&w.best, 4)); VMAT_CUDA(cudaMalloc((void **)&w.F, 8));
+    VMAT_CUDA(cudaMalloc((void **)&w.mask, na));
+    VMAT_CUDA(cudaMemsetAsync(w.mask, 0, na, s));
+    VMAT_CUDA(cudaMemsetAsync(z, 0, nv * 4, s));                                         // L56: start with z = 0 ...
+    if (h->n_leaf_rows > 0) {
+        VMAT_CUDA(cudaMemsetAsync(L, 0, nr * 4, s));
+        VMAT_CUDA(cudaMemsetAsync(R, 0, nr * 4, s));
+    }
+    mp->m = 0;                                                                           // ... and no apertures
+    int launches = 0, count = 0, stop = 1;
+    if (F_hist_host) {                                                                   // F(z = 0)
+        double F0 = 0.0;
+        int rc0 = vmat_launch_objective(h, z, voxel_struct, n_struct, T, w_over, w_under, w.g, w.F, s);
+        if (rc0 != VMAT_OK) return rc0;
+        VMAT_CUDA(cudaMemcpyAsync(&F0, w.F, 8, cudaMemcpyDeviceToHost, s));
+        VMAT_CUDA(cudaStreamSynchronize(s));
+        F_hist_host[0] = F0;
+    }
+    while (count < max_apertures) {
+        // PP1: gradient at the current dose, beamlet prices; PP2: best opening per leaf row, best control point
+        int rc = vmat_launch_objective(h, z, voxel_struct, n_struct, T, w_over, w_under, w.g, w.F, s);
+        if (rc == VMAT_OK) rc = vmat_launch_price_select(h, w.g, w.mask, w.p, w.Lw, w.Rw, w.row_price, s);
+        if (rc == VMAT_OK) rc = vmat_launch_angle_price(h, w.row_price, w.mask, w.angle_price, w.best, s);
+        if (rc != VMAT_OK) return rc;
+        int32_t best = -1;
+        double F = 0.0;
+        VMAT_CUDA(cudaMemcpyAsync(&best, w.best, 4, cudaMemcpyDeviceToHost, s));
+        VMAT_CUDA(cudaStreamSynchronize(s));
+        launches += g_vmat_launches;
+        if (best < 0) { stop = 0; break; }                                               // nothing decreases F any more
+        const int32_t r0 = h->h_angle_row_offset[best], r1 = h->h_angle_row_offset[best + 1];
+        if (r1 > r0) {
+            VMAT_CUDA(cudaMemcpyAsync(L + r0, w.Lw + r0, (size_t)(r1 - r0) * 4, cudaMemcpyDeviceToDevice, s));
+            VMAT_CUDA(cudaMemcpyAsync(R + r0, w.Rw + r0, (size_t)(r1 - r0) * 4, cudaMemcpyDeviceToDevice, s));
+        }
+        if (aperture_price_host)
+            VMAT_CUDA(cudaMemcpyAsync(aperture_price_host + count, w.angle_price + best, 8, cudaMemcpyDeviceToHost, s));
+        // Eq. (5): the aperture's dose vector; then the master problem over all apertures so far (warm start)
+        rc = vmat_aperture_dose(h, best, w.Lw, w.Rw, w.xs, w.DA, s);
+        launches += g_vmat_launches;
+        if (rc == VMAT_OK) rc = vmat_mp_add_aperture(mp, w.DA, 0.0, y_lo, y_hi, s);
+        launches += g_vmat_launches;
+        if (rc != VMAT_OK) return rc;
+        VMAT_CUDA(cudaMemsetAsync(w.mask + best, 1, 1, s));
+        int32_t nit = 0, reason = 0;
+        rc = vmat_mp_solve(mp, voxel_struct, n_struct, T, w_over, w_under, mp_max_iter, eps_F, eps_y, z, nullptr, &F,
+                           &nit, &reason, s);
+        launches += g_vmat_launches;
+        if (rc != VMAT_OK) return rc;
+        if (angles_host) angles_host[count] = best;
+        if (F_hist_host) F_hist_host[count + 1] = F;
+        if (mp_iters_host) mp_iters_host[count] = nit;
+        ++count;
+    }
+    if (y_host && count > 0) VMAT_CUDA(cudaMemcpyAsync(y_host, mp->y, (size_t)count * 8, cudaMemcpyDeviceToHost, s));
+    VMAT_CUDA(cudaStreamSynchronize(s));
+    *n_apertures_host = count;
+    if (stop_host) *stop_host = stop;
+    g_vmat_launches = launches;
+    return VMAT_OK;
+}
+
 int vmat_mp_size(const vmat_mp *h, int32_t *n_apertures, int32_t *max_apertures)
 {
     REQUIRE(h != nullptr, "handle is NULL");

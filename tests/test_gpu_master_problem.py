@@ -156,74 +156,44 @@ def test_argument_errors(vm):
         vm.MasterProblem(10, 385, DEV)
 
 
+def _compare_plans(A, plan, ref, h):
+    """GPU plan against the oracle's: same control points in the same order, same openings, fluence rates / dose /
+    objective within the FP32 tolerances (the GPU's master problem runs on FP32 aperture dose vectors, the
+    oracle's on FP64 ones, so the iteration counts of the master problems may differ)."""
+    assert plan.stop == ref.stop
+    assert plan.angles.tolist() == ref.angles
+    assert np.array_equal(plan.L.cpu().numpy(), ref.L) and np.array_equal(plan.R.cpu().numpy(), ref.R)
+    assert plan.y.numel() == ref.y.size
+    if ref.y.size:
+        assert np.abs(plan.y.numpy() - ref.y).max() <= 1e-4 * max(1.0, np.abs(ref.y).max())
+    assert np.allclose(plan.F_hist.numpy(), np.array(ref.F_hist), rtol=1e-5, atol=0.0)
+    assert np.allclose(plan.aperture_price.numpy(), np.array(ref.aperture_price), rtol=1e-5, atol=0.0)
+    assert_vec_close("z", plan.z.cpu().numpy(), ref.z)
+
+
 def test_column_generation_on_config0(vm, cfg0):
-    """The paper's loop (L56) on the tiny phantom, every step on the GPU: start z = 0, no apertures; price all
-    beamlets at the unoccupied control points, select the best aperture, compute its dose vector (Eq. (5)),
-    add it, solve the MP, repeat.  The oracle runs the same loop on its own (FP64, from COO; it never sees a GPU
-    value); at every outer iteration: same control point, same openings, fluence rates / dose / objective within
-    the FP32 tolerances; F decreases monotonically over the outer iterations."""
-    import oracle
+    """The paper's loop (L56) on the tiny phantom, every step on the GPU (vmat_column_generation), against the
+    oracle's loop, which runs on its own in FP64 from the COO triplets and never sees a GPU value."""
+    from oracle import column_generation as ocg
     A = as_np(cfg0)
     h = ddc_from_arrays(A, DEV)
     obj = obj_to_device(A, DEV)
-    n_v, n_b, n_a = A["n_v"], A["n_b"], len(A["aro"]) - 1
-    Tv, wov, wuv = (A[k][A["sid"]].astype(np.float64) for k in ("T", "wo", "wu"))
-    mp = vm.MasterProblem(n_v, n_a, DEV)
-    out = h.alloc_outputs()
-    z = torch.zeros(n_v, dtype=torch.float32, device=DEV)
-    mask = torch.zeros(n_a, dtype=torch.uint8, device=DEV)
-    xs = torch.empty(n_b, dtype=torch.float32, device=DEV)
-    DAk = torch.empty(n_v, dtype=torch.float32, device=DEV)
-    # oracle side
-    o_z = np.zeros(n_v)
-    o_mask = np.zeros(n_a, np.uint8)
-    o_cols, o_y, F_outer = [], np.zeros(0), []
-    y_hi = 50.0
-    for outer in range(n_a):
-        vm.vmat_objective_grad(h, z, obj, out.g, out.F)
-        vm.vmat_price(h, out.g, out.p)
-        vm.vmat_select_apertures(h, out.p, mask, out.L, out.R, out.row_price, out.angle_price, out.best_angle)
-        best = int(out.best_angle.item())
-        # oracle: the same pricing step from its own dose
-        oF, og = oracle.objective_grad(o_z, A["sid"], A["T"], A["wo"], A["wu"])
-        op = oracle.price(A["vox"], A["beam"], A["val"], n_b, og)
-        oL, oR, orp = oracle.select_rows(op.astype(np.float32), A["lco"])
-        for a in np.nonzero(o_mask)[0]:
-            sl = slice(A["aro"][a], A["aro"][a + 1])
-            oL[sl] = 0; oR[sl] = 0; orp[sl] = 0.0
-        oap, obest = oracle.angle_price(orp, A["aro"], o_mask)
-        assert best == obest
-        if best < 0:
-            break
-        rows = slice(A["aro"][best], A["aro"][best + 1])
-        assert np.array_equal(out.L.cpu().numpy()[rows], oL[rows]) and np.array_equal(out.R.cpu().numpy()[rows], oR[rows])
-        vm.vmat_aperture_dose(h, best, out.L, out.R, xs, DAk)
-        mp.add_aperture(DAk, 0.0, 0.0, y_hi)
-        mask[best] = 1
-        sol = mp.solve(obj, max_iter=300, eps_F=1e-10, eps_y=1e-12, z=z)
-        # oracle: Eq. (5) from COO, then its own MP from its own warm start
-        ind = np.zeros(n_b)
-        for r in range(A["aro"][best], A["aro"][best + 1]):
-            j0 = A["lco"][r]
-            ind[j0 + oL[r]: j0 + oR[r]] = 1.0
-        col = oracle.dose(A["vox"], A["beam"], A["val"], n_v, ind.astype(np.float32))
-        assert_vec_close("DA", DAk.cpu().numpy(), col)
-        o_cols.append(col)                                       # the oracle chain never sees a GPU value
-        o_mask[best] = 1
-        m = len(o_cols)
-        ref = omp.solve(np.stack(o_cols, 1), np.concatenate([o_y, [0.0]]), np.zeros(m), np.full(m, y_hi), Tv, wov, wuv,
-                        max_iter=300, eps_F=1e-10, eps_y=1e-12)
-        o_y, o_z = ref.y, ref.z
-        # the GPU's MP runs on FP32 aperture dose vectors (2^-24 relative rounding of DA), the oracle's on FP64
-        # ones: the two converged solutions agree to the FP32 tolerances of `north_star`
-        assert sol.reason in (1, 2, 3) and ref.reason in (1, 2, 3)
-        assert np.abs(sol.y.numpy() - ref.y).max() <= 1e-4 * max(1.0, np.abs(ref.y).max())
-        assert abs(sol.F - ref.F) <= 1e-5 * ref.F
-        assert_vec_close("z", z.cpu().numpy(), ref.z)
-        F_outer.append(sol.F)
-    assert len(F_outer) >= 3
-    assert all(b <= a * (1 + 1e-12) for a, b in zip(F_outer, F_outer[1:]))
-    F0, _ = oracle.objective_grad(np.zeros(n_v), A["sid"], A["T"], A["wo"], A["wu"])
-    assert F_outer[-1] < 0.2 * F0                                 # the plan covers the target
+    n_a = len(A["aro"]) - 1
+    mp = vm.MasterProblem(A["n_v"], n_a, DEV)
+    for cap in (n_a, 3, 0):
+        plan = vm.vmat_column_generation(h, mp, obj, cap, 0.0, 50.0)
+        ref = ocg.run(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], A["sid"], A["T"], A["wo"], A["wu"], A["lco"],
+                      A["aro"], max_apertures=cap, y_lo=0.0, y_hi=50.0)
+        _compare_plans(A, plan, ref, h)
+        assert mp.n_apertures == len(ref.angles)
+        if cap == n_a:
+            assert len(ref.angles) >= 3 and ref.F_hist[-1] < 0.01 * ref.F_hist[0]      # the plan covers the target
+            assert vm.last_launch_count() > 10 * len(ref.angles)                       # every step ran on the device
+    # tight upper bounds on the fluence rates: more apertures are needed and the bounds bind
+    plan = vm.vmat_column_generation(h, mp, obj, n_a, 0.0, 6.0)
+    ref = ocg.run(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], A["sid"], A["T"], A["wo"], A["wu"], A["lco"],
+                  A["aro"], max_apertures=n_a, y_lo=0.0, y_hi=6.0)
+    _compare_plans(A, plan, ref, h)
+    assert (ref.y >= 6.0).any()
     mp.close()
     h.close()
