@@ -257,6 +257,27 @@ def bench_master_problem(vm, h, obj, out, dev, m: int) -> dict:
     return res
 
 
+def bench_plan(vm, h, obj, dev) -> dict:
+    """One whole plan optimisation by column generation (vmat_column_generation, PAPER.md L56 / Figure 1(a)): one
+    aperture per control point until every control point is occupied or no aperture improves F; master problems
+    with eps_F = 1e-6, at most 200 BB iterations each, fluence rates in [0, 100].  Wall clock of the synchronous call
+    (the paper's headline is this loop: ~1 minute per H&N case on 4 GPUs; context, other constraints)."""
+    n_a = h.n_angles
+    cap = min(n_a, 384)
+    mp = vm.MasterProblem(h.n_voxels, cap, dev)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    plan = vm.vmat_column_generation(h, mp, obj, cap, 0.0, 100.0, mp_max_iter=200, eps_F=1e-6, eps_y=1e-9)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    res = {"seconds": dt, "apertures": int(plan.angles.numel()), "control_points": n_a, "stop": plan.stop,
+           "F_start": float(plan.F_hist[0]), "F_end": float(plan.F_hist[-1]),
+           "mp_iterations_total": int(plan.mp_iters.sum()), "gpu_launches": vm.last_launch_count(),
+           "settings": "y in [0, 100], MP: eps_F 1e-6, eps_y 1e-9, <= 200 BB iterations"}
+    mp.close()
+    return res
+
+
 # ----------------------------------------------------------------------------- the CUDA path, timed
 def run_ours(args):
     import paper_1503_01721_b200 as vm
@@ -353,9 +374,11 @@ def run_ours(args):
     d2h = 4 * n_rows * 2 + 8 * n_rows + 8 * n_a + 4 + 8
 
     # ---- NEXT-2: the master problem on the same phantom, rank 0 at N = 1 only
-    mp_line = None
+    mp_line = plan_line = None
     if world == 1 and not args.no_mp:
         mp_line = bench_master_problem(vm, h, obj, out, dev, args.mp_apertures)
+    if world == 1 and not args.no_plan:
+        plan_line = bench_plan(vm, h, obj, dev)
 
     # ---- max over ranks
     elapsed_ms, e2e_ms = reduce_max([elapsed_ms, e2e_ms], dist if use_dist else None, dev)
@@ -417,6 +440,8 @@ def run_ours(args):
         if mp_line is not None:
             mp_line["frac_of_measured"] = mp_line["gbs"] / peak
             line["master_problem"] = mp_line
+        if plan_line is not None:
+            line["plan_optimisation"] = plan_line
         if not args.no_cpu_baseline and world == 1:
             v, desc, _, _, _ = oracle_rate(spec, dev, 12.0, 40, reps_auto=True)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc}
@@ -439,6 +464,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-mp", action="store_true", help="skip the master-problem measurement")
     ap.add_argument("--mp-apertures", type=int, default=128)
+    ap.add_argument("--no-plan", action="store_true", help="skip the whole-plan (column generation) measurement")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -197,3 +197,24 @@ def test_column_generation_on_config0(vm, cfg0):
     assert (ref.y >= 6.0).any()
     mp.close()
     h.close()
+
+
+def test_column_generation_on_config1_coarsened(vm):
+    """The loop on the H&N-like phantom of config 1 coarsened by 3.2 (1.5e7 nnz, 180 control points): the first
+    apertures against the oracle's loop (ragged leaf rows, thousands of voxels per beamlet)."""
+    from oracle import column_generation as ocg
+    ph = synth.generate(synth.config_spec(1, 3.2), device=DEV)
+    A = as_np(ph)
+    h = vm.vmat_ddc_create(ph.n_voxels, ph.n_beamlets, ph.coo_voxel, ph.coo_beamlet, ph.coo_val,
+                           ph.angle_col_offset, ph.angle_row_offset, ph.leafrow_col_offset, device=DEV)
+    obj = obj_to_device(A, DEV)
+    mp = vm.MasterProblem(A["n_v"], 8, DEV)
+    plan = vm.vmat_column_generation(h, mp, obj, 5, 0.0, 100.0, mp_max_iter=500)
+    ref = ocg.run(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], A["sid"], A["T"], A["wo"], A["wu"], A["lco"],
+                  A["aro"], max_apertures=5, y_lo=0.0, y_hi=100.0, mp_max_iter=500)
+    print(f"\n[cfg1/3.2] control points {ref.angles}, F {ref.F_hist[0]:.4e} -> {ref.F_hist[-1]:.4e}, "
+          f"MP iterations {ref.mp_iters} (GPU {plan.mp_iters.tolist()})")
+    _compare_plans(A, plan, ref, h)
+    assert len(ref.angles) == 5 and ref.F_hist[-1] < 0.5 * ref.F_hist[0]
+    mp.close()
+    h.close()
