@@ -47,6 +47,8 @@ def _load():
         lib.oracle_select_rows.restype = None
         lib.oracle_angle_price.argtypes = [i32, vp, vp, vp, vp]
         lib.oracle_angle_price.restype = i32
+        lib.oracle_select_constrained.argtypes = [i32, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
+        lib.oracle_select_constrained.restype = i32
         _lib = lib
     return _lib
 
@@ -116,6 +118,35 @@ def angle_price(row_price, angle_row_offset, angle_mask=None):
         m, pm = None, None
     best = _load().oracle_angle_price(n_a, po, prp, pm, ap.ctypes.data)
     return ap, int(best)
+
+
+def select_constrained(p_f32, angle_row_offset, leafrow_col_offset, leafrow_pos0, interdigitation: bool,
+                       angle_mask=None, L_lo=None, L_hi=None, R_lo=None, R_hi=None):
+    """O6: aperture selection with the interdigitation constraint of L135 and / or per-row leaf windows (L66):
+    (L, R, row_price, angle_price, best_angle).  See vmat_oracle.c for the readings."""
+    p, pp = _c(p_f32, np.float32)
+    aro, pa = _c(angle_row_offset, np.int32)
+    lco, pl = _c(leafrow_col_offset, np.int32)
+    u0, pu = _c(leafrow_pos0, np.int32)
+    n_a, n_rows = aro.size - 1, lco.size - 1
+    keep = [p, aro, lco, u0]
+
+    def opt(a, dt):
+        if a is None:
+            return None
+        arr, ptr = _c(a, dt)
+        keep.append(arr)
+        return ptr
+
+    pm = opt(angle_mask, np.uint8)
+    w = [opt(a, np.int32) for a in (L_lo, L_hi, R_lo, R_hi)]
+    L = np.zeros(n_rows, dtype=np.int32)
+    R = np.zeros(n_rows, dtype=np.int32)
+    rp = np.zeros(n_rows, dtype=np.float64)
+    ap = np.zeros(n_a, dtype=np.float64)
+    best = _load().oracle_select_constrained(n_a, pa, pl, pu, pp, pm, 1 if interdigitation else 0, w[0], w[1], w[2],
+                                             w[3], L.ctypes.data, R.ctypes.data, rp.ctypes.data, ap.ctypes.data)
+    return L, R, rp, ap, int(best)
 
 
 @dataclass

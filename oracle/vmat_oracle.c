@@ -114,3 +114,124 @@ int32_t oracle_angle_price(int32_t n_angles, const int32_t *angle_row_offset,
     }
     return best;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * O6 (NEXT-3) aperture selection under MLC hardware constraints, PAPER.md L133-L135 and L66:
+ *   "When there is an interdigitation constraint of MLC leaves in adjacent rows, that is,
+ *    L_{k,irow} <= min{R_{k,irow-1}, R_{k,irow+1}}, the MLC rows are not independent any longer ...
+ *    each thread would be responsible for one control point and for calculating the prices of all the
+ *    combinations of openings at different MLC rows that can satisfy the interdigitation constraint.
+ *    It would then choose the best aperture for that control point."                       (L135)
+ *   "the candidate apertures need to be compatible with those chosen apertures" (neighbouring
+ *    control points, L66): here per-row windows on the two leaf positions.
+ * Readings C22-C24 of DESIGN.md:
+ *   - A leaf row r of a control point has a state (a, b), a <= b: the physical positions of its left
+ *     and right leaf ends in beamlet widths on the control point's grid; row-local L = a - pos0[r],
+ *     R = b - pos0[r] (pos0 = physical column of the row's first beamlet).  Open states a < b need
+ *     pos0 <= a and b <= pos0 + n (they expose beamlets L .. R-1 of the row); a closed pair a == b
+ *     may be parked at any position of the control point's field range [Pmin, Pmax] = [min pos0,
+ *     max pos0 + n] over its non-empty rows (0, 0 when it has none).  The formula of L135 applies to
+ *     every row, closed ones included.
+ *   - Windows (each array may be NULL): L_lo[r] <= L <= L_hi[r], R_lo[r] <= R <= R_hi[r], row-local.
+ *   - Value of a state: V = S_R - S_L for an open one (S as in O4: FP64 prefix sums of the FP32
+ *     prices, left to right), 0 for a closed one.
+ *   - Interdigitation between adjacent rows r, r+1 of one control point: a_r <= b_{r+1} and
+ *     a_{r+1} <= b_r (L135 written for both rows of the pair).
+ *   - The aperture price is f_last with f_0 = V_0, f_r = V_r + min over compatible states s of row
+ *     r-1 of f_{r-1}(s): the exhaustive minimum over all combinations, organised row by row.
+ *   - Ties: the last row takes its smallest optimal state in the order (a, b); every earlier row
+ *     the smallest state, in the same order, among those attaining the minimum it feeds.
+ *   - A control point with no feasible combination: price +inf, rows L = R = 0, row prices 0.
+ * Returns the best control point as O5 does.  O(states^2) per row pair: the plain recursion, no
+ * prefix-minimum tables. */
+#include <stdlib.h>
+
+int32_t oracle_select_constrained(int32_t n_angles, const int32_t *angle_row_offset,
+                                  const int32_t *leafrow_col_offset, const int32_t *pos0, const float *p,
+                                  const uint8_t *angle_mask, int32_t interdigitation,
+                                  const int32_t *L_lo, const int32_t *L_hi, const int32_t *R_lo,
+                                  const int32_t *R_hi, int32_t *Lout, int32_t *Rout, double *row_price,
+                                  double *angle_price)
+{
+    int32_t best_angle = -1;
+    double best_price = 0.0;
+    for (int32_t k = 0; k < n_angles; ++k) {
+        const int32_t r0 = angle_row_offset[k], r1 = angle_row_offset[k + 1], nr = r1 - r0;
+        for (int32_t r = r0; r < r1; ++r) { Lout[r] = 0; Rout[r] = 0; row_price[r] = 0.0; }
+        if (angle_mask && angle_mask[k]) { angle_price[k] = INFINITY; continue; }
+        if (nr == 0) { angle_price[k] = 0.0; continue; }
+        /* field range of the control point */
+        int32_t Pmin = 0, Pmax = 0, any = 0, nmax = 0;
+        for (int32_t r = r0; r < r1; ++r) {
+            const int32_t n = leafrow_col_offset[r + 1] - leafrow_col_offset[r];
+            if (n <= 0) continue;
+            if (!any || pos0[r] < Pmin) Pmin = pos0[r];
+            if (!any || pos0[r] + n > Pmax) Pmax = pos0[r] + n;
+            if (n > nmax) nmax = n;
+            any = 1;
+        }
+        const int32_t Wd = Pmax - Pmin + 1;
+        const size_t cap = (size_t)Wd * (Wd + 1) / 2;                    /* states per row at most */
+        int32_t *sa = (int32_t *)malloc(sizeof(int32_t) * cap * nr), *sb = (int32_t *)malloc(sizeof(int32_t) * cap * nr);
+        int32_t *arg = (int32_t *)malloc(sizeof(int32_t) * cap * nr), *cnt = (int32_t *)malloc(sizeof(int32_t) * nr);
+        double *V = (double *)malloc(sizeof(double) * cap * nr), *f = (double *)malloc(sizeof(double) * cap * nr);
+        double *S = (double *)malloc(sizeof(double) * (nmax + 1));
+        int feasible = 1;
+        for (int32_t q = 0; q < nr && feasible; ++q) {
+            const int32_t r = r0 + q, j0 = leafrow_col_offset[r], n = leafrow_col_offset[r + 1] - j0;
+            const int32_t u0 = n > 0 ? pos0[r] : Pmin;                    /* empty rows: row-local = offset from Pmin */
+            S[0] = 0.0;
+            for (int32_t c = 0; c < n; ++c) S[c + 1] = S[c] + (double)p[j0 + c];
+            int32_t m = 0;
+            for (int32_t a = Pmin; a <= Pmax; ++a)
+                for (int32_t b = a; b <= Pmax; ++b) {
+                    const int32_t L = a - u0, R = b - u0;
+                    if (a < b && !(n > 0 && L >= 0 && R <= n)) continue;  /* an open state exposes existing beamlets */
+                    if (L_lo && L < L_lo[r]) continue;
+                    if (L_hi && L > L_hi[r]) continue;
+                    if (R_lo && R < R_lo[r]) continue;
+                    if (R_hi && R > R_hi[r]) continue;
+                    sa[q * cap + m] = a; sb[q * cap + m] = b;
+                    V[q * cap + m] = a < b ? S[R] - S[L] : 0.0;
+                    ++m;
+                }
+            cnt[q] = m;
+            /* the recursion */
+            for (int32_t t = 0; t < m; ++t) {
+                if (q == 0) { f[t] = V[t]; arg[t] = -1; continue; }
+                double bestf = INFINITY;
+                int32_t bests = -1;
+                for (int32_t s = 0; s < cnt[q - 1]; ++s) {
+                    const double fs = f[(q - 1) * cap + s];
+                    if (interdigitation) {
+                        if (sa[(q - 1) * cap + s] > sb[q * cap + t]) continue;       /* a_{r-1} <= b_r  */
+                        if (sa[q * cap + t] > sb[(q - 1) * cap + s]) continue;       /* a_r <= b_{r-1}  */
+                    }
+                    if (fs < bestf) { bestf = fs; bests = s; }                       /* strict: first in (a,b) order */
+                }
+                f[q * cap + t] = bests >= 0 ? V[q * cap + t] + bestf : INFINITY;
+                arg[q * cap + t] = bests;
+            }
+            int ok = 0;
+            for (int32_t t = 0; t < m; ++t) ok |= f[q * cap + t] < INFINITY;
+            if (!ok) feasible = 0;
+        }
+        if (!feasible) angle_price[k] = INFINITY;
+        else {
+            int32_t t = -1;
+            double bf = INFINITY;
+            for (int32_t s = 0; s < cnt[nr - 1]; ++s)
+                if (f[(nr - 1) * cap + s] < bf) { bf = f[(nr - 1) * cap + s]; t = s; }
+            angle_price[k] = bf;
+            for (int32_t q = nr - 1; q >= 0; --q) {
+                const int32_t r = r0 + q, n = leafrow_col_offset[r + 1] - leafrow_col_offset[r];
+                const int32_t u0 = n > 0 ? pos0[r] : Pmin;
+                Lout[r] = sa[q * cap + t] - u0; Rout[r] = sb[q * cap + t] - u0; row_price[r] = V[q * cap + t];
+                t = arg[q * cap + t];
+            }
+            if (bf < best_price) { best_price = bf; best_angle = k; }
+        }
+        free(sa); free(sb); free(arg); free(cnt); free(V); free(f); free(S);
+    }
+    return best_angle;
+}

@@ -164,6 +164,11 @@ class Phantom:
     struct_w_over: torch.Tensor
     struct_w_under: torch.Tensor
     angles_generated: Sequence[int] = field(default_factory=list)
+    # MLC geometry for the constrained selection (NEXT-3): physical column (in beamlet widths, on the control
+    # point's potential grid) of the first beamlet of every leaf row, host int32 [n_rows_total] (0 for empty
+    # rows), and the control points of every arc, host int32 [n_arcs+1]
+    leafrow_pos0: Optional[torch.Tensor] = None
+    arc_angle_offset: Optional[torch.Tensor] = None
 
     @property
     def nnz(self) -> int:
@@ -467,7 +472,11 @@ def generate(spec: PhantomSpec, device="cpu", angles: Optional[Sequence[int]] = 
         voxel_struct=sid.cpu(), struct_T=torch.tensor(T, dtype=torch.float32),
         struct_w_over=torch.tensor(wo, dtype=torch.float32),
         struct_w_under=torch.tensor(wu, dtype=torch.float32),
-        angles_generated=todo)
+        angles_generated=todo,
+        leafrow_pos0=torch.cat([torch.where(cx >= cn, cn, torch.zeros_like(cn)) for cn, cx in zip(cmins, cmaxs)]
+                               ).to(torch.int32),
+        arc_angle_offset=torch.tensor([sum(a.n_angles for a in spec.arcs[:i]) for i in range(len(spec.arcs) + 1)],
+                                      dtype=torch.int32))
 
 
 def draw_x(n_beamlets: int, eval_index: int, device="cpu", scale: float = 1.0) -> torch.Tensor:
