@@ -175,6 +175,35 @@ int vmat_aperture_dose(const vmat_ddc *h, int32_t angle, const int32_t *L, const
                        float *x_scratch, float *DA, void *stream);
 
 /* ------------------------------------------------------------------------------------------------------
+ * NEXT-3: aperture selection under MLC hardware constraints.
+ *
+ * MLC geometry, once per handle: leafrow_pos0 host int32 [n_leaf_rows] = physical column (in beamlet widths, on
+ * the control point's own grid) of the first beamlet of every leaf row (ignored for rows without beamlets).  The
+ * field range of a control point is [Pmin, Pmax] = [min pos0, max pos0 + n] over its non-empty rows and may span
+ * at most 255 beamlet widths (and what fits the SM's shared memory: ~148 on B200).  Synchronous. */
+int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0);
+
+/* A4 + A5 with constraints.  A leaf row has a state (a, b), a <= b: the physical positions of its two leaf ends;
+ * row-local L = a - pos0, R = b - pos0 (C8).  Open states (a < b) lie inside the row's beamlets, 0 <= L < R <= n;
+ * a closed pair (a == b, value 0) may be parked anywhere in the control point's field range, so for a closed row
+ * L = R may be negative or exceed n (rows without beamlets count from Pmin).  Readings C22-C24:
+ *   interdigitation != 0: adjacent rows r, r+1 of a control point must satisfy a_r <= b_{r+1} and a_{r+1} <= b_r
+ *       (L135: "L_{k,irow} <= min{R_{k,irow-1}, R_{k,irow+1}}", for every row, closed ones included);
+ *   windows (L66: apertures "compatible with those chosen" at neighbouring control points): L_lo[r] <= L <= L_hi[r],
+ *       R_lo[r] <= R <= R_hi[r]; each of the four dev int32 [n_leaf_rows] arrays may be NULL (no bound).
+ * Per control point the aperture minimising the summed price over ALL feasible combinations of row states is
+ * returned (the paper enumerates them; here a row-by-row recursion with exact minima): value of a state V = S_R -
+ * S_L as in vmat_select_apertures (C6), aperture price = V_last + (... + (V_1 + V_0)).  Ties: the last row takes its
+ * smallest optimal state in (a, b) order, every earlier row the smallest state attaining the minimum it feeds.  A
+ * control point without a feasible combination (or occupied, angle_mask) gets price +inf and L = R = 0.  Unlike
+ * vmat_select_apertures an aperture is reported even when its price is >= 0; best_angle is -1 then.
+ * Outputs as vmat_select_apertures; bit-identical to the oracle on the same FP32 p.  Asynchronous. */
+int vmat_select_apertures_constrained(vmat_ddc *h, const float *p, const uint8_t *angle_mask, int32_t interdigitation,
+                                      const int32_t *L_lo, const int32_t *L_hi, const int32_t *R_lo,
+                                      const int32_t *R_hi, int32_t *L, int32_t *R, double *row_price,
+                                      double *angle_price, int32_t *best_angle, void *stream);
+
+/* ------------------------------------------------------------------------------------------------------
  * NEXT-2: the master problem (MP), Eq. (6)-(10) L70-L101 and the four BB steps of L139.
  * With the apertures chosen so far and their dose vectors DA(A_k) (Eq. (5)), find fluence rates
  * y_k in [y_lo_k, y_hi_k] (Eq. (6): R^L/S^U_k and R^U/S^L_k, supplied by the caller) minimising F(z),

@@ -32,6 +32,7 @@ EXPORTS = [
     "vmat_aperture_dose", "vmat_ddc_set_profile_events", "vmat_last_error", "vmat_last_launch_count",
     "vmat_mp_create", "vmat_mp_destroy", "vmat_mp_reset", "vmat_mp_add_aperture", "vmat_mp_set_fluence", "vmat_mp_size",
     "vmat_mp_solve", "vmat_mp_history", "vmat_column_generation",
+    "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained",
 ]
 
 
@@ -83,6 +84,8 @@ def load_library():
     lib.vmat_mp_history.argtypes = [vp, vp, vp]
     lib.vmat_column_generation.argtypes = [vp, vp, vp, i32, vp, vp, vp, i32, f64, f64, i32, f64, f64, vp, vp, vp,
                                            vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.vmat_ddc_set_leaf_geometry.argtypes = [vp, vp]
+    lib.vmat_select_apertures_constrained.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_last_error.restype = ctypes.c_char_p
     lib.vmat_last_launch_count.restype = ctypes.c_int
     for name in EXPORTS:
@@ -260,6 +263,28 @@ def vmat_select_apertures(h: DDC, p: torch.Tensor, angle_mask: Optional[torch.Te
         _ptr(L, torch.int32, "cuda", h.n_leaf_rows), _ptr(R, torch.int32, "cuda", h.n_leaf_rows),
         _ptr(row_price, torch.float64, "cuda", h.n_leaf_rows), _ptr(angle_price, torch.float64, "cuda", h.n_angles),
         _ptr(best_angle, torch.int32, "cuda", 1), _stream()))
+
+
+def vmat_ddc_set_leaf_geometry(h: DDC, leafrow_pos0: torch.Tensor):
+    """NEXT-3: physical column of the first beamlet of every leaf row (host int32 [n_leaf_rows])."""
+    pos0 = leafrow_pos0.to(torch.int32).cpu().contiguous()
+    if pos0.numel() != h.n_leaf_rows:
+        raise ValueError("leafrow_pos0 must have n_leaf_rows entries")
+    with torch.cuda.device(h.device):
+        _check(load_library().vmat_ddc_set_leaf_geometry(h._h, pos0.data_ptr() if pos0.numel() else None))
+
+
+def vmat_select_apertures_constrained(h: DDC, p: torch.Tensor, angle_mask: Optional[torch.Tensor],
+                                      interdigitation: bool, L, R, row_price, angle_price, best_angle,
+                                      L_lo=None, L_hi=None, R_lo=None, R_hi=None):
+    """NEXT-3: A4 + A5 under the interdigitation constraint (L135) and / or per-row leaf windows (L66)."""
+    n = h.n_leaf_rows
+    _check(load_library().vmat_select_apertures_constrained(
+        h._h, _ptr(p, torch.float32, "cuda", h.n_beamlets), _ptr(angle_mask, torch.uint8, "cuda", h.n_angles),
+        1 if interdigitation else 0, _ptr(L_lo, torch.int32, "cuda", n), _ptr(L_hi, torch.int32, "cuda", n),
+        _ptr(R_lo, torch.int32, "cuda", n), _ptr(R_hi, torch.int32, "cuda", n),
+        _ptr(L, torch.int32, "cuda", n), _ptr(R, torch.int32, "cuda", n), _ptr(row_price, torch.float64, "cuda", n),
+        _ptr(angle_price, torch.float64, "cuda", h.n_angles), _ptr(best_angle, torch.int32, "cuda", 1), _stream()))
 
 
 def vmat_price_eval(h: DDC, x: torch.Tensor, obj: Objective, out: PriceEvalOut,

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <limits.h>
 #include <vector>
 #include "../../include/vmat.h"
 
@@ -95,6 +96,15 @@ struct vmat_ddc {
     int64_t bytes_device = 0;
     int device = 0;
     cudaEvent_t prof_ev[4] = {nullptr, nullptr, nullptr, nullptr};   // vmat_ddc_set_profile_events
+    // NEXT-3 (constrained.cu): MLC geometry, set by vmat_ddc_set_leaf_geometry
+    int32_t *leafrow_pos0 = nullptr;        // [n_leaf_rows] physical column of each leaf row's first beamlet
+    int32_t *angle_pmin = nullptr;          // [n_angles] left end of the control point's field range
+    int32_t *angle_wd = nullptr;            // [n_angles] positions in the field range (Pmax - Pmin + 1)
+    int64_t *angle_bp_offset = nullptr;     // [n_angles+1] start of the control point's back-pointer tables in cs_bp
+    uint16_t *cs_bp = nullptr;              // back pointers of the row-by-row recursion (allocated on first use)
+    int64_t cs_bp_elems = 0, cs_bp_alloc = 0;
+    int32_t cs_max_wd = 0;
+    std::vector<int32_t> h_leafrow_pos0;
     // scratch for the end-to-end host call (allocated on first use)
     float *e2e_x = nullptr, *e2e_d = nullptr, *e2e_g = nullptr, *e2e_p = nullptr;
     int32_t *e2e_L = nullptr, *e2e_R = nullptr, *e2e_best = nullptr;
@@ -199,3 +209,7 @@ int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *a
                              int32_t *L, int32_t *R, double *row_price, cudaStream_t st);
 int vmat_launch_angle_price(const vmat_ddc *h, const double *row_price, const uint8_t *angle_mask,
                             double *angle_price, int32_t *best_angle, cudaStream_t st);
+int vmat_launch_select_constrained(vmat_ddc *h, const float *p, const uint8_t *angle_mask, int interdigitation,
+                                   const int32_t *L_lo, const int32_t *L_hi, const int32_t *R_lo, const int32_t *R_hi,
+                                   int32_t *L, int32_t *R, double *row_price, double *angle_price, int32_t *best_angle,
+                                   cudaStream_t st);

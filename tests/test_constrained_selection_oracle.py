@@ -135,8 +135,16 @@ def config0_prices(scale):
     return ph, ev
 
 
-def satisfies_interdigitation(L, R, pos0, aro):
-    a, b = L + pos0, R + pos0
+def satisfies_interdigitation(L, R, pos0, aro, lco=None):
+    """L135 for every adjacent pair of rows, in physical positions (rows without beamlets count from Pmin)."""
+    u0 = np.array(pos0, dtype=np.int64)
+    if lco is not None:
+        n = np.diff(lco)
+        for k in range(len(aro) - 1):
+            sl = slice(aro[k], aro[k + 1])
+            ne = n[sl] > 0
+            u0[sl][~ne] = u0[sl][ne].min() if ne.any() else 0
+    a, b = L + u0, R + u0
     for k in range(len(aro) - 1):
         for r in range(aro[k], aro[k + 1] - 1):
             if a[r] > b[r + 1] or a[r + 1] > b[r]:
