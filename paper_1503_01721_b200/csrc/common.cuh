@@ -100,10 +100,9 @@ struct vmat_ddc {
     int32_t *leafrow_pos0 = nullptr;        // [n_leaf_rows] physical column of each leaf row's first beamlet
     int32_t *angle_pmin = nullptr;          // [n_angles] left end of the control point's field range
     int32_t *angle_wd = nullptr;            // [n_angles] positions in the field range (Pmax - Pmin + 1)
-    int64_t *angle_bp_offset = nullptr;     // [n_angles+1] start of the control point's back-pointer tables in cs_bp
-    uint16_t *cs_bp = nullptr;              // back pointers of the row-by-row recursion (allocated on first use)
-    int64_t cs_bp_elems = 0, cs_bp_alloc = 0;
-    int32_t cs_max_wd = 0;
+    int64_t *row_bp_offset = nullptr;       // [n_leaf_rows+1] start of each leaf row's back pointers in cs_bp
+    uint16_t *cs_bp = nullptr;              // back pointers of the row-by-row recursion: per row wd + (n+1)^2
+    int32_t cs_max_wd = 0, cs_max_n = 0;
     std::vector<int32_t> h_leafrow_pos0;
     // scratch for the end-to-end host call (allocated on first use)
     float *e2e_x = nullptr, *e2e_d = nullptr, *e2e_g = nullptr, *e2e_p = nullptr;

@@ -8,12 +8,16 @@
 // The paper enumerates the combinations with one thread per control point.  Here one CTA owns a control point
 // and walks its leaf rows once: f_r(a,b) = V_r(a,b) + min{ f_{r-1}(a',b') : a' <= b, a <= b' } is the exact
 // minimum over all compatible combinations of rows 0..r ending in state (a,b) (readings C22-C24).
-// The inner minimum is a 2-D dominance query, answered for every (a,b) at once by a prefix-minimum table
-//   M_r[x][y] = min{ f_r(a',b') : a' <= x, b' >= y }      (so the query above is M_{r-1}[b][a]),
-// built in shared memory by two sweeps (down the columns, then right-to-left along the rows).  The table holds
-// Wd x Wd doubles, Wd = positions of the control point's field range; minima carry their arg (a',b') packed in
-// 16 bits, smaller packed value = smaller (a',b') in lexicographic order = the oracle's tie rule.  The arg tables
-// go to global memory row by row and are walked backwards by one thread at the end.
+// The inner minimum is a 2-D dominance query.  The states of a row are its closed pairs (c,c), c anywhere in
+// the control point's field range (wd positions), and its open states inside its own n beamlets, so the query
+// splits into
+//   - a range minimum of the previous row's closed values over c in [a, b], carried along as b grows, and
+//   - a look-up in the prefix-minimum table PB[I][J] = min{ f(i,j) : i <= I, j >= J, i < j } of the previous
+//     row's open states (row-local i, j), built in shared memory by two sweeps of n+1 steps.
+// Work per row is O(n^2 + wd) instead of the O(wd^2) of a table over the whole field range (the first version of
+// this kernel: 10.4 ms per call on config 3, where rows hold 14 beamlets on average in fields 100-130 wide).
+// Minima carry their arg (a',b') packed in 16 bits; a smaller packed value is a smaller (a',b') in lexicographic
+// order = the oracle's tie rule.  Every state's predecessor goes to global memory and one thread walks them back.
 // Every value is produced by the oracle's operations in the oracle's order (S_R - S_L, then V + minimum; minima
 // are exact), so leaf positions, row prices and aperture prices are bit-identical to oracle_select_constrained
 // applied to the same FP32 price vector.
@@ -21,8 +25,15 @@
 
 constexpr int CS_THREADS = 256;
 constexpr int CS_MAX_POS = 255;                       // positions are packed in 8 bits each
+constexpr unsigned CS_NONE = 0xffffu;
 
 __device__ __forceinline__ double cs_inf() { return __longlong_as_double(0x7ff0000000000000LL); }
+
+// (v, g) <- the smaller of (v, g) and (c, cg): by value, ties by packed arg
+__device__ __forceinline__ void cs_take(double &v, unsigned &g, double c, unsigned cg)
+{
+    if (c < v || (c == v && cg < g)) { v = c; g = cg; }
+}
 
 // FP64 prefix sums of every leaf row, left to right (C6): S[j0 + r + c], c = 0 .. n.  One thread per leaf row.
 __global__ void k_cs_prefix(int n_rows, const int32_t *__restrict__ leafrow_col_offset, const float *__restrict__ p,
@@ -39,7 +50,7 @@ __global__ void k_cs_prefix(int n_rows, const int32_t *__restrict__ leafrow_col_
 
 struct CsArgs {
     const int32_t *angle_row_offset, *leafrow_col_offset, *pos0, *angle_pmin, *angle_wd;
-    const int64_t *angle_bp_offset;
+    const int64_t *row_bp_offset;
     const uint8_t *angle_mask;
     const int32_t *L_lo, *L_hi, *R_lo, *R_hi;         // each may be NULL
     const double *S;
@@ -47,12 +58,13 @@ struct CsArgs {
     int32_t *L, *R;
     double *row_price, *angle_price;
     int interdigitation;
+    int tab_n, max_wd;                                // shared-memory table: tab_n x tab_n entries; fc arrays: max_wd
 };
 
-__device__ __forceinline__ int cs_stride_d(int wd) { return wd | 1; }                 // doubles per table row: odd
-__device__ __forceinline__ int cs_stride_a(int wd)                                  // u16 per arg row: 2 * odd
+static __host__ __device__ __forceinline__ int cs_stride_d(int t) { return t | 1; }   // doubles per table row: odd
+static __host__ __device__ __forceinline__ int cs_stride_a(int t)                     // u16 per arg row: 2 * odd
 {
-    int s = (wd + 1) & ~1;
+    const int s = (t + 1) & ~1;
     return ((s >> 1) & 1) ? s : s + 2;
 }
 
@@ -60,104 +72,217 @@ __global__ void __launch_bounds__(CS_THREADS)
 k_cs_dp(CsArgs A)
 {
     extern __shared__ __align__(16) unsigned char cs_smem[];
-    const int k = blockIdx.x;
+    const int k = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int r0 = A.angle_row_offset[k], r1 = A.angle_row_offset[k + 1], nr = r1 - r0;
     const bool masked = A.angle_mask != nullptr && A.angle_mask[k] != 0;
     if (masked || nr == 0) {                                                          // C7: occupied control point
-        for (int r = r0 + threadIdx.x; r < r1; r += CS_THREADS) { A.L[r] = 0; A.R[r] = 0; A.row_price[r] = 0.0; }
-        if (threadIdx.x == 0) A.angle_price[k] = masked ? cs_inf() : 0.0;
+        for (int r = r0 + tid; r < r1; r += CS_THREADS) { A.L[r] = 0; A.R[r] = 0; A.row_price[r] = 0.0; }
+        if (tid == 0) A.angle_price[k] = masked ? cs_inf() : 0.0;
         return;
     }
     const int pmin = A.angle_pmin[k], wd = A.angle_wd[k];
-    const int SD = cs_stride_d(wd), SA = cs_stride_a(wd);
-    double *T = (double *)cs_smem;                                                    // [wd][SD]
-    uint16_t *G = (uint16_t *)(T + (size_t)wd * SD);                                  // [wd][SA]
-    __shared__ double s_gmin;
-    uint16_t *bp_k = A.bp + A.angle_bp_offset[k];
-    const size_t bp_row = A.interdigitation ? (size_t)wd * wd : 1;                    // u16 stored per leaf row
-    const int cells = wd * wd;
+    const int SD = cs_stride_d(A.tab_n), SA = cs_stride_a(A.tab_n);
+    // PB [tab_n][SD]: on and below the diagonal the prefix minima of the PREVIOUS row's open states (the queries
+    // read PB[I][J] with I >= J only); strictly above it the open states of THIS row are written while those
+    // queries run - the two regions never meet, so one table serves both rows.
+    double *PB = (double *)cs_smem;
+    double *fcp = PB + (size_t)A.tab_n * SD;                                          // [max_wd] closed states, previous row
+    double *fcn = fcp + A.max_wd;                                                     // [max_wd] closed states, this row
+    double *Sa = fcn + A.max_wd;                                                      // [tab_n] prefix sums of this row ...
+    double *Sb = Sa + A.tab_n;                                                        // [tab_n] ... and of the next one
+    uint16_t *PG = (uint16_t *)(Sb + A.tab_n);                                        // [tab_n][SA] args of PB
+    __shared__ double s_gv;                                                           // minimum of the previous row ...
+    __shared__ unsigned s_ga;                                                         // ... and its smallest state
+    const bool inter = A.interdigitation != 0;
+    int np = 0, offp = 0;                                                             // previous row: beamlets, table position of its 0
+    {
+        const int j0 = A.leafrow_col_offset[r0], n = A.leafrow_col_offset[r0 + 1] - j0;
+        for (int t = tid; t <= n; t += CS_THREADS) Sa[t] = A.S[j0 + r0 + t];
+    }
+    __syncthreads();
     for (int q = 0; q < nr; ++q) {
         const int r = r0 + q;
-        const int j0 = A.leafrow_col_offset[r], n = A.leafrow_col_offset[r + 1] - j0;
-        const int off = n > 0 ? A.pos0[r] - pmin : 0;                                 // table position of row-local 0
+        const int j0 = A.leafrow_col_offset[r], n = A.leafrow_col_offset[r + 1] - j0, n1 = n + 1;
+        const int off = n > 0 ? A.pos0[r] - pmin : 0;
         const int llo = A.L_lo ? A.L_lo[r] : INT_MIN, lhi = A.L_hi ? A.L_hi[r] : INT_MAX;
         const int rlo = A.R_lo ? A.R_lo[r] : INT_MIN, rhi = A.R_hi ? A.R_hi[r] : INT_MAX;
-        const double *S = A.S + j0 + r;
-        if (q > 0 && threadIdx.x == 0) s_gmin = T[(size_t)(wd - 1) * SD];             // M[wd-1][0]: the row's minimum
-        __syncthreads();
-        // ---- f_q(a,b) for a <= b: reads M_{q-1}[b][a] (on or below the diagonal), writes on or above it
-        for (int e = threadIdx.x; e < cells; e += CS_THREADS) {
-            const int a = e / wd, b = e - a * wd;
-            if (a > b) continue;
-            const int L = a - off, R = b - off;
-            bool ok = L >= llo && L <= lhi && R >= rlo && R <= rhi;
-            if (a < b) ok = ok && n > 0 && L >= 0 && R <= n;                          // an open state exposes existing beamlets
+        uint16_t *bp_row = A.bp + A.row_bp_offset[r];
+        const bool first = q == 0, last = q == nr - 1;
+        const bool query = !first && inter;                                           // predecessors depend on the state
+        double gv = 0.0;
+        unsigned ga = CS_NONE;
+        if (!first && !inter) { gv = s_gv; ga = s_ga; }
+        // ---- closed states (c,c), c anywhere in the field range
+        for (int c = tid; c < wd; c += CS_THREADS) {
+            const int Lc = c - off;
             double f = cs_inf();
-            if (ok) {
-                const double V = a < b ? S[R] - S[L] : 0.0;
-                if (q == 0) f = V;
+            unsigned pg = CS_NONE;
+            if (Lc >= llo && Lc <= lhi && Lc >= rlo && Lc <= rhi) {
+                if (first) f = 0.0;
                 else {
-                    const double m = A.interdigitation ? T[(size_t)b * SD + a] : s_gmin;
-                    f = V + m;                                                        // +inf when no compatible predecessor
+                    double pv = gv;
+                    unsigned pa = ga;
+                    if (inter) {                                                      // a' <= c <= b'
+                        pv = fcp[c]; pa = (unsigned)((c << 8) | c);
+                        const int I = c - offp;
+                        if (np > 0 && I >= 0 && I <= np) cs_take(pv, pa, PB[(size_t)I * SD + I], PG[(size_t)I * SA + I]);
+                    }
+                    f = 0.0 + pv;
+                    pg = pa;
                 }
             }
-            T[(size_t)a * SD + b] = f;
-            G[(size_t)a * SA + b] = (uint16_t)((a << 8) | b);
+            fcn[c] = f;
+            bp_row[c] = (uint16_t)pg;
         }
-        __syncthreads();
-        for (int e = threadIdx.x; e < cells; e += CS_THREADS) {                       // no states below the diagonal
-            const int a = e / wd, b = e - a * wd;
-            if (a > b) { T[(size_t)a * SD + b] = cs_inf(); G[(size_t)a * SA + b] = 0xffffu; }
-        }
-        __syncthreads();
-        // ---- sweep 1: down every column b: min over a' <= a (ascending a: strict < keeps the smaller arg)
-        if (threadIdx.x < wd) {
-            const int b = threadIdx.x;
-            double v = cs_inf();
-            uint16_t g = 0xffffu;
-            for (int a = 0; a < wd; ++a) {
-                const double c = T[(size_t)a * SD + b];
-                if (c < v) { v = c; g = G[(size_t)a * SA + b]; }
-                T[(size_t)a * SD + b] = v;
-                G[(size_t)a * SA + b] = g;
+        // ---- open states (off+i, off+j), 0 <= i < j <= n: thread i walks j upwards, four at a time (loads first),
+        //      and carries the range minimum of the previous row's closed states over [a, b]
+        for (int i = tid; i < n; i += CS_THREADS) {
+            const int a = off + i;
+            double rv = cs_inf();
+            unsigned ra = CS_NONE;
+            if (query) { rv = fcp[a]; ra = (unsigned)((a << 8) | a); }
+            const double Si = Sa[i];
+            const int J = a - offp, Jc = max(J, 0);
+            const bool okL = i >= llo && i <= lhi;
+            for (int jb = i + 1; jb <= n; jb += 4) {
+                double cf[4], cS[4], cp[4];
+                unsigned cg[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int j = min(jb + u, n), b = off + j, I = b - offp;
+                    cS[u] = Sa[j];
+                    cf[u] = cs_inf(); cp[u] = cs_inf(); cg[u] = CS_NONE;
+                    if (query) {
+                        cf[u] = fcp[b];
+                        if (np > 0 && I >= 0 && J <= np) {                            // a' <= b and b' >= a
+                            const int Ic = min(I, np);
+                            cp[u] = PB[(size_t)Ic * SD + Jc];
+                            cg[u] = PG[(size_t)Ic * SA + Jc];
+                        }
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int j = jb + u, b = off + j;
+                    if (j > n) break;
+                    if (query && cf[u] < rv) { rv = cf[u]; ra = (unsigned)((b << 8) | b); }   // ascending b: strict < keeps the leftmost
+                    double f = cs_inf();
+                    unsigned pg = CS_NONE;
+                    if (okL && j >= rlo && j <= rhi) {
+                        const double V = cS[u] - Si;
+                        if (first) f = V;
+                        else {
+                            double pv = gv;
+                            unsigned pa = ga;
+                            if (inter) { pv = rv; pa = ra; cs_take(pv, pa, cp[u], cg[u]); }
+                            f = V + pv;                                               // +inf when no compatible predecessor
+                            pg = pa;
+                        }
+                    }
+                    PB[(size_t)i * SD + j] = f;
+                    PG[(size_t)i * SA + j] = (uint16_t)((a << 8) | b);
+                    bp_row[wd + j * n1 + i] = (uint16_t)pg;
+                }
             }
         }
-        __syncthreads();
-        // ---- sweep 2: along every row a from the right: min over b' >= b; ties -> smaller packed arg
-        if (threadIdx.x < wd) {
-            const int a = threadIdx.x;
-            double v = cs_inf();
-            uint16_t g = 0xffffu;
-            for (int b = wd - 1; b >= 0; --b) {
-                const double c = T[(size_t)a * SD + b];
-                const uint16_t cg = G[(size_t)a * SA + b];
-                if (c < v || (c == v && cg < g)) { v = c; g = cg; }
-                T[(size_t)a * SD + b] = v;
-                G[(size_t)a * SA + b] = g;
-            }
+        if (!last) {                                                                  // prefix sums of the next row
+            const int jn = A.leafrow_col_offset[r + 1], nn = A.leafrow_col_offset[r + 2] - jn;
+            for (int t = tid; t <= nn; t += CS_THREADS) Sb[t] = A.S[jn + r + 1 + t];
         }
         __syncthreads();
-        // ---- the arg table of this row goes to global memory for the walk back
-        uint16_t *dst = bp_k + (size_t)q * bp_row;
-        if (A.interdigitation) {
-            for (int e = threadIdx.x; e < cells; e += CS_THREADS) {
-                const int x = e / wd, y = e - x * wd;
-                dst[e] = G[(size_t)x * SA + y];
+        // ---- PB of this row: sweep down the columns, then along the rows from the right
+        if (n > 0) {
+            if (tid <= n) {                                                           // min over i' <= i (ascending: strict <)
+                const int j = tid;
+                double v = cs_inf();
+                unsigned g = CS_NONE;
+                for (int i0 = 0; i0 <= n; i0 += 4) {
+                    double c[4];
+                    unsigned cg[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int i = min(i0 + u, n);
+                        const bool st = i < j;                                        // states live strictly above the diagonal
+                        c[u] = st ? PB[(size_t)i * SD + j] : cs_inf();
+                        cg[u] = st ? PG[(size_t)i * SA + j] : CS_NONE;
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int i = i0 + u;
+                        if (i <= n) {
+                            if (c[u] < v) { v = c[u]; g = cg[u]; }
+                            PB[(size_t)i * SD + j] = v;
+                            PG[(size_t)i * SA + j] = (uint16_t)g;
+                        }
+                    }
+                }
             }
-        } else if (threadIdx.x == 0) dst[0] = G[(size_t)(wd - 1) * SA];
+            __syncthreads();
+            if (tid <= n) {                                                           // min over j' >= j; ties -> smaller arg
+                const int i = tid;
+                double v = cs_inf();
+                unsigned g = CS_NONE;
+                for (int jt = n; jt >= 0; jt -= 4) {
+                    double c[4];
+                    unsigned cg[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int j = max(jt - u, 0);
+                        c[u] = PB[(size_t)i * SD + j];
+                        cg[u] = PG[(size_t)i * SA + j];
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int j = jt - u;
+                        if (j >= 0) {
+                            cs_take(v, g, c[u], cg[u]);
+                            PB[(size_t)i * SD + j] = v;
+                            PG[(size_t)i * SA + j] = (uint16_t)g;
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+        }
+        // ---- the row's minimum and its smallest state: the predecessor of every state of the next row when the
+        //      rows are independent, and the whole answer after the last row
+        if (!inter || last) {
+            if (warp == 0) {
+                double v = cs_inf();
+                unsigned g = CS_NONE;
+                for (int c = lane; c < wd; c += 32) {
+                    const double x = fcn[c];
+                    if (x < v) { v = x; g = (unsigned)((c << 8) | c); }
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    const double ov = __shfl_xor_sync(0xffffffffu, v, o);
+                    const unsigned og = __shfl_xor_sync(0xffffffffu, g, o);
+                    cs_take(v, g, ov, og);
+                }
+                if (lane == 0) {
+                    if (n > 0) cs_take(v, g, PB[(size_t)n * SD], PG[(size_t)n * SA]);
+                    s_gv = v;
+                    s_ga = g;
+                }
+            }
+            __syncthreads();
+        }
+        double *t = fcp; fcp = fcn; fcn = t;
+        t = Sa; Sa = Sb; Sb = t;
+        np = n; offp = off;
     }
-    __syncthreads();                                                                  // the stores above are visible to thread 0
-    if (threadIdx.x != 0) return;
-    const double total = T[(size_t)(wd - 1) * SD];
+    if (tid != 0) return;
+    const double total = s_gv;
     if (!(total < cs_inf())) {                                                        // no feasible combination
         for (int r = r0; r < r1; ++r) { A.L[r] = 0; A.R[r] = 0; A.row_price[r] = 0.0; }
         A.angle_price[k] = cs_inf();
         return;
     }
     A.angle_price[k] = total;
-    int g = G[(size_t)(wd - 1) * SA];
+    unsigned g = s_ga;
     for (int q = nr - 1; q >= 0; --q) {
-        const int r = r0 + q, a = g >> 8, b = g & 255;
+        const int r = r0 + q, a = (int)(g >> 8), b = (int)(g & 255u);
         const int j0 = A.leafrow_col_offset[r], n = A.leafrow_col_offset[r + 1] - j0;
         const int off = n > 0 ? A.pos0[r] - pmin : 0;
         const double *S = A.S + j0 + r;
@@ -165,8 +290,8 @@ k_cs_dp(CsArgs A)
         A.R[r] = b - off;
         A.row_price[r] = a < b ? S[b - off] - S[a - off] : 0.0;
         if (q > 0) {
-            const uint16_t *src = bp_k + (size_t)(q - 1) * bp_row;
-            g = A.interdigitation ? src[(size_t)b * wd + a] : src[0];
+            const uint16_t *bp_row = A.bp + A.row_bp_offset[r];
+            g = a == b ? bp_row[a] : bp_row[wd + (b - off) * (n + 1) + (a - off)];
         }
     }
 }
@@ -192,12 +317,10 @@ k_cs_best(int n_angles, const double *__restrict__ angle_price, int32_t *__restr
     }
 }
 
-static size_t cs_smem_bytes(int wd)
+static size_t cs_smem_bytes(int tab_n, int max_wd)
 {
-    const int SD = wd | 1;
-    int SA = (wd + 1) & ~1;
-    if (!((SA >> 1) & 1)) SA += 2;
-    return (size_t)wd * SD * 8 + (size_t)wd * SA * 2;
+    return (size_t)tab_n * cs_stride_d(tab_n) * 8 + (size_t)max_wd * 16 + (size_t)tab_n * 16 +
+           (size_t)tab_n * cs_stride_a(tab_n) * 2;
 }
 
 #define REQUIRE(cond, msg)                                            \
@@ -211,22 +334,15 @@ int vmat_launch_select_constrained(vmat_ddc *h, const float *p, const uint8_t *a
                                    cudaStream_t st)
 {
     REQUIRE(h->leafrow_pos0 != nullptr, "call vmat_ddc_set_leaf_geometry first");
-    // back-pointer tables: wd^2 u16 per leaf row with interdigitation, one u16 without
-    const int64_t need = interdigitation ? h->cs_bp_elems : (int64_t)h->n_leaf_rows + 1;
-    if (need > h->cs_bp_alloc) {
-        if (h->cs_bp) { VMAT_CUDA(cudaStreamSynchronize(st)); cudaFree(h->cs_bp); h->cs_bp = nullptr; h->cs_bp_alloc = 0; }
-        VMAT_CUDA(cudaMalloc((void **)&h->cs_bp, (size_t)need * 2));
-        h->cs_bp_alloc = need;
-    }
     if (h->n_leaf_rows > 0) {
         k_cs_prefix<<<(h->n_leaf_rows + 127) / 128, 128, 0, st>>>(h->n_leaf_rows, h->leafrow_col_offset, p, h->S_scratch);
         VMAT_LAUNCH_CHECK();
     }
     if (h->n_angles > 0) {
+        const int tab_n = h->cs_max_n + 1;
         CsArgs A{h->angle_row_offset, h->leafrow_col_offset, h->leafrow_pos0, h->angle_pmin, h->angle_wd,
-                 h->angle_bp_offset, angle_mask, L_lo, L_hi, R_lo, R_hi, h->S_scratch, h->cs_bp, L, R, row_price,
-                 angle_price, interdigitation ? 1 : 0};
-        k_cs_dp<<<h->n_angles, CS_THREADS, cs_smem_bytes(h->cs_max_wd), st>>>(A);
+                 h->row_bp_offset, angle_mask, L_lo, L_hi, R_lo, R_hi, h->S_scratch, h->cs_bp, L, R, row_price, angle_price, interdigitation ? 1 : 0, tab_n, h->cs_max_wd};
+        k_cs_dp<<<h->n_angles, CS_THREADS, cs_smem_bytes(tab_n, h->cs_max_wd), st>>>(A);
         VMAT_LAUNCH_CHECK();
     }
     k_cs_best<<<1, CS_THREADS, 0, st>>>(h->n_angles, angle_price, best_angle);
@@ -244,18 +360,20 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
     std::vector<int32_t> lco((size_t)n_rows + 1, 0);
     VMAT_CUDA(cudaMemcpy(lco.data(), h->leafrow_col_offset, ((size_t)n_rows + 1) * 4, cudaMemcpyDeviceToHost));
     std::vector<int32_t> pmin((size_t)(n_a > 0 ? n_a : 1), 0), wd((size_t)(n_a > 0 ? n_a : 1), 1);
-    std::vector<int64_t> bpo((size_t)n_a + 1, 0);
-    int max_wd = 1;
+    std::vector<int64_t> bpo((size_t)n_rows + 1, 0);
+    int max_wd = 1, max_n = 0;
     for (int k = 0; k < n_a; ++k) {
         bool any = false;
         int lo = 0, hi = 0;
-        for (int r = h->h_angle_row_offset[k]; r < h->h_angle_row_offset[k + 1]; ++r) {
+        const int ra = h->h_angle_row_offset[k], rb = h->h_angle_row_offset[k + 1];
+        for (int r = ra; r < rb; ++r) {
             const int n = lco[r + 1] - lco[r];
             if (n <= 0) continue;
             const int64_t e = (int64_t)leafrow_pos0[r] + n;
             REQUIRE(e <= INT32_MAX, "leaf row position overflows int32");
             if (!any || leafrow_pos0[r] < lo) lo = leafrow_pos0[r];
             if (!any || (int)e > hi) hi = (int)e;
+            max_n = n > max_n ? n : max_n;
             any = true;
         }
         REQUIRE((int64_t)hi - lo + 1 <= CS_MAX_POS + 1,
@@ -263,31 +381,36 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
         pmin[k] = lo;
         wd[k] = hi - lo + 1;
         max_wd = wd[k] > max_wd ? wd[k] : max_wd;
-        bpo[k + 1] = bpo[k] + (int64_t)wd[k] * wd[k] * (h->h_angle_row_offset[k + 1] - h->h_angle_row_offset[k]);
+        for (int r = ra; r < rb; ++r) {                          // back pointers of a row: wd closed + (n+1)^2 open states
+            const int64_t n1 = (int64_t)(lco[r + 1] - lco[r]) + 1;
+            bpo[r + 1] = bpo[r] + wd[k] + n1 * n1;
+        }
     }
+    const int tab_n = max_n + 1;
     int smem_optin = 0;
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
-    if (smem_optin > 0 && cs_smem_bytes(max_wd) > (size_t)smem_optin) {
-        vmat_set_error("vmat_ddc_set_leaf_geometry: a field range of %d positions needs %zu bytes of shared memory (%d available)",
-                       max_wd, cs_smem_bytes(max_wd), smem_optin);
+    if (smem_optin > 0 && cs_smem_bytes(tab_n, max_wd) + 64 > (size_t)smem_optin) {
+        vmat_set_error("vmat_ddc_set_leaf_geometry: leaf rows of %d beamlets need %zu bytes of shared memory (%d available)",
+                       max_n, cs_smem_bytes(tab_n, max_wd), smem_optin);
         return VMAT_ERR_INVALID_ARG;
     }
-    VMAT_CUDA(cudaFuncSetAttribute(k_cs_dp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cs_smem_bytes(max_wd)));
-    for (void **q : {(void **)&h->leafrow_pos0, (void **)&h->angle_pmin, (void **)&h->angle_wd, (void **)&h->angle_bp_offset})
+    VMAT_CUDA(cudaFuncSetAttribute(k_cs_dp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cs_smem_bytes(tab_n, max_wd)));
+    for (void **q : {(void **)&h->leafrow_pos0, (void **)&h->angle_pmin, (void **)&h->angle_wd, (void **)&h->row_bp_offset,
+                     (void **)&h->cs_bp})
         if (*q) { cudaFree(*q); *q = nullptr; }
     auto up = [&](void **dst, const void *src, size_t bytes) -> int {
         VMAT_CUDA(cudaMalloc(dst, bytes > 0 ? bytes : 1));
-        if (bytes > 0) VMAT_CUDA(cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice));
+        if (bytes > 0 && src) VMAT_CUDA(cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice));
         return VMAT_OK;
     };
     int rc = up((void **)&h->leafrow_pos0, leafrow_pos0, (size_t)n_rows * 4);
     if (rc == VMAT_OK) rc = up((void **)&h->angle_pmin, pmin.data(), (size_t)n_a * 4);
     if (rc == VMAT_OK) rc = up((void **)&h->angle_wd, wd.data(), (size_t)n_a * 4);
-    if (rc == VMAT_OK) rc = up((void **)&h->angle_bp_offset, bpo.data(), ((size_t)n_a + 1) * 8);
+    if (rc == VMAT_OK) rc = up((void **)&h->row_bp_offset, bpo.data(), ((size_t)n_rows + 1) * 8);
+    if (rc == VMAT_OK) rc = up((void **)&h->cs_bp, nullptr, (size_t)bpo[n_rows] * 2);
     if (rc != VMAT_OK) return rc;
-    h->cs_bp_elems = bpo[n_a] > 0 ? bpo[n_a] : 1;
     h->cs_max_wd = max_wd;
-    h->h_leafrow_pos0.assign(leafrow_pos0, leafrow_pos0 + n_rows);
+    h->cs_max_n = max_n;
     return VMAT_OK;
 }
 
