@@ -113,3 +113,77 @@ def test_max_apertures_caps_the_loop(cfg0):
     res = cg.run(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], A["sid"], A["T"], A["wo"], A["wu"], A["lco"],
                  A["aro"], max_apertures=2, y_lo=0.0, y_hi=50.0)
     assert res.stop == "max_apertures" and len(res.angles) == 2 and len(res.F_hist) == 3
+
+
+# ---------------------------------------------------------------- NEXT-3: the loop under hardware constraints
+def test_leaf_windows_hand_worked():
+    """Reading C25 on one arc of five control points with two leaf rows each (3 beamlets per row; row 1 starts one
+    beamlet to the right: pos0 = 0, 1).  Occupied: k = 1 with rows (0,2), (1,3) and k = 4 with rows (1,1), (0,1);
+    leaf travel 1 per step.  Physical positions: k = 1: (0,2), (2,4); k = 4: (1,1), (1,2).
+      k = 0: only k = 1 (one step away): row 0: a in [-1,1], b in [1,3]; row 1: a in [1,3], b in [3,5]
+             -> row-local (pos0 = 0, 1): row 0: L [-1,1], R [1,3]; row 1: L [0,2], R [2,4]
+      k = 2: k = 1 one step, k = 4 two steps: row 0: a in [-1,1] & [-1,3] = [-1,1], b in [1,3] & [-1,3] = [1,3];
+             row 1: a in [1,3] & [-1,3] = [1,3], b in [3,5] & [0,4] = [3,4] -> row-local L [0,2], R [2,3]
+      k = 3: k = 1 two steps, k = 4 one step: row 0: a in [-2,2] & [0,2] = [0,2], b in [0,4] & [0,2] = [0,2];
+             row 1: a in [0,4] & [0,2] = [0,2], b in [2,6] & [1,3] = [2,3] -> row-local L [-1,1], R [1,2]"""
+    aro = np.arange(0, 11, 2)
+    lco = np.arange(0, 31, 3)
+    pos0 = np.tile([0, 1], 5)
+    mask = np.array([0, 1, 0, 0, 1], np.uint8)
+    L = np.zeros(10, np.int32); R = np.zeros(10, np.int32)
+    L[2:4], R[2:4] = [0, 1], [2, 3]
+    L[8:10], R[8:10] = [1, 0], [1, 1]
+    W = cg.leaf_windows(mask, L, R, lco, aro, pos0, [0, 5], 1)
+    got = np.stack(W, 1)
+    B = cg.BIG
+    assert got[0].tolist() == [-1, 1, 1, 3] and got[1].tolist() == [0, 2, 2, 4]
+    assert got[4].tolist() == [-1, 1, 1, 3] and got[5].tolist() == [0, 2, 2, 3]
+    assert got[6].tolist() == [0, 2, 0, 2] and got[7].tolist() == [-1, 1, 1, 2]
+    for r in (2, 3, 8, 9):                                          # occupied control points: no bound
+        assert got[r].tolist() == [-B, B, -B, B]
+    # two arcs: a control point sees only its own arc
+    W2 = np.stack(cg.leaf_windows(mask, L, R, lco, aro, pos0, [0, 2, 5], 1), 1)
+    assert W2[0].tolist() == [-1, 1, 1, 3]                          # k = 0 sees k = 1
+    assert W2[4].tolist() == [-1, 3, -1, 3]                         # k = 2 (second arc) sees only k = 4, two steps away
+
+
+@pytest.fixture(scope="module")
+def run0_constrained(cfg0):
+    A = as_np(cfg0)
+    n_a = len(A["aro"]) - 1
+    res = cg.run(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], A["sid"], A["T"], A["wo"], A["wu"], A["lco"],
+                 A["aro"], max_apertures=n_a, y_lo=0.0, y_hi=50.0, interdigitation=True, max_leaf_travel=1,
+                 leafrow_pos0=cfg0.leafrow_pos0.numpy(), arc_angle_offset=cfg0.arc_angle_offset.numpy())
+    return A, res
+
+
+def test_constrained_loop_invariants(run0_constrained, run0, cfg0):
+    A, res = run0_constrained
+    free = run0[1]
+    u0 = cfg0.leafrow_pos0.numpy()
+    assert len(res.angles) >= 2 and len(set(res.angles)) == len(res.angles)
+    assert all(p < 0 for p in res.aperture_price)
+    F = np.array(res.F_hist)
+    assert (F[1:] <= F[:-1] * (1 + 1e-12)).all()                    # every master problem starts from the previous optimum
+    a, b = res.L + u0, res.R + u0
+    occ = sorted(res.angles)
+    for k in occ:                                                   # L135 inside every chosen aperture
+        for r in range(A["aro"][k], A["aro"][k + 1] - 1):
+            assert a[r] <= b[r + 1] and a[r + 1] <= b[r]
+    for k, kk in zip(occ[:-1], occ[1:]):                            # C25 between consecutive occupied control points
+        ra, rb = slice(A["aro"][k], A["aro"][k + 1]), slice(A["aro"][kk], A["aro"][kk + 1])
+        assert (np.abs(a[ra] - a[rb]) <= kk - k).all() and (np.abs(b[ra] - b[rb]) <= kk - k).all()
+    assert res.angles[0] == free.angles[0]                          # z = 0: all prices <= 0, every row opens fully
+    assert res.F_hist[-1] >= free.F_hist[-1] * (1 - 1e-9)           # constraints cannot help
+
+
+def test_constrained_loop_reduces_to_the_free_one(run0, cfg0):
+    """No interdigitation and a leaf travel nobody can exceed: the same control points, openings and objective."""
+    A, free, _ = run0
+    n_a = len(A["aro"]) - 1
+    res = cg.run(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], A["sid"], A["T"], A["wo"], A["wu"], A["lco"],
+                 A["aro"], max_apertures=n_a, y_lo=0.0, y_hi=50.0, interdigitation=False, max_leaf_travel=1000,
+                 leafrow_pos0=cfg0.leafrow_pos0.numpy(), arc_angle_offset=cfg0.arc_angle_offset.numpy())
+    assert res.angles == free.angles and res.F_hist == free.F_hist and res.stop == free.stop
+    opened = free.R > free.L
+    assert np.array_equal(res.L[opened], free.L[opened]) and np.array_equal(res.R[opened], free.R[opened])
