@@ -203,6 +203,20 @@ int vmat_select_apertures_constrained(vmat_ddc *h, const float *p, const uint8_t
                                       const int32_t *R_hi, int32_t *L, int32_t *R, double *row_price,
                                       double *angle_price, int32_t *best_angle, void *stream);
 
+/* Leaf-travel windows (L66: candidate apertures "need to be compatible with those chosen" at neighbouring control
+ * points, through s_k <= S^U_{k,k+1}(A_k, A_{k+1}); PAPER.md does not define S^U - reading C25): a leaf end moves at
+ * most max_leaf_travel beamlet widths per control-point step.  For every leaf row of every UNOCCUPIED control point
+ * k (angle_mask[k] == 0) the nearest occupied control point k' on either side of k within k's arc bounds both leaf
+ * ends of the same leaf row: |a_k - a_k'| <= max_leaf_travel |k - k'|, likewise b.  Writes the windows row-local,
+ * -2^30 / +2^30 where nothing binds (all rows of occupied control points).
+ *   angle_mask dev u8 [n_angles]; L, R dev int32 [n_leaf_rows]: openings of the occupied control points (row-local);
+ *   arc_angle_offset host int32 [n_arcs+1], n_arcs <= 16: control points of every arc, each arc with one MLC (the
+ *   same number of leaf rows at all its control points);  L_lo .. R_hi dev int32 [n_leaf_rows] out.
+ * Needs vmat_ddc_set_leaf_geometry.  Asynchronous. */
+int vmat_leaf_windows(const vmat_ddc *h, const uint8_t *angle_mask, const int32_t *L, const int32_t *R, int32_t n_arcs,
+                      const int32_t *arc_angle_offset, int32_t max_leaf_travel, int32_t *L_lo, int32_t *L_hi,
+                      int32_t *R_lo, int32_t *R_hi, void *stream);
+
 /* ------------------------------------------------------------------------------------------------------
  * NEXT-2: the master problem (MP), Eq. (6)-(10) L70-L101 and the four BB steps of L139.
  * With the apertures chosen so far and their dose vectors DA(A_k) (Eq. (5)), find fluence rates
@@ -259,6 +273,19 @@ int vmat_column_generation(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_struct
                            int32_t mp_max_iter, double eps_F, double eps_y, float *z, int32_t *L, int32_t *R,
                            int32_t *n_apertures_host, int32_t *angles_host, double *y_host, double *F_hist_host,
                            double *aperture_price_host, int32_t *mp_iters_host, int32_t *stop_host, void *stream);
+
+/* The same loop with the pricing problem under hardware constraints (NEXT-3): interdigitation != 0 applies
+ * inside every new aperture, max_leaf_travel >= 0 (with n_arcs, arc_angle_offset as for vmat_leaf_windows; < 0 =
+ * off) keeps every new aperture reachable from the occupied control points next to it (C25).  With both off this
+ * is vmat_column_generation.  The loop also stops (stop 0) when the best feasible aperture has a price >= 0.  Closed
+ * rows of a chosen aperture report their parked position in L = R. */
+int vmat_column_generation_ex(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_struct, int32_t n_struct, const float *T,
+                              const float *w_over, const float *w_under, int32_t max_apertures, double y_lo, double y_hi,
+                              int32_t mp_max_iter, double eps_F, double eps_y, int32_t interdigitation,
+                              int32_t max_leaf_travel, int32_t n_arcs, const int32_t *arc_angle_offset, float *z,
+                              int32_t *L, int32_t *R, int32_t *n_apertures_host, int32_t *angles_host, double *y_host,
+                              double *F_hist_host, double *aperture_price_host, int32_t *mp_iters_host,
+                              int32_t *stop_host, void *stream);
 
 /* Profiling hook for bench.py's roofline: four CUDA events (cudaEvent_t passed as void*, any may be NULL)
  * that every following vmat_price_eval / vmat_price_eval_host on this handle records on its stream:

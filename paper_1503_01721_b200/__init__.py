@@ -32,7 +32,8 @@ EXPORTS = [
     "vmat_aperture_dose", "vmat_ddc_set_profile_events", "vmat_last_error", "vmat_last_launch_count",
     "vmat_mp_create", "vmat_mp_destroy", "vmat_mp_reset", "vmat_mp_add_aperture", "vmat_mp_set_fluence", "vmat_mp_size",
     "vmat_mp_solve", "vmat_mp_history", "vmat_column_generation",
-    "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained",
+    "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained", "vmat_leaf_windows",
+    "vmat_column_generation_ex",
 ]
 
 
@@ -86,6 +87,9 @@ def load_library():
                                            vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_ddc_set_leaf_geometry.argtypes = [vp, vp]
     lib.vmat_select_apertures_constrained.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.vmat_leaf_windows.argtypes = [vp, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp]
+    lib.vmat_column_generation_ex.argtypes = [vp, vp, vp, i32, vp, vp, vp, i32, f64, f64, i32, f64, f64, i32, i32, i32, vp,
+                                              vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_last_error.restype = ctypes.c_char_p
     lib.vmat_last_launch_count.restype = ctypes.c_int
     for name in EXPORTS:
@@ -287,6 +291,18 @@ def vmat_select_apertures_constrained(h: DDC, p: torch.Tensor, angle_mask: Optio
         _ptr(angle_price, torch.float64, "cuda", h.n_angles), _ptr(best_angle, torch.int32, "cuda", 1), _stream()))
 
 
+def vmat_leaf_windows(h: DDC, angle_mask: torch.Tensor, L: torch.Tensor, R: torch.Tensor, arc_angle_offset: torch.Tensor,
+                      max_leaf_travel: int, L_lo, L_hi, R_lo, R_hi):
+    """NEXT-3: per-row leaf windows of the unoccupied control points from their occupied neighbours (reading C25)."""
+    n = h.n_leaf_rows
+    arcs = arc_angle_offset.to(torch.int32).cpu().contiguous()
+    _check(load_library().vmat_leaf_windows(
+        h._h, _ptr(angle_mask, torch.uint8, "cuda", h.n_angles), _ptr(L, torch.int32, "cuda", n),
+        _ptr(R, torch.int32, "cuda", n), arcs.numel() - 1, arcs.data_ptr(), int(max_leaf_travel),
+        _ptr(L_lo, torch.int32, "cuda", n), _ptr(L_hi, torch.int32, "cuda", n), _ptr(R_lo, torch.int32, "cuda", n),
+        _ptr(R_hi, torch.int32, "cuda", n), _stream()))
+
+
 def vmat_price_eval(h: DDC, x: torch.Tensor, obj: Objective, out: PriceEvalOut,
                     angle_mask: Optional[torch.Tensor] = None):
     """One whole price evaluation A1 -> A5 with the fused kernels; outputs are written into `out`."""
@@ -410,8 +426,11 @@ class CGPlan:
 
 
 def vmat_column_generation(h: DDC, mp: MasterProblem, obj: Objective, max_apertures: int, y_lo: float, y_hi: float,
-                           mp_max_iter: int = 300, eps_F: float = 1e-10, eps_y: float = 1e-12) -> CGPlan:
-    """The column-generation loop on the device; see vmat_column_generation in include/vmat.h."""
+                           mp_max_iter: int = 300, eps_F: float = 1e-10, eps_y: float = 1e-12,
+                           interdigitation: bool = False, max_leaf_travel: int = -1,
+                           arc_angle_offset: Optional[torch.Tensor] = None) -> CGPlan:
+    """The column-generation loop on the device; see vmat_column_generation and (with
+    interdigitation / max_leaf_travel, NEXT-3) vmat_column_generation_ex in include/vmat.h."""
     dev = h.device
     z = torch.empty(h.n_voxels, dtype=torch.float32, device=dev)
     L = torch.empty(h.n_leaf_rows, dtype=torch.int32, device=dev)
@@ -424,12 +443,19 @@ def vmat_column_generation(h: DDC, mp: MasterProblem, obj: Objective, max_apertu
     Fh = torch.zeros(cap + 1, dtype=torch.float64)
     ap = torch.zeros(cap, dtype=torch.float64)
     its = torch.zeros(cap, dtype=torch.int32)
-    _check(load_library().vmat_column_generation(
-        h._h, mp._h, _ptr(obj.voxel_struct, torch.uint8, "cuda", h.n_voxels), obj.n_struct,
-        _ptr(obj.T, torch.float32, "cuda"), _ptr(obj.w_over, torch.float32, "cuda"),
-        _ptr(obj.w_under, torch.float32, "cuda"), int(max_apertures), float(y_lo), float(y_hi), int(mp_max_iter),
-        float(eps_F), float(eps_y), z.data_ptr(), L.data_ptr(), R.data_ptr(), ctypes.addressof(n), angles.data_ptr(),
-        y.data_ptr(), Fh.data_ptr(), ap.data_ptr(), its.data_ptr(), ctypes.addressof(stop), _stream()))
+    head = (h._h, mp._h, _ptr(obj.voxel_struct, torch.uint8, "cuda", h.n_voxels), obj.n_struct,
+            _ptr(obj.T, torch.float32, "cuda"), _ptr(obj.w_over, torch.float32, "cuda"),
+            _ptr(obj.w_under, torch.float32, "cuda"), int(max_apertures), float(y_lo), float(y_hi), int(mp_max_iter),
+            float(eps_F), float(eps_y))
+    tail = (z.data_ptr(), L.data_ptr(), R.data_ptr(), ctypes.addressof(n), angles.data_ptr(), y.data_ptr(),
+            Fh.data_ptr(), ap.data_ptr(), its.data_ptr(), ctypes.addressof(stop), _stream())
+    if interdigitation or max_leaf_travel >= 0:
+        arcs = None if arc_angle_offset is None else arc_angle_offset.to(torch.int32).cpu().contiguous()
+        _check(load_library().vmat_column_generation_ex(
+            *head, 1 if interdigitation else 0, int(max_leaf_travel), 0 if arcs is None else arcs.numel() - 1,
+            None if arcs is None else arcs.data_ptr(), *tail))
+    else:
+        _check(load_library().vmat_column_generation(*head, *tail))
     k = int(n.value)
     return CGPlan(angles[:k], y[:k], Fh[:k + 1], ap[:k], its[:k],
                   "max_apertures" if stop.value == 1 else "no improving aperture", z, L, R)

@@ -212,3 +212,6 @@ int vmat_launch_select_constrained(vmat_ddc *h, const float *p, const uint8_t *a
                                    const int32_t *L_lo, const int32_t *L_hi, const int32_t *R_lo, const int32_t *R_hi,
                                    int32_t *L, int32_t *R, double *row_price, double *angle_price, int32_t *best_angle,
                                    cudaStream_t st);
+int vmat_launch_leaf_windows(const vmat_ddc *h, const uint8_t *angle_mask, const int32_t *L, const int32_t *R,
+                              int32_t n_arcs, const int32_t *arc_angle_offset, int32_t max_leaf_travel, int32_t *L_lo,
+                              int32_t *L_hi, int32_t *R_lo, int32_t *R_hi, cudaStream_t st);

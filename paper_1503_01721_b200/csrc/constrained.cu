@@ -317,6 +317,44 @@ k_cs_best(int n_angles, const double *__restrict__ angle_price, int32_t *__restr
     }
 }
 
+// Leaf-travel windows (reading C25): one thread per leaf row of every unoccupied control point k.  The nearest
+// occupied control point on either side of k inside k's arc bounds both leaf ends of the same leaf row:
+// |a_k - a_k'| <= travel * |k - k'|.  Positions are physical; the windows are written row-local, -/+ CS_BIG where
+// nothing binds.
+constexpr int CS_MAX_ARCS = 16;
+constexpr int CS_BIG = 1 << 30;
+struct CsArcs { int n; int off[CS_MAX_ARCS + 1]; };
+
+__global__ void k_leaf_windows(int n_rows, CsArcs arcs, int travel, const uint8_t *__restrict__ angle_mask,
+                               const int32_t *__restrict__ leafrow_angle, const int32_t *__restrict__ angle_row_offset,
+                               const int32_t *__restrict__ leafrow_col_offset, const int32_t *__restrict__ pos0,
+                               const int32_t *__restrict__ angle_pmin, const int32_t *__restrict__ L,
+                               const int32_t *__restrict__ R, int32_t *__restrict__ L_lo, int32_t *__restrict__ L_hi,
+                               int32_t *__restrict__ R_lo, int32_t *__restrict__ R_hi)
+{
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_rows) return;
+    const int k = leafrow_angle[r];
+    int llo = -CS_BIG, lhi = CS_BIG, rlo = -CS_BIG, rhi = CS_BIG;
+    if (angle_mask[k] == 0) {
+        int s = 0;
+        while (s + 1 < arcs.n && k >= arcs.off[s + 1]) ++s;
+        const int rho = r - angle_row_offset[k];
+        const int u0 = leafrow_col_offset[r + 1] > leafrow_col_offset[r] ? pos0[r] : angle_pmin[k];
+        for (int step = -1; step <= 1; step += 2) {
+            int kk = k + step;
+            while (kk >= arcs.off[s] && kk < arcs.off[s + 1] && angle_mask[kk] == 0) kk += step;
+            if (kk < arcs.off[s] || kk >= arcs.off[s + 1]) continue;
+            const int rr = angle_row_offset[kk] + rho;
+            const int v0 = leafrow_col_offset[rr + 1] > leafrow_col_offset[rr] ? pos0[rr] : angle_pmin[kk];
+            const int a = L[rr] + v0, b = R[rr] + v0, reach = travel * abs(kk - k);
+            llo = max(llo, a - reach - u0); lhi = min(lhi, a + reach - u0);
+            rlo = max(rlo, b - reach - u0); rhi = min(rhi, b + reach - u0);
+        }
+    }
+    L_lo[r] = llo; L_hi[r] = lhi; R_lo[r] = rlo; R_hi[r] = rhi;
+}
+
 static size_t cs_smem_bytes(int tab_n, int max_wd)
 {
     return (size_t)tab_n * cs_stride_d(tab_n) * 8 + (size_t)max_wd * 16 + (size_t)tab_n * 16 +
@@ -350,7 +388,46 @@ int vmat_launch_select_constrained(vmat_ddc *h, const float *p, const uint8_t *a
     return VMAT_OK;
 }
 
+int vmat_launch_leaf_windows(const vmat_ddc *h, const uint8_t *angle_mask, const int32_t *L, const int32_t *R,
+                              int32_t n_arcs, const int32_t *arc_angle_offset, int32_t max_leaf_travel, int32_t *L_lo,
+                              int32_t *L_hi, int32_t *R_lo, int32_t *R_hi, cudaStream_t st)
+{
+    REQUIRE(h->leafrow_pos0 != nullptr, "call vmat_ddc_set_leaf_geometry first");
+    REQUIRE(n_arcs >= 1 && n_arcs <= CS_MAX_ARCS && arc_angle_offset != nullptr, "n_arcs must be in 1..16");
+    REQUIRE(max_leaf_travel >= 0 && max_leaf_travel <= (1 << 16), "max_leaf_travel out of range");
+    REQUIRE(arc_angle_offset[0] == 0 && arc_angle_offset[n_arcs] == h->n_angles, "arc_angle_offset must span the control points");
+    CsArcs arcs;
+    arcs.n = n_arcs;
+    for (int s = 0; s <= n_arcs; ++s) arcs.off[s] = arc_angle_offset[s];
+    for (int s = 0; s < n_arcs; ++s) {
+        REQUIRE(arcs.off[s + 1] >= arcs.off[s], "arc_angle_offset not monotone");
+        for (int k = arcs.off[s]; k + 1 < arcs.off[s + 1]; ++k)                          // one MLC per arc
+            REQUIRE(h->h_angle_row_offset[k + 1] - h->h_angle_row_offset[k] ==
+                        h->h_angle_row_offset[k + 2] - h->h_angle_row_offset[k + 1],
+                    "the control points of an arc must have the same number of leaf rows");
+    }
+    if (h->n_leaf_rows == 0) return VMAT_OK;
+    k_leaf_windows<<<(h->n_leaf_rows + 127) / 128, 128, 0, st>>>(h->n_leaf_rows, arcs, max_leaf_travel, angle_mask,
+                                                                 h->leafrow_angle, h->angle_row_offset,
+                                                                 h->leafrow_col_offset, h->leafrow_pos0, h->angle_pmin, L,
+                                                                 R, L_lo, L_hi, R_lo, R_hi);
+    VMAT_LAUNCH_CHECK();
+    return VMAT_OK;
+}
+
 extern "C" {
+
+int vmat_leaf_windows(const vmat_ddc *h, const uint8_t *angle_mask, const int32_t *L, const int32_t *R, int32_t n_arcs,
+                      const int32_t *arc_angle_offset, int32_t max_leaf_travel, int32_t *L_lo, int32_t *L_hi,
+                      int32_t *R_lo, int32_t *R_hi, void *stream)
+{
+    REQUIRE(h != nullptr, "handle is NULL");
+    REQUIRE(h->n_angles == 0 || angle_mask != nullptr, "angle_mask is NULL");
+    REQUIRE(h->n_leaf_rows == 0 || (L && R && L_lo && L_hi && R_lo && R_hi), "NULL leaf-row array");
+    g_vmat_launches = 0;
+    return vmat_launch_leaf_windows(h, angle_mask, L, R, n_arcs, arc_angle_offset, max_leaf_travel, L_lo, L_hi, R_lo, R_hi,
+                                    (cudaStream_t)stream);
+}
 
 int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
 {

@@ -525,6 +525,21 @@ int vmat_column_generation(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_struct
                            int32_t *n_apertures_host, int32_t *angles_host, double *y_host, double *F_hist_host,
                            double *aperture_price_host, int32_t *mp_iters_host, int32_t *stop_host, void *stream)
 {
+    return vmat_column_generation_ex(h, mp, voxel_struct, n_struct, T, w_over, w_under, max_apertures, y_lo, y_hi,
+                                     mp_max_iter, eps_F, eps_y, 0, -1, 0, nullptr, z, L, R, n_apertures_host, angles_host,
+                                     y_host, F_hist_host, aperture_price_host, mp_iters_host, stop_host, stream);
+}
+
+// With interdigitation != 0 or max_leaf_travel >= 0 the pricing step is: price kernel, leaf-travel windows from the
+// occupied control points (reading C25), constrained selection (constrained.cu).
+int vmat_column_generation_ex(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_struct, int32_t n_struct, const float *T,
+                              const float *w_over, const float *w_under, int32_t max_apertures, double y_lo, double y_hi,
+                              int32_t mp_max_iter, double eps_F, double eps_y, int32_t interdigitation,
+                              int32_t max_leaf_travel, int32_t n_arcs, const int32_t *arc_angle_offset, float *z,
+                              int32_t *L, int32_t *R, int32_t *n_apertures_host, int32_t *angles_host, double *y_host,
+                              double *F_hist_host, double *aperture_price_host, int32_t *mp_iters_host,
+                              int32_t *stop_host, void *stream)
+{
     REQUIRE(h && mp && T && w_over && w_under && n_apertures_host, "NULL argument");
     REQUIRE(h->n_voxels == mp->n_voxels, "the DDC handle and the master problem differ in n_voxels");
     REQUIRE(h->n_voxels == 0 || (voxel_struct && z), "NULL voxel vector");
@@ -532,16 +547,19 @@ int vmat_column_generation(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_struct
     REQUIRE(max_apertures >= 0 && max_apertures <= mp->m_cap, "max_apertures exceeds the master problem's capacity");
     REQUIRE(n_struct >= 1 && n_struct <= 256, "n_struct must be in 1..256");
     REQUIRE(y_lo <= y_hi, "y_lo > y_hi");
+    const bool constrained = interdigitation != 0 || max_leaf_travel >= 0;
+    REQUIRE(!constrained || h->leafrow_pos0 != nullptr, "constraints need vmat_ddc_set_leaf_geometry");
+    REQUIRE(max_leaf_travel < 0 || (n_arcs >= 1 && arc_angle_offset != nullptr), "max_leaf_travel needs the arcs");
     cudaStream_t s = (cudaStream_t)stream;
     const size_t nv = (size_t)(h->n_voxels > 0 ? h->n_voxels : 1), nb = (size_t)(h->n_beamlets > 0 ? h->n_beamlets : 1);
     const size_t nr = (size_t)(h->n_leaf_rows > 0 ? h->n_leaf_rows : 1), na = (size_t)(h->n_angles > 0 ? h->n_angles : 1);
     // scratch of the pricing step, freed on every exit path
     struct Scratch {
         float *g = nullptr, *p = nullptr, *xs = nullptr, *DA = nullptr;
-        int32_t *Lw = nullptr, *Rw = nullptr, *best = nullptr;
+        int32_t *Lw = nullptr, *Rw = nullptr, *best = nullptr, *win = nullptr;
         double *row_price = nullptr, *angle_price = nullptr, *F = nullptr;
         uint8_t *mask = nullptr;
-        ~Scratch() { for (void *q : {(void *)g, (void *)p, (void *)xs, (void *)DA, (void *)Lw, (void *)Rw, (void *)best,
+        ~Scratch() { for (void *q : {(void *)g, (void *)p, (void *)xs, (void *)DA, (void *)Lw, (void *)Rw, (void *)best, (void *)win,
                                      (void *)row_price, (void *)angle_price, (void *)F, (void *)mask}) if (q) cudaFree(q); }
     } w;
     VMAT_CUDA(cudaMalloc((void **)&w.g, nv * 4)); VMAT_CUDA(cudaMalloc((void **)&w.DA, nv * 4));
@@ -550,6 +568,7 @@ int vmat_column_generation(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_struct
     VMAT_CUDA(cudaMalloc((void **)&w.row_price, nr * 8)); VMAT_CUDA(cudaMalloc((void **)&w.angle_price, na * 8));
     VMAT_CUDA(cudaMalloc((void **)&w.best, 4)); VMAT_CUDA(cudaMalloc((void **)&w.F, 8));
     VMAT_CUDA(cudaMalloc((void **)&w.mask, na));
+    if (max_leaf_travel >= 0) VMAT_CUDA(cudaMalloc((void **)&w.win, nr * 16));              // L_lo, L_hi, R_lo, R_hi
     VMAT_CUDA(cudaMemsetAsync(w.mask, 0, na, s));
     VMAT_CUDA(cudaMemsetAsync(z, 0, nv * 4, s));                                         // L56: start with z = 0 ...
     if (h->n_leaf_rows > 0) {
@@ -569,8 +588,20 @@ int vmat_column_generation(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_struct
     while (count < max_apertures) {
         // PP1: gradient at the current dose, beamlet prices; PP2: best opening per leaf row, best control point
         int rc = vmat_launch_objective(h, z, voxel_struct, n_struct, T, w_over, w_under, w.g, w.F, s);
-        if (rc == VMAT_OK) rc = vmat_launch_price_select(h, w.g, w.mask, w.p, w.Lw, w.Rw, w.row_price, s);
-        if (rc == VMAT_OK) rc = vmat_launch_angle_price(h, w.row_price, w.mask, w.angle_price, w.best, s);
+        if (!constrained) {
+            if (rc == VMAT_OK) rc = vmat_launch_price_select(h, w.g, w.mask, w.p, w.Lw, w.Rw, w.row_price, s);
+            if (rc == VMAT_OK) rc = vmat_launch_angle_price(h, w.row_price, w.mask, w.angle_price, w.best, s);
+        } else {
+            int32_t *wl[4] = {nullptr, nullptr, nullptr, nullptr};
+            if (rc == VMAT_OK) rc = vmat_launch_price(h, w.g, w.p, s);
+            if (rc == VMAT_OK && max_leaf_travel >= 0) {
+                for (int q = 0; q < 4; ++q) wl[q] = w.win + (size_t)q * nr;
+                rc = vmat_launch_leaf_windows(h, w.mask, L, R, n_arcs, arc_angle_offset, max_leaf_travel, wl[0], wl[1],
+                                              wl[2], wl[3], s);
+            }
+            if (rc == VMAT_OK) rc = vmat_launch_select_constrained(h, w.p, w.mask, interdigitation, wl[0], wl[1], wl[2],
+                                                                   wl[3], w.Lw, w.Rw, w.row_price, w.angle_price, w.best, s);
+        }
         if (rc != VMAT_OK) return rc;
         int32_t best = -1;
         double F = 0.0;

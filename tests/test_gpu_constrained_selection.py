@@ -188,3 +188,85 @@ def test_errors(vm):
         vm.vmat_ddc_set_leaf_geometry(h3, torch.tensor([0, 400], dtype=torch.int32))
     for x in (h, h2, h3):
         x.close()
+
+
+# ---------------------------------------------------------------- leaf-travel windows and the constrained loop
+def test_leaf_windows_against_the_oracle(vm):
+    """vmat_leaf_windows against oracle.column_generation.leaf_windows, integer for integer: random occupied sets and
+    openings on two arcs with ragged, partly empty rows."""
+    from oracle import column_generation as ocg
+    rng = np.random.default_rng(66)
+    arcs = np.array([0, 23, 40], np.int32)
+    rows_of = [5] * 23 + [7] * 17
+    aro = np.concatenate([[0], np.cumsum(rows_of)]).astype(np.int32)
+    n_rows = int(aro[-1])
+    lens = rng.integers(0, 9, n_rows)
+    lco = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+    pos0 = rng.integers(0, 5, n_rows).astype(np.int32)
+    h = selection_handle(vm, aro, lco, pos0)
+    for trial, travel in enumerate((0, 1, 3, 50)):
+        mask = (rng.random(40) < (0.1, 0.3, 0.6, 1.0)[trial]).astype(np.uint8)
+        L = rng.integers(-2, 8, n_rows).astype(np.int32)
+        R = (L + rng.integers(0, 6, n_rows)).astype(np.int32)
+        ref = ocg.leaf_windows(mask, L, R, lco, aro, pos0, arcs, travel)
+        dv = lambda a: torch.from_numpy(a).to(DEV)
+        W = [torch.empty(n_rows, dtype=torch.int32, device=DEV) for _ in range(4)]
+        vm.vmat_leaf_windows(h, dv(mask), dv(L), dv(R), torch.from_numpy(arcs), travel, *W)
+        for got, want in zip(W, ref):
+            assert np.array_equal(got.cpu().numpy(), want)
+    with pytest.raises(vm.VmatError):                               # an arc whose control points differ in leaf rows
+        vm.vmat_leaf_windows(h, dv(mask), dv(L), dv(R), torch.tensor([0, 30, 40]), 1, *W)
+    h.close()
+
+
+def _compare_constrained_plans(plan, ref):
+    from helpers import assert_vec_close
+    assert plan.stop == ref.stop
+    assert plan.angles.tolist() == ref.angles
+    assert np.array_equal(plan.L.cpu().numpy(), ref.L) and np.array_equal(plan.R.cpu().numpy(), ref.R)
+    assert np.abs(plan.y.numpy() - ref.y).max() <= 1e-4 * max(1.0, np.abs(ref.y).max())
+    assert np.allclose(plan.F_hist.numpy(), np.array(ref.F_hist), rtol=1e-5, atol=0.0)
+    assert np.allclose(plan.aperture_price.numpy(), np.array(ref.aperture_price), rtol=1e-5, atol=0.0)
+    assert_vec_close("z", plan.z.cpu().numpy(), ref.z)
+
+
+@pytest.mark.parametrize("interdig,travel", [(True, 1), (True, -1), (False, 2)])
+def test_constrained_column_generation_on_config0(vm, cfg0, interdig, travel):
+    """The paper's loop (L56) with the pricing problem under hardware constraints, every step on the GPU, against the
+    oracle's constrained loop (same control points in the same order, same leaf positions incl. parked closed rows)."""
+    from oracle import column_generation as ocg
+    A = as_np(cfg0)
+    h = ddc_from_arrays(A, DEV)
+    vm.vmat_ddc_set_leaf_geometry(h, cfg0.leafrow_pos0)
+    obj = obj_to_device(A, DEV)
+    n_a = len(A["aro"]) - 1
+    mp = vm.MasterProblem(A["n_v"], n_a, DEV)
+    plan = vm.vmat_column_generation(h, mp, obj, n_a, 0.0, 50.0, interdigitation=interdig, max_leaf_travel=travel,
+                                     arc_angle_offset=cfg0.arc_angle_offset)
+    ref = ocg.run(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], A["sid"], A["T"], A["wo"], A["wu"], A["lco"],
+                  A["aro"], max_apertures=n_a, y_lo=0.0, y_hi=50.0, interdigitation=interdig, max_leaf_travel=travel,
+                  leafrow_pos0=cfg0.leafrow_pos0.numpy(), arc_angle_offset=cfg0.arc_angle_offset.numpy())
+    _compare_constrained_plans(plan, ref)
+    assert len(ref.angles) >= 2
+    mp.close()
+    h.close()
+
+
+def test_constrained_column_generation_on_config1_coarsened(vm):
+    from oracle import column_generation as ocg
+    ph = synth.generate(synth.config_spec(1, 3.2), device=DEV)
+    A = as_np(ph)
+    h = vm.vmat_ddc_create(ph.n_voxels, ph.n_beamlets, ph.coo_voxel, ph.coo_beamlet, ph.coo_val,
+                           ph.angle_col_offset, ph.angle_row_offset, ph.leafrow_col_offset, device=DEV)
+    vm.vmat_ddc_set_leaf_geometry(h, ph.leafrow_pos0)
+    obj = obj_to_device(A, DEV)
+    mp = vm.MasterProblem(A["n_v"], 8, DEV)
+    kw = dict(interdigitation=True, max_leaf_travel=1)
+    plan = vm.vmat_column_generation(h, mp, obj, 5, 0.0, 100.0, mp_max_iter=500, arc_angle_offset=ph.arc_angle_offset, **kw)
+    ref = ocg.run(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], A["sid"], A["T"], A["wo"], A["wu"], A["lco"],
+                  A["aro"], max_apertures=5, y_lo=0.0, y_hi=100.0, mp_max_iter=500, leafrow_pos0=ph.leafrow_pos0.numpy(),
+                  arc_angle_offset=ph.arc_angle_offset.numpy(), **kw)
+    _compare_constrained_plans(plan, ref)
+    assert len(ref.angles) == 5
+    mp.close()
+    h.close()
