@@ -257,7 +257,40 @@ def bench_master_problem(vm, h, obj, out, dev, m: int) -> dict:
     return res
 
 
-def bench_plan(vm, h, obj, dev) -> dict:
+def bench_constrained_selection(vm, h, ph, obj, dev) -> dict:
+    """NEXT-3: vmat_select_apertures_constrained (interdigitation) on the bench phantom's fields with
+    the prices of a mixed-sign evaluation (x scaled so that rows open partially); ms per call, CUDA events."""
+    vm.vmat_ddc_set_leaf_geometry(h, ph.leafrow_pos0)
+    out = h.alloc_outputs()
+    res = {}
+    for scale in (0.6, 0.45, 0.35, 0.27, 0.2, 0.15, 0.1):       # a fluence level at which the prices have both signs
+        vm.vmat_price_eval(h, synth.draw_x(h.n_beamlets, 424242, device=dev, scale=scale), obj, out)
+        neg = float((out.p < 0).float().mean())
+        res["x_scale"], res["negative_price_fraction"] = scale, neg
+        if 0.25 <= neg:
+            break
+    o2 = h.alloc_outputs()
+    for name, inter in (("interdigitation", True), ("windows_only_path", False)):
+        for _ in range(3):
+            vm.vmat_select_apertures_constrained(h, out.p, None, inter, o2.L, o2.R, o2.row_price, o2.angle_price, o2.best_angle)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(20):
+            vm.vmat_select_apertures_constrained(h, out.p, None, inter, o2.L, o2.R, o2.row_price, o2.angle_price, o2.best_angle)
+        e1.record()
+        torch.cuda.synchronize()
+        res[name + "_ms"] = e0.elapsed_time(e1) / 20
+        if inter:
+            res["rows_changed_by_constraint"] = int(((o2.L != out.L) | (o2.R != out.R)).logical_and(out.R > out.L).sum())
+            res["price_ratio_constrained_over_free"] = float(o2.angle_price.min() / out.angle_price.min()) \
+                if float(out.angle_price.min()) < 0 else None
+    res["gpu_launches_per_call"] = vm.last_launch_count()
+    res["workload"] = f"{h.n_angles} control points, {h.n_leaf_rows} leaf rows, longest row {h.info['max_leaf_row_len']} beamlets"
+    return res
+
+
+def bench_plan(vm, h, obj, dev, constrained=None) -> dict:
     """One whole plan optimisation by column generation (vmat_column_generation, PAPER.md L56 / Figure 1(a)): one
     aperture per control point until every control point is occupied or no aperture improves F; master problems
     with eps_F = 1e-6, at most 200 BB iterations each, fluence rates in [0, 100].  Wall clock of the synchronous call
@@ -267,13 +300,16 @@ def bench_plan(vm, h, obj, dev) -> dict:
     mp = vm.MasterProblem(h.n_voxels, cap, dev)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    plan = vm.vmat_column_generation(h, mp, obj, cap, 0.0, 100.0, mp_max_iter=200, eps_F=1e-6, eps_y=1e-9)
+    kw = constrained or {}
+    plan = vm.vmat_column_generation(h, mp, obj, cap, 0.0, 100.0, mp_max_iter=200, eps_F=1e-6, eps_y=1e-9, **kw)
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
     res = {"seconds": dt, "apertures": int(plan.angles.numel()), "control_points": n_a, "stop": plan.stop,
            "F_start": float(plan.F_hist[0]), "F_end": float(plan.F_hist[-1]),
            "mp_iterations_total": int(plan.mp_iters.sum()), "gpu_launches": vm.last_launch_count(),
-           "settings": "y in [0, 100], MP: eps_F 1e-6, eps_y 1e-9, <= 200 BB iterations"}
+           "settings": "y in [0, 100], MP: eps_F 1e-6, eps_y 1e-9, <= 200 BB iterations"
+                       + (", interdigitation, leaf travel <= %d beamlet widths per control point" % kw["max_leaf_travel"]
+                          if kw else "")}
     mp.close()
     return res
 
@@ -379,6 +415,12 @@ def run_ours(args):
         mp_line = bench_master_problem(vm, h, obj, out, dev, args.mp_apertures)
     if world == 1 and not args.no_plan:
         plan_line = bench_plan(vm, h, obj, dev)
+    cs_line = cplan_line = None
+    if world == 1 and not args.no_constrained and ph.leafrow_pos0 is not None:
+        cs_line = bench_constrained_selection(vm, h, ph, obj, dev)
+        if not args.no_plan:
+            cplan_line = bench_plan(vm, h, obj, dev, dict(interdigitation=True, max_leaf_travel=4,
+                                                          arc_angle_offset=ph.arc_angle_offset))
 
     # ---- max over ranks
     elapsed_ms, e2e_ms = reduce_max([elapsed_ms, e2e_ms], dist if use_dist else None, dev)
@@ -442,6 +484,10 @@ def run_ours(args):
             line["master_problem"] = mp_line
         if plan_line is not None:
             line["plan_optimisation"] = plan_line
+        if cs_line is not None:
+            line["constrained_selection"] = cs_line
+        if cplan_line is not None:
+            line["plan_optimisation_constrained"] = cplan_line
         if not args.no_cpu_baseline and world == 1:
             v, desc, _, _, _ = oracle_rate(spec, dev, 12.0, 40, reps_auto=True)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc}
@@ -464,7 +510,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-mp", action="store_true", help="skip the master-problem measurement")
     ap.add_argument("--mp-apertures", type=int, default=128)
-    ap.add_argument("--no-plan", action="store_true", help="skip the whole-plan (column generation) measurement")
+    ap.add_argument("--no-plan", action="store_true", help="skip the whole-plan (column generation) measurements")
+    ap.add_argument("--no-constrained", action="store_true", help="skip the constrained-selection (NEXT-3) measurements")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
