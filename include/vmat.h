@@ -156,6 +156,12 @@ int vmat_price_eval(const vmat_ddc *h, const float *x,
                     int32_t *L, int32_t *R, double *row_price, double *angle_price,
                     int32_t *best_angle, void *stream);
 
+/* A3 -> A5 with the fused kernels, from a gradient the caller already holds: (price + row opening), aperture price.
+ * This is the second half of vmat_price_eval; the angle-sharded multi-GPU path (NEXT-4) calls it after the
+ * all-reduce of the dose.  Arguments as for vmat_price and vmat_select_apertures. */
+int vmat_price_select(const vmat_ddc *h, const float *g, const uint8_t *angle_mask, float *p, int32_t *L, int32_t *R,
+                      double *row_price, double *angle_price, int32_t *best_angle, void *stream);
+
 /* End-to-end variant with HOST buffers: copies x (host, ideally pinned, [n_beamlets]) to the device,
  * runs vmat_price_eval on device scratch owned by the handle, copies F, L, R, row_price, angle_price
  * and best_angle back to the host arrays, and synchronises the stream before returning.

@@ -33,7 +33,7 @@ EXPORTS = [
     "vmat_mp_create", "vmat_mp_destroy", "vmat_mp_reset", "vmat_mp_add_aperture", "vmat_mp_set_fluence", "vmat_mp_size",
     "vmat_mp_solve", "vmat_mp_history", "vmat_column_generation",
     "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained", "vmat_leaf_windows",
-    "vmat_column_generation_ex",
+    "vmat_column_generation_ex", "vmat_price_select",
 ]
 
 
@@ -90,6 +90,7 @@ def load_library():
     lib.vmat_leaf_windows.argtypes = [vp, vp, vp, vp, i32, vp, i32, vp, vp, vp, vp, vp]
     lib.vmat_column_generation_ex.argtypes = [vp, vp, vp, i32, vp, vp, vp, i32, f64, f64, i32, f64, f64, i32, i32, i32, vp,
                                               vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.vmat_price_select.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_last_error.restype = ctypes.c_char_p
     lib.vmat_last_launch_count.restype = ctypes.c_int
     for name in EXPORTS:
@@ -267,6 +268,16 @@ def vmat_select_apertures(h: DDC, p: torch.Tensor, angle_mask: Optional[torch.Te
         _ptr(L, torch.int32, "cuda", h.n_leaf_rows), _ptr(R, torch.int32, "cuda", h.n_leaf_rows),
         _ptr(row_price, torch.float64, "cuda", h.n_leaf_rows), _ptr(angle_price, torch.float64, "cuda", h.n_angles),
         _ptr(best_angle, torch.int32, "cuda", 1), _stream()))
+
+
+def vmat_price_select(h: DDC, g: torch.Tensor, out: PriceEvalOut, angle_mask: Optional[torch.Tensor] = None):
+    """A3 -> A5 fused, from a gradient g: writes out.p, out.L, out.R, out.row_price, out.angle_price, out.best_angle."""
+    _check(load_library().vmat_price_select(
+        h._h, _ptr(g, torch.float32, "cuda", h.n_voxels), _ptr(angle_mask, torch.uint8, "cuda", h.n_angles),
+        _ptr(out.p, torch.float32, "cuda", h.n_beamlets), _ptr(out.L, torch.int32, "cuda", h.n_leaf_rows),
+        _ptr(out.R, torch.int32, "cuda", h.n_leaf_rows), _ptr(out.row_price, torch.float64, "cuda", h.n_leaf_rows),
+        _ptr(out.angle_price, torch.float64, "cuda", h.n_angles), _ptr(out.best_angle, torch.int32, "cuda", 1),
+        _stream()))
 
 
 def vmat_ddc_set_leaf_geometry(h: DDC, leafrow_pos0: torch.Tensor):

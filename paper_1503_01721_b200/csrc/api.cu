@@ -291,6 +291,20 @@ int vmat_price_eval(const vmat_ddc *h, const float *x,
     return vmat_launch_angle_price(h, row_price, angle_mask, angle_price, best_angle, st);
 }
 
+int vmat_price_select(const vmat_ddc *h, const float *g, const uint8_t *angle_mask, float *p, int32_t *L, int32_t *R,
+                      double *row_price, double *angle_price, int32_t *best_angle, void *stream)
+{
+    REQUIRE(h && best_angle, "NULL argument");
+    REQUIRE(h->n_voxels == 0 || g, "g is NULL");
+    REQUIRE(h->n_beamlets == 0 || p, "p is NULL");
+    REQUIRE(h->n_leaf_rows == 0 || (L && R && row_price), "NULL leaf-row output");
+    REQUIRE(h->n_angles == 0 || angle_price, "angle_price is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    g_vmat_launches = 0;
+    TRY(vmat_launch_price_select(h, g, angle_mask, p, L, R, row_price, st));
+    return vmat_launch_angle_price(h, row_price, angle_mask, angle_price, best_angle, st);
+}
+
 int vmat_ddc_set_profile_events(vmat_ddc *h, void *const *ev)
 {
     REQUIRE(h != nullptr, "handle is NULL");
