@@ -314,6 +314,92 @@ def bench_plan(vm, h, obj, dev, constrained=None) -> dict:
     return res
 
 
+# ----------------------------------------------------------------------------- NEXT-4: angle shards, timed
+def run_sharded(args):
+    """--parallelism angle-shards: ONE matrix split by control point over the N ranks (PAPER.md L119; sharded.py);
+    every step is one evaluation of the whole matrix: dose on every block, all-reduce of d (NCCL), objective on every
+    rank, price + selection on every block, all-gather of the best control points.  Strong scaling: value = K / t."""
+    import paper_1503_01721_b200 as vm
+    from paper_1503_01721_b200 import sharded
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device - the product path has no CPU fallback")
+    vm.load_library()
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    spec = synth.config_spec(args.config, args.scale)
+    n_a = spec.n_angles
+    from synth import phantom as P
+    _, _, aco, aro, lco = P._fields(spec)
+    # balance by beamlets (the non-zeros per beamlet are even, DESIGN.md section 3); every rank generates its block only
+    offs = sharded.partition_angles((aco[1:] - aco[:-1]).tolist(), world)
+    ph = synth.generate(spec, device=dev, angles=list(range(offs[rank], offs[rank + 1])))
+    sh = sharded.ShardedDDC.create(ph.n_voxels, ph.n_beamlets, ph.coo_voxel, ph.coo_beamlet, ph.coo_val,
+                                   ph.angle_col_offset, ph.angle_row_offset, ph.leafrow_col_offset, offs[rank],
+                                   offs[rank + 1], device=dev, index_bits=args.index_bits)
+    ph.coo_voxel = ph.coo_beamlet = ph.coo_val = None
+    torch.cuda.empty_cache()
+    obj = vm.Objective(ph.voxel_struct.to(dev), ph.struct_T.to(dev), ph.struct_w_over.to(dev), ph.struct_w_under.to(dev))
+    out = sh.h.alloc_outputs()
+    K, W = args.steps, args.warmup
+    b0, b1 = sh.block.beamlet_lo, sh.block.beamlet_hi
+    xs = [synth.draw_x(ph.n_beamlets, k, device=dev)[b0:b1].contiguous() for k in range(K + W)]   # same x on every rank
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for k in range(W):
+        best = sh.price_eval(xs[k], obj, out)
+    start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    launches = 0
+    start.record()
+    for k in range(K):
+        best = sh.price_eval(xs[W + k], obj, out)
+        launches += 4                                           # dose, objective (+ partial sum), price+select, angle price
+    stop.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    elapsed_ms, nnz_total, bytes_total = reduce_max([start.elapsed_time(stop), 0.0, 0.0], dist, dev)
+    tot = torch.tensor([float(sh.h.nnz), float(sh.h.info["bytes_stream_d"] + sh.h.info["bytes_stream_dt"])],
+                       dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(tot)
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        ms = elapsed_ms / K
+        gbs = float(tot[1]) / (ms * 1e-3) / 1e9
+        print(json.dumps({
+            "metric": METRIC, "value": K / (elapsed_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": spec.name, "parallelism": f"angle-shards x{world}", "n_angles": n_a,
+                       "angle_offsets": offs, "nnz": int(tot[0]), "bytes_streamed_per_step_all_ranks": int(tot[1]),
+                       "exchange": f"all-reduce of d ({4 * ph.n_voxels} bytes) + all-gather of {world} (price, control point) pairs per step",
+                       "x": "re-drawn per step, seeded Uniform[0,1)"},
+            "hbm_gbs": gbs, "hbm_frac_of_measured_per_gpu": gbs / world / peak, "clocks": clocks,
+            "gpu_launches": launches,
+            "roofline": {"bound": "hbm", "kernel": "whole step incl. the exchange (no per-kernel events on this path)",
+                         "achieved": gbs / world, "peak": peak, "unit": "GB/s", "frac": gbs / world / peak,
+                         "peak_source": peak_src, "traffic": None},
+            "result_check": {"best_angle_last": best[0], "best_price_last": best[1], "F_last": float(out.F.item())},
+        }))
+    sh.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 # ----------------------------------------------------------------------------- the CUDA path, timed
 def run_ours(args):
     import paper_1503_01721_b200 as vm
@@ -507,6 +593,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--index-bits", type=int, default=0, choices=[0, 16, 32],
                     help="index encoding of the layouts (vmat_ddc_create_ex): 0 = chosen per layout")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "angle-shards"],
+                    help="N > 1: independent replicas (default; the path needs one GPU) or ONE matrix split by control "
+                         "point over the ranks (NEXT-4)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-mp", action="store_true", help="skip the master-problem measurement")
     ap.add_argument("--mp-apertures", type=int, default=128)
@@ -516,6 +605,8 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.parallelism == "angle-shards":
+        run_sharded(args)
     else:
         run_ours(args)
 
