@@ -12,6 +12,7 @@
 // from the FP64 oracle's by summation order only.
 #include "common.cuh"
 #include <new>
+#include <stdlib.h>
 #include <vector>
 
 constexpr int MP_THREADS = 256;
@@ -19,6 +20,9 @@ constexpr int MP_WARPS = MP_THREADS / 32;
 constexpr int MP_STEP_THREADS = 1024;         // the one-CTA step kernel
 constexpr int MP_STEP_WARPS = MP_STEP_THREADS / 32;
 constexpr int MP_MAX_NC = 12;                 // up to 12 x 32 = 384 apertures
+#ifndef VMAT_MP_CTAS_PER_SM
+#define VMAT_MP_CTAS_PER_SM 2
+#endif
 constexpr int MP_HIST = 6;                    // objective values the "last five changes" rule looks at
 
 struct MpState {                              // device-resident scalars of one solve
@@ -80,145 +84,195 @@ __global__ void k_mp_clip(int m, double *__restrict__ y, const double *__restric
 // CURV = false: z = DA y, F, dF/dz, partials of g_A = DA^T dF/dz            (steps 4 and 1 of L139)
 // CURV = true : z = DA y, q = DA g, partials of sum_i w_i q_i^2              (first step size, C17)
 //
-// Persistent CTAs walk over tiles of RT voxel rows.  A tile is brought into shared memory with 16-byte
-// cp.async copies (every load of the tile in flight at once, no register staging), stored with a row stride of
-// m32 = m rounded up to 32 floats.  Phase Z: TPR = 256 / RT threads per row add up the row dot product; thread
-// (row, part) visits column (TPR (j + row) + part) mod m32 at step j, so the 32 lanes of a warp hit 32
-// different banks and no shuffle is needed beyond the TPR partial sums.  The objective is evaluated once per row.
-// Phase G: thread t owns column t mod KT of every RG-th row (KT = min(m32, 256), RG = 256 / KT) and adds
-// DA_ik dF/dz_i to its FP64 accumulator, which it keeps over all its tiles.  The first version of this pass (a
-// group of lanes per row, FP64 shuffle tree per row) issued 118-161 warp instructions per row and ran at
-// 0.7-1.3 TB/s (issue-bound at m = 32, latency-bound at m = 128).
-#ifndef VMAT_MP_TILE_FLOATS
-#define VMAT_MP_TILE_FLOATS 16384
-#endif
-#ifndef VMAT_MP_CTAS_PER_SM
-#define VMAT_MP_CTAS_PER_SM 3
-#endif
-constexpr int MP_TILE_FLOATS = VMAT_MP_TILE_FLOATS;   // shared memory per tile, in floats
+// A group of LPR = 2^LOG lanes owns a voxel row, lane gl of the group holds
+// columns (c LPR + gl) 4 .. + 3 of it for c < NC (one 16-byte load each; the group reads the row contiguously), and a
+// warp works on 8 x (32 / LPR) rows at a time.  Every lane forms its part
+// of the 8 row dot products in FP64; a halving butterfly (8 -> 4 -> 2 -> 1 values per lane, 7 + LOG - 3 double
+// shuffles for 8 rows instead of 8 LOG) leaves the sum of row (gl >> (LOG - 3)) in the lane.  The objective and
+// dF/dz_i follow per row, dF/dz_i is broadcast back, and every lane adds DA_ik dF/dz_i into the FP64 accumulators of
+// its own columns, which it keeps over all its rows - the row's entries are still in the lane's own shared-memory
+// FIFO slot (filled by cp.async two or three steps ahead, read conflict-free), so DA is read from HBM once.
+// Fixed assignment of rows to warps and fixed reduction trees: deterministic.
+// (History: lanes-per-row with a full FP64 shuffle tree per row ran at 0.7-1.3 TB/s; shared-memory tiles filled by
+// cp.async with thread-per-row dot products at 3.6 TB/s under ncu, L1TEX-bound at 79 % by the tile being written
+// once and read twice plus 32 bytes of y per 16 bytes of tile.)
+// 8 values per lane, summed over the LPR lanes of a group: lane gl ends with the total of value gl >> (LOG - 3)
+template <int LOG>
+__device__ __forceinline__ double mp_reduce8(const double (&v)[8], int gl)
+{
+    constexpr int LPR = 1 << LOG;
+    double w4[4], w2[2];
+    {
+        const bool up = (gl & (LPR / 2)) != 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const double keep = up ? v[i + 4] : v[i], send = up ? v[i] : v[i + 4];
+            w4[i] = keep + shfl_xor_d(send, LPR / 2);
+        }
+    }
+    {
+        const bool up = (gl & (LPR / 4)) != 0;
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const double keep = up ? w4[i + 2] : w4[i], send = up ? w4[i] : w4[i + 2];
+            w2[i] = keep + shfl_xor_d(send, LPR / 4);
+        }
+    }
+    const bool up = (gl & (LPR / 8)) != 0;
+    double w1 = (up ? w2[1] : w2[0]) + shfl_xor_d(up ? w2[0] : w2[1], LPR / 8);
+#pragma unroll
+    for (int o = LPR / 16; o > 0; o >>= 1) w1 += shfl_xor_d(w1, o);
+    return w1;
+}
 
-__device__ __forceinline__ void cp_async_16(void *smem, const void *gmem)
+// 16-byte asynchronous copy global -> shared, bypassing L1
+__device__ __forceinline__ void mp_cp_async16(void *smem, const void *gmem)
 {
     const uint32_t sa = (uint32_t)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(sa), "l"(gmem) : "memory");
 }
-__device__ __forceinline__ void cp_async_wait_all()
+__device__ __forceinline__ void mp_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+// a shared-memory read the compiler may not merge with an earlier one of the same address
+__device__ __forceinline__ float4 mp_lds_again(const float4 *p)
 {
-    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
+    float4 r;
+    const uint32_t sa = (uint32_t)__cvta_generic_to_shared(p);
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "r"(sa));
+    return r;
 }
+template <int N>
+__device__ __forceinline__ void mp_cp_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
 
-template <bool CURV>
-__global__ void __launch_bounds__(MP_THREADS)
-k_mp_pass(int n_voxels, int m, int m_cap, int RT, const float *__restrict__ DA,
+__host__ __device__ constexpr int mp_stages(int NC) { return NC == 3 ? 2 : 3; }
+__host__ __device__ constexpr size_t mp_ring_bytes(int NC) { return (size_t)MP_WARPS * mp_stages(NC) * 8 * NC * 32 * 16; }
+
+template <bool CURV, int LOG, int NC>
+__global__ void __launch_bounds__(MP_THREADS, 2)
+k_mp_pass(int n_voxels, int m, int m_cap, const float *__restrict__ DA,
           const double *__restrict__ y, const double *__restrict__ gvec,
           const uint8_t *__restrict__ vstruct, int n_struct, const float *__restrict__ T,
           const float *__restrict__ w_over, const float *__restrict__ w_under, float *__restrict__ z_out,
           double *__restrict__ gpart, double *__restrict__ spart, const MpState *__restrict__ st)
 {
     if (st->reason != 0) return;                              // the solve has stopped: nothing to do
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int m32 = (m + 31) & ~31, m4 = (m + 3) >> 2;        // row stride in floats; 16-byte chunks per row
-    float *tile = (float *)smem_raw;                          // [RT][m32]
-    double *y_s = (double *)(tile + (size_t)RT * m32);        // [m32] fluence rates (0 beyond m)
-    double *v_s = y_s + m32;                                  // [m32] CURV: g_A;  else unused
-    double *gz_s = v_s + m32;                                 // [RT] dF/dz of the tile's rows
+    constexpr int LPR = 1 << LOG, GPW = 32 / LPR, LOWB = LOG - 3, RB = 8, COLS = LPR * NC * 4;
+    constexpr int STAGES = mp_stages(NC), ITEMS = RB * NC;    // 16-byte chunks per lane and stage
+    extern __shared__ float4 mp_ring[];                       // [warp][STAGES][ITEMS][32]: every lane's own prefetch FIFO
     __shared__ double red_s[MP_WARPS + 1];
     __shared__ float sT[256], sWo[256], sWu[256];             // the objective's tables
+    __shared__ double accs[CURV ? 1 : MP_WARPS * COLS];       // per-warp partials of g_A
     for (int t = threadIdx.x; t < n_struct; t += MP_THREADS) { sT[t] = T[t]; sWo[t] = w_over[t]; sWu[t] = w_under[t]; }
-    for (int k = threadIdx.x; k < m32; k += MP_THREADS) {
-        y_s[k] = k < m ? y[k] : 0.0;
-        v_s[k] = (CURV && k < m) ? gvec[k] : 0.0;
-    }
-    for (int e = threadIdx.x; e < RT * m32; e += MP_THREADS) tile[e] = 0.f;     // the pad columns stay 0
     __syncthreads();
-    const int nq = m32 >> 2;                                  // 16-byte chunks per stored row (a multiple of 8)
-    const int TPR = MP_THREADS / RT;                          // threads per row in phase Z: 1, 2, 4 or 8
-    const int zrow = threadIdx.x / TPR, zpart = threadIdx.x % TPR;
-    const int RG = MP_THREADS / nq;                           // phase G: thread = (row group, chunk of 4 columns)
-    const int gq = threadIdx.x % nq, grg = threadIdx.x / nq;
-    const int c_r = MP_THREADS / m4, c_q = MP_THREADS % m4;   // the copy loop steps (row, chunk) by 256 chunks
-    double acc[4] = {0.0, 0.0, 0.0, 0.0};                     // g_A partials of columns 4 gq .. 4 gq + 3
-    double ssum = 0.0;
-    const int n_tiles = (n_voxels + RT - 1) / RT;
-    for (int tix = blockIdx.x; tix < n_tiles; tix += gridDim.x) {
-        const int row0 = tix * RT;
-        // ---- the tile: RT x m4 chunks of 16 bytes, all in flight at once
-        for (int r = threadIdx.x / m4, q = threadIdx.x % m4; r < RT;) {
-            float *dst = tile + (size_t)r * m32 + 4 * q;
-            if (row0 + r < n_voxels) cp_async_16(dst, DA + (size_t)(row0 + r) * m_cap + 4 * q);
-            else *(float4 *)dst = make_float4(0.f, 0.f, 0.f, 0.f);
-            r += c_r; q += c_q;
-            if (q >= m4) { q -= m4; ++r; }
-        }
-        cp_async_wait_all();
-        __syncthreads();
-        // ---- phase Z: row dot products, 4 columns per step; thread (row, part) starts at chunk TPR row + part, so
-        //      the 8 lanes of a quarter warp read 8 different bank groups
-        {
-            const float4 *trow = (const float4 *)(tile + (size_t)zrow * m32);
-            const double2 *y2 = (const double2 *)y_s, *v2 = (const double2 *)v_s;
-            double zi = 0.0, qi = 0.0;
-            int cq = (TPR * zrow + zpart) % nq;
-            const int nj = nq / TPR;
-#pragma unroll 2
-            for (int j = 0; j < nj; ++j) {
-                const float4 a = trow[cq];
-                const double2 ya = y2[2 * cq], yb = y2[2 * cq + 1];
-                const double a0 = (double)a.x, a1 = (double)a.y, a2 = (double)a.z, a3 = (double)a.w;
-                zi = fma(a0, ya.x, zi); zi = fma(a1, ya.y, zi); zi = fma(a2, yb.x, zi); zi = fma(a3, yb.y, zi);
-                if (CURV) {
-                    const double2 va = v2[2 * cq], vb = v2[2 * cq + 1];
-                    qi = fma(a0, va.x, qi); qi = fma(a1, va.y, qi); qi = fma(a2, vb.x, qi); qi = fma(a3, vb.y, qi);
-                }
-                cq += TPR;
-                if (cq >= nq) cq -= nq;
-            }
-            for (int o = 1; o < TPR; o <<= 1) {               // the row's TPR parts sit in neighbouring lanes
-                zi += shfl_xor_d(zi, o);
-                if (CURV) qi += shfl_xor_d(qi, o);
-            }
-            const int i = row0 + zrow;
-            if (zpart == 0) {
-                double gz = 0.0;
-                if (i < n_voxels) {
-                    const int sid = vstruct[i];
-                    const double Ti = (double)sT[sid], wo = (double)sWo[sid], wu = (double)sWu[sid];
-                    if (!CURV) {
-                        const double over = fmax(zi - Ti, 0.0), under = fmax(Ti - zi, 0.0);
-                        gz = 2.0 * wo * over - 2.0 * wu * under;                         // Eq. (1), sign C1
-                        ssum += wo * over * over + wu * under * under;
-                        if (z_out) z_out[i] = (float)zi;
-                    } else {
-                        const double w = zi > Ti ? wo : (zi < Ti ? wu : 0.0);            // C17
-                        ssum += w * qi * qi;
-                    }
-                }
-                gz_s[zrow] = gz;
-            }
-        }
-        __syncthreads();
-        // ---- phase G: g_A += DA_i: * dF/dz_i; a thread owns 4 columns of every RG-th row
-        if (!CURV && grg < RG) {                               // (256 is no multiple of nq = 24, 40, ...: a few threads idle)
-            for (int r = grg; r < RT; r += RG) {
-                const double gz = gz_s[r];
-                const float4 a = ((const float4 *)(tile + (size_t)r * m32))[gq];
-                acc[0] = fma((double)a.x, gz, acc[0]); acc[1] = fma((double)a.y, gz, acc[1]);
-                acc[2] = fma((double)a.z, gz, acc[2]); acc[3] = fma((double)a.w, gz, acc[3]);
-            }
-        }
-        __syncthreads();                                      // the tile is overwritten next
-    }
-    // ---- CTA partials in a fixed order: the RG row groups of every column
-    if (!CURV) {
-        double *red = (double *)tile;                         // [RG][m32] doubles <= 8 KB; the tile is free now
-        if (grg < RG) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gl = lane & (LPR - 1), grp = lane >> LOG;
+    double yk[NC][4], vk[NC][4], acc[NC][4];
+    bool colok[NC];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) red[(size_t)grg * m32 + 4 * gq + j] = acc[j];
+    for (int c = 0; c < NC; ++c) {
+        const int col = (c * LPR + gl) * 4;
+        colok[c] = col < m;                                   // m_cap is a multiple of 8: the 16-byte chunk stays inside the row
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            yk[c][j] = col + j < m ? y[col + j] : 0.0;
+            vk[c][j] = (CURV && col + j < m) ? gvec[col + j] : 0.0;
+            acc[c][j] = 0.0;
         }
+    }
+    double ssum = 0.0;
+    const int my_slot = gl >> LOWB;                           // the row slot whose total this lane ends up with
+    const bool leader = (gl & ((1 << LOWB) - 1)) == 0;        // one lane per row adds to F and writes z
+    const int64_t step = (int64_t)gridDim.x * MP_WARPS * (RB * GPW);
+    const int64_t base0 = (int64_t)(blockIdx.x * MP_WARPS + warp) * (RB * GPW);
+    float4 *my = mp_ring + (size_t)warp * STAGES * ITEMS * 32 + lane;
+    // a stage = the 8 row slots of one step; every lane copies the chunks it will read itself, so no barrier is needed
+    auto issue = [&](int64_t base, int st) {
+        if (base < n_voxels) {
+#pragma unroll
+            for (int s = 0; s < RB; ++s) {                    // slot s of group grp is row base + s GPW + grp
+                const int64_t row = base + s * GPW + grp;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    float4 *dst = my + (size_t)(st * ITEMS + s * NC + c) * 32;
+                    if (row < n_voxels && colok[c]) mp_cp_async16(dst, DA + row * m_cap + (c * LPR + gl) * 4);
+                    else *dst = make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+            }
+        }
+        mp_cp_commit();
+    };
+#pragma unroll
+    for (int st = 0; st < STAGES - 1; ++st) issue(base0 + st * step, st);
+    int cur = 0;
+    for (int64_t base = base0; base < n_voxels; base += step) {
+        {
+            int nxt = cur + STAGES - 1;
+            if (nxt >= STAGES) nxt -= STAGES;
+            issue(base + (STAGES - 1) * step, nxt);
+        }
+        mp_cp_wait<STAGES - 1>();
+        const float4 *stg = my + (size_t)cur * ITEMS * 32;
+        if (++cur == STAGES) cur = 0;
+        double pz[RB], pq[RB];
+#pragma unroll
+        for (int s = 0; s < RB; ++s) {
+            double zi = 0.0, qi = 0.0;
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                const float4 e = stg[(size_t)(s * NC + c) * 32];
+                const double a0 = (double)e.x, a1 = (double)e.y, a2 = (double)e.z, a3 = (double)e.w;
+                zi = fma(a0, yk[c][0], zi); zi = fma(a1, yk[c][1], zi); zi = fma(a2, yk[c][2], zi); zi = fma(a3, yk[c][3], zi);
+                if (CURV) {
+                    qi = fma(a0, vk[c][0], qi); qi = fma(a1, vk[c][1], qi); qi = fma(a2, vk[c][2], qi); qi = fma(a3, vk[c][3], qi);
+                }
+            }
+            pz[s] = zi; pq[s] = qi;
+        }
+        const double zi = mp_reduce8<LOG>(pz, gl);
+        const double qi = CURV ? mp_reduce8<LOG>(pq, gl) : 0.0;
+        const int64_t i = base + my_slot * GPW + grp;
+        double gz = 0.0;
+        if (i < n_voxels) {
+            const int sid = vstruct[i];
+            const double Ti = (double)sT[sid], wo = (double)sWo[sid], wu = (double)sWu[sid];
+            if (!CURV) {
+                const double over = fmax(zi - Ti, 0.0), under = fmax(Ti - zi, 0.0);
+                gz = 2.0 * wo * over - 2.0 * wu * under;                                 // Eq. (1), sign C1
+                if (leader) {
+                    ssum += wo * over * over + wu * under * under;
+                    if (z_out) z_out[i] = (float)zi;
+                }
+            } else if (leader) {
+                const double w = zi > Ti ? wo : (zi < Ti ? wu : 0.0);                    // C17
+                ssum += w * qi * qi;
+            }
+        }
+        if (!CURV) {
+#pragma unroll NC >= 2 ? 1 : 2
+            for (int s = 0; s < RB; ++s) {                    // g_A += DA_i: * dF/dz_i; wide rows: rolled, to bound the registers
+                const double gs = __shfl_sync(0xffffffffu, gz, (grp << LOG) + (s << LOWB));
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    const float4 e = mp_lds_again(stg + (size_t)(s * NC + c) * 32);   // not kept in registers
+                    acc[c][0] = fma((double)e.x, gs, acc[c][0]); acc[c][1] = fma((double)e.y, gs, acc[c][1]);
+                    acc[c][2] = fma((double)e.z, gs, acc[c][2]); acc[c][3] = fma((double)e.w, gs, acc[c][3]);
+                }
+            }
+        }
+    }
+    // ---- CTA partials in a fixed order: the groups of a warp, then the warps
+    if (!CURV) {
+#pragma unroll
+        for (int c = 0; c < NC; ++c)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                double v = acc[c][j];
+#pragma unroll
+                for (int o = LPR; o < 32; o <<= 1) v += shfl_xor_d(v, o);
+                if (grp == 0) accs[warp * COLS + (c * LPR + gl) * 4 + j] = v;
+            }
         __syncthreads();
         for (int k = threadIdx.x; k < m; k += MP_THREADS) {
             double sacc = 0.0;
-            for (int g2 = 0; g2 < RG; ++g2) sacc += red[(size_t)g2 * m32 + k];
+            for (int w = 0; w < MP_WARPS; ++w) sacc += accs[w * COLS + k];
             gpart[(size_t)k * gridDim.x + blockIdx.x] = sacc;                             // [m_cap][n_cta]
         }
     }
@@ -330,26 +384,29 @@ k_mp_step(int m, int m_cap, int n_cta, double *__restrict__ y, double *__restric
 }
 
 // ---------------------------------------------------------------- host side
-static int mp_tile_rows(int m)
+static void mp_set_smem_attributes()
 {
-    const int m32 = (m + 31) & ~31;
-    int rt = MP_THREADS;                                     // 256, 128, 64 or 32 rows so that RT * m32 <= 16384 floats
-    while (rt > 32 && rt * m32 > MP_TILE_FLOATS) rt >>= 1;
-    return rt;
-}
-static size_t mp_pass_smem(int m)
-{
-    const int m32 = (m + 31) & ~31, rt = mp_tile_rows(m);
-    return (size_t)rt * m32 * 4 + (size_t)m32 * 16 + (size_t)rt * 8;
+#define MP_ATTR(CURV, LOG, NC) \
+    cudaFuncSetAttribute(k_mp_pass<CURV, LOG, NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mp_ring_bytes(NC))
+    MP_ATTR(false, 3, 1); MP_ATTR(false, 4, 1); MP_ATTR(false, 5, 1); MP_ATTR(false, 5, 2); MP_ATTR(false, 5, 3);
+    MP_ATTR(true, 3, 1); MP_ATTR(true, 4, 1); MP_ATTR(true, 5, 1); MP_ATTR(true, 5, 2); MP_ATTR(true, 5, 3);
+#undef MP_ATTR
 }
 
 template <bool CURV>
 static void mp_launch_pass(const vmat_mp *h, const uint8_t *vs, int n_struct, const float *T, const float *wo,
                            const float *wu, float *z, cudaStream_t s)
 {
-    k_mp_pass<CURV><<<h->n_cta, MP_THREADS, mp_pass_smem(h->m), s>>>(h->n_voxels, h->m, h->m_cap, mp_tile_rows(h->m),
-                                                                     h->DA, h->y, h->g, vs, n_struct, T, wo, wu, z,
-                                                                     h->gpart, h->spart, h->st);
+#define MP_PASS(LOG, NC)                                                                                            \
+    k_mp_pass<CURV, LOG, NC><<<h->n_cta, MP_THREADS, mp_ring_bytes(NC), s>>>(h->n_voxels, h->m, h->m_cap, h->DA, h->y, h->g, vs,   \
+                                                             n_struct, T, wo, wu, z, h->gpart, h->spart, h->st)
+    const int m = h->m;                                      // lanes per row x 16-byte chunks per lane covering m columns
+    if (m <= 32) MP_PASS(3, 1);                              // (8 columns per lane up to m = 128 measured 6-13 % slower)
+    else if (m <= 64) MP_PASS(4, 1);
+    else if (m <= 128) MP_PASS(5, 1);
+    else if (m <= 256) MP_PASS(5, 2);
+    else MP_PASS(5, 3);
+#undef MP_PASS
 }
 
 template <int PHASE>
@@ -389,11 +446,8 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
     cudaGetDevice(&h->device);
     int n_sm = 1;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, h->device);
+    mp_set_smem_attributes();
     h->n_cta = n_sm * VMAT_MP_CTAS_PER_SM;                                     // fixed for the handle: fixes every summation order
-    size_t smem_max = 0;
-    for (int mm = 32; mm <= MP_MAX_NC * 32; mm += 32) smem_max = mp_pass_smem(mm) > smem_max ? mp_pass_smem(mm) : smem_max;
-    cudaFuncSetAttribute(k_mp_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
-    cudaFuncSetAttribute(k_mp_pass<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
     cudaStream_t s = (cudaStream_t)stream;
     auto alloc = [&](void **p, size_t bytes) { return cudaMalloc(p, bytes > 0 ? bytes : 1) == cudaSuccess; };
     const size_t mc = (size_t)h->m_cap;
