@@ -176,7 +176,9 @@ int vmat_price_eval_host(vmat_ddc *h, const float *x_host,
 /* Aperture dose vector DA(A_k) = sum_{j in A_k} D_:j (Eq. (5)) of the aperture given by the
  * openings [L,R) of the leaf rows of control point `angle`: DA = D 1_A, on the device (the paper did
  * this on the CPU from COO, L137).  L, R dev int32 [n_leaf_rows] (as written by the selection);
- * x_scratch dev [n_beamlets] (overwritten with the indicator); DA dev [n_voxels] out. */
+ * x_scratch dev [n_beamlets] (overwritten with the indicator); DA dev [n_voxels] out.
+ * Only the beamlet rows of that control point are read (layout D^T); their entries are summed per voxel in 64-bit
+ * fixed point (exact, order-free), so DA is deterministic and within one FP32 rounding of the exact sum. */
 int vmat_aperture_dose(const vmat_ddc *h, int32_t angle, const int32_t *L, const int32_t *R,
                        float *x_scratch, float *DA, void *stream);
 

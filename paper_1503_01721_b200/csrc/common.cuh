@@ -90,6 +90,9 @@ struct vmat_ddc {
     uint32_t *angle_ticket = nullptr;       // [1] ticket of the aperture-price kernel (self-resetting)
     uint32_t *leafrow_done = nullptr;       // [n_leaf_rows] tickets of the fused price+selection kernel (self-resetting)
     std::vector<int32_t> h_angle_row_offset; // host copy
+    std::vector<int32_t> h_angle_col_offset; // host copy
+    unsigned long long *ad_acc = nullptr;    // [n_voxels] fixed-point accumulators of vmat_aperture_dose
+    int ad_shift = 0;                        // its scale: 2^ad_shift
     std::vector<int32_t> h_seg_row;          // host copy of seg_row (export undoes the tile interleave)
     int32_t max_leaf_row_len = 0;
     int64_t max_voxel_row_nnz = 0, max_beamlet_row_nnz = 0;

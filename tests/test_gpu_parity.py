@@ -247,4 +247,42 @@ def test_aperture_dose(vm, A0, h0):
         ind[A0["lco"][r] + L[r]:A0["lco"][r] + R[r]] = 1.0
     assert ind.sum() > 0
     assert np.array_equal(xs.cpu().numpy(), ind)
-    assert_vec_close("DA", DA.cpu().numpy(), oracle.dose(A0["vox"], A0["beam"], A0["val"], A0["n_v"], ind))
+    ref = oracle.dose(A0["vox"], A0["beam"], A0["val"], A0["n_v"], ind)
+    assert_vec_close("DA", DA.cpu().numpy(), ref)
+    # the sums are exact fixed-point sums rounded once: within one FP32 rounding of the FP64 oracle, and order-free
+    assert np.abs(DA.cpu().numpy().astype(np.float64) - ref).max() <= 2.0 ** -23 * np.abs(ref).max()
+    DA2 = torch.empty_like(DA)
+    vm.vmat_aperture_dose(h0, a, out.L, out.R, xs, DA2)
+    assert torch.equal(DA, DA2)
+
+
+def test_aperture_dose_signed_and_large_values(vm):
+    """Eq. (5) on a random matrix with entries of both signs up to 1e6 (the fixed-point scale adapts to max |D_ij|),
+    leaf rows of several lengths, openings incl. closed and full rows, for every control point."""
+    rng = np.random.default_rng(55)
+    n_v, rows = 700, [[5, 0, 9], [40, 3], [1], [33, 33, 2, 7]]
+    lens = np.concatenate([np.array(r) for r in rows])
+    n_b = int(lens.sum())
+    lco = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+    aro = np.concatenate([[0], np.cumsum([len(r) for r in rows])]).astype(np.int32)
+    dense = rng.random((n_v, n_b)) < 0.3
+    vox, beam = np.nonzero(dense)
+    val = ((rng.random(vox.size) - 0.5) * 2e6).astype(np.float32)
+    h = vm.vmat_ddc_create(n_v, n_b, torch.from_numpy(vox.astype(np.int32)).to(DEV), torch.from_numpy(beam.astype(np.int32)).to(DEV),
+                           torch.from_numpy(val).to(DEV), torch.from_numpy(lco[aro]), torch.from_numpy(aro),
+                           torch.from_numpy(lco), device=DEV)
+    L = np.array([rng.integers(0, n + 1) for n in lens], np.int32)
+    R = np.array([rng.integers(l, n + 1) for l, n in zip(L, lens)], np.int32)
+    L[1], R[1] = 0, 0
+    L[3], R[3] = 0, lens[3]
+    DA = torch.empty(n_v, dtype=torch.float32, device=DEV)
+    xs = torch.empty(n_b, dtype=torch.float32, device=DEV)
+    for a in range(len(rows)):
+        vm.vmat_aperture_dose(h, a, torch.from_numpy(L).to(DEV), torch.from_numpy(R).to(DEV), xs, DA)
+        ind = np.zeros(n_b, np.float32)
+        for r in range(aro[a], aro[a + 1]):
+            ind[lco[r] + L[r]:lco[r] + R[r]] = 1.0
+        ref = oracle.dose(vox.astype(np.int32), beam.astype(np.int32), val, n_v, ind)
+        assert np.array_equal(xs.cpu().numpy(), ind)
+        assert np.abs(DA.cpu().numpy().astype(np.float64) - ref).max() <= 2.0 ** -23 * max(np.abs(ref).max(), 1e-30)
+    h.close()
