@@ -127,7 +127,7 @@ int vmat_ddc_destroy(vmat_ddc *h)
                     h->angle_row_offset, h->leafrow_col_offset, h->leafrow_angle, h->seg_row, h->F_partial,
                     h->F_partial_obj, h->S_scratch, h->beamlet_leafrow, h->leafrow_done, h->e2e_x, h->e2e_d, h->e2e_g, h->e2e_p, h->e2e_L, h->e2e_R,
                     h->e2e_best, h->e2e_row_price, h->e2e_angle_price, h->e2e_F,
-                    h->leafrow_pos0, h->angle_pmin, h->angle_wd, h->row_bp_offset, h->cs_bp, h->ad_acc};
+                    h->leafrow_pos0, h->angle_pmin, h->angle_wd, h->row_bp_offset, h->cs_bp, h->ad_acc, h->angle_order};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     delete h;

@@ -103,6 +103,7 @@ struct vmat_ddc {
     int32_t *leafrow_pos0 = nullptr;        // [n_leaf_rows] physical column of each leaf row's first beamlet
     int32_t *angle_pmin = nullptr;          // [n_angles] left end of the control point's field range
     int32_t *angle_wd = nullptr;            // [n_angles] positions in the field range (Pmax - Pmin + 1)
+    int32_t *angle_order = nullptr;         // [n_angles] launch order of k_cs_dp: heaviest control points first
     int64_t *row_bp_offset = nullptr;       // [n_leaf_rows+1] start of each leaf row's back pointers in cs_bp
     uint16_t *cs_bp = nullptr;              // back pointers of the row-by-row recursion: per row wd + (n+1)^2
     int32_t cs_max_wd = 0, cs_max_n = 0;

@@ -22,6 +22,7 @@
 // are exact), so leaf positions, row prices and aperture prices are bit-identical to oracle_select_constrained
 // applied to the same FP32 price vector.
 #include "common.cuh"
+#include <algorithm>
 
 constexpr int CS_THREADS = 256;
 constexpr int CS_MAX_POS = 255;                       // positions are packed in 8 bits each
@@ -49,7 +50,7 @@ __global__ void k_cs_prefix(int n_rows, const int32_t *__restrict__ leafrow_col_
 }
 
 struct CsArgs {
-    const int32_t *angle_row_offset, *leafrow_col_offset, *pos0, *angle_pmin, *angle_wd;
+    const int32_t *angle_row_offset, *leafrow_col_offset, *pos0, *angle_pmin, *angle_wd, *angle_order;
     const int64_t *row_bp_offset;
     const uint8_t *angle_mask;
     const int32_t *L_lo, *L_hi, *R_lo, *R_hi;         // each may be NULL
@@ -72,7 +73,8 @@ __global__ void __launch_bounds__(CS_THREADS)
 k_cs_dp(CsArgs A)
 {
     extern __shared__ __align__(16) unsigned char cs_smem[];
-    const int k = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int k = A.angle_order[blockIdx.x];                                          // heaviest control points first
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int r0 = A.angle_row_offset[k], r1 = A.angle_row_offset[k + 1], nr = r1 - r0;
     const bool masked = A.angle_mask != nullptr && A.angle_mask[k] != 0;
     if (masked || nr == 0) {                                                          // C7: occupied control point
@@ -379,7 +381,7 @@ int vmat_launch_select_constrained(vmat_ddc *h, const float *p, const uint8_t *a
     if (h->n_angles > 0) {
         const int tab_n = h->cs_max_n + 1;
         CsArgs A{h->angle_row_offset, h->leafrow_col_offset, h->leafrow_pos0, h->angle_pmin, h->angle_wd,
-                 h->row_bp_offset, angle_mask, L_lo, L_hi, R_lo, R_hi, h->S_scratch, h->cs_bp, L, R, row_price, angle_price, interdigitation ? 1 : 0, tab_n, h->cs_max_wd};
+                 h->angle_order, h->row_bp_offset, angle_mask, L_lo, L_hi, R_lo, R_hi, h->S_scratch, h->cs_bp, L, R, row_price, angle_price, interdigitation ? 1 : 0, tab_n, h->cs_max_wd};
         k_cs_dp<<<h->n_angles, CS_THREADS, cs_smem_bytes(tab_n, h->cs_max_wd), st>>>(A);
         VMAT_LAUNCH_CHECK();
     }
@@ -438,6 +440,7 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
     VMAT_CUDA(cudaMemcpy(lco.data(), h->leafrow_col_offset, ((size_t)n_rows + 1) * 4, cudaMemcpyDeviceToHost));
     std::vector<int32_t> pmin((size_t)(n_a > 0 ? n_a : 1), 0), wd((size_t)(n_a > 0 ? n_a : 1), 1);
     std::vector<int64_t> bpo((size_t)n_rows + 1, 0);
+    std::vector<int64_t> work((size_t)(n_a > 0 ? n_a : 1), 0);                            // ~ sequential steps of k_cs_dp
     int max_wd = 1, max_n = 0;
     for (int k = 0; k < n_a; ++k) {
         bool any = false;
@@ -461,6 +464,7 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
         for (int r = ra; r < rb; ++r) {                          // back pointers of a row: wd closed + (n+1)^2 open states
             const int64_t n1 = (int64_t)(lco[r + 1] - lco[r]) + 1;
             bpo[r + 1] = bpo[r] + wd[k] + n1 * n1;
+            work[k] += 3 * n1 + 40;
         }
     }
     const int tab_n = max_n + 1;
@@ -472,8 +476,12 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
         return VMAT_ERR_INVALID_ARG;
     }
     VMAT_CUDA(cudaFuncSetAttribute(k_cs_dp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cs_smem_bytes(tab_n, max_wd)));
+    // launch order: the control points with the most sequential work first, so that the last wave is made of light ones
+    std::vector<int32_t> order((size_t)(n_a > 0 ? n_a : 1), 0);
+    for (int k = 0; k < n_a; ++k) order[k] = k;
+    std::stable_sort(order.begin(), order.begin() + n_a, [&](int a, int b) { return work[a] > work[b]; });
     for (void **q : {(void **)&h->leafrow_pos0, (void **)&h->angle_pmin, (void **)&h->angle_wd, (void **)&h->row_bp_offset,
-                     (void **)&h->cs_bp})
+                     (void **)&h->cs_bp, (void **)&h->angle_order})
         if (*q) { cudaFree(*q); *q = nullptr; }
     auto up = [&](void **dst, const void *src, size_t bytes) -> int {
         VMAT_CUDA(cudaMalloc(dst, bytes > 0 ? bytes : 1));
@@ -483,6 +491,7 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
     int rc = up((void **)&h->leafrow_pos0, leafrow_pos0, (size_t)n_rows * 4);
     if (rc == VMAT_OK) rc = up((void **)&h->angle_pmin, pmin.data(), (size_t)n_a * 4);
     if (rc == VMAT_OK) rc = up((void **)&h->angle_wd, wd.data(), (size_t)n_a * 4);
+    if (rc == VMAT_OK) rc = up((void **)&h->angle_order, order.data(), (size_t)n_a * 4);
     if (rc == VMAT_OK) rc = up((void **)&h->row_bp_offset, bpo.data(), ((size_t)n_rows + 1) * 8);
     if (rc == VMAT_OK) rc = up((void **)&h->cs_bp, nullptr, (size_t)bpo[n_rows] * 2);
     if (rc != VMAT_OK) return rc;
