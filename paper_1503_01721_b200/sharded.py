@@ -70,21 +70,38 @@ def local_block(angle_col_offset: torch.Tensor, angle_row_offset: torch.Tensor, 
                       (lco[r0:r1 + 1] - b0).to(torch.int32))
 
 
-def merge_best(local_best: int, local_price: float, angle_lo: int, group=None):
-    """Best control point over all ranks from every rank's best one: smallest price, ties -> smallest global control
-    point, none below 0 -> -1 (the rule of A5).  Returns (global control point or -1, its price or 0.0)."""
-    import torch.distributed as dist
-    mine = [float(local_price) if local_best >= 0 else 0.0, int(angle_lo + local_best) if local_best >= 0 else -1]
-    if group is None and not (dist.is_available() and dist.is_initialized()):
-        pairs = [mine]
-    else:
-        pairs = [None] * dist.get_world_size(group)
-        dist.all_gather_object(pairs, mine, group=group)
+def pick_best(pairs) -> tuple:
+    """The rule of A5 over (price, global control point) pairs, one per rank (control point -1 = that rank has no
+    improving aperture): smallest price, ties -> smallest control point, none -> (-1, 0.0)."""
     best, best_price = -1, 0.0
     for price, k in pairs:
+        k = int(k)
         if k >= 0 and (price < best_price or (price == best_price and best >= 0 and k < best)):
-            best, best_price = k, price
+            best, best_price = k, float(price)
     return best, best_price
+
+
+def merge_best(local_best, local_price, angle_lo: int, group=None):
+    """Best control point over all ranks from every rank's best one.  `local_best` (local numbering, -1 = none) and
+    `local_price` are Python numbers or one-element tensors (on the device of the process group's backend: CUDA for
+    NCCL, CPU for gloo); one all-gather of two doubles per rank, one copy to the host.  Returns (global control point
+    or -1, its price or 0.0)."""
+    import torch.distributed as dist
+    lb = local_best if torch.is_tensor(local_best) else torch.tensor([int(local_best)])
+    lb = lb.reshape(1).to(torch.int64)
+    lp = local_price if torch.is_tensor(local_price) else torch.tensor([float(local_price)], dtype=torch.float64)
+    lp = lp.reshape(1).to(device=lb.device, dtype=torch.float64)
+    valid = lb >= 0
+    pair = torch.cat([torch.where(valid, lp, torch.zeros_like(lp)),
+                      torch.where(valid, lb + angle_lo, torch.full_like(lb, -1)).to(torch.float64)])
+    if group is None and not (dist.is_available() and dist.is_initialized()):
+        pairs = pair.reshape(1, 2)
+    else:
+        world = dist.get_world_size(group)
+        pairs = torch.empty(world * 2, dtype=torch.float64, device=pair.device)
+        dist.all_gather_into_tensor(pairs, pair, group=group)
+        pairs = pairs.reshape(world, 2)
+    return pick_best(pairs.cpu().tolist())
 
 
 class ShardedDDC:
@@ -127,8 +144,11 @@ class ShardedDDC:
             dist.all_reduce(out.d, op=dist.ReduceOp.SUM, group=self.group)          # d = sum_m D_m x_m
         vmat_objective_grad(self.h, out.d, obj, out.g, out.F)
         vmat_price_select(self.h, out.g, out, angle_mask_local)
-        lb = int(out.best_angle.item())
-        lp = float(out.angle_price[lb].item()) if lb >= 0 else 0.0
+        lb = out.best_angle.to(torch.int64)                                            # stays on the device until the merge
+        if self.h.n_angles > 0:
+            lp = out.angle_price[lb.clamp(min=0)]
+        else:
+            lp = torch.zeros(1, dtype=torch.float64, device=lb.device)
         return merge_best(lb, lp, self.block.angle_lo, self.group)
 
     def close(self):
