@@ -69,6 +69,15 @@ static __host__ __device__ __forceinline__ int cs_stride_a(int t)               
     return ((s >> 1) & 1) ? s : s + 2;
 }
 
+// threads sharing one line (an i of the open-state walk, a column or a row of the sweeps) of a row with n1 = n + 1
+// positions: the largest power of two that keeps n1 lines inside the CTA, at most 16
+__device__ __forceinline__ int cs_segments(int n1)
+{
+    int s = 1;
+    while (s < 16 && 2 * s * n1 <= CS_THREADS) s <<= 1;
+    return s;
+}
+
 __global__ void __launch_bounds__(CS_THREADS)
 k_cs_dp(CsArgs A)
 {
@@ -93,6 +102,8 @@ k_cs_dp(CsArgs A)
     double *Sa = fcn + A.max_wd;                                                      // [tab_n] prefix sums of this row ...
     double *Sb = Sa + A.tab_n;                                                        // [tab_n] ... and of the next one
     uint16_t *PG = (uint16_t *)(Sb + A.tab_n);                                        // [tab_n][SA] args of PB
+    __shared__ double tot_v[CS_THREADS];                                              // chunk totals of the segmented sweeps
+    __shared__ unsigned tot_g[CS_THREADS];
     __shared__ double s_gv;                                                           // minimum of the previous row ...
     __shared__ unsigned s_ga;                                                         // ... and its smallest state
     const bool inter = A.interdigitation != 0;
@@ -136,54 +147,67 @@ k_cs_dp(CsArgs A)
             fcn[c] = f;
             bp_row[c] = (uint16_t)pg;
         }
-        // ---- open states (off+i, off+j), 0 <= i < j <= n: thread i walks j upwards, four at a time (loads first),
-        //      and carries the range minimum of the previous row's closed states over [a, b]
-        for (int i = tid; i < n; i += CS_THREADS) {
-            const int a = off + i;
-            double rv = cs_inf();
-            unsigned ra = CS_NONE;
-            if (query) { rv = fcp[a]; ra = (unsigned)((a << 8) | a); }
-            const double Si = Sa[i];
-            const int J = a - offp, Jc = max(J, 0);
-            const bool okL = i >= llo && i <= lhi;
-            for (int jb = i + 1; jb <= n; jb += 4) {
-                double cf[4], cS[4], cp[4];
-                unsigned cg[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int j = min(jb + u, n), b = off + j, I = b - offp;
-                    cS[u] = Sa[j];
-                    cf[u] = cs_inf(); cp[u] = cs_inf(); cg[u] = CS_NONE;
-                    if (query) {
-                        cf[u] = fcp[b];
-                        if (np > 0 && I >= 0 && J <= np) {                            // a' <= b and b' >= a
-                            const int Ic = min(I, np);
-                            cp[u] = PB[(size_t)Ic * SD + Jc];
-                            cg[u] = PG[(size_t)Ic * SA + Jc];
-                        }
+        // ---- open states (off+i, off+j), 0 <= i < j <= n.  SEG threads share the j range of one i; each first scans
+        //      the previous row's closed states from a up to its first b (the range minimum it would have carried),
+        //      then walks its own j's four at a time (loads first)
+        const int SEG = cs_segments(n1);
+        {
+            const int i = tid / SEG, seg = tid - i * SEG;
+            const int chunk = i < n ? (n - i + SEG - 1) / SEG : 0;
+            const int js = i + 1 + seg * chunk, je = min(n, js + chunk - 1);
+            if (i < n && js <= je) {
+                const int a = off + i;
+                double rv = cs_inf();
+                unsigned ra = CS_NONE;
+                if (query) {
+                    rv = fcp[a]; ra = (unsigned)((a << 8) | a);
+                    for (int b = a + 1; b < off + js; ++b) {                          // ascending b: strict < keeps the leftmost
+                        const double c = fcp[b];
+                        if (c < rv) { rv = c; ra = (unsigned)((b << 8) | b); }
                     }
                 }
+                const double Si = Sa[i];
+                const int J = a - offp, Jc = max(J, 0);
+                const bool okL = i >= llo && i <= lhi;
+                for (int jb = js; jb <= je; jb += 4) {
+                    double cf[4], cS[4], cp[4];
+                    unsigned cg[4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int j = jb + u, b = off + j;
-                    if (j > n) break;
-                    if (query && cf[u] < rv) { rv = cf[u]; ra = (unsigned)((b << 8) | b); }   // ascending b: strict < keeps the leftmost
-                    double f = cs_inf();
-                    unsigned pg = CS_NONE;
-                    if (okL && j >= rlo && j <= rhi) {
-                        const double V = cS[u] - Si;
-                        if (first) f = V;
-                        else {
-                            double pv = gv;
-                            unsigned pa = ga;
-                            if (inter) { pv = rv; pa = ra; cs_take(pv, pa, cp[u], cg[u]); }
-                            f = V + pv;                                               // +inf when no compatible predecessor
-                            pg = pa;
+                    for (int u = 0; u < 4; ++u) {
+                        const int j = min(jb + u, je), b = off + j, I = b - offp;
+                        cS[u] = Sa[j];
+                        cf[u] = cs_inf(); cp[u] = cs_inf(); cg[u] = CS_NONE;
+                        if (query) {
+                            cf[u] = fcp[b];
+                            if (np > 0 && I >= 0 && J <= np) {                        // a' <= b and b' >= a
+                                const int Ic = min(I, np);
+                                cp[u] = PB[(size_t)Ic * SD + Jc];
+                                cg[u] = PG[(size_t)Ic * SA + Jc];
+                            }
                         }
                     }
-                    PB[(size_t)i * SD + j] = f;
-                    PG[(size_t)i * SA + j] = (uint16_t)((a << 8) | b);
-                    bp_row[wd + j * n1 + i] = (uint16_t)pg;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int j = jb + u, b = off + j;
+                        if (j > je) break;
+                        if (query && cf[u] < rv) { rv = cf[u]; ra = (unsigned)((b << 8) | b); }
+                        double f = cs_inf();
+                        unsigned pg = CS_NONE;
+                        if (okL && j >= rlo && j <= rhi) {
+                            const double V = cS[u] - Si;
+                            if (first) f = V;
+                            else {
+                                double pv = gv;
+                                unsigned pa = ga;
+                                if (inter) { pv = rv; pa = ra; cs_take(pv, pa, cp[u], cg[u]); }
+                                f = V + pv;                                           // +inf when no compatible predecessor
+                                pg = pa;
+                            }
+                        }
+                        PB[(size_t)i * SD + j] = f;
+                        PG[(size_t)i * SA + j] = (uint16_t)((a << 8) | b);
+                        bp_row[wd + j * n1 + i] = (uint16_t)pg;
+                    }
                 }
             }
         }
@@ -192,18 +216,23 @@ k_cs_dp(CsArgs A)
             for (int t = tid; t <= nn; t += CS_THREADS) Sb[t] = A.S[jn + r + 1 + t];
         }
         __syncthreads();
-        // ---- PB of this row: sweep down the columns, then along the rows from the right
+        // ---- PB of this row: sweep down the columns, then along the rows from the right.  SEG threads share a line:
+        //      each scans its chunk, leaves the chunk's total in shared memory, and after a barrier folds the totals
+        //      of the chunks before it into its own entries
         if (n > 0) {
-            if (tid <= n) {                                                           // min over i' <= i (ascending: strict <)
-                const int j = tid;
+            const int line = tid / SEG, seg = tid - line * SEG;
+            const int chunk = (n1 + SEG - 1) / SEG, cs0 = seg * chunk, cs1 = min(n, cs0 + chunk - 1);
+            const bool act = line <= n && cs0 <= cs1;
+            if (act) {                                                                // column j: min over i' <= i (ascending: strict <)
+                const int j = line;
                 double v = cs_inf();
                 unsigned g = CS_NONE;
-                for (int i0 = 0; i0 <= n; i0 += 4) {
+                for (int i0 = cs0; i0 <= cs1; i0 += 4) {
                     double c[4];
                     unsigned cg[4];
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
-                        const int i = min(i0 + u, n);
+                        const int i = min(i0 + u, cs1);
                         const bool st = i < j;                                        // states live strictly above the diagonal
                         c[u] = st ? PB[(size_t)i * SD + j] : cs_inf();
                         cg[u] = st ? PG[(size_t)i * SA + j] : CS_NONE;
@@ -211,40 +240,71 @@ k_cs_dp(CsArgs A)
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
                         const int i = i0 + u;
-                        if (i <= n) {
+                        if (i <= cs1) {
                             if (c[u] < v) { v = c[u]; g = cg[u]; }
                             PB[(size_t)i * SD + j] = v;
                             PG[(size_t)i * SA + j] = (uint16_t)g;
                         }
                     }
                 }
+                if (SEG > 1) { tot_v[tid] = v; tot_g[tid] = g; }
             }
             __syncthreads();
-            if (tid <= n) {                                                           // min over j' >= j; ties -> smaller arg
-                const int i = tid;
+            if (SEG > 1) {
+                if (act && seg > 0) {
+                    const int j = line;
+                    double cv = cs_inf();
+                    unsigned cgc = CS_NONE;
+                    for (int t = 0; t < seg; ++t)                                     // earlier chunks hold smaller i: they win ties
+                        if (tot_v[tid - seg + t] < cv) { cv = tot_v[tid - seg + t]; cgc = tot_g[tid - seg + t]; }
+                    for (int i = cs0; i <= cs1; ++i)
+                        if (!(PB[(size_t)i * SD + j] < cv)) { PB[(size_t)i * SD + j] = cv; PG[(size_t)i * SA + j] = (uint16_t)cgc; }
+                }
+                __syncthreads();
+            }
+            if (act) {                                                                // row i: min over j' >= j; ties -> smaller arg
+                const int i = line;
                 double v = cs_inf();
                 unsigned g = CS_NONE;
-                for (int jt = n; jt >= 0; jt -= 4) {
+                for (int jt = cs1; jt >= cs0; jt -= 4) {
                     double c[4];
                     unsigned cg[4];
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
-                        const int j = max(jt - u, 0);
+                        const int j = max(jt - u, cs0);
                         c[u] = PB[(size_t)i * SD + j];
                         cg[u] = PG[(size_t)i * SA + j];
                     }
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
                         const int j = jt - u;
-                        if (j >= 0) {
+                        if (j >= cs0) {
                             cs_take(v, g, c[u], cg[u]);
                             PB[(size_t)i * SD + j] = v;
                             PG[(size_t)i * SA + j] = (uint16_t)g;
                         }
                     }
                 }
+                if (SEG > 1) { tot_v[tid] = v; tot_g[tid] = g; }
             }
             __syncthreads();
+            if (SEG > 1) {
+                if (act && seg < SEG - 1) {
+                    const int i = line;
+                    double cv = cs_inf();
+                    unsigned cgc = CS_NONE;
+                    for (int t = seg + 1; t < SEG; ++t)                               // the chunks to the right
+                        if ((line * SEG + t) < CS_THREADS && t * chunk <= n) cs_take(cv, cgc, tot_v[tid - seg + t], tot_g[tid - seg + t]);
+                    for (int j = cs0; j <= cs1; ++j) {
+                        double v = PB[(size_t)i * SD + j];
+                        unsigned g = PG[(size_t)i * SA + j];
+                        cs_take(v, g, cv, cgc);
+                        PB[(size_t)i * SD + j] = v;
+                        PG[(size_t)i * SA + j] = (uint16_t)g;
+                    }
+                }
+                __syncthreads();
+            }
         }
         // ---- the row's minimum and its smallest state: the predecessor of every state of the next row when the
         //      rows are independent, and the whole answer after the last row
@@ -470,7 +530,7 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
     const int tab_n = max_n + 1;
     int smem_optin = 0;
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
-    if (smem_optin > 0 && cs_smem_bytes(tab_n, max_wd) + 64 > (size_t)smem_optin) {
+    if (smem_optin > 0 && cs_smem_bytes(tab_n, max_wd) + 8192 > (size_t)smem_optin) {
         vmat_set_error("vmat_ddc_set_leaf_geometry: leaf rows of %d beamlets need %zu bytes of shared memory (%d available)",
                        max_n, cs_smem_bytes(tab_n, max_wd), smem_optin);
         return VMAT_ERR_INVALID_ARG;
