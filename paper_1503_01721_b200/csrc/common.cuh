@@ -106,7 +106,7 @@ struct vmat_ddc {
     int32_t *angle_order = nullptr;         // [n_angles] launch order of k_cs_dp: heaviest control points first
     int64_t *row_bp_offset = nullptr;       // [n_leaf_rows+1] start of each leaf row's back pointers in cs_bp
     uint16_t *cs_bp = nullptr;              // back pointers of the row-by-row recursion: per row wd + (n+1)^2
-    int32_t cs_max_wd = 0, cs_max_n = 0;
+    int32_t cs_max_wd = 0, cs_max_n = 0, cs_max_rows = 0;
     std::vector<int32_t> h_leafrow_pos0;
     // scratch for the end-to-end host call (allocated on first use)
     float *e2e_x = nullptr, *e2e_d = nullptr, *e2e_g = nullptr, *e2e_p = nullptr;

@@ -59,7 +59,7 @@ struct CsArgs {
     int32_t *L, *R;
     double *row_price, *angle_price;
     int interdigitation;
-    int tab_n, max_wd;                                // shared-memory table: tab_n x tab_n entries; fc arrays: max_wd
+    int tab_n, max_wd, max_rows;                      // shared-memory table: tab_n x tab_n entries; fc arrays: max_wd; chain: max_rows
 };
 
 static __host__ __device__ __forceinline__ int cs_stride_d(int t) { return t | 1; }   // doubles per table row: odd
@@ -113,13 +113,26 @@ k_cs_dp(CsArgs A)
         for (int t = tid; t <= n; t += CS_THREADS) Sa[t] = A.S[j0 + r0 + t];
     }
     __syncthreads();
+    // the tables of a row are fetched one row ahead, so their latency hides behind the previous row's work
+    struct RowMeta { int n, pos0, llo, lhi, rlo, rhi; int64_t bpo; };
+    auto fetch = [&](int r) {
+        RowMeta m;
+        m.n = A.leafrow_col_offset[r + 1] - A.leafrow_col_offset[r];
+        m.pos0 = A.pos0[r];
+        m.llo = A.L_lo ? A.L_lo[r] : INT_MIN; m.lhi = A.L_hi ? A.L_hi[r] : INT_MAX;
+        m.rlo = A.R_lo ? A.R_lo[r] : INT_MIN; m.rhi = A.R_hi ? A.R_hi[r] : INT_MAX;
+        m.bpo = A.row_bp_offset[r];
+        return m;
+    };
+    RowMeta nxt = fetch(r0);
     for (int q = 0; q < nr; ++q) {
         const int r = r0 + q;
-        const int j0 = A.leafrow_col_offset[r], n = A.leafrow_col_offset[r + 1] - j0, n1 = n + 1;
-        const int off = n > 0 ? A.pos0[r] - pmin : 0;
-        const int llo = A.L_lo ? A.L_lo[r] : INT_MIN, lhi = A.L_hi ? A.L_hi[r] : INT_MAX;
-        const int rlo = A.R_lo ? A.R_lo[r] : INT_MIN, rhi = A.R_hi ? A.R_hi[r] : INT_MAX;
-        uint16_t *bp_row = A.bp + A.row_bp_offset[r];
+        const RowMeta cur = nxt;
+        if (q + 1 < nr) nxt = fetch(r + 1);
+        const int n = cur.n, n1 = n + 1;
+        const int off = n > 0 ? cur.pos0 - pmin : 0;
+        const int llo = cur.llo, lhi = cur.lhi, rlo = cur.rlo, rhi = cur.rhi;
+        uint16_t *bp_row = A.bp + cur.bpo;
         const bool first = q == 0, last = q == nr - 1;
         const bool query = !first && inter;                                           // predecessors depend on the state
         double gv = 0.0;
@@ -212,8 +225,8 @@ k_cs_dp(CsArgs A)
             }
         }
         if (!last) {                                                                  // prefix sums of the next row
-            const int jn = A.leafrow_col_offset[r + 1], nn = A.leafrow_col_offset[r + 2] - jn;
-            for (int t = tid; t <= nn; t += CS_THREADS) Sb[t] = A.S[jn + r + 1 + t];
+            const int jn = A.leafrow_col_offset[r + 1];
+            for (int t = tid; t <= nxt.n; t += CS_THREADS) Sb[t] = A.S[jn + r + 1 + t];
         }
         __syncthreads();
         // ---- PB of this row: sweep down the columns, then along the rows from the right.  SEG threads share a line:
@@ -334,27 +347,38 @@ k_cs_dp(CsArgs A)
         t = Sa; Sa = Sb; Sb = t;
         np = n; offp = off;
     }
-    if (tid != 0) return;
+    // ---- walk back: one thread follows the predecessors (one dependent load per row) into shared memory, then all
+    //      threads write the rows out
     const double total = s_gv;
     if (!(total < cs_inf())) {                                                        // no feasible combination
-        for (int r = r0; r < r1; ++r) { A.L[r] = 0; A.R[r] = 0; A.row_price[r] = 0.0; }
-        A.angle_price[k] = cs_inf();
+        for (int r = r0 + tid; r < r1; r += CS_THREADS) { A.L[r] = 0; A.R[r] = 0; A.row_price[r] = 0.0; }
+        if (tid == 0) A.angle_price[k] = cs_inf();
         return;
     }
-    A.angle_price[k] = total;
-    unsigned g = s_ga;
-    for (int q = nr - 1; q >= 0; --q) {
-        const int r = r0 + q, a = (int)(g >> 8), b = (int)(g & 255u);
+    uint16_t *chain = (uint16_t *)(PG + (size_t)A.tab_n * SA);                        // [max_rows] state of every row
+    if (tid == 0) {
+        A.angle_price[k] = total;
+        unsigned g = s_ga;
+        for (int q = nr - 1; q >= 0; --q) {
+            chain[q] = (uint16_t)g;
+            if (q > 0) {
+                const int r = r0 + q, a = (int)(g >> 8), b = (int)(g & 255u);
+                const int n = A.leafrow_col_offset[r + 1] - A.leafrow_col_offset[r];
+                const int off = n > 0 ? A.pos0[r] - pmin : 0;
+                const uint16_t *bp_row = A.bp + A.row_bp_offset[r];
+                g = a == b ? bp_row[a] : bp_row[wd + (b - off) * (n + 1) + (a - off)];
+            }
+        }
+    }
+    __syncthreads();
+    for (int q = tid; q < nr; q += CS_THREADS) {
+        const int r = r0 + q, a = chain[q] >> 8, b = chain[q] & 255;
         const int j0 = A.leafrow_col_offset[r], n = A.leafrow_col_offset[r + 1] - j0;
         const int off = n > 0 ? A.pos0[r] - pmin : 0;
         const double *S = A.S + j0 + r;
         A.L[r] = a - off;
         A.R[r] = b - off;
         A.row_price[r] = a < b ? S[b - off] - S[a - off] : 0.0;
-        if (q > 0) {
-            const uint16_t *bp_row = A.bp + A.row_bp_offset[r];
-            g = a == b ? bp_row[a] : bp_row[wd + (b - off) * (n + 1) + (a - off)];
-        }
     }
 }
 
@@ -417,10 +441,10 @@ __global__ void k_leaf_windows(int n_rows, CsArcs arcs, int travel, const uint8_
     L_lo[r] = llo; L_hi[r] = lhi; R_lo[r] = rlo; R_hi[r] = rhi;
 }
 
-static size_t cs_smem_bytes(int tab_n, int max_wd)
+static size_t cs_smem_bytes(int tab_n, int max_wd, int max_rows)
 {
     return (size_t)tab_n * cs_stride_d(tab_n) * 8 + (size_t)max_wd * 16 + (size_t)tab_n * 16 +
-           (size_t)tab_n * cs_stride_a(tab_n) * 2;
+           (size_t)tab_n * cs_stride_a(tab_n) * 2 + (size_t)max_rows * 2;
 }
 
 #define REQUIRE(cond, msg)                                            \
@@ -441,8 +465,8 @@ int vmat_launch_select_constrained(vmat_ddc *h, const float *p, const uint8_t *a
     if (h->n_angles > 0) {
         const int tab_n = h->cs_max_n + 1;
         CsArgs A{h->angle_row_offset, h->leafrow_col_offset, h->leafrow_pos0, h->angle_pmin, h->angle_wd,
-                 h->angle_order, h->row_bp_offset, angle_mask, L_lo, L_hi, R_lo, R_hi, h->S_scratch, h->cs_bp, L, R, row_price, angle_price, interdigitation ? 1 : 0, tab_n, h->cs_max_wd};
-        k_cs_dp<<<h->n_angles, CS_THREADS, cs_smem_bytes(tab_n, h->cs_max_wd), st>>>(A);
+                 h->angle_order, h->row_bp_offset, angle_mask, L_lo, L_hi, R_lo, R_hi, h->S_scratch, h->cs_bp, L, R, row_price, angle_price, interdigitation ? 1 : 0, tab_n, h->cs_max_wd, h->cs_max_rows};
+        k_cs_dp<<<h->n_angles, CS_THREADS, cs_smem_bytes(tab_n, h->cs_max_wd, h->cs_max_rows), st>>>(A);
         VMAT_LAUNCH_CHECK();
     }
     k_cs_best<<<1, CS_THREADS, 0, st>>>(h->n_angles, angle_price, best_angle);
@@ -501,11 +525,12 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
     std::vector<int32_t> pmin((size_t)(n_a > 0 ? n_a : 1), 0), wd((size_t)(n_a > 0 ? n_a : 1), 1);
     std::vector<int64_t> bpo((size_t)n_rows + 1, 0);
     std::vector<int64_t> work((size_t)(n_a > 0 ? n_a : 1), 0);                            // ~ sequential steps of k_cs_dp
-    int max_wd = 1, max_n = 0;
+    int max_wd = 1, max_n = 0, max_rows = 1;
     for (int k = 0; k < n_a; ++k) {
         bool any = false;
         int lo = 0, hi = 0;
         const int ra = h->h_angle_row_offset[k], rb = h->h_angle_row_offset[k + 1];
+        max_rows = rb - ra > max_rows ? rb - ra : max_rows;
         for (int r = ra; r < rb; ++r) {
             const int n = lco[r + 1] - lco[r];
             if (n <= 0) continue;
@@ -530,12 +555,12 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
     const int tab_n = max_n + 1;
     int smem_optin = 0;
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
-    if (smem_optin > 0 && cs_smem_bytes(tab_n, max_wd) + 8192 > (size_t)smem_optin) {
+    if (smem_optin > 0 && cs_smem_bytes(tab_n, max_wd, max_rows) + 8192 > (size_t)smem_optin) {
         vmat_set_error("vmat_ddc_set_leaf_geometry: leaf rows of %d beamlets need %zu bytes of shared memory (%d available)",
-                       max_n, cs_smem_bytes(tab_n, max_wd), smem_optin);
+                       max_n, cs_smem_bytes(tab_n, max_wd, max_rows), smem_optin);
         return VMAT_ERR_INVALID_ARG;
     }
-    VMAT_CUDA(cudaFuncSetAttribute(k_cs_dp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cs_smem_bytes(tab_n, max_wd)));
+    VMAT_CUDA(cudaFuncSetAttribute(k_cs_dp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cs_smem_bytes(tab_n, max_wd, max_rows)));
     // launch order: the control points with the most sequential work first, so that the last wave is made of light ones
     std::vector<int32_t> order((size_t)(n_a > 0 ? n_a : 1), 0);
     for (int k = 0; k < n_a; ++k) order[k] = k;
@@ -557,6 +582,7 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
     if (rc != VMAT_OK) return rc;
     h->cs_max_wd = max_wd;
     h->cs_max_n = max_n;
+    h->cs_max_rows = max_rows;
     return VMAT_OK;
 }
 
