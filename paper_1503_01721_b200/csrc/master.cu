@@ -86,7 +86,7 @@ __global__ void k_mp_clip(int m, double *__restrict__ y, const double *__restric
 //
 // A group of LPR = 2^LOG lanes owns a voxel row, lane gl of the group holds
 // columns (c LPR + gl) 4 .. + 3 of it for c < NC (one 16-byte load each; the group reads the row contiguously), and a
-// warp works on 8 x (32 / LPR) rows at a time.  Every lane forms its part
+// warp works on 8 x (32 / LPR) rows at a time (4 when a row is wider than 128 entries).  Every lane forms its part
 // of the 8 row dot products in FP64; a halving butterfly (8 -> 4 -> 2 -> 1 values per lane, 7 + LOG - 3 double
 // shuffles for 8 rows instead of 8 LOG) leaves the sum of row (gl >> (LOG - 3)) in the lane.  The objective and
 // dF/dz_i follow per row, dF/dz_i is broadcast back, and every lane adds DA_ik dF/dz_i into the FP64 accumulators of
@@ -96,32 +96,37 @@ __global__ void k_mp_clip(int m, double *__restrict__ y, const double *__restric
 // (History: lanes-per-row with a full FP64 shuffle tree per row ran at 0.7-1.3 TB/s; shared-memory tiles filled by
 // cp.async with thread-per-row dot products at 3.6 TB/s under ncu, L1TEX-bound at 79 % by the tile being written
 // once and read twice plus 32 bytes of y per 16 bytes of tile.)
-// 8 values per lane, summed over the LPR lanes of a group: lane gl ends with the total of value gl >> (LOG - 3)
-template <int LOG>
-__device__ __forceinline__ double mp_reduce8(const double (&v)[8], int gl)
+// 2^RBL (8 or 4) values per lane, summed over the LPR lanes of a group by a halving butterfly: lane gl ends with the
+// total of value gl >> (LOG - RBL)
+template <int LOG, int RBL>
+__device__ __forceinline__ double mp_reduce(const double (&v)[1 << RBL], int gl)
 {
     constexpr int LPR = 1 << LOG;
     double w4[4], w2[2];
-    {
+    if (RBL == 3) {
         const bool up = (gl & (LPR / 2)) != 0;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-            const double keep = up ? v[i + 4] : v[i], send = up ? v[i] : v[i + 4];
+            const double keep = up ? v[(i + 4) & ((1 << RBL) - 1)] : v[i], send = up ? v[i] : v[(i + 4) & ((1 << RBL) - 1)];
             w4[i] = keep + shfl_xor_d(send, LPR / 2);
         }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) w4[i] = v[i & ((1 << RBL) - 1)];
     }
+    constexpr int O2 = RBL == 3 ? LPR / 4 : LPR / 2;          // offsets of the 4 -> 2 and 2 -> 1 steps
     {
-        const bool up = (gl & (LPR / 4)) != 0;
+        const bool up = (gl & O2) != 0;
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
             const double keep = up ? w4[i + 2] : w4[i], send = up ? w4[i] : w4[i + 2];
-            w2[i] = keep + shfl_xor_d(send, LPR / 4);
+            w2[i] = keep + shfl_xor_d(send, O2);
         }
     }
-    const bool up = (gl & (LPR / 8)) != 0;
-    double w1 = (up ? w2[1] : w2[0]) + shfl_xor_d(up ? w2[0] : w2[1], LPR / 8);
+    const bool up = (gl & (O2 / 2)) != 0;
+    double w1 = (up ? w2[1] : w2[0]) + shfl_xor_d(up ? w2[0] : w2[1], O2 / 2);
 #pragma unroll
-    for (int o = LPR / 16; o > 0; o >>= 1) w1 += shfl_xor_d(w1, o);
+    for (int o = O2 / 4; o > 0; o >>= 1) w1 += shfl_xor_d(w1, o);
     return w1;
 }
 
@@ -143,8 +148,13 @@ __device__ __forceinline__ float4 mp_lds_again(const float4 *p)
 template <int N>
 __device__ __forceinline__ void mp_cp_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
 
+// rows per lane group and step: 8, or 4 for wide rows, so that a stage stays at 4-6 KB per warp and two CTAs fit an SM
+__host__ __device__ constexpr int mp_rbl(int NC) { return NC >= 2 ? 2 : 3; }
 __host__ __device__ constexpr int mp_stages(int NC) { return NC == 3 ? 2 : 3; }
-__host__ __device__ constexpr size_t mp_ring_bytes(int NC) { return (size_t)MP_WARPS * mp_stages(NC) * 8 * NC * 32 * 16; }
+__host__ __device__ constexpr size_t mp_ring_bytes(int NC)
+{
+    return (size_t)MP_WARPS * mp_stages(NC) * (1 << mp_rbl(NC)) * NC * 32 * 16;
+}
 
 template <bool CURV, int LOG, int NC>
 __global__ void __launch_bounds__(MP_THREADS, 2)
@@ -155,12 +165,12 @@ k_mp_pass(int n_voxels, int m, int m_cap, const float *__restrict__ DA,
           double *__restrict__ gpart, double *__restrict__ spart, const MpState *__restrict__ st)
 {
     if (st->reason != 0) return;                              // the solve has stopped: nothing to do
-    constexpr int LPR = 1 << LOG, GPW = 32 / LPR, LOWB = LOG - 3, RB = 8, COLS = LPR * NC * 4;
+    constexpr int RBL = mp_rbl(NC), RB = 1 << RBL;
+    constexpr int LPR = 1 << LOG, GPW = 32 / LPR, LOWB = LOG - RBL, COLS = LPR * NC * 4;
     constexpr int STAGES = mp_stages(NC), ITEMS = RB * NC;    // 16-byte chunks per lane and stage
     extern __shared__ float4 mp_ring[];                       // [warp][STAGES][ITEMS][32]: every lane's own prefetch FIFO
     __shared__ double red_s[MP_WARPS + 1];
     __shared__ float sT[256], sWo[256], sWu[256];             // the objective's tables
-    __shared__ double accs[CURV ? 1 : MP_WARPS * COLS];       // per-warp partials of g_A
     for (int t = threadIdx.x; t < n_struct; t += MP_THREADS) { sT[t] = T[t]; sWo[t] = w_over[t]; sWu[t] = w_under[t]; }
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gl = lane & (LPR - 1), grp = lane >> LOG;
@@ -226,8 +236,8 @@ k_mp_pass(int n_voxels, int m, int m_cap, const float *__restrict__ DA,
             }
             pz[s] = zi; pq[s] = qi;
         }
-        const double zi = mp_reduce8<LOG>(pz, gl);
-        const double qi = CURV ? mp_reduce8<LOG>(pq, gl) : 0.0;
+        const double zi = mp_reduce<LOG, RBL>(pz, gl);
+        const double qi = CURV ? mp_reduce<LOG, RBL>(pq, gl) : 0.0;
         const int64_t i = base + my_slot * GPW + grp;
         double gz = 0.0;
         if (i < n_voxels) {
@@ -258,8 +268,11 @@ k_mp_pass(int n_voxels, int m, int m_cap, const float *__restrict__ DA,
             }
         }
     }
-    // ---- CTA partials in a fixed order: the groups of a warp, then the warps
+    // ---- CTA partials in a fixed order: the groups of a warp, then the warps (in the ring's memory, free by now)
     if (!CURV) {
+        double *accs = (double *)mp_ring;                     // [MP_WARPS][COLS] <= 24 KB
+        mp_cp_wait<0>();
+        __syncthreads();
 #pragma unroll
         for (int c = 0; c < NC; ++c)
 #pragma unroll
