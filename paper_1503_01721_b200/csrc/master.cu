@@ -21,7 +21,7 @@ constexpr int MP_STEP_THREADS = 1024;         // the one-CTA step kernel
 constexpr int MP_STEP_WARPS = MP_STEP_THREADS / 32;
 constexpr int MP_MAX_NC = 12;                 // up to 12 x 32 = 384 apertures
 #ifndef VMAT_MP_CTAS_PER_SM
-#define VMAT_MP_CTAS_PER_SM 2
+#define VMAT_MP_CTAS_PER_SM 3
 #endif
 constexpr int MP_HIST = 6;                    // objective values the "last five changes" rule looks at
 
@@ -37,7 +37,7 @@ struct MpState {                              // device-resident scalars of one 
 
 struct vmat_mp {
     int32_t n_voxels = 0, m_cap = 0, m = 0;
-    int n_cta = 0, device = 0;
+    int n_cta = 0, n_sm = 0, device = 0;         // n_cta: CTAs of the pass = n_sm x (3 up to 128 apertures, else 2)
     float *DA = nullptr;                      // [n_voxels][m_cap]
     double *y = nullptr, *y_prev = nullptr, *g = nullptr, *g_prev = nullptr, *lo = nullptr, *hi = nullptr;   // [m_cap]
     double *gpart = nullptr;                  // [m_cap][n_cta] per-CTA partials of g_A
@@ -150,14 +150,14 @@ __device__ __forceinline__ void mp_cp_wait() { asm volatile("cp.async.wait_group
 
 // rows per lane group and step: 8, or 4 for wide rows, so that a stage stays at 4-6 KB per warp and two CTAs fit an SM
 __host__ __device__ constexpr int mp_rbl(int NC) { return NC >= 2 ? 2 : 3; }
-__host__ __device__ constexpr int mp_stages(int NC) { return NC == 3 ? 2 : 3; }
+__host__ __device__ constexpr int mp_stages(int NC) { return NC == 2 ? 3 : 2; }
 __host__ __device__ constexpr size_t mp_ring_bytes(int NC)
 {
     return (size_t)MP_WARPS * mp_stages(NC) * (1 << mp_rbl(NC)) * NC * 32 * 16;
 }
 
 template <bool CURV, int LOG, int NC>
-__global__ void __launch_bounds__(MP_THREADS, 2)
+__global__ void __launch_bounds__(MP_THREADS, NC == 1 ? 3 : 2)
 k_mp_pass(int n_voxels, int m, int m_cap, const float *__restrict__ DA,
           const double *__restrict__ y, const double *__restrict__ gvec,
           const uint8_t *__restrict__ vstruct, int n_struct, const float *__restrict__ T,
@@ -460,7 +460,8 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
     int n_sm = 1;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, h->device);
     mp_set_smem_attributes();
-    h->n_cta = n_sm * VMAT_MP_CTAS_PER_SM;                                     // fixed for the handle: fixes every summation order
+    h->n_sm = n_sm;
+    h->n_cta = n_sm * VMAT_MP_CTAS_PER_SM;                                     // the most a pass uses (allocation)
     cudaStream_t s = (cudaStream_t)stream;
     auto alloc = [&](void **p, size_t bytes) { return cudaMalloc(p, bytes > 0 ? bytes : 1) == cudaSuccess; };
     const size_t mc = (size_t)h->m_cap;
@@ -478,6 +479,7 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
     cudaMemsetAsync(h->DA, 0, (size_t)n_voxels * mc * 4, s);
     cudaMemsetAsync(h->y, 0, mc * 8, s);
     cudaMemsetAsync(h->spart, 0, (size_t)h->n_cta * 16, s);
+    h->n_cta = 0;                                                              // set per solve
     VMAT_CUDA(cudaStreamSynchronize(s));
     *out = h;
     return VMAT_OK;
@@ -534,6 +536,8 @@ int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, con
     REQUIRE(eps_F >= 0.0 && eps_y >= 0.0, "negative tolerance");
     cudaStream_t s = (cudaStream_t)stream;
     g_vmat_launches = 0;
+    // resident CTAs per SM of the pass kernel that m selects; fixed by m, so every summation order is fixed by m
+    h->n_cta = h->n_sm * (h->m <= 128 ? 3 : 2);
     if (max_iter + 1 > h->hist_cap) {
         if (h->F_hist) cudaFree(h->F_hist);
         if (h->delta_hist) cudaFree(h->delta_hist);
