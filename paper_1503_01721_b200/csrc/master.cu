@@ -150,14 +150,14 @@ __device__ __forceinline__ void mp_cp_wait() { asm volatile("cp.async.wait_group
 
 // rows per lane group and step: 8, or 4 for wide rows, so that a stage stays at 4-6 KB per warp and two CTAs fit an SM
 __host__ __device__ constexpr int mp_rbl(int NC) { return NC >= 2 ? 2 : 3; }
-__host__ __device__ constexpr int mp_stages(int NC) { return NC == 2 ? 3 : 2; }
+__host__ __device__ constexpr int mp_stages(int NC) { return 2; }
 __host__ __device__ constexpr size_t mp_ring_bytes(int NC)
 {
     return (size_t)MP_WARPS * mp_stages(NC) * (1 << mp_rbl(NC)) * NC * 32 * 16;
 }
 
 template <bool CURV, int LOG, int NC>
-__global__ void __launch_bounds__(MP_THREADS, NC == 1 ? 3 : 2)
+__global__ void __launch_bounds__(MP_THREADS, NC <= 2 ? 3 : 2)
 k_mp_pass(int n_voxels, int m, int m_cap, const float *__restrict__ DA,
           const double *__restrict__ y, const double *__restrict__ gvec,
           const uint8_t *__restrict__ vstruct, int n_struct, const float *__restrict__ T,
@@ -537,7 +537,7 @@ int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, con
     cudaStream_t s = (cudaStream_t)stream;
     g_vmat_launches = 0;
     // resident CTAs per SM of the pass kernel that m selects; fixed by m, so every summation order is fixed by m
-    h->n_cta = h->n_sm * (h->m <= 128 ? 3 : 2);
+    h->n_cta = h->n_sm * (h->m <= 256 ? 3 : 2);
     if (max_iter + 1 > h->hist_cap) {
         if (h->F_hist) cudaFree(h->F_hist);
         if (h->delta_hist) cudaFree(h->delta_hist);
