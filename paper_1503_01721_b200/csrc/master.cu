@@ -316,8 +316,14 @@ k_mp_step(int m, int m_cap, int n_cta, double *__restrict__ y, double *__restric
         for (int k = threadIdx.x >> 5; k < m; k += MP_STEP_WARPS) {
             const double *col = gpart + (size_t)k * n_cta;
             double s = 0.0;
-#pragma unroll 4
-            for (int c = threadIdx.x & 31; c < n_cta; c += 32) s += col[c];
+            for (int c0 = threadIdx.x & 31; c0 < n_cta; c0 += 32 * 16) {        // 16 loads in flight, added in the same order
+                double v[16];
+#pragma unroll
+                for (int u = 0; u < 16; ++u) v[u] = c0 + 32 * u < n_cta ? col[c0 + 32 * u] : 0.0;
+#pragma unroll
+                for (int u = 0; u < 16; ++u)
+                    if (c0 + 32 * u < n_cta) s += v[u];
+            }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) s += shfl_xor_d(s, o);
             const double yk = y[k];
