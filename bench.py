@@ -216,7 +216,7 @@ def bench_master_problem(vm, h, obj, out, dev, m: int) -> dict:
     """BB iterations of the master problem (vmat_mp_solve, Eq. (6)-(10)) on `m` apertures of the bench
     phantom: one aperture at each of m evenly spaced control points, every leaf row opened over a seeded random
     contiguous range, dose vectors by vmat_aperture_dose (Eq. (5)).  One iteration = one pass over the dense
-    voxel-major aperture dose matrix (4 m n_voxels bytes) + the one-CTA step kernel; the time per iteration is
+    voxel-major aperture dose matrix (the rows of the voxels some aperture reaches: 4 m n_reached bytes) + the one-CTA step kernel; the time per iteration is
     the whole synchronous solve (host looks at the stop flag every 8 iterations) divided by its iterations."""
     n_v, n_a, n_rows = h.n_voxels, h.n_angles, h.n_leaf_rows
     m = max(1, min(m, n_a, 384))
@@ -248,9 +248,10 @@ def bench_master_problem(vm, h, obj, out, dev, m: int) -> dict:
     ms = e0.elapsed_time(e1)
     Fh, _ = mp.history()
     n_it = max(sol.n_iter, 1)
-    bytes_it = 4 * m * n_v
+    n_reached = mp.n_reached_voxels                                           # only these rows of DA are read
+    bytes_it = 4 * m * n_reached
     res = {"apertures": m, "iterations": sol.n_iter, "stop_reason": sol.reason, "us_per_iteration": 1e3 * ms / n_it,
-           "algorithmic_bytes_per_iteration": bytes_it, "gbs": bytes_it / (ms / n_it * 1e-3) / 1e9,
+           "algorithmic_bytes_per_iteration": bytes_it, "reached_voxels": n_reached, "gbs": bytes_it / (ms / n_it * 1e-3) / 1e9,
            "F_start": float(Fh[0]), "F_end": sol.F, "dtype": "f32 storage, f64 sums", "build_s": round(t_build, 2),
            "workload": f"{m} apertures (random contiguous openings, one per control point), {n_v} voxels"}
     mp.close()

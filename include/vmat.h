@@ -236,7 +236,7 @@ int vmat_leaf_windows(const vmat_ddc *h, const uint8_t *angle_mask, const int32_
  * of the current quadratic piece; iteration 1, 3, .. use Eq. (7), 2, 4, .. Eq. (8), the previous delta is kept
  * when <s,t> <= 0; z is recomputed as DA y every iteration.
  * The handle owns a dense voxel-major copy of the aperture dose vectors (float [n_voxels][max_apertures],
- * max_apertures <= 384) and the FP64 iteration state; y persists between solves (warm start, as in the
+ * max_apertures <= 384; rows of voxels no aperture reaches are never read) and the FP64 iteration state; y persists between solves (warm start, as in the
  * column-generation loop L56).  All sums are FP64 in a fixed order: results are deterministic. */
 typedef struct vmat_mp vmat_mp;
 int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void *stream);
@@ -249,6 +249,10 @@ int vmat_mp_add_aperture(vmat_mp *h, const float *DA, double y0, double y_lo, do
 /* Overwrites the fluence rates of the current apertures (y_host host double [count]); clipped by the solve. */
 int vmat_mp_set_fluence(vmat_mp *h, const double *y_host, void *stream);
 int vmat_mp_size(const vmat_mp *h, int32_t *n_apertures, int32_t *max_apertures /* host, out, may be NULL */);
+/* Voxels that at least one of the current apertures reaches (a non-zero in their row of the aperture dose matrix), as
+ * of the last solve.  Only these rows are read by the BB passes (4 m n_reached bytes per iteration); the dose of the
+ * others is 0 whatever y, and their constant terms of Eq. (1) are added to F once per solve. */
+int vmat_mp_reached_voxels(const vmat_mp *h, int32_t *n_reached /* host, out */);
 /* Runs the BB iteration from the handle's current y until a stopping rule fires (tested at the top of every
  * iteration, in this order):  reason 1 "stationary": every entry of g_A is 0 after the subspace rule;
  * 2 "objective": it >= 5 and |F(j) - F(j-1)| <= eps_F |F(j-1)| for the five latest j;  3 "step": it >= 1 and

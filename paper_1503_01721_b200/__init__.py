@@ -33,7 +33,7 @@ EXPORTS = [
     "vmat_mp_create", "vmat_mp_destroy", "vmat_mp_reset", "vmat_mp_add_aperture", "vmat_mp_set_fluence", "vmat_mp_size",
     "vmat_mp_solve", "vmat_mp_history", "vmat_column_generation",
     "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained", "vmat_leaf_windows",
-    "vmat_column_generation_ex", "vmat_price_select",
+    "vmat_column_generation_ex", "vmat_price_select", "vmat_mp_reached_voxels",
 ]
 
 
@@ -81,6 +81,7 @@ def load_library():
     lib.vmat_mp_add_aperture.argtypes = [vp, vp, f64, f64, f64, vp]
     lib.vmat_mp_set_fluence.argtypes = [vp, vp, vp]
     lib.vmat_mp_size.argtypes = [vp, vp, vp]
+    lib.vmat_mp_reached_voxels.argtypes = [vp, vp]
     lib.vmat_mp_solve.argtypes = [vp, vp, i32, vp, vp, vp, i32, f64, f64, vp, vp, vp, vp, vp, vp]
     lib.vmat_mp_history.argtypes = [vp, vp, vp]
     lib.vmat_column_generation.argtypes = [vp, vp, vp, i32, vp, vp, vp, i32, f64, f64, i32, f64, f64, vp, vp, vp,
@@ -390,6 +391,13 @@ class MasterProblem:
     def n_apertures(self) -> int:
         n = ctypes.c_int32()
         _check(load_library().vmat_mp_size(self._h, ctypes.byref(n), None))
+        return int(n.value)
+
+    @property
+    def n_reached_voxels(self) -> int:
+        """Voxels reached by at least one aperture as of the last solve (the rows the BB passes read)."""
+        n = ctypes.c_int32()
+        _check(load_library().vmat_mp_reached_voxels(self._h, ctypes.byref(n)))
         return int(n.value)
 
     def reset(self):

@@ -11,6 +11,8 @@
 // All sums are FP64 in a fixed order (FP32 storage of DA, T, weights): deterministic, and a trajectory differs
 // from the FP64 oracle's by summation order only.
 #include "common.cuh"
+#include <cub/device/device_select.cuh>
+#include <thrust/iterator/counting_iterator.h>
 #include <new>
 #include <stdlib.h>
 #include <vector>
@@ -46,6 +48,15 @@ struct vmat_mp {
     double *F_hist = nullptr, *delta_hist = nullptr;   // [hist_cap + 1]
     int32_t hist_cap = 0;
     int32_t last_n_iter = 0;
+    // the voxels some aperture reaches (rows of DA with a non-zero): only they are visited by the passes
+    uint8_t *row_flag = nullptr;              // [n_voxels] set by vmat_mp_add_aperture
+    int32_t *active = nullptr;                // [n_voxels] their indices, ascending; valid while active_valid
+    int32_t *n_active_dev = nullptr;          // [1]
+    void *select_tmp = nullptr;               // scratch of the compaction
+    size_t select_tmp_bytes = 0;
+    int32_t n_active = 0;
+    bool active_valid = false;
+    double *F_unreached = nullptr;            // [1] F of the other voxels (z = 0), per solve
 };
 
 __device__ __forceinline__ double shfl_xor_d(double v, int o) { return __shfl_xor_sync(0xffffffffu, v, o); }
@@ -68,10 +79,34 @@ __device__ __forceinline__ double mp_block_sum(double v, double *red /* [NW + 1]
     return red[NW];
 }
 
-__global__ void k_mp_set_column(int n_voxels, int m_cap, int k, const float *__restrict__ col, float *__restrict__ DA)
+// column k of DA; a voxel that any aperture reaches is flagged: only those rows are ever read again
+__global__ void k_mp_set_column(int n_voxels, int m_cap, int k, const float *__restrict__ col, float *__restrict__ DA,
+                                uint8_t *__restrict__ row_flag)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n_voxels) DA[(size_t)i * m_cap + k] = col[i];
+    if (i < n_voxels) {
+        const float v = col[i];
+        DA[(size_t)i * m_cap + k] = v;
+        if (v != 0.f) row_flag[i] = 1;
+    }
+}
+
+// F of the voxels no aperture reaches (z_i = 0 whatever y): their terms of Eq. (1) at z = 0.  One CTA, fixed order.
+__global__ void __launch_bounds__(1024)
+k_mp_unreached_F(int n_voxels, const uint8_t *__restrict__ row_flag, const uint8_t *__restrict__ vstruct,
+                 const float *__restrict__ T, const float *__restrict__ w_over, const float *__restrict__ w_under,
+                 double *__restrict__ out)
+{
+    __shared__ double red[33];
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n_voxels; i += 1024)
+        if (!row_flag[i]) {
+            const int sid = vstruct[i];
+            const double Ti = (double)T[sid], over = fmax(0.0 - Ti, 0.0), under = fmax(Ti - 0.0, 0.0);
+            s += (double)w_over[sid] * over * over + (double)w_under[sid] * under * under;
+        }
+    const double tot = mp_block_sum<32>(s, red);
+    if (threadIdx.x == 0) out[0] = tot;
 }
 
 __global__ void k_mp_clip(int m, double *__restrict__ y, const double *__restrict__ lo, const double *__restrict__ hi)
@@ -158,8 +193,8 @@ __host__ __device__ constexpr size_t mp_ring_bytes(int NC)
 
 template <bool CURV, int LOG, int NC>
 __global__ void __launch_bounds__(MP_THREADS, NC <= 2 ? 3 : 2)
-k_mp_pass(int n_voxels, int m, int m_cap, const float *__restrict__ DA,
-          const double *__restrict__ y, const double *__restrict__ gvec,
+k_mp_pass(int n_voxels /* rows to visit: the reached voxels */, const int32_t *__restrict__ active /* their indices */,
+          int m, int m_cap, const float *__restrict__ DA, const double *__restrict__ y, const double *__restrict__ gvec,
           const uint8_t *__restrict__ vstruct, int n_struct, const float *__restrict__ T,
           const float *__restrict__ w_over, const float *__restrict__ w_under, float *__restrict__ z_out,
           double *__restrict__ gpart, double *__restrict__ spart, const MpState *__restrict__ st)
@@ -198,11 +233,12 @@ k_mp_pass(int n_voxels, int m, int m_cap, const float *__restrict__ DA,
         if (base < n_voxels) {
 #pragma unroll
             for (int s = 0; s < RB; ++s) {                    // slot s of group grp is row base + s GPW + grp
-                const int64_t row = base + s * GPW + grp;
+                const int64_t pos = base + s * GPW + grp;
+                const int64_t row = pos < n_voxels ? (int64_t)active[pos] : 0;
 #pragma unroll
                 for (int c = 0; c < NC; ++c) {
                     float4 *dst = my + (size_t)(st * ITEMS + s * NC + c) * 32;
-                    if (row < n_voxels && colok[c]) mp_cp_async16(dst, DA + row * m_cap + (c * LPR + gl) * 4);
+                    if (pos < n_voxels && colok[c]) mp_cp_async16(dst, DA + row * m_cap + (c * LPR + gl) * 4);
                     else *dst = make_float4(0.f, 0.f, 0.f, 0.f);
                 }
             }
@@ -238,9 +274,10 @@ k_mp_pass(int n_voxels, int m, int m_cap, const float *__restrict__ DA,
         }
         const double zi = mp_reduce<LOG, RBL>(pz, gl);
         const double qi = CURV ? mp_reduce<LOG, RBL>(pq, gl) : 0.0;
-        const int64_t i = base + my_slot * GPW + grp;
+        const int64_t pos = base + my_slot * GPW + grp;
         double gz = 0.0;
-        if (i < n_voxels) {
+        if (pos < n_voxels) {
+            const int i = active[pos];
             const int sid = vstruct[i];
             const double Ti = (double)sT[sid], wo = (double)sWo[sid], wu = (double)sWu[sid];
             if (!CURV) {
@@ -302,7 +339,7 @@ __global__ void __launch_bounds__(MP_STEP_THREADS)
 k_mp_step(int m, int m_cap, int n_cta, double *__restrict__ y, double *__restrict__ y_prev, double *__restrict__ g,
           double *__restrict__ g_prev, const double *__restrict__ lo, const double *__restrict__ hi,
           const double *__restrict__ gpart, const double *__restrict__ spart, MpState *__restrict__ st,
-          double *__restrict__ F_hist, double *__restrict__ delta_hist)
+          double *__restrict__ F_hist, double *__restrict__ delta_hist, const double *__restrict__ F_unreached)
 {
     if (st->reason != 0) return;
     __shared__ double red_s[MP_STEP_WARPS + 1];
@@ -334,7 +371,7 @@ k_mp_step(int m, int m_cap, int n_cta, double *__restrict__ y, double *__restric
         }
         double fs = 0.0;
         for (int c = threadIdx.x; c < n_cta; c += MP_STEP_THREADS) fs += spart[2 * c];
-        const double F = mp_block_sum<MP_STEP_WARPS>(fs, red_s);
+        const double F = mp_block_sum<MP_STEP_WARPS>(fs, red_s) + F_unreached[0];
         if (threadIdx.x == 0) s_flag = 0;
         __syncthreads();
         if (nonzero) atomicOr(&s_flag, 1);
@@ -417,7 +454,7 @@ static void mp_launch_pass(const vmat_mp *h, const uint8_t *vs, int n_struct, co
                            const float *wu, float *z, cudaStream_t s)
 {
 #define MP_PASS(LOG, NC)                                                                                            \
-    k_mp_pass<CURV, LOG, NC><<<h->n_cta, MP_THREADS, mp_ring_bytes(NC), s>>>(h->n_voxels, h->m, h->m_cap, h->DA, h->y, h->g, vs,   \
+    k_mp_pass<CURV, LOG, NC><<<h->n_cta, MP_THREADS, mp_ring_bytes(NC), s>>>(h->n_active, h->active, h->m, h->m_cap, h->DA, h->y, h->g, vs,   \
                                                              n_struct, T, wo, wu, z, h->gpart, h->spart, h->st)
     const int m = h->m;                                      // lanes per row x 16-byte chunks per lane covering m columns
     if (m <= 32) MP_PASS(3, 1);                              // (8 columns per lane up to m = 128 measured 6-13 % slower)
@@ -432,7 +469,7 @@ template <int PHASE>
 static void mp_launch_step(const vmat_mp *h, cudaStream_t s)
 {
     k_mp_step<PHASE><<<1, MP_STEP_THREADS, 0, s>>>(h->m, h->m_cap, h->n_cta, h->y, h->y_prev, h->g, h->g_prev, h->lo, h->hi,
-                                              h->gpart, h->spart, h->st, h->F_hist, h->delta_hist);
+                                              h->gpart, h->spart, h->st, h->F_hist, h->delta_hist, h->F_unreached);
 }
 
 #define REQUIRE(cond, msg)                                            \
@@ -446,7 +483,7 @@ int vmat_mp_destroy(vmat_mp *h)
 {
     if (!h) return VMAT_OK;
     void *ptrs[] = {h->DA, h->y, h->y_prev, h->g, h->g_prev, h->lo, h->hi, h->gpart, h->spart, h->st, h->F_hist,
-                    h->delta_hist};
+                    h->delta_hist, h->row_flag, h->active, h->n_active_dev, h->select_tmp, h->F_unreached};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     delete h;
@@ -475,7 +512,14 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
               alloc((void **)&h->y_prev, mc * 8) && alloc((void **)&h->g, mc * 8) && alloc((void **)&h->g_prev, mc * 8) &&
               alloc((void **)&h->lo, mc * 8) && alloc((void **)&h->hi, mc * 8) &&
               alloc((void **)&h->gpart, (size_t)h->n_cta * mc * 8) && alloc((void **)&h->spart, (size_t)h->n_cta * 16) &&
-              alloc((void **)&h->st, sizeof(MpState));
+              alloc((void **)&h->st, sizeof(MpState)) && alloc((void **)&h->row_flag, (size_t)n_voxels) &&
+              alloc((void **)&h->active, (size_t)n_voxels * 4) && alloc((void **)&h->n_active_dev, 4) &&
+              alloc((void **)&h->F_unreached, 8);
+    if (ok) {
+        cub::DeviceSelect::Flagged(nullptr, h->select_tmp_bytes, thrust::counting_iterator<int32_t>(0), h->row_flag, h->active,
+                                   h->n_active_dev, n_voxels, s);
+        ok = alloc(&h->select_tmp, h->select_tmp_bytes);
+    }
     if (!ok) {
         cudaGetLastError();
         vmat_mp_destroy(h);
@@ -483,6 +527,7 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
         return VMAT_ERR_OOM;
     }
     cudaMemsetAsync(h->DA, 0, (size_t)n_voxels * mc * 4, s);
+    cudaMemsetAsync(h->row_flag, 0, (size_t)(n_voxels > 0 ? n_voxels : 1), s);
     cudaMemsetAsync(h->y, 0, mc * 8, s);
     cudaMemsetAsync(h->spart, 0, (size_t)h->n_cta * 16, s);
     h->n_cta = 0;                                                              // set per solve
@@ -491,11 +536,22 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
     return VMAT_OK;
 }
 
+// forgets the apertures and the reached-voxel flags (on stream s)
+static int mp_forget(vmat_mp *h, cudaStream_t s)
+{
+    h->m = 0;
+    h->active_valid = false;
+    if (h->n_voxels > 0) VMAT_CUDA(cudaMemsetAsync(h->row_flag, 0, (size_t)h->n_voxels, s));
+    return VMAT_OK;
+}
+
 int vmat_mp_reset(vmat_mp *h)
 {
     REQUIRE(h != nullptr, "handle is NULL");
-    h->m = 0;
-    return VMAT_OK;
+    VMAT_CUDA(cudaDeviceSynchronize());                      // no stream argument: order against everything
+    int rc = mp_forget(h, nullptr);
+    if (rc == VMAT_OK) VMAT_CUDA(cudaDeviceSynchronize());
+    return rc;
 }
 
 int vmat_mp_add_aperture(vmat_mp *h, const float *DA, double y0, double y_lo, double y_hi, void *stream)
@@ -508,7 +564,8 @@ int vmat_mp_add_aperture(vmat_mp *h, const float *DA, double y0, double y_lo, do
     g_vmat_launches = 0;
     const int k = h->m;
     if (h->n_voxels > 0) {
-        k_mp_set_column<<<(h->n_voxels + 255) / 256, 256, 0, s>>>(h->n_voxels, h->m_cap, k, DA, h->DA);
+        k_mp_set_column<<<(h->n_voxels + 255) / 256, 256, 0, s>>>(h->n_voxels, h->m_cap, k, DA, h->DA, h->row_flag);
+        h->active_valid = false;
         VMAT_LAUNCH_CHECK();
     }
     const double v[3] = {y0 < y_lo ? y_lo : (y0 > y_hi ? y_hi : y0), y_lo, y_hi};
@@ -544,6 +601,22 @@ int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, con
     g_vmat_launches = 0;
     // resident CTAs per SM of the pass kernel that m selects; fixed by m, so every summation order is fixed by m
     h->n_cta = h->n_sm * (h->m <= 256 ? 3 : 2);
+    // the voxels some aperture reaches, ascending; F of the others (their dose is 0 whatever y)
+    if (!h->active_valid) {
+        h->n_active = 0;
+        if (h->n_voxels > 0) {
+            size_t tb = h->select_tmp_bytes;
+            VMAT_CUDA(cub::DeviceSelect::Flagged(h->select_tmp, tb, thrust::counting_iterator<int32_t>(0), h->row_flag,
+                                                 h->active, h->n_active_dev, h->n_voxels, s));
+            g_vmat_launches += 2;
+            VMAT_CUDA(cudaMemcpyAsync(&h->n_active, h->n_active_dev, 4, cudaMemcpyDeviceToHost, s));
+            VMAT_CUDA(cudaStreamSynchronize(s));
+        }
+        h->active_valid = true;
+    }
+    k_mp_unreached_F<<<1, 1024, 0, s>>>(h->n_voxels, h->row_flag, voxel_struct, T, w_over, w_under, h->F_unreached);
+    VMAT_LAUNCH_CHECK();
+    if (z && h->n_voxels > 0) VMAT_CUDA(cudaMemsetAsync(z, 0, (size_t)h->n_voxels * 4, s));   // unreached voxels: z = 0
     if (max_iter + 1 > h->hist_cap) {
         if (h->F_hist) cudaFree(h->F_hist);
         if (h->delta_hist) cudaFree(h->delta_hist);
@@ -652,7 +725,7 @@ int vmat_column_generation_ex(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_str
         VMAT_CUDA(cudaMemsetAsync(L, 0, nr * 4, s));
         VMAT_CUDA(cudaMemsetAsync(R, 0, nr * 4, s));
     }
-    mp->m = 0;                                                                           // ... and no apertures
+    { int rcf = mp_forget(mp, s); if (rcf != VMAT_OK) return rcf; }                      // ... and no apertures
     int launches = 0, count = 0, stop = 1;
     if (F_hist_host) {                                                                   // F(z = 0)
         double F0 = 0.0;
@@ -715,6 +788,14 @@ int vmat_column_generation_ex(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_str
     *n_apertures_host = count;
     if (stop_host) *stop_host = stop;
     g_vmat_launches = launches;
+    return VMAT_OK;
+}
+
+int vmat_mp_reached_voxels(const vmat_mp *h, int32_t *n_reached)
+{
+    REQUIRE(h != nullptr && n_reached != nullptr, "NULL argument");
+    REQUIRE(h->active_valid, "no solve has run since the last aperture was added");
+    *n_reached = h->n_active;
     return VMAT_OK;
 }
 
