@@ -218,3 +218,37 @@ def test_column_generation_on_config1_coarsened(vm):
     assert len(ref.angles) == 5 and ref.F_hist[-1] < 0.5 * ref.F_hist[0]
     mp.close()
     h.close()
+
+
+def test_only_reached_voxels_are_visited(vm):
+    """70 % of the voxels are reached by no aperture (all-zero rows of DA), among them under-dosed target voxels whose
+    constant terms of Eq. (1) must still be in F; the count of reached voxels follows the apertures, also after a
+    reset and after adding an aperture that reaches new voxels."""
+    rng = np.random.default_rng(77)
+    n_v, m = 6000, 40
+    DA, sid, T, wo, wu = _random_mp(rng, n_v, m)
+    dead = rng.random(n_v) < 0.7
+    DA[dead] = 0.0
+    reached = int((DA != 0).any(axis=1).sum())
+    assert (wu[sid][dead] > 0).any()
+    lo, hi = np.zeros(m), np.full(m, 40.0)
+    y0 = rng.uniform(0.0, 1.0, m)
+    ref, sol, z, Fh, dh, mp, obj = _solve_both(vm, DA, sid, T, wo, wu, y0, lo, hi, max_iter=15, eps_F=0.0, eps_y=0.0)
+    _check(ref, sol, z, Fh, dh)
+    assert mp.n_reached_voxels == reached and (z[dead] == 0).all()
+    const = float((wu[sid][dead].astype(np.float64) * T[sid][dead].astype(np.float64) ** 2).sum())
+    assert const > 0.1 * ref.F                                                  # the constant part matters here
+    # one more aperture that reaches every voxel
+    col = np.full(n_v, 0.25, np.float32)
+    mp2_DA = np.concatenate([DA, col[:, None]], axis=1)
+    mp.close()
+    ref2, sol2, z2, Fh2, dh2, mp2, _ = _solve_both(vm, mp2_DA, sid, T, wo, wu, np.append(y0, 0.0), np.append(lo, 0.0),
+                                                   np.append(hi, 40.0), max_iter=15, eps_F=0.0, eps_y=0.0)
+    _check(ref2, sol2, z2, Fh2, dh2)
+    assert mp2.n_reached_voxels == n_v
+    # reset forgets the reached voxels
+    mp2.reset()
+    mp2.add_aperture(torch.from_numpy(np.ascontiguousarray(DA[:, 0])).to(DEV), 1.0, 0.0, 40.0)
+    mp2.solve(obj, max_iter=3, eps_F=0.0, eps_y=0.0)
+    assert mp2.n_reached_voxels == int((DA[:, 0] != 0).sum())
+    mp2.close()
