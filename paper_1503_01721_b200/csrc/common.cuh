@@ -209,7 +209,8 @@ int vmat_launch_price(const vmat_ddc *h, const float *g, float *p, cudaStream_t 
 int vmat_launch_select(const vmat_ddc *h, const float *p, const uint8_t *angle_mask, int32_t *L, int32_t *R,
                        double *row_price, cudaStream_t st);
 int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *angle_mask, float *p,
-                             int32_t *L, int32_t *R, double *row_price, cudaStream_t st);
+                             int32_t *L, int32_t *R, double *row_price, cudaStream_t st, bool skip_occupied = false);
+int vmat_launch_price_unoccupied(const vmat_ddc *h, const float *g, const uint8_t *angle_mask, float *p, cudaStream_t st);
 int vmat_launch_angle_price(const vmat_ddc *h, const double *row_price, const uint8_t *angle_mask,
                             double *angle_price, int32_t *best_angle, cudaStream_t st);
 int vmat_launch_select_constrained(vmat_ddc *h, const float *p, const uint8_t *angle_mask, int interdigitation,

@@ -739,11 +739,11 @@ int vmat_column_generation_ex(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_str
         // PP1: gradient at the current dose, beamlet prices; PP2: best opening per leaf row, best control point
         int rc = vmat_launch_objective(h, z, voxel_struct, n_struct, T, w_over, w_under, w.g, w.F, s);
         if (!constrained) {
-            if (rc == VMAT_OK) rc = vmat_launch_price_select(h, w.g, w.mask, w.p, w.Lw, w.Rw, w.row_price, s);
+            if (rc == VMAT_OK) rc = vmat_launch_price_select(h, w.g, w.mask, w.p, w.Lw, w.Rw, w.row_price, s, true);   // k not in C only (L58)
             if (rc == VMAT_OK) rc = vmat_launch_angle_price(h, w.row_price, w.mask, w.angle_price, w.best, s);
         } else {
             int32_t *wl[4] = {nullptr, nullptr, nullptr, nullptr};
-            if (rc == VMAT_OK) rc = vmat_launch_price(h, w.g, w.p, s);
+            if (rc == VMAT_OK) rc = vmat_launch_price_unoccupied(h, w.g, w.mask, w.p, s);                 // k not in C only (L58)
             if (rc == VMAT_OK && max_leaf_travel >= 0) {
                 for (int q = 0; q < 4; ++q) wl[q] = w.win + (size_t)q * nr;
                 rc = vmat_launch_leaf_windows(h, w.mask, L, R, n_arcs, arc_angle_offset, max_leaf_travel, wl[0], wl[1],

@@ -112,7 +112,9 @@ struct SelectArgs {
 #ifndef VMAT_PRICE_MINB
 #define VMAT_PRICE_MINB 6        // 40 registers, 1536 threads per SM: fastest of 4..8 on B200 (cfg 3)
 #endif
-template <bool SELECT, int FMT>
+// SKIP (the column-generation loop: prices are computed "at the unoccupied control points (k not in
+// C)"): beamlet rows of occupied control points (sa.angle_mask) are not streamed, their price is written as 0.
+template <bool SELECT, int FMT, bool SKIP = false>
 __global__ void __launch_bounds__(PRICE_THREADS, VMAT_PRICE_MINB)
 k_price(const int64_t *__restrict__ pptr, const MatView A, int n_rows, const float *__restrict__ g,
         float *__restrict__ p, SelectArgs sa)
@@ -127,8 +129,12 @@ k_price(const int64_t *__restrict__ pptr, const MatView A, int n_rows, const flo
     const int warp = threadIdx.x >> 5;
     const int row = blockIdx.x * PRICE_WARPS + warp;
     if (row < n_rows) {
-        const float acc = warp_sum(segment_dot<FMT, VMAT_PRICE_PIPELINE>(A, pptr[row], pptr[row + 1], g, lane));
-        if (lane == 0) p[row] = acc;
+        if (SKIP && sa.angle_mask[sa.leafrow_angle[sa.beamlet_leafrow[row]]] != 0) {
+            if (lane == 0) p[row] = 0.f;
+        } else {
+            const float acc = warp_sum(segment_dot<FMT, VMAT_PRICE_PIPELINE>(A, pptr[row], pptr[row + 1], g, lane));
+            if (lane == 0) p[row] = acc;
+        }
     }
     if (SELECT) {
         // One ticket per CTA and leaf row: the CTA's 8 consecutive beamlet rows lie in a few leaf rows.
@@ -265,14 +271,14 @@ k_angle_price(int n_angles, const int32_t *__restrict__ angle_row_offset, const 
 }
 
 // ---------------------------------------------------------------- launchers
-template <bool SELECT>
+template <bool SELECT, bool SKIP = false>
 static void launch_k_price(const vmat_ddc *h, int grid, const float *g, float *p, const SelectArgs &sa, cudaStream_t st)
 {
     const MatView A = view_of(h->Dt);
     switch (fmt_of(h->Dt)) {
-    case 0: k_price<SELECT, FMT_WIDE><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
-    case 1: k_price<SELECT, FMT_NARROW><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
-    default: k_price<SELECT, FMT_NARROW_1BASE><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
+    case 0: k_price<SELECT, FMT_WIDE, SKIP><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
+    case 1: k_price<SELECT, FMT_NARROW, SKIP><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
+    default: k_price<SELECT, FMT_NARROW_1BASE, SKIP><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
     }
 }
 
@@ -295,8 +301,20 @@ int vmat_launch_select(const vmat_ddc *h, const float *p, const uint8_t *angle_m
     return VMAT_OK;
 }
 
+// Prices of the unoccupied control points only (angle_mask != NULL): the others' rows are not read, their p is 0.
+int vmat_launch_price_unoccupied(const vmat_ddc *h, const float *g, const uint8_t *angle_mask, float *p, cudaStream_t st)
+{
+    if (h->n_beamlets == 0) return VMAT_OK;
+    const int grid = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
+    SelectArgs sa{};
+    sa.beamlet_leafrow = h->beamlet_leafrow; sa.leafrow_angle = h->leafrow_angle; sa.angle_mask = angle_mask;
+    launch_k_price<false, true>(h, grid, g, p, sa, st);
+    VMAT_LAUNCH_CHECK();
+    return VMAT_OK;
+}
+
 int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *angle_mask, float *p,
-                             int32_t *L, int32_t *R, double *row_price, cudaStream_t st)
+                             int32_t *L, int32_t *R, double *row_price, cudaStream_t st, bool skip_occupied)
 {
     if (h->n_leaf_rows == 0) return VMAT_OK;
     const int grid = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
@@ -307,7 +325,8 @@ int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *a
     }
     SelectArgs sa{h->beamlet_leafrow, h->leafrow_col_offset, h->leafrow_angle, angle_mask, h->leafrow_done,
                   h->S_scratch, L, R, row_price, h->n_leaf_rows};
-    launch_k_price<true>(h, grid, g, p, sa, st);
+    if (skip_occupied && angle_mask != nullptr) launch_k_price<true, true>(h, grid, g, p, sa, st);
+    else launch_k_price<true>(h, grid, g, p, sa, st);
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }
