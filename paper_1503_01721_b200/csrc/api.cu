@@ -130,6 +130,9 @@ int vmat_ddc_destroy(vmat_ddc *h)
                     h->leafrow_pos0, h->angle_pmin, h->angle_wd, h->row_bp_offset, h->cs_bp, h->ad_acc, h->angle_order};
     for (void *p : ptrs)
         if (p) cudaFree(p);
+    if (h->cs_fork) cudaEventDestroy(h->cs_fork);
+    if (h->cs_join) cudaEventDestroy(h->cs_join);
+    if (h->cs_aux) cudaStreamDestroy(h->cs_aux);
     delete h;
     return VMAT_OK;
 }

@@ -107,6 +107,12 @@ struct vmat_ddc {
     int64_t *row_bp_offset = nullptr;       // [n_leaf_rows+1] start of each leaf row's back pointers in cs_bp
     uint16_t *cs_bp = nullptr;              // back pointers of the row-by-row recursion: per row wd + (n+1)^2
     int32_t cs_max_wd = 0, cs_max_n = 0, cs_max_rows = 0;
+    // k_cs_dp runs as two concurrent launches: control points whose longest leaf row is <= CS_SMALL_ROW get a small
+    // shared-memory table (several CTAs per SM) on an auxiliary stream, the others the full-size table on the caller's
+    int32_t cs_bin_off[3] = {0, 0, 0};      // angle_order[off[b] .. off[b+1]): bin 0 = long rows, bin 1 = short rows
+    int32_t cs_bin_tab[2] = {1, 1};         // table dimension (longest row + 1) of each bin
+    cudaStream_t cs_aux = nullptr;
+    cudaEvent_t cs_fork = nullptr, cs_join = nullptr;
     std::vector<int32_t> h_leafrow_pos0;
     // scratch for the end-to-end host call (allocated on first use)
     float *e2e_x = nullptr, *e2e_d = nullptr, *e2e_g = nullptr, *e2e_p = nullptr;

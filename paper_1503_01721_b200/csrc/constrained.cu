@@ -25,6 +25,7 @@
 #include <algorithm>
 
 constexpr int CS_THREADS = 256;
+constexpr int CS_SMALL_ROW = 64;                      // control points without a longer leaf row use the small table
 constexpr int CS_MAX_POS = 255;                       // positions are packed in 8 bits each
 constexpr unsigned CS_NONE = 0xffffu;
 
@@ -462,12 +463,28 @@ int vmat_launch_select_constrained(vmat_ddc *h, const float *p, const uint8_t *a
         k_cs_prefix<<<(h->n_leaf_rows + 127) / 128, 128, 0, st>>>(h->n_leaf_rows, h->leafrow_col_offset, p, h->S_scratch);
         VMAT_LAUNCH_CHECK();
     }
-    if (h->n_angles > 0) {
-        const int tab_n = h->cs_max_n + 1;
+    // bin 0 (long rows, full-size table, one CTA per SM) on the caller's stream, bin 1 (short rows, small table, several
+    // CTAs per SM) on the auxiliary stream at the same time; fork / join by events
+    const int cnt0 = h->cs_bin_off[1] - h->cs_bin_off[0], cnt1 = h->cs_bin_off[2] - h->cs_bin_off[1];
+    const bool both = cnt0 > 0 && cnt1 > 0;
+    if (both) {
+        VMAT_CUDA(cudaEventRecord(h->cs_fork, st));
+        VMAT_CUDA(cudaStreamWaitEvent(h->cs_aux, h->cs_fork, 0));
+    }
+    for (int b = 0; b < 2; ++b) {
+        const int cnt = b == 0 ? cnt0 : cnt1;
+        if (cnt <= 0) continue;
+        const int tab_n = h->cs_bin_tab[b];
+        cudaStream_t sb = (b == 1 && both) ? h->cs_aux : st;
         CsArgs A{h->angle_row_offset, h->leafrow_col_offset, h->leafrow_pos0, h->angle_pmin, h->angle_wd,
-                 h->angle_order, h->row_bp_offset, angle_mask, L_lo, L_hi, R_lo, R_hi, h->S_scratch, h->cs_bp, L, R, row_price, angle_price, interdigitation ? 1 : 0, tab_n, h->cs_max_wd, h->cs_max_rows};
-        k_cs_dp<<<h->n_angles, CS_THREADS, cs_smem_bytes(tab_n, h->cs_max_wd, h->cs_max_rows), st>>>(A);
+                 h->angle_order + h->cs_bin_off[b], h->row_bp_offset, angle_mask, L_lo, L_hi, R_lo, R_hi, h->S_scratch,
+                 h->cs_bp, L, R, row_price, angle_price, interdigitation ? 1 : 0, tab_n, h->cs_max_wd, h->cs_max_rows};
+        k_cs_dp<<<cnt, CS_THREADS, cs_smem_bytes(tab_n, h->cs_max_wd, h->cs_max_rows), sb>>>(A);
         VMAT_LAUNCH_CHECK();
+    }
+    if (both) {
+        VMAT_CUDA(cudaEventRecord(h->cs_join, h->cs_aux));
+        VMAT_CUDA(cudaStreamWaitEvent(st, h->cs_join, 0));
     }
     k_cs_best<<<1, CS_THREADS, 0, st>>>(h->n_angles, angle_price, best_angle);
     VMAT_LAUNCH_CHECK();
@@ -525,6 +542,7 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
     std::vector<int32_t> pmin((size_t)(n_a > 0 ? n_a : 1), 0), wd((size_t)(n_a > 0 ? n_a : 1), 1);
     std::vector<int64_t> bpo((size_t)n_rows + 1, 0);
     std::vector<int64_t> work((size_t)(n_a > 0 ? n_a : 1), 0);                            // ~ sequential steps of k_cs_dp
+    std::vector<int32_t> amax((size_t)(n_a > 0 ? n_a : 1), 0);                            // longest leaf row of a control point
     int max_wd = 1, max_n = 0, max_rows = 1;
     for (int k = 0; k < n_a; ++k) {
         bool any = false;
@@ -539,6 +557,7 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
             if (!any || leafrow_pos0[r] < lo) lo = leafrow_pos0[r];
             if (!any || (int)e > hi) hi = (int)e;
             max_n = n > max_n ? n : max_n;
+            amax[k] = n > amax[k] ? n : amax[k];
             any = true;
         }
         REQUIRE((int64_t)hi - lo + 1 <= CS_MAX_POS + 1,
@@ -564,7 +583,24 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
     // launch order: the control points with the most sequential work first, so that the last wave is made of light ones
     std::vector<int32_t> order((size_t)(n_a > 0 ? n_a : 1), 0);
     for (int k = 0; k < n_a; ++k) order[k] = k;
-    std::stable_sort(order.begin(), order.begin() + n_a, [&](int a, int b) { return work[a] > work[b]; });
+    // ... within two bins: control points with a leaf row beyond CS_SMALL_ROW beamlets first, then the others
+    auto bin_of = [&](int k) { return amax[k] > CS_SMALL_ROW ? 0 : 1; };
+    std::stable_sort(order.begin(), order.begin() + n_a, [&](int a, int b) {
+        return bin_of(a) != bin_of(b) ? bin_of(a) < bin_of(b) : work[a] > work[b];
+    });
+    h->cs_bin_off[0] = h->cs_bin_off[1] = h->cs_bin_off[2] = 0;
+    h->cs_bin_tab[0] = h->cs_bin_tab[1] = 1;
+    for (int k = 0; k < n_a; ++k) {
+        const int b = bin_of(k);
+        h->cs_bin_off[b + 1]++;
+        h->cs_bin_tab[b] = amax[k] + 1 > h->cs_bin_tab[b] ? amax[k] + 1 : h->cs_bin_tab[b];
+    }
+    h->cs_bin_off[2] += h->cs_bin_off[1];
+    if (!h->cs_aux) {
+        VMAT_CUDA(cudaStreamCreateWithFlags(&h->cs_aux, cudaStreamNonBlocking));
+        VMAT_CUDA(cudaEventCreateWithFlags(&h->cs_fork, cudaEventDisableTiming));
+        VMAT_CUDA(cudaEventCreateWithFlags(&h->cs_join, cudaEventDisableTiming));
+    }
     for (void **q : {(void **)&h->leafrow_pos0, (void **)&h->angle_pmin, (void **)&h->angle_wd, (void **)&h->row_bp_offset,
                      (void **)&h->cs_bp, (void **)&h->angle_order})
         if (*q) { cudaFree(*q); *q = nullptr; }
