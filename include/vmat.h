@@ -188,7 +188,8 @@ int vmat_aperture_dose(const vmat_ddc *h, int32_t angle, const int32_t *L, const
  * MLC geometry, once per handle: leafrow_pos0 host int32 [n_leaf_rows] = physical column (in beamlet widths, on
  * the control point's own grid) of the first beamlet of every leaf row (ignored for rows without beamlets).  The
  * field range of a control point is [Pmin, Pmax] = [min pos0, max pos0 + n] over its non-empty rows and may span
- * at most 255 beamlet widths (and what fits the SM's shared memory: ~148 on B200).  Synchronous. */
+ * at most 255 beamlet widths; the longest leaf row is bounded by the SM's shared memory ((n+1)^2 table entries of
+ * 10 bytes: about 145 beamlets on B200).  Returns VMAT_ERR_INVALID_ARG beyond either.  Synchronous. */
 int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0);
 
 /* A4 + A5 with constraints.  A leaf row has a state (a, b), a <= b: the physical positions of its two leaf ends;
