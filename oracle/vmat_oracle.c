@@ -27,6 +27,11 @@
  * finite differences, closed forms for 1x1, the paper's first iteration (z=0, L56), scipy.sparse
  * products, O(n^3) direct enumeration, hand-worked rows in tests/golden/.  O4/O5 have no example
  * printed in the paper: pinned by brute force and invariants only.
+ *
+ *   O6  constrained aperture selection (interdigitation L135, leaf windows L66), at the end of this file;
+ *       pins in tests/test_constrained_selection_oracle.py: hand-worked control points, exhaustive enumeration of
+ *       all combinations, reduction to O4/O5.  No example is printed in the paper either ("parity unpinned" by
+ *       publication).
  */
 #include <stdint.h>
 #include <stddef.h>
