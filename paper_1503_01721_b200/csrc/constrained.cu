@@ -114,22 +114,27 @@ k_cs_dp(CsArgs A)
         for (int t = tid; t <= n; t += CS_THREADS) Sa[t] = A.S[j0 + r0 + t];
     }
     __syncthreads();
-    // the tables of a row are fetched one row ahead, so their latency hides behind the previous row's work
-    struct RowMeta { int n, pos0, llo, lhi, rlo, rhi; int64_t bpo; };
+    // the tables of a row are fetched two rows ahead and its prefix sums one row ahead, so their latency hides behind
+    // the work on the rows before
+    struct RowMeta { int j0, n, pos0, llo, lhi, rlo, rhi; int64_t bpo; };
     auto fetch = [&](int r) {
         RowMeta m;
-        m.n = A.leafrow_col_offset[r + 1] - A.leafrow_col_offset[r];
+        m.j0 = A.leafrow_col_offset[r];
+        m.n = A.leafrow_col_offset[r + 1] - m.j0;
         m.pos0 = A.pos0[r];
         m.llo = A.L_lo ? A.L_lo[r] : INT_MIN; m.lhi = A.L_hi ? A.L_hi[r] : INT_MAX;
         m.rlo = A.R_lo ? A.R_lo[r] : INT_MIN; m.rhi = A.R_hi ? A.R_hi[r] : INT_MAX;
         m.bpo = A.row_bp_offset[r];
         return m;
     };
-    RowMeta nxt = fetch(r0);
+    RowMeta nxt = fetch(r0), nn = nr > 1 ? fetch(r0 + 1) : nxt;                        // rows q + 1 and q + 2 of the loop below
     for (int q = 0; q < nr; ++q) {
         const int r = r0 + q;
         const RowMeta cur = nxt;
-        if (q + 1 < nr) nxt = fetch(r + 1);
+        nxt = nn;
+        if (q + 2 < nr) nn = fetch(r + 2);
+        double s_ahead = 0.0;                                                         // this thread's prefix sum of the next row: in
+        if (q + 1 < nr && tid <= nxt.n) s_ahead = A.S[nxt.j0 + r + 1 + tid];          // flight during this row's work
         const int n = cur.n, n1 = n + 1;
         const int off = n > 0 ? cur.pos0 - pmin : 0;
         const int llo = cur.llo, lhi = cur.lhi, rlo = cur.rlo, rhi = cur.rhi;
@@ -226,8 +231,7 @@ k_cs_dp(CsArgs A)
             }
         }
         if (!last) {                                                                  // prefix sums of the next row
-            const int jn = A.leafrow_col_offset[r + 1];
-            for (int t = tid; t <= nxt.n; t += CS_THREADS) Sb[t] = A.S[jn + r + 1 + t];
+            if (tid <= nxt.n) Sb[tid] = s_ahead;                                      // n + 1 <= CS_THREADS
         }
         __syncthreads();
         // ---- PB of this row: sweep down the columns, then along the rows from the right.  SEG threads share a line:
