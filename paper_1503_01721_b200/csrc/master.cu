@@ -126,7 +126,7 @@ __global__ void k_mp_clip(int m, double *__restrict__ y, const double *__restric
 // shuffles for 8 rows instead of 8 LOG) leaves the sum of row (gl >> (LOG - 3)) in the lane.  The objective and
 // dF/dz_i follow per row, dF/dz_i is broadcast back, and every lane adds DA_ik dF/dz_i into the FP64 accumulators of
 // its own columns, which it keeps over all its rows - the row's entries are still in the lane's own shared-memory
-// FIFO slot (filled by cp.async two or three steps ahead, read conflict-free), so DA is read from HBM once.
+// FIFO slot (filled by cp.async one step ahead, read conflict-free), so DA is read from HBM once.
 // Fixed assignment of rows to warps and fixed reduction trees: deterministic.
 // (History: lanes-per-row with a full FP64 shuffle tree per row ran at 0.7-1.3 TB/s; shared-memory tiles filled by
 // cp.async with thread-per-row dot products at 3.6 TB/s under ncu, L1TEX-bound at 79 % by the tile being written
