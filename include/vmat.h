@@ -254,6 +254,10 @@ int vmat_mp_size(const vmat_mp *h, int32_t *n_apertures, int32_t *max_apertures 
  * of the last solve.  Only these rows are read by the BB passes (4 m n_reached bytes per iteration); the dose of the
  * others is 0 whatever y, and their constant terms of Eq. (1) are added to F once per solve. */
 int vmat_mp_reached_voxels(const vmat_mp *h, int32_t *n_reached /* host, out */);
+/* Launch geometry of the pass kernel for m apertures on this handle's device: CTAs of the grid and the number of
+ * voxel rows the whole grid takes per step of its grid-stride loop (parity tests size their cases with it so that
+ * the loop's steady state is reached).  Either output may be NULL. */
+int vmat_mp_pass_geometry(const vmat_mp *h, int32_t m, int32_t *n_cta, int32_t *rows_per_grid_step /* host, out */);
 /* Runs the BB iteration from the handle's current y until a stopping rule fires (tested at the top of every
  * iteration, in this order):  reason 1 "stationary": every entry of g_A is 0 after the subspace rule;
  * 2 "objective": it >= 5 and |F(j) - F(j-1)| <= eps_F |F(j-1)| for the five latest j;  3 "step": it >= 1 and

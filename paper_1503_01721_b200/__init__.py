@@ -33,7 +33,7 @@ EXPORTS = [
     "vmat_mp_create", "vmat_mp_destroy", "vmat_mp_reset", "vmat_mp_add_aperture", "vmat_mp_set_fluence", "vmat_mp_size",
     "vmat_mp_solve", "vmat_mp_history", "vmat_column_generation",
     "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained", "vmat_leaf_windows",
-    "vmat_column_generation_ex", "vmat_price_select", "vmat_mp_reached_voxels",
+    "vmat_column_generation_ex", "vmat_price_select", "vmat_mp_reached_voxels", "vmat_mp_pass_geometry",
 ]
 
 
@@ -82,6 +82,7 @@ def load_library():
     lib.vmat_mp_set_fluence.argtypes = [vp, vp, vp]
     lib.vmat_mp_size.argtypes = [vp, vp, vp]
     lib.vmat_mp_reached_voxels.argtypes = [vp, vp]
+    lib.vmat_mp_pass_geometry.argtypes = [vp, i32, vp, vp]
     lib.vmat_mp_solve.argtypes = [vp, vp, i32, vp, vp, vp, i32, f64, f64, vp, vp, vp, vp, vp, vp]
     lib.vmat_mp_history.argtypes = [vp, vp, vp]
     lib.vmat_column_generation.argtypes = [vp, vp, vp, i32, vp, vp, vp, i32, f64, f64, i32, f64, f64, vp, vp, vp,
@@ -400,6 +401,12 @@ class MasterProblem:
         _check(load_library().vmat_mp_reached_voxels(self._h, ctypes.byref(n)))
         return int(n.value)
 
+    def pass_geometry(self, m: int) -> dict:
+        """CTAs and voxel rows per grid step of the pass kernel for m apertures (vmat_mp_pass_geometry)."""
+        c, r = ctypes.c_int32(), ctypes.c_int32()
+        _check(load_library().vmat_mp_pass_geometry(self._h, int(m), ctypes.byref(c), ctypes.byref(r)))
+        return {"n_cta": int(c.value), "rows_per_grid_step": int(r.value)}
+
     def reset(self):
         _check(load_library().vmat_mp_reset(self._h))
 
@@ -478,6 +485,15 @@ def vmat_column_generation(h: DDC, mp: MasterProblem, obj: Objective, max_apertu
     k = int(n.value)
     return CGPlan(angles[:k], y[:k], Fh[:k + 1], ap[:k], its[:k],
                   "max_apertures" if stop.value == 1 else "no improving aperture", z, L, R)
+
+
+def mp_pass_geometry(m: int, device="cuda:0") -> dict:
+    """vmat_mp_pass_geometry on a throw-away one-voxel handle of capacity m."""
+    mp = MasterProblem(1, m, device)
+    try:
+        return mp.pass_geometry(m)
+    finally:
+        mp.close()
 
 
 def last_launch_count() -> int:

@@ -799,6 +799,18 @@ int vmat_mp_reached_voxels(const vmat_mp *h, int32_t *n_reached)
     return VMAT_OK;
 }
 
+int vmat_mp_pass_geometry(const vmat_mp *h, int32_t m, int32_t *n_cta, int32_t *rows_per_grid_step)
+{
+    REQUIRE(h != nullptr, "handle is NULL");
+    REQUIRE(m >= 1 && m <= h->m_cap, "m must be in 1..max_apertures");
+    // mirrors mp_launch_pass: lanes per row 2^LOG, 16-byte chunks per lane NC, rows per lane group and step 2^RBL
+    const int LOG = m <= 32 ? 3 : (m <= 64 ? 4 : 5), NC = m <= 128 ? 1 : (m <= 256 ? 2 : 3);
+    const int cta = h->n_sm * (m <= 256 ? 3 : 2);
+    if (n_cta) *n_cta = cta;
+    if (rows_per_grid_step) *rows_per_grid_step = cta * MP_WARPS * ((1 << mp_rbl(NC)) * (32 >> LOG));
+    return VMAT_OK;
+}
+
 int vmat_mp_size(const vmat_mp *h, int32_t *n_apertures, int32_t *max_apertures)
 {
     REQUIRE(h != nullptr, "handle is NULL");

@@ -174,6 +174,40 @@ def test_config3_full_size_fields_sampled(vm):
     h.close()
 
 
+def test_config3_full_size_fields_all_control_points(vm):
+    """As above, but O6 on ALL 360 control points of config 3 (about a minute of oracle time), with interdigitation
+    and - second pass - with interdigitation plus seeded leaf windows."""
+    import time
+    from synth import phantom as P
+    spec = synth.config_spec(3)
+    cmins, cmaxs, aco, aro, lco = P._fields(spec)
+    pos0 = torch.cat([torch.where(cx >= cn, cn, torch.zeros_like(cn)) for cn, cx in zip(cmins, cmaxs)]).numpy().astype(np.int32)
+    aro, lco = aro.numpy().astype(np.int32), lco.numpy().astype(np.int32)
+    n_b, n_rows = int(lco[-1]), lco.size - 1
+    j = np.arange(n_b, dtype=np.float64)
+    u = synth.draw_x(n_b, 78).numpy().astype(np.float64)
+    p = (np.sin(j * 0.41) + 0.5 * np.sin(j * 0.013) + (u - 0.5) - 0.15).astype(np.float32)
+    h = selection_handle(vm, aro, lco, pos0)
+    rng = np.random.default_rng(11)
+    # windows around a feasible aperture (the interdigitation-constrained optimum of a second price vector), a few
+    # positions wide: they bind for most rows but leave every control point feasible
+    p2 = (np.sin(j * 0.29 + 1.0) + 0.5 * np.sin(j * 0.017) + (u - 0.5) - 0.2).astype(np.float32)
+    L2, R2 = gpu_select(vm, h, p2, True)[:2]
+    W = [(L2 - rng.integers(0, 5, n_rows)).astype(np.int32), (L2 + rng.integers(0, 5, n_rows)).astype(np.int32),
+         (R2 - rng.integers(0, 5, n_rows)).astype(np.int32), (R2 + rng.integers(0, 5, n_rows)).astype(np.int32)]
+    for win in (None, W):
+        t0 = time.time()
+        kw = {} if win is None else dict(L_lo=win[0], L_hi=win[1], R_lo=win[2], R_hi=win[3])
+        ref = oracle.select_constrained(p, aro, lco, pos0, True, **kw)
+        got = gpu_select(vm, h, p, True, W=win)
+        assert_same(got, ref)
+        print(f"\n[cfg3 fields, all control points{' + windows' if win else ''}] oracle {time.time() - t0:.0f} s, "
+              f"{int((ref[1] > ref[0]).sum())} open rows, {int(np.isinf(ref[3]).sum())} infeasible control points, "
+              f"best {ref[4]}")
+        assert (ref[1] > ref[0]).sum() > 1000 and not np.isinf(ref[3]).any()
+    h.close()
+
+
 def test_errors(vm):
     h = selection_handle(vm, [0, 1], [0, 3], [0])
     out = h.alloc_outputs()
@@ -268,5 +302,38 @@ def test_constrained_column_generation_on_config1_coarsened(vm):
                   arc_angle_offset=ph.arc_angle_offset.numpy(), **kw)
     _compare_constrained_plans(plan, ref)
     assert len(ref.angles) == 5
+    mp.close()
+    h.close()
+
+
+@pytest.mark.parametrize("constrained", [False, True])
+def test_column_generation_on_config1_full(vm, constrained):
+    """The loop (free, and under interdigitation + leaf travel) on the FULL config 1 (3.3e8 nnz, 180 control points, 434 688
+    voxels): the first three apertures against the oracle's loop."""
+    import time
+    from oracle import column_generation as ocg
+    ph = synth.generate(synth.config_spec(1), device=DEV)
+    A = as_np(ph)
+    h = vm.vmat_ddc_create(ph.n_voxels, ph.n_beamlets, ph.coo_voxel, ph.coo_beamlet, ph.coo_val,
+                           ph.angle_col_offset, ph.angle_row_offset, ph.leafrow_col_offset, device=DEV)
+    ph.coo_voxel = ph.coo_beamlet = ph.coo_val = None
+    vm.vmat_ddc_set_leaf_geometry(h, ph.leafrow_pos0)
+    obj = obj_to_device(A, DEV)
+    mp = vm.MasterProblem(A["n_v"], 8, DEV)
+    kw = dict(interdigitation=True, max_leaf_travel=2) if constrained else {}
+    okw = dict(leafrow_pos0=ph.leafrow_pos0.numpy(), arc_angle_offset=ph.arc_angle_offset.numpy(), **kw) if constrained else {}
+    plan = vm.vmat_column_generation(h, mp, obj, 3, 0.0, 100.0, mp_max_iter=300,
+                                     arc_angle_offset=ph.arc_angle_offset if constrained else None, **kw)
+    t0 = time.time()
+    ref = ocg.run(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], A["sid"], A["T"], A["wo"], A["wu"], A["lco"],
+                  A["aro"], max_apertures=3, y_lo=0.0, y_hi=100.0, mp_max_iter=300, **okw)
+    print(f"\n[cfg1 full, {'constrained' if constrained else 'free'}] control points {ref.angles}, F {ref.F_hist[0]:.4e} -> "
+          f"{ref.F_hist[-1]:.4e}, MP iterations {ref.mp_iters} (GPU {plan.mp_iters.tolist()}), oracle {time.time() - t0:.0f} s")
+    if constrained:
+        _compare_constrained_plans(plan, ref)
+    else:
+        from test_gpu_master_problem import _compare_plans
+        _compare_plans(A, plan, ref, h)
+    assert len(ref.angles) == 3 and ref.F_hist[-1] < ref.F_hist[0]
     mp.close()
     h.close()

@@ -328,3 +328,64 @@ def test_config3_full_size_sampled(vm):
     print(f"  selection: {n_open} open rows of {L.size}, {n_partial} not fully open, best control point {best}")
     assert n_open > 0 and n_partial > 0
     h.close()
+
+
+def test_config3_full_size_all_elements(vm):
+    """Config 3 at full size, EVERY element: the oracle streams the COO triplets block by block (O1 and O3 are sums
+    over triplets, so a pass over consecutive blocks of the input with the partial sums added in FP64 is the one
+    pass of the definition up to FP64 rounding; P6 pins the additivity) and every d_i, g_i, p_j and F
+    is compared at the `north_star` tolerances; the whole selection bit for bit (C6 (ii)) and against the oracle's
+    pure FP64 path (C6 (iii))."""
+    import paper_1503_01721_b200 as vmod
+    t_start = time.time()
+    ph = _phantom_on_gpu(3)
+    n_v, n_b, nnz = ph.n_voxels, ph.n_beamlets, ph.nnz
+    h = vmod.vmat_ddc_create(n_v, n_b, ph.coo_voxel, ph.coo_beamlet, ph.coo_val, ph.angle_col_offset,
+                             ph.angle_row_offset, ph.leafrow_col_offset, device=DEV)
+    info = h.info
+    # both tile kinds (one base per tile / one base per group) and pads occur in this run
+    assert 0 < info["tiles_uniform_d"] < info["tiles_d"] and info["padded_d"] > nnz and info["padded_dt"] > nnz
+    A = dict(sid=ph.voxel_struct.numpy(), T=ph.struct_T.numpy(), wo=ph.struct_w_over.numpy(),
+             wu=ph.struct_w_under.numpy(), lco=ph.leafrow_col_offset.numpy(), aro=ph.angle_row_offset.numpy())
+    obj = obj_to_device(A, DEV)
+    out = h.alloc_outputs()
+    for scale in (0.55, 0.5, 0.47, 0.44, 0.41, 0.38):          # near balance: mixed-sign gradient and prices
+        x = synth.draw_x(n_b, 7, scale=scale)
+        vmod.vmat_price_eval(h, x.to(DEV), obj, out)
+        torch.cuda.synchronize()
+        if bool((out.p > 0).any()) and bool((out.p < 0).any()) and bool((out.g < 0).any()):
+            break
+    xn = x.numpy()
+    CH = 1 << 28                                                # triplets per block: 3.2 GB on the host
+    t0 = time.time()
+    d_ref = np.zeros(n_v, dtype=np.float64)
+    for c0 in range(0, nnz, CH):
+        sl = slice(c0, min(c0 + CH, nnz))
+        d_ref += oracle.dose(ph.coo_voxel[sl].cpu().numpy(), ph.coo_beamlet[sl].cpu().numpy(),
+                             ph.coo_val[sl].cpu().numpy(), n_v, xn)
+    F_ref, g_ref = oracle.objective_grad(d_ref, A["sid"], A["T"], A["wo"], A["wu"])
+    p_ref = np.zeros(n_b, dtype=np.float64)
+    for c0 in range(0, nnz, CH):
+        sl = slice(c0, min(c0 + CH, nnz))
+        p_ref += oracle.price(ph.coo_voxel[sl].cpu().numpy(), ph.coo_beamlet[sl].cpu().numpy(),
+                              ph.coo_val[sl].cpu().numpy(), n_b, g_ref)
+    t_oracle = time.time() - t0
+    d, g, p = out.d.cpu().numpy(), out.g.cpu().numpy(), out.p.cpu().numpy()
+    assert_vec_close("d", d, d_ref)
+    assert_vec_close("g", g, g_ref)
+    assert_vec_close("p", p, p_ref)
+    assert abs(out.F.item() - F_ref) <= REL_L2 * abs(F_ref)
+    assert (g_ref > 0).any() and (g_ref < 0).any() and (p_ref > 0).any() and (p_ref < 0).any()
+    rel = lambda a, b: np.linalg.norm(a - b) / np.linalg.norm(b)
+    print(f"  all {n_v} d, {n_v} g, {n_b} p: rel L2 err {rel(d, d_ref):.2e} {rel(g, g_ref):.2e} {rel(p, p_ref):.2e}; "
+          f"F rel err {abs(out.F.item() - F_ref) / F_ref:.2e}")
+    # selection: protocol (ii) bit for bit on the GPU's p, (iii) against the pure FP64 path
+    p32 = p_ref.astype(np.float32)
+    L_ref, R_ref, rp_ref = oracle.select_rows(p32, A["lco"])
+    ap_ref, best_ref = oracle.angle_price(rp_ref, A["aro"])
+    ev = oracle.PriceEval(d_ref, F_ref, g_ref, p_ref, p32, L_ref, R_ref, rp_ref, ap_ref, best_ref)
+    n_diff = check_selection_protocol(A, out, ev)
+    print(f"  selection: {(R_ref > L_ref).sum()} open rows of {L_ref.size}, best control point {best_ref}, rows differing "
+          f"from the pure-FP64 path: {n_diff}; oracle passes {t_oracle:.0f} s, whole test {time.time() - t_start:.0f} s")
+    assert n_diff <= L_ref.size // 1000
+    h.close()

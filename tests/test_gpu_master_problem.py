@@ -76,6 +76,97 @@ def test_trace_and_solution_match_the_oracle(vm, n_v, m):
     mp.close()
 
 
+# ---- the pass kernel in its steady state (every instantiation runs >= 3 grid steps with a ragged tail)
+# vmat_mp_pass_geometry reports, for m apertures, the number of voxel rows the whole grid takes per step of its
+# grid-stride loop; a parity case only exercises the prefetch ring's wrap and the accumulation over steps when the
+# reached voxels span several such steps (PAPER.md L139 steps 4 + 1, Eq. (6)-(10) L70-L101).
+STEADY_CASES = [8, 32, 48, 64, 100, 128, 200, 256, 300, 384]
+
+
+def _steady_problem(vm, m, rng, steps=3.4, dead_frac=0.3):
+    rows = vm.mp_pass_geometry(m)["rows_per_grid_step"]
+    n_reached_target = int(steps * rows) + 37                 # ragged tail: not a multiple of anything
+    n_v = int(n_reached_target / (1.0 - dead_frac)) + 1
+    DA, sid, T, wo, wu = _random_mp(rng, n_v, m, density=0.5)
+    dead = rng.random(n_v) < dead_frac
+    DA[dead] = 0.0
+    DA[~dead, rng.integers(0, m)] += np.float32(0.125)        # every other row is reached for certain
+    return DA, sid, T, wo, wu, rows
+
+
+@pytest.mark.parametrize("m", STEADY_CASES)
+def test_pass_kernel_steady_state_matches_the_oracle(vm, m):
+    rng = np.random.default_rng(31000 + m)
+    DA, sid, T, wo, wu, rows = _steady_problem(vm, m, rng)
+    n_v = DA.shape[0]
+    reached = int((DA != 0).any(axis=1).sum())
+    assert reached >= 3.3 * rows and reached % rows != 0      # >= 3 full grid steps + a ragged one
+    lo, hi = np.zeros(m), np.full(m, 40.0)
+    y0 = rng.uniform(0.0, 1.0, m)
+    ref, sol, z, Fh, dh, mp, _ = _solve_both(vm, DA, sid, T, wo, wu, y0, lo, hi, max_iter=12, eps_F=0.0, eps_y=0.0)
+    print(f"\n[mp steady] m={m}: {n_v} voxels, {reached} reached = {reached / rows:.2f} grid steps of {rows} rows, "
+          f"F {ref.F_hist[0]:.4e} -> {ref.F:.4e}")
+    assert mp.n_reached_voxels == reached
+    _check(ref, sol, z, Fh, dh)
+    assert ref.n_iter == 12
+    mp.close()
+
+
+@pytest.mark.parametrize("n_v,m", [(1800, 129), (1200, 200), (900, 256), (2500, 64), (2100, 40), (1700, 160)])
+def test_trace_matches_the_oracle_more_widths(vm, n_v, m):
+    """Aperture counts the first parametrisation leaves out: 129..256 (two 16-byte chunks per lane) and 33..64."""
+    rng = np.random.default_rng(2000 + n_v + m)
+    DA, sid, T, wo, wu = _random_mp(rng, n_v, m)
+    lo, hi = np.zeros(m), np.full(m, 40.0)
+    y0 = rng.uniform(0.0, 1.0, m)
+    ref, sol, z, Fh, dh, mp, _ = _solve_both(vm, DA, sid, T, wo, wu, y0, lo, hi, max_iter=12, eps_F=0.0, eps_y=0.0)
+    _check(ref, sol, z, Fh, dh)
+    mp.close()
+
+
+def test_master_problem_at_the_bench_shape_config3(vm):
+    """The shape bench.py times (`master_problem`): 128 apertures on config 3's voxel set (1.24e6 voxels), one per
+    evenly spaced control point, random contiguous openings, columns by vmat_aperture_dose (Eq. (5)); 12 BB
+    iterations against the oracle fed the SAME FP32 columns (downloaded from the device)."""
+    m = 128
+    ph = synth.generate(synth.config_spec(3), device=DEV)
+    h = vm.vmat_ddc_create(ph.n_voxels, ph.n_beamlets, ph.coo_voxel, ph.coo_beamlet, ph.coo_val,
+                           ph.angle_col_offset, ph.angle_row_offset, ph.leafrow_col_offset, device=DEV)
+    ph.coo_voxel = ph.coo_beamlet = ph.coo_val = None
+    torch.cuda.empty_cache()
+    n_v, n_a, n_rows = h.n_voxels, h.n_angles, h.n_leaf_rows
+    gen = torch.Generator().manual_seed(20150301)
+    lco = ph.leafrow_col_offset.to(torch.int64)
+    lens = (lco[1:] - lco[:-1]).to(torch.float64)
+    a, b = torch.rand(n_rows, generator=gen, dtype=torch.float64), torch.rand(n_rows, generator=gen, dtype=torch.float64)
+    L = (torch.minimum(a, b) * lens).floor().to(torch.int32).to(DEV)
+    R = (torch.maximum(a, b) * lens).ceil().to(torch.int32).to(DEV)
+    mp = vm.MasterProblem(n_v, m, DEV)
+    xs = torch.empty(h.n_beamlets, dtype=torch.float32, device=DEV)
+    col = torch.empty(n_v, dtype=torch.float32, device=DEV)
+    DA = np.empty((n_v, m), dtype=np.float64)
+    for k in range(m):
+        vm.vmat_aperture_dose(h, (k * n_a) // m, L, R, xs, col)
+        mp.add_aperture(col, 0.0, 0.0, 50.0)
+        DA[:, k] = col.cpu().numpy()
+    h.close()
+    A = dict(sid=ph.voxel_struct.numpy(), T=ph.struct_T.numpy(), wo=ph.struct_w_over.numpy(), wu=ph.struct_w_under.numpy())
+    obj = obj_to_device(A, DEV)
+    z = torch.empty(n_v, dtype=torch.float32, device=DEV)
+    sol = mp.solve(obj, max_iter=12, eps_F=0.0, eps_y=0.0, z=z)
+    Fh, dh = mp.history()
+    rows = vm.mp_pass_geometry(m)["rows_per_grid_step"]
+    reached = int((DA != 0).any(axis=1).sum())
+    print(f"\n[mp cfg3] {reached} of {n_v} voxels reached = {reached / rows:.1f} grid steps of {rows} rows")
+    assert mp.n_reached_voxels == reached and reached >= 3.3 * rows
+    sid = A["sid"]
+    ref = omp.solve(DA, np.zeros(m), np.zeros(m), np.full(m, 50.0), A["T"][sid].astype(np.float64),
+                    A["wo"][sid].astype(np.float64), A["wu"][sid].astype(np.float64), max_iter=12, eps_F=0.0, eps_y=0.0)
+    _check(ref, sol, z.cpu().numpy(), Fh.numpy(), dh.numpy())
+    assert ref.n_iter == 12 and ref.F < 0.5 * ref.F_hist[0]
+    mp.close()
+
+
 def test_each_stopping_rule(vm):
     rng = np.random.default_rng(5)
     DA, sid, T, wo, wu = _random_mp(rng, 3000, 12)
