@@ -242,10 +242,11 @@ int vmat_leaf_windows(const vmat_ddc *h, const uint8_t *angle_mask, const int32_
 typedef struct vmat_mp vmat_mp;
 int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void *stream);
 int vmat_mp_destroy(vmat_mp *h);
-/* Forgets every aperture (the storage is kept). */
-int vmat_mp_reset(vmat_mp *h);
+/* Forgets every aperture (the storage is kept).  Enqueued on `stream`, like every other call. */
+int vmat_mp_reset(vmat_mp *h, void *stream);
 /* Appends aperture k = current count: DA dev float [n_voxels] (e.g. from vmat_aperture_dose), its starting
- * fluence rate y0 (clipped into the box) and bounds.  Synchronises the stream. */
+ * fluence rate y0 (clipped into the box) and bounds.  Asynchronous: the three scalars travel through a pinned
+ * staging buffer of the handle. */
 int vmat_mp_add_aperture(vmat_mp *h, const float *DA, double y0, double y_lo, double y_hi, void *stream);
 /* Overwrites the fluence rates of the current apertures (y_host host double [count]); clipped by the solve. */
 int vmat_mp_set_fluence(vmat_mp *h, const double *y_host, void *stream);
@@ -254,8 +255,8 @@ int vmat_mp_size(const vmat_mp *h, int32_t *n_apertures, int32_t *max_apertures 
  * of the last solve.  Only these rows are read by the BB passes (4 m n_reached bytes per iteration); the dose of the
  * others is 0 whatever y, and their constant terms of Eq. (1) are added to F once per solve. */
 int vmat_mp_reached_voxels(const vmat_mp *h, int32_t *n_reached /* host, out */);
-/* Launch geometry of the pass kernel for m apertures on this handle's device: CTAs of the grid and the number of
- * voxel rows the whole grid takes per step of its grid-stride loop (parity tests size their cases with it so that
+/* Launch geometry of the solve kernel for m apertures on this handle's device: CTAs of the grid and the number of
+ * voxel rows the whole grid takes per step of the grid-stride loop of a pass (parity tests size their cases with it so that
  * the loop's steady state is reached).  Either output may be NULL. */
 int vmat_mp_pass_geometry(const vmat_mp *h, int32_t m, int32_t *n_cta, int32_t *rows_per_grid_step /* host, out */);
 /* Runs the BB iteration from the handle's current y until a stopping rule fires (tested at the top of every
@@ -265,7 +266,8 @@ int vmat_mp_pass_geometry(const vmat_mp *h, int32_t m, int32_t *n_cta, int32_t *
  *   voxel_struct, T, w_over, w_under: the objective, as for vmat_objective_grad (device pointers);
  *   z dev float [n_voxels] out or NULL: the dose z = DA y of the returned iterate;
  *   y_host double [count], F_host, n_iter_host, reason_host: host, out, each may be NULL.
- * Synchronous: the stream is synchronised every 8 iterations to read the stop flag. */
+ * The whole iteration runs in ONE cooperative kernel launch (one persistent CTA per SM; the stopping rules are
+ * evaluated on the device); the call synchronises the stream once, at the end, to return the host outputs. */
 int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, const float *T, const float *w_over,
                   const float *w_under, int32_t max_iter, double eps_F, double eps_y, float *z, double *y_host,
                   double *F_host, int32_t *n_iter_host, int32_t *reason_host, void *stream);

@@ -77,7 +77,7 @@ def load_library():
     f64 = ctypes.c_double
     lib.vmat_mp_create.argtypes = [ctypes.POINTER(vp), i32, i32, vp]
     lib.vmat_mp_destroy.argtypes = [vp]
-    lib.vmat_mp_reset.argtypes = [vp]
+    lib.vmat_mp_reset.argtypes = [vp, vp]
     lib.vmat_mp_add_aperture.argtypes = [vp, vp, f64, f64, f64, vp]
     lib.vmat_mp_set_fluence.argtypes = [vp, vp, vp]
     lib.vmat_mp_size.argtypes = [vp, vp, vp]
@@ -408,7 +408,7 @@ class MasterProblem:
         return {"n_cta": int(c.value), "rows_per_grid_step": int(r.value)}
 
     def reset(self):
-        _check(load_library().vmat_mp_reset(self._h))
+        _check(load_library().vmat_mp_reset(self._h, _stream()))
 
     def add_aperture(self, DA: torch.Tensor, y0: float, y_lo: float, y_hi: float):
         _check(load_library().vmat_mp_add_aperture(self._h, _ptr(DA, torch.float32, "cuda", self.n_voxels),

@@ -11,38 +11,33 @@
 // All sums are FP64 in a fixed order (FP32 storage of DA, T, weights): deterministic, and a trajectory differs
 // from the FP64 oracle's by summation order only.
 #include "common.cuh"
+#include <cooperative_groups.h>
 #include <cub/device/device_select.cuh>
 #include <thrust/iterator/counting_iterator.h>
 #include <new>
 #include <stdlib.h>
 #include <vector>
 
-constexpr int MP_THREADS = 256;
+constexpr int MP_THREADS = 512;             // ONE persistent CTA per SM, 16 warps
 constexpr int MP_WARPS = MP_THREADS / 32;
-constexpr int MP_STEP_THREADS = 1024;         // the one-CTA step kernel
-constexpr int MP_STEP_WARPS = MP_STEP_THREADS / 32;
 constexpr int MP_MAX_NC = 12;                 // up to 12 x 32 = 384 apertures
-#ifndef VMAT_MP_CTAS_PER_SM
-#define VMAT_MP_CTAS_PER_SM 3
-#endif
+constexpr int MP_MAX_M = MP_MAX_NC * 32;
 constexpr int MP_HIST = 6;                    // objective values the "last five changes" rule looks at
 
-struct MpState {                              // device-resident scalars of one solve
-    int it;                                   // iteration counter
-    int reason;                               // 0 running, 1 stationary, 2 objective, 3 step, 4 max_iter (C19)
-    int max_iter;
-    double eps_F, eps_y;
+struct MpState {                              // device-resident scalars of one solve (written once, when it stops)
+    int it;                                   // iterations done
+    int reason;                               // 1 stationary, 2 objective, 3 step, 4 max_iter (C19)
     double delta;                             // last step size
-    double F;                                 // objective at the current iterate
-    double Fh[MP_HIST];                       // F(it), F(it-1), ...
+    double F;                                 // objective at the returned iterate
 };
 
 struct vmat_mp {
     int32_t n_voxels = 0, m_cap = 0, m = 0;
-    int n_cta = 0, n_sm = 0, device = 0;         // n_cta: CTAs of the pass = n_sm x (3 up to 128 apertures, else 2)
+    int n_cta = 0, n_sm = 0, device = 0;      // n_cta: CTAs of the solve kernel = SMs (one persistent CTA each)
     float *DA = nullptr;                      // [n_voxels][m_cap]
-    double *y = nullptr, *y_prev = nullptr, *g = nullptr, *g_prev = nullptr, *lo = nullptr, *hi = nullptr;   // [m_cap]
+    double *y = nullptr, *g = nullptr, *lo = nullptr, *hi = nullptr;   // [m_cap]
     double *gpart = nullptr;                  // [m_cap][n_cta] per-CTA partials of g_A
+    double *gsum = nullptr;                   // [m_cap] g_A of the current iterate, after the subspace rule
     double *spart = nullptr;                  // [n_cta][2]: F partial, curvature partial
     MpState *st = nullptr;
     double *F_hist = nullptr, *delta_hist = nullptr;   // [hist_cap + 1]
@@ -57,6 +52,11 @@ struct vmat_mp {
     int32_t n_active = 0;
     bool active_valid = false;
     double *F_unreached = nullptr;            // [1] F of the other voxels (z = 0), per solve
+    double *stage3 = nullptr;                 // pinned host [3]: y0, lo, hi of the aperture being added
+    cudaEvent_t stage3_free = nullptr;        // recorded after the copies that read stage3
+    // scratch of the column-generation loop (allocated on first use, sized by the DDC handle it ran with)
+    void *cg_scratch = nullptr;
+    size_t cg_scratch_bytes = 0;
 };
 
 __device__ __forceinline__ double shfl_xor_d(double v, int o) { return __shfl_xor_sync(0xffffffffu, v, o); }
@@ -79,7 +79,8 @@ __device__ __forceinline__ double mp_block_sum(double v, double *red /* [NW + 1]
     return red[NW];
 }
 
-// column k of DA; a voxel that any aperture reaches is flagged: only those rows are ever read again
+// column k of DA; a voxel that any aperture reaches is flagged: only those rows are ever read again.  y0, lo, hi of
+// the aperture arrive in a pinned staging buffer (no stream synchronisation on the host side).
 __global__ void k_mp_set_column(int n_voxels, int m_cap, int k, const float *__restrict__ col, float *__restrict__ DA,
                                 uint8_t *__restrict__ row_flag)
 {
@@ -109,207 +110,265 @@ k_mp_unreached_F(int n_voxels, const uint8_t *__restrict__ row_flag, const uint8
     if (threadIdx.x == 0) out[0] = tot;
 }
 
-__global__ void k_mp_clip(int m, double *__restrict__ y, const double *__restrict__ lo, const double *__restrict__ hi)
-{
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k < m) y[k] = fmin(fmax(y[k], lo[k]), hi[k]);
-}
-
-// ---------------------------------------------------------------- the pass over DA
-// CURV = false: z = DA y, F, dF/dz, partials of g_A = DA^T dF/dz            (steps 4 and 1 of L139)
-// CURV = true : z = DA y, q = DA g, partials of sum_i w_i q_i^2              (first step size, C17)
+// ---------------------------------------------------------------- the whole BB solve: one persistent kernel
+// One CTA of 16 warps per SM, launched cooperatively; the BB iteration (the four steps of L139) runs on the device
+// until a stopping rule fires.  Per iteration:
+//   pass    z = DA y, F, dF/dz, per-CTA partials of g_A = DA^T dF/dz (steps 4 and 1), DA read from HBM once;
+//   sync    grid barrier;
+//   reduce  one warp per aperture sums that aperture's partials in a fixed order, applies the subspace rule
+//           Eq. (9)/(10) with the sign of C15, publishes g_A;
+//   sync    grid barrier;
+//   step    EVERY CTA forms F, the stopping rules (C19), the step size Eq. (7)/(8) (C17 at iteration 0, after one
+//           extra "curvature" pass) and the clipped update of y from the same published numbers by the same
+//           instructions in the same order, so all CTAs hold bit-identical y, y_prev, g_prev in their own shared
+//           memory and agree on when to stop; CTA 0 alone writes the trace and the result.
+// No kernel launch and no host round trip per iteration (the first version launched a pass and a one-CTA step kernel
+// per iteration and let the host look at the stop flag every 8: 61 us per launch on average over a plan).
 //
-// A group of LPR = 2^LOG lanes owns a voxel row, lane gl of the group holds
-// columns (c LPR + gl) 4 .. + 3 of it for c < NC (one 16-byte load each; the group reads the row contiguously), and a
-// warp works on 8 x (32 / LPR) rows at a time (4 when a row is wider than 128 entries).  Every lane forms its part
-// of the 8 row dot products in FP64; a halving butterfly (8 -> 4 -> 2 -> 1 values per lane, 7 + LOG - 3 double
-// shuffles for 8 rows instead of 8 LOG) leaves the sum of row (gl >> (LOG - 3)) in the lane.  The objective and
-// dF/dz_i follow per row, dF/dz_i is broadcast back, and every lane adds DA_ik dF/dz_i into the FP64 accumulators of
-// its own columns, which it keeps over all its rows - the row's entries are still in the lane's own shared-memory
-// FIFO slot (filled by cp.async one step ahead, read conflict-free), so DA is read from HBM once.
-// Fixed assignment of rows to warps and fixed reduction trees: deterministic.
-// (History: lanes-per-row with a full FP64 shuffle tree per row ran at 0.7-1.3 TB/s; shared-memory tiles filled by
-// cp.async with thread-per-row dot products at 3.6 TB/s under ncu, L1TEX-bound at 79 % by the tile being written
-// once and read twice plus 32 bytes of y per 16 bytes of tile.)
-// 2^RBL (8 or 4) values per lane, summed over the LPR lanes of a group by a halving butterfly: lane gl ends with the
-// total of value gl >> (LOG - RBL)
-template <int LOG, int RBL>
-__device__ __forceinline__ double mp_reduce(const double (&v)[1 << RBL], int gl)
+// The pass.  A warp owns R consecutive reached rows per pipeline stage, prefetched STAGES - 1 stages ahead by
+// 1-D bulk copies (cp.async.bulk, one per row, issued by R different lanes; completion counted in bytes on the
+// stage's mbarrier): no per-lane address arithmetic, no registers held across the flight.  Two lane mappings read
+// a stage from shared memory:
+//   z phase  LZ lanes per row, each CZ 16-byte chunks interleaved by LZ (so a quarter-warp reads 128 contiguous
+//            bytes or rows whose stride keeps them in different banks): the row dot in FP64 needs log2(LZ) plain
+//            shuffle steps for 32 / LZ rows at once instead of an 8-row butterfly over all 32 lanes;
+//   g phase  lane gl of a group of LPR lanes owns NC chunks of columns, as the partial sums of g_A demand, and adds
+//            DA_ik dF/dz_i for the rows of the stage, dF/dz_i broadcast through shared memory.
+// ~29 warp instructions per 512 bytes of DA instead of 64 (ncu: profiles/r2_*_mp.md).
+// All sums are FP64 in a fixed order given (m, SM count): deterministic.
+template <int V> struct MpCfg;
+//                                    bytes of a row at most | z phase: lanes per row, chunks per lane | rows per stage |
+//                                    g phase: lanes per row, chunks per lane | row padding (bank spread) | stages
+template <> struct MpCfg<0> { static constexpr int VB = 128,  LZ = 2,  CZ = 4, R = 16, LPR = 8,  NC = 1, PAD = 32, STAGES = 4; };
+template <> struct MpCfg<1> { static constexpr int VB = 256,  LZ = 4,  CZ = 4, R = 8,  LPR = 16, NC = 1, PAD = 64, STAGES = 4; };
+template <> struct MpCfg<2> { static constexpr int VB = 512,  LZ = 8,  CZ = 4, R = 8,  LPR = 32, NC = 1, PAD = 0,  STAGES = 3; };
+template <> struct MpCfg<3> { static constexpr int VB = 1024, LZ = 16, CZ = 4, R = 4,  LPR = 32, NC = 2, PAD = 0,  STAGES = 3; };
+template <> struct MpCfg<4> { static constexpr int VB = 1536, LZ = 32, CZ = 3, R = 2,  LPR = 32, NC = 3, PAD = 0,  STAGES = 4; };
+static inline int mp_variant(int m) { return m <= 32 ? 0 : (m <= 64 ? 1 : (m <= 128 ? 2 : (m <= 256 ? 3 : 4))); }
+template <int V> __host__ __device__ constexpr size_t mp_ring_bytes()
 {
-    constexpr int LPR = 1 << LOG;
-    double w4[4], w2[2];
-    if (RBL == 3) {
-        const bool up = (gl & (LPR / 2)) != 0;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const double keep = up ? v[(i + 4) & ((1 << RBL) - 1)] : v[i], send = up ? v[i] : v[(i + 4) & ((1 << RBL) - 1)];
-            w4[i] = keep + shfl_xor_d(send, LPR / 2);
-        }
-    } else {
-#pragma unroll
-        for (int i = 0; i < 4; ++i) w4[i] = v[i & ((1 << RBL) - 1)];
-    }
-    constexpr int O2 = RBL == 3 ? LPR / 4 : LPR / 2;          // offsets of the 4 -> 2 and 2 -> 1 steps
-    {
-        const bool up = (gl & O2) != 0;
-#pragma unroll
-        for (int i = 0; i < 2; ++i) {
-            const double keep = up ? w4[i + 2] : w4[i], send = up ? w4[i] : w4[i + 2];
-            w2[i] = keep + shfl_xor_d(send, O2);
-        }
-    }
-    const bool up = (gl & (O2 / 2)) != 0;
-    double w1 = (up ? w2[1] : w2[0]) + shfl_xor_d(up ? w2[0] : w2[1], O2 / 2);
-#pragma unroll
-    for (int o = O2 / 4; o > 0; o >>= 1) w1 += shfl_xor_d(w1, o);
-    return w1;
+    return (size_t)MP_WARPS * MpCfg<V>::STAGES * MpCfg<V>::R * (MpCfg<V>::VB + MpCfg<V>::PAD);
+}
+template <int V> __host__ __device__ constexpr size_t mp_smem_bytes()      // ring (>= the 16 x 384 FP64 accumulators that reuse it) + barriers
+{
+    return (mp_ring_bytes<V>() > (size_t)MP_WARPS * MP_MAX_M * 8 ? mp_ring_bytes<V>() : (size_t)MP_WARPS * MP_MAX_M * 8) +
+           (size_t)MP_WARPS * MpCfg<V>::STAGES * 8;
 }
 
-// 16-byte asynchronous copy global -> shared, bypassing L1
-__device__ __forceinline__ void mp_cp_async16(void *smem, const void *gmem)
-{
-    const uint32_t sa = (uint32_t)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(sa), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void mp_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-// a shared-memory read the compiler may not merge with an earlier one of the same address
-__device__ __forceinline__ float4 mp_lds_again(const float4 *p)
-{
-    float4 r;
-    const uint32_t sa = (uint32_t)__cvta_generic_to_shared(p);
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "r"(sa));
-    return r;
-}
-template <int N>
-__device__ __forceinline__ void mp_cp_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
+struct MpArgs {
+    int n;                      // rows to visit: the reached voxels
+    const int32_t *active;      // their indices, ascending
+    int m, m_cap;
+    const float *DA;
+    double *y, *g;              // in: start (feasible); out: returned iterate and its g_A after the subspace rule
+    const double *lo, *hi;
+    const uint8_t *vstruct;
+    int n_struct;
+    const float *T, *w_over, *w_under;
+    float *z_out;               // or NULL
+    double *gpart, *spart, *gsum;
+    MpState *st;
+    double *F_hist, *delta_hist;
+    const double *F_unreached;
+    int max_iter;
+    double eps_F, eps_y;
+};
 
-// rows per lane group and step: 8, or 4 for wide rows, so that a stage stays at 4-6 KB per warp and two CTAs fit an SM
-__host__ __device__ constexpr int mp_rbl(int NC) { return NC >= 2 ? 2 : 3; }
-__host__ __device__ constexpr int mp_stages(int NC) { return 2; }
-__host__ __device__ constexpr size_t mp_ring_bytes(int NC)
+__device__ __forceinline__ uint32_t mp_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mp_mbar_init(uint32_t bar, int count)
 {
-    return (size_t)MP_WARPS * mp_stages(NC) * (1 << mp_rbl(NC)) * NC * 32 * 16;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
 }
-
-template <bool CURV, int LOG, int NC>
-__global__ void __launch_bounds__(MP_THREADS, NC <= 2 ? 3 : 2)
-k_mp_pass(int n_voxels /* rows to visit: the reached voxels */, const int32_t *__restrict__ active /* their indices */,
-          int m, int m_cap, const float *__restrict__ DA, const double *__restrict__ y, const double *__restrict__ gvec,
-          const uint8_t *__restrict__ vstruct, int n_struct, const float *__restrict__ T,
-          const float *__restrict__ w_over, const float *__restrict__ w_under, float *__restrict__ z_out,
-          double *__restrict__ gpart, double *__restrict__ spart, const MpState *__restrict__ st)
+__device__ __forceinline__ void mp_mbar_expect_tx(uint32_t bar, uint32_t bytes)
 {
-    if (st->reason != 0) return;                              // the solve has stopped: nothing to do
-    constexpr int RBL = mp_rbl(NC), RB = 1 << RBL;
-    constexpr int LPR = 1 << LOG, GPW = 32 / LPR, LOWB = LOG - RBL, COLS = LPR * NC * 4;
-    constexpr int STAGES = mp_stages(NC), ITEMS = RB * NC;    // 16-byte chunks per lane and stage
-    extern __shared__ float4 mp_ring[];                       // [warp][STAGES][ITEMS][32]: every lane's own prefetch FIFO
-    __shared__ double red_s[MP_WARPS + 1];
-    __shared__ float sT[256], sWo[256], sWu[256];             // the objective's tables
-    for (int t = threadIdx.x; t < n_struct; t += MP_THREADS) { sT[t] = T[t]; sWo[t] = w_over[t]; sWu[t] = w_under[t]; }
-    __syncthreads();
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, gl = lane & (LPR - 1), grp = lane >> LOG;
-    double yk[NC][4], vk[NC][4], acc[NC][4];
-    bool colok[NC];
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mp_mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+// 1-D bulk copy global -> shared (the TMA unit; SASS UBLKCP), completion in bytes on an mbarrier
+__device__ __forceinline__ void mp_bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mp_fence_async_proxy() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// per-warp pipeline bookkeeping that lives across the passes of a solve
+struct MpPipe {
+    uint32_t phases;            // bit s: parity the next wait on stage s must see
+    int cstage;                 // next stage to consume
+};
+
+// One pass over the reached rows.  CURV = false: z = DA y, F, dF/dz, g_A partials (acc).  CURV = true: z = DA y,
+// q = DA v, sum_i w_i q_i^2 (C17).  ssum: this thread's part of F (or of the curvature).
+template <int V, bool CURV>
+__device__ __forceinline__ void mp_pass(const MpArgs &a, uint32_t ring_w, uint32_t bar_w, double *gzs_w, MpPipe &pp,
+                                        const double *sy, const double *sv, const float *sT, const float *sWo,
+                                        const float *sWu, double (&acc)[MpCfg<V>::NC][4], double &ssum)
+{
+    using C = MpCfg<V>;
+    constexpr int LZ = C::LZ, CZ = C::CZ, R = C::R, LPR = C::LPR, NC = C::NC, STAGES = C::STAGES;
+    constexpr int RS = C::VB + C::PAD, STAGE_BYTES = R * RS;
+    constexpr int RZ = 32 / LZ, NSUB = R / RZ, GPW = 32 / LPR, RG = R / GPW;
+    static_assert(R % RZ == 0 && R % GPW == 0 && NSUB >= 1 && NSUB <= LZ && LZ * CZ * 16 == C::VB && LPR * NC * 16 == C::VB, "mapping");
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int rz = lane / LZ, qz = lane % LZ, grp = lane / LPR, gl = lane % LPR;
+    const int n = a.n;
+    const uint32_t W = (uint32_t)((a.m + 7) / 8) * 32u;           // bytes of a row that hold apertures (32-byte sectors)
+    const int64_t step = (int64_t)gridDim.x * MP_WARPS * R;
+    int64_t base = (int64_t)(blockIdx.x * MP_WARPS + warp) * R;
+    double yz[CZ][4];                                             // y of this lane's z-phase columns
 #pragma unroll
-    for (int c = 0; c < NC; ++c) {
-        const int col = (c * LPR + gl) * 4;
-        colok[c] = col < m;                                   // m_cap is a multiple of 8: the 16-byte chunk stays inside the row
+    for (int j = 0; j < CZ; ++j)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            yk[c][j] = col + j < m ? y[col + j] : 0.0;
-            vk[c][j] = (CURV && col + j < m) ? gvec[col + j] : 0.0;
-            acc[c][j] = 0.0;
-        }
-    }
-    double ssum = 0.0;
-    const int my_slot = gl >> LOWB;                           // the row slot whose total this lane ends up with
-    const bool leader = (gl & ((1 << LOWB) - 1)) == 0;        // one lane per row adds to F and writes z
-    const int64_t step = (int64_t)gridDim.x * MP_WARPS * (RB * GPW);
-    const int64_t base0 = (int64_t)(blockIdx.x * MP_WARPS + warp) * (RB * GPW);
-    float4 *my = mp_ring + (size_t)warp * STAGES * ITEMS * 32 + lane;
-    // a stage = the 8 row slots of one step; every lane copies the chunks it will read itself, so no barrier is needed
-    auto issue = [&](int64_t base, int st) {
-        if (base < n_voxels) {
-#pragma unroll
-            for (int s = 0; s < RB; ++s) {                    // slot s of group grp is row base + s GPW + grp
-                const int64_t pos = base + s * GPW + grp;
-                const int64_t row = pos < n_voxels ? (int64_t)active[pos] : 0;
-#pragma unroll
-                for (int c = 0; c < NC; ++c) {
-                    float4 *dst = my + (size_t)(st * ITEMS + s * NC + c) * 32;
-                    if (pos < n_voxels && colok[c]) mp_cp_async16(dst, DA + row * m_cap + (c * LPR + gl) * 4);
-                    else *dst = make_float4(0.f, 0.f, 0.f, 0.f);
-                }
+        for (int k = 0; k < 4; ++k) yz[j][k] = sy[(j * LZ + qz) * 4 + k];   // 0 beyond m
+    int istage = pp.cstage;
+    int64_t ibase = base;
+    auto issue = [&]() {                                          // R rows starting at reached position ibase
+        if (ibase < n) {
+            const int nvalid = (int)min((int64_t)R, (int64_t)n - ibase);
+            const uint32_t bar = bar_w + 8u * istage;
+            if (lane == 0) mp_mbar_expect_tx(bar, (uint32_t)nvalid * W);
+            __syncwarp();
+            if (lane < nvalid) {
+                const int64_t row = __ldg(a.active + ibase + lane);
+                mp_bulk_g2s(ring_w + (uint32_t)(istage * STAGE_BYTES + lane * RS), a.DA + row * a.m_cap, W, bar);
             }
         }
-        mp_cp_commit();
+        ibase += step;
+        if (++istage == STAGES) istage = 0;
     };
+#pragma unroll 1
+    for (int s = 0; s < STAGES - 1; ++s) issue();
+#pragma unroll 1
+    for (; base < n; base += step) {
+        __syncwarp();                                             // every lane is done with the slot refilled now
+        issue();
+        const int cs = pp.cstage;
+        mp_mbar_wait(bar_w + 8u * cs, (pp.phases >> cs) & 1u);
+        pp.phases ^= 1u << cs;
+        if (++pp.cstage == STAGES) pp.cstage = 0;
+        const uint32_t stg = ring_w + (uint32_t)(cs * STAGE_BYTES);
+        // the row this lane finishes (objective, dF/dz): sub-step qz, row rz of it
+        const int rsel = qz * RZ + rz;
+        const bool fin = qz < NSUB;
+        const bool own = fin && base + rsel < n;
+        int vi = 0, sid = 0;
+        if (own) { vi = __ldg(a.active + base + rsel); sid = __ldg(a.vstruct + vi); }
+        // ---- z phase
+        double zmine = 0.0, qmine = 0.0;
 #pragma unroll
-    for (int st = 0; st < STAGES - 1; ++st) issue(base0 + st * step, st);
-    int cur = 0;
-    for (int64_t base = base0; base < n_voxels; base += step) {
-        {
-            int nxt = cur + STAGES - 1;
-            if (nxt >= STAGES) nxt -= STAGES;
-            issue(base + (STAGES - 1) * step, nxt);
-        }
-        mp_cp_wait<STAGES - 1>();
-        const float4 *stg = my + (size_t)cur * ITEMS * 32;
-        if (++cur == STAGES) cur = 0;
-        double pz[RB], pq[RB];
+        for (int u = 0; u < NSUB; ++u) {
+            const uint32_t rowp = stg + (uint32_t)((u * RZ + rz) * RS + qz * 16);
+            double z4[4] = {0.0, 0.0, 0.0, 0.0}, q4[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
-        for (int s = 0; s < RB; ++s) {
-            double zi = 0.0, qi = 0.0;
-#pragma unroll
-            for (int c = 0; c < NC; ++c) {
-                const float4 e = stg[(size_t)(s * NC + c) * 32];
-                const double a0 = (double)e.x, a1 = (double)e.y, a2 = (double)e.z, a3 = (double)e.w;
-                zi = fma(a0, yk[c][0], zi); zi = fma(a1, yk[c][1], zi); zi = fma(a2, yk[c][2], zi); zi = fma(a3, yk[c][3], zi);
+            for (int j = 0; j < CZ; ++j) {
+                float4 e;
+                asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(e.x), "=f"(e.y), "=f"(e.z), "=f"(e.w)
+                             : "r"(rowp + (uint32_t)(j * LZ * 16)));
+                const double e0 = (double)e.x, e1 = (double)e.y, e2 = (double)e.z, e3 = (double)e.w;
+                z4[0] = fma(e0, yz[j][0], z4[0]); z4[1] = fma(e1, yz[j][1], z4[1]);
+                z4[2] = fma(e2, yz[j][2], z4[2]); z4[3] = fma(e3, yz[j][3], z4[3]);
                 if (CURV) {
-                    qi = fma(a0, vk[c][0], qi); qi = fma(a1, vk[c][1], qi); qi = fma(a2, vk[c][2], qi); qi = fma(a3, vk[c][3], qi);
+                    const double *v = sv + (j * LZ + qz) * 4;
+                    q4[0] = fma(e0, v[0], q4[0]); q4[1] = fma(e1, v[1], q4[1]);
+                    q4[2] = fma(e2, v[2], q4[2]); q4[3] = fma(e3, v[3], q4[3]);
                 }
             }
-            pz[s] = zi; pq[s] = qi;
+            double zs = (z4[0] + z4[1]) + (z4[2] + z4[3]), qs = (q4[0] + q4[1]) + (q4[2] + q4[3]);
+#pragma unroll
+            for (int o = LZ / 2; o > 0; o >>= 1) {
+                zs += shfl_xor_d(zs, o);
+                if (CURV) qs += shfl_xor_d(qs, o);
+            }
+            if (qz == u) { zmine = zs; qmine = qs; }
         }
-        const double zi = mp_reduce<LOG, RBL>(pz, gl);
-        const double qi = CURV ? mp_reduce<LOG, RBL>(pq, gl) : 0.0;
-        const int64_t pos = base + my_slot * GPW + grp;
+        // ---- objective and dF/dz of the finished rows (Eq. (1), sign C1)
         double gz = 0.0;
-        if (pos < n_voxels) {
-            const int i = active[pos];
-            const int sid = vstruct[i];
+        if (own) {
             const double Ti = (double)sT[sid], wo = (double)sWo[sid], wu = (double)sWu[sid];
             if (!CURV) {
-                const double over = fmax(zi - Ti, 0.0), under = fmax(Ti - zi, 0.0);
-                gz = 2.0 * wo * over - 2.0 * wu * under;                                 // Eq. (1), sign C1
-                if (leader) {
-                    ssum += wo * over * over + wu * under * under;
-                    if (z_out) z_out[i] = (float)zi;
-                }
-            } else if (leader) {
-                const double w = zi > Ti ? wo : (zi < Ti ? wu : 0.0);                    // C17
-                ssum += w * qi * qi;
+                const double over = fmax(zmine - Ti, 0.0), under = fmax(Ti - zmine, 0.0);
+                gz = 2.0 * wo * over - 2.0 * wu * under;
+                ssum += wo * over * over + wu * under * under;
+                if (a.z_out) a.z_out[vi] = (float)zmine;
+            } else {
+                const double w = zmine > Ti ? wo : (zmine < Ti ? wu : 0.0);              // C17
+                ssum += w * qmine * qmine;
             }
         }
         if (!CURV) {
-#pragma unroll NC >= 2 ? 1 : 2
-            for (int s = 0; s < RB; ++s) {                    // g_A += DA_i: * dF/dz_i; wide rows: rolled, to bound the registers
-                const double gs = __shfl_sync(0xffffffffu, gz, (grp << LOG) + (s << LOWB));
+            if (fin) gzs_w[rsel] = gz;                            // rows past the end: 0
+            __syncwarp();
+            // ---- g phase: g_A += DA_i: * dF/dz_i
+#pragma unroll
+            for (int s = 0; s < RG; ++s) {
+                const int row = s * GPW + grp;
+                const double gs = gzs_w[row];
 #pragma unroll
                 for (int c = 0; c < NC; ++c) {
-                    const float4 e = mp_lds_again(stg + (size_t)(s * NC + c) * 32);   // not kept in registers
+                    float4 e;
+                    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(e.x), "=f"(e.y), "=f"(e.z), "=f"(e.w)
+                                 : "r"(stg + (uint32_t)(row * RS + (c * LPR + gl) * 16)));
                     acc[c][0] = fma((double)e.x, gs, acc[c][0]); acc[c][1] = fma((double)e.y, gs, acc[c][1]);
                     acc[c][2] = fma((double)e.z, gs, acc[c][2]); acc[c][3] = fma((double)e.w, gs, acc[c][3]);
                 }
             }
         }
     }
-    // ---- CTA partials in a fixed order: the groups of a warp, then the warps (in the ring's memory, free by now)
-    if (!CURV) {
-        double *accs = (double *)mp_ring;                     // [MP_WARPS][COLS] <= 24 KB
-        mp_cp_wait<0>();
+}
+
+template <int V>
+__global__ void __launch_bounds__(MP_THREADS, 1)
+k_mp_solve(const MpArgs a)
+{
+    using C = MpCfg<V>;
+    constexpr int LPR = C::LPR, NC = C::NC, STAGES = C::STAGES, COLS = C::VB / 4;
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    extern __shared__ __align__(128) unsigned char mp_dyn[];      // ring [warp][stage][row][RS]; then the barriers
+    __shared__ double red_s[MP_WARPS + 1];
+    __shared__ double sy[MP_MAX_M], syp[MP_MAX_M], sg[MP_MAX_M], sgp[MP_MAX_M];
+    __shared__ double gzs[MP_WARPS][32];
+    __shared__ float sT[256], sWo[256], sWu[256];
+    __shared__ double sFh[MP_HIST];
+    __shared__ int s_flag;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, grp = lane / LPR, gl = lane % LPR;
+    const int m = a.m, n_cta = gridDim.x;
+    constexpr size_t RING = mp_ring_bytes<V>() > (size_t)MP_WARPS * MP_MAX_M * 8 ? mp_ring_bytes<V>() : (size_t)MP_WARPS * MP_MAX_M * 8;
+    uint64_t *bars = (uint64_t *)(mp_dyn + RING);
+    for (int t = tid; t < (int)(RING / 16); t += MP_THREADS) ((float4 *)mp_dyn)[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int t = tid; t < a.n_struct; t += MP_THREADS) { sT[t] = a.T[t]; sWo[t] = a.w_over[t]; sWu[t] = a.w_under[t]; }
+    for (int k = tid; k < MP_MAX_M; k += MP_THREADS) {
+        sy[k] = k < m ? fmin(fmax(a.y[k], a.lo[k]), a.hi[k]) : 0.0;          // the start must be feasible (C16)
+        syp[k] = 0.0; sg[k] = 0.0; sgp[k] = 0.0;
+    }
+    if (tid < MP_WARPS * STAGES) mp_mbar_init(mp_smem_u32(bars + tid), 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    mp_fence_async_proxy();
+    __syncthreads();
+    const uint32_t ring_w = mp_smem_u32(mp_dyn) + (uint32_t)(warp * STAGES * C::R * (C::VB + C::PAD));
+    const uint32_t bar_w = mp_smem_u32(bars + warp * STAGES);
+    MpPipe pp = {0u, 0};
+    int it = 0, reason = 0;
+    double delta = 0.0, F = 0.0;
+    for (;;) {
+        // ---- steps 4 + 1 of L139: the gradient pass
+        double acc[NC][4];
+#pragma unroll
+        for (int c = 0; c < NC; ++c)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc[c][j] = 0.0;
+        double ssum = 0.0;
+        mp_pass<V, false>(a, ring_w, bar_w, gzs[warp], pp, sy, sg, sT, sWo, sWu, acc, ssum);
+        // CTA partials in a fixed order: the lane groups of a warp, then the warps (in the ring's memory, idle now)
         __syncthreads();
+        double *accs = (double *)mp_dyn;                          // [MP_WARPS][COLS]
 #pragma unroll
         for (int c = 0; c < NC; ++c)
 #pragma unroll
@@ -320,156 +379,156 @@ k_mp_pass(int n_voxels /* rows to visit: the reached voxels */, const int32_t *_
                 if (grp == 0) accs[warp * COLS + (c * LPR + gl) * 4 + j] = v;
             }
         __syncthreads();
-        for (int k = threadIdx.x; k < m; k += MP_THREADS) {
+        for (int k = tid; k < m; k += MP_THREADS) {
             double sacc = 0.0;
             for (int w = 0; w < MP_WARPS; ++w) sacc += accs[w * COLS + k];
-            gpart[(size_t)k * gridDim.x + blockIdx.x] = sacc;                             // [m_cap][n_cta]
+            a.gpart[(size_t)k * n_cta + blockIdx.x] = sacc;       // [m_cap][n_cta]
         }
-    }
-    const double tot = mp_block_sum(ssum, red_s);
-    if (threadIdx.x == 0) spart[2 * blockIdx.x + (CURV ? 1 : 0)] = tot;
-}
-
-// ---------------------------------------------------------------- the step: one CTA
-// PHASE 0: after the first gradient pass (it = 0): finish g_A, subspace rule, stopping rules; no update.
-// PHASE 1: after the curvature pass: delta_0 (C17), update.
-// PHASE 2: after a gradient pass, it >= 1: finish g_A, subspace rule, stopping rules, Eq. (7)/(8), update.
-template <int PHASE>
-__global__ void __launch_bounds__(MP_STEP_THREADS)
-k_mp_step(int m, int m_cap, int n_cta, double *__restrict__ y, double *__restrict__ y_prev, double *__restrict__ g,
-          double *__restrict__ g_prev, const double *__restrict__ lo, const double *__restrict__ hi,
-          const double *__restrict__ gpart, const double *__restrict__ spart, MpState *__restrict__ st,
-          double *__restrict__ F_hist, double *__restrict__ delta_hist, const double *__restrict__ F_unreached)
-{
-    if (st->reason != 0) return;
-    __shared__ double red_s[MP_STEP_WARPS + 1];
-    __shared__ int s_flag;
-    const int it = st->it;
-    if (PHASE != 1) {
-        // ---- g_A = sum of the CTA partials (fixed order), subspace rule Eq. (9)/(10) with the sign of C15
-        int nonzero = 0;
-        double dy_max = 0.0;
-        // one warp per aperture: lane l adds partials l, l+32, ... in that order, then a fixed shuffle tree
-        for (int k = threadIdx.x >> 5; k < m; k += MP_STEP_WARPS) {
-            const double *col = gpart + (size_t)k * n_cta;
+        {
+            const double tot = mp_block_sum(ssum, red_s);
+            if (tid == 0) a.spart[2 * blockIdx.x] = tot;
+        }
+        // the accumulators zeroed what the z phase relies on to be zero beyond a row's bytes: restore, then hand
+        // the ring back to the async proxy
+        __syncthreads();
+        for (int t = tid; t < MP_WARPS * COLS / 2; t += MP_THREADS) ((float4 *)mp_dyn)[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+        mp_fence_async_proxy();
+        grid.sync();
+        // ---- g_A = sum of the CTA partials (one warp per aperture, fixed order), subspace rule Eq. (9)/(10), C15
+        for (int k = blockIdx.x * MP_WARPS + warp; k < m; k += n_cta * MP_WARPS) {
+            const double *col = a.gpart + (size_t)k * n_cta;
             double s = 0.0;
-            for (int c0 = threadIdx.x & 31; c0 < n_cta; c0 += 32 * 16) {        // 16 loads in flight, added in the same order
-                double v[16];
-#pragma unroll
-                for (int u = 0; u < 16; ++u) v[u] = c0 + 32 * u < n_cta ? col[c0 + 32 * u] : 0.0;
-#pragma unroll
-                for (int u = 0; u < 16; ++u)
-                    if (c0 + 32 * u < n_cta) s += v[u];
-            }
+            for (int c0 = lane; c0 < n_cta; c0 += 32) s += __ldcg(col + c0);
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) s += shfl_xor_d(s, o);
-            const double yk = y[k];
-            if ((yk <= lo[k] && s > 0.0) || (yk >= hi[k] && s < 0.0)) s = 0.0;
-            if ((threadIdx.x & 31) == 0) g[k] = s;
-            nonzero |= s != 0.0;
-            if (it >= 1) dy_max = fmax(dy_max, fabs(yk - y_prev[k]));
+            const double yk = sy[k];
+            if ((yk <= a.lo[k] && s > 0.0) || (yk >= a.hi[k] && s < 0.0)) s = 0.0;
+            if (lane == 0) a.gsum[k] = s;
         }
-        double fs = 0.0;
-        for (int c = threadIdx.x; c < n_cta; c += MP_STEP_THREADS) fs += spart[2 * c];
-        const double F = mp_block_sum<MP_STEP_WARPS>(fs, red_s) + F_unreached[0];
-        if (threadIdx.x == 0) s_flag = 0;
+        {                                                         // F: every CTA, same order
+            double fs = 0.0;
+            for (int c = tid; c < n_cta; c += MP_THREADS) fs += __ldcg(a.spart + 2 * c);
+            F = mp_block_sum(fs, red_s) + a.F_unreached[0];
+        }
+        grid.sync();
+        // ---- every CTA: stopping rules (C19), tested at the top of the iteration
+        int nonzero = 0;
+        double dy_max = 0.0;
+        for (int k = tid; k < m; k += MP_THREADS) {
+            const double gk = __ldcg(a.gsum + k);
+            sg[k] = gk;
+            nonzero |= gk != 0.0;
+            if (it >= 1) dy_max = fmax(dy_max, fabs(sy[k] - syp[k]));
+        }
+        if (tid == 0) s_flag = 0;
         __syncthreads();
         if (nonzero) atomicOr(&s_flag, 1);
-        // max over the block of dy_max (exact, order-free)
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) dy_max = fmax(dy_max, shfl_xor_d(dy_max, o));
-        __shared__ double red_m[MP_STEP_WARPS];
-        if ((threadIdx.x & 31) == 0) red_m[threadIdx.x >> 5] = dy_max;
+        for (int o = 16; o > 0; o >>= 1) dy_max = fmax(dy_max, shfl_xor_d(dy_max, o));   // max: exact, order-free
         __syncthreads();
-        if (threadIdx.x == 0) {
-            for (int i = 0; i < MP_STEP_WARPS; ++i) dy_max = fmax(dy_max, red_m[i]);
-            for (int j = MP_HIST - 1; j > 0; --j) st->Fh[j] = st->Fh[j - 1];
-            st->Fh[0] = F;
-            st->F = F;
-            F_hist[it] = F;
-            // ---- stopping rules, in the order of C19
-            int reason = 0;
-            if (!s_flag) reason = 1;
+        if (lane == 0) red_s[warp] = dy_max;
+        __syncthreads();
+        if (tid == 0) {
+            for (int i = 0; i < MP_WARPS; ++i) dy_max = fmax(dy_max, red_s[i]);
+            for (int j = MP_HIST - 1; j > 0; --j) sFh[j] = sFh[j - 1];
+            sFh[0] = F;
+            int r = 0;
+            if (!s_flag) r = 1;
             else {
                 bool flat = it >= 5;
-                for (int j = 0; flat && j < 5; ++j)
-                    flat = fabs(st->Fh[j] - st->Fh[j + 1]) <= st->eps_F * fabs(st->Fh[j + 1]);
-                if (flat) reason = 2;
-                else if (it >= 1 && dy_max <= st->eps_y) reason = 3;
-                else if (it >= st->max_iter) reason = 4;
+                for (int j = 0; flat && j < 5; ++j) flat = fabs(sFh[j] - sFh[j + 1]) <= a.eps_F * fabs(sFh[j + 1]);
+                if (flat) r = 2;
+                else if (it >= 1 && dy_max <= a.eps_y) r = 3;
+                else if (it >= a.max_iter) r = 4;
             }
-            st->reason = reason;
-            s_flag = reason;
+            s_flag = r;
+            if (blockIdx.x == 0) a.F_hist[it] = F;
         }
         __syncthreads();
-        if (s_flag != 0 || PHASE == 0) return;           // (the barrier above also publishes g to the whole CTA)
-    }
-    // ---- step size
-    double delta;
-    if (PHASE == 1) {
-        double cs = 0.0, gg = 0.0;
-        for (int c = threadIdx.x; c < n_cta; c += MP_STEP_THREADS) cs += spart[2 * c + 1];
-        for (int k = threadIdx.x; k < m; k += MP_STEP_THREADS) gg += g[k] * g[k];
-        const double den = 2.0 * mp_block_sum<MP_STEP_WARPS>(cs, red_s);
-        const double num = mp_block_sum<MP_STEP_WARPS>(gg, red_s);
-        delta = den > 0.0 ? num / den : 1.0;                                             // C17
-    } else {
-        double ss = 0.0, sv = 0.0, tt = 0.0;
-        for (int k = threadIdx.x; k < m; k += MP_STEP_THREADS) {
-            const double s = y[k] - y_prev[k], t = g[k] - g_prev[k];
-            ss += s * s; sv += s * t; tt += t * t;
+        reason = s_flag;
+        __syncthreads();
+        if (reason != 0) break;
+        // ---- step 2: the step size
+        if (it == 0) {                                            // C17: one more pass, q = DA g_A
+            double csum = 0.0;
+            mp_pass<V, true>(a, ring_w, bar_w, gzs[warp], pp, sy, sg, sT, sWo, sWu, acc, csum);
+            const double tot = mp_block_sum(csum, red_s);
+            if (tid == 0) a.spart[2 * blockIdx.x + 1] = tot;
+            grid.sync();
+            double cs = 0.0, gg = 0.0;
+            for (int c = tid; c < n_cta; c += MP_THREADS) cs += __ldcg(a.spart + 2 * c + 1);
+            for (int k = tid; k < m; k += MP_THREADS) gg += sg[k] * sg[k];
+            const double den = 2.0 * mp_block_sum(cs, red_s);
+            const double num = mp_block_sum(gg, red_s);
+            delta = den > 0.0 ? num / den : 1.0;
+        } else {                                                  // Eq. (7) odd iterations, Eq. (8) even ones (C18)
+            double ss = 0.0, sv = 0.0, tt = 0.0;
+            for (int k = tid; k < m; k += MP_THREADS) {
+                const double s = sy[k] - syp[k], t = sg[k] - sgp[k];
+                ss += s * s; sv += s * t; tt += t * t;
+            }
+            ss = mp_block_sum(ss, red_s);
+            sv = mp_block_sum(sv, red_s);
+            tt = mp_block_sum(tt, red_s);
+            if (sv > 0.0 && tt > 0.0) delta = (it & 1) ? ss / sv : sv / tt;   // else: the previous delta is kept
         }
-        ss = mp_block_sum<MP_STEP_WARPS>(ss, red_s);
-        sv = mp_block_sum<MP_STEP_WARPS>(sv, red_s);
-        tt = mp_block_sum<MP_STEP_WARPS>(tt, red_s);
-        delta = st->delta;                                                               // kept when <s,t> <= 0 (C18)
-        if (sv > 0.0 && tt > 0.0) delta = (it & 1) ? ss / sv : sv / tt;                  // Eq. (7) odd, Eq. (8) even
+        // ---- step 3: update within the box (C16)
+        for (int k = tid; k < m; k += MP_THREADS) {
+            const double yk = sy[k], gk = sg[k];
+            syp[k] = yk;
+            sgp[k] = gk;
+            sy[k] = fmin(fmax(yk - delta * gk, a.lo[k]), a.hi[k]);
+        }
+        if (blockIdx.x == 0 && tid == 0) a.delta_hist[it] = delta;
+        ++it;
+        __syncthreads();
     }
-    // ---- update within the box (step 3; C16)
-    for (int k = threadIdx.x; k < m; k += MP_STEP_THREADS) {
-        const double yk = y[k], gk = g[k];
-        y_prev[k] = yk;
-        g_prev[k] = gk;
-        y[k] = fmin(fmax(yk - delta * gk, lo[k]), hi[k]);
-    }
-    if (threadIdx.x == 0) {
-        st->delta = delta;
-        delta_hist[it] = delta;
-        st->it = it + 1;
+    if (blockIdx.x == 0) {                                        // the iterate at which the rule fired
+        for (int k = tid; k < m; k += MP_THREADS) { a.y[k] = sy[k]; a.g[k] = sg[k]; }
+        if (tid == 0) { a.st->it = it; a.st->reason = reason; a.st->delta = delta; a.st->F = F; }
     }
 }
 
 // ---------------------------------------------------------------- host side
-static void mp_set_smem_attributes()
+template <int V>
+static cudaError_t mp_launch_solve_v(const vmat_mp *h, const MpArgs &a, cudaStream_t s)
 {
-#define MP_ATTR(CURV, LOG, NC) \
-    cudaFuncSetAttribute(k_mp_pass<CURV, LOG, NC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mp_ring_bytes(NC))
-    MP_ATTR(false, 3, 1); MP_ATTR(false, 4, 1); MP_ATTR(false, 5, 1); MP_ATTR(false, 5, 2); MP_ATTR(false, 5, 3);
-    MP_ATTR(true, 3, 1); MP_ATTR(true, 4, 1); MP_ATTR(true, 5, 1); MP_ATTR(true, 5, 2); MP_ATTR(true, 5, 3);
-#undef MP_ATTR
+    void *args[] = {(void *)&a};
+    return cudaLaunchCooperativeKernel((const void *)k_mp_solve<V>, dim3(h->n_cta), dim3(MP_THREADS), args, mp_smem_bytes<V>(), s);
 }
-
-template <bool CURV>
-static void mp_launch_pass(const vmat_mp *h, const uint8_t *vs, int n_struct, const float *T, const float *wo,
-                           const float *wu, float *z, cudaStream_t s)
+static cudaError_t mp_launch_solve(const vmat_mp *h, const MpArgs &a, cudaStream_t s)
 {
-#define MP_PASS(LOG, NC)                                                                                            \
-    k_mp_pass<CURV, LOG, NC><<<h->n_cta, MP_THREADS, mp_ring_bytes(NC), s>>>(h->n_active, h->active, h->m, h->m_cap, h->DA, h->y, h->g, vs,   \
-                                                             n_struct, T, wo, wu, z, h->gpart, h->spart, h->st)
-    const int m = h->m;                                      // lanes per row x 16-byte chunks per lane covering m columns
-    if (m <= 32) MP_PASS(3, 1);                              // (8 columns per lane up to m = 128 measured 6-13 % slower)
-    else if (m <= 64) MP_PASS(4, 1);
-    else if (m <= 128) MP_PASS(5, 1);
-    else if (m <= 256) MP_PASS(5, 2);
-    else MP_PASS(5, 3);
-#undef MP_PASS
+    switch (mp_variant(a.m)) {
+    case 0: return mp_launch_solve_v<0>(h, a, s);
+    case 1: return mp_launch_solve_v<1>(h, a, s);
+    case 2: return mp_launch_solve_v<2>(h, a, s);
+    case 3: return mp_launch_solve_v<3>(h, a, s);
+    default: return mp_launch_solve_v<4>(h, a, s);
+    }
 }
-
-template <int PHASE>
-static void mp_launch_step(const vmat_mp *h, cudaStream_t s)
+static int mp_rows_per_stage(int m)
 {
-    k_mp_step<PHASE><<<1, MP_STEP_THREADS, 0, s>>>(h->m, h->m_cap, h->n_cta, h->y, h->y_prev, h->g, h->g_prev, h->lo, h->hi,
-                                              h->gpart, h->spart, h->st, h->F_hist, h->delta_hist, h->F_unreached);
+    switch (mp_variant(m)) {
+    case 0: return MpCfg<0>::R;
+    case 1: return MpCfg<1>::R;
+    case 2: return MpCfg<2>::R;
+    case 3: return MpCfg<3>::R;
+    default: return MpCfg<4>::R;
+    }
+}
+// dynamic shared memory of every variant; true if one CTA of each fits an SM
+static bool mp_prepare_kernels()
+{
+    bool ok = true;
+#define MP_PREP(V)                                                                                                    \
+    {                                                                                                                 \
+        ok = ok && cudaFuncSetAttribute(k_mp_solve<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mp_smem_bytes<V>()) == cudaSuccess; \
+        int nb = 0;                                                                                                   \
+        ok = ok && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_mp_solve<V>, MP_THREADS, mp_smem_bytes<V>()) == cudaSuccess && nb >= 1; \
+    }
+    MP_PREP(0) MP_PREP(1) MP_PREP(2) MP_PREP(3) MP_PREP(4)
+#undef MP_PREP
+    return ok;
 }
 
 #define REQUIRE(cond, msg)                                            \
@@ -482,10 +541,12 @@ extern "C" {
 int vmat_mp_destroy(vmat_mp *h)
 {
     if (!h) return VMAT_OK;
-    void *ptrs[] = {h->DA, h->y, h->y_prev, h->g, h->g_prev, h->lo, h->hi, h->gpart, h->spart, h->st, h->F_hist,
-                    h->delta_hist, h->row_flag, h->active, h->n_active_dev, h->select_tmp, h->F_unreached};
+    void *ptrs[] = {h->DA, h->y, h->g, h->lo, h->hi, h->gpart, h->spart, h->gsum, h->st, h->F_hist,
+                    h->delta_hist, h->row_flag, h->active, h->n_active_dev, h->select_tmp, h->F_unreached, h->cg_scratch};
     for (void *p : ptrs)
         if (p) cudaFree(p);
+    if (h->stage3) cudaFreeHost(h->stage3);
+    if (h->stage3_free) cudaEventDestroy(h->stage3_free);
     delete h;
     return VMAT_OK;
 }
@@ -494,27 +555,35 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
 {
     REQUIRE(out != nullptr, "out is NULL");
     REQUIRE(n_voxels >= 0, "negative n_voxels");
-    REQUIRE(max_apertures >= 1 && max_apertures <= MP_MAX_NC * 32, "max_apertures must be in 1..384");
+    REQUIRE(max_apertures >= 1 && max_apertures <= MP_MAX_M, "max_apertures must be in 1..384");
     vmat_mp *h = new (std::nothrow) vmat_mp();
     if (!h) { vmat_set_error("vmat_mp_create: host allocation failed"); return VMAT_ERR_OOM; }
     h->n_voxels = n_voxels;
     h->m_cap = (max_apertures + 7) / 8 * 8;                  // rows start on 32-byte boundaries
     cudaGetDevice(&h->device);
-    int n_sm = 1;
+    int n_sm = 1, coop = 0;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, h->device);
-    mp_set_smem_attributes();
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, h->device);
+    if (!coop || !mp_prepare_kernels()) {
+        cudaGetLastError();
+        delete h;
+        vmat_set_error("vmat_mp_create: the device cannot hold one cooperative CTA of the solve kernel per SM");
+        return VMAT_ERR_CUDA;
+    }
     h->n_sm = n_sm;
-    h->n_cta = n_sm * VMAT_MP_CTAS_PER_SM;                                     // the most a pass uses (allocation)
+    h->n_cta = n_sm;                                          // one persistent CTA per SM
     cudaStream_t s = (cudaStream_t)stream;
     auto alloc = [&](void **p, size_t bytes) { return cudaMalloc(p, bytes > 0 ? bytes : 1) == cudaSuccess; };
     const size_t mc = (size_t)h->m_cap;
     bool ok = alloc((void **)&h->DA, (size_t)n_voxels * mc * 4) && alloc((void **)&h->y, mc * 8) &&
-              alloc((void **)&h->y_prev, mc * 8) && alloc((void **)&h->g, mc * 8) && alloc((void **)&h->g_prev, mc * 8) &&
+              alloc((void **)&h->g, mc * 8) && alloc((void **)&h->gsum, mc * 8) &&
               alloc((void **)&h->lo, mc * 8) && alloc((void **)&h->hi, mc * 8) &&
               alloc((void **)&h->gpart, (size_t)h->n_cta * mc * 8) && alloc((void **)&h->spart, (size_t)h->n_cta * 16) &&
               alloc((void **)&h->st, sizeof(MpState)) && alloc((void **)&h->row_flag, (size_t)n_voxels) &&
               alloc((void **)&h->active, (size_t)n_voxels * 4) && alloc((void **)&h->n_active_dev, 4) &&
-              alloc((void **)&h->F_unreached, 8);
+              alloc((void **)&h->F_unreached, 8) &&
+              cudaMallocHost((void **)&h->stage3, 3 * sizeof(double)) == cudaSuccess &&
+              cudaEventCreateWithFlags(&h->stage3_free, cudaEventDisableTiming) == cudaSuccess;
     if (ok) {
         cub::DeviceSelect::Flagged(nullptr, h->select_tmp_bytes, thrust::counting_iterator<int32_t>(0), h->row_flag, h->active,
                                    h->n_active_dev, n_voxels, s);
@@ -530,7 +599,7 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
     cudaMemsetAsync(h->row_flag, 0, (size_t)(n_voxels > 0 ? n_voxels : 1), s);
     cudaMemsetAsync(h->y, 0, mc * 8, s);
     cudaMemsetAsync(h->spart, 0, (size_t)h->n_cta * 16, s);
-    h->n_cta = 0;                                                              // set per solve
+    cudaEventRecord(h->stage3_free, s);
     VMAT_CUDA(cudaStreamSynchronize(s));
     *out = h;
     return VMAT_OK;
@@ -545,13 +614,10 @@ static int mp_forget(vmat_mp *h, cudaStream_t s)
     return VMAT_OK;
 }
 
-int vmat_mp_reset(vmat_mp *h)
+int vmat_mp_reset(vmat_mp *h, void *stream)
 {
     REQUIRE(h != nullptr, "handle is NULL");
-    VMAT_CUDA(cudaDeviceSynchronize());                      // no stream argument: order against everything
-    int rc = mp_forget(h, nullptr);
-    if (rc == VMAT_OK) VMAT_CUDA(cudaDeviceSynchronize());
-    return rc;
+    return mp_forget(h, (cudaStream_t)stream);               // ordered on the caller's stream like every other call
 }
 
 int vmat_mp_add_aperture(vmat_mp *h, const float *DA, double y0, double y_lo, double y_hi, void *stream)
@@ -568,11 +634,16 @@ int vmat_mp_add_aperture(vmat_mp *h, const float *DA, double y0, double y_lo, do
         h->active_valid = false;
         VMAT_LAUNCH_CHECK();
     }
-    const double v[3] = {y0 < y_lo ? y_lo : (y0 > y_hi ? y_hi : y0), y_lo, y_hi};
-    VMAT_CUDA(cudaMemcpyAsync(h->y + k, &v[0], 8, cudaMemcpyHostToDevice, s));
-    VMAT_CUDA(cudaMemcpyAsync(h->lo + k, &v[1], 8, cudaMemcpyHostToDevice, s));
-    VMAT_CUDA(cudaMemcpyAsync(h->hi + k, &v[2], 8, cudaMemcpyHostToDevice, s));
-    VMAT_CUDA(cudaStreamSynchronize(s));                     // v lives on this stack frame
+    // y0 / lo / hi through the handle's pinned staging buffer: wait (normally not at all) until the copies of the
+    // previous aperture have read it, no synchronisation with the stream otherwise
+    VMAT_CUDA(cudaEventSynchronize(h->stage3_free));
+    h->stage3[0] = y0 < y_lo ? y_lo : (y0 > y_hi ? y_hi : y0);
+    h->stage3[1] = y_lo;
+    h->stage3[2] = y_hi;
+    VMAT_CUDA(cudaMemcpyAsync(h->y + k, h->stage3 + 0, 8, cudaMemcpyHostToDevice, s));
+    VMAT_CUDA(cudaMemcpyAsync(h->lo + k, h->stage3 + 1, 8, cudaMemcpyHostToDevice, s));
+    VMAT_CUDA(cudaMemcpyAsync(h->hi + k, h->stage3 + 2, 8, cudaMemcpyHostToDevice, s));
+    VMAT_CUDA(cudaEventRecord(h->stage3_free, s));
     h->m = k + 1;
     return VMAT_OK;
 }
@@ -599,8 +670,6 @@ int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, con
     REQUIRE(eps_F >= 0.0 && eps_y >= 0.0, "negative tolerance");
     cudaStream_t s = (cudaStream_t)stream;
     g_vmat_launches = 0;
-    // resident CTAs per SM of the pass kernel that m selects; fixed by m, so every summation order is fixed by m
-    h->n_cta = h->n_sm * (h->m <= 256 ? 3 : 2);
     // the voxels some aperture reaches, ascending; F of the others (their dose is 0 whatever y)
     if (!h->active_valid) {
         h->n_active = 0;
@@ -622,34 +691,25 @@ int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, con
         if (h->delta_hist) cudaFree(h->delta_hist);
         h->F_hist = h->delta_hist = nullptr;
         h->hist_cap = 0;
-        VMAT_CUDA(cudaMalloc((void **)&h->F_hist, ((size_t)max_iter + 1) * 8));
-        VMAT_CUDA(cudaMalloc((void **)&h->delta_hist, ((size_t)max_iter + 1) * 8));
-        h->hist_cap = max_iter + 1;
+        const size_t cap = (size_t)max_iter + 1 < 4096 ? 4096 : (size_t)max_iter + 1;
+        VMAT_CUDA(cudaMalloc((void **)&h->F_hist, cap * 8));
+        VMAT_CUDA(cudaMalloc((void **)&h->delta_hist, cap * 8));
+        h->hist_cap = (int32_t)cap;
     }
-    MpState init = {};
-    init.max_iter = max_iter; init.eps_F = eps_F; init.eps_y = eps_y;
-    VMAT_CUDA(cudaMemcpyAsync(h->st, &init, sizeof(init), cudaMemcpyHostToDevice, s));
-    k_mp_clip<<<(h->m + 127) / 128, 128, 0, s>>>(h->m, h->y, h->lo, h->hi);          // the start must be feasible (C16)
+    // the whole BB iteration in one cooperative launch; the start is clipped into the box inside (C16)
+    MpArgs a;
+    a.n = h->n_active; a.active = h->active; a.m = h->m; a.m_cap = h->m_cap; a.DA = h->DA; a.y = h->y; a.g = h->g;
+    a.lo = h->lo; a.hi = h->hi; a.vstruct = voxel_struct; a.n_struct = n_struct; a.T = T; a.w_over = w_over;
+    a.w_under = w_under; a.z_out = z; a.gpart = h->gpart; a.spart = h->spart; a.gsum = h->gsum; a.st = h->st;
+    a.F_hist = h->F_hist; a.delta_hist = h->delta_hist; a.F_unreached = h->F_unreached; a.max_iter = max_iter;
+    a.eps_F = eps_F; a.eps_y = eps_y;
+    VMAT_CUDA(mp_launch_solve(h, a, s));
     VMAT_LAUNCH_CHECK();
-    // iteration 0: gradient pass, step A, curvature pass, step B
-    mp_launch_pass<false>(h, voxel_struct, n_struct, T, w_over, w_under, z, s); VMAT_LAUNCH_CHECK();
-    mp_launch_step<0>(h, s); VMAT_LAUNCH_CHECK();
-    mp_launch_pass<true>(h, voxel_struct, n_struct, T, w_over, w_under, nullptr, s); VMAT_LAUNCH_CHECK();
-    mp_launch_step<1>(h, s); VMAT_LAUNCH_CHECK();
     MpState cur;
-    const int BATCH = 8;                                     // iterations enqueued between two looks at the stop flag
-    for (;;) {
-        VMAT_CUDA(cudaMemcpyAsync(&cur, h->st, sizeof(cur), cudaMemcpyDeviceToHost, s));
-        VMAT_CUDA(cudaStreamSynchronize(s));
-        if (cur.reason != 0) break;
-        for (int b = 0; b < BATCH; ++b) {                    // kernels after the stop are no-ops (they read the flag)
-            mp_launch_pass<false>(h, voxel_struct, n_struct, T, w_over, w_under, z, s); VMAT_LAUNCH_CHECK();
-            mp_launch_step<2>(h, s); VMAT_LAUNCH_CHECK();
-        }
-    }
-    h->last_n_iter = cur.it;
+    VMAT_CUDA(cudaMemcpyAsync(&cur, h->st, sizeof(cur), cudaMemcpyDeviceToHost, s));
     if (y_host) VMAT_CUDA(cudaMemcpyAsync(y_host, h->y, (size_t)h->m * 8, cudaMemcpyDeviceToHost, s));
     VMAT_CUDA(cudaStreamSynchronize(s));
+    h->last_n_iter = cur.it;
     if (F_host) *F_host = cur.F;
     if (n_iter_host) *n_iter_host = cur.it;
     if (reason_host) *reason_host = cur.reason;
@@ -703,22 +763,33 @@ int vmat_column_generation_ex(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_str
     cudaStream_t s = (cudaStream_t)stream;
     const size_t nv = (size_t)(h->n_voxels > 0 ? h->n_voxels : 1), nb = (size_t)(h->n_beamlets > 0 ? h->n_beamlets : 1);
     const size_t nr = (size_t)(h->n_leaf_rows > 0 ? h->n_leaf_rows : 1), na = (size_t)(h->n_angles > 0 ? h->n_angles : 1);
-    // scratch of the pricing step, freed on every exit path
+    // scratch of the pricing step: one allocation owned by the master-problem handle, kept between calls
     struct Scratch {
-        float *g = nullptr, *p = nullptr, *xs = nullptr, *DA = nullptr;
-        int32_t *Lw = nullptr, *Rw = nullptr, *best = nullptr, *win = nullptr;
-        double *row_price = nullptr, *angle_price = nullptr, *F = nullptr;
-        uint8_t *mask = nullptr;
-        ~Scratch() { for (void *q : {(void *)g, (void *)p, (void *)xs, (void *)DA, (void *)Lw, (void *)Rw, (void *)best, (void *)win,
-                                     (void *)row_price, (void *)angle_price, (void *)F, (void *)mask}) if (q) cudaFree(q); }
+        float *g, *p, *xs, *DA;
+        int32_t *Lw, *Rw, *best, *win;
+        double *row_price, *angle_price, *F;
+        uint8_t *mask;
     } w;
-    VMAT_CUDA(cudaMalloc((void **)&w.g, nv * 4)); VMAT_CUDA(cudaMalloc((void **)&w.DA, nv * 4));
-    VMAT_CUDA(cudaMalloc((void **)&w.p, nb * 4)); VMAT_CUDA(cudaMalloc((void **)&w.xs, nb * 4));
-    VMAT_CUDA(cudaMalloc((void **)&w.Lw, nr * 4)); VMAT_CUDA(cudaMalloc((void **)&w.Rw, nr * 4));
-    VMAT_CUDA(cudaMalloc((void **)&w.row_price, nr * 8)); VMAT_CUDA(cudaMalloc((void **)&w.angle_price, na * 8));
-    VMAT_CUDA(cudaMalloc((void **)&w.best, 4)); VMAT_CUDA(cudaMalloc((void **)&w.F, 8));
-    VMAT_CUDA(cudaMalloc((void **)&w.mask, na));
-    if (max_leaf_travel >= 0) VMAT_CUDA(cudaMalloc((void **)&w.win, nr * 16));              // L_lo, L_hi, R_lo, R_hi
+    {
+        auto up = [](size_t b) { return (b + 255) / 256 * 256; };
+        const size_t need = 2 * up(nv * 4) + 2 * up(nb * 4) + 2 * up(nr * 4) + up(nr * 8) + up(na * 8) + up(4) + up(8) +
+                            up(na) + up(nr * 16);
+        if (need > mp->cg_scratch_bytes) {
+            if (mp->cg_scratch) { VMAT_CUDA(cudaStreamSynchronize(s)); cudaFree(mp->cg_scratch); }
+            mp->cg_scratch = nullptr; mp->cg_scratch_bytes = 0;
+            VMAT_CUDA(cudaMalloc(&mp->cg_scratch, need));
+            mp->cg_scratch_bytes = need;
+        }
+        char *q = (char *)mp->cg_scratch;
+        auto take = [&](size_t b) { char *r = q; q += up(b); return (void *)r; };
+        w.g = (float *)take(nv * 4); w.DA = (float *)take(nv * 4);
+        w.p = (float *)take(nb * 4); w.xs = (float *)take(nb * 4);
+        w.Lw = (int32_t *)take(nr * 4); w.Rw = (int32_t *)take(nr * 4);
+        w.row_price = (double *)take(nr * 8); w.angle_price = (double *)take(na * 8);
+        w.best = (int32_t *)take(4); w.F = (double *)take(8);
+        w.mask = (uint8_t *)take(na);
+        w.win = (int32_t *)take(nr * 16);                                                // L_lo, L_hi, R_lo, R_hi
+    }
     VMAT_CUDA(cudaMemsetAsync(w.mask, 0, na, s));
     VMAT_CUDA(cudaMemsetAsync(z, 0, nv * 4, s));                                         // L56: start with z = 0 ...
     if (h->n_leaf_rows > 0) {
@@ -803,11 +874,8 @@ int vmat_mp_pass_geometry(const vmat_mp *h, int32_t m, int32_t *n_cta, int32_t *
 {
     REQUIRE(h != nullptr, "handle is NULL");
     REQUIRE(m >= 1 && m <= h->m_cap, "m must be in 1..max_apertures");
-    // mirrors mp_launch_pass: lanes per row 2^LOG, 16-byte chunks per lane NC, rows per lane group and step 2^RBL
-    const int LOG = m <= 32 ? 3 : (m <= 64 ? 4 : 5), NC = m <= 128 ? 1 : (m <= 256 ? 2 : 3);
-    const int cta = h->n_sm * (m <= 256 ? 3 : 2);
-    if (n_cta) *n_cta = cta;
-    if (rows_per_grid_step) *rows_per_grid_step = cta * MP_WARPS * ((1 << mp_rbl(NC)) * (32 >> LOG));
+    if (n_cta) *n_cta = h->n_cta;
+    if (rows_per_grid_step) *rows_per_grid_step = h->n_cta * MP_WARPS * mp_rows_per_stage(m);
     return VMAT_OK;
 }
 
