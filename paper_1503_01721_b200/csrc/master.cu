@@ -52,6 +52,8 @@ struct vmat_mp {
     int32_t n_active = 0;
     bool active_valid = false;
     double *F_unreached = nullptr;            // [1] F of the other voxels (z = 0), per solve
+    uint8_t *sidc = nullptr;                  // [n_voxels] structure ids of the reached voxels, in reached order
+    float *zc = nullptr;                      // [n_voxels] their doses, in reached order
     double *stage3 = nullptr;                 // pinned host [3]: y0, lo, hi of the aperture being added
     cudaEvent_t stage3_free = nullptr;        // recorded after the copies that read stage3
     // scratch of the column-generation loop (allocated on first use, sized by the DDC handle it ran with)
@@ -137,35 +139,36 @@ k_mp_unreached_F(int n_voxels, const uint8_t *__restrict__ row_flag, const uint8
 // ~29 warp instructions per 512 bytes of DA instead of 64 (ncu: profiles/r2_*_mp.md).
 // All sums are FP64 in a fixed order given (m, SM count): deterministic.
 template <int V> struct MpCfg;
-//                                    bytes of a row at most | z phase: lanes per row, chunks per lane | rows per stage |
-//                                    g phase: lanes per row, chunks per lane | row padding (bank spread) | stages
-template <> struct MpCfg<0> { static constexpr int VB = 128,  LZ = 2,  CZ = 4, R = 16, LPR = 8,  NC = 1, PAD = 32, STAGES = 4; };
-template <> struct MpCfg<1> { static constexpr int VB = 256,  LZ = 4,  CZ = 4, R = 8,  LPR = 16, NC = 1, PAD = 64, STAGES = 4; };
-template <> struct MpCfg<2> { static constexpr int VB = 512,  LZ = 8,  CZ = 4, R = 8,  LPR = 32, NC = 1, PAD = 0,  STAGES = 3; };
-template <> struct MpCfg<3> { static constexpr int VB = 1024, LZ = 16, CZ = 4, R = 4,  LPR = 32, NC = 2, PAD = 0,  STAGES = 3; };
-template <> struct MpCfg<4> { static constexpr int VB = 1536, LZ = 32, CZ = 3, R = 2,  LPR = 32, NC = 3, PAD = 0,  STAGES = 4; };
+//                                    bytes of a row at most | lanes per row, 16-byte chunks per lane | rows per stage |
+//                                    row padding (bank spread) | stages
+template <> struct MpCfg<0> { static constexpr int VB = 128,  LZ = 2,  CZ = 4, R = 16, PAD = 32, STAGES = 4; };
+template <> struct MpCfg<1> { static constexpr int VB = 256,  LZ = 4,  CZ = 4, R = 8,  PAD = 64, STAGES = 4; };
+template <> struct MpCfg<2> { static constexpr int VB = 512,  LZ = 8,  CZ = 4, R = 8,  PAD = 0,  STAGES = 3; };
+template <> struct MpCfg<3> { static constexpr int VB = 1024, LZ = 16, CZ = 4, R = 4,  PAD = 0,  STAGES = 3; };
+template <> struct MpCfg<4> { static constexpr int VB = 1536, LZ = 32, CZ = 3, R = 2,  PAD = 0,  STAGES = 4; };
 static inline int mp_variant(int m) { return m <= 32 ? 0 : (m <= 64 ? 1 : (m <= 128 ? 2 : (m <= 256 ? 3 : 4))); }
 template <int V> __host__ __device__ constexpr size_t mp_ring_bytes()
 {
     return (size_t)MP_WARPS * MpCfg<V>::STAGES * MpCfg<V>::R * (MpCfg<V>::VB + MpCfg<V>::PAD);
 }
-template <int V> __host__ __device__ constexpr size_t mp_smem_bytes()      // ring (>= the 16 x 384 FP64 accumulators that reuse it) + barriers
+template <int V> __host__ __device__ constexpr size_t mp_accs_bytes() { return (size_t)MP_WARPS * (MpCfg<V>::VB / 4) * 8; }
+template <int V> __host__ __device__ constexpr size_t mp_ring_alloc()   // the FP64 accumulators of a CTA reuse the ring
 {
-    return (mp_ring_bytes<V>() > (size_t)MP_WARPS * MP_MAX_M * 8 ? mp_ring_bytes<V>() : (size_t)MP_WARPS * MP_MAX_M * 8) +
-           (size_t)MP_WARPS * MpCfg<V>::STAGES * 8;
+    return mp_ring_bytes<V>() > mp_accs_bytes<V>() ? mp_ring_bytes<V>() : mp_accs_bytes<V>();
 }
+template <int V> __host__ __device__ constexpr size_t mp_smem_bytes() { return mp_ring_alloc<V>() + (size_t)MP_WARPS * MpCfg<V>::STAGES * 8; }
 
 struct MpArgs {
     int n;                      // rows to visit: the reached voxels
-    const int32_t *active;      // their indices, ascending
+    const int32_t *active;      // their voxel indices, ascending
+    const uint8_t *sidc;        // [n] structure id of reached voxel pos
+    float *zc;                  // [n] dose of reached voxel pos (scattered into z by the caller afterwards)
     int m, m_cap;
     const float *DA;
-    double *y, *g;              // in: start (feasible); out: returned iterate and its g_A after the subspace rule
+    double *y, *g;              // in: start; out: returned iterate and its g_A after the subspace rule
     const double *lo, *hi;
-    const uint8_t *vstruct;
     int n_struct;
     const float *T, *w_over, *w_under;
-    float *z_out;               // or NULL
     double *gpart, *spart, *gsum;
     MpState *st;
     double *F_hist, *delta_hist;
@@ -192,12 +195,44 @@ __device__ __forceinline__ void mp_mbar_wait(uint32_t bar, uint32_t parity)
     } while (!done);
 }
 // 1-D bulk copy global -> shared (the TMA unit; SASS UBLKCP), completion in bytes on an mbarrier
-__device__ __forceinline__ void mp_bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+// L2 policy: DA is far larger than L2 and read once per pass -> evict_first, so that the small per-row tables
+// (evict_last) stay L2-resident from pass to pass; a table load that misses queues behind the whole bulk stream.
+__device__ __forceinline__ void mp_bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar, uint64_t pol)
 {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 :: "r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
+__device__ __forceinline__ uint64_t mp_policy_evict_first()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t mp_policy_evict_last()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ int mp_ld_keep_i32(const int32_t *p, uint64_t pol)
+{
+    int r;
+    asm volatile("ld.global.nc.L2::cache_hint.s32 %0, [%1], %2;" : "=r"(r) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ uint32_t mp_ld_keep_u8(const uint8_t *p, uint64_t pol)
+{
+    uint32_t r;
+    asm volatile("ld.global.nc.L2::cache_hint.u8 %0, [%1], %2;" : "=r"(r) : "l"(p), "l"(pol));
+    return r;
 }
 __device__ __forceinline__ void mp_fence_async_proxy() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ float4 mp_lds128(uint32_t addr)
+{
+    float4 e;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(e.x), "=f"(e.y), "=f"(e.z), "=f"(e.w) : "r"(addr));
+    return e;
+}
 
 // per-warp pipeline bookkeeping that lives across the passes of a solve
 struct MpPipe {
@@ -207,118 +242,116 @@ struct MpPipe {
 
 // One pass over the reached rows.  CURV = false: z = DA y, F, dF/dz, g_A partials (acc).  CURV = true: z = DA y,
 // q = DA v, sum_i w_i q_i^2 (C17).  ssum: this thread's part of F (or of the curvature).
+// sT2: per structure {T, 2 w_over, 2 w_under} in FP64.
 template <int V, bool CURV>
-__device__ __forceinline__ void mp_pass(const MpArgs &a, uint32_t ring_w, uint32_t bar_w, double *gzs_w, MpPipe &pp,
-                                        const double *sy, const double *sv, const float *sT, const float *sWo,
-                                        const float *sWu, double (&acc)[MpCfg<V>::NC][4], double &ssum)
+__device__ __forceinline__ void mp_pass(const MpArgs &a, uint32_t ring_w, uint32_t bar_w, MpPipe &pp, const double *sy,
+                                        const double *sv, const double *sT2, double (&acc)[MpCfg<V>::CZ][4], double &ssum)
 {
     using C = MpCfg<V>;
-    constexpr int LZ = C::LZ, CZ = C::CZ, R = C::R, LPR = C::LPR, NC = C::NC, STAGES = C::STAGES;
+    constexpr int LZ = C::LZ, CZ = C::CZ, R = C::R, STAGES = C::STAGES;
     constexpr int RS = C::VB + C::PAD, STAGE_BYTES = R * RS;
-    constexpr int RZ = 32 / LZ, NSUB = R / RZ, GPW = 32 / LPR, RG = R / GPW;
-    static_assert(R % RZ == 0 && R % GPW == 0 && NSUB >= 1 && NSUB <= LZ && LZ * CZ * 16 == C::VB && LPR * NC * 16 == C::VB, "mapping");
+    constexpr int RZ = 32 / LZ, NSUB = R / RZ;
+    static_assert(R % RZ == 0 && NSUB >= 1 && NSUB <= 4 && LZ * CZ * 16 == C::VB && R <= 32, "mapping");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int rz = lane / LZ, qz = lane % LZ, grp = lane / LPR, gl = lane % LPR;
+    const int rz = lane / LZ, qz = lane % LZ;
     const int n = a.n;
     const uint32_t W = (uint32_t)((a.m + 7) / 8) * 32u;           // bytes of a row that hold apertures (32-byte sectors)
     const int64_t step = (int64_t)gridDim.x * MP_WARPS * R;
     int64_t base = (int64_t)(blockIdx.x * MP_WARPS + warp) * R;
-    double yz[CZ][4];                                             // y of this lane's z-phase columns
+    double yz[CZ][4];                                             // y of this lane's columns
 #pragma unroll
     for (int j = 0; j < CZ; ++j)
 #pragma unroll
         for (int k = 0; k < 4; ++k) yz[j][k] = sy[(j * LZ + qz) * 4 + k];   // 0 beyond m
     int istage = pp.cstage;
     int64_t ibase = base;
+    // row of DA this lane will ask the TMA unit for at the next issue, loaded one step early: the load's latency
+    // (the voxel index goes straight into the copy's address) would otherwise stall the warp at every stage
+    const uint64_t pol_stream = mp_policy_evict_first(), pol_keep = mp_policy_evict_last();
+    int64_t nrow = (lane < R && ibase + lane < n) ? (int64_t)mp_ld_keep_i32(a.active + ibase + lane, pol_keep) : 0;
     auto issue = [&]() {                                          // R rows starting at reached position ibase
+        const int64_t row = nrow;
+        const int64_t nb = ibase + step;
+        nrow = (lane < R && nb + lane < n) ? (int64_t)mp_ld_keep_i32(a.active + nb + lane, pol_keep) : 0;
         if (ibase < n) {
             const int nvalid = (int)min((int64_t)R, (int64_t)n - ibase);
             const uint32_t bar = bar_w + 8u * istage;
             if (lane == 0) mp_mbar_expect_tx(bar, (uint32_t)nvalid * W);
             __syncwarp();
-            if (lane < nvalid) {
-                const int64_t row = __ldg(a.active + ibase + lane);
-                mp_bulk_g2s(ring_w + (uint32_t)(istage * STAGE_BYTES + lane * RS), a.DA + row * a.m_cap, W, bar);
-            }
+            if (lane < nvalid)
+                mp_bulk_g2s(ring_w + (uint32_t)(istage * STAGE_BYTES + lane * RS), a.DA + row * a.m_cap, W, bar, pol_stream);
         }
-        ibase += step;
+        ibase = nb;
         if (++istage == STAGES) istage = 0;
     };
 #pragma unroll 1
     for (int s = 0; s < STAGES - 1; ++s) issue();
+    // structure ids of this lane's rows of the stage after the current one (sub-step u: row u RZ + rz)
+    uint32_t sid_next = 0;
+    auto load_sids = [&](int64_t b) {
+        uint32_t r = 0;
+#pragma unroll
+        for (int u = 0; u < NSUB; ++u)
+            if (b + u * RZ + rz < n) r |= mp_ld_keep_u8(a.sidc + b + u * RZ + rz, pol_keep) << (8 * u);
+        return r;
+    };
+    sid_next = load_sids(base);
 #pragma unroll 1
     for (; base < n; base += step) {
         __syncwarp();                                             // every lane is done with the slot refilled now
         issue();
+        const uint32_t sids = sid_next;
+        sid_next = load_sids(base + step);
         const int cs = pp.cstage;
         mp_mbar_wait(bar_w + 8u * cs, (pp.phases >> cs) & 1u);
         pp.phases ^= 1u << cs;
         if (++pp.cstage == STAGES) pp.cstage = 0;
         const uint32_t stg = ring_w + (uint32_t)(cs * STAGE_BYTES);
-        // the row this lane finishes (objective, dF/dz): sub-step qz, row rz of it
-        const int rsel = qz * RZ + rz;
-        const bool fin = qz < NSUB;
-        const bool own = fin && base + rsel < n;
-        int vi = 0, sid = 0;
-        if (own) { vi = __ldg(a.active + base + rsel); sid = __ldg(a.vstruct + vi); }
-        // ---- z phase
-        double zmine = 0.0, qmine = 0.0;
 #pragma unroll
         for (int u = 0; u < NSUB; ++u) {
+            // ---- row u RZ + rz of the stage: this lane's CZ chunks, converted to FP64 once
             const uint32_t rowp = stg + (uint32_t)((u * RZ + rz) * RS + qz * 16);
+            double e[CZ][4];
             double z4[4] = {0.0, 0.0, 0.0, 0.0}, q4[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
             for (int j = 0; j < CZ; ++j) {
-                float4 e;
-                asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(e.x), "=f"(e.y), "=f"(e.z), "=f"(e.w)
-                             : "r"(rowp + (uint32_t)(j * LZ * 16)));
-                const double e0 = (double)e.x, e1 = (double)e.y, e2 = (double)e.z, e3 = (double)e.w;
-                z4[0] = fma(e0, yz[j][0], z4[0]); z4[1] = fma(e1, yz[j][1], z4[1]);
-                z4[2] = fma(e2, yz[j][2], z4[2]); z4[3] = fma(e3, yz[j][3], z4[3]);
+                const float4 f = mp_lds128(rowp + (uint32_t)(j * LZ * 16));
+                e[j][0] = (double)f.x; e[j][1] = (double)f.y; e[j][2] = (double)f.z; e[j][3] = (double)f.w;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) z4[k] = fma(e[j][k], yz[j][k], z4[k]);
                 if (CURV) {
                     const double *v = sv + (j * LZ + qz) * 4;
-                    q4[0] = fma(e0, v[0], q4[0]); q4[1] = fma(e1, v[1], q4[1]);
-                    q4[2] = fma(e2, v[2], q4[2]); q4[3] = fma(e3, v[3], q4[3]);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) q4[k] = fma(e[j][k], v[k], q4[k]);
                 }
             }
             double zs = (z4[0] + z4[1]) + (z4[2] + z4[3]), qs = (q4[0] + q4[1]) + (q4[2] + q4[3]);
 #pragma unroll
-            for (int o = LZ / 2; o > 0; o >>= 1) {
+            for (int o = LZ / 2; o > 0; o >>= 1) {                // every lane of the row ends with the row's sums
                 zs += shfl_xor_d(zs, o);
                 if (CURV) qs += shfl_xor_d(qs, o);
             }
-            if (qz == u) { zmine = zs; qmine = qs; }
-        }
-        // ---- objective and dF/dz of the finished rows (Eq. (1), sign C1)
-        double gz = 0.0;
-        if (own) {
-            const double Ti = (double)sT[sid], wo = (double)sWo[sid], wu = (double)sWu[sid];
-            if (!CURV) {
-                const double over = fmax(zmine - Ti, 0.0), under = fmax(Ti - zmine, 0.0);
-                gz = 2.0 * wo * over - 2.0 * wu * under;
-                ssum += wo * over * over + wu * under * under;
-                if (a.z_out) a.z_out[vi] = (float)zmine;
-            } else {
-                const double w = zmine > Ti ? wo : (zmine < Ti ? wu : 0.0);              // C17
-                ssum += w * qmine * qmine;
-            }
-        }
-        if (!CURV) {
-            if (fin) gzs_w[rsel] = gz;                            // rows past the end: 0
-            __syncwarp();
-            // ---- g phase: g_A += DA_i: * dF/dz_i
-#pragma unroll
-            for (int s = 0; s < RG; ++s) {
-                const int row = s * GPW + grp;
-                const double gs = gzs_w[row];
-#pragma unroll
-                for (int c = 0; c < NC; ++c) {
-                    float4 e;
-                    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(e.x), "=f"(e.y), "=f"(e.z), "=f"(e.w)
-                                 : "r"(stg + (uint32_t)(row * RS + (c * LPR + gl) * 16)));
-                    acc[c][0] = fma((double)e.x, gs, acc[c][0]); acc[c][1] = fma((double)e.y, gs, acc[c][1]);
-                    acc[c][2] = fma((double)e.z, gs, acc[c][2]); acc[c][3] = fma((double)e.w, gs, acc[c][3]);
+            // ---- the voxel's term of F and dF/dz (Eq. (1), sign C1): with u = z - T and w2 = 2 w_over (u > 0) or
+            //      2 w_under, dF/dz = w2 u and the term is w2 u^2 / 2
+            const int64_t pos = base + u * RZ + rz;
+            const bool live = pos < n;
+            const double *tp = sT2 + 3 * ((sids >> (8 * u)) & 0xffu);
+            const double du = zs - tp[0];
+            const double w2 = du > 0.0 ? tp[1] : tp[2];
+            double gz = 0.0;
+            if (live) {
+                if (!CURV) {
+                    gz = w2 * du;
+                    if (qz == 0) { ssum = fma(0.5 * gz, du, ssum); a.zc[pos] = (float)zs; }
+                } else if (qz == 0) {
+                    ssum = fma(du != 0.0 ? 0.5 * w2 : 0.0, qs * qs, ssum);   // C17
                 }
+            }
+            if (!CURV) {                                          // g_A += DA_i: * dF/dz_i, same lanes, same registers
+#pragma unroll
+                for (int j = 0; j < CZ; ++j)
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) acc[j][k] = fma(e[j][k], gz, acc[j][k]);
             }
         }
     }
@@ -329,21 +362,22 @@ __global__ void __launch_bounds__(MP_THREADS, 1)
 k_mp_solve(const MpArgs a)
 {
     using C = MpCfg<V>;
-    constexpr int LPR = C::LPR, NC = C::NC, STAGES = C::STAGES, COLS = C::VB / 4;
+    constexpr int LZ = C::LZ, CZ = C::CZ, STAGES = C::STAGES, COLS = C::VB / 4;
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     extern __shared__ __align__(128) unsigned char mp_dyn[];      // ring [warp][stage][row][RS]; then the barriers
     __shared__ double red_s[MP_WARPS + 1];
     __shared__ double sy[MP_MAX_M], syp[MP_MAX_M], sg[MP_MAX_M], sgp[MP_MAX_M];
-    __shared__ double gzs[MP_WARPS][32];
-    __shared__ float sT[256], sWo[256], sWu[256];
+    __shared__ double sT2[3 * 256];
     __shared__ double sFh[MP_HIST];
     __shared__ int s_flag;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, grp = lane / LPR, gl = lane % LPR;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, qz = lane % LZ;
     const int m = a.m, n_cta = gridDim.x;
-    constexpr size_t RING = mp_ring_bytes<V>() > (size_t)MP_WARPS * MP_MAX_M * 8 ? mp_ring_bytes<V>() : (size_t)MP_WARPS * MP_MAX_M * 8;
+    constexpr size_t RING = mp_ring_alloc<V>();
     uint64_t *bars = (uint64_t *)(mp_dyn + RING);
     for (int t = tid; t < (int)(RING / 16); t += MP_THREADS) ((float4 *)mp_dyn)[t] = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int t = tid; t < a.n_struct; t += MP_THREADS) { sT[t] = a.T[t]; sWo[t] = a.w_over[t]; sWu[t] = a.w_under[t]; }
+    for (int t = tid; t < a.n_struct; t += MP_THREADS) {
+        sT2[3 * t] = (double)a.T[t]; sT2[3 * t + 1] = 2.0 * (double)a.w_over[t]; sT2[3 * t + 2] = 2.0 * (double)a.w_under[t];
+    }
     for (int k = tid; k < MP_MAX_M; k += MP_THREADS) {
         sy[k] = k < m ? fmin(fmax(a.y[k], a.lo[k]), a.hi[k]) : 0.0;          // the start must be feasible (C16)
         syp[k] = 0.0; sg[k] = 0.0; sgp[k] = 0.0;
@@ -359,24 +393,24 @@ k_mp_solve(const MpArgs a)
     double delta = 0.0, F = 0.0;
     for (;;) {
         // ---- steps 4 + 1 of L139: the gradient pass
-        double acc[NC][4];
+        double acc[CZ][4];
 #pragma unroll
-        for (int c = 0; c < NC; ++c)
+        for (int j = 0; j < CZ; ++j)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) acc[c][j] = 0.0;
+            for (int k = 0; k < 4; ++k) acc[j][k] = 0.0;
         double ssum = 0.0;
-        mp_pass<V, false>(a, ring_w, bar_w, gzs[warp], pp, sy, sg, sT, sWo, sWu, acc, ssum);
-        // CTA partials in a fixed order: the lane groups of a warp, then the warps (in the ring's memory, idle now)
+        mp_pass<V, false>(a, ring_w, bar_w, pp, sy, sg, sT2, acc, ssum);
+        // CTA partials in a fixed order: the row groups of a warp, then the warps (in the ring's memory, idle now)
         __syncthreads();
         double *accs = (double *)mp_dyn;                          // [MP_WARPS][COLS]
 #pragma unroll
-        for (int c = 0; c < NC; ++c)
+        for (int j = 0; j < CZ; ++j)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                double v = acc[c][j];
+            for (int k = 0; k < 4; ++k) {
+                double v = acc[j][k];
 #pragma unroll
-                for (int o = LPR; o < 32; o <<= 1) v += shfl_xor_d(v, o);
-                if (grp == 0) accs[warp * COLS + (c * LPR + gl) * 4 + j] = v;
+                for (int o = LZ; o < 32; o <<= 1) v += shfl_xor_d(v, o);
+                if (lane < LZ) accs[warp * COLS + (j * LZ + qz) * 4 + k] = v;
             }
         __syncthreads();
         for (int k = tid; k < m; k += MP_THREADS) {
@@ -388,10 +422,10 @@ k_mp_solve(const MpArgs a)
             const double tot = mp_block_sum(ssum, red_s);
             if (tid == 0) a.spart[2 * blockIdx.x] = tot;
         }
-        // the accumulators zeroed what the z phase relies on to be zero beyond a row's bytes: restore, then hand
-        // the ring back to the async proxy
+        // the accumulators overwrote bytes the passes rely on to be zero (beyond a row's apertures): restore, then
+        // hand the ring back to the async proxy
         __syncthreads();
-        for (int t = tid; t < MP_WARPS * COLS / 2; t += MP_THREADS) ((float4 *)mp_dyn)[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int t = tid; t < (int)(mp_accs_bytes<V>() / 16); t += MP_THREADS) ((float4 *)mp_dyn)[t] = make_float4(0.f, 0.f, 0.f, 0.f);
         mp_fence_async_proxy();
         grid.sync();
         // ---- g_A = sum of the CTA partials (one warp per aperture, fixed order), subspace rule Eq. (9)/(10), C15
@@ -451,7 +485,7 @@ k_mp_solve(const MpArgs a)
         // ---- step 2: the step size
         if (it == 0) {                                            // C17: one more pass, q = DA g_A
             double csum = 0.0;
-            mp_pass<V, true>(a, ring_w, bar_w, gzs[warp], pp, sy, sg, sT, sWo, sWu, acc, csum);
+            mp_pass<V, true>(a, ring_w, bar_w, pp, sy, sg, sT2, acc, csum);
             const double tot = mp_block_sum(csum, red_s);
             if (tid == 0) a.spart[2 * blockIdx.x + 1] = tot;
             grid.sync();
@@ -462,15 +496,15 @@ k_mp_solve(const MpArgs a)
             const double num = mp_block_sum(gg, red_s);
             delta = den > 0.0 ? num / den : 1.0;
         } else {                                                  // Eq. (7) odd iterations, Eq. (8) even ones (C18)
-            double ss = 0.0, sv = 0.0, tt = 0.0;
+            double ss = 0.0, st = 0.0, tt = 0.0;
             for (int k = tid; k < m; k += MP_THREADS) {
                 const double s = sy[k] - syp[k], t = sg[k] - sgp[k];
-                ss += s * s; sv += s * t; tt += t * t;
+                ss += s * s; st += s * t; tt += t * t;
             }
             ss = mp_block_sum(ss, red_s);
-            sv = mp_block_sum(sv, red_s);
+            st = mp_block_sum(st, red_s);
             tt = mp_block_sum(tt, red_s);
-            if (sv > 0.0 && tt > 0.0) delta = (it & 1) ? ss / sv : sv / tt;   // else: the previous delta is kept
+            if (st > 0.0 && tt > 0.0) delta = (it & 1) ? ss / st : st / tt;   // else: the previous delta is kept
         }
         // ---- step 3: update within the box (C16)
         for (int k = tid; k < m; k += MP_THREADS) {
@@ -487,6 +521,20 @@ k_mp_solve(const MpArgs a)
         for (int k = tid; k < m; k += MP_THREADS) { a.y[k] = sy[k]; a.g[k] = sg[k]; }
         if (tid == 0) { a.st->it = it; a.st->reason = reason; a.st->delta = delta; a.st->F = F; }
     }
+}
+
+// structure ids of the reached voxels, in reached order (once per solve: the passes then need no indirection)
+__global__ void k_mp_gather_sid(int n, const int32_t *__restrict__ active, const uint8_t *__restrict__ vstruct,
+                                uint8_t *__restrict__ sidc)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) sidc[i] = vstruct[active[i]];
+}
+// z of the returned iterate: the reached voxels' doses back to their places (the others were zeroed)
+__global__ void k_mp_scatter_z(int n, const int32_t *__restrict__ active, const float *__restrict__ zc, float *__restrict__ z)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) z[active[i]] = zc[i];
 }
 
 // ---------------------------------------------------------------- host side
@@ -542,7 +590,8 @@ int vmat_mp_destroy(vmat_mp *h)
 {
     if (!h) return VMAT_OK;
     void *ptrs[] = {h->DA, h->y, h->g, h->lo, h->hi, h->gpart, h->spart, h->gsum, h->st, h->F_hist,
-                    h->delta_hist, h->row_flag, h->active, h->n_active_dev, h->select_tmp, h->F_unreached, h->cg_scratch};
+                    h->delta_hist, h->row_flag, h->active, h->n_active_dev, h->select_tmp, h->F_unreached, h->cg_scratch,
+                    h->sidc, h->zc};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     if (h->stage3) cudaFreeHost(h->stage3);
@@ -581,7 +630,8 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
               alloc((void **)&h->gpart, (size_t)h->n_cta * mc * 8) && alloc((void **)&h->spart, (size_t)h->n_cta * 16) &&
               alloc((void **)&h->st, sizeof(MpState)) && alloc((void **)&h->row_flag, (size_t)n_voxels) &&
               alloc((void **)&h->active, (size_t)n_voxels * 4) && alloc((void **)&h->n_active_dev, 4) &&
-              alloc((void **)&h->F_unreached, 8) &&
+              alloc((void **)&h->F_unreached, 8) && alloc((void **)&h->sidc, (size_t)n_voxels) &&
+              alloc((void **)&h->zc, (size_t)n_voxels * 4) &&
               cudaMallocHost((void **)&h->stage3, 3 * sizeof(double)) == cudaSuccess &&
               cudaEventCreateWithFlags(&h->stage3_free, cudaEventDisableTiming) == cudaSuccess;
     if (ok) {
@@ -697,14 +747,22 @@ int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, con
         h->hist_cap = (int32_t)cap;
     }
     // the whole BB iteration in one cooperative launch; the start is clipped into the box inside (C16)
+    if (h->n_active > 0) {
+        k_mp_gather_sid<<<(h->n_active + 255) / 256, 256, 0, s>>>(h->n_active, h->active, voxel_struct, h->sidc);
+        VMAT_LAUNCH_CHECK();
+    }
     MpArgs a;
-    a.n = h->n_active; a.active = h->active; a.m = h->m; a.m_cap = h->m_cap; a.DA = h->DA; a.y = h->y; a.g = h->g;
-    a.lo = h->lo; a.hi = h->hi; a.vstruct = voxel_struct; a.n_struct = n_struct; a.T = T; a.w_over = w_over;
-    a.w_under = w_under; a.z_out = z; a.gpart = h->gpart; a.spart = h->spart; a.gsum = h->gsum; a.st = h->st;
+    a.n = h->n_active; a.active = h->active; a.sidc = h->sidc; a.zc = h->zc; a.m = h->m; a.m_cap = h->m_cap; a.DA = h->DA;
+    a.y = h->y; a.g = h->g; a.lo = h->lo; a.hi = h->hi; a.n_struct = n_struct; a.T = T; a.w_over = w_over;
+    a.w_under = w_under; a.gpart = h->gpart; a.spart = h->spart; a.gsum = h->gsum; a.st = h->st;
     a.F_hist = h->F_hist; a.delta_hist = h->delta_hist; a.F_unreached = h->F_unreached; a.max_iter = max_iter;
     a.eps_F = eps_F; a.eps_y = eps_y;
     VMAT_CUDA(mp_launch_solve(h, a, s));
     VMAT_LAUNCH_CHECK();
+    if (z && h->n_active > 0) {
+        k_mp_scatter_z<<<(h->n_active + 255) / 256, 256, 0, s>>>(h->n_active, h->active, h->zc, z);
+        VMAT_LAUNCH_CHECK();
+    }
     MpState cur;
     VMAT_CUDA(cudaMemcpyAsync(&cur, h->st, sizeof(cur), cudaMemcpyDeviceToHost, s));
     if (y_host) VMAT_CUDA(cudaMemcpyAsync(y_host, h->y, (size_t)h->m * 8, cudaMemcpyDeviceToHost, s));
