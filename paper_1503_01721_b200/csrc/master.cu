@@ -3,11 +3,14 @@
 // F(z), z = sum_k DA(A_k) y_k, by the Barzilai-Borwein iteration with the subspace step rule.
 // Readings C15-C20: DESIGN.md section 2.
 //
-// Storage: DA is dense, VOXEL-MAJOR, float [n_voxels][m_cap] (the paper's aperture dose vectors are "dense-ish",
-// <= 0.15 % of the DDC matrix, L264).  One BB iteration then needs ONE pass over DA: a group of G lanes owns a
-// voxel row, its lanes hold the row's entries in registers, the row dot gives z_i (step 4 of L139), the
-// voxel's gradient follows (Eq. (1)), and every lane adds DA_ik * dF/dz_i to its own entries of the aperture
-// gradient g_A (step 1) - no second read, no atomics.  HBM-bound: 4 m n_voxels bytes per iteration.
+// Storage: DA is dense (the paper's aperture dose vectors are "dense-ish", <= 0.15 % of the DDC matrix, L264), in
+// COLUMN BLOCKS of 32 apertures: float [column block][voxel][32].  A run of consecutive voxels is then one
+// contiguous piece of memory per column block, whatever the capacity of the handle and however many apertures
+// exist so far, and a pipeline stage of the solve kernel (R consecutive voxels) is ceil(m / 32) bulk copies of
+// R x 128 bytes.  One BB iteration needs ONE pass over DA: the row dot gives z_i (step 4 of L139), the voxel's
+// gradient follows (Eq. (1)), and every lane adds DA_ik * dF/dz_i to its own entries of the aperture gradient g_A
+// (step 1) - no second read, no atomics.  HBM-bound: 4 m n_reached bytes per iteration.  Only BLOCKS of R
+// consecutive voxels of which some aperture reaches at least one are visited.
 // All sums are FP64 in a fixed order (FP32 storage of DA, T, weights): deterministic, and a trajectory differs
 // from the FP64 oracle's by summation order only.
 #include "common.cuh"
@@ -33,8 +36,9 @@ struct MpState {                              // device-resident scalars of one 
 
 struct vmat_mp {
     int32_t n_voxels = 0, m_cap = 0, m = 0;
+    int64_t n_vox_pad = 0;                    // voxels rounded up to a multiple of 16 (rows beyond n_voxels stay 0)
     int n_cta = 0, n_sm = 0, device = 0;      // n_cta: CTAs of the solve kernel = SMs (one persistent CTA each)
-    float *DA = nullptr;                      // [n_voxels][m_cap]
+    float *DA = nullptr;                      // [ceil(m_cap / 32)][n_vox_pad][32]
     double *y = nullptr, *g = nullptr, *lo = nullptr, *hi = nullptr;   // [m_cap]
     double *gpart = nullptr;                  // [m_cap][n_cta] per-CTA partials of g_A
     double *gsum = nullptr;                   // [m_cap] g_A of the current iterate, after the subspace rule
@@ -43,17 +47,18 @@ struct vmat_mp {
     double *F_hist = nullptr, *delta_hist = nullptr;   // [hist_cap + 1]
     int32_t hist_cap = 0;
     int32_t last_n_iter = 0;
-    // the voxels some aperture reaches (rows of DA with a non-zero): only they are visited by the passes
+    // the voxels some aperture reaches (rows of DA with a non-zero), and the blocks of R consecutive voxels that
+    // hold at least one of them: only those blocks are visited by the passes
     uint8_t *row_flag = nullptr;              // [n_voxels] set by vmat_mp_add_aperture
-    int32_t *active = nullptr;                // [n_voxels] their indices, ascending; valid while active_valid
-    int32_t *n_active_dev = nullptr;          // [1]
+    uint8_t *blk_flag = nullptr;              // [n_vox_pad / 2] per block of active_R voxels
+    int32_t *active = nullptr;                // [n_vox_pad / 2] indices of the flagged blocks, ascending
+    int32_t *n_active_dev = nullptr;          // [2]: flagged blocks, reached voxels
     void *select_tmp = nullptr;               // scratch of the compaction
     size_t select_tmp_bytes = 0;
-    int32_t n_active = 0;
-    bool active_valid = false;
-    double *F_unreached = nullptr;            // [1] F of the other voxels (z = 0), per solve
-    uint8_t *sidc = nullptr;                  // [n_voxels] structure ids of the reached voxels, in reached order
-    float *zc = nullptr;                      // [n_voxels] their doses, in reached order
+    int32_t n_active = 0;                     // flagged blocks
+    int32_t n_reached = 0;                    // reached voxels
+    int32_t active_R = 0;                     // block size the list was built for; 0 = stale
+    double *upart = nullptr;                  // [n_cta] partials of F over the voxels outside the flagged blocks
     double *stage3 = nullptr;                 // pinned host [3]: y0, lo, hi of the aperture being added
     cudaEvent_t stage3_free = nullptr;        // recorded after the copies that read stage3
     // scratch of the column-generation loop (allocated on first use, sized by the DDC handle it ran with)
@@ -81,35 +86,34 @@ __device__ __forceinline__ double mp_block_sum(double v, double *red /* [NW + 1]
     return red[NW];
 }
 
-// column k of DA; a voxel that any aperture reaches is flagged: only those rows are ever read again.  y0, lo, hi of
-// the aperture arrive in a pinned staging buffer (no stream synchronisation on the host side).
-__global__ void k_mp_set_column(int n_voxels, int m_cap, int k, const float *__restrict__ col, float *__restrict__ DA,
-                                uint8_t *__restrict__ row_flag)
+// column k of DA; a voxel that any aperture reaches is flagged: only blocks with such a voxel are ever read again
+__global__ void k_mp_set_column(int n_voxels, int64_t n_vox_pad, int k, const float *__restrict__ col,
+                                float *__restrict__ DA, uint8_t *__restrict__ row_flag)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n_voxels) {
         const float v = col[i];
-        DA[(size_t)i * m_cap + k] = v;
+        DA[((size_t)(k >> 5) * n_vox_pad + i) * 32 + (k & 31)] = v;
         if (v != 0.f) row_flag[i] = 1;
     }
 }
 
-// F of the voxels no aperture reaches (z_i = 0 whatever y): their terms of Eq. (1) at z = 0.  One CTA, fixed order.
-__global__ void __launch_bounds__(1024)
-k_mp_unreached_F(int n_voxels, const uint8_t *__restrict__ row_flag, const uint8_t *__restrict__ vstruct,
-                 const float *__restrict__ T, const float *__restrict__ w_over, const float *__restrict__ w_under,
-                 double *__restrict__ out)
+// flags of the blocks of R consecutive voxels (R = 4, 8 or 16) that hold a reached voxel; counts the reached voxels
+__global__ void k_mp_block_flags(int n_voxels, int R, const uint8_t *__restrict__ row_flag, uint8_t *__restrict__ blk_flag,
+                                 int32_t *__restrict__ n_reached)
 {
-    __shared__ double red[33];
-    double s = 0.0;
-    for (int i = threadIdx.x; i < n_voxels; i += 1024)
-        if (!row_flag[i]) {
-            const int sid = vstruct[i];
-            const double Ti = (double)T[sid], over = fmax(0.0 - Ti, 0.0), under = fmax(Ti - 0.0, 0.0);
-            s += (double)w_over[sid] * over * over + (double)w_under[sid] * under * under;
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    int cnt = 0;
+    if ((int64_t)b * R < n_voxels) {
+        for (int r = 0; r < R; ++r) {
+            const int64_t i = (int64_t)b * R + r;
+            if (i < n_voxels && row_flag[i]) ++cnt;
         }
-    const double tot = mp_block_sum<32>(s, red);
-    if (threadIdx.x == 0) out[0] = tot;
+        blk_flag[b] = cnt > 0;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    if ((threadIdx.x & 31) == 0 && cnt) atomicAdd(n_reached, cnt);      // integer: order-free
 }
 
 // ---------------------------------------------------------------- the whole BB solve: one persistent kernel
@@ -127,31 +131,31 @@ k_mp_unreached_F(int n_voxels, const uint8_t *__restrict__ row_flag, const uint8
 // No kernel launch and no host round trip per iteration (the first version launched a pass and a one-CTA step kernel
 // per iteration and let the host look at the stop flag every 8: 61 us per launch on average over a plan).
 //
-// The pass.  A warp owns R consecutive reached rows per pipeline stage, prefetched STAGES - 1 stages ahead by
-// 1-D bulk copies (cp.async.bulk, one per row, issued by R different lanes; completion counted in bytes on the
-// stage's mbarrier): no per-lane address arithmetic, no registers held across the flight.  Two lane mappings read
-// a stage from shared memory:
-//   z phase  LZ lanes per row, each CZ 16-byte chunks interleaved by LZ (so a quarter-warp reads 128 contiguous
-//            bytes or rows whose stride keeps them in different banks): the row dot in FP64 needs log2(LZ) plain
-//            shuffle steps for 32 / LZ rows at once instead of an 8-row butterfly over all 32 lanes;
-//   g phase  lane gl of a group of LPR lanes owns NC chunks of columns, as the partial sums of g_A demand, and adds
-//            DA_ik dF/dz_i for the rows of the stage, dF/dz_i broadcast through shared memory.
-// ~29 warp instructions per 512 bytes of DA instead of 64 (ncu: profiles/r2_*_mp.md).
+// The pass.  A warp owns one flagged block of R consecutive voxels per pipeline stage, prefetched STAGES - 1 stages
+// ahead by 1-D bulk copies (cp.async.bulk, SASS UBLKCP: one per column block, R x 128 contiguous bytes each, issued
+// by different lanes; completion counted in bytes on the stage's mbarrier): no per-lane address arithmetic, no
+// registers held across the flight.  LZ lanes share a row, each CZ 16-byte chunks interleaved by LZ; an entry is
+// converted to FP64 ONCE (F2F runs on the 16-lane XU pipe: converting twice made it the busiest pipe), the row dot
+// needs log2(LZ) plain shuffle steps for 32 / LZ rows at once, every lane of the row then forms dF/dz_i itself and
+// adds DA_ik dF/dz_i to the accumulators of ITS columns from the same registers; the row groups of a warp and the
+// warps are summed once per pass.  The block indices and structure ids a stage needs are loaded when the stage is
+// ISSUED and ride along in registers: a load on the critical path would queue behind the whole bulk stream.
+// ~30 warp instructions per 512 bytes of DA instead of 64 (ncu: profiles/r2_mp_solve.md).
 // All sums are FP64 in a fixed order given (m, SM count): deterministic.
 template <int V> struct MpCfg;
-//                                    bytes of a row at most | lanes per row, 16-byte chunks per lane | rows per stage |
-//                                    row padding (bank spread) | stages
-template <> struct MpCfg<0> { static constexpr int VB = 128,  LZ = 2,  CZ = 4, R = 16, PAD = 32, STAGES = 4; };
-template <> struct MpCfg<1> { static constexpr int VB = 256,  LZ = 4,  CZ = 4, R = 8,  PAD = 64, STAGES = 4; };
-template <> struct MpCfg<2> { static constexpr int VB = 512,  LZ = 8,  CZ = 4, R = 8,  PAD = 0,  STAGES = 3; };
-template <> struct MpCfg<3> { static constexpr int VB = 1024, LZ = 16, CZ = 4, R = 4,  PAD = 0,  STAGES = 3; };
-template <> struct MpCfg<4> { static constexpr int VB = 1536, LZ = 32, CZ = 3, R = 2,  PAD = 0,  STAGES = 4; };
+//                                    column blocks of 32 | lanes per row, 16-byte chunks per lane | voxels per block
+//                                    (= rows per stage) | stages
+template <> struct MpCfg<0> { static constexpr int NCB = 1,  LZ = 2,  CZ = 4, R = 16, STAGES = 4; };
+template <> struct MpCfg<1> { static constexpr int NCB = 2,  LZ = 4,  CZ = 4, R = 8,  STAGES = 4; };
+template <> struct MpCfg<2> { static constexpr int NCB = 4,  LZ = 8,  CZ = 4, R = 8,  STAGES = 3; };
+template <> struct MpCfg<3> { static constexpr int NCB = 8,  LZ = 16, CZ = 4, R = 4,  STAGES = 3; };
+template <> struct MpCfg<4> { static constexpr int NCB = 12, LZ = 32, CZ = 3, R = 4,  STAGES = 2; };
 static inline int mp_variant(int m) { return m <= 32 ? 0 : (m <= 64 ? 1 : (m <= 128 ? 2 : (m <= 256 ? 3 : 4))); }
 template <int V> __host__ __device__ constexpr size_t mp_ring_bytes()
 {
-    return (size_t)MP_WARPS * MpCfg<V>::STAGES * MpCfg<V>::R * (MpCfg<V>::VB + MpCfg<V>::PAD);
+    return (size_t)MP_WARPS * MpCfg<V>::STAGES * MpCfg<V>::R * MpCfg<V>::NCB * 128;
 }
-template <int V> __host__ __device__ constexpr size_t mp_accs_bytes() { return (size_t)MP_WARPS * (MpCfg<V>::VB / 4) * 8; }
+template <int V> __host__ __device__ constexpr size_t mp_accs_bytes() { return (size_t)MP_WARPS * (MpCfg<V>::NCB * 32) * 8; }
 template <int V> __host__ __device__ constexpr size_t mp_ring_alloc()   // the FP64 accumulators of a CTA reuse the ring
 {
     return mp_ring_bytes<V>() > mp_accs_bytes<V>() ? mp_ring_bytes<V>() : mp_accs_bytes<V>();
@@ -159,20 +163,24 @@ template <int V> __host__ __device__ constexpr size_t mp_ring_alloc()   // the F
 template <int V> __host__ __device__ constexpr size_t mp_smem_bytes() { return mp_ring_alloc<V>() + (size_t)MP_WARPS * MpCfg<V>::STAGES * 8; }
 
 struct MpArgs {
-    int n;                      // rows to visit: the reached voxels
-    const int32_t *active;      // their voxel indices, ascending
-    const uint8_t *sidc;        // [n] structure id of reached voxel pos
-    float *zc;                  // [n] dose of reached voxel pos (scattered into z by the caller afterwards)
-    int m, m_cap;
+    int n;                      // flagged blocks to visit
+    const int32_t *active;      // their indices, ascending (block b = voxels b R .. b R + R - 1)
+    int n_voxels;
+    int64_t n_vox_pad;
+    int m;
     const float *DA;
     double *y, *g;              // in: start; out: returned iterate and its g_A after the subspace rule
     const double *lo, *hi;
+    const uint8_t *vstruct;
+    int sid_aligned;            // vstruct is 16-byte aligned: the structure ids of a block can travel by cp.async
     int n_struct;
     const float *T, *w_over, *w_under;
+    float *z_out;               // or NULL
     double *gpart, *spart, *gsum;
     MpState *st;
     double *F_hist, *delta_hist;
-    const double *F_unreached;
+    const uint8_t *blk_flag;    // per block of R voxels: visited by the passes
+    double *upart;              // [n_cta] partials of F over the voxels outside the flagged blocks
     int max_iter;
     double eps_F, eps_y;
 };
@@ -234,88 +242,122 @@ __device__ __forceinline__ float4 mp_lds128(uint32_t addr)
     return e;
 }
 
+template <int BYTES>
+__device__ __forceinline__ void mp_cp_async(uint32_t dst, const void *src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" :: "r"(dst), "l"(src), "n"(BYTES) : "memory");
+}
+__device__ __forceinline__ void mp_cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void mp_cp_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
+__device__ __forceinline__ void mp_sts_u8(uint32_t dst, uint8_t v)
+{
+    asm volatile("st.shared.u8 [%0], %1;" :: "r"(dst), "r"((uint32_t)v) : "memory");
+}
+__device__ __forceinline__ uint32_t mp_lds_u8(uint32_t addr)
+{
+    uint32_t r;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(r) : "r"(addr));
+    return r;
+}
+
 // per-warp pipeline bookkeeping that lives across the passes of a solve
 struct MpPipe {
     uint32_t phases;            // bit s: parity the next wait on stage s must see
     int cstage;                 // next stage to consume
 };
 
-// One pass over the reached rows.  CURV = false: z = DA y, F, dF/dz, g_A partials (acc).  CURV = true: z = DA y,
+// One pass over the flagged blocks.  CURV = false: z = DA y, F, dF/dz, g_A partials (acc).  CURV = true: z = DA y,
 // q = DA v, sum_i w_i q_i^2 (C17).  ssum: this thread's part of F (or of the curvature).
 // sT2: per structure {T, 2 w_over, 2 w_under} in FP64.
 template <int V, bool CURV>
-__device__ __forceinline__ void mp_pass(const MpArgs &a, uint32_t ring_w, uint32_t bar_w, MpPipe &pp, const double *sy,
+__device__ __forceinline__ void mp_pass(const MpArgs &a, uint32_t ring_w, uint32_t bar_w, uint32_t sid_w, MpPipe &pp, const double *sy,
                                         const double *sv, const double *sT2, double (&acc)[MpCfg<V>::CZ][4], double &ssum)
 {
     using C = MpCfg<V>;
-    constexpr int LZ = C::LZ, CZ = C::CZ, R = C::R, STAGES = C::STAGES;
-    constexpr int RS = C::VB + C::PAD, STAGE_BYTES = R * RS;
+    constexpr int LZ = C::LZ, CZ = C::CZ, R = C::R, STAGES = C::STAGES, NCB = C::NCB;
+    constexpr int CB_BYTES = R * 128, STAGE_BYTES = NCB * CB_BYTES;
     constexpr int RZ = 32 / LZ, NSUB = R / RZ;
-    static_assert(R % RZ == 0 && NSUB >= 1 && NSUB <= 4 && LZ * CZ * 16 == C::VB && R <= 32, "mapping");
+    static_assert(R % RZ == 0 && NSUB >= 1 && NSUB <= 4 && LZ * CZ == NCB * 8 && NCB <= 32, "mapping");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int rz = lane / LZ, qz = lane % LZ;
     const int n = a.n;
-    const uint32_t W = (uint32_t)((a.m + 7) / 8) * 32u;           // bytes of a row that hold apertures (32-byte sectors)
-    const int64_t step = (int64_t)gridDim.x * MP_WARPS * R;
-    int64_t base = (int64_t)(blockIdx.x * MP_WARPS + warp) * R;
+    const int ncb = (a.m + 31) >> 5;                              // column blocks that hold apertures
+    const int step = gridDim.x * MP_WARPS;
+    int pos = blockIdx.x * MP_WARPS + warp;                       // position in the list of flagged blocks
     double yz[CZ][4];                                             // y of this lane's columns
 #pragma unroll
     for (int j = 0; j < CZ; ++j)
 #pragma unroll
         for (int k = 0; k < 4; ++k) yz[j][k] = sy[(j * LZ + qz) * 4 + k];   // 0 beyond m
-    int istage = pp.cstage;
-    int64_t ibase = base;
-    // row of DA this lane will ask the TMA unit for at the next issue, loaded one step early: the load's latency
-    // (the voxel index goes straight into the copy's address) would otherwise stall the warp at every stage
     const uint64_t pol_stream = mp_policy_evict_first(), pol_keep = mp_policy_evict_last();
-    int64_t nrow = (lane < R && ibase + lane < n) ? (int64_t)mp_ld_keep_i32(a.active + ibase + lane, pol_keep) : 0;
-    auto issue = [&]() {                                          // R rows starting at reached position ibase
-        const int64_t row = nrow;
-        const int64_t nb = ibase + step;
-        nrow = (lane < R && nb + lane < n) ? (int64_t)mp_ld_keep_i32(a.active + nb + lane, pol_keep) : 0;
-        if (ibase < n) {
-            const int nvalid = (int)min((int64_t)R, (int64_t)n - ibase);
-            const uint32_t bar = bar_w + 8u * istage;
-            if (lane == 0) mp_mbar_expect_tx(bar, (uint32_t)nvalid * W);
-            __syncwarp();
-            if (lane < nvalid)
-                mp_bulk_g2s(ring_w + (uint32_t)(istage * STAGE_BYTES + lane * RS), a.DA + row * a.m_cap, W, bar, pol_stream);
+    // lane part of the shared-memory offset of this lane's chunks of row rz: chunk c = j LZ + qz lies in column
+    // block c / 8 at 16-byte slot c % 8
+    const uint32_t lane_off = (uint32_t)((qz >> 3) * CB_BYTES + (qz & 7) * 16 + rz * 128);
+    // Block indices: lane l holds the index of the block this warp takes l steps after the start of the current batch
+    // of 32 steps; the next batch is loaded 32 steps before its first use, so no step ever waits for such a load
+    // (a load on the critical path would queue behind the whole bulk stream).  Structure ids: R bytes per block,
+    // copied by cp.async into the stage's slot of a small shared-memory FIFO when the stage is issued.
+    auto load_batch = [&](int p0) {
+        const int64_t p = (int64_t)p0 + (int64_t)lane * step;
+        return p < n ? mp_ld_keep_i32(a.active + p, pol_keep) : 0;
+    };
+    int batch_cur = load_batch(pos), batch_next = load_batch(pos + 32 * step);
+    int bi = 0;                                                   // steps issued out of batch_cur
+    int blk_q[STAGES];                                            // block indices of the stages in flight, oldest first
+#pragma unroll
+    for (int q = 0; q < STAGES; ++q) blk_q[q] = 0;
+    int istage = pp.cstage;
+    int ipos = pos;
+    auto issue = [&]() {                                          // the block at list position ipos
+        const int blk = __shfl_sync(0xffffffffu, batch_cur, bi);
+        if (++bi == 32) {
+            bi = 0;
+            batch_cur = batch_next;
+            batch_next = load_batch(ipos + step + 32 * step);
         }
-        ibase = nb;
+        if (ipos < n) {
+            const uint32_t bar = bar_w + 8u * istage;
+            if (lane == 0) {
+                mp_mbar_expect_tx(bar, (uint32_t)(ncb * CB_BYTES));
+                const int nb = min(R, a.n_voxels - blk * R);      // the volume may end inside the last block
+                if (nb == R && a.sid_aligned) mp_cp_async<R>(sid_w + (uint32_t)(istage * 16), a.vstruct + (size_t)blk * R);
+                else for (int r = 0; r < nb; ++r) mp_sts_u8(sid_w + (uint32_t)(istage * 16 + r), a.vstruct[(size_t)blk * R + r]);
+            }
+            __syncwarp();
+            if (lane < ncb)
+                mp_bulk_g2s(ring_w + (uint32_t)(istage * STAGE_BYTES + lane * CB_BYTES),
+                            a.DA + ((size_t)lane * a.n_vox_pad + (size_t)blk * R) * 32, CB_BYTES, bar, pol_stream);
+        }
+        mp_cp_commit();
+#pragma unroll
+        for (int q = 0; q < STAGES - 1; ++q) blk_q[q] = blk_q[q + 1];
+        blk_q[STAGES - 1] = blk;
+        ipos += step;
         if (++istage == STAGES) istage = 0;
     };
-#pragma unroll 1
-    for (int s = 0; s < STAGES - 1; ++s) issue();
-    // structure ids of this lane's rows of the stage after the current one (sub-step u: row u RZ + rz)
-    uint32_t sid_next = 0;
-    auto load_sids = [&](int64_t b) {
-        uint32_t r = 0;
 #pragma unroll
-        for (int u = 0; u < NSUB; ++u)
-            if (b + u * RZ + rz < n) r |= mp_ld_keep_u8(a.sidc + b + u * RZ + rz, pol_keep) << (8 * u);
-        return r;
-    };
-    sid_next = load_sids(base);
+    for (int s = 0; s < STAGES - 1; ++s) issue();
 #pragma unroll 1
-    for (; base < n; base += step) {
+    for (; pos < n; pos += step) {
         __syncwarp();                                             // every lane is done with the slot refilled now
         issue();
-        const uint32_t sids = sid_next;
-        sid_next = load_sids(base + step);
+        const int blk = blk_q[0];                                 // the stage consumed now was issued STAGES - 1 steps ago
         const int cs = pp.cstage;
+        mp_cp_wait<STAGES - 1>();                                 // lane 0: this stage's structure ids have landed
+        __syncwarp();
         mp_mbar_wait(bar_w + 8u * cs, (pp.phases >> cs) & 1u);
         pp.phases ^= 1u << cs;
         if (++pp.cstage == STAGES) pp.cstage = 0;
-        const uint32_t stg = ring_w + (uint32_t)(cs * STAGE_BYTES);
+        const uint32_t stg = ring_w + (uint32_t)(cs * STAGE_BYTES) + lane_off;
 #pragma unroll
         for (int u = 0; u < NSUB; ++u) {
-            // ---- row u RZ + rz of the stage: this lane's CZ chunks, converted to FP64 once
-            const uint32_t rowp = stg + (uint32_t)((u * RZ + rz) * RS + qz * 16);
+            // ---- row u RZ + rz of the block: this lane's CZ chunks, converted to FP64 once
             double e[CZ][4];
             double z4[4] = {0.0, 0.0, 0.0, 0.0}, q4[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
             for (int j = 0; j < CZ; ++j) {
-                const float4 f = mp_lds128(rowp + (uint32_t)(j * LZ * 16));
+                const float4 f = mp_lds128(stg + (uint32_t)(u * RZ * 128 + ((j * LZ) >> 3) * CB_BYTES + ((j * LZ) & 7) * 16));
                 e[j][0] = (double)f.x; e[j][1] = (double)f.y; e[j][2] = (double)f.z; e[j][3] = (double)f.w;
 #pragma unroll
                 for (int k = 0; k < 4; ++k) z4[k] = fma(e[j][k], yz[j][k], z4[k]);
@@ -333,16 +375,19 @@ __device__ __forceinline__ void mp_pass(const MpArgs &a, uint32_t ring_w, uint32
             }
             // ---- the voxel's term of F and dF/dz (Eq. (1), sign C1): with u = z - T and w2 = 2 w_over (u > 0) or
             //      2 w_under, dF/dz = w2 u and the term is w2 u^2 / 2
-            const int64_t pos = base + u * RZ + rz;
-            const bool live = pos < n;
-            const double *tp = sT2 + 3 * ((sids >> (8 * u)) & 0xffu);
+            const int vox = blk * R + u * RZ + rz;
+            const bool live = vox < a.n_voxels;                   // the last block may reach beyond the volume
+            const double *tp = sT2 + 3 * mp_lds_u8(sid_w + (uint32_t)(cs * 16 + u * RZ + rz));
             const double du = zs - tp[0];
             const double w2 = du > 0.0 ? tp[1] : tp[2];
             double gz = 0.0;
             if (live) {
                 if (!CURV) {
                     gz = w2 * du;
-                    if (qz == 0) { ssum = fma(0.5 * gz, du, ssum); a.zc[pos] = (float)zs; }
+                    if (qz == 0) {
+                        ssum = fma(0.5 * gz, du, ssum);
+                        if (a.z_out) a.z_out[vox] = (float)zs;
+                    }
                 } else if (qz == 0) {
                     ssum = fma(du != 0.0 ? 0.5 * w2 : 0.0, qs * qs, ssum);   // C17
                 }
@@ -362,14 +407,15 @@ __global__ void __launch_bounds__(MP_THREADS, 1)
 k_mp_solve(const MpArgs a)
 {
     using C = MpCfg<V>;
-    constexpr int LZ = C::LZ, CZ = C::CZ, STAGES = C::STAGES, COLS = C::VB / 4;
+    constexpr int LZ = C::LZ, CZ = C::CZ, STAGES = C::STAGES, COLS = C::NCB * 32;
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
-    extern __shared__ __align__(128) unsigned char mp_dyn[];      // ring [warp][stage][row][RS]; then the barriers
+    extern __shared__ __align__(128) unsigned char mp_dyn[];      // ring [warp][stage][column block][row][128 B]; then the barriers
     __shared__ double red_s[MP_WARPS + 1];
     __shared__ double sy[MP_MAX_M], syp[MP_MAX_M], sg[MP_MAX_M], sgp[MP_MAX_M];
     __shared__ double sT2[3 * 256];
     __shared__ double sFh[MP_HIST];
     __shared__ int s_flag;
+    __shared__ __align__(16) uint8_t s_sid[MP_WARPS][4][16];      // structure ids of the blocks in flight, per warp and stage
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, qz = lane % LZ;
     const int m = a.m, n_cta = gridDim.x;
     constexpr size_t RING = mp_ring_alloc<V>();
@@ -382,15 +428,29 @@ k_mp_solve(const MpArgs a)
         sy[k] = k < m ? fmin(fmax(a.y[k], a.lo[k]), a.hi[k]) : 0.0;          // the start must be feasible (C16)
         syp[k] = 0.0; sg[k] = 0.0; sgp[k] = 0.0;
     }
+    {   // F of the voxels outside the flagged blocks (z_i = 0 whatever y): their terms of Eq. (1) at z = 0, this CTA's
+        // slice of the volume; summed over the CTAs in a fixed order after the first grid barrier
+        const int per = (a.n_voxels + n_cta - 1) / n_cta, i0 = blockIdx.x * per, i1 = min(a.n_voxels, i0 + per);
+        double us = 0.0;
+        for (int i = i0 + tid; i < i1; i += MP_THREADS)
+            if (!a.blk_flag[i / C::R]) {
+                const int sid = a.vstruct[i];
+                const double Ti = (double)a.T[sid], over = fmax(0.0 - Ti, 0.0), under = fmax(Ti - 0.0, 0.0);
+                us += (double)a.w_over[sid] * over * over + (double)a.w_under[sid] * under * under;
+            }
+        const double tot = mp_block_sum(us, red_s);
+        if (tid == 0) a.upart[blockIdx.x] = tot;
+    }
     if (tid < MP_WARPS * STAGES) mp_mbar_init(mp_smem_u32(bars + tid), 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     mp_fence_async_proxy();
     __syncthreads();
-    const uint32_t ring_w = mp_smem_u32(mp_dyn) + (uint32_t)(warp * STAGES * C::R * (C::VB + C::PAD));
+    const uint32_t ring_w = mp_smem_u32(mp_dyn) + (uint32_t)(warp * STAGES * C::R * C::NCB * 128);
     const uint32_t bar_w = mp_smem_u32(bars + warp * STAGES);
+    const uint32_t sid_w = mp_smem_u32(&s_sid[warp][0][0]);
     MpPipe pp = {0u, 0};
     int it = 0, reason = 0;
-    double delta = 0.0, F = 0.0;
+    double delta = 0.0, F = 0.0, F_unreached = 0.0;
     for (;;) {
         // ---- steps 4 + 1 of L139: the gradient pass
         double acc[CZ][4];
@@ -399,7 +459,7 @@ k_mp_solve(const MpArgs a)
 #pragma unroll
             for (int k = 0; k < 4; ++k) acc[j][k] = 0.0;
         double ssum = 0.0;
-        mp_pass<V, false>(a, ring_w, bar_w, pp, sy, sg, sT2, acc, ssum);
+        mp_pass<V, false>(a, ring_w, bar_w, sid_w, pp, sy, sg, sT2, acc, ssum);
         // CTA partials in a fixed order: the row groups of a warp, then the warps (in the ring's memory, idle now)
         __syncthreads();
         double *accs = (double *)mp_dyn;                          // [MP_WARPS][COLS]
@@ -442,7 +502,12 @@ k_mp_solve(const MpArgs a)
         {                                                         // F: every CTA, same order
             double fs = 0.0;
             for (int c = tid; c < n_cta; c += MP_THREADS) fs += __ldcg(a.spart + 2 * c);
-            F = mp_block_sum(fs, red_s) + a.F_unreached[0];
+            if (it == 0) {
+                double us = 0.0;
+                for (int c = tid; c < n_cta; c += MP_THREADS) us += __ldcg(a.upart + c);
+                F_unreached = mp_block_sum(us, red_s);
+            }
+            F = mp_block_sum(fs, red_s) + F_unreached;
         }
         grid.sync();
         // ---- every CTA: stopping rules (C19), tested at the top of the iteration
@@ -485,7 +550,7 @@ k_mp_solve(const MpArgs a)
         // ---- step 2: the step size
         if (it == 0) {                                            // C17: one more pass, q = DA g_A
             double csum = 0.0;
-            mp_pass<V, true>(a, ring_w, bar_w, pp, sy, sg, sT2, acc, csum);
+            mp_pass<V, true>(a, ring_w, bar_w, sid_w, pp, sy, sg, sT2, acc, csum);
             const double tot = mp_block_sum(csum, red_s);
             if (tid == 0) a.spart[2 * blockIdx.x + 1] = tot;
             grid.sync();
@@ -521,20 +586,6 @@ k_mp_solve(const MpArgs a)
         for (int k = tid; k < m; k += MP_THREADS) { a.y[k] = sy[k]; a.g[k] = sg[k]; }
         if (tid == 0) { a.st->it = it; a.st->reason = reason; a.st->delta = delta; a.st->F = F; }
     }
-}
-
-// structure ids of the reached voxels, in reached order (once per solve: the passes then need no indirection)
-__global__ void k_mp_gather_sid(int n, const int32_t *__restrict__ active, const uint8_t *__restrict__ vstruct,
-                                uint8_t *__restrict__ sidc)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) sidc[i] = vstruct[active[i]];
-}
-// z of the returned iterate: the reached voxels' doses back to their places (the others were zeroed)
-__global__ void k_mp_scatter_z(int n, const int32_t *__restrict__ active, const float *__restrict__ zc, float *__restrict__ z)
-{
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) z[active[i]] = zc[i];
 }
 
 // ---------------------------------------------------------------- host side
@@ -590,8 +641,8 @@ int vmat_mp_destroy(vmat_mp *h)
 {
     if (!h) return VMAT_OK;
     void *ptrs[] = {h->DA, h->y, h->g, h->lo, h->hi, h->gpart, h->spart, h->gsum, h->st, h->F_hist,
-                    h->delta_hist, h->row_flag, h->active, h->n_active_dev, h->select_tmp, h->F_unreached, h->cg_scratch,
-                    h->sidc, h->zc};
+                    h->delta_hist, h->row_flag, h->blk_flag, h->active, h->n_active_dev, h->select_tmp, h->upart,
+                    h->cg_scratch};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     if (h->stage3) cudaFreeHost(h->stage3);
@@ -608,7 +659,8 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
     vmat_mp *h = new (std::nothrow) vmat_mp();
     if (!h) { vmat_set_error("vmat_mp_create: host allocation failed"); return VMAT_ERR_OOM; }
     h->n_voxels = n_voxels;
-    h->m_cap = (max_apertures + 7) / 8 * 8;                  // rows start on 32-byte boundaries
+    h->m_cap = (max_apertures + 7) / 8 * 8;
+    h->n_vox_pad = ((int64_t)n_voxels + 15) / 16 * 16;       // whole voxel blocks of every size (4, 8, 16)
     cudaGetDevice(&h->device);
     int n_sm = 1, coop = 0;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, h->device);
@@ -624,19 +676,21 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
     cudaStream_t s = (cudaStream_t)stream;
     auto alloc = [&](void **p, size_t bytes) { return cudaMalloc(p, bytes > 0 ? bytes : 1) == cudaSuccess; };
     const size_t mc = (size_t)h->m_cap;
-    bool ok = alloc((void **)&h->DA, (size_t)n_voxels * mc * 4) && alloc((void **)&h->y, mc * 8) &&
+    const size_t da_bytes = (size_t)((h->m_cap + 31) / 32) * (size_t)h->n_vox_pad * 128;
+    const size_t nblk_max = (size_t)(h->n_vox_pad / 4);       // the smallest blocks hold 4 voxels
+    bool ok = alloc((void **)&h->DA, da_bytes) && alloc((void **)&h->y, mc * 8) &&
               alloc((void **)&h->g, mc * 8) && alloc((void **)&h->gsum, mc * 8) &&
               alloc((void **)&h->lo, mc * 8) && alloc((void **)&h->hi, mc * 8) &&
               alloc((void **)&h->gpart, (size_t)h->n_cta * mc * 8) && alloc((void **)&h->spart, (size_t)h->n_cta * 16) &&
               alloc((void **)&h->st, sizeof(MpState)) && alloc((void **)&h->row_flag, (size_t)n_voxels) &&
-              alloc((void **)&h->active, (size_t)n_voxels * 4) && alloc((void **)&h->n_active_dev, 4) &&
-              alloc((void **)&h->F_unreached, 8) && alloc((void **)&h->sidc, (size_t)n_voxels) &&
-              alloc((void **)&h->zc, (size_t)n_voxels * 4) &&
+              alloc((void **)&h->blk_flag, nblk_max) &&
+              alloc((void **)&h->active, nblk_max * 4) && alloc((void **)&h->n_active_dev, 8) &&
+              alloc((void **)&h->upart, (size_t)h->n_cta * 8) &&
               cudaMallocHost((void **)&h->stage3, 3 * sizeof(double)) == cudaSuccess &&
               cudaEventCreateWithFlags(&h->stage3_free, cudaEventDisableTiming) == cudaSuccess;
     if (ok) {
-        cub::DeviceSelect::Flagged(nullptr, h->select_tmp_bytes, thrust::counting_iterator<int32_t>(0), h->row_flag, h->active,
-                                   h->n_active_dev, n_voxels, s);
+        cub::DeviceSelect::Flagged(nullptr, h->select_tmp_bytes, thrust::counting_iterator<int32_t>(0), h->blk_flag, h->active,
+                                   h->n_active_dev, (int)nblk_max, s);
         ok = alloc(&h->select_tmp, h->select_tmp_bytes);
     }
     if (!ok) {
@@ -645,7 +699,7 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
         vmat_set_error("vmat_mp_create: device allocation failed (%lld voxels x %d apertures)", (long long)n_voxels, h->m_cap);
         return VMAT_ERR_OOM;
     }
-    cudaMemsetAsync(h->DA, 0, (size_t)n_voxels * mc * 4, s);
+    cudaMemsetAsync(h->DA, 0, da_bytes, s);
     cudaMemsetAsync(h->row_flag, 0, (size_t)(n_voxels > 0 ? n_voxels : 1), s);
     cudaMemsetAsync(h->y, 0, mc * 8, s);
     cudaMemsetAsync(h->spart, 0, (size_t)h->n_cta * 16, s);
@@ -659,7 +713,7 @@ int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void 
 static int mp_forget(vmat_mp *h, cudaStream_t s)
 {
     h->m = 0;
-    h->active_valid = false;
+    h->active_R = 0;
     if (h->n_voxels > 0) VMAT_CUDA(cudaMemsetAsync(h->row_flag, 0, (size_t)h->n_voxels, s));
     return VMAT_OK;
 }
@@ -680,8 +734,8 @@ int vmat_mp_add_aperture(vmat_mp *h, const float *DA, double y0, double y_lo, do
     g_vmat_launches = 0;
     const int k = h->m;
     if (h->n_voxels > 0) {
-        k_mp_set_column<<<(h->n_voxels + 255) / 256, 256, 0, s>>>(h->n_voxels, h->m_cap, k, DA, h->DA, h->row_flag);
-        h->active_valid = false;
+        k_mp_set_column<<<(h->n_voxels + 255) / 256, 256, 0, s>>>(h->n_voxels, h->n_vox_pad, k, DA, h->DA, h->row_flag);
+        h->active_R = 0;
         VMAT_LAUNCH_CHECK();
     }
     // y0 / lo / hi through the handle's pinned staging buffer: wait (normally not at all) until the copies of the
@@ -720,22 +774,28 @@ int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, con
     REQUIRE(eps_F >= 0.0 && eps_y >= 0.0, "negative tolerance");
     cudaStream_t s = (cudaStream_t)stream;
     g_vmat_launches = 0;
-    // the voxels some aperture reaches, ascending; F of the others (their dose is 0 whatever y)
-    if (!h->active_valid) {
-        h->n_active = 0;
+    // the blocks of R consecutive voxels (R by the kernel variant m selects) with a voxel some aperture reaches,
+    // ascending; F of the voxels outside them (their dose is 0 whatever y)
+    const int R = mp_rows_per_stage(h->m);
+    if (h->active_R != R) {
+        h->n_active = h->n_reached = 0;
         if (h->n_voxels > 0) {
+            const int nblk = (int)(((int64_t)h->n_voxels + R - 1) / R);
+            VMAT_CUDA(cudaMemsetAsync(h->n_active_dev, 0, 8, s));
+            k_mp_block_flags<<<(nblk + 255) / 256, 256, 0, s>>>(h->n_voxels, R, h->row_flag, h->blk_flag, h->n_active_dev + 1);
+            VMAT_LAUNCH_CHECK();
             size_t tb = h->select_tmp_bytes;
-            VMAT_CUDA(cub::DeviceSelect::Flagged(h->select_tmp, tb, thrust::counting_iterator<int32_t>(0), h->row_flag,
-                                                 h->active, h->n_active_dev, h->n_voxels, s));
+            VMAT_CUDA(cub::DeviceSelect::Flagged(h->select_tmp, tb, thrust::counting_iterator<int32_t>(0), h->blk_flag,
+                                                 h->active, h->n_active_dev, nblk, s));
             g_vmat_launches += 2;
-            VMAT_CUDA(cudaMemcpyAsync(&h->n_active, h->n_active_dev, 4, cudaMemcpyDeviceToHost, s));
+            int32_t cnt[2] = {0, 0};
+            VMAT_CUDA(cudaMemcpyAsync(cnt, h->n_active_dev, 8, cudaMemcpyDeviceToHost, s));
             VMAT_CUDA(cudaStreamSynchronize(s));
+            h->n_active = cnt[0]; h->n_reached = cnt[1];
         }
-        h->active_valid = true;
+        h->active_R = R;
     }
-    k_mp_unreached_F<<<1, 1024, 0, s>>>(h->n_voxels, h->row_flag, voxel_struct, T, w_over, w_under, h->F_unreached);
-    VMAT_LAUNCH_CHECK();
-    if (z && h->n_voxels > 0) VMAT_CUDA(cudaMemsetAsync(z, 0, (size_t)h->n_voxels * 4, s));   // unreached voxels: z = 0
+    if (z && h->n_voxels > 0) VMAT_CUDA(cudaMemsetAsync(z, 0, (size_t)h->n_voxels * 4, s));   // voxels outside the blocks: z = 0
     if (max_iter + 1 > h->hist_cap) {
         if (h->F_hist) cudaFree(h->F_hist);
         if (h->delta_hist) cudaFree(h->delta_hist);
@@ -747,22 +807,14 @@ int vmat_mp_solve(vmat_mp *h, const uint8_t *voxel_struct, int32_t n_struct, con
         h->hist_cap = (int32_t)cap;
     }
     // the whole BB iteration in one cooperative launch; the start is clipped into the box inside (C16)
-    if (h->n_active > 0) {
-        k_mp_gather_sid<<<(h->n_active + 255) / 256, 256, 0, s>>>(h->n_active, h->active, voxel_struct, h->sidc);
-        VMAT_LAUNCH_CHECK();
-    }
     MpArgs a;
-    a.n = h->n_active; a.active = h->active; a.sidc = h->sidc; a.zc = h->zc; a.m = h->m; a.m_cap = h->m_cap; a.DA = h->DA;
-    a.y = h->y; a.g = h->g; a.lo = h->lo; a.hi = h->hi; a.n_struct = n_struct; a.T = T; a.w_over = w_over;
-    a.w_under = w_under; a.gpart = h->gpart; a.spart = h->spart; a.gsum = h->gsum; a.st = h->st;
-    a.F_hist = h->F_hist; a.delta_hist = h->delta_hist; a.F_unreached = h->F_unreached; a.max_iter = max_iter;
-    a.eps_F = eps_F; a.eps_y = eps_y;
+    a.n = h->n_active; a.active = h->active; a.n_voxels = h->n_voxels; a.n_vox_pad = h->n_vox_pad; a.m = h->m; a.DA = h->DA;
+    a.y = h->y; a.g = h->g; a.lo = h->lo; a.hi = h->hi; a.vstruct = voxel_struct; a.sid_aligned = ((uintptr_t)voxel_struct & 15) == 0; a.n_struct = n_struct; a.T = T;
+    a.w_over = w_over; a.w_under = w_under; a.z_out = z; a.gpart = h->gpart; a.spart = h->spart; a.gsum = h->gsum;
+    a.st = h->st; a.F_hist = h->F_hist; a.delta_hist = h->delta_hist; a.blk_flag = h->blk_flag; a.upart = h->upart;
+    a.max_iter = max_iter; a.eps_F = eps_F; a.eps_y = eps_y;
     VMAT_CUDA(mp_launch_solve(h, a, s));
     VMAT_LAUNCH_CHECK();
-    if (z && h->n_active > 0) {
-        k_mp_scatter_z<<<(h->n_active + 255) / 256, 256, 0, s>>>(h->n_active, h->active, h->zc, z);
-        VMAT_LAUNCH_CHECK();
-    }
     MpState cur;
     VMAT_CUDA(cudaMemcpyAsync(&cur, h->st, sizeof(cur), cudaMemcpyDeviceToHost, s));
     if (y_host) VMAT_CUDA(cudaMemcpyAsync(y_host, h->y, (size_t)h->m * 8, cudaMemcpyDeviceToHost, s));
@@ -866,6 +918,7 @@ int vmat_column_generation_ex(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_str
     }
     while (count < max_apertures) {
         // PP1: gradient at the current dose, beamlet prices; PP2: best opening per leaf row, best control point
+        g_vmat_launches = 0;
         int rc = vmat_launch_objective(h, z, voxel_struct, n_struct, T, w_over, w_under, w.g, w.F, s);
         if (!constrained) {
             if (rc == VMAT_OK) rc = vmat_launch_price_select(h, w.g, w.mask, w.p, w.Lw, w.Rw, w.row_price, s, true);   // k not in C only (L58)
@@ -923,8 +976,8 @@ int vmat_column_generation_ex(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_str
 int vmat_mp_reached_voxels(const vmat_mp *h, int32_t *n_reached)
 {
     REQUIRE(h != nullptr && n_reached != nullptr, "NULL argument");
-    REQUIRE(h->active_valid, "no solve has run since the last aperture was added");
-    *n_reached = h->n_active;
+    REQUIRE(h->active_R != 0, "no solve has run since the last aperture was added");
+    *n_reached = h->n_reached;
     return VMAT_OK;
 }
 
@@ -933,7 +986,7 @@ int vmat_mp_pass_geometry(const vmat_mp *h, int32_t m, int32_t *n_cta, int32_t *
     REQUIRE(h != nullptr, "handle is NULL");
     REQUIRE(m >= 1 && m <= h->m_cap, "m must be in 1..max_apertures");
     if (n_cta) *n_cta = h->n_cta;
-    if (rows_per_grid_step) *rows_per_grid_step = h->n_cta * MP_WARPS * mp_rows_per_stage(m);
+    if (rows_per_grid_step) *rows_per_grid_step = h->n_cta * MP_WARPS * mp_rows_per_stage(m);   // one block per warp and step
     return VMAT_OK;
 }
 
