@@ -148,66 +148,141 @@ def phantom_arrays_host(ph):
 
 
 # ----------------------------------------------------------------------------- the CPU oracle, timed
-def oracle_rate(spec, gen_device, budget_s: float, reps: int, reps_auto: bool = False):
-    """Times the oracle (one whole price evaluation, O1-O5) on an angle-block sample of `spec`
-    (D = [D_1 ... D_A]; the evaluation is additive over angle blocks) sized to about
-    `budget_s` seconds of single-thread CPU work.  Returns (evals/s extrapolated to the full matrix,
-    description, per-rep seconds, nnz_sample, nnz_full_estimate)."""
+ORACLE_KINDS = {
+    "oracle": "oracle (oracle/vmat_oracle.c, plain single-thread FP64 loops over the COO triplets)",
+    "oracle_mt": "oracle_mt (oracle/vmat_oracle_mt.c: the same C functions, every thread on its share of the triplets / "
+                 "voxels / leaf rows, PAPER.md L191)",
+}
+
+
+def host_ram_available() -> int:
+    try:
+        import psutil
+        return int(psutil.virtual_memory().available)
+    except Exception:
+        return 0
+
+
+def oracle_probe(spec, gen_device):
+    """Seconds of the single-thread oracle per control point, and non-zeros per control point (one control point timed)."""
     import oracle
-    n_a = spec.n_angles
-    # calibrate on one control point
-    probe = synth.generate(spec, device=gen_device, angles=[n_a // 3])
+    probe = synth.generate(spec, device=gen_device, angles=[spec.n_angles // 3])
     A = phantom_arrays_host(probe)
     x = synth.draw_x(probe.n_beamlets, 0).numpy()
     t0 = time.perf_counter()
     oracle.price_eval(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], x, A["sid"], A["T"], A["wo"], A["wu"],
                       A["lco"], A["aro"])
-    t1 = time.perf_counter() - t0
-    k = int(max(1, min(n_a, budget_s / max(t1, 1e-4), 4e8 / max(probe.nnz, 1))))   # <= ~4e8 nnz (5 GB of host COO)
+    return time.perf_counter() - t0, probe.nnz
+
+
+def oracle_workload(spec, gen_device, budget_s: float, t_cp: float, nnz_cp: int, coo_host=None):
+    """The data one oracle step evaluates: the WHOLE matrix when one single-thread evaluation fits `budget_s` and the
+    triplets fit the host's memory, else an evenly spaced sample of control points (angle blocks: the
+    evaluation is additive over them) sized to the budget.  Returns (arrays, description dict)."""
+    n_a = spec.n_angles
+    full_ok = t_cp * n_a <= budget_s and 12.0 * nnz_cp * n_a * 1.6 <= max(host_ram_available(), 8e9)
+    if full_ok:
+        A = coo_host if coo_host is not None else phantom_arrays_host(synth.generate(spec, device=gen_device))
+        return A, {"control_points": n_a, "of": n_a, "nnz": int(A["val"].size), "fraction": 1.0}
+    k = int(max(1, min(n_a, budget_s / max(t_cp, 1e-4), 4e8 / max(nnz_cp, 1))))     # <= ~4e8 nnz (5 GB of host COO)
     angles = sorted(set(int(round(i * n_a / k)) % n_a for i in range(k)))
     smp = synth.generate(spec, device=gen_device, angles=angles)
-    A = phantom_arrays_host(smp)
+    return phantom_arrays_host(smp), {"control_points": len(angles), "of": n_a, "nnz": int(smp.nnz),
+                                      "fraction": len(angles) / n_a}
+
+
+def oracle_step(A, k: int, kind: str, cores: int):
+    """One whole price evaluation O1-O5 on x draw k; returns seconds."""
+    import oracle
+    x = synth.draw_x(A["n_b"], k).numpy()
+    args = (A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], x, A["sid"], A["T"], A["wo"], A["wu"], A["lco"], A["aro"])
+    t0 = time.perf_counter()
+    if kind == "oracle":
+        oracle.price_eval(*args)
+    else:
+        oracle.price_eval_mt(*args, n_threads=cores)
+    return time.perf_counter() - t0
+
+
+def oracle_leg(A, desc, spec, kind: str, cores: int, reps: int, budget_s: float, warm: int = 0) -> dict:
+    """Times `reps` evaluations (stops early beyond `budget_s`); the reported value is what was MEASURED on the data
+    evaluated; when that is a sample of the control points, the full-matrix figure by additivity sits in its own key."""
     times = []
-    for r in range(reps):
-        if r >= 3 and reps_auto and sum(times) > budget_s:
+    for r in range(warm + reps):
+        t = oracle_step(A, r, kind, cores)
+        if r >= warm:
+            times.append(t)
+        if r >= warm and sum(times) > budget_s:
             break
-        x = synth.draw_x(smp.n_beamlets, r).numpy()
-        t0 = time.perf_counter()
-        oracle.price_eval(A["vox"], A["beam"], A["val"], A["n_v"], A["n_b"], x, A["sid"], A["T"], A["wo"],
-                          A["wu"], A["lco"], A["aro"])
-        times.append(time.perf_counter() - t0)
-    frac = len(angles) / n_a
-    t_full = float(np.median(times)) / frac                 # the evaluation is additive over angle blocks
-    desc = (f"{len(angles)} of {n_a} control points of {spec.name} (every {n_a / len(angles):.1f}th angle block, "
-            f"{smp.nnz} nnz), whole evaluation O1-O5 per rep, {len(times)} reps, median; evals/s extrapolated by "
-            f"angle-block additivity (x{1 / frac:.1f})")
-    return 1.0 / t_full, desc, times, smp.nnz, smp.nnz / frac
+    t_med = float(np.median(times))
+    frac = desc["fraction"]
+    what = "the whole matrix" if frac == 1.0 else \
+        f"{desc['control_points']} of {desc['of']} control points (every {1 / frac:.1f}th angle block)"
+    leg = {"value": 1.0 / t_med, "unit": UNIT, "cores": cores, "kind": "oracle", "variant": ORACLE_KINDS[kind],
+           "ms_per_step": 1e3 * t_med,
+           "reps": len(times), "sample_nnz": desc["nnz"],
+           "sample": f"{what} of {spec.name}, {desc['nnz']} nnz; one whole evaluation O1-O5 per rep, {len(times)} reps, "
+                     f"median; measured, not extrapolated"}
+    if frac < 1.0:
+        leg["full_matrix"] = {"value": frac / t_med, "unit": UNIT, "ms_per_step": 1e3 * t_med / frac, "extrapolated": True,
+                              "factor": 1.0 / frac, "how": "angle-block additivity of the evaluation (PAPER.md L119, pin P6)"}
+    return leg
+
+
+def cpu_baseline(spec, gen_device, coo_host=None) -> dict:
+    """bench.py's `cpu_baseline`: the plain oracle on one core (about 20 s of CPU work) and the all-cores variant on the
+    same data."""
+    import oracle
+    t_cp, nnz_cp = oracle_probe(spec, gen_device)
+    A, desc = oracle_workload(spec, gen_device, 25.0, t_cp, nnz_cp, coo_host)
+    one = oracle_leg(A, desc, spec, "oracle", 1, 5, 20.0)
+    cores = oracle.available_cores()
+    one["all_cores"] = oracle_leg(A, desc, spec, "oracle_mt", cores, 7, 10.0, warm=1)
+    return one
 
 
 def run_reference(args):
-    """--impl reference: the oracle as it stands on the host cores (rank 0 only)."""
+    """--impl reference: the CPU oracle on the host cores (rank 0 only), K timed steps after W warm-up steps, every step
+    one whole evaluation.  The plain single-thread oracle on the whole matrix when K + W such steps fit the time budget
+    (configs 0-2); else the all-cores variant on the whole matrix (config 3 on a 16-core box); else an angle-block
+    sample.  `value` and `ms_per_step` are what was measured on the data evaluated."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    import oracle
     spec = synth.config_spec(args.config, args.scale)
     gen_dev = "cuda:0" if torch.cuda.is_available() else "cpu"
     total_budget = 150.0                                     # seconds for the whole --steps/--warmup run
-    per_step = min(15.0, total_budget / max(1, args.steps + args.warmup))
-    # warm-up reps are part of `reps`; only the last `steps` are reported
-    value, desc, times, nnz_s, nnz_full = oracle_rate(spec, gen_dev, per_step, args.steps + args.warmup)
+    n_steps = max(1, args.steps + args.warmup)
+    per_step = total_budget / n_steps
+    t_cp, nnz_cp = oracle_probe(spec, gen_dev)
+    cores = oracle.available_cores()
+    t_full = t_cp * spec.n_angles
+    if t_full <= per_step or cores == 1:
+        kind, n_thr = "oracle", 1
+        A, desc = oracle_workload(spec, gen_dev, per_step, t_cp, nnz_cp)
+    else:
+        kind, n_thr = "oracle_mt", cores
+        A, desc = oracle_workload(spec, gen_dev, per_step * 0.5 * cores, t_cp, nnz_cp)   # threads scale ~0.5 x cores
+    times = [oracle_step(A, k, kind, n_thr) for k in range(n_steps)]
     timed = times[args.warmup:] if len(times) > args.warmup else times
-    frac = nnz_s / nnz_full
-    t_full = float(np.median(timed)) / frac
-    value = 1.0 / t_full
+    t_med = float(np.median(timed))
+    frac = desc["fraction"]
+    what = "the whole matrix" if frac == 1.0 else f"{desc['control_points']} of {desc['of']} control points"
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_full, "higher_is_better": True,
+        "impl": "reference", "metric": METRIC, "value": 1.0 / t_med, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_med, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": spec.name, "nnz_full_estimate": int(nnz_full), "sample_nnz": int(nnz_s)},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
-        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "config": {"workload": spec.name, "evaluated": what, "sample_nnz": desc["nnz"], "fraction_of_matrix": frac},
+        "cpu_baseline": {"value": 1.0 / t_med, "unit": UNIT, "cores": n_thr, "kind": "oracle", "variant": ORACLE_KINDS[kind],
+                         "sample": f"{what} of {spec.name}, {desc['nnz']} nnz; every step one whole evaluation O1-O5, "
+                                   f"median of the {len(timed)} timed steps; measured, not extrapolated"},
+        "e2e": {"value": 1.0 / t_med, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
+    if frac < 1.0:
+        line["full_matrix"] = {"value": frac / t_med, "unit": UNIT, "ms_per_step": 1e3 * t_med / frac, "extrapolated": True,
+                               "factor": 1.0 / frac, "how": "angle-block additivity of the evaluation (PAPER.md L119)"}
     print(json.dumps(line))
 
 
@@ -430,6 +505,10 @@ def run_ours(args):
     t_ingest = time.time() - t0
     stats = ph.stats()
     h.leafrow_col_offset_host = ph.leafrow_col_offset.to(torch.int64).cpu()
+    # the CPU baseline evaluates the very same triplets: keep a host copy when they fit the host's memory
+    coo_host = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and 12.0 * ph.nnz * 1.6 <= max(host_ram_available(), 8e9):
+        coo_host = phantom_arrays_host(ph)
     ph.coo_voxel = ph.coo_beamlet = ph.coo_val = None      # the handle holds its own layouts
     torch.cuda.empty_cache()
     obj = vm.Objective(ph.voxel_struct.to(dev), ph.struct_T.to(dev), ph.struct_w_over.to(dev),
@@ -576,8 +655,7 @@ def run_ours(args):
         if cplan_line is not None:
             line["plan_optimisation_constrained"] = cplan_line
         if not args.no_cpu_baseline and world == 1:
-            v, desc, _, _, _ = oracle_rate(spec, dev, 12.0, 40, reps_auto=True)
-            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc}
+            line["cpu_baseline"] = cpu_baseline(spec, dev, coo_host)
         print(json.dumps(line))
     h.close()
     if use_dist:

@@ -130,6 +130,12 @@ int vmat_objective_grad(const vmat_ddc *h, const float *d, const uint8_t *voxel_
  * beamlet row as in L127).  g dev [n_voxels] in, p dev [n_beamlets] out. */
 int vmat_price(const vmat_ddc *h, const float *g, float *p, void *stream);
 
+/* Contract check for the objective arguments of every call that takes them: voxel_struct dev u8 [n_voxels] must hold
+ * ids < n_struct (they index T / w_over / w_under; the compute calls do not re-check them on the device: an id
+ * beyond n_struct reads past the tables).  Synchronous.  Returns VMAT_ERR_INDEX_RANGE if an id is out of range,
+ * VMAT_ERR_INVALID_ARG for n_struct outside 1..256. */
+int vmat_check_structure_ids(const uint8_t *voxel_struct, int32_t n_voxels, int32_t n_struct, void *stream);
+
 /* A4 + A5 aperture selection without interdigitation (L133): for every MLC leaf row the contiguous
  * opening [L,R) (beamlet columns within the row, 0 <= L <= R <= n_row; C8) minimising the summed
  * price, the closed opening (value 0, L = R = 0) included (C4); then per control point the sum of its
@@ -188,7 +194,7 @@ int vmat_aperture_dose(const vmat_ddc *h, int32_t angle, const int32_t *L, const
  * MLC geometry, once per handle: leafrow_pos0 host int32 [n_leaf_rows] = physical column (in beamlet widths, on
  * the control point's own grid) of the first beamlet of every leaf row (ignored for rows without beamlets).  The
  * field range of a control point is [Pmin, Pmax] = [min pos0, max pos0 + n] over its non-empty rows and may span
- * at most 255 beamlet widths; the longest leaf row is bounded by the SM's shared memory ((n+1)^2 table entries of
+ * at most 254 beamlet widths (255 leaf positions); the longest leaf row is bounded by the SM's shared memory ((n+1)^2 table entries of
  * 10 bytes: about 145 beamlets on B200).  Returns VMAT_ERR_INVALID_ARG beyond either.  Synchronous. */
 int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0);
 

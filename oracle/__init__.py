@@ -179,3 +179,75 @@ def price_eval(coo_voxel, coo_beamlet, coo_val, n_voxels, n_beamlets, x, voxel_s
             rp[aro[a]:aro[a + 1]] = 0.0
     ap, best = angle_price(rp, angle_row_offset, angle_mask)
     return PriceEval(d, F, g, p, p32, L, R, rp, ap, best)
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# All-cores variant for the TIMED baseline only (vmat_oracle_mt.c: the same C functions, each thread on its share of
+# the triplets / voxels / leaf rows).  Pinned against the functions above in tests/test_oracle_mt.py.
+_SRC_MT = os.path.join(_HERE, "vmat_oracle_mt.c")
+_SO_MT = os.path.join(_HERE, "libvmat_oracle_mt.so")
+_lib_mt = None
+
+
+def build_mt(force: bool = False) -> str:
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_MT))
+    if force or not os.path.exists(_SO_MT) or os.path.getmtime(_SO_MT) < newest:
+        tmp = _SO_MT + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared", "-pthread",
+                               "-o", tmp, _SRC, _SRC_MT, "-lm"])
+        os.replace(tmp, _SO_MT)
+    return _SO_MT
+
+
+def _load_mt():
+    global _lib_mt
+    if _lib_mt is None:
+        lib = ctypes.CDLL(build_mt())
+        i32, i64, vp, f64, ci = ctypes.c_int32, ctypes.c_int64, ctypes.c_void_p, ctypes.c_double, ctypes.c_int
+        lib.oracle_mt_dose.argtypes = [ci, i64, vp, vp, vp, i32, vp, vp, vp]
+        lib.oracle_mt_dose.restype = None
+        lib.oracle_mt_price.argtypes = [ci, i64, vp, vp, vp, i32, vp, vp, vp]
+        lib.oracle_mt_price.restype = None
+        lib.oracle_mt_objective_grad.argtypes = [ci, i32, vp, vp, vp, vp, vp, vp]
+        lib.oracle_mt_objective_grad.restype = f64
+        lib.oracle_mt_select_rows.argtypes = [ci, i32, vp, vp, vp, vp, vp, i32]
+        lib.oracle_mt_select_rows.restype = None
+        _lib_mt = lib
+    return _lib_mt
+
+
+def available_cores() -> int:
+    return len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+
+
+def price_eval_mt(coo_voxel, coo_beamlet, coo_val, n_voxels, n_beamlets, x, voxel_struct, T, w_over, w_under,
+                  leafrow_col_offset, angle_row_offset, n_threads: Optional[int] = None) -> PriceEval:
+    """One whole price evaluation O1 -> O5 with the work of O1-O4 spread over `n_threads` (default: every core
+    this process may run on)."""
+    lib = _load_mt()
+    nt = int(n_threads or available_cores())
+    v, pv = _c(coo_voxel, np.int32)
+    b, pb = _c(coo_beamlet, np.int32)
+    a, pa = _c(coo_val, np.float32)
+    xx, px = _c(x, np.float32)
+    s, ps = _c(voxel_struct, np.uint8)
+    t, pt = _c(T, np.float32)
+    wo, pwo = _c(w_over, np.float32)
+    wu, pwu = _c(w_under, np.float32)
+    off, po = _c(leafrow_col_offset, np.int32)
+    priv = np.empty(nt * max(n_voxels, n_beamlets, 1), dtype=np.float64)
+    d = np.empty(n_voxels, dtype=np.float64)
+    lib.oracle_mt_dose(nt, v.size, pv, pb, pa, n_voxels, px, d.ctypes.data, priv.ctypes.data)
+    g = np.empty(n_voxels, dtype=np.float64)
+    F = float(lib.oracle_mt_objective_grad(nt, n_voxels, d.ctypes.data, ps, pt, pwo, pwu, g.ctypes.data))
+    p = np.empty(n_beamlets, dtype=np.float64)
+    lib.oracle_mt_price(nt, v.size, pv, pb, pa, n_beamlets, g.ctypes.data, p.ctypes.data, priv.ctypes.data)
+    p32 = p.astype(np.float32)
+    n_rows = off.size - 1
+    L = np.zeros(n_rows, dtype=np.int32)
+    R = np.zeros(n_rows, dtype=np.int32)
+    rp = np.zeros(n_rows, dtype=np.float64)
+    max_n = int(np.max(np.diff(off))) if n_rows > 0 else 0
+    lib.oracle_mt_select_rows(nt, n_rows, po, p32.ctypes.data, L.ctypes.data, R.ctypes.data, rp.ctypes.data, max_n)
+    ap, best = angle_price(rp, angle_row_offset)
+    return PriceEval(d, F, g, p, p32, L, R, rp, ap, best)

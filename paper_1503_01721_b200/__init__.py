@@ -33,7 +33,7 @@ EXPORTS = [
     "vmat_mp_create", "vmat_mp_destroy", "vmat_mp_reset", "vmat_mp_add_aperture", "vmat_mp_set_fluence", "vmat_mp_size",
     "vmat_mp_solve", "vmat_mp_history", "vmat_column_generation",
     "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained", "vmat_leaf_windows",
-    "vmat_column_generation_ex", "vmat_price_select", "vmat_mp_reached_voxels", "vmat_mp_pass_geometry",
+    "vmat_column_generation_ex", "vmat_price_select", "vmat_mp_reached_voxels", "vmat_mp_pass_geometry", "vmat_check_structure_ids",
 ]
 
 
@@ -69,6 +69,7 @@ def load_library():
     lib.vmat_dose.argtypes = [vp, vp, vp, vp]
     lib.vmat_objective_grad.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp]
     lib.vmat_price.argtypes = [vp, vp, vp, vp]
+    lib.vmat_check_structure_ids.argtypes = [vp, i32, i32, vp]
     lib.vmat_select_apertures.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_price_eval.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_price_eval_host.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -136,6 +137,12 @@ class Objective:
     @property
     def n_struct(self) -> int:
         return int(self.T.numel())
+
+    def validate(self):
+        """vmat_check_structure_ids: every id indexes the per-structure tables (raises VmatError otherwise)."""
+        with torch.cuda.device(self.voxel_struct.device):
+            _check(load_library().vmat_check_structure_ids(_ptr(self.voxel_struct, torch.uint8, "cuda"),
+                                                           int(self.voxel_struct.numel()), self.n_struct, _stream()))
 
 
 @dataclass

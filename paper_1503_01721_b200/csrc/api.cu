@@ -114,9 +114,41 @@ __global__ void k_aperture_finish(int n_voxels, const unsigned long long *__rest
     if (i < n_voxels) DA[i] = (float)((double)(long long)acc[i] * inv_scale);
 }
 
+__global__ void k_max_u8(const uint8_t *__restrict__ v, int n, unsigned *__restrict__ out)
+{
+    unsigned m = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) m = max(m, (unsigned)v[i]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
+}
+
 extern "C" {
 
 const char *vmat_last_error(void) { return g_err; }
+
+int vmat_check_structure_ids(const uint8_t *voxel_struct, int32_t n_voxels, int32_t n_struct, void *stream)
+{
+    REQUIRE(n_struct >= 1 && n_struct <= 256, "n_struct must be in 1..256");
+    REQUIRE(n_voxels >= 0 && (voxel_struct || n_voxels == 0), "NULL argument");
+    if (n_voxels == 0) return VMAT_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned *d_max = nullptr, h_max = 0;
+    VMAT_CUDA(cudaMalloc((void **)&d_max, 4));
+    cudaError_t e = cudaMemsetAsync(d_max, 0, 4, st);
+    if (e == cudaSuccess) {
+        k_max_u8<<<256, 256, 0, st>>>(voxel_struct, n_voxels, d_max);
+        e = cudaMemcpyAsync(&h_max, d_max, 4, cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d_max);
+    VMAT_CUDA(e);
+    if ((int)h_max >= n_struct) {
+        vmat_set_error("vmat_check_structure_ids: structure id %u >= n_struct %d", h_max, n_struct);
+        return VMAT_ERR_INDEX_RANGE;
+    }
+    return VMAT_OK;
+}
 int vmat_last_launch_count(void) { return g_vmat_launches; }
 
 int vmat_ddc_destroy(vmat_ddc *h)
@@ -367,13 +399,7 @@ int vmat_price_eval(const vmat_ddc *h, const float *x,
     g_vmat_launches = 0;
     TRY(vmat_launch_dose(h, x, d, true, voxel_struct, n_struct, T, w_over, w_under, g, F, st));
     if (h->prof_ev[2]) VMAT_CUDA(cudaEventRecord(h->prof_ev[2], st));
-    static const bool unfused = getenv("VMAT_UNFUSED_SELECT") != nullptr;   // measurement knob: A3 and A4 as two kernels
-    if (unfused) {
-        TRY(vmat_launch_price(h, g, p, st));
-        TRY(vmat_launch_select(h, p, angle_mask, L, R, row_price, st));
-    } else {
-        TRY(vmat_launch_price_select(h, g, angle_mask, p, L, R, row_price, st));
-    }
+    TRY(vmat_launch_price_select(h, g, angle_mask, p, L, R, row_price, st));
     if (h->prof_ev[3]) VMAT_CUDA(cudaEventRecord(h->prof_ev[3], st));
     return vmat_launch_angle_price(h, row_price, angle_mask, angle_price, best_angle, st);
 }

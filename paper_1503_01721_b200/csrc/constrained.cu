@@ -564,8 +564,9 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
             amax[k] = n > amax[k] ? n : amax[k];
             any = true;
         }
-        REQUIRE((int64_t)hi - lo + 1 <= CS_MAX_POS + 1,
-                "a control point's field range exceeds 255 beamlet widths (positions are packed in 8 bits)");
+        REQUIRE((int64_t)hi - lo + 1 <= CS_MAX_POS,
+                "a control point's field range exceeds 254 beamlet widths (positions 0..254 are packed in 8 bits each; "
+                "the pair (255, 255) is the 'no predecessor' mark)");
         pmin[k] = lo;
         wd[k] = hi - lo + 1;
         max_wd = wd[k] > max_wd ? wd[k] : max_wd;
@@ -583,7 +584,16 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
                        max_n, cs_smem_bytes(tab_n, max_wd, max_rows), smem_optin);
         return VMAT_ERR_INVALID_ARG;
     }
-    VMAT_CUDA(cudaFuncSetAttribute(k_cs_dp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cs_smem_bytes(tab_n, max_wd, max_rows)));
+    // The attribute belongs to the kernel on a device, not to this handle: always the device's maximum, so that a
+    // second handle with shorter leaf rows can never lower it under what this one launches with.
+    {
+        int cur = 0;
+        VMAT_CUDA(cudaGetDevice(&cur));
+        if (cur != h->device) VMAT_CUDA(cudaSetDevice(h->device));
+        cudaError_t e = cudaFuncSetAttribute(k_cs_dp, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        if (cur != h->device) cudaSetDevice(cur);
+        VMAT_CUDA(e);
+    }
     // launch order: the control points with the most sequential work first, so that the last wave is made of light ones
     std::vector<int32_t> order((size_t)(n_a > 0 ? n_a : 1), 0);
     for (int k = 0; k < n_a; ++k) order[k] = k;

@@ -220,8 +220,37 @@ def test_errors(vm):
     h3 = selection_handle(vm, [0, 2], [0, 3, 6], [0, 0])
     with pytest.raises(vm.VmatError):                               # a field range beyond 255 positions
         vm.vmat_ddc_set_leaf_geometry(h3, torch.tensor([0, 400], dtype=torch.int32))
+    with pytest.raises(vm.VmatError):                               # 256 positions: one more than the packing holds
+        vm.vmat_ddc_set_leaf_geometry(h3, torch.tensor([0, 252], dtype=torch.int32))
     for x in (h, h2, h3):
         x.close()
+
+
+def test_field_range_at_the_limit_and_two_handles(vm):
+    """A control point whose field range holds exactly 255 leaf positions (the most the 8-bit packing takes; the pair
+    (255, 255) is the kernel's 'no predecessor' mark), against O6; and a SECOND handle with short rows created and
+    used in between: the first one's launches must not be affected (the shared-memory attribute of the kernel
+    belongs to the device, not to a handle)."""
+    rng = np.random.default_rng(255)
+    n0, n1 = 100, 120
+    lco = np.array([0, n0, n0 + n1, n0 + n1 + 90], np.int32)
+    pos0 = np.array([0, 134, 60], np.int32)                        # max pos0 + n = 254 -> 255 positions
+    aro = np.array([0, 3], np.int32)
+    h = selection_handle(vm, aro, lco, pos0)
+    p = rng.integers(-3, 4, int(lco[-1])).astype(np.float32)
+    small = selection_handle(vm, [0, 2], [0, 4, 8], [0, 1])        # lowers nothing
+    ps = rng.integers(-3, 4, 8).astype(np.float32)
+    assert_same(gpu_select(vm, small, ps, True), oracle.select_constrained(ps, [0, 2], [0, 4, 8], [0, 1], True))
+    for interdig in (True, False):
+        assert_same(gpu_select(vm, h, p, interdig), oracle.select_constrained(p, aro, lco, pos0, interdig))
+    W = [np.array([0, 0, 0], np.int32), np.array([254, 254, 254], np.int32), np.array([0, 0, 0], np.int32),
+         np.array([254, 254, 254], np.int32)]                      # windows over the whole range: closed pairs park at 254
+    assert_same(gpu_select(vm, h, p, True, W=W), oracle.select_constrained(p, aro, lco, pos0, True, L_lo=W[0], L_hi=W[1],
+                                                                          R_lo=W[2], R_hi=W[3]))
+    p_pos = np.abs(p) + 1.0                                         # nothing to gain: every row closed somewhere feasible
+    assert_same(gpu_select(vm, h, p_pos, True), oracle.select_constrained(p_pos, aro, lco, pos0, True))
+    small.close()
+    h.close()
 
 
 # ---------------------------------------------------------------- leaf-travel windows and the constrained loop

@@ -286,3 +286,15 @@ def test_aperture_dose_signed_and_large_values(vm):
         assert np.array_equal(xs.cpu().numpy(), ind)
         assert np.abs(DA.cpu().numpy().astype(np.float64) - ref).max() <= 2.0 ** -23 * max(np.abs(ref).max(), 1e-30)
     h.close()
+
+
+def test_structure_id_contract_check(vm):
+    """vmat_check_structure_ids: ids must index the per-structure tables (the compute calls do not re-check)."""
+    sid = torch.tensor([0, 1, 2, 1, 0, 3], dtype=torch.uint8, device=DEV)
+    t4 = torch.ones(4, device=DEV)
+    vm.Objective(sid, t4, t4, t4).validate()
+    t3 = torch.ones(3, device=DEV)
+    with pytest.raises(vm.VmatError) as e:
+        vm.Objective(sid, t3, t3, t3).validate()
+    assert e.value.status == -2
+    vm.Objective(torch.zeros(0, dtype=torch.uint8, device=DEV), t3, t3, t3).validate()
