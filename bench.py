@@ -5,7 +5,7 @@ One "step" = one whole price evaluation (d = D x -> F, g -> p = D^T g -> leaf-ro
 control point) on a fresh fluence vector x, through the C ABI
 (`vmat_price_eval`).  Inputs are synthetic (synth/), shaped like BASELINE.json `configs`.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config {0,1,2,3}] [--scale S] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config {0,1,2,3,4}] [--scale S] [--impl reference]
 
 Prints ONE JSON line (rank 0).  Multi-GPU: the path does not need a second GPU (BASELINE.json
 north_star), so N > 1 runs N independent replicas, one process per GPU ("replicas only", weak scaling).
@@ -94,31 +94,41 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def ncu_capture_file(index_bits: int) -> str:
-    """The committed ncu --set full capture of config 3 for the layout in use (u16 offsets: v6, int32: v4)."""
-    return "r1_ncu_full_cfg3_v6.csv" if index_bits == 16 else "r1_ncu_full_cfg3_v4.csv"
+NCU_CAPTURES = ["r2_ncu_full_cfg3.csv", "r1_ncu_full_cfg3_v6.csv", "r1_ncu_full_cfg3_v4.csv"]   # newest first
 
 
-def ncu_traffic(kernel_prefix: str, cfg: int, scale: float, index_bits: int):
-    """dram bytes (read + write) per launch of the dominant kernel from the committed ncu --set full capture
-    (profiles/r1_ncu_full_cfg3_v{4,6}.csv, config 3 only); None for other workloads."""
-    if cfg != 3 or scale != 1.0:
-        return None
-    try:
-        import csv
-        rows = [r for r in csv.reader(open(os.path.join(ROOT, "profiles", ncu_capture_file(index_bits)))) if len(r) > 3]
-        hdr, units = rows[0], rows[1]
-        mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
-        for r in rows[2:]:
-            if kernel_prefix in r[hdr.index("Kernel Name")]:
+def ncu_traffic(kernel_prefix: str, grid: int, algorithmic_bytes: int):
+    """dram bytes (read + write) per launch of the dominant kernel from a committed `ncu --set full` capture under
+    profiles/ - but only from a capture of THIS launch: its grid size must equal the running handle's and its bytes
+    must lie within [0.9, 1.3] x the algorithmic bytes.  Returns (bytes or None, source or the reason for None)."""
+    import csv
+    why = "no committed ncu capture of this kernel"
+    mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    for name in NCU_CAPTURES:
+        path = os.path.join(ROOT, "profiles", name)
+        if not os.path.exists(path):
+            continue
+        try:
+            rows = [r for r in csv.reader(open(path)) if len(r) > 3]
+            hdr, units = rows[0], rows[1]
+            for r in rows[2:]:
+                if kernel_prefix not in r[hdr.index("Kernel Name")]:
+                    continue
+                g = int(r[hdr.index("Grid Size")].strip("() ").split(",")[0])
+                if g != grid:
+                    why = f"profiles/{name}: captured grid {g} != this launch's {grid} (another layout or workload)"
+                    continue
                 tot = 0.0
                 for col in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
                     i = hdr.index(col)
                     tot += float(r[i]) * mult[units[i]]
-                return tot
-    except Exception:
-        return None
-    return None
+                if not 0.9 * algorithmic_bytes <= tot <= 1.3 * algorithmic_bytes:
+                    why = f"profiles/{name}: captured {tot:.4g} B is not this launch ({algorithmic_bytes} algorithmic bytes)"
+                    continue
+                return tot, f"profiles/{name} (ncu --set full, one launch; grid {g} matches this run)"
+        except Exception as e:                                # a malformed file is a reason, not a crash
+            why = f"profiles/{name}: {e}"
+    return None, why
 
 
 def rank_eval_index(rank: int, k: int) -> int:
@@ -476,6 +486,121 @@ def run_sharded(args):
         dist.destroy_process_group()
 
 
+# ----------------------------------------------------------------------------- configs[4]: the roofline sweep
+SWEEP_SCALES = [(1e7, 3.74), (1e8, 1.546), (1e9, 0.667), (4e9, 0.4097)]      # target nnz -> scale of the config 1 generator
+
+
+def run_sweep(args):
+    """--config 4 (BASELINE.json configs[4]): the config 1 generator with voxel and beamlet size scaled so that nnz spans
+    1e7, 1e8, 1e9 and 4e9; at each size K consecutive price evaluations with x re-drawn every time; GB/s and fraction of
+    the HBM peak for the D x and the D^T g kernels separately and for the whole fused step.  One JSON line, `sweep` = one
+    entry per size; the headline value is the largest size's."""
+    import paper_1503_01721_b200 as vm
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device - the product path has no CPU fallback")
+    vm.load_library()
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("bench.py --config 4 runs on one GPU")
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+    peak, peak_src = measured_peaks()
+    K, W = args.steps, args.warmup
+    points = []
+    for target, scale in SWEEP_SCALES:
+        if args.sweep_max_nnz and target > args.sweep_max_nnz:
+            continue
+        spec = synth.config_spec(1, scale)
+        pt = {"target_nnz": target, "scale": scale, "workload": spec.name}
+        try:
+            t0 = time.time()
+            ph = synth.generate(spec, device=dev)
+            torch.cuda.synchronize()
+            pt["gen_s"] = round(time.time() - t0, 2)
+            t0 = time.time()
+            try:
+                h = vm.vmat_ddc_create(ph.n_voxels, ph.n_beamlets, ph.coo_voxel, ph.coo_beamlet, ph.coo_val,
+                                       ph.angle_col_offset, ph.angle_row_offset, ph.leafrow_col_offset, device=dev,
+                                       index_bits=args.index_bits)
+                pt["ingest"] = "COO on the device"
+            except vm.VmatError as e:
+                if e.status != -4:
+                    raise
+                # the device cannot hold the triplets next to the build's scratch: stream them from the host
+                hv, hb, hw = ph.coo_voxel.cpu(), ph.coo_beamlet.cpu(), ph.coo_val.cpu()
+                ph.coo_voxel = ph.coo_beamlet = ph.coo_val = None
+                torch.cuda.empty_cache()
+                h = vm.vmat_ddc_create(ph.n_voxels, ph.n_beamlets, hv, hb, hw, ph.angle_col_offset, ph.angle_row_offset,
+                                       ph.leafrow_col_offset, device=dev, index_bits=args.index_bits)
+                del hv, hb, hw
+                pt["ingest"] = "COO streamed from host memory (the device build ran out of memory with the triplets resident)"
+            pt["ingest_s"] = round(time.time() - t0, 2)
+            ph.coo_voxel = ph.coo_beamlet = ph.coo_val = None
+            torch.cuda.empty_cache()
+            obj = vm.Objective(ph.voxel_struct.to(dev), ph.struct_T.to(dev), ph.struct_w_over.to(dev), ph.struct_w_under.to(dev))
+            out = h.alloc_outputs()
+            n_b, n_v, nnz, n_rows = h.n_beamlets, h.n_voxels, h.nnz, h.n_leaf_rows
+            xs = [synth.draw_x(n_b, k, device=dev) for k in range(K + W)]
+            for k in range(W):
+                vm.vmat_price_eval(h, xs[k], obj, out)
+            ev_k = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
+            for evs in ev_k:
+                for e in evs:
+                    e.record()
+            start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            sampler = ClockSampler(local)
+            sampler.start()
+            time.sleep(0.25)
+            start.record()
+            for k in range(K):
+                h.set_profile_events(ev_k[k])
+                vm.vmat_price_eval(h, xs[W + k], obj, out)
+            stop.record()
+            torch.cuda.synchronize()
+            clocks = sampler.stop()
+            h.set_profile_events(None)
+            ms = start.elapsed_time(stop) / K
+            t_dose = float(np.mean([e[0].elapsed_time(e[1]) for e in ev_k]))
+            t_price = float(np.mean([e[2].elapsed_time(e[3]) for e in ev_k]))
+            info = h.info
+            B_dose = info["bytes_stream_d"] + 4 * n_b + 4 * n_v + 5 * n_v
+            B_price = info["bytes_stream_dt"] + 4 * n_v + 4 * n_b + 4 * (n_rows + 1) + 16 * n_rows
+            l2 = (B_dose + B_price) <= 4 * 126e6
+            gb = lambda b, t: b / (t * 1e-3) / 1e9
+            pt.update({"nnz": nnz, "n_voxels": n_v, "n_beamlets": n_b, "evals_per_s": 1e3 / ms, "ms_per_eval": ms,
+                       "index_bits": [info["index_bits_d"], info["index_bits_dt"]],
+                       "dose": {"ms": t_dose, "bytes": B_dose, "gbs": gb(B_dose, t_dose), "gbs_8B_csr_equiv": gb(8 * nnz, t_dose)},
+                       "price": {"ms": t_price, "bytes": B_price, "gbs": gb(B_price, t_price), "gbs_8B_csr_equiv": gb(8 * nnz, t_price)},
+                       "fused_step": {"ms": ms, "bytes": B_dose + B_price, "gbs": gb(B_dose + B_price, ms),
+                                      "gbs_8B_csr_equiv": gb(16 * nnz, ms)},
+                       "l2_resident": l2, "clocks": clocks, "F_last": float(out.F.item())})
+            if not l2:                                       # an HBM fraction only where the streams come from HBM
+                for k in ("dose", "price", "fused_step"):
+                    pt[k]["frac_of_measured"] = pt[k]["gbs"] / peak
+                    pt[k]["frac_of_8TBs"] = pt[k]["gbs"] / 8000.0
+            else:
+                pt["note"] = "L2-resident: both layouts fit the 126 MB L2; no HBM fraction is claimed"
+            h.close()
+            del out, xs, obj, ph
+        except Exception as e:                               # a size the box cannot hold is reported, not hidden
+            pt["failed"] = f"{type(e).__name__}: {e}"[:400]
+        torch.cuda.empty_cache()
+        points.append(pt)
+    ok = [p for p in points if "failed" not in p]
+    top = ok[-1] if ok else None
+    line = {"metric": METRIC, "value": top["evals_per_s"] if top else None, "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W,
+            "ms_per_step": top["ms_per_eval"] if top else None, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "cfg4-roofline-sweep (config 1 generator, scaled)", "headline_point": top["workload"] if top else None,
+                       "x": "re-drawn per evaluation, seeded Uniform[0,1)", "evaluations_per_size": K},
+            "roofline": ({"bound": "hbm", "kernel": "fused step at the largest size", "achieved": top["fused_step"]["gbs"],
+                          "peak": peak, "unit": "GB/s", "frac": top["fused_step"]["gbs"] / peak, "peak_source": peak_src,
+                          "traffic": None} if top else None),
+            "sweep": points}
+    print(json.dumps(line))
+
+
 # ----------------------------------------------------------------------------- the CUDA path, timed
 def run_ours(args):
     import paper_1503_01721_b200 as vm
@@ -605,17 +730,20 @@ def run_ours(args):
         B_price_8B = 8 * nnz + 8 * (n_b + 1) + vec_price
         B_eval = B_dose + B_price
         B_eval_8B = B_dose_8B + B_price_8B
-        k_dose = {"name": "k_dose<true> (dose + fused objective/gradient)", "ncu": "k_dose<1", "ms": float(t_dose.mean()), "ms_min": float(t_dose.min()),
+        k_dose = {"name": "k_dose<true> (dose + fused objective/gradient)", "ncu": "k_dose<1", "grid": info["grid_dose"],
+                  "ms": float(t_dose.mean()), "ms_min": float(t_dose.min()),
                   "bytes": B_dose, "gbs": B_dose / (t_dose.mean() * 1e-3) / 1e9,
                   "gbs_8B_csr_equiv": B_dose_8B / (t_dose.mean() * 1e-3) / 1e9, "index_bits": info["index_bits_d"],
                   "padded_over_nnz": info["padded_d"] / max(nnz, 1),
                   "tiles_one_base_frac": info["tiles_uniform_d"] / max(info["tiles_d"], 1)}
-        k_price = {"name": "k_price<true> (price + fused leaf-row selection)", "ncu": "k_price<1", "ms": float(t_price.mean()), "ms_min": float(t_price.min()),
+        k_price = {"name": "k_price<true> (price + fused leaf-row selection)", "ncu": "k_price<1", "grid": info["grid_price"],
+                   "ms": float(t_price.mean()), "ms_min": float(t_price.min()),
                    "bytes": B_price, "gbs": B_price / (t_price.mean() * 1e-3) / 1e9,
                    "gbs_8B_csr_equiv": B_price_8B / (t_price.mean() * 1e-3) / 1e9, "index_bits": info["index_bits_dt"],
                    "padded_over_nnz": info["padded_dt"] / max(nnz, 1),
                    "tiles_one_base_frac": info["tiles_uniform_dt"] / max(info["tiles_dt"], 1)}
         dom = k_price if k_price["ms"] >= k_dose["ms"] else k_dose
+        traffic, traffic_src = ncu_traffic(dom["ncu"], dom["grid"], dom["bytes"])
         agg = aggregate(world, K, elapsed_ms)
         ms_per_step, value = agg["ms_per_step"], agg["value"]
         eval_gbs = B_eval / (ms_per_step * 1e-3) / 1e9
@@ -639,8 +767,8 @@ def run_ours(args):
             "gpu_launches": launches,
             "roofline": {"bound": "hbm", "kernel": dom["name"], "achieved": dom["gbs"], "peak": peak,
                          "unit": "GB/s", "frac": dom["gbs"] / peak, "frac_of_8TBs": dom["gbs"] / 8000.0,
-                         "peak_source": peak_src, "traffic": ncu_traffic(dom["ncu"], args.config, args.scale, dom["index_bits"]),
-                         "traffic_source": f"profiles/{ncu_capture_file(dom['index_bits'])} (ncu --set full, one launch)", "algorithmic_bytes": dom["bytes"],
+                         "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
+                         "algorithmic_bytes": dom["bytes"],
                          "ms": dom["ms"]},
             "kernels": [k_dose, k_price],
             "result_check": {"F_last": F_last, "best_angle_last": best_last},
@@ -667,7 +795,9 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (default 3: the largest DDC)")
+    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3, 4],
+                    help="BASELINE.json config (default 3: the largest DDC; 4: the roofline sweep, one line with a `sweep` array)")
+    ap.add_argument("--sweep-max-nnz", type=float, default=0.0, help="--config 4: skip the sizes beyond this many non-zeros")
     ap.add_argument("--scale", type=float, default=1.0, help="config 4 sweep: coarsen voxels/beamlets by this factor")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--index-bits", type=int, default=0, choices=[0, 16, 32],
@@ -683,7 +813,11 @@ def main():
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
+        if args.config == 4:
+            args.config, args.scale = 1, SWEEP_SCALES[-1][1]
         run_reference(args)
+    elif args.config == 4:
+        run_sweep(args)
     elif args.parallelism == "angle-shards":
         run_sharded(args)
     else:

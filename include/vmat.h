@@ -64,6 +64,8 @@ typedef struct vmat_ddc_info {
     int64_t bytes_stream_dt;    /* bytes vmat_price streams per call: the same for D^T (no segment table) */
     int64_t tiles_d, tiles_uniform_d;        /* u16 layouts: 256-entry tiles, and those stored with ONE base     */
     int64_t tiles_dt, tiles_uniform_dt;      /* (span <= 65535) instead of one per 32-entry group; 0 for int32   */
+    int64_t grid_dose, grid_price;           /* CTAs the dose and the price kernel are launched with (bench.py checks
+                                                a stored ncu capture against them before quoting its DRAM traffic)  */
 } vmat_ddc_info;
 
 /* A0 ingest / layout build (D arrives as COO - values, voxel (row) index,

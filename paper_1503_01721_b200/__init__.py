@@ -48,7 +48,7 @@ class _Info(ctypes.Structure):
         "n_voxels", "n_beamlets", "nnz", "n_angles", "n_leaf_rows", "bytes_csr_d", "bytes_csr_dt",
         "bytes_device_total", "n_dose_blocks", "max_leaf_row_len", "max_voxel_row_nnz", "max_beamlet_row_nnz",
         "index_bits_d", "index_bits_dt", "padded_d", "padded_dt", "bytes_stream_d", "bytes_stream_dt",
-        "tiles_d", "tiles_uniform_d", "tiles_dt", "tiles_uniform_dt")]
+        "tiles_d", "tiles_uniform_d", "tiles_dt", "tiles_uniform_dt", "grid_dose", "grid_price")]
 
 
 def load_library():

@@ -295,6 +295,8 @@ int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info)
     info->bytes_stream_dt = h->Dt.bytes();
     info->tiles_d = h->D.n_tiles; info->tiles_uniform_d = h->D.n_tiles_uniform;
     info->tiles_dt = h->Dt.n_tiles; info->tiles_uniform_dt = h->Dt.n_tiles_uniform;
+    info->grid_dose = h->n_blocks;
+    info->grid_price = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
     return VMAT_OK;
 }
 
