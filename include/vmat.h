@@ -181,6 +181,20 @@ int vmat_price_eval_host(vmat_ddc *h, const float *x_host,
                          double *F_host, int32_t *L_host, int32_t *R_host, double *row_price_host,
                          double *angle_price_host, int32_t *best_angle_host, void *stream);
 
+/* The same end-to-end call, pipelined over two slots so that the host <-> device copies of one evaluation overlap the
+ * kernels of the other: _submit enqueues, for slot 0 or 1, the copy of x_host (pinned host memory) on a copy-in
+ * stream, the evaluation on `stream`, and the copies of the results into the host buffers on a copy-out stream, and
+ * returns at once; _wait blocks until that slot's host outputs are complete.  A slot must be waited for before it
+ * is submitted again; x_host and the output buffers of a slot belong to the library between _submit and _wait.
+ * The objective arguments are device pointers as in vmat_price_eval.  Results are identical to vmat_price_eval_host. */
+int vmat_price_eval_host_submit(vmat_ddc *h, int32_t slot, const float *x_host,
+                                const uint8_t *voxel_struct, int32_t n_struct,
+                                const float *T, const float *w_over, const float *w_under,
+                                const uint8_t *angle_mask,
+                                double *F_host, int32_t *L_host, int32_t *R_host, double *row_price_host,
+                                double *angle_price_host, int32_t *best_angle_host, void *stream);
+int vmat_price_eval_host_wait(vmat_ddc *h, int32_t slot);
+
 /* Aperture dose vector DA(A_k) = sum_{j in A_k} D_:j (Eq. (5)) of the aperture given by the
  * openings [L,R) of the leaf rows of control point `angle`: DA = D 1_A, on the device (the paper did
  * this on the CPU from COO, L137).  L, R dev int32 [n_leaf_rows] (as written by the selection);
@@ -313,6 +327,17 @@ int vmat_column_generation_ex(vmat_ddc *h, vmat_mp *mp, const uint8_t *voxel_str
                               int32_t *L, int32_t *R, int32_t *n_apertures_host, int32_t *angles_host, double *y_host,
                               double *F_hist_host, double *aperture_price_host, int32_t *mp_iters_host,
                               int32_t *stop_host, void *stream);
+
+/* NEXT-4 (angle shards): the A5 rule across column blocks, on the device.
+ * vmat_best_pair: this block's candidate as a pair of doubles {aperture price, control point in GLOBAL numbering}
+ *   from the outputs of vmat_price_select / vmat_price_eval on the block (angle_price dev double [n_angles of the
+ *   block], best_angle dev int32 [1], local numbering); {0.0, -1.0} when the block has no improving aperture.
+ * vmat_merge_best: the rule of A5 over n such pairs (dev double [n][2], e.g. all-gathered over the ranks): smallest
+ *   price, ties -> smallest control point, none below 0 -> {0.0, -1.0}; result in best dev double [2].
+ * Both enqueue one tiny kernel on `stream`; nothing comes to the host. */
+int vmat_best_pair(const vmat_ddc *h, const double *angle_price, const int32_t *best_angle, int32_t angle_lo,
+                   double *pair, void *stream);
+int vmat_merge_best(const double *pairs, int32_t n, double *best, void *stream);
 
 /* Profiling hook for bench.py's roofline: four CUDA events (cudaEvent_t passed as void*, any may be NULL)
  * that every following vmat_price_eval / vmat_price_eval_host on this handle records on its stream:

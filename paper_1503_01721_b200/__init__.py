@@ -33,7 +33,8 @@ EXPORTS = [
     "vmat_mp_create", "vmat_mp_destroy", "vmat_mp_reset", "vmat_mp_add_aperture", "vmat_mp_set_fluence", "vmat_mp_size",
     "vmat_mp_solve", "vmat_mp_history", "vmat_column_generation",
     "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained", "vmat_leaf_windows",
-    "vmat_column_generation_ex", "vmat_price_select", "vmat_mp_reached_voxels", "vmat_mp_pass_geometry", "vmat_check_structure_ids",
+    "vmat_column_generation_ex", "vmat_price_select", "vmat_mp_reached_voxels", "vmat_mp_pass_geometry", "vmat_check_structure_ids", "vmat_best_pair", "vmat_merge_best",
+    "vmat_price_eval_host_submit", "vmat_price_eval_host_wait",
 ]
 
 
@@ -74,6 +75,8 @@ def load_library():
     lib.vmat_price_eval.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_price_eval_host.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_aperture_dose.argtypes = [vp, i32, vp, vp, vp, vp, vp]
+    lib.vmat_price_eval_host_submit.argtypes = [vp, i32, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.vmat_price_eval_host_wait.argtypes = [vp, i32]
     lib.vmat_ddc_set_profile_events.argtypes = [vp, vp]
     f64 = ctypes.c_double
     lib.vmat_mp_create.argtypes = [ctypes.POINTER(vp), i32, i32, vp]
@@ -94,6 +97,8 @@ def load_library():
     lib.vmat_column_generation_ex.argtypes = [vp, vp, vp, i32, vp, vp, vp, i32, f64, f64, i32, f64, f64, i32, i32, i32, vp,
                                               vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_price_select.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.vmat_best_pair.argtypes = [vp, vp, vp, i32, vp, vp]
+    lib.vmat_merge_best.argtypes = [vp, i32, vp, vp]
     lib.vmat_last_error.restype = ctypes.c_char_p
     lib.vmat_last_launch_count.restype = ctypes.c_int
     for name in EXPORTS:
@@ -289,6 +294,21 @@ def vmat_price_select(h: DDC, g: torch.Tensor, out: PriceEvalOut, angle_mask: Op
         _stream()))
 
 
+def vmat_best_pair(h: DDC, out: PriceEvalOut, angle_lo: int, pair: torch.Tensor):
+    """NEXT-4: this block's candidate {aperture price, GLOBAL control point} (or {0, -1}) into pair (float64 [2], device)."""
+    _check(load_library().vmat_best_pair(h._h, _ptr(out.angle_price, torch.float64, "cuda", h.n_angles),
+                                         _ptr(out.best_angle, torch.int32, "cuda", 1), int(angle_lo),
+                                         _ptr(pair, torch.float64, "cuda", 2), _stream()))
+
+
+def vmat_merge_best(pairs: torch.Tensor, best: torch.Tensor):
+    """NEXT-4: the A5 rule over n candidate pairs (float64 [n, 2], device) into best (float64 [2], device)."""
+    n = int(pairs.numel() // 2)
+    with torch.cuda.device(pairs.device):
+        _check(load_library().vmat_merge_best(_ptr(pairs, torch.float64, "cuda", 2 * n), n,
+                                              _ptr(best, torch.float64, "cuda", 2), _stream()))
+
+
 def vmat_ddc_set_leaf_geometry(h: DDC, leafrow_pos0: torch.Tensor):
     """NEXT-3: physical column of the first beamlet of every leaf row (host int32 [n_leaf_rows])."""
     pos0 = leafrow_pos0.to(torch.int32).cpu().contiguous()
@@ -349,6 +369,24 @@ def vmat_price_eval_host(h: DDC, x_host: torch.Tensor, obj: Objective, F_host, L
         _ptr(R_host, torch.int32, "cpu", h.n_leaf_rows), _ptr(row_price_host, torch.float64, "cpu", h.n_leaf_rows),
         _ptr(angle_price_host, torch.float64, "cpu", h.n_angles), _ptr(best_angle_host, torch.int32, "cpu", 1),
         _stream()))
+
+
+def vmat_price_eval_host_submit(h: DDC, slot: int, x_host: torch.Tensor, obj: Objective, F_host, L_host, R_host,
+                                row_price_host, angle_price_host, best_angle_host, angle_mask: Optional[torch.Tensor] = None):
+    """Pipelined end-to-end call, slot 0 or 1: enqueues copy-in, evaluation and copy-out and returns at once; the host
+    tensors (pinned) belong to the library until vmat_price_eval_host_wait(h, slot) returns."""
+    _check(load_library().vmat_price_eval_host_submit(
+        h._h, int(slot), _ptr(x_host, torch.float32, "cpu", h.n_beamlets),
+        _ptr(obj.voxel_struct, torch.uint8, "cuda", h.n_voxels), obj.n_struct, _ptr(obj.T, torch.float32, "cuda"),
+        _ptr(obj.w_over, torch.float32, "cuda"), _ptr(obj.w_under, torch.float32, "cuda"),
+        _ptr(angle_mask, torch.uint8, "cuda", h.n_angles), _ptr(F_host, torch.float64, "cpu", 1),
+        _ptr(L_host, torch.int32, "cpu", h.n_leaf_rows), _ptr(R_host, torch.int32, "cpu", h.n_leaf_rows),
+        _ptr(row_price_host, torch.float64, "cpu", h.n_leaf_rows), _ptr(angle_price_host, torch.float64, "cpu", h.n_angles),
+        _ptr(best_angle_host, torch.int32, "cpu", 1), _stream()))
+
+
+def vmat_price_eval_host_wait(h: DDC, slot: int):
+    _check(load_library().vmat_price_eval_host_wait(h._h, int(slot)))
 
 
 def vmat_aperture_dose(h: DDC, angle: int, L: torch.Tensor, R: torch.Tensor, x_scratch: torch.Tensor,

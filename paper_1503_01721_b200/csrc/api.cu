@@ -162,6 +162,14 @@ int vmat_ddc_destroy(vmat_ddc *h)
                     h->leafrow_pos0, h->angle_pmin, h->angle_wd, h->row_bp_offset, h->cs_bp, h->ad_acc, h->angle_order};
     for (void *p : ptrs)
         if (p) cudaFree(p);
+    for (auto &sl : h->slot) {
+        for (void *p : {(void *)sl.x, (void *)sl.L, (void *)sl.R, (void *)sl.best, (void *)sl.row_price, (void *)sl.angle_price, (void *)sl.F})
+            if (p) cudaFree(p);
+        for (cudaEvent_t e : {sl.x_ready, sl.done, sl.out_ready})
+            if (e) cudaEventDestroy(e);
+    }
+    if (h->e2e_in) cudaStreamDestroy(h->e2e_in);
+    if (h->e2e_out) cudaStreamDestroy(h->e2e_out);
     if (h->cs_fork) cudaEventDestroy(h->cs_fork);
     if (h->cs_join) cudaEventDestroy(h->cs_join);
     if (h->cs_aux) cudaStreamDestroy(h->cs_aux);
@@ -420,6 +428,22 @@ int vmat_price_select(const vmat_ddc *h, const float *g, const uint8_t *angle_ma
     return vmat_launch_angle_price(h, row_price, angle_mask, angle_price, best_angle, st);
 }
 
+int vmat_best_pair(const vmat_ddc *h, const double *angle_price, const int32_t *best_angle, int32_t angle_lo,
+                   double *pair, void *stream)
+{
+    REQUIRE(h && best_angle && pair, "NULL argument");
+    REQUIRE(h->n_angles == 0 || angle_price, "angle_price is NULL");
+    g_vmat_launches = 0;
+    return vmat_launch_best_pair(h, angle_price, best_angle, angle_lo, pair, (cudaStream_t)stream);
+}
+
+int vmat_merge_best(const double *pairs, int32_t n, double *best, void *stream)
+{
+    REQUIRE(n >= 0 && (pairs || n == 0) && best, "NULL argument");
+    g_vmat_launches = 0;
+    return vmat_launch_merge_best(pairs, n, best, (cudaStream_t)stream);
+}
+
 int vmat_ddc_set_profile_events(vmat_ddc *h, void *const *ev)
 {
     REQUIRE(h != nullptr, "handle is NULL");
@@ -443,9 +467,11 @@ int vmat_price_eval_host(vmat_ddc *h, const float *x_host,
         const size_t nv = h->n_voxels > 0 ? h->n_voxels : 1, nb = h->n_beamlets > 0 ? h->n_beamlets : 1;
         const size_t nr = h->n_leaf_rows > 0 ? h->n_leaf_rows : 1, na = h->n_angles > 0 ? h->n_angles : 1;
         VMAT_CUDA(cudaMalloc((void **)&h->e2e_x, nb * 4));
-        VMAT_CUDA(cudaMalloc((void **)&h->e2e_p, nb * 4));
-        VMAT_CUDA(cudaMalloc((void **)&h->e2e_d, nv * 4));
-        VMAT_CUDA(cudaMalloc((void **)&h->e2e_g, nv * 4));
+        if (!h->e2e_d) {
+            VMAT_CUDA(cudaMalloc((void **)&h->e2e_p, nb * 4));
+            VMAT_CUDA(cudaMalloc((void **)&h->e2e_d, nv * 4));
+            VMAT_CUDA(cudaMalloc((void **)&h->e2e_g, nv * 4));
+        }
         VMAT_CUDA(cudaMalloc((void **)&h->e2e_L, nr * 4));
         VMAT_CUDA(cudaMalloc((void **)&h->e2e_R, nr * 4));
         VMAT_CUDA(cudaMalloc((void **)&h->e2e_row_price, nr * 8));
@@ -468,6 +494,80 @@ int vmat_price_eval_host(vmat_ddc *h, const float *x_host,
     VMAT_CUDA(cudaMemcpyAsync(best_angle_host, h->e2e_best, 4, cudaMemcpyDeviceToHost, st));
     VMAT_CUDA(cudaMemcpyAsync(F_host, h->e2e_F, 8, cudaMemcpyDeviceToHost, st));
     VMAT_CUDA(cudaStreamSynchronize(st));
+    return VMAT_OK;
+}
+
+int vmat_price_eval_host_submit(vmat_ddc *h, int32_t slot, const float *x_host,
+                                const uint8_t *voxel_struct, int32_t n_struct,
+                                const float *T, const float *w_over, const float *w_under,
+                                const uint8_t *angle_mask,
+                                double *F_host, int32_t *L_host, int32_t *R_host, double *row_price_host,
+                                double *angle_price_host, int32_t *best_angle_host, void *stream)
+{
+    REQUIRE(h && F_host && best_angle_host, "NULL argument");
+    REQUIRE(slot == 0 || slot == 1, "slot must be 0 or 1");
+    REQUIRE(h->n_beamlets == 0 || x_host, "x_host is NULL");
+    REQUIRE(h->n_leaf_rows == 0 || (L_host && R_host && row_price_host), "NULL leaf-row output");
+    REQUIRE(h->n_angles == 0 || angle_price_host, "angle_price_host is NULL");
+    REQUIRE(!h->slot[slot].in_flight, "the slot is still in flight: call vmat_price_eval_host_wait first");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nv = h->n_voxels > 0 ? h->n_voxels : 1, nb = h->n_beamlets > 0 ? h->n_beamlets : 1;
+    const size_t nr = h->n_leaf_rows > 0 ? h->n_leaf_rows : 1, na = h->n_angles > 0 ? h->n_angles : 1;
+    if (!h->e2e_in) {                                     // streams, events and device scratch, allocated once
+        VMAT_CUDA(cudaStreamCreateWithFlags(&h->e2e_in, cudaStreamNonBlocking));
+        VMAT_CUDA(cudaStreamCreateWithFlags(&h->e2e_out, cudaStreamNonBlocking));
+        if (!h->e2e_d) {
+            VMAT_CUDA(cudaMalloc((void **)&h->e2e_d, nv * 4));
+            VMAT_CUDA(cudaMalloc((void **)&h->e2e_g, nv * 4));
+            VMAT_CUDA(cudaMalloc((void **)&h->e2e_p, nb * 4));
+            h->bytes_device += (int64_t)(8 * nv + 4 * nb);
+        }
+        for (auto &s : h->slot) {
+            VMAT_CUDA(cudaMalloc((void **)&s.x, nb * 4));
+            VMAT_CUDA(cudaMalloc((void **)&s.L, nr * 4));
+            VMAT_CUDA(cudaMalloc((void **)&s.R, nr * 4));
+            VMAT_CUDA(cudaMalloc((void **)&s.row_price, nr * 8));
+            VMAT_CUDA(cudaMalloc((void **)&s.angle_price, na * 8));
+            VMAT_CUDA(cudaMalloc((void **)&s.best, 4));
+            VMAT_CUDA(cudaMalloc((void **)&s.F, 8));
+            VMAT_CUDA(cudaEventCreateWithFlags(&s.x_ready, cudaEventDisableTiming));
+            VMAT_CUDA(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
+            VMAT_CUDA(cudaEventCreateWithFlags(&s.out_ready, cudaEventDisableTiming));
+            h->bytes_device += (int64_t)(4 * nb + 16 * nr + 8 * na + 12);
+        }
+    }
+    vmat_ddc::E2ESlot &s = h->slot[slot];
+    // x of this slot was last read by the evaluation submitted two calls ago: its `done` event has long fired
+    // (that slot was waited for), so the copy-in stream may overwrite it now
+    if (h->n_beamlets > 0)
+        VMAT_CUDA(cudaMemcpyAsync(s.x, x_host, (size_t)h->n_beamlets * 4, cudaMemcpyHostToDevice, h->e2e_in));
+    VMAT_CUDA(cudaEventRecord(s.x_ready, h->e2e_in));
+    VMAT_CUDA(cudaStreamWaitEvent(st, s.x_ready, 0));
+    TRY(vmat_price_eval(h, s.x, voxel_struct, n_struct, T, w_over, w_under, angle_mask, h->e2e_d, h->e2e_g, s.F, h->e2e_p,
+                        s.L, s.R, s.row_price, s.angle_price, s.best, st));
+    VMAT_CUDA(cudaEventRecord(s.done, st));
+    VMAT_CUDA(cudaStreamWaitEvent(h->e2e_out, s.done, 0));
+    if (h->n_leaf_rows > 0) {
+        VMAT_CUDA(cudaMemcpyAsync(L_host, s.L, (size_t)h->n_leaf_rows * 4, cudaMemcpyDeviceToHost, h->e2e_out));
+        VMAT_CUDA(cudaMemcpyAsync(R_host, s.R, (size_t)h->n_leaf_rows * 4, cudaMemcpyDeviceToHost, h->e2e_out));
+        VMAT_CUDA(cudaMemcpyAsync(row_price_host, s.row_price, (size_t)h->n_leaf_rows * 8, cudaMemcpyDeviceToHost, h->e2e_out));
+    }
+    if (h->n_angles > 0)
+        VMAT_CUDA(cudaMemcpyAsync(angle_price_host, s.angle_price, (size_t)h->n_angles * 8, cudaMemcpyDeviceToHost, h->e2e_out));
+    VMAT_CUDA(cudaMemcpyAsync(best_angle_host, s.best, 4, cudaMemcpyDeviceToHost, h->e2e_out));
+    VMAT_CUDA(cudaMemcpyAsync(F_host, s.F, 8, cudaMemcpyDeviceToHost, h->e2e_out));
+    VMAT_CUDA(cudaEventRecord(s.out_ready, h->e2e_out));
+    s.in_flight = true;
+    return VMAT_OK;
+}
+
+int vmat_price_eval_host_wait(vmat_ddc *h, int32_t slot)
+{
+    REQUIRE(h != nullptr, "handle is NULL");
+    REQUIRE(slot == 0 || slot == 1, "slot must be 0 or 1");
+    if (!h->slot[slot].in_flight) return VMAT_OK;
+    VMAT_CUDA(cudaEventSynchronize(h->slot[slot].out_ready));
+    h->slot[slot].in_flight = false;
     return VMAT_OK;
 }
 

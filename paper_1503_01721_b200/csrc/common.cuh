@@ -118,6 +118,16 @@ struct vmat_ddc {
     float *e2e_x = nullptr, *e2e_d = nullptr, *e2e_g = nullptr, *e2e_p = nullptr;
     int32_t *e2e_L = nullptr, *e2e_R = nullptr, *e2e_best = nullptr;
     double *e2e_row_price = nullptr, *e2e_angle_price = nullptr, *e2e_F = nullptr;
+    // the two-slot pipelined host call (vmat_price_eval_host_submit / _wait): per slot the device copy of x and of the
+    // results, and the events that order copy-in stream -> caller's stream -> copy-out stream
+    struct E2ESlot {
+        float *x = nullptr;
+        int32_t *L = nullptr, *R = nullptr, *best = nullptr;
+        double *row_price = nullptr, *angle_price = nullptr, *F = nullptr;
+        cudaEvent_t x_ready = nullptr, done = nullptr, out_ready = nullptr;
+        bool in_flight = false;
+    } slot[2];
+    cudaStream_t e2e_in = nullptr, e2e_out = nullptr;
 };
 
 // ------------------------------------------------------------------ tuning constants
@@ -219,6 +229,9 @@ int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *a
 int vmat_launch_price_unoccupied(const vmat_ddc *h, const float *g, const uint8_t *angle_mask, float *p, cudaStream_t st);
 int vmat_launch_angle_price(const vmat_ddc *h, const double *row_price, const uint8_t *angle_mask,
                             double *angle_price, int32_t *best_angle, cudaStream_t st);
+int vmat_launch_best_pair(const vmat_ddc *h, const double *angle_price, const int32_t *best_angle, int32_t angle_lo,
+                          double *pair, cudaStream_t st);
+int vmat_launch_merge_best(const double *pairs, int32_t n, double *best, cudaStream_t st);
 int vmat_launch_select_constrained(vmat_ddc *h, const float *p, const uint8_t *angle_mask, int interdigitation,
                                    const int32_t *L_lo, const int32_t *L_hi, const int32_t *R_lo, const int32_t *R_hi,
                                    int32_t *L, int32_t *R, double *row_price, double *angle_price, int32_t *best_angle,

@@ -590,7 +590,10 @@ int vmat_ddc_set_leaf_geometry(vmat_ddc *h, const int32_t *leafrow_pos0)
         int cur = 0;
         VMAT_CUDA(cudaGetDevice(&cur));
         if (cur != h->device) VMAT_CUDA(cudaSetDevice(h->device));
-        cudaError_t e = cudaFuncSetAttribute(k_cs_dp, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+        cudaFuncAttributes fa;
+        cudaError_t e = cudaFuncGetAttributes(&fa, k_cs_dp);      // the opt-in maximum covers static + dynamic
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k_cs_dp, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - (int)fa.sharedSizeBytes);
         if (cur != h->device) cudaSetDevice(cur);
         VMAT_CUDA(e);
     }

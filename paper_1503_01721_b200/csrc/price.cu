@@ -270,6 +270,41 @@ k_angle_price(int n_angles, const int32_t *__restrict__ angle_row_offset, const 
     }
 }
 
+// ---------------------------------------------------------------- A5 across column blocks (NEXT-4)
+__global__ void k_best_pair(int n_angles, const double *__restrict__ angle_price, const int32_t *__restrict__ best_angle,
+                            int angle_lo, double *__restrict__ pair)
+{
+    const int b = best_angle[0];
+    const bool ok = b >= 0 && b < n_angles;
+    pair[0] = ok ? angle_price[b] : 0.0;
+    pair[1] = ok ? (double)(b + angle_lo) : -1.0;
+}
+// smaller price wins, ties -> smaller control point; a pair without a control point (-1) never wins (L56)
+__global__ void k_merge_best(const double *__restrict__ pairs, int n, double *__restrict__ best)
+{
+    double bp = 0.0, bk = -1.0;
+    for (int i = 0; i < n; ++i) {
+        const double p = pairs[2 * i], k = pairs[2 * i + 1];
+        if (k >= 0.0 && (p < bp || (p == bp && bk >= 0.0 && k < bk))) { bp = p; bk = k; }
+    }
+    best[0] = bp;
+    best[1] = bk;
+}
+
+int vmat_launch_best_pair(const vmat_ddc *h, const double *angle_price, const int32_t *best_angle, int32_t angle_lo,
+                          double *pair, cudaStream_t st)
+{
+    k_best_pair<<<1, 1, 0, st>>>(h->n_angles, angle_price, best_angle, angle_lo, pair);
+    VMAT_LAUNCH_CHECK();
+    return VMAT_OK;
+}
+int vmat_launch_merge_best(const double *pairs, int32_t n, double *best, cudaStream_t st)
+{
+    k_merge_best<<<1, 1, 0, st>>>(pairs, n, best);
+    VMAT_LAUNCH_CHECK();
+    return VMAT_OK;
+}
+
 // ---------------------------------------------------------------- launchers
 template <bool SELECT, bool SKIP = false>
 static void launch_k_price(const vmat_ddc *h, int grid, const float *g, float *p, const SelectArgs &sa, cudaStream_t st)

@@ -13,7 +13,9 @@ holds both layouts of its block.  One evaluation:
 In the paper this exchange is the broadcast of z over a P2P tree and the gather of the prices to GPU 1 (L127);
 here it is NCCL over NVLink (a 5 MB all-reduce next to two kernels that stream tens of GB).  Everything numerical runs
 in the library's kernels; this module only partitions the control points, re-bases the offset tables and calls
-torch.distributed.  With no process group (one rank) the collectives are skipped and the result is the unsharded one.
+torch.distributed; the A5 rule over the gathered candidates runs on the device too (vmat_best_pair, vmat_merge_best), so
+an evaluation never synchronises with the host.  With no process group (one rank) the collectives are skipped and the
+result is the unsharded one.
 
 `north_star` fixes one GPU for the hot path, so the bench's default for N > 1 stays "replicas only"; this path is for
 matrices beyond one GPU (`bench.py --parallelism angle-shards`).
@@ -25,7 +27,8 @@ from typing import List, Optional, Sequence
 
 import torch
 
-from . import DDC, Objective, PriceEvalOut, vmat_ddc_create, vmat_dose, vmat_objective_grad, vmat_price_select
+from . import (DDC, Objective, PriceEvalOut, vmat_best_pair, vmat_ddc_create, vmat_dose, vmat_merge_best,
+               vmat_objective_grad, vmat_price_select)
 
 
 def partition_angles(weight_per_angle: Sequence[float], world: int) -> List[int]:
@@ -70,38 +73,32 @@ def local_block(angle_col_offset: torch.Tensor, angle_row_offset: torch.Tensor, 
                       (lco[r0:r1 + 1] - b0).to(torch.int32))
 
 
-def pick_best(pairs) -> tuple:
-    """The rule of A5 over (price, global control point) pairs, one per rank (control point -1 = that rank has no
-    improving aperture): smallest price, ties -> smallest control point, none -> (-1, 0.0)."""
-    best, best_price = -1, 0.0
-    for price, k in pairs:
-        k = int(k)
-        if k >= 0 and (price < best_price or (price == best_price and best >= 0 and k < best)):
-            best, best_price = k, float(price)
-    return best, best_price
-
-
-def merge_best(local_best, local_price, angle_lo: int, group=None):
-    """Best control point over all ranks from every rank's best one.  `local_best` (local numbering, -1 = none) and
-    `local_price` are Python numbers or one-element tensors (on the device of the process group's backend: CUDA for
-    NCCL, CPU for gloo); one all-gather of two doubles per rank, one copy to the host.  Returns (global control point
-    or -1, its price or 0.0)."""
+def gather_pairs(pair: torch.Tensor, group=None) -> torch.Tensor:
+    """All-gather of one candidate pair {aperture price, global control point} (float64 [2]) per rank -> [world, 2] on
+    the pair's device (CUDA for NCCL, CPU for gloo).  Communication only; one rank without a process group: [1, 2]."""
     import torch.distributed as dist
-    lb = local_best if torch.is_tensor(local_best) else torch.tensor([int(local_best)])
-    lb = lb.reshape(1).to(torch.int64)
-    lp = local_price if torch.is_tensor(local_price) else torch.tensor([float(local_price)], dtype=torch.float64)
-    lp = lp.reshape(1).to(device=lb.device, dtype=torch.float64)
-    valid = lb >= 0
-    pair = torch.cat([torch.where(valid, lp, torch.zeros_like(lp)),
-                      torch.where(valid, lb + angle_lo, torch.full_like(lb, -1)).to(torch.float64)])
     if group is None and not (dist.is_available() and dist.is_initialized()):
-        pairs = pair.reshape(1, 2)
-    else:
-        world = dist.get_world_size(group)
-        pairs = torch.empty(world * 2, dtype=torch.float64, device=pair.device)
-        dist.all_gather_into_tensor(pairs, pair, group=group)
-        pairs = pairs.reshape(world, 2)
-    return pick_best(pairs.cpu().tolist())
+        return pair.reshape(1, 2)
+    world = dist.get_world_size(group)
+    pairs = torch.empty(world * 2, dtype=torch.float64, device=pair.device)
+    dist.all_gather_into_tensor(pairs, pair.contiguous(), group=group)
+    return pairs.reshape(world, 2)
+
+
+def merge_best(pair: torch.Tensor, group=None) -> torch.Tensor:
+    """Best control point over all ranks from every rank's candidate pair (device float64 [2], from vmat_best_pair):
+    one all-gather, then the A5 rule on the device (vmat_merge_best).  Returns a device float64 [2] = {price, global
+    control point or -1}; nothing comes to the host."""
+    pairs = gather_pairs(pair, group)
+    best = torch.empty(2, dtype=torch.float64, device=pair.device)
+    vmat_merge_best(pairs.contiguous(), best)
+    return best
+
+
+def best_to_host(best: torch.Tensor) -> tuple:
+    """(global control point or -1, its aperture price) from the device pair; this is the synchronising read."""
+    p, k = best.cpu().tolist()
+    return int(k), float(p)
 
 
 class ShardedDDC:
@@ -111,6 +108,7 @@ class ShardedDDC:
         self.h, self.block, self.group = handle, block, group
         self.n_angles_total, self.n_beamlets_total = n_angles_total, n_beamlets_total
         self.n_voxels = handle.n_voxels
+        self._pair = None
 
     @classmethod
     def create(cls, n_voxels: int, n_beamlets: int, coo_voxel: torch.Tensor, coo_beamlet: torch.Tensor,
@@ -136,20 +134,18 @@ class ShardedDDC:
     def price_eval(self, x_local: torch.Tensor, obj: Objective, out: PriceEvalOut,
                    angle_mask_local: Optional[torch.Tensor] = None):
         """One evaluation; `x_local` and the beamlet / leaf-row / control-point outputs in `out` are this rank's block
-        (local numbering), d, g and F are the global ones.  Returns (best control point in global numbering or -1, its
-        aperture price) after the second exchange (this synchronises the stream: two scalars come to the host)."""
+        (local numbering), d, g and F are the global ones.  Returns a device float64 [2] = {aperture price, best control
+        point in global numbering or -1} after the second exchange; no host synchronisation (`best_to_host` reads it)."""
         dist = self._dist()
         vmat_dose(self.h, x_local, out.d)
         if dist is not None:
             dist.all_reduce(out.d, op=dist.ReduceOp.SUM, group=self.group)          # d = sum_m D_m x_m
         vmat_objective_grad(self.h, out.d, obj, out.g, out.F)
         vmat_price_select(self.h, out.g, out, angle_mask_local)
-        lb = out.best_angle.to(torch.int64)                                            # stays on the device until the merge
-        if self.h.n_angles > 0:
-            lp = out.angle_price[lb.clamp(min=0)]
-        else:
-            lp = torch.zeros(1, dtype=torch.float64, device=lb.device)
-        return merge_best(lb, lp, self.block.angle_lo, self.group)
+        if self._pair is None:
+            self._pair = torch.empty(2, dtype=torch.float64, device=out.d.device)
+        vmat_best_pair(self.h, out, self.block.angle_lo, self._pair)
+        return merge_best(self._pair, self.group)
 
     def close(self):
         self.h.close()

@@ -1,5 +1,5 @@
 """Worker of test_sharded_host_logic.py: the host logic of the angle-sharded evaluation (paper_1503_01721_b200/sharded.py:
-partition, re-based offset tables, the all-reduce of the dose, the merge of the best control points) under
+partition, re-based offset tables, the all-reduce of the dose, the all-gather of the candidate control points) under
 torch.distributed.run with gloo.  No GPU here, so every rank's kernels are stood in for by the oracle applied to the
 rank's own column block - which is exactly the angle-block additivity of PAPER.md L119 (pin P6)."""
 import json
@@ -35,7 +35,12 @@ F, g = oracle.objective_grad(d.numpy(), sid, T, wo, wu)
 p = oracle.price(vox[keep], lbeam, val[keep], n_b_local, g)
 L, R, rp = oracle.select_rows(p.astype(np.float32), blk.leafrow_col_offset.numpy())
 ap, lbest = oracle.angle_price(rp, blk.angle_row_offset.numpy())
-best, best_price = sharded.merge_best(lbest, ap[lbest] if lbest >= 0 else 0.0, blk.angle_lo)
+# every rank's candidate {price, global control point}; the exchange is sharded.gather_pairs; the A5 rule over the
+# gathered candidates (vmat_merge_best on a GPU) is stood in for by the oracle's O5 with one "control point" per rank
+pair = torch.tensor([ap[lbest] if lbest >= 0 else 0.0, float(lbest + blk.angle_lo) if lbest >= 0 else -1.0], dtype=torch.float64)
+pairs = sharded.gather_pairs(pair).numpy()
+_, win = oracle.angle_price(pairs[:, 0].copy(), np.arange(world + 1, dtype=np.int32))
+best, best_price = (int(pairs[win, 1]), float(pairs[win, 0])) if win >= 0 else (-1, 0.0)
 # the unsharded evaluation
 ev = oracle.price_eval(vox, beam, val, ph.n_voxels, ph.n_beamlets, x, sid, T, wo, wu, lco.numpy(), aro.numpy())
 res = {

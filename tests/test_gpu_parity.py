@@ -232,6 +232,40 @@ def test_host_buffer_call_matches_device_call(vm, A0, h0):
     assert torch.equal(rp, out.row_price.cpu()) and torch.equal(ap, out.angle_price.cpu())
 
 
+def test_pipelined_host_call_matches_the_device_call(vm, A0, h0):
+    """vmat_price_eval_host_submit / _wait: seven evaluations through the two slots, every result equal to the device
+    call's bit for bit; a slot in flight refuses a second submit."""
+    obj = obj_to_device(A0, DEV)
+    xs = [_x(A0["n_b"], 40 + k, (1.0, 8.0, 14.0, 16.0)[k % 4]) for k in range(7)]
+    refs = []
+    for x in xs:
+        o = _eval_gpu(vm, h0, A0, x)
+        refs.append({f: getattr(o, f).cpu().clone() for f in ("F", "L", "R", "row_price", "angle_price", "best_angle")})
+    pin = lambda n, dt: torch.empty(n, dtype=dt).pin_memory()
+    hb = [dict(F=pin(1, torch.float64), L=pin(h0.n_leaf_rows, torch.int32), R=pin(h0.n_leaf_rows, torch.int32),
+               rp=pin(h0.n_leaf_rows, torch.float64), ap=pin(h0.n_angles, torch.float64), b=pin(1, torch.int32)) for _ in range(2)]
+    xh = [x.pin_memory() for x in xs]
+
+    def check(k):
+        o, r = hb[k % 2], refs[k]
+        vm.vmat_price_eval_host_wait(h0, k % 2)
+        assert o["F"].item() == r["F"].item() and o["b"].item() == r["best_angle"].item(), k
+        assert torch.equal(o["L"], r["L"]) and torch.equal(o["R"], r["R"]), k
+        assert torch.equal(o["rp"], r["row_price"]) and torch.equal(o["ap"], r["angle_price"]), k
+
+    for k in range(7):
+        if k >= 2:
+            check(k - 2)
+        o = hb[k % 2]
+        vm.vmat_price_eval_host_submit(h0, k % 2, xh[k], obj, o["F"], o["L"], o["R"], o["rp"], o["ap"], o["b"])
+    with pytest.raises(vm.VmatError, match="in flight"):
+        o = hb[0]
+        vm.vmat_price_eval_host_submit(h0, 0, xh[0], obj, o["F"], o["L"], o["R"], o["rp"], o["ap"], o["b"])
+    check(5)
+    check(6)
+    vm.vmat_price_eval_host_wait(h0, 0)                          # waiting for an idle slot is a no-op
+
+
 def test_aperture_dose(vm, A0, h0):
     """NEXT-1, Eq. (5): DA = sum of the columns of the beamlets inside the chosen aperture."""
     x = _x(A0["n_b"], 26, 14.0)

@@ -65,14 +65,17 @@ def test_blocks_add_up_to_the_unsharded_evaluation(vm, cfg0, n_shards, scale):
         assert np.array_equal(o.row_price.cpu().numpy(), rp) and np.array_equal(o.angle_price.cpu().numpy(), ap)
         assert int(o.best_angle.item()) == lbest
         assert np.array_equal(L, ev.L[b.row_lo:b.row_hi]) and np.array_equal(R, ev.R[b.row_lo:b.row_hi])
-        cands.append((lbest, float(ap[lbest]) if lbest >= 0 else 0.0, b.angle_lo))
-    # the merge rule over the blocks (what merge_best does with the gathered pairs)
-    best, price = -1, 0.0
-    for lb, lp, lo in cands:
-        k, pr = sharded.merge_best(lb, lp, lo)
-        if k >= 0 and (pr < price or (pr == price and best >= 0 and k < best)):
-            best, price = k, pr
-    assert best == ev.best_angle
+        pair = torch.empty(2, dtype=torch.float64, device=DEV)
+        vm.vmat_best_pair(s.h, o, b.angle_lo, pair)                   # {price, global control point} or {0, -1}
+        assert pair.tolist() == ([float(ap[lbest]), float(lbest + b.angle_lo)] if lbest >= 0 else [0.0, -1.0])
+        cands.append(pair)
+    # the A5 rule over the blocks' candidates, on the device (what merge_best runs on the all-gathered pairs)
+    best = torch.empty(2, dtype=torch.float64, device=DEV)
+    vm.vmat_merge_best(torch.stack(cands).contiguous(), best)
+    k, price = sharded.best_to_host(best)
+    assert k == ev.best_angle
+    if k >= 0:
+        assert abs(price - ev.angle_price[k]) <= 1e-4 * abs(ev.angle_price[k])
     for s in shards:
         s.close()
 
@@ -86,9 +89,36 @@ def test_one_block_is_the_unsharded_call(vm, cfg0):
     vm.vmat_price_eval(h, x, obj, ref)
     _, (s,) = _shards(cfg0, A, 1)
     out = s.h.alloc_outputs()
-    best, price = s.price_eval(x, obj, out)
+    from paper_1503_01721_b200 import sharded
+    best, price = sharded.best_to_host(s.price_eval(x, obj, out))
     for name in ("d", "g", "F", "p", "L", "R", "row_price", "angle_price", "best_angle"):
         assert torch.equal(getattr(out, name), getattr(ref, name)), name
     assert best == int(ref.best_angle.item()) and price == float(ref.angle_price[best].item())
     s.close()
     h.close()
+
+
+def test_merge_rule_on_the_device(vm):
+    """vmat_merge_best against hand-worked candidate lists: smallest price, ties -> smallest control point, candidates
+    without a control point never win, none below 0 -> {0, -1}."""
+    cases = [([[-1.0, 7.0], [-3.0, 2.0], [-3.0, 1.0]], [-3.0, 1.0]), ([[0.0, -1.0], [-0.5, 9.0]], [-0.5, 9.0]),
+             ([[0.0, -1.0], [0.0, -1.0]], [0.0, -1.0]), ([[-2.0, 5.0]], [-2.0, 5.0]), ([[-2.0, 5.0], [-2.0, 3.0], [0.0, -1.0]], [-2.0, 3.0])]
+    for pairs, want in cases:
+        best = torch.empty(2, dtype=torch.float64, device=DEV)
+        vm.vmat_merge_best(torch.tensor(pairs, dtype=torch.float64, device=DEV), best)
+        assert best.tolist() == want
+
+
+def test_collective_path_on_one_gpu_with_nccl(tmp_path):
+    """ShardedDDC.price_eval through a REAL torch.distributed process group of world size 1 with the nccl backend: the
+    all-reduce of the dose and the all-gather of the candidates run (not the no-process-group bypass), and the result
+    is the unsharded call bit for bit (tests/_nccl1_worker.py)."""
+    import json, os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29593", RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, os.path.join(root, "tests", "_nccl1_worker.py")], cwd=root, env=env,
+                       capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-3000:]
+    res = json.loads([ln for ln in r.stdout.splitlines() if ln.startswith("{")][-1])
+    assert res["backend"] == "nccl" and res["world"] == 1 and res["collectives_ran"] >= 2
+    assert res["equal"] and res["best"] == res["best_ref"] and res["price"] == res["price_ref"]

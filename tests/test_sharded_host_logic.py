@@ -45,9 +45,9 @@ def test_local_block_rebases_the_offset_tables():
     assert e.angle_col_offset.tolist() == [0, 0] and e.leafrow_col_offset.tolist() == [0]
 
 
-def test_merge_best_without_a_process_group():
-    assert sharded.merge_best(3, -2.5, 10) == (13, -2.5)
-    assert sharded.merge_best(-1, 0.0, 10) == (-1, 0.0)
+def test_gather_pairs_without_a_process_group():
+    pair = torch.tensor([-2.5, 13.0], dtype=torch.float64)
+    assert sharded.gather_pairs(pair).tolist() == [[-2.5, 13.0]]
 
 
 @pytest.mark.parametrize("xscale", ["14", "1"])
