@@ -7,6 +7,8 @@
 #include <stdlib.h>
 #include <new>
 #include <vector>
+#include <algorithm>
+#include <utility>
 
 static thread_local char g_err[512] = "";
 thread_local int g_vmat_launches = 0;
@@ -159,7 +161,8 @@ int vmat_ddc_destroy(vmat_ddc *h)
                     h->angle_row_offset, h->leafrow_col_offset, h->leafrow_angle, h->seg_row, h->F_partial,
                     h->F_partial_obj, h->S_scratch, h->beamlet_leafrow, h->leafrow_done, h->e2e_x, h->e2e_d, h->e2e_g, h->e2e_p, h->e2e_L, h->e2e_R,
                     h->e2e_best, h->e2e_row_price, h->e2e_angle_price, h->e2e_F,
-                    h->leafrow_pos0, h->angle_pmin, h->angle_wd, h->row_bp_offset, h->cs_bp, h->ad_acc, h->angle_order};
+                    h->leafrow_pos0, h->angle_pmin, h->angle_wd, h->row_bp_offset, h->cs_bp, h->ad_acc, h->angle_order,
+                    h->col_perm, h->x_perm};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     for (auto &sl : h->slot) {
@@ -227,7 +230,40 @@ int vmat_ddc_create_ex(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int
     h->h_angle_row_offset.assign(angle_row_offset, angle_row_offset + n_angles + 1);
     h->h_angle_col_offset.assign(angle_col_offset, angle_col_offset + n_angles + 1);
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = vmat_build_layouts(h, coo_voxel, coo_beamlet, coo_val, index_bits, st);
+    int rc = VMAT_OK;
+    {   // column order of CSR(D): per control point, tiles of COL_TILE columns x all leaf rows (common.cuh)
+#ifndef VMAT_COL_TILE
+#define VMAT_COL_TILE 8
+#endif
+        constexpr int COL_TILE = VMAT_COL_TILE;               // 8 floats = one 32-byte sector of x
+        std::vector<int32_t> perm((size_t)(n_beamlets > 0 ? n_beamlets : 1), 0);
+        bool identity = true;
+        for (int a = 0; a < n_angles; ++a) {
+            const int ra = angle_row_offset[a], rb = angle_row_offset[a + 1];
+            int32_t nxt = angle_col_offset[a], longest = 0;
+            for (int r = ra; r < rb; ++r)
+                longest = std::max(longest, leafrow_col_offset[r + 1] - leafrow_col_offset[r]);
+            for (int c0 = 0; c0 < longest; c0 += COL_TILE)
+                for (int r = ra; r < rb; ++r) {
+                    const int j0 = leafrow_col_offset[r], n = leafrow_col_offset[r + 1] - j0;
+                    for (int c = c0; c < std::min(c0 + COL_TILE, n); ++c) {
+                        identity = identity && nxt == j0 + c;
+                        perm[j0 + c] = nxt++;
+                    }
+                }
+        }
+        if (!identity && n_beamlets > 0) {
+            h->h_col_inv.assign((size_t)n_beamlets, 0);
+            for (int j = 0; j < n_beamlets; ++j) h->h_col_inv[perm[j]] = j;
+            rc = upload(&h->col_perm, perm.data(), (int64_t)n_beamlets, &h->bytes_device);
+            if (rc == VMAT_OK) {
+                cudaError_t e = cudaMalloc((void **)&h->x_perm, (size_t)n_beamlets * 4);
+                if (e != cudaSuccess) { vmat_set_error("vmat_ddc_create: cudaMalloc(x_perm) failed"); rc = VMAT_ERR_OOM; }
+                h->bytes_device += (int64_t)n_beamlets * 4;
+            }
+        }
+    }
+    if (rc == VMAT_OK) rc = vmat_build_layouts(h, coo_voxel, coo_beamlet, coo_val, index_bits, st);
     if (rc == VMAT_OK) rc = upload(&h->angle_col_offset, angle_col_offset, (int64_t)n_angles + 1, &h->bytes_device);
     if (rc == VMAT_OK) rc = upload(&h->angle_row_offset, angle_row_offset, (int64_t)n_angles + 1, &h->bytes_device);
     if (rc == VMAT_OK) rc = upload(&h->leafrow_col_offset, leafrow_col_offset, (int64_t)n_rows + 1, &h->bytes_device);
@@ -347,6 +383,13 @@ int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx
                 idx[o] = c; val[o] = pv[sp]; prev = c; ++o;
             }
             if (o != ptr[r + 1]) { vmat_set_error("vmat_ddc_export_csr: layout inconsistent (row %d)", r); return VMAT_ERR_CUDA; }
+            if (which == 0 && !h->h_col_inv.empty()) {                // back to the caller's beamlet numbers, ascending
+                const int64_t a = ptr[r], n = ptr[r + 1] - a;
+                std::vector<std::pair<int32_t, float>> row((size_t)n);
+                for (int64_t i = 0; i < n; ++i) row[(size_t)i] = {h->h_col_inv[idx[a + i]], val[a + i]};
+                std::sort(row.begin(), row.end(), [](const std::pair<int32_t, float> &x, const std::pair<int32_t, float> &y) { return x.first < y.first; });
+                for (int64_t i = 0; i < n; ++i) { idx[a + i] = row[(size_t)i].first; val[a + i] = row[(size_t)i].second; }
+            }
         }
     }
     return VMAT_OK;

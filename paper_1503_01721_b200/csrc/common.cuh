@@ -73,6 +73,12 @@ struct vmat_ddc {
     int64_t nnz = 0;
     PackedLayout D;    // rows = voxels,   secondary index = beamlet   (for d = D x)
     PackedLayout Dt;   // rows = beamlets, secondary index = voxel     (for p = D^T g; the paper's format, L121)
+    // Column order of CSR(D) (dose.cu): within a control point the beamlets are renumbered in tiles of 8 columns x all
+    // leaf rows, so that the ~8 x 8 patch of beamlets a voxel sees at one control point lies in few 128-byte lines of
+    // x.  NULL = identity (every leaf row fits one tile).  D^T, p, x at the boundary keep the caller's numbering.
+    int32_t *col_perm = nullptr;            // [n_beamlets] caller's beamlet -> position in x_perm / secondary index of D
+    float *x_perm = nullptr;                // [n_beamlets] x in that order, refilled by every dose launch
+    std::vector<int32_t> h_col_inv;         // host: position -> caller's beamlet (export undoes the renumbering)
     // offset tables (device)
     int32_t *angle_col_offset = nullptr;    // [n_angles+1]
     int32_t *angle_row_offset = nullptr;    // [n_angles+1]

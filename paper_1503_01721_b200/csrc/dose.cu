@@ -139,11 +139,23 @@ k_sum_partials(const double *__restrict__ part, int n, double *__restrict__ out)
     if (threadIdx.x == 0) out[0] = tot;
 }
 
+// x in the column order of CSR(D) (common.cuh: tiles of 8 columns x all leaf rows per control point)
+__global__ void k_permute_x(int n, const int32_t *__restrict__ perm, const float *__restrict__ x, float *__restrict__ xp)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < n) xp[perm[j]] = x[j];
+}
+
 int vmat_launch_dose(const vmat_ddc *h, const float *x, float *d, bool fuse,
                      const uint8_t *voxel_struct, int32_t n_struct, const float *T, const float *w_over,
                      const float *w_under, float *g, double *F, cudaStream_t st)
 {
     if (fuse && h->prof_ev[0]) VMAT_CUDA(cudaEventRecord(h->prof_ev[0], st));
+    if (h->col_perm != nullptr && h->n_blocks > 0) {
+        k_permute_x<<<(h->n_beamlets + 255) / 256, 256, 0, st>>>(h->n_beamlets, h->col_perm, x, h->x_perm);
+        VMAT_LAUNCH_CHECK();
+        x = h->x_perm;
+    }
     if (h->n_blocks > 0) {
         const MatView A = view_of(h->D);
 #define VMAT_DOSE_LAUNCH(FUSE_, FMT_, ...)                                                              \

@@ -90,7 +90,7 @@ __global__ void __launch_bounds__(ING_THREADS)
 k_scatter(const int32_t *__restrict__ vox, const int32_t *__restrict__ beam, const float *__restrict__ val,
           int64_t n, const int64_t *__restrict__ ptrD, const int64_t *__restrict__ ptrT,
           uint32_t *curV, uint32_t *curB, int32_t *__restrict__ idxD, float *__restrict__ valD,
-          int32_t *__restrict__ idxT, float *__restrict__ valT)
+          int32_t *__restrict__ idxT, float *__restrict__ valT, const int32_t *__restrict__ col_perm)
 {
     const int64_t stride = (int64_t)gridDim.x * ING_THREADS;
     const int64_t n_round = (n + 31) / 32 * 32;
@@ -103,7 +103,7 @@ k_scatter(const int32_t *__restrict__ vox, const int32_t *__restrict__ beam, con
         const uint32_t sb = warp_agg_take(curB, b, ok);
         if (ok) {
             const int64_t pd = ptrD[v] + sv, pt = ptrT[b] + sb;
-            idxD[pd] = b; valD[pd] = a;
+            idxD[pd] = col_perm ? col_perm[b] : b; valD[pd] = a;       // CSR(D) in the tiled column order (common.cuh)
             idxT[pt] = v; valT[pt] = a;
         }
     }
@@ -525,7 +525,7 @@ int vmat_build_layouts(vmat_ddc *h, const int32_t *coo_voxel, const int32_t *coo
                 k_count<<<grid_for(n), ING_THREADS, 0, st>>>(v, b, a, n, nv, nb, cntV, cntB, flags);
             else
                 k_scatter<<<grid_for(n), ING_THREADS, 0, st>>>(v, b, a, n, cD.ptr, cT.ptr, cntV, cntB,
-                                                               cD.idx, cD.val, cT.idx, cT.val);
+                                                               cD.idx, cD.val, cT.idx, cT.val, h->col_perm);
             VMAT_LAUNCH_CHECK();
         }
         if (pass == 0) {
