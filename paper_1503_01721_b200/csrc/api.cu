@@ -252,7 +252,8 @@ int vmat_ddc_create_ex(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int
                     }
                 }
         }
-        if (!identity && n_beamlets > 0) {
+        // worth a pass over x per dose launch only where leaf rows are several tiles long (max_len = the longest)
+        if (!identity && n_beamlets > 0 && max_len >= 4 * COL_TILE) {
             h->h_col_inv.assign((size_t)n_beamlets, 0);
             for (int j = 0; j < n_beamlets; ++j) h->h_col_inv[perm[j]] = j;
             rc = upload(&h->col_perm, perm.data(), (int64_t)n_beamlets, &h->bytes_device);

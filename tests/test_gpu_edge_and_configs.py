@@ -121,6 +121,36 @@ def test_ragged_rows_spanning_every_kernel_path(vm):
     assert (ev.g > 0).any() and (ev.g < 0).any() and (ev.R > ev.L).any()
 
 
+def test_tiled_column_order_is_invisible_at_the_boundary(vm):
+    """Leaf rows of several tiles (the handle renumbers the beamlets of CSR(D) in tiles of 8 columns x all leaf rows
+    of a control point and permutes x before the dose kernel): vmat_ddc_export_csr still returns both layouts in the
+    caller's numbering, canonical order, exactly the input triplets; the evaluation matches the oracle."""
+    rng = np.random.default_rng(8)
+    n_v = 4000
+    rows = [np.array([70, 33, 0, 41, 8, 64]), np.array([9, 120, 35]), np.array([40, 40, 40, 40])]
+    n_b = int(sum(r.sum() for r in rows))
+    lens = rng.integers(0, 120, n_v)
+    A = _random_problem(rng, n_v, n_b, rows, lens)
+    x = (rng.random(n_b) * 0.5).astype(np.float32)
+    out, ev, info = _run_and_check(vm, A, x)
+    h = ddc_from_arrays(A, DEV)
+    order = np.lexsort((A["beam"], A["vox"]))
+    ptr, idx, val = [t.numpy() for t in h.export_csr(0)]
+    assert np.array_equal(ptr, np.concatenate([[0], np.cumsum(np.bincount(A["vox"], minlength=n_v))]))
+    assert np.array_equal(idx, A["beam"][order]) and np.array_equal(val, A["val"][order])
+    order_t = np.lexsort((A["vox"], A["beam"]))
+    ptr, idx, val = [t.numpy() for t in h.export_csr(1)]
+    assert np.array_equal(idx, A["vox"][order_t]) and np.array_equal(val, A["val"][order_t])
+    # D e_j reproduces column j (P1) for beamlets in different tiles of the same leaf row
+    for j in (0, 7, 8, 69, 70, 103, int(n_b) - 1):
+        e = torch.zeros(n_b, device=DEV); e[j] = 1.0
+        d = torch.empty(n_v, device=DEV)
+        vm.vmat_dose(h, e, d)
+        col = np.zeros(n_v, np.float32); m = A["beam"] == j; col[A["vox"][m]] = A["val"][m]
+        assert np.array_equal(d.cpu().numpy(), col), j
+    h.close()
+
+
 def test_short_leaf_rows_fused_path_and_masks(vm):
     rng = np.random.default_rng(2)
     n_v, n_b = 20000, 4000
