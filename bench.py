@@ -194,7 +194,8 @@ def oracle_workload(spec, gen_device, budget_s: float, t_cp: float, nnz_cp: int,
     if full_ok:
         A = coo_host if coo_host is not None else phantom_arrays_host(synth.generate(spec, device=gen_device))
         return A, {"control_points": n_a, "of": n_a, "nnz": int(A["val"].size), "fraction": 1.0}
-    k = int(max(1, min(n_a, budget_s / max(t_cp, 1e-4), 4e8 / max(nnz_cp, 1))))     # <= ~4e8 nnz (5 GB of host COO)
+    ram_cap = max(4e8, 0.4 * host_ram_available() / 12.0)                             # triplets the host can hold (>= 5 GB worth)
+    k = int(max(1, min(n_a, budget_s / max(t_cp, 1e-4), ram_cap / max(nnz_cp, 1))))
     angles = sorted(set(int(round(i * n_a / k)) % n_a for i in range(k)))
     smp = synth.generate(spec, device=gen_device, angles=angles)
     return phantom_arrays_host(smp), {"control_points": len(angles), "of": n_a, "nnz": int(smp.nnz),
