@@ -167,6 +167,28 @@ def test_master_problem_at_the_bench_shape_config3(vm):
     mp.close()
 
 
+def test_unaligned_structure_ids(vm):
+    """voxel_struct at an address that is not a multiple of 16 (a view one byte into a buffer): the kernel's cp.async
+    path for the structure ids needs aligned blocks and must fall back, with the same result."""
+    rng = np.random.default_rng(123)
+    n_v, m = 20011, 70
+    DA, sid, T, wo, wu = _random_mp(rng, n_v, m)
+    lo, hi, y0 = np.zeros(m), np.full(m, 40.0), rng.uniform(0.0, 1.0, m)
+    ref, sol, z, Fh, dh, mp, obj = _solve_both(vm, DA, sid, T, wo, wu, y0, lo, hi, max_iter=8, eps_F=0.0, eps_y=0.0)
+    buf = torch.zeros(n_v + 1, dtype=torch.uint8, device=DEV)
+    buf[1:] = obj.voxel_struct
+    view = buf[1:]
+    assert view.data_ptr() % 16 != 0 and view.is_contiguous()
+    mp.set_fluence(torch.from_numpy(y0))
+    z2 = torch.empty(n_v, dtype=torch.float32, device=DEV)
+    sol2 = mp.solve(vm.Objective(view, obj.T, obj.w_over, obj.w_under), max_iter=8, eps_F=0.0, eps_y=0.0, z=z2)
+    Fh2, dh2 = mp.history()
+    assert np.array_equal(Fh2.numpy(), Fh) and np.array_equal(dh2.numpy(), dh) and np.array_equal(z2.cpu().numpy(), z)
+    assert torch.equal(sol2.y, sol.y)
+    _check(ref, sol2, z2.cpu().numpy(), Fh2.numpy(), dh2.numpy())
+    mp.close()
+
+
 def test_each_stopping_rule(vm):
     rng = np.random.default_rng(5)
     DA, sid, T, wo, wu = _random_mp(rng, 3000, 12)
