@@ -630,6 +630,7 @@ def run_ours(args):
                            ph.angle_col_offset, ph.angle_row_offset, ph.leafrow_col_offset, device=dev,
                            index_bits=args.index_bits)
     t_ingest = time.time() - t0
+    h.set_schedule(args.schedule == "sm-affine")
     stats = ph.stats()
     h.leafrow_col_offset_host = ph.leafrow_col_offset.to(torch.int64).cpu()
     # the CPU baseline evaluates the very same triplets: keep a host copy when they fit the host's memory
@@ -780,7 +781,8 @@ def run_ours(args):
                        "l2": f"inputs larger than L2: {B_eval / 1e9:.2f} GB streamed per step vs 126 MB L2"
                              if B_eval > 4 * 126e6 else "L2-resident: matrix fits the 126 MB L2, no HBM fraction claimed",
                        "x": "re-drawn per step, seeded Uniform[0,1)", "gen_s": round(t_gen, 2),
-                       "ingest_s": round(t_ingest, 2)},
+                       "ingest_s": round(t_ingest, 2), "schedule": args.schedule,
+                       "grid": [info["grid_dose"], info["grid_price"]]},
             "hbm_gbs": eval_gbs, "hbm_frac_of_8TBs": eval_gbs / 8000.0, "hbm_frac_of_measured": eval_gbs / peak,
             "hbm_gbs_8B_csr_equiv": B_eval_8B / (ms_per_step * 1e-3) / 1e9,
             "clocks": clocks,
@@ -831,6 +833,8 @@ def main():
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "angle-shards"],
                     help="N > 1: independent replicas (default; the path needs one GPU) or ONE matrix split by control "
                          "point over the ranks (NEXT-4)")
+    ap.add_argument("--schedule", default="sm-affine", choices=["sm-affine", "static"],
+                    help="work distribution of the dose and price kernels (vmat_ddc_set_schedule)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-mp", action="store_true", help="skip the master-problem measurement")
     ap.add_argument("--mp-apertures", type=int, default=128)

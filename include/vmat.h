@@ -345,6 +345,16 @@ int vmat_merge_best(const double *pairs, int32_t n, double *best, void *stream);
  * after the price(+row opening) kernel.  Pass NULL for `ev` to clear.  The events stay owned by the caller. */
 int vmat_ddc_set_profile_events(vmat_ddc *h, void *const *ev /* host [4] or NULL */);
 
+/* Work distribution of the two streaming kernels (vmat_dose, vmat_price and every fused call).
+ *   sm_affine = 1 (default)  persistent kernels, SM count x resident CTAs per SM; the items (4 voxel segments; 8
+ *                            beamlet rows) are cut into one contiguous queue per SM with equal stored bytes, and a
+ *                            CTA draws from the queue of the SM it runs on, then from the next non-empty one: the
+ *                            CTAs resident on an SM work on neighbouring items, whose gathers of x / g overlap.
+ *   sm_affine = 0            one CTA per item, in the order the hardware dispatches them.
+ * Every output is bit-identical under both settings (an item's sums have a fixed order).  Takes effect from the
+ * next launch; not to be called while a launch on this handle is in flight. */
+int vmat_ddc_set_schedule(vmat_ddc *h, int32_t sm_affine);
+
 /* Thread-local, static storage; never NULL. */
 const char *vmat_last_error(void);
 

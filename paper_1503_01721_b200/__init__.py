@@ -34,7 +34,7 @@ EXPORTS = [
     "vmat_mp_solve", "vmat_mp_history", "vmat_column_generation",
     "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained", "vmat_leaf_windows",
     "vmat_column_generation_ex", "vmat_price_select", "vmat_mp_reached_voxels", "vmat_mp_pass_geometry", "vmat_check_structure_ids", "vmat_best_pair", "vmat_merge_best",
-    "vmat_price_eval_host_submit", "vmat_price_eval_host_wait",
+    "vmat_price_eval_host_submit", "vmat_price_eval_host_wait", "vmat_ddc_set_schedule",
 ]
 
 
@@ -78,6 +78,7 @@ def load_library():
     lib.vmat_price_eval_host_submit.argtypes = [vp, i32, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.vmat_price_eval_host_wait.argtypes = [vp, i32]
     lib.vmat_ddc_set_profile_events.argtypes = [vp, vp]
+    lib.vmat_ddc_set_schedule.argtypes = [vp, i32]
     f64 = ctypes.c_double
     lib.vmat_mp_create.argtypes = [ctypes.POINTER(vp), i32, i32, vp]
     lib.vmat_mp_destroy.argtypes = [vp]
@@ -204,6 +205,10 @@ class DDC:
             return
         arr = (ctypes.c_void_p * 4)(*[e.cuda_event for e in events])
         _check(load_library().vmat_ddc_set_profile_events(self._h, arr))
+
+    def set_schedule(self, sm_affine: bool):
+        """vmat_ddc_set_schedule: SM-affine persistent kernels (default) or one CTA per item."""
+        _check(load_library().vmat_ddc_set_schedule(self._h, 1 if sm_affine else 0))
 
     def export_ptr(self, which: int) -> torch.Tensor:
         """Row pointers (int64 [rows+1], host) of CSR(D) (0) or CSR(D^T) (1)."""

@@ -95,9 +95,9 @@ k_aperture_scatter(const int64_t *__restrict__ pptr, MatView A, int j_lo, int j_
     TileCursor<FMT> tc(A, s, lane);
     for (int ti = 0; ti < nt; ++ti, tc.advance()) {
         TileRegs<FMT> t;
-        tile_load<FMT>(tc, t);
+        tile_load<FMT>(A, tc, lane, t);
         int vx[8];
-        tile_indices<FMT>(tc, t, lane, vx);
+        tile_indices<FMT>(A, tc, t, lane, vx);
 #pragma unroll
         for (int q = 0; q < 8; ++q) add(__uint_as_float(t.v.w[q]), vx[q]);
     }
@@ -162,7 +162,7 @@ int vmat_ddc_destroy(vmat_ddc *h)
                     h->F_partial_obj, h->S_scratch, h->beamlet_leafrow, h->leafrow_done, h->e2e_x, h->e2e_d, h->e2e_g, h->e2e_p, h->e2e_L, h->e2e_R,
                     h->e2e_best, h->e2e_row_price, h->e2e_angle_price, h->e2e_F,
                     h->leafrow_pos0, h->angle_pmin, h->angle_wd, h->row_bp_offset, h->cs_bp, h->ad_acc, h->angle_order,
-                    h->col_perm, h->x_perm};
+                    h->col_perm, h->x_perm, h->q_start, h->q_next};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     for (auto &sl : h->slot) {
@@ -177,6 +177,53 @@ int vmat_ddc_destroy(vmat_ddc *h)
     if (h->cs_join) cudaEventDestroy(h->cs_join);
     if (h->cs_aux) cudaStreamDestroy(h->cs_aux);
     delete h;
+    return VMAT_OK;
+}
+
+// Queue q of a kernel (smqueue.cuh) starts at the first item whose first stored entry lies at or beyond q / nq of the
+// layout's padded entries.  seg_row != NULL: item = `per` consecutive segments of the dose kernel; NULL: `per` rows.
+__global__ void k_queue_starts(int nq, int n_items, int per, int n_units, const int32_t *__restrict__ seg_row,
+                               const int64_t *__restrict__ pptr, int64_t P, int32_t *__restrict__ start)
+{
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q > nq) return;
+    const int64_t target = q == nq ? P : (P / nq) * q;
+    int lo = 0, hi = n_items;                                      // smallest item with pos(item) >= target
+    if (q == nq) lo = n_items;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        const int u = min(mid * per, n_units);
+        const int64_t pos = pptr[seg_row ? seg_row[u] : u];
+        if (pos >= target) hi = mid; else lo = mid + 1;
+    }
+    start[q] = lo;
+}
+
+static int build_sm_queues(vmat_ddc *h, cudaStream_t st)
+{
+    int n_sm = 0;
+    VMAT_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, h->device));
+    h->n_sm = n_sm;
+    if (n_sm <= 0) return VMAT_OK;
+    const size_t n = 2 * ((size_t)n_sm + 1);
+    VMAT_CUDA(cudaMalloc((void **)&h->q_start, n * 4));
+    VMAT_CUDA(cudaMalloc((void **)&h->q_next, n * 4));
+    h->bytes_device += (int64_t)n * 8;
+    VMAT_CUDA(cudaMemsetAsync(h->q_next, 0, n * 4, st));
+    const int tb = 64, gb = (n_sm + 1 + tb - 1) / tb;
+    k_queue_starts<<<gb, tb, 0, st>>>(n_sm, h->n_blocks, DOSE_THREADS / 32, h->n_seg, h->seg_row, h->D.pptr, h->D.P, h->q_start);
+    VMAT_LAUNCH_CHECK();
+    k_queue_starts<<<gb, tb, 0, st>>>(n_sm, (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS, PRICE_WARPS, h->n_beamlets,
+                                      nullptr, h->Dt.pptr, h->Dt.P, h->q_start + n_sm + 1);
+    VMAT_LAUNCH_CHECK();
+    return VMAT_OK;
+}
+
+int vmat_ddc_set_schedule(vmat_ddc *h, int32_t sm_affine)
+{
+    REQUIRE(h != nullptr, "handle is NULL");
+    REQUIRE(sm_affine == 0 || sm_affine == 1, "sm_affine must be 0 or 1");
+    h->sched = sm_affine;
     return VMAT_OK;
 }
 
@@ -265,6 +312,7 @@ int vmat_ddc_create_ex(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int
         }
     }
     if (rc == VMAT_OK) rc = vmat_build_layouts(h, coo_voxel, coo_beamlet, coo_val, index_bits, st);
+    if (rc == VMAT_OK) rc = build_sm_queues(h, st);
     if (rc == VMAT_OK) rc = upload(&h->angle_col_offset, angle_col_offset, (int64_t)n_angles + 1, &h->bytes_device);
     if (rc == VMAT_OK) rc = upload(&h->angle_row_offset, angle_row_offset, (int64_t)n_angles + 1, &h->bytes_device);
     if (rc == VMAT_OK) rc = upload(&h->leafrow_col_offset, leafrow_col_offset, (int64_t)n_rows + 1, &h->bytes_device);
@@ -340,8 +388,8 @@ int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info)
     info->bytes_stream_dt = h->Dt.bytes();
     info->tiles_d = h->D.n_tiles; info->tiles_uniform_d = h->D.n_tiles_uniform;
     info->tiles_dt = h->Dt.n_tiles; info->tiles_uniform_dt = h->Dt.n_tiles_uniform;
-    info->grid_dose = h->n_blocks;
-    info->grid_price = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
+    info->grid_dose = h->n_blocks > 0 ? vmat_dose_grid(h, true) : 0;
+    info->grid_price = h->n_beamlets > 0 ? vmat_price_grid(h) : 0;
     return VMAT_OK;
 }
 

@@ -6,6 +6,7 @@
 #include <limits.h>
 #include <vector>
 #include "../../include/vmat.h"
+#include "smqueue.cuh"
 
 // ------------------------------------------------------------------ error plumbing
 void vmat_set_error(const char *fmt, ...);
@@ -87,7 +88,14 @@ struct vmat_ddc {
     // dose kernel work list: segment i (one warp) covers voxel rows [seg_row[i], seg_row[i+1])
     int32_t *seg_row = nullptr;             // [n_seg+1]
     int32_t n_seg = 0;
-    int32_t n_blocks = 0;                   // CTAs of the dose kernel = ceil(n_seg / warps per CTA)
+    int32_t n_blocks = 0;                   // items of the dose kernel = ceil(n_seg / warps per CTA)
+    // SM-affine schedule of the two streaming kernels (smqueue.cuh): per SM one contiguous queue of items with equal
+    // stored bytes; sched = 1 (default): persistent kernels drawing from them, 0: one CTA per item
+    int sched = 1, n_sm = 0;
+    int32_t *q_start = nullptr;             // [2][n_sm + 1]: dose items, price items
+    uint32_t *q_next = nullptr;             // [2][n_sm + 1] self-resetting counters
+    SmQueues queues_dose() const { return SmQueues{q_start, q_next, sched && q_start ? n_sm : 0}; }
+    SmQueues queues_price() const { return SmQueues{q_start + n_sm + 1, q_next + n_sm + 1, sched && q_start ? n_sm : 0}; }
     double *F_partial = nullptr;            // [n_blocks] per-CTA objective partials
     int32_t n_obj_blocks = 0;               // blocks of the standalone objective kernel
     double *F_partial_obj = nullptr;        // [n_obj_blocks]
@@ -221,6 +229,8 @@ __device__ __forceinline__ float ld_gather(const float *p)
 // ------------------------------------------------------------------ internal entry points
 int vmat_build_layouts(vmat_ddc *h, const int32_t *coo_voxel, const int32_t *coo_beamlet,
                        const float *coo_val, int index_bits, cudaStream_t st);
+int vmat_dose_grid(const vmat_ddc *h, bool fuse);      // CTAs of the dose launch (fused or plain)
+int vmat_price_grid(const vmat_ddc *h);                // CTAs of the fused price + selection launch
 int vmat_launch_dose(const vmat_ddc *h, const float *x, float *d, bool fuse,
                      const uint8_t *voxel_struct, int32_t n_struct, const float *T, const float *w_over,
                      const float *w_under, float *g, double *F, cudaStream_t st);

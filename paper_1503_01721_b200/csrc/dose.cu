@@ -14,6 +14,7 @@
 // 21 % of its issue slots to barrier stalls - profiles/).  Everything is FP32 with a fixed summation
 // order; the objective partials are FP64, one per CTA, summed afterwards in a fixed order (no atomics).
 #include "spmv.cuh"
+#include "smqueue.cuh"
 
 // g_i and the voxel's term of F for dose v (Eq. (1); sign and factor 2: C1, C2)
 __device__ __forceinline__ float voxel_grad(float v, float T, float wo, float wu, double &f)
@@ -38,74 +39,84 @@ __device__ __forceinline__ double block_sum_double(double v, double *red /* [NT/
     return s;
 }
 
+// Item = DOSE_THREADS / 32 consecutive segments (one per warp); F_partial has one slot per item.
 template <bool FUSE, int FMT>
 __global__ void __launch_bounds__(DOSE_THREADS, VMAT_DOSE_MINB)
 k_dose(const int64_t *__restrict__ pptr, const MatView A, const int32_t *__restrict__ seg_row, int n_seg,
        const float *__restrict__ x, float *__restrict__ d,
        const uint8_t *__restrict__ vstruct, const float *__restrict__ T,
        const float *__restrict__ w_over, const float *__restrict__ w_under, float *__restrict__ g,
-       double *__restrict__ F_partial)
+       double *__restrict__ F_partial, const SmQueues Q)
 {
     __shared__ float prod[DOSE_THREADS / 32][DOSE_SEG_NNZ];
     __shared__ double red_d[DOSE_THREADS / 32];
+    __shared__ int s_item[2];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int sgi = blockIdx.x * (DOSE_THREADS / 32) + warp;
-    double fsum = 0.0;
-    auto epilogue = [&](int r, float v) {          // d, and the fused A2: g and the voxel's term of F
-        d[r] = v;
-        if (FUSE) {
-            const int sid = vstruct[r];
-            g[r] = voxel_grad(v, __ldg(T + sid), __ldg(w_over + sid), __ldg(w_under + sid), fsum);
-        }
-    };
-    if (sgi < n_seg) {
-        const int r0 = seg_row[sgi], r1 = seg_row[sgi + 1];
-        const int nr = r1 - r0;
-        const int64_t s = pptr[r0], e = pptr[r1];               // padded positions, multiples of 32
-        if (nr == 1) {
-            // ---- one row: register accumulation
-            const float acc = warp_sum(segment_dot<FMT, VMAT_DOSE_PIPELINE>(A, s, e, x, lane));
-            if (lane == 0) epilogue(r0, acc);
-        } else {
-            // ---- several short rows: products into this warp's slice at their padded position k - s ...
-            float *wp = prod[warp];
-            const int nt = (int)((e - s) >> 8);
-            TileCursor<FMT> tc(A, s, lane);
+    const int n_items = (n_seg + DOSE_THREADS / 32 - 1) / (DOSE_THREADS / 32);
+    sq_init(Q, s_item);
 #pragma unroll 1
-            for (int ti = 0; ti < nt; ++ti, tc.advance()) {
-                TileRegs<FMT> tr;
-                tile_load<FMT>(tc, tr);
-                int c[8];
-                tile_indices<FMT>(tc, tr, lane, c);
-                float *dst = wp + ti * TILE + lane;
-#pragma unroll
-                for (int t = 0; t < 8; ++t) dst[32 * t] = __uint_as_float(tr.v.w[t]) * ld_gather(x + c[t]);
+    for (;;) {
+        const int item = sq_next_item(Q, s_item);
+        if (item < 0 || item >= n_items) break;
+        const int sgi = item * (DOSE_THREADS / 32) + warp;
+        double fsum = 0.0;
+        auto epilogue = [&](int r, float v) {          // d, and the fused A2: g and the voxel's term of F
+            d[r] = v;
+            if (FUSE) {
+                const int sid = vstruct[r];
+                g[r] = voxel_grad(v, __ldg(T + sid), __ldg(w_over + sid), __ldg(w_under + sid), fsum);
             }
-            const int64_t k0 = s + (int64_t)nt * TILE;
-            float *dst = wp + nt * TILE + lane;
-            tail_foreach<FMT>(A, k0, (int)((e - k0) >> 5), x, lane, [&](int t, float q) { dst[32 * t] = q; });
-            __syncwarp();
-            // ... then G lanes per row, G = power of two near (mean row length)/4, 1..32
-            const int mean = (int)((e - s) / nr);
-            int G = 1;
-            while (G < 32 && G * 4 < mean) G <<= 1;
-            const int grp = lane / G, gl = lane % G, n_grp = 32 / G;
-            const int n_iter = (nr + n_grp - 1) / n_grp;        // uniform trip count: shuffles stay converged
-            for (int it = 0; it < n_iter; ++it) {
-                const int r = r0 + grp + it * n_grp;
-                float acc = 0.f;
-                if (r < r1) {
-                    const int b = (int)(pptr[r] - s), f = (int)(pptr[r + 1] - s);
-                    for (int k = b + gl; k < f; k += G) acc += wp[k];
+        };
+        if (sgi < n_seg) {
+            const int r0 = seg_row[sgi], r1 = seg_row[sgi + 1];
+            const int nr = r1 - r0;
+            const int64_t s = pptr[r0], e = pptr[r1];               // padded positions, multiples of 32
+            if (nr == 1) {
+                // ---- one row: register accumulation
+                const float acc = warp_sum(segment_dot<FMT, VMAT_DOSE_PIPELINE>(A, s, e, x, lane));
+                if (lane == 0) epilogue(r0, acc);
+            } else {
+                // ---- several short rows: products into this warp's slice at their padded position k - s ...
+                float *wp = prod[warp];
+                const int nt = (int)((e - s) >> 8);
+                TileCursor<FMT> tc(A, s, lane);
+#pragma unroll 1
+                for (int ti = 0; ti < nt; ++ti, tc.advance()) {
+                    TileRegs<FMT> tr;
+                    tile_load<FMT>(A, tc, lane, tr);
+                    int c[8];
+                    tile_indices<FMT>(A, tc, tr, lane, c);
+                    float *dst = wp + ti * TILE + lane;
+#pragma unroll
+                    for (int t = 0; t < 8; ++t) dst[32 * t] = __uint_as_float(tr.v.w[t]) * ld_gather(x + c[t]);
                 }
-                for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-                if (r < r1 && gl == 0) epilogue(r, acc);
+                const int64_t k0 = s + (int64_t)nt * TILE;
+                float *dst = wp + nt * TILE + lane;
+                tail_foreach<FMT>(A, k0, (int)((e - k0) >> 5), x, lane, [&](int t, float q_) { dst[32 * t] = q_; });
+                __syncwarp();
+                // ... then G lanes per row, G = power of two near (mean row length)/4, 1..32
+                const int mean = (int)((e - s) / nr);
+                int G = 1;
+                while (G < 32 && G * 4 < mean) G <<= 1;
+                const int grp = lane / G, gl = lane % G, n_grp = 32 / G;
+                const int n_iter = (nr + n_grp - 1) / n_grp;        // uniform trip count: shuffles stay converged
+                for (int it = 0; it < n_iter; ++it) {
+                    const int r = r0 + grp + it * n_grp;
+                    float acc = 0.f;
+                    if (r < r1) {
+                        const int b = (int)(pptr[r] - s), f = (int)(pptr[r + 1] - s);
+                        for (int k = b + gl; k < f; k += G) acc += wp[k];
+                    }
+                    for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+                    if (r < r1 && gl == 0) epilogue(r, acc);
+                }
+                __syncwarp();                                       // the slice is refilled by the next item
             }
         }
-    }
-    if (FUSE) {
-        const double tot = block_sum_double<DOSE_THREADS>(fsum, red_d);
-        if (threadIdx.x == 0) F_partial[blockIdx.x] = tot;
+        if (FUSE) {
+            const double tot = block_sum_double<DOSE_THREADS>(fsum, red_d);
+            if (threadIdx.x == 0) F_partial[((volatile int *)s_item)[0]] = tot;     // re-read: no register held across the loop
+        }
     }
 }
 
@@ -146,6 +157,31 @@ __global__ void k_permute_x(int n, const int32_t *__restrict__ perm, const float
     if (j < n) xp[perm[j]] = x[j];
 }
 
+// Launch geometry: SM-affine queues -> a persistent grid of SM count x resident CTAs per SM; static -> one CTA per item.
+template <bool FUSE, int FMT>
+static int dose_grid(const vmat_ddc *h)
+{
+    if (h->queues_dose().nq == 0) return h->n_blocks;
+    static int occ = 0;                                               // per kernel instance
+    if (occ == 0) {
+        int o = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_dose<FUSE, FMT>, DOSE_THREADS, 0);
+        occ = o > 0 ? o : 1;
+    }
+    return min(h->n_blocks, h->n_sm * occ);
+}
+int vmat_dose_grid(const vmat_ddc *h, bool fuse)
+{
+    switch (fmt_of(h->D) + (fuse ? 3 : 0)) {
+    case 0: return dose_grid<false, FMT_WIDE>(h);
+    case 1: return dose_grid<false, FMT_NARROW>(h);
+    case 2: return dose_grid<false, FMT_NARROW_1BASE>(h);
+    case 3: return dose_grid<true, FMT_WIDE>(h);
+    case 4: return dose_grid<true, FMT_NARROW>(h);
+    default: return dose_grid<true, FMT_NARROW_1BASE>(h);
+    }
+}
+
 int vmat_launch_dose(const vmat_ddc *h, const float *x, float *d, bool fuse,
                      const uint8_t *voxel_struct, int32_t n_struct, const float *T, const float *w_over,
                      const float *w_under, float *g, double *F, cudaStream_t st)
@@ -158,8 +194,9 @@ int vmat_launch_dose(const vmat_ddc *h, const float *x, float *d, bool fuse,
     }
     if (h->n_blocks > 0) {
         const MatView A = view_of(h->D);
+        const SmQueues Q = h->queues_dose();
 #define VMAT_DOSE_LAUNCH(FUSE_, FMT_, ...)                                                              \
-        k_dose<FUSE_, FMT_><<<h->n_blocks, DOSE_THREADS, 0, st>>>(h->D.pptr, A, h->seg_row, h->n_seg, x, d, __VA_ARGS__)
+        k_dose<FUSE_, FMT_><<<dose_grid<FUSE_, FMT_>(h), DOSE_THREADS, 0, st>>>(h->D.pptr, A, h->seg_row, h->n_seg, x, d, __VA_ARGS__, Q)
 #define VMAT_DOSE_ARGS_FUSED voxel_struct, T, w_over, w_under, g, h->F_partial
 #define VMAT_DOSE_ARGS_PLAIN nullptr, nullptr, nullptr, nullptr, nullptr, nullptr
         switch (fmt_of(h->D) + (fuse ? 3 : 0)) {

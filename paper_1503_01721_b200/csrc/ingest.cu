@@ -395,6 +395,10 @@ static int plan_layout(const CanonCsr &C, bool narrow, bool group_short, PackPla
     VMAT_CUDA(cudaMemcpyAsync(&total, pl->d_gstart + pl->n_seg, 8, cudaMemcpyDeviceToHost, st));
     VMAT_CUDA(cudaStreamSynchronize(st));
     pl->P = total * GROUP;
+    if (pl->P >= (int64_t)1 << 35) {                     // spmv.cuh: the kernels' cursor counts units of 8 entries in 32 bits
+        vmat_set_error("vmat_ddc_create: %lld padded entries exceed the layout limit of 2^35", (long long)pl->P);
+        return VMAT_ERR_INVALID_ARG;
+    }
     return VMAT_OK;
 }
 

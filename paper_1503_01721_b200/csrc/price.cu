@@ -14,6 +14,7 @@
 // All pairs are enumerated - the definition itself, n <= ~10^2 - so the leaf positions are
 // bit-identical to the exhaustive CPU definition for the same FP32 p.
 #include "spmv.cuh"
+#include "smqueue.cuh"
 
 struct Opening {
     double V;
@@ -117,63 +118,72 @@ struct SelectArgs {
 template <bool SELECT, int FMT, bool SKIP = false>
 __global__ void __launch_bounds__(PRICE_THREADS, VMAT_PRICE_MINB)
 k_price(const int64_t *__restrict__ pptr, const MatView A, int n_rows, const float *__restrict__ g,
-        float *__restrict__ p, SelectArgs sa)
+        float *__restrict__ p, SelectArgs sa, const SmQueues Q)
 {
+    __shared__ int s_item[2];
+    __shared__ int done_rows[PRICE_WARPS];
+    __shared__ int n_done;
     const int lane = threadIdx.x & 31;
     if (SELECT) {                                   // leaf rows without beamlets draw no ticket: close them here
-        const int r = blockIdx.x * PRICE_THREADS + threadIdx.x;
-        if (r < sa.n_leaf_rows && sa.leafrow_col_offset[r + 1] == sa.leafrow_col_offset[r]) {
-            sa.L[r] = 0; sa.R[r] = 0; sa.row_price[r] = 0.0;
-        }
+        for (int r = blockIdx.x * PRICE_THREADS + threadIdx.x; r < sa.n_leaf_rows; r += gridDim.x * PRICE_THREADS)
+            if (sa.leafrow_col_offset[r + 1] == sa.leafrow_col_offset[r]) {
+                sa.L[r] = 0; sa.R[r] = 0; sa.row_price[r] = 0.0;
+            }
     }
     const int warp = threadIdx.x >> 5;
-    const int row = blockIdx.x * PRICE_WARPS + warp;
-    if (row < n_rows) {
-        if (SKIP && sa.angle_mask[sa.leafrow_angle[sa.beamlet_leafrow[row]]] != 0) {
-            if (lane == 0) p[row] = 0.f;
-        } else {
-            const float acc = warp_sum(segment_dot<FMT, VMAT_PRICE_PIPELINE>(A, pptr[row], pptr[row + 1], g, lane));
-            if (lane == 0) p[row] = acc;
+    const int n_items = (n_rows + PRICE_WARPS - 1) / PRICE_WARPS;      // item = 8 consecutive beamlet rows
+    sq_init(Q, s_item);
+#pragma unroll 1
+    for (;;) {
+        const int item = sq_next_item(Q, s_item);
+        if (item < 0 || item >= n_items) break;
+        {
+            const int row = item * PRICE_WARPS + warp;
+            float acc = 0.f;
+            if (row < n_rows && !(SKIP && sa.angle_mask[sa.leafrow_angle[sa.beamlet_leafrow[row]]] != 0))
+                acc = warp_sum(segment_dot<FMT, VMAT_PRICE_PIPELINE>(A, pptr[row], pptr[row + 1], g, lane));
+            // the item is re-read from shared memory (nobody writes it before the next fetch): no register holds it
+            // across the streaming loop, which has none to spare at 40 registers
+            const int row_w = ((volatile int *)s_item)[0] * PRICE_WARPS + warp;
+            if (lane == 0 && row_w < n_rows) p[row_w] = acc;                // 0 for a skipped row
         }
-    }
-    if (SELECT) {
-        // One ticket per CTA and leaf row: the CTA's 8 consecutive beamlet rows lie in a few leaf rows.
-        // Thread 0 adds, for each of them, the number of its rows this CTA priced; the CTA whose add
-        // completes a leaf row selects that row's opening (warp w takes the w-th completed row).
-        __shared__ int done_rows[PRICE_WARPS];
-        __shared__ int n_done;
-        __syncthreads();                                                // the CTA's prices are written
-        if (threadIdx.x == 0) {
-            __threadfence();                                            // ... and visible before the tickets
-            int nd = 0;
-            const int row0 = blockIdx.x * PRICE_WARPS;
-            const int row1 = min(row0 + PRICE_WARPS, n_rows);
-            int c = row0;
-            while (c < row1) {
-                const int r = sa.beamlet_leafrow[c];
-                const int j1 = sa.leafrow_col_offset[r + 1];
-                const int cnt = min(row1, j1) - c;                      // rows of leaf row r priced here
-                const int n = j1 - sa.leafrow_col_offset[r];
-                if (atomicAdd(sa.leafrow_done + r, (uint32_t)cnt) + cnt == (uint32_t)n) {
-                    sa.leafrow_done[r] = 0;                             // ready for the next launch
-                    done_rows[nd++] = r;
+        if (SELECT) {
+            // One ticket per item and leaf row: the item's 8 consecutive beamlet rows lie in a few leaf rows.
+            // Thread 0 adds, for each of them, the number of its rows priced here; the CTA whose add
+            // completes a leaf row selects that row's opening (warp w takes the w-th completed row).
+            __syncthreads();                                                // the item's prices are written
+            if (threadIdx.x == 0) {
+                __threadfence();                                            // ... and visible before the tickets
+                int nd = 0;
+                const int row0 = ((volatile int *)s_item)[0] * PRICE_WARPS;
+                const int row1 = min(row0 + PRICE_WARPS, n_rows);
+                int c = row0;
+                while (c < row1) {
+                    const int r = sa.beamlet_leafrow[c];
+                    const int j1 = sa.leafrow_col_offset[r + 1];
+                    const int cnt = min(row1, j1) - c;                      // rows of leaf row r priced here
+                    const int n = j1 - sa.leafrow_col_offset[r];
+                    if (atomicAdd(sa.leafrow_done + r, (uint32_t)cnt) + cnt == (uint32_t)n) {
+                        sa.leafrow_done[r] = 0;                             // ready for the next launch
+                        done_rows[nd++] = r;
+                    }
+                    c += cnt;
                 }
-                c += cnt;
+                if (nd > 0) __threadfence();
+                n_done = nd;
             }
-            if (nd > 0) __threadfence();
-            n_done = nd;
-        }
-        __syncthreads();
-        if (warp < n_done) {                                            // every price of leaf row r is written
-            const int r = done_rows[warp];
-            const int j0 = sa.leafrow_col_offset[r];
-            const int n = sa.leafrow_col_offset[r + 1] - j0;
-            const bool occupied = sa.angle_mask != nullptr && sa.angle_mask[sa.leafrow_angle[r]] != 0;   // C7
-            const Opening best = warp_select_row(p + j0, occupied ? 0 : n, sa.S + j0 + r, lane);
-            if (lane == 0) {
-                sa.L[r] = best.L;
-                sa.R[r] = best.R;
-                sa.row_price[r] = best.V;
+            __syncthreads();
+            if (warp < n_done) {                                            // every price of leaf row r is written
+                const int r = done_rows[warp];
+                const int j0 = sa.leafrow_col_offset[r];
+                const int n = sa.leafrow_col_offset[r + 1] - j0;
+                const bool occupied = sa.angle_mask != nullptr && sa.angle_mask[sa.leafrow_angle[r]] != 0;   // C7
+                const Opening best = warp_select_row(p + j0, occupied ? 0 : n, sa.S + j0 + r, lane);
+                if (lane == 0) {
+                    sa.L[r] = best.L;
+                    sa.R[r] = best.R;
+                    sa.row_price[r] = best.V;
+                }
             }
         }
     }
@@ -306,22 +316,48 @@ int vmat_launch_merge_best(const double *pairs, int32_t n, double *best, cudaStr
 }
 
 // ---------------------------------------------------------------- launchers
-template <bool SELECT, bool SKIP = false>
-static void launch_k_price(const vmat_ddc *h, int grid, const float *g, float *p, const SelectArgs &sa, cudaStream_t st)
+// Launch geometry: SM-affine queues -> a persistent grid of SM count x resident CTAs per SM; static -> one CTA per item.
+template <bool SELECT, int FMT, bool SKIP>
+static int price_grid(const vmat_ddc *h)
 {
-    const MatView A = view_of(h->Dt);
+    const int n_items = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
+    if (h->queues_price().nq == 0) return n_items;
+    static int occ = 0;                                               // per kernel instance
+    if (occ == 0) {
+        int o = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_price<SELECT, FMT, SKIP>, PRICE_THREADS, 0);
+        occ = o > 0 ? o : 1;
+    }
+    return min(n_items, h->n_sm * occ);
+}
+int vmat_price_grid(const vmat_ddc *h)                                // of the fused price + selection launch
+{
     switch (fmt_of(h->Dt)) {
-    case 0: k_price<SELECT, FMT_WIDE, SKIP><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
-    case 1: k_price<SELECT, FMT_NARROW, SKIP><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
-    default: k_price<SELECT, FMT_NARROW_1BASE, SKIP><<<grid, PRICE_THREADS, 0, st>>>(h->Dt.pptr, A, h->n_beamlets, g, p, sa); break;
+    case 0: return price_grid<true, FMT_WIDE, false>(h);
+    case 1: return price_grid<true, FMT_NARROW, false>(h);
+    default: return price_grid<true, FMT_NARROW_1BASE, false>(h);
+    }
+}
+template <bool SELECT, int FMT, bool SKIP>
+static void launch_k_price_fmt(const vmat_ddc *h, const float *g, float *p, const SelectArgs &sa, cudaStream_t st)
+{
+    k_price<SELECT, FMT, SKIP><<<price_grid<SELECT, FMT, SKIP>(h), PRICE_THREADS, 0, st>>>(
+        h->Dt.pptr, view_of(h->Dt), h->n_beamlets, g, p, sa, h->queues_price());
+}
+template <bool SELECT, bool SKIP = false>
+static void launch_k_price(const vmat_ddc *h, const float *g, float *p, const SelectArgs &sa, cudaStream_t st)
+{
+    switch (fmt_of(h->Dt)) {
+    case 0: launch_k_price_fmt<SELECT, FMT_WIDE, SKIP>(h, g, p, sa, st); break;
+    case 1: launch_k_price_fmt<SELECT, FMT_NARROW, SKIP>(h, g, p, sa, st); break;
+    default: launch_k_price_fmt<SELECT, FMT_NARROW_1BASE, SKIP>(h, g, p, sa, st); break;
     }
 }
 
 int vmat_launch_price(const vmat_ddc *h, const float *g, float *p, cudaStream_t st)
 {
     if (h->n_beamlets == 0) return VMAT_OK;
-    const int grid = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
-    launch_k_price<false>(h, grid, g, p, SelectArgs{}, st);
+    launch_k_price<false>(h, g, p, SelectArgs{}, st);
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }
@@ -340,10 +376,9 @@ int vmat_launch_select(const vmat_ddc *h, const float *p, const uint8_t *angle_m
 int vmat_launch_price_unoccupied(const vmat_ddc *h, const float *g, const uint8_t *angle_mask, float *p, cudaStream_t st)
 {
     if (h->n_beamlets == 0) return VMAT_OK;
-    const int grid = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
     SelectArgs sa{};
     sa.beamlet_leafrow = h->beamlet_leafrow; sa.leafrow_angle = h->leafrow_angle; sa.angle_mask = angle_mask;
-    launch_k_price<false, true>(h, grid, g, p, sa, st);
+    launch_k_price<false, true>(h, g, p, sa, st);
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }
@@ -352,16 +387,14 @@ int vmat_launch_price_select(const vmat_ddc *h, const float *g, const uint8_t *a
                              int32_t *L, int32_t *R, double *row_price, cudaStream_t st, bool skip_occupied)
 {
     if (h->n_leaf_rows == 0) return VMAT_OK;
-    const int grid = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
-    // the "no beamlets" pass needs one thread per leaf row: fall back to the two-kernel path otherwise
-    if (h->n_beamlets == 0 || (int64_t)grid * PRICE_THREADS < h->n_leaf_rows) {
+    if (h->n_beamlets == 0) {                       // nothing to price: the selection kernel closes every row
         int rc = vmat_launch_price(h, g, p, st);
         return rc != VMAT_OK ? rc : vmat_launch_select(h, p, angle_mask, L, R, row_price, st);
     }
     SelectArgs sa{h->beamlet_leafrow, h->leafrow_col_offset, h->leafrow_angle, angle_mask, h->leafrow_done,
                   h->S_scratch, L, R, row_price, h->n_leaf_rows};
-    if (skip_occupied && angle_mask != nullptr) launch_k_price<true, true>(h, grid, g, p, sa, st);
-    else launch_k_price<true>(h, grid, g, p, sa, st);
+    if (skip_occupied && angle_mask != nullptr) launch_k_price<true, true>(h, g, p, sa, st);
+    else launch_k_price<true>(h, g, p, sa, st);
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }

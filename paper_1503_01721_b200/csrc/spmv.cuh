@@ -47,21 +47,25 @@ __host__ __device__ __forceinline__ int64_t stored_pos(int64_t S, int64_t G, int
 constexpr int TILE_UNIFORM_BIT = int(0x80000000u);
 __host__ __device__ __forceinline__ int base_index(int word) { return word & 0x7fffffff; }
 
-// Per-lane stream pointers into a segment's interleaved tiles; advance() steps to the next tile.
+// This lane's position in a segment's interleaved tiles, in ONE register: units of 8 stored entries (32 bytes of
+// values), u = s / 8 + lane + 32 * tile; the stream addresses are formed from it with one multiply-add each against
+// the layout's base pointers (constant bank).  The first version kept three 64-bit pointers (6 registers), which at
+// the kernels' 40 registers left none for the item loop of the persistent kernels.  P / 8 < 2^32 is checked at ingest.
 template <int FMT>
 struct TileCursor {
-    const float *v;          // this lane's 8 values of the tile
-    const char *i;           // this lane's 8 offsets (u16) or indices (i32)
-    const int32_t *b;        // the tile's 8 base words (narrow only)
-    __device__ __forceinline__ TileCursor(const MatView &A, int64_t s, int lane)
-        : v(A.val + s + lane * 8), i((const char *)A.sec + (s + lane * 8) * (FMT != FMT_WIDE ? 2 : 4)),
-          b(FMT != FMT_WIDE ? A.base + (s >> 5) : nullptr) {}
-    __device__ __forceinline__ void advance()
+    uint32_t u;
+    __device__ __forceinline__ TileCursor(const MatView &, int64_t s, int lane) : u((uint32_t)(s >> 3) + (uint32_t)lane) {}
+    __device__ __forceinline__ void advance() { u += TILE / 8; }
+    __device__ __forceinline__ const float *v(const MatView &A) const { return A.val + (size_t)u * 8; }   // 8 values
+    __device__ __forceinline__ const char *i(const MatView &A) const                // 8 offsets (u16) or indices (i32)
     {
-        v += TILE;
-        i += TILE * (FMT != FMT_WIDE ? 2 : 4);
-        if (FMT != FMT_WIDE) b += TILE / GROUP;
+        return (const char *)A.sec + (size_t)u * (FMT != FMT_WIDE ? 16 : 32);
     }
+    __device__ __forceinline__ const int32_t *b(const MatView &A, int lane) const   // the tile's 8 base words
+    {
+        return A.base + ((u - (uint32_t)lane) >> 2);
+    }
+    __device__ __forceinline__ int64_t pos(int lane) const { return (int64_t)(u - (uint32_t)lane) << 3; }   // padded position of the tile
 };
 
 // This lane's share of one tile's streams, in registers: loading and using are separate steps so that a loop
@@ -72,21 +76,22 @@ struct TileRegs {
     Vec8 o;                  // wide: 8 int32 indices; narrow: o.w[0..3] = 8 u16 offsets, o.w[4] = the tile's base word
 };
 template <int FMT>
-__device__ __forceinline__ void tile_load(const TileCursor<FMT> &tc, TileRegs<FMT> &r)
+__device__ __forceinline__ void tile_load(const MatView &A, const TileCursor<FMT> &tc, int lane, TileRegs<FMT> &r)
 {
-    r.v = ld_stream_256(tc.v);
+    r.v = ld_stream_256(tc.v(A));
     if (FMT != FMT_WIDE) {
-        const Vec4 o = ld_stream_128(tc.i);
+        const Vec4 o = ld_stream_128(tc.i(A));
         r.o.w[0] = o.w[0]; r.o.w[1] = o.w[1]; r.o.w[2] = o.w[2]; r.o.w[3] = o.w[3];
-        r.o.w[4] = (uint32_t)ld_stream_i(tc.b);                             // broadcast: one 128-byte wavefront
+        r.o.w[4] = (uint32_t)ld_stream_i(tc.b(A, lane));                    // broadcast: one 128-byte wavefront
     } else {
-        r.o = ld_stream_256(tc.i);
+        r.o = ld_stream_256(tc.i(A));
     }
 }
 
 // Secondary indices of this lane's 8 entries of the tile (entry `lane` of groups 0..7).
 template <int FMT>
-__device__ __forceinline__ void tile_indices(const TileCursor<FMT> &tc, const TileRegs<FMT> &r, int lane, int (&c)[8])
+__device__ __forceinline__ void tile_indices(const MatView &A, const TileCursor<FMT> &tc, const TileRegs<FMT> &r, int lane,
+                                             int (&c)[8])
 {
     if (FMT != FMT_WIDE) {
         const int b0 = (int)r.o.w[4];
@@ -96,7 +101,7 @@ __device__ __forceinline__ void tile_indices(const TileCursor<FMT> &tc, const Ti
             for (int t = 0; t < 8; ++t)
                 c[t] = bb + (int)((t & 1) ? (r.o.w[t >> 1] >> 16) : (r.o.w[t >> 1] & 0xffffu));
         } else {                                                            // one base per group, by shuffles
-            const int b = ld_stream_i(tc.b + (lane & 7));
+            const int b = ld_stream_i(tc.b(A, lane) + (lane & 7));
 #pragma unroll
             for (int t = 0; t < 8; ++t) {
                 const int bt = __shfl_sync(0xffffffffu, b, t);
@@ -111,11 +116,11 @@ __device__ __forceinline__ void tile_indices(const TileCursor<FMT> &tc, const Ti
 
 // One interleaved tile: this lane's partial of sum val*vec[idx].
 template <int FMT>
-__device__ __forceinline__ float tile_dot(const TileCursor<FMT> &tc, const TileRegs<FMT> &r,
+__device__ __forceinline__ float tile_dot(const MatView &A, const TileCursor<FMT> &tc, const TileRegs<FMT> &r,
                                           const float *__restrict__ vec, int lane)
 {
     int c[8];
-    tile_indices<FMT>(tc, r, lane, c);
+    tile_indices<FMT>(A, tc, r, lane, c);
     float acc = 0.f;
 #pragma unroll
     for (int t = 0; t < 8; ++t) acc = fmaf(__uint_as_float(r.v.w[t]), ld_gather(vec + c[t]), acc);
@@ -154,40 +159,53 @@ __device__ __forceinline__ void tail_foreach(const MatView &A, int64_t k0, int n
 }
 
 // A whole segment [s, e) (padded positions, multiples of 32) as one dot product: this lane's partial.
-// PIPELINE: the next tile's stream loads are issued before this tile's gathers (13 more live registers).
+// PIPELINE: the next tile's stream loads are issued before this tile's gathers; two tiles per trip in two register
+// sets that swap roles, so nothing is copied.  Only the cursor, two counts and the sum live across the loop (s and e
+// are dead once the counts are formed: the tail starts where the cursor stands).
 template <int FMT, bool PIPELINE>
 __device__ __forceinline__ float segment_dot(const MatView &A, int64_t s, int64_t e, const float *__restrict__ vec,
                                              int lane)
 {
     const int nt = (int)((e - s) >> 8);
+    const int ngt = (int)((e - s) >> 5) & 7;
     float acc = 0.f;
     TileCursor<FMT> tc(A, s, lane);
     if (PIPELINE) {
         if (nt > 0) {
-            TileRegs<FMT> cur;
-            tile_load<FMT>(tc, cur);
+            TileRegs<FMT> ra, rb;
+            tile_load<FMT>(A, tc, lane, ra);
+            int left = nt - 1;                                   // tiles not yet loaded
 #pragma unroll 1
-            for (int ti = 1; ti < nt; ++ti) {
-                TileCursor<FMT> tn = tc;
-                tn.advance();
-                TileRegs<FMT> nxt;
-                tile_load<FMT>(tn, nxt);
-                acc += tile_dot<FMT>(tc, cur, vec, lane);
-                cur = nxt;
-                tc = tn;
+            for (; left >= 2; left -= 2) {
+                TileCursor<FMT> t0 = tc;
+                tc.advance();
+                tile_load<FMT>(A, tc, lane, rb);
+                acc += tile_dot<FMT>(A, t0, ra, vec, lane);
+                t0 = tc;
+                tc.advance();
+                tile_load<FMT>(A, tc, lane, ra);
+                acc += tile_dot<FMT>(A, t0, rb, vec, lane);
             }
-            acc += tile_dot<FMT>(tc, cur, vec, lane);
+            if (left == 1) {
+                TileCursor<FMT> t0 = tc;
+                tc.advance();
+                tile_load<FMT>(A, tc, lane, rb);
+                acc += tile_dot<FMT>(A, t0, ra, vec, lane);
+                acc += tile_dot<FMT>(A, tc, rb, vec, lane);
+            } else {
+                acc += tile_dot<FMT>(A, tc, ra, vec, lane);
+            }
+            tc.advance();
         }
     } else {
 #pragma unroll 1
         for (int ti = 0; ti < nt; ++ti, tc.advance()) {
             TileRegs<FMT> r;
-            tile_load<FMT>(tc, r);
-            acc += tile_dot<FMT>(tc, r, vec, lane);
+            tile_load<FMT>(A, tc, lane, r);
+            acc += tile_dot<FMT>(A, tc, r, vec, lane);
         }
     }
-    const int64_t k0 = s + (int64_t)nt * TILE;
-    tail_foreach<FMT>(A, k0, (int)((e - k0) >> 5), vec, lane, [&](int, float q) { acc += q; });
+    tail_foreach<FMT>(A, tc.pos(lane), ngt, vec, lane, [&](int, float q) { acc += q; });
     return acc;
 }
 

@@ -46,6 +46,26 @@ def _random_problem(rng, n_v, n_b, rows_spec, row_lens, n_struct=4):
                 wu=np.array([0.0, 1.0, 0.0, 0.3], np.float32)[:n_struct], lco=lco, aro=aro, aco=aco)
 
 
+OUT_FIELDS = ("d", "g", "F", "p", "L", "R", "row_price", "angle_price", "best_angle")
+
+
+def _assert_schedules_agree(vm, h, x, obj, out, mask=None):
+    """`out` was computed under the default schedule (SM-affine queues, persistent kernels): one CTA per item gives
+    the same bits in every output, fused and unfused (vmat_ddc_set_schedule), and so does a second SM-affine run
+    (the queue counters reset themselves)."""
+    for sm_affine in (False, True):
+        h.set_schedule(sm_affine)
+        o2 = h.alloc_outputs()
+        vm.vmat_price_eval(h, x, obj, o2, mask)
+        d2 = torch.empty_like(out.d); p2 = torch.empty_like(out.p)
+        vm.vmat_dose(h, x, d2)
+        vm.vmat_price(h, out.g, p2)
+        torch.cuda.synchronize()
+        for f in OUT_FIELDS:
+            assert torch.equal(getattr(o2, f), getattr(out, f)), (f, sm_affine)
+        assert torch.equal(d2, out.d) and torch.equal(p2, out.p)
+
+
 def _run_and_check(vm, A, x, mask=None, expect_no_diff=True):
     """Whole evaluation against the oracle, once per index encoding (int32 indices; u16 offsets + group
     bases; the automatic choice).  Returns the outputs / info of the automatic choice."""
@@ -69,6 +89,7 @@ def _run_and_check(vm, A, x, mask=None, expect_no_diff=True):
         vm.vmat_dose(h, torch.from_numpy(x).to(DEV), d2)
         vm.vmat_price(h, out.g, p2)
         assert torch.equal(d2, out.d) and torch.equal(p2, out.p)
+        _assert_schedules_agree(vm, h, torch.from_numpy(x).to(DEV), obj_to_device(A, DEV), out, m)
         info = h.info
         if bits:
             assert info["index_bits_d"] == info["index_bits_dt"] == bits
@@ -256,6 +277,7 @@ def _full_parity(vm, ph, scales):
         assert_vec_close("p", out.p.cpu().numpy(), ev.p)
         assert abs(out.F.item() - ev.F) <= REL_L2 * abs(ev.F)
         n_diff = check_selection_protocol(A, out, ev)
+        _assert_schedules_agree(vm, h, x.to(DEV), obj, out)
         print(f"  x*{sc}: F={ev.F:.6e} open rows={(ev.R > ev.L).sum()} best={ev.best_angle} "
               f"rows differing from the pure-FP64 path={n_diff}")
         assert n_diff <= max(1, A["lco"].size // 1000)
