@@ -537,6 +537,8 @@ def run_sweep(args):
                 del hv, hb, hw
                 pt["ingest"] = "COO streamed from host memory (the device build ran out of memory with the triplets resident)"
             pt["ingest_s"] = round(time.time() - t0, 2)
+            h.set_schedule({"auto": None, "sm-affine": True, "static": False}[args.schedule])
+            pt["sm_affine"] = [bool(h.info["sm_affine_dose"]), bool(h.info["sm_affine_price"])]
             ph.coo_voxel = ph.coo_beamlet = ph.coo_val = None
             torch.cuda.empty_cache()
             obj = vm.Objective(ph.voxel_struct.to(dev), ph.struct_T.to(dev), ph.struct_w_over.to(dev), ph.struct_w_under.to(dev))
@@ -630,7 +632,7 @@ def run_ours(args):
                            ph.angle_col_offset, ph.angle_row_offset, ph.leafrow_col_offset, device=dev,
                            index_bits=args.index_bits)
     t_ingest = time.time() - t0
-    h.set_schedule(args.schedule == "sm-affine")
+    h.set_schedule({"auto": None, "sm-affine": True, "static": False}[args.schedule])
     stats = ph.stats()
     h.leafrow_col_offset_host = ph.leafrow_col_offset.to(torch.int64).cpu()
     # the CPU baseline evaluates the very same triplets: keep a host copy when they fit the host's memory
@@ -782,6 +784,7 @@ def run_ours(args):
                              if B_eval > 4 * 126e6 else "L2-resident: matrix fits the 126 MB L2, no HBM fraction claimed",
                        "x": "re-drawn per step, seeded Uniform[0,1)", "gen_s": round(t_gen, 2),
                        "ingest_s": round(t_ingest, 2), "schedule": args.schedule,
+                       "sm_affine": [bool(info["sm_affine_dose"]), bool(info["sm_affine_price"])],
                        "grid": [info["grid_dose"], info["grid_price"]]},
             "hbm_gbs": eval_gbs, "hbm_frac_of_8TBs": eval_gbs / 8000.0, "hbm_frac_of_measured": eval_gbs / peak,
             "hbm_gbs_8B_csr_equiv": B_eval_8B / (ms_per_step * 1e-3) / 1e9,
@@ -833,7 +836,7 @@ def main():
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "angle-shards"],
                     help="N > 1: independent replicas (default; the path needs one GPU) or ONE matrix split by control "
                          "point over the ranks (NEXT-4)")
-    ap.add_argument("--schedule", default="sm-affine", choices=["sm-affine", "static"],
+    ap.add_argument("--schedule", default="auto", choices=["auto", "sm-affine", "static"],
                     help="work distribution of the dose and price kernels (vmat_ddc_set_schedule)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-mp", action="store_true", help="skip the master-problem measurement")

@@ -66,6 +66,7 @@ typedef struct vmat_ddc_info {
     int64_t tiles_dt, tiles_uniform_dt;      /* (span <= 65535) instead of one per 32-entry group; 0 for int32   */
     int64_t grid_dose, grid_price;           /* CTAs the dose and the price kernel are launched with (bench.py checks
                                                 a stored ncu capture against them before quoting its DRAM traffic)  */
+    int64_t sm_affine_dose, sm_affine_price; /* 1: the kernel draws its items from per-SM queues (vmat_ddc_set_schedule) */
 } vmat_ddc_info;
 
 /* A0 ingest / layout build (D arrives as COO - values, voxel (row) index,
@@ -346,12 +347,14 @@ int vmat_merge_best(const double *pairs, int32_t n, double *best, void *stream);
 int vmat_ddc_set_profile_events(vmat_ddc *h, void *const *ev /* host [4] or NULL */);
 
 /* Work distribution of the two streaming kernels (vmat_dose, vmat_price and every fused call).
- *   sm_affine = 1 (default)  persistent kernels, SM count x resident CTAs per SM; the items (4 voxel segments; 8
- *                            beamlet rows) are cut into one contiguous queue per SM with equal stored bytes, and a
- *                            CTA draws from the queue of the SM it runs on, then from the next non-empty one: the
- *                            CTAs resident on an SM work on neighbouring items, whose gathers of x / g overlap.
- *   sm_affine = 0            one CTA per item, in the order the hardware dispatches them.
- * Every output is bit-identical under both settings (an item's sums have a fixed order).  Takes effect from the
+ *   sm_affine = 1   persistent kernels, SM count x resident CTAs per SM; the items (4 voxel segments; 8 beamlet rows)
+ *                   are cut into one contiguous queue per SM with equal stored bytes, and a CTA draws from the queue of
+ *                   the SM it runs on, then from the next non-empty one: the CTAs resident on an SM work on
+ *                   neighbouring items, whose gathers of x / g overlap.
+ *   sm_affine = 0   one CTA per item, in the order the hardware dispatches them.
+ *   sm_affine = -1  (what vmat_ddc_create sets) per kernel, 1 where the layout has >= 16 items per resident CTA of
+ *                   >= 64 KB each, else 0; vmat_ddc_info.sm_affine_dose / _price say which.
+ * Every output is bit-identical under all settings (an item's sums have a fixed order).  Takes effect from the
  * next launch; not to be called while a launch on this handle is in flight. */
 int vmat_ddc_set_schedule(vmat_ddc *h, int32_t sm_affine);
 

@@ -49,7 +49,8 @@ class _Info(ctypes.Structure):
         "n_voxels", "n_beamlets", "nnz", "n_angles", "n_leaf_rows", "bytes_csr_d", "bytes_csr_dt",
         "bytes_device_total", "n_dose_blocks", "max_leaf_row_len", "max_voxel_row_nnz", "max_beamlet_row_nnz",
         "index_bits_d", "index_bits_dt", "padded_d", "padded_dt", "bytes_stream_d", "bytes_stream_dt",
-        "tiles_d", "tiles_uniform_d", "tiles_dt", "tiles_uniform_dt", "grid_dose", "grid_price")]
+        "tiles_d", "tiles_uniform_d", "tiles_dt", "tiles_uniform_dt", "grid_dose", "grid_price",
+        "sm_affine_dose", "sm_affine_price")]
 
 
 def load_library():
@@ -170,9 +171,7 @@ class DDC:
     def __init__(self, handle: int, device: torch.device):
         self._h = ctypes.c_void_p(handle)
         self.device = device
-        info = _Info()
-        _check(load_library().vmat_ddc_info_get(self._h, ctypes.byref(info)))
-        self.info = {n: int(getattr(info, n)) for n, _ in _Info._fields_}
+        self._read_info()
         self.n_voxels, self.n_beamlets = self.info["n_voxels"], self.info["n_beamlets"]
         self.n_angles, self.n_leaf_rows, self.nnz = self.info["n_angles"], self.info["n_leaf_rows"], self.info["nnz"]
 
@@ -206,9 +205,17 @@ class DDC:
         arr = (ctypes.c_void_p * 4)(*[e.cuda_event for e in events])
         _check(load_library().vmat_ddc_set_profile_events(self._h, arr))
 
-    def set_schedule(self, sm_affine: bool):
-        """vmat_ddc_set_schedule: SM-affine persistent kernels (default) or one CTA per item."""
-        _check(load_library().vmat_ddc_set_schedule(self._h, 1 if sm_affine else 0))
+    def _read_info(self):
+        info = _Info()
+        _check(load_library().vmat_ddc_info_get(self._h, ctypes.byref(info)))
+        self.info = {n: int(getattr(info, n)) for n, _ in _Info._fields_}
+
+    def set_schedule(self, sm_affine):
+        """vmat_ddc_set_schedule: True / 1 = SM-affine persistent kernels, False / 0 = one CTA per item,
+        None / -1 = the automatic per-kernel choice (what create sets)."""
+        mode = -1 if sm_affine is None else int(sm_affine)
+        _check(load_library().vmat_ddc_set_schedule(self._h, mode))
+        self._read_info()
 
     def export_ptr(self, which: int) -> torch.Tensor:
         """Row pointers (int64 [rows+1], host) of CSR(D) (0) or CSR(D^T) (1)."""

@@ -218,12 +218,28 @@ static int build_sm_queues(vmat_ddc *h, cudaStream_t st)
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }
+// The automatic choice, per kernel.  Measured on B200 (profiles/r2_sm_affine.md): the queues pay where a kernel runs
+// many items per resident CTA and an item is long (config 3: 76 KB per dose item, 188 KB per price item, ~100 items
+// per CTA: +2.3 % per evaluation, more under the power cap).  With short items the visit to the queue (two block
+// barriers and an atomic's round trip to L2) costs more than a fresh CTA from the hardware scheduler (dose items of
+// 23 - 55 KB, configs 1 and 2 and the config-4 sweep: -4 %), and with a handful of items per CTA (price kernel of
+// configs 1 and 2: 7 and 3) there is nothing to share and the tail is coarser.
+static bool sm_affine_pays(int64_t stored_bytes, int64_t n_items, int n_sm, int ctas_per_sm, int64_t min_item_bytes)
+{
+    if (n_items <= 0 || n_sm <= 0) return false;
+    return n_items >= (int64_t)16 * n_sm * ctas_per_sm && stored_bytes / n_items >= min_item_bytes;
+}
 
 int vmat_ddc_set_schedule(vmat_ddc *h, int32_t sm_affine)
 {
     REQUIRE(h != nullptr, "handle is NULL");
-    REQUIRE(sm_affine == 0 || sm_affine == 1, "sm_affine must be 0 or 1");
-    h->sched = sm_affine;
+    REQUIRE(sm_affine >= -1 && sm_affine <= 1, "sm_affine must be -1 (automatic), 0 or 1");
+    if (sm_affine < 0) {
+        h->sched_dose = sm_affine_pays(h->D.bytes(), h->n_blocks, h->n_sm, VMAT_DOSE_MINB, 64 * 1024);
+        h->sched_price = sm_affine_pays(h->Dt.bytes(), (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS, h->n_sm, 6, 64 * 1024);
+    } else {
+        h->sched_dose = h->sched_price = sm_affine;
+    }
     return VMAT_OK;
 }
 
@@ -313,6 +329,7 @@ int vmat_ddc_create_ex(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int
     }
     if (rc == VMAT_OK) rc = vmat_build_layouts(h, coo_voxel, coo_beamlet, coo_val, index_bits, st);
     if (rc == VMAT_OK) rc = build_sm_queues(h, st);
+    if (rc == VMAT_OK) rc = vmat_ddc_set_schedule(h, -1);
     if (rc == VMAT_OK) rc = upload(&h->angle_col_offset, angle_col_offset, (int64_t)n_angles + 1, &h->bytes_device);
     if (rc == VMAT_OK) rc = upload(&h->angle_row_offset, angle_row_offset, (int64_t)n_angles + 1, &h->bytes_device);
     if (rc == VMAT_OK) rc = upload(&h->leafrow_col_offset, leafrow_col_offset, (int64_t)n_rows + 1, &h->bytes_device);
@@ -390,6 +407,7 @@ int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info)
     info->tiles_dt = h->Dt.n_tiles; info->tiles_uniform_dt = h->Dt.n_tiles_uniform;
     info->grid_dose = h->n_blocks > 0 ? vmat_dose_grid(h, true) : 0;
     info->grid_price = h->n_beamlets > 0 ? vmat_price_grid(h) : 0;
+    info->sm_affine_dose = h->queues_dose().nq > 0; info->sm_affine_price = h->queues_price().nq > 0;
     return VMAT_OK;
 }
 

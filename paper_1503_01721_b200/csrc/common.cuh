@@ -7,6 +7,14 @@
 #include <vector>
 #include "../../include/vmat.h"
 #include "smqueue.cuh"
+// items a CTA takes per visit to its SM's queue (smqueue.cuh): one atomic per chunk
+#ifndef VMAT_DOSE_QUEUE_CHUNK
+#define VMAT_DOSE_QUEUE_CHUNK 4
+#endif
+#ifndef VMAT_PRICE_QUEUE_CHUNK
+#define VMAT_PRICE_QUEUE_CHUNK 1
+#endif
+constexpr int DOSE_QUEUE_CHUNK = VMAT_DOSE_QUEUE_CHUNK, PRICE_QUEUE_CHUNK = VMAT_PRICE_QUEUE_CHUNK;
 
 // ------------------------------------------------------------------ error plumbing
 void vmat_set_error(const char *fmt, ...);
@@ -90,13 +98,16 @@ struct vmat_ddc {
     int32_t n_seg = 0;
     int32_t n_blocks = 0;                   // items of the dose kernel = ceil(n_seg / warps per CTA)
     // SM-affine schedule of the two streaming kernels (smqueue.cuh): per SM one contiguous queue of items with equal
-    // stored bytes; sched = 1 (default): persistent kernels drawing from them, 0: one CTA per item
-    int sched = 1, n_sm = 0;
+    // stored bytes; per kernel 1: persistent CTAs drawing from them, 0: one CTA per item.  vmat_ddc_set_schedule.
+    int sched_dose = 0, sched_price = 0, n_sm = 0;
     int32_t *q_start = nullptr;             // [2][n_sm + 1]: dose items, price items
     uint32_t *q_next = nullptr;             // [2][n_sm + 1] self-resetting counters
-    SmQueues queues_dose() const { return SmQueues{q_start, q_next, sched && q_start ? n_sm : 0}; }
-    SmQueues queues_price() const { return SmQueues{q_start + n_sm + 1, q_next + n_sm + 1, sched && q_start ? n_sm : 0}; }
-    double *F_partial = nullptr;            // [n_blocks] per-CTA objective partials
+    SmQueues queues_dose() const { return SmQueues{q_start, q_next, sched_dose && q_start ? n_sm : 0, DOSE_QUEUE_CHUNK}; }
+    SmQueues queues_price() const
+    {
+        return SmQueues{q_start + n_sm + 1, q_next + n_sm + 1, sched_price && q_start ? n_sm : 0, PRICE_QUEUE_CHUNK};
+    }
+    double *F_partial = nullptr;            // [n_blocks] per-item objective partials
     int32_t n_obj_blocks = 0;               // blocks of the standalone objective kernel
     double *F_partial_obj = nullptr;        // [n_obj_blocks]
     double *S_scratch = nullptr;            // [n_beamlets + n_leaf_rows + 1] prefix sums of the row selection
@@ -155,13 +166,15 @@ struct vmat_ddc {
 #ifndef VMAT_DOSE_MINB
 #define VMAT_DOSE_MINB 12
 #endif
-// Software pipelining of the tile loop (next tile's stream loads in flight while this tile gathers): measured on
-// B200, +9 % for the price kernel at 6 CTAs/SM; the dose kernel (12 CTAs of 4 warps) has no registers for it.
-#ifndef VMAT_PRICE_PIPELINE
-#define VMAT_PRICE_PIPELINE true
+// Depth of the software pipeline of the tile loop (spmv.cuh: tiles whose stream loads are in flight at once).
+// Measured on B200 (config 3): the price kernel is fastest at depth 2 and 6 CTAs/SM (40 registers); the dose kernel at
+// depth 1 and 12 CTAs of 4 warps - depth 2 spills at 40 registers in its u16 + per-group-base variant and 10 or 8 CTAs
+// lose more than the pipeline gains (profiles/r2_sm_affine.md).
+#ifndef VMAT_PRICE_DEPTH
+#define VMAT_PRICE_DEPTH 2
 #endif
-#ifndef VMAT_DOSE_PIPELINE
-#define VMAT_DOSE_PIPELINE false
+#ifndef VMAT_DOSE_DEPTH
+#define VMAT_DOSE_DEPTH 1
 #endif
 constexpr int DOSE_THREADS = VMAT_DOSE_THREADS;
 constexpr int DOSE_SEG_NNZ = VMAT_DOSE_SEG_NNZ;   // a warp's run of short rows holds at most this many padded entries

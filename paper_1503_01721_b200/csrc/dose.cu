@@ -50,7 +50,7 @@ k_dose(const int64_t *__restrict__ pptr, const MatView A, const int32_t *__restr
 {
     __shared__ float prod[DOSE_THREADS / 32][DOSE_SEG_NNZ];
     __shared__ double red_d[DOSE_THREADS / 32];
-    __shared__ int s_item[2];
+    __shared__ int s_item[3];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int n_items = (n_seg + DOSE_THREADS / 32 - 1) / (DOSE_THREADS / 32);
     sq_init(Q, s_item);
@@ -73,7 +73,7 @@ k_dose(const int64_t *__restrict__ pptr, const MatView A, const int32_t *__restr
             const int64_t s = pptr[r0], e = pptr[r1];               // padded positions, multiples of 32
             if (nr == 1) {
                 // ---- one row: register accumulation
-                const float acc = warp_sum(segment_dot<FMT, VMAT_DOSE_PIPELINE>(A, s, e, x, lane));
+                const float acc = warp_sum(segment_dot<FMT, VMAT_DOSE_DEPTH>(A, s, e, x, lane));
                 if (lane == 0) epilogue(r0, acc);
             } else {
                 // ---- several short rows: products into this warp's slice at their padded position k - s ...

@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(PRICE_THREADS, VMAT_PRICE_MINB)
 k_price(const int64_t *__restrict__ pptr, const MatView A, int n_rows, const float *__restrict__ g,
         float *__restrict__ p, SelectArgs sa, const SmQueues Q)
 {
-    __shared__ int s_item[2];
+    __shared__ int s_item[3];
     __shared__ int done_rows[PRICE_WARPS];
     __shared__ int n_done;
     const int lane = threadIdx.x & 31;
@@ -141,7 +141,7 @@ k_price(const int64_t *__restrict__ pptr, const MatView A, int n_rows, const flo
             const int row = item * PRICE_WARPS + warp;
             float acc = 0.f;
             if (row < n_rows && !(SKIP && sa.angle_mask[sa.leafrow_angle[sa.beamlet_leafrow[row]]] != 0))
-                acc = warp_sum(segment_dot<FMT, VMAT_PRICE_PIPELINE>(A, pptr[row], pptr[row + 1], g, lane));
+                acc = warp_sum(segment_dot<FMT, VMAT_PRICE_DEPTH>(A, pptr[row], pptr[row + 1], g, lane));
             // the item is re-read from shared memory (nobody writes it before the next fetch): no register holds it
             // across the streaming loop, which has none to spare at 40 registers
             const int row_w = ((volatile int *)s_item)[0] * PRICE_WARPS + warp;

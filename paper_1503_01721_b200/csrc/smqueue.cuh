@@ -22,6 +22,7 @@ struct SmQueues {
     uint32_t *next;         // [nq + 1] items handed out per queue (may run past the queue's size); next[nq] = CTAs
                             // that have finished - the last one zeroes everything for the next launch
     int nq;                 // 0 = static schedule: one CTA per item, CTA b takes item b
+    int chunk;              // consecutive items a CTA takes per visit to a queue (one atomic per chunk)
 };
 
 __device__ __forceinline__ unsigned sq_smid()
@@ -37,16 +38,17 @@ __device__ __forceinline__ unsigned sq_peek(const uint32_t *p)
     return r;
 }
 
-// Next item for this CTA, or -1 when every queue is empty.  Called by ALL lanes of ONE warp of the CTA; q = the
-// queue to try first (in: the CTA's current queue, out: the queue the item came from).
-__device__ __forceinline__ int sq_fetch(const SmQueues &Q, int &q, int lane)
+// Next chunk of items for this CTA: first item, or -1 when every queue is empty; n = items in it (1..Q.chunk).
+// Called by ALL lanes of ONE warp of the CTA; q = the queue to try first (in: the CTA's current queue, out: the queue
+// the chunk came from).
+__device__ __forceinline__ int sq_fetch(const SmQueues &Q, int &q, int lane, int &n)
 {
     unsigned i = 0;
-    if (lane == 0) i = atomicAdd(Q.next + q, 1u);
-    i = __shfl_sync(0xffffffffu, i, 0);
     {
-        const int s0 = Q.start[q];
-        if (i < (unsigned)(Q.start[q + 1] - s0)) return s0 + (int)i;
+        const int s0 = Q.start[q], s1 = Q.start[q + 1];             // loaded before the atomic, not behind it
+        if (lane == 0) i = atomicAdd(Q.next + q, (unsigned)Q.chunk);
+        i = __shfl_sync(0xffffffffu, i, 0);
+        if (i < (unsigned)(s1 - s0)) { n = min(Q.chunk, s1 - s0 - (int)i); return s0 + (int)i; }
     }
     for (int t0 = 1; t0 < Q.nq; t0 += 32) {                         // 32 queues looked at per round
         const int t = t0 + lane;
@@ -59,10 +61,10 @@ __device__ __forceinline__ int sq_fetch(const SmQueues &Q, int &q, int lane)
             m &= m - 1;
             int qv = q + t0 + l;
             if (qv >= Q.nq) qv -= Q.nq;
-            if (lane == 0) i = atomicAdd(Q.next + qv, 1u);
+            const int s0 = Q.start[qv], s1 = Q.start[qv + 1];
+            if (lane == 0) i = atomicAdd(Q.next + qv, (unsigned)Q.chunk);
             i = __shfl_sync(0xffffffffu, i, 0);
-            const int s0 = Q.start[qv];
-            if (i < (unsigned)(Q.start[qv + 1] - s0)) { q = qv; return s0 + (int)i; }
+            if (i < (unsigned)(s1 - s0)) { q = qv; n = min(Q.chunk, s1 - s0 - (int)i); return s0 + (int)i; }
         }
     }
     if (lane == 0) {                                                // this CTA is done: the last one resets the counters
@@ -72,24 +74,31 @@ __device__ __forceinline__ int sq_fetch(const SmQueues &Q, int &q, int lane)
             __threadfence();
         }
     }
+    n = 0;
     return -1;
 }
 
 // Next item of a CTA, -1 when there is none.  Static schedule (Q.nq == 0): the CTA's one item is blockIdx.x, then
-// -1.  st: two ints of shared memory {item, current queue (static: items taken)}, st[1] set by sq_init.  All
-// threads call it; the state lives in shared memory so that no register is held across the caller's streaming loop.
+// -1.  st: three ints of shared memory {item, current queue (static: items taken), items left in the chunk}, set up by
+// sq_init.  All threads call it; the state lives in shared memory so that no register is held across the caller's
+// streaming loop, and st[0] stays valid until the next call.
 __device__ __forceinline__ void sq_init(const SmQueues &Q, int *st)
 {
-    if (threadIdx.x == 0) st[1] = Q.nq > 0 ? (int)(sq_smid() % (unsigned)Q.nq) : 0;
+    if (threadIdx.x == 0) { st[1] = Q.nq > 0 ? (int)(sq_smid() % (unsigned)Q.nq) : 0; st[2] = 0; }
 }
 __device__ __forceinline__ int sq_next_item(const SmQueues &Q, int *st)
 {
     __syncthreads();                      // everyone is done with the previous item: st[0] may be read all through it
     if (threadIdx.x < 32) {
-        int q = st[1], it;
-        if (Q.nq > 0) it = sq_fetch(Q, q, (int)threadIdx.x);
-        else it = q++ == 0 ? (int)blockIdx.x : -1;
-        if (threadIdx.x == 0) { st[0] = it; st[1] = q; }
+        int left = st[2];
+        if (left > 0) {                   // the next item of the chunk in hand
+            if (threadIdx.x == 0) { st[0] = st[0] + 1; st[2] = left - 1; }
+        } else {
+            int q = st[1], it, n = 1;
+            if (Q.nq > 0) it = sq_fetch(Q, q, (int)threadIdx.x, n);
+            else it = q++ == 0 ? (int)blockIdx.x : -1;
+            if (threadIdx.x == 0) { st[0] = it; st[1] = q; st[2] = n - 1; }
+        }
     }
     __syncthreads();
     return st[0];

@@ -121,6 +121,10 @@ __device__ __forceinline__ float tile_dot(const MatView &A, const TileCursor<FMT
 {
     int c[8];
     tile_indices<FMT>(A, tc, r, lane, c);
+#ifdef VMAT_DIAG_NOGATHER                      /* measurement only: every gather hits the same 128 bytes */
+#pragma unroll
+    for (int t = 0; t < 8; ++t) c[t] &= 31;
+#endif
     float acc = 0.f;
 #pragma unroll
     for (int t = 0; t < 8; ++t) acc = fmaf(__uint_as_float(r.v.w[t]), ld_gather(vec + c[t]), acc);
@@ -159,18 +163,20 @@ __device__ __forceinline__ void tail_foreach(const MatView &A, int64_t k0, int n
 }
 
 // A whole segment [s, e) (padded positions, multiples of 32) as one dot product: this lane's partial.
-// PIPELINE: the next tile's stream loads are issued before this tile's gathers; two tiles per trip in two register
-// sets that swap roles, so nothing is copied.  Only the cursor, two counts and the sum live across the loop (s and e
-// are dead once the counts are formed: the tail starts where the cursor stands).
-template <int FMT, bool PIPELINE>
+// DEPTH = tiles whose stream loads are in flight or in registers at once (1: load, use, load ...; 2: the next tile's
+// loads are issued before this tile's gathers; 3: two tiles ahead).  DEPTH register sets take turns (the loop body is
+// unrolled DEPTH times), so nothing is copied.  Only the cursor, the counts and the sum live across the loop (s and e
+// are dead once the counts are formed: the tail starts where the cursor stands).  Tiles are added in order whatever
+// the depth: the result does not depend on it.
+template <int FMT, int DEPTH>
 __device__ __forceinline__ float segment_dot(const MatView &A, int64_t s, int64_t e, const float *__restrict__ vec,
                                              int lane)
 {
     const int nt = (int)((e - s) >> 8);
     const int ngt = (int)((e - s) >> 5) & 7;
     float acc = 0.f;
-    TileCursor<FMT> tc(A, s, lane);
-    if (PIPELINE) {
+    TileCursor<FMT> tc(A, s, lane);                              // the next tile to LOAD
+    if (DEPTH == 2) {                                            // written out: one count, no spare register at 40
         if (nt > 0) {
             TileRegs<FMT> ra, rb;
             tile_load<FMT>(A, tc, lane, ra);
@@ -196,6 +202,25 @@ __device__ __forceinline__ float segment_dot(const MatView &A, int64_t s, int64_
                 acc += tile_dot<FMT>(A, tc, ra, vec, lane);
             }
             tc.advance();
+        }
+    } else if (DEPTH > 2) {
+        TileRegs<FMT> r[DEPTH];
+        int to_load = nt, to_use = nt;
+#pragma unroll
+        for (int j = 0; j < DEPTH - 1; ++j)
+            if (to_load > 0) { tile_load<FMT>(A, tc, lane, r[j]); tc.advance(); --to_load; }
+#pragma unroll 1
+        while (to_use > 0) {
+#pragma unroll
+            for (int j = 0; j < DEPTH; ++j) {
+                if (to_load > 0) { tile_load<FMT>(A, tc, lane, r[(j + DEPTH - 1) % DEPTH]); tc.advance(); --to_load; }
+                if (to_use > 0) {
+                    TileCursor<FMT> tu = tc;                     // the tile in r[j]: DEPTH - 1 (or fewer, at the end) behind
+                    tu.u -= (uint32_t)((to_use - to_load) * (TILE / 8));
+                    acc += tile_dot<FMT>(A, tu, r[j], vec, lane);
+                    --to_use;
+                }
+            }
         }
     } else {
 #pragma unroll 1

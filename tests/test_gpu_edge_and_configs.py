@@ -64,6 +64,8 @@ def _assert_schedules_agree(vm, h, x, obj, out, mask=None):
         for f in OUT_FIELDS:
             assert torch.equal(getattr(o2, f), getattr(out, f)), (f, sm_affine)
         assert torch.equal(d2, out.d) and torch.equal(p2, out.p)
+        assert h.info["sm_affine_dose"] == h.info["sm_affine_price"] == int(sm_affine)
+    h.set_schedule(None)                                                   # back to the automatic choice
 
 
 def _run_and_check(vm, A, x, mask=None, expect_no_diff=True):
