@@ -358,6 +358,12 @@ int vmat_ddc_set_profile_events(vmat_ddc *h, void *const *ev /* host [4] or NULL
  * next launch; not to be called while a launch on this handle is in flight. */
 int vmat_ddc_set_schedule(vmat_ddc *h, int32_t sm_affine);
 
+/* Measurement aid (bench.py: roofline.read_only_stream): GB/s of a kernel that does nothing but read `bytes` of a
+ * scratch buffer, `reps` times back to back, with the 256-bit streaming loads of the dose and price kernels - what a
+ * READ-ONLY stream reaches on this device at the clock it runs at (MEASURED_PEAKS.json's hbm_gbs is a copy: read +
+ * write).  Allocates and frees its buffer; synchronous.  gbs host [1] out. */
+int vmat_hbm_read_probe(int64_t bytes, int32_t reps, double *gbs, void *stream);
+
 /* Thread-local, static storage; never NULL. */
 const char *vmat_last_error(void);
 

@@ -34,7 +34,7 @@ EXPORTS = [
     "vmat_mp_solve", "vmat_mp_history", "vmat_column_generation",
     "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained", "vmat_leaf_windows",
     "vmat_column_generation_ex", "vmat_price_select", "vmat_mp_reached_voxels", "vmat_mp_pass_geometry", "vmat_check_structure_ids", "vmat_best_pair", "vmat_merge_best",
-    "vmat_price_eval_host_submit", "vmat_price_eval_host_wait", "vmat_ddc_set_schedule",
+    "vmat_price_eval_host_submit", "vmat_price_eval_host_wait", "vmat_ddc_set_schedule", "vmat_hbm_read_probe",
 ]
 
 
@@ -80,6 +80,7 @@ def load_library():
     lib.vmat_price_eval_host_wait.argtypes = [vp, i32]
     lib.vmat_ddc_set_profile_events.argtypes = [vp, vp]
     lib.vmat_ddc_set_schedule.argtypes = [vp, i32]
+    lib.vmat_hbm_read_probe.argtypes = [ctypes.c_int64, i32, vp, vp]
     f64 = ctypes.c_double
     lib.vmat_mp_create.argtypes = [ctypes.POINTER(vp), i32, i32, vp]
     lib.vmat_mp_destroy.argtypes = [vp]
@@ -551,6 +552,14 @@ def mp_pass_geometry(m: int, device="cuda:0") -> dict:
         return mp.pass_geometry(m)
     finally:
         mp.close()
+
+
+def vmat_hbm_read_probe(n_bytes: int, reps: int = 20) -> float:
+    """GB/s of a read-only stream over a scratch buffer of n_bytes (vmat_hbm_read_probe); needs a CUDA device."""
+    load_library()
+    gbs = ctypes.c_double(0.0)
+    _check(load_library().vmat_hbm_read_probe(int(n_bytes), int(reps), ctypes.byref(gbs), _stream()))
+    return float(gbs.value)
 
 
 def last_launch_count() -> int:

@@ -29,16 +29,20 @@ def needs_build() -> bool:
     return any(os.path.getmtime(p) > t for p in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not needs_build():
+def build(force: bool = False, verbose: bool = False, defines=()) -> str:
+    """defines: extra -D... flags (the tuning constants of csrc/common.cuh, e.g. -DVMAT_PRICE_MINB=5, and the
+    measurement switch -DVMAT_DIAG_NOGATHER of csrc/spmv.cuh); a build with any of them replaces libvmat.so until the
+    next plain build."""
+    if not force and not defines and not needs_build():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + sources()
+    cmd = [nvcc] + NVCC_FLAGS + list(defines) + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + sources()
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
     return LIB
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv,
+                defines=[a for a in sys.argv[1:] if a.startswith("-D")]))
