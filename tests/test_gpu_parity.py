@@ -332,3 +332,22 @@ def test_structure_id_contract_check(vm):
         vm.Objective(sid, t3, t3, t3).validate()
     assert e.value.status == -2
     vm.Objective(torch.zeros(0, dtype=torch.uint8, device=DEV), t3, t3, t3).validate()
+
+
+def test_schedule_setting_and_read_probe(vm, A0, h0):
+    """vmat_ddc_set_schedule: argument check, what info reports, the automatic choice on a tiny matrix (one CTA per item);
+    vmat_hbm_read_probe: runs, returns a plausible rate, rejects bad arguments."""
+    assert h0.info["sm_affine_dose"] == 0 and h0.info["sm_affine_price"] == 0          # config 0: a handful of items
+    g0 = (h0.info["grid_dose"], h0.info["grid_price"])
+    h0.set_schedule(True)
+    assert h0.info["sm_affine_dose"] == 1 and h0.info["sm_affine_price"] == 1
+    assert h0.info["grid_dose"] <= g0[0] and h0.info["grid_price"] <= g0[1]            # persistent grids never exceed the items
+    with pytest.raises(vm.VmatError):
+        h0.set_schedule(2)
+    h0.set_schedule(None)
+    assert h0.info["sm_affine_dose"] == 0 and (h0.info["grid_dose"], h0.info["grid_price"]) == g0
+    gbs = vm.vmat_hbm_read_probe(256 << 20, 5)
+    assert 500.0 < gbs < 20000.0, gbs
+    assert vm.last_launch_count() == 6                                                   # warm-up + 5 passes
+    with pytest.raises(vm.VmatError):
+        vm.vmat_hbm_read_probe(1000, 1)
