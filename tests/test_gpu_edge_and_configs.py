@@ -291,6 +291,36 @@ def test_config1_scaled_down(vm):
     _full_parity(vm, _phantom_on_gpu(1, scale=2.5), [1.0, 0.7])
 
 
+def test_sm_affine_queues_repeat_bit_for_bit(vm):
+    """The persistent kernels with per-SM queues on a matrix with many items per CTA (config 1 at 1.6x coarser voxels:
+    ~1e8 nnz, several thousand items against 1776 / 888 CTAs): 40 evaluations launched back to back without a host
+    synchronisation, alternating between two fluence vectors - whoever steals what at the tail, and however the
+    self-resetting counters are left, every evaluation of the same x gives the same bits, equal to one CTA per item."""
+    import paper_1503_01721_b200 as vmod
+    ph = _phantom_on_gpu(1, scale=1.6)
+    A = as_np(ph)
+    h = vmod.vmat_ddc_create(ph.n_voxels, ph.n_beamlets, ph.coo_voxel, ph.coo_beamlet, ph.coo_val,
+                             ph.angle_col_offset, ph.angle_row_offset, ph.leafrow_col_offset, device=DEV)
+    obj = obj_to_device(A, DEV)
+    xs = [synth.draw_x(ph.n_beamlets, 7 + k, scale=0.8 + 0.4 * k).to(DEV) for k in range(2)]
+    h.set_schedule(False)
+    ref = []
+    for x in xs:
+        o = h.alloc_outputs()
+        vmod.vmat_price_eval(h, x, obj, o)
+        ref.append(o)
+    h.set_schedule(True)
+    assert h.info["grid_dose"] < (h.info["n_dose_blocks"] + 3) // 4 and h.info["grid_price"] < (ph.n_beamlets + 7) // 8
+    outs = [h.alloc_outputs() for _ in range(40)]
+    for k, o in enumerate(outs):
+        vmod.vmat_price_eval(h, xs[k % 2], obj, o)                      # no synchronisation in between
+    torch.cuda.synchronize()
+    for k, o in enumerate(outs):
+        for f in OUT_FIELDS:
+            assert torch.equal(getattr(o, f), getattr(ref[k % 2], f)), (k, f)
+    h.close()
+
+
 def test_config1_full(vm):
     _full_parity(vm, _phantom_on_gpu(1), [1.0, 0.6])
 
