@@ -10,9 +10,11 @@
 //              range once, parks the products in its private slice of shared memory, then groups of
 //              G lanes (G sized to the segment's mean row length) reduce one row each with shuffles
 //              (pads hold 0 and belong to the row before them, so they change no sum).
-// No block-wide barrier sits in the hot path (the first version, one CTA per 4096-entry block, lost
-// 21 % of its issue slots to barrier stalls - profiles/).  Everything is FP32 with a fixed summation
-// order; the objective partials are FP64, one per CTA, summed afterwards in a fixed order (no atomics).
+// No block-wide barrier sits inside the streaming of a segment (the first version, one CTA per 4096-entry
+// block, lost 21 % of its issue slots to barrier stalls - profiles/).  Everything is FP32 with a fixed summation
+// order; the objective partials are FP64, one per ITEM (4 consecutive segments, the unit a CTA takes at a time),
+// summed afterwards in a fixed order (no atomics).  Items reach the CTAs either one CTA per item or, where items
+// are long and many, through per-SM queues drawn by a persistent grid (smqueue.cuh): same bits either way.
 #include "spmv.cuh"
 #include "smqueue.cuh"
 

@@ -5,9 +5,10 @@
 // so the paper's mapping holds on sm_100a: one warp per beamlet row (L127), here over lane-interleaved
 // 256-entry tiles read with 256-bit loads, with u16 index offsets where the layout allows (spmv.cuh).  Measured on B200 the warp-per-row kernel beats
 // a CTA-per-leaf-row kernel by 12 % (perfect balance, more independent streams), so the row selection
-// is fused differently: every CTA (8 consecutive beamlet rows) hands in tickets for the leaf rows it
-// priced, and the CTA whose ticket completes a leaf row selects that row's opening on the spot - the
-// selection costs no launch and no second pass over p, and the price kernel keeps its balance.
+// is fused differently: for every ITEM (8 consecutive beamlet rows, the unit a CTA takes at a time) the CTA
+// hands in tickets for the leaf rows it priced, and the CTA whose ticket completes a leaf row selects that
+// row's opening on the spot - the selection costs no launch and no second pass over p, and the price kernel
+// keeps its balance.  Items reach the CTAs one CTA per item or through the per-SM queues of smqueue.cuh.
 //
 // Selection arithmetic (readings C4-C6, C8): S_0 = 0, S_{c+1} = S_c + (double)p_c left to
 // right in FP64; candidates all 0 <= L <= R <= n with V = S_R - S_L; result = smallest (V, L, R).
