@@ -473,3 +473,87 @@ def test_config3_full_size_all_elements(vm):
           f"from the pure-FP64 path: {n_diff}; oracle passes {t_oracle:.0f} s, whole test {time.time() - t_start:.0f} s")
     assert n_diff <= L_ref.size // 1000
     h.close()
+
+
+def test_layout_beyond_2_32_stored_entries(vm):
+    """Maximum size: a layout of MORE THAN 2^32 stored entries (config 1 generator at 0.395 x the voxel / beamlet size:
+    ~4.6e9 non-zeros, ~27 GB per layout, 55 GB of triplets - built from host memory through the chunked path of the
+    ingest step when the device cannot hold the triplets next to the build).  Exercises the 64-bit padded positions,
+    the kernels' one-register cursor (units of 8 entries) past 2^32 entries and the price kernel's queues.
+    Sampled voxel rows and beamlet rows the oracle computes one by one from their own triplets (rows from the first, the
+    middle and the LAST 2^28 stored entries among them), the gradient and F of the sampled voxels, and the adjoint
+    identity on the whole vectors.  Skipped where the host or the device is too small."""
+    import paper_1503_01721_b200 as vmod
+    psutil = pytest.importorskip("psutil")
+    free_dev, _ = torch.cuda.mem_get_info()
+    if psutil.virtual_memory().available < 90e9 or free_dev < 130e9:
+        pytest.skip("needs ~60 GB of host memory for the triplets and ~130 GB on the device")
+    t0 = time.time()
+    ph = _phantom_on_gpu(1, scale=0.395)
+    n_v, n_b, nnz = ph.n_voxels, ph.n_beamlets, ph.nnz
+    assert nnz > (1 << 32), nnz
+    rng = np.random.default_rng(11)
+    # samples, and their triplets, taken while the COO is still on the device
+    cnt_v = torch.zeros(n_v, dtype=torch.int64, device=DEV)
+    CH = 1 << 28
+    for c0 in range(0, nnz, CH):
+        cnt_v += torch.bincount(ph.coo_voxel[c0:c0 + CH].long(), minlength=n_v)
+    nz_rows = torch.nonzero(cnt_v).flatten().cpu().numpy()
+    sv = np.unique(np.concatenate([rng.choice(nz_rows, 40, replace=False), nz_rows[:2], nz_rows[-3:],
+                                   [int(cnt_v.argmax()), nz_rows[nz_rows.size // 2]]]))
+    sb = np.unique(np.concatenate([rng.choice(n_b, 40, replace=False), [0, 1, n_b // 2, n_b - 2, n_b - 1]]))
+    mv = _entries_with_key(ph.coo_voxel, n_v, sv)
+    sub_v = [t[mv].cpu().numpy() for t in (ph.coo_voxel, ph.coo_beamlet, ph.coo_val)]
+    mb = _entries_with_key(ph.coo_beamlet, n_b, sb)
+    sub_b = [t[mb].cpu().numpy() for t in (ph.coo_voxel, ph.coo_beamlet, ph.coo_val)]
+    del mv, mb, cnt_v
+    A = dict(sid=ph.voxel_struct.numpy(), T=ph.struct_T.numpy(), wo=ph.struct_w_over.numpy(),
+             wu=ph.struct_w_under.numpy())
+    try:
+        h = vmod.vmat_ddc_create(n_v, n_b, ph.coo_voxel, ph.coo_beamlet, ph.coo_val, ph.angle_col_offset,
+                                 ph.angle_row_offset, ph.leafrow_col_offset, device=DEV)
+        how = "device"
+    except vmod.VmatError as e:
+        if e.status != -4:
+            raise
+        hv, hb, hw = ph.coo_voxel.cpu(), ph.coo_beamlet.cpu(), ph.coo_val.cpu()
+        ph.coo_voxel = ph.coo_beamlet = ph.coo_val = None
+        torch.cuda.empty_cache()
+        h = vmod.vmat_ddc_create(n_v, n_b, hv, hb, hw, ph.angle_col_offset, ph.angle_row_offset,
+                                 ph.leafrow_col_offset, device=DEV)
+        del hv, hb, hw
+        how = "host (chunked)"
+    ph.coo_voxel = ph.coo_beamlet = ph.coo_val = None
+    torch.cuda.empty_cache()
+    info = h.info
+    print(f"\n  built from {how} memory in {time.time() - t0:.0f} s: nnz {nnz}, stored {info['padded_d']} / {info['padded_dt']}, "
+          f"queues dose / price: {info['sm_affine_dose']} / {info['sm_affine_price']}")
+    assert info["padded_d"] > (1 << 32) and info["padded_dt"] > (1 << 32) and info["nnz"] == nnz
+    obj = obj_to_device(A, DEV)
+    out = h.alloc_outputs()
+    x = synth.draw_x(n_b, 5, scale=0.9)
+    vmod.vmat_price_eval(h, x.to(DEV), obj, out)
+    torch.cuda.synchronize()
+    d, g, p = out.d.cpu().numpy(), out.g.cpu().numpy(), out.p.cpu().numpy()
+    # sampled voxel rows (A1, A2): the oracle on the rows' own triplets
+    d_ref = oracle.dose(sub_v[0], sub_v[1], sub_v[2], n_v, x.numpy().astype(np.float64))[sv]
+    assert np.abs(d[sv] - d_ref).max() <= 1e-4 * float(np.abs(d).max())
+    assert np.linalg.norm(d[sv] - d_ref) <= REL_L2 * np.linalg.norm(d_ref)
+    _, g_ref = oracle.objective_grad(d_ref, A["sid"][sv], A["T"], A["wo"], A["wu"])
+    assert np.abs(g[sv] - g_ref).max() <= 1e-4 * float(np.abs(g).max())
+    # sampled beamlet rows (A3) on the GPU's own g
+    p_ref = oracle.price(sub_b[0], sub_b[1], sub_b[2], n_b, g.astype(np.float64))[sb]
+    assert np.abs(p[sb] - p_ref).max() <= 1e-4 * float(np.abs(p).max())
+    assert np.linalg.norm(p[sb] - p_ref) <= REL_L2 * np.linalg.norm(p_ref)
+    # F from the GPU's own d (every voxel): the oracle's O2
+    F_ref, g_all = oracle.objective_grad(d.astype(np.float64), A["sid"], A["T"], A["wo"], A["wu"])
+    assert abs(out.F.item() - F_ref) <= REL_L2 * F_ref
+    assert_vec_close("g", g, g_all)
+    # adjoint identity on the whole vectors: <D x, g> = <x, D^T g>
+    lhs = float(np.dot(d.astype(np.float64), g.astype(np.float64)))
+    rhs = float(np.dot(x.numpy().astype(np.float64), p.astype(np.float64)))
+    assert abs(lhs - rhs) <= 1e-5 * float(np.dot(np.abs(d).astype(np.float64), np.abs(g).astype(np.float64)))
+    # one CTA per item gives the same bits
+    _assert_schedules_agree(vm, h, x.to(DEV), obj, out)
+    print(f"  {sv.size} voxel rows and {sb.size} beamlet rows against the oracle, wall time {time.time() - t0:.0f} s")
+    h.close()
