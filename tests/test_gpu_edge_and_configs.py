@@ -411,6 +411,24 @@ def test_config3_full_size_sampled(vm):
     n_partial = int(((R - L) < np.diff(A["lco"])).sum())
     print(f"  selection: {n_open} open rows of {L.size}, {n_partial} not fully open, best control point {best}")
     assert n_open > 0 and n_partial > 0
+
+    # -- NEXT-1 at this size: the aperture dose vector DA = D 1_A (Eq. (5)) of the apertures just selected at three
+    #    control points (first arc, second arc with the rotated collimator, the best one), every voxel, against the
+    #    oracle's O1 on the control point's own triplets with the aperture's indicator as x
+    aco = ph.angle_col_offset.numpy()
+    xs, DA = torch.empty(n_b, dtype=torch.float32, device=DEV), torch.empty(n_v, dtype=torch.float32, device=DEV)
+    for a in sorted({17, 180 + 95, max(best, 0)}):
+        vmod.vmat_aperture_dose(h, a, out.L, out.R, xs, DA)
+        ind = np.zeros(n_b, np.float64)
+        for r in range(int(A["aro"][a]), int(A["aro"][a + 1])):
+            ind[A["lco"][r] + L[r]:A["lco"][r] + R[r]] = 1.0
+        assert np.array_equal(xs.cpu().numpy().astype(np.float64), ind)
+        m = _entries_with_key(ph.coo_beamlet, n_b, np.arange(aco[a], aco[a + 1]))
+        DA_ref = oracle.dose(ph.coo_voxel[m].cpu().numpy(), ph.coo_beamlet[m].cpu().numpy(), ph.coo_val[m].cpu().numpy(),
+                             n_v, ind)
+        del m
+        got = DA.cpu().numpy()
+        assert ind.sum() > 0 and np.abs(got - DA_ref).max() <= 2.0 ** -23 * max(float(np.abs(DA_ref).max()), 1e-30) * 1.01
     h.close()
 
 
