@@ -129,6 +129,27 @@ int vmat_objective_grad(const vmat_ddc *h, const float *d, const uint8_t *voxel_
                         const float *T, const float *w_over, const float *w_under,
                         float *g, double *F, void *stream);
 
+/* A2 once more, for callers that cannot allocate device memory: no handle, no cudaMalloc / cudaFree, no allocating
+ * library routine, neither in this call nor before it.  Meant for code that runs where an allocation is forbidden or
+ * impossible: a host application that gave the whole GPU to its own memory pool at start-up, a latency-bound control
+ * loop that must stay clear of the driver's allocation lock (cudaMalloc may wait for the whole device), a plug-in whose
+ * host forbids driver allocations once it is initialised.  vmat_objective_grad does not fit them because its scratch lives in a vmat_ddc, and vmat_ddc_create allocates.
+ *   Arguments and results are those of vmat_objective_grad with n_voxels passed in place of the handle; F and g are
+ * bit-identical to vmat_objective_grad's.  Works on the current device; enqueues two kernels on `stream`.
+ *   Scratch: the per-block FP64 partial sums of F sit in an array compiled into the library (256 KiB; every GPU that
+ * loads libvmat.so holds it until the process exits).  Hence the limit: n_voxels <= VMAT_OBJECTIVE_STATIC_MAX_VOXELS,
+ * beyond it the call returns VMAT_ERR_INVALID_ARG and vmat_last_error() names the limit.
+ *   First call on a device: looks up the array's device address (cudaGetSymbolAddress, no allocation) and keeps it.
+ * Make that first call outside any stream capture, e.g. once at start-up with n_voxels = 0.
+ *   Sharing: all calls on a device, from every thread and stream, use the same array.  Calls that follow one another on
+ * one stream are fine - each call overwrites every slot it later reads, so nothing has to be cleared and leftovers of
+ * an earlier call are never seen.  Two calls whose kernels may run at the same time (different streams, no event between
+ * them) race on the array and return a wrong F; order them yourself. */
+#define VMAT_OBJECTIVE_STATIC_MAX_VOXELS (1 << 23)
+int vmat_objective_grad_static(int32_t n_voxels, const float *d, const uint8_t *voxel_struct, int32_t n_struct,
+                               const float *T, const float *w_over, const float *w_under,
+                               float *g, double *F, void *stream);
+
 /* A3 beamlet prices p = D^T g, p_j = sum_i D_ij g_i (Eq. (3); "Pi = D^T g", L121; one warp per
  * beamlet row as in L127).  g dev [n_voxels] in, p dev [n_beamlets] out. */
 int vmat_price(const vmat_ddc *h, const float *g, float *p, void *stream);

@@ -35,6 +35,7 @@ EXPORTS = [
     "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained", "vmat_leaf_windows",
     "vmat_column_generation_ex", "vmat_price_select", "vmat_mp_reached_voxels", "vmat_mp_pass_geometry", "vmat_check_structure_ids", "vmat_best_pair", "vmat_merge_best",
     "vmat_price_eval_host_submit", "vmat_price_eval_host_wait", "vmat_ddc_set_schedule", "vmat_hbm_read_probe",
+    "vmat_objective_grad_static",
 ]
 
 
@@ -70,6 +71,7 @@ def load_library():
     lib.vmat_ddc_create_ex.argtypes = [ctypes.POINTER(vp), i32, i32, i64, vp, vp, vp, i32, vp, vp, vp, i32, vp]
     lib.vmat_dose.argtypes = [vp, vp, vp, vp]
     lib.vmat_objective_grad.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp, vp, vp]
+    lib.vmat_objective_grad_static.argtypes = [i32, vp, vp, i32, vp, vp, vp, vp, vp, vp]
     lib.vmat_price.argtypes = [vp, vp, vp, vp]
     lib.vmat_check_structure_ids.argtypes = [vp, i32, i32, vp]
     lib.vmat_select_apertures.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -279,6 +281,25 @@ def vmat_objective_grad(h: DDC, d: torch.Tensor, obj: Objective, g: torch.Tensor
         obj.n_struct, _ptr(obj.T, torch.float32, "cuda"), _ptr(obj.w_over, torch.float32, "cuda"),
         _ptr(obj.w_under, torch.float32, "cuda"), _ptr(g, torch.float32, "cuda", h.n_voxels),
         _ptr(F, torch.float64, "cuda", 1), _stream()))
+
+
+OBJECTIVE_STATIC_MAX_VOXELS = 1 << 23      # VMAT_OBJECTIVE_STATIC_MAX_VOXELS of include/vmat.h
+
+
+def vmat_objective_grad_static(d: torch.Tensor, obj: Objective, g: torch.Tensor, F: torch.Tensor):
+    """A2 for callers that may not allocate device memory (a host that pooled the whole GPU at start-up, a real-time
+    loop, a plug-in whose host forbids allocations after start-up): same F and g as vmat_objective_grad, bit for bit, but no
+    handle and no cudaMalloc anywhere on the path - the partial sums of F go to a 256 KiB array built into libvmat.so.
+    At most OBJECTIVE_STATIC_MAX_VOXELS voxels (VmatError beyond).  Runs on d's device; the first call on a device
+    looks up the array's address and should not happen inside a stream capture.  All calls share the array: keep them
+    on one stream or order them with events, overlapping calls corrupt F."""
+    n = int(d.numel())
+    with torch.cuda.device(d.device):
+        _check(load_library().vmat_objective_grad_static(
+            n, _ptr(d, torch.float32, "cuda"), _ptr(obj.voxel_struct, torch.uint8, "cuda", n), obj.n_struct,
+            _ptr(obj.T, torch.float32, "cuda"), _ptr(obj.w_over, torch.float32, "cuda"),
+            _ptr(obj.w_under, torch.float32, "cuda"), _ptr(g, torch.float32, "cuda", n),
+            _ptr(F, torch.float64, "cuda", 1), _stream()))
 
 
 def vmat_price(h: DDC, g: torch.Tensor, p: torch.Tensor):

@@ -17,6 +17,7 @@
 // are long and many, through per-SM queues drawn by a persistent grid (smqueue.cuh): same bits either way.
 #include "spmv.cuh"
 #include "smqueue.cuh"
+#include <mutex>
 
 // g_i and the voxel's term of F for dose v (Eq. (1); sign and factor 2: C1, C2)
 __device__ __forceinline__ float voxel_grad(float v, float T, float wo, float wu, double &f)
@@ -232,6 +233,81 @@ int vmat_launch_objective(const vmat_ddc *h, const float *d, const uint8_t *voxe
         VMAT_LAUNCH_CHECK();
     }
     k_sum_partials<<<1, SUM_THREADS, 0, st>>>(h->F_partial_obj, h->n_obj_blocks, F);
+    VMAT_LAUNCH_CHECK();
+    return VMAT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// vmat_objective_grad_static (include/vmat.h): A2 without a handle and without a single allocation.
+//
+// Who needs this: code that is not allowed to call cudaMalloc at the moment it wants F and g.  Examples are a treatment
+// planning host that hands the GPU's whole memory to its own pool at start-up, so that a later driver allocation fails
+// or eats into that pool's headroom; a real-time control loop that must not take the driver's allocation lock
+// (cudaMalloc can wait for all work on the device); and a plug-in whose host forbids driver allocations once it is
+// initialised.  The handle-based vmat_objective_grad cannot serve them: its scratch (one FP64 partial sum of F per block
+// of 256 voxels) belongs to a vmat_ddc, and vmat_ddc_create allocates.
+//
+// Here that scratch is the file-scope array below.  It is part of the library image: every GPU on which libvmat.so
+// gets loaded holds its 256 KiB from the moment the CUDA module is loaded until the process exits, whether this entry
+// point is ever called or not.  That is why the maximum is modest: VMAT_OBJECTIVE_STATIC_MAX_VOXELS = 2^23 voxels
+// (config 3 of BASELINE.json, the largest, has 1.24 million).
+//
+// In host code `g_static_F_partial` is only a host-side shadow of the symbol: handing that name to a kernel would give it
+// a host address.  The device address is asked for with cudaGetSymbolAddress, once per device, with that device current,
+// and kept in g_static_F_partial_dev[device]; the kernels get that pointer.
+static __device__ __align__(256) double g_static_F_partial[VMAT_OBJECTIVE_STATIC_MAX_VOXELS / OBJ_THREADS];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+static double *g_static_F_partial_dev[STATIC_MAX_DEVICES];   // device address of the array on device i; NULL = not set up
+static std::mutex g_static_mu;
+
+extern "C" int vmat_objective_grad_static(int32_t n_voxels, const float *d, const uint8_t *voxel_struct, int32_t n_struct,
+                                          const float *T, const float *w_over, const float *w_under, float *g, double *F,
+                                          void *stream)
+{
+    static_assert(VMAT_OBJECTIVE_STATIC_MAX_VOXELS % OBJ_THREADS == 0, "whole blocks");
+    if (n_voxels < 0 || !F || !T || !w_over || !w_under || (n_voxels > 0 && (!d || !voxel_struct || !g))) {
+        vmat_set_error("vmat_objective_grad_static: NULL argument or negative n_voxels");
+        return VMAT_ERR_INVALID_ARG;
+    }
+    if (n_struct < 1 || n_struct > 256) {
+        vmat_set_error("vmat_objective_grad_static: n_struct must be in 1..256");
+        return VMAT_ERR_INVALID_ARG;
+    }
+    if (n_voxels > VMAT_OBJECTIVE_STATIC_MAX_VOXELS) {
+        vmat_set_error("vmat_objective_grad_static: n_voxels = %d exceeds VMAT_OBJECTIVE_STATIC_MAX_VOXELS = %d, the size "
+                       "the built-in scratch was compiled for; use vmat_objective_grad (handle-owned scratch) instead",
+                       n_voxels, (int)VMAT_OBJECTIVE_STATIC_MAX_VOXELS);
+        return VMAT_ERR_INVALID_ARG;
+    }
+    int dev = -1;
+    VMAT_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) {
+        vmat_set_error("vmat_objective_grad_static: device ordinal %d beyond the %d this entry point keeps addresses for",
+                       dev, STATIC_MAX_DEVICES);
+        return VMAT_ERR_INVALID_ARG;
+    }
+    double *part = nullptr;
+    {   // set-up, first call on this device only: no allocation, just the address of the array on the current device
+        std::lock_guard<std::mutex> lk(g_static_mu);
+        if (!g_static_F_partial_dev[dev]) {
+            void *p = nullptr;
+            VMAT_CUDA(cudaGetSymbolAddress(&p, g_static_F_partial));
+            g_static_F_partial_dev[dev] = (double *)p;
+        }
+        part = g_static_F_partial_dev[dev];
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    g_vmat_launches = 0;
+    // Same two kernels, same block size and same summation order as vmat_objective_grad, hence the same bits.  Every
+    // slot k_sum_partials reads was written by k_objective in this very call, so nothing of the array has to start at
+    // zero and what an earlier (possibly larger) call left behind is never read.
+    const int n_blocks = (n_voxels + OBJ_THREADS - 1) / OBJ_THREADS;
+    if (n_blocks > 0) {
+        k_objective<<<n_blocks, OBJ_THREADS, 0, st>>>(n_voxels, d, voxel_struct, n_struct, T, w_over, w_under, g, part);
+        VMAT_LAUNCH_CHECK();
+    }
+    k_sum_partials<<<1, SUM_THREADS, 0, st>>>(part, n_blocks, F);
     VMAT_LAUNCH_CHECK();
     return VMAT_OK;
 }
