@@ -114,7 +114,11 @@ int vmat_ddc_info_get(const vmat_ddc *h, vmat_ddc_info *info /* host, out */);
 int vmat_ddc_export_csr(const vmat_ddc *h, int which, int64_t *ptr, int32_t *idx, float *val /* host, out */);
 
 /* A1 forward dose d = D x, d_i = sum_j D_ij x_j ("repeated forward dose
- * calculation", L27).  x dev [n_beamlets] in, d dev [n_voxels] out. */
+ * calculation", L27).  x dev [n_beamlets] in, d dev [n_voxels] out.
+ * The handle is const for the caller but holds scratch the launch writes (the reordered copy of x, the work-queue
+ * counters of the persistent schedule): as for every compute call, ONE launch per handle may be in flight at a time;
+ * two streams must be ordered with an event.  Overlapping launches give wrong or stale outputs without an error;
+ * vmat_ddc_set_schedule puts the queue counters back in order afterwards. */
 int vmat_dose(const vmat_ddc *h, const float *x, float *d, void *stream);
 
 /* A2 objective and gradient (Eq. (1); Eq. (4)):
@@ -151,7 +155,8 @@ int vmat_objective_grad_static(int32_t n_voxels, const float *d, const uint8_t *
                                float *g, double *F, void *stream);
 
 /* A3 beamlet prices p = D^T g, p_j = sum_i D_ij g_i (Eq. (3); "Pi = D^T g", L121; one warp per
- * beamlet row as in L127).  g dev [n_voxels] in, p dev [n_beamlets] out. */
+ * beamlet row as in L127).  g dev [n_voxels] in, p dev [n_beamlets] out.  One launch per handle in flight at a time
+ * (the work-queue counters and, in the fused calls, the leaf-row tickets belong to the handle; see vmat_dose). */
 int vmat_price(const vmat_ddc *h, const float *g, float *p, void *stream);
 
 /* Contract check for the objective arguments of every call that takes them: voxel_struct dev u8 [n_voxels] must hold
@@ -376,7 +381,9 @@ int vmat_ddc_set_profile_events(vmat_ddc *h, void *const *ev /* host [4] or NULL
  *   sm_affine = -1  (what vmat_ddc_create sets) per kernel, 1 where the layout has >= 16 items per resident CTA of
  *                   >= 64 KB each, else 0; vmat_ddc_info.sm_affine_dose / _price say which.
  * Every output is bit-identical under all settings (an item's sums have a fixed order).  Takes effect from the
- * next launch; not to be called while a launch on this handle is in flight. */
+ * next launch; not to be called while a launch on this handle is in flight.  Also zeroes the queue counters (they reset
+ * themselves after every completed launch; this repairs them after an aborted or overlapping one) and waits for that:
+ * synchronises the legacy default stream. */
 int vmat_ddc_set_schedule(vmat_ddc *h, int32_t sm_affine);
 
 /* Measurement aid (bench.py: roofline.read_only_stream): GB/s of a kernel that does nothing but read `bytes` of a

@@ -125,6 +125,36 @@ __global__ void k_max_u8(const uint8_t *__restrict__ v, int n, unsigned *__restr
     if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
 }
 
+// n device buffers, committed to their owners only when every one of them could be allocated: after a failure the
+// owners are as before (NULL), nothing leaks and *bytes is untouched, so the caller may simply try again later.
+static int alloc_all_or_none(void **const *dst, const size_t *bytes_each, int n, int64_t *bytes)
+{
+    void *tmp[8] = {nullptr};
+    size_t total = 0;
+    for (int i = 0; i < n; ++i) {
+        const cudaError_t e = cudaMalloc(&tmp[i], bytes_each[i]);
+        if (e != cudaSuccess) {
+            for (int k = 0; k < i; ++k) cudaFree(tmp[k]);
+            vmat_set_error("device allocation of %zu bytes failed: %s", bytes_each[i], cudaGetErrorString(e));
+            cudaGetLastError();
+            return e == cudaErrorMemoryAllocation ? VMAT_ERR_OOM : VMAT_ERR_CUDA;
+        }
+        total += bytes_each[i];
+    }
+    for (int i = 0; i < n; ++i) *dst[i] = tmp[i];
+    *bytes += (int64_t)total;
+    return VMAT_OK;
+}
+// d, g and p of the end-to-end host calls (shared by the synchronous and the two-slot variant)
+static int e2e_alloc_vectors(vmat_ddc *h)
+{
+    if (h->e2e_d) return VMAT_OK;
+    const size_t nv = h->n_voxels > 0 ? h->n_voxels : 1, nb = h->n_beamlets > 0 ? h->n_beamlets : 1;
+    void **const dst[] = {(void **)&h->e2e_d, (void **)&h->e2e_g, (void **)&h->e2e_p};
+    const size_t sz[] = {nv * 4, nv * 4, nb * 4};
+    return alloc_all_or_none(dst, sz, 3, &h->bytes_device);
+}
+
 extern "C" {
 
 const char *vmat_last_error(void) { return g_err; }
@@ -289,6 +319,14 @@ int vmat_ddc_set_schedule(vmat_ddc *h, int32_t sm_affine)
         h->sched_price = sm_affine_pays(h->Dt.bytes(), (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS, h->n_sm, 6, 64 * 1024);
     } else {
         h->sched_dose = h->sched_price = sm_affine;
+    }
+    // The queue counters reset themselves at the end of every launch that runs to completion (smqueue.cuh).  A launch
+    // that was cut short, or two launches that overlapped on this handle against the rule above, leave them non-zero,
+    // and every later persistent launch would then find its queues "empty" and write nothing.  No launch is in flight
+    // here by contract, so this is the place to put them back to zero.
+    if (h->q_next != nullptr) {
+        VMAT_CUDA(cudaMemsetAsync(h->q_next, 0, 2 * ((size_t)h->n_sm + 1) * 4, (cudaStream_t)0));
+        VMAT_CUDA(cudaStreamSynchronize((cudaStream_t)0));
     }
     return VMAT_OK;
 }
@@ -623,22 +661,15 @@ int vmat_price_eval_host(vmat_ddc *h, const float *x_host,
     REQUIRE(h->n_leaf_rows == 0 || (L_host && R_host && row_price_host), "NULL leaf-row output");
     REQUIRE(h->n_angles == 0 || angle_price_host, "angle_price_host is NULL");
     cudaStream_t st = (cudaStream_t)stream;
-    if (!h->e2e_F) {                                      // device scratch, allocated once
-        const size_t nv = h->n_voxels > 0 ? h->n_voxels : 1, nb = h->n_beamlets > 0 ? h->n_beamlets : 1;
+    if (!h->e2e_sync_ready) {                             // device scratch, allocated once: all of it or none of it
+        const size_t nb = h->n_beamlets > 0 ? h->n_beamlets : 1;
         const size_t nr = h->n_leaf_rows > 0 ? h->n_leaf_rows : 1, na = h->n_angles > 0 ? h->n_angles : 1;
-        VMAT_CUDA(cudaMalloc((void **)&h->e2e_x, nb * 4));
-        if (!h->e2e_d) {
-            VMAT_CUDA(cudaMalloc((void **)&h->e2e_p, nb * 4));
-            VMAT_CUDA(cudaMalloc((void **)&h->e2e_d, nv * 4));
-            VMAT_CUDA(cudaMalloc((void **)&h->e2e_g, nv * 4));
-        }
-        VMAT_CUDA(cudaMalloc((void **)&h->e2e_L, nr * 4));
-        VMAT_CUDA(cudaMalloc((void **)&h->e2e_R, nr * 4));
-        VMAT_CUDA(cudaMalloc((void **)&h->e2e_row_price, nr * 8));
-        VMAT_CUDA(cudaMalloc((void **)&h->e2e_angle_price, na * 8));
-        VMAT_CUDA(cudaMalloc((void **)&h->e2e_best, 4));
-        VMAT_CUDA(cudaMalloc((void **)&h->e2e_F, 8));
-        h->bytes_device += (int64_t)(8 * nb + 8 * nv + 16 * nr + 8 * na + 12);
+        TRY(e2e_alloc_vectors(h));
+        void **const dst[] = {(void **)&h->e2e_x, (void **)&h->e2e_L, (void **)&h->e2e_R, (void **)&h->e2e_row_price,
+                              (void **)&h->e2e_angle_price, (void **)&h->e2e_best, (void **)&h->e2e_F};
+        const size_t sz[] = {nb * 4, nr * 4, nr * 4, nr * 8, na * 8, 4, 8};
+        TRY(alloc_all_or_none(dst, sz, 7, &h->bytes_device));
+        h->e2e_sync_ready = true;
     }
     if (h->n_beamlets > 0)
         VMAT_CUDA(cudaMemcpyAsync(h->e2e_x, x_host, (size_t)h->n_beamlets * 4, cudaMemcpyHostToDevice, st));
@@ -671,30 +702,26 @@ int vmat_price_eval_host_submit(vmat_ddc *h, int32_t slot, const float *x_host,
     REQUIRE(h->n_angles == 0 || angle_price_host, "angle_price_host is NULL");
     REQUIRE(!h->slot[slot].in_flight, "the slot is still in flight: call vmat_price_eval_host_wait first");
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t nv = h->n_voxels > 0 ? h->n_voxels : 1, nb = h->n_beamlets > 0 ? h->n_beamlets : 1;
+    const size_t nb = h->n_beamlets > 0 ? h->n_beamlets : 1;
     const size_t nr = h->n_leaf_rows > 0 ? h->n_leaf_rows : 1, na = h->n_angles > 0 ? h->n_angles : 1;
-    if (!h->e2e_in) {                                     // streams, events and device scratch, allocated once
-        VMAT_CUDA(cudaStreamCreateWithFlags(&h->e2e_in, cudaStreamNonBlocking));
-        VMAT_CUDA(cudaStreamCreateWithFlags(&h->e2e_out, cudaStreamNonBlocking));
-        if (!h->e2e_d) {
-            VMAT_CUDA(cudaMalloc((void **)&h->e2e_d, nv * 4));
-            VMAT_CUDA(cudaMalloc((void **)&h->e2e_g, nv * 4));
-            VMAT_CUDA(cudaMalloc((void **)&h->e2e_p, nb * 4));
-            h->bytes_device += (int64_t)(8 * nv + 4 * nb);
-        }
+    if (!h->e2e_slots_ready) {                            // streams, events and device scratch, allocated once.  A
+        // failure part-way leaves the flag down: the next call creates what is still missing (every step below skips
+        // what exists) and never launches with a NULL stream, event or buffer.
+        if (!h->e2e_in) VMAT_CUDA(cudaStreamCreateWithFlags(&h->e2e_in, cudaStreamNonBlocking));
+        if (!h->e2e_out) VMAT_CUDA(cudaStreamCreateWithFlags(&h->e2e_out, cudaStreamNonBlocking));
+        TRY(e2e_alloc_vectors(h));
         for (auto &s : h->slot) {
-            VMAT_CUDA(cudaMalloc((void **)&s.x, nb * 4));
-            VMAT_CUDA(cudaMalloc((void **)&s.L, nr * 4));
-            VMAT_CUDA(cudaMalloc((void **)&s.R, nr * 4));
-            VMAT_CUDA(cudaMalloc((void **)&s.row_price, nr * 8));
-            VMAT_CUDA(cudaMalloc((void **)&s.angle_price, na * 8));
-            VMAT_CUDA(cudaMalloc((void **)&s.best, 4));
-            VMAT_CUDA(cudaMalloc((void **)&s.F, 8));
-            VMAT_CUDA(cudaEventCreateWithFlags(&s.x_ready, cudaEventDisableTiming));
-            VMAT_CUDA(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
-            VMAT_CUDA(cudaEventCreateWithFlags(&s.out_ready, cudaEventDisableTiming));
-            h->bytes_device += (int64_t)(4 * nb + 16 * nr + 8 * na + 12);
+            if (!s.F) {
+                void **const dst[] = {(void **)&s.x, (void **)&s.L, (void **)&s.R, (void **)&s.row_price,
+                                      (void **)&s.angle_price, (void **)&s.best, (void **)&s.F};
+                const size_t sz[] = {nb * 4, nr * 4, nr * 4, nr * 8, na * 8, 4, 8};
+                TRY(alloc_all_or_none(dst, sz, 7, &h->bytes_device));
+            }
+            if (!s.x_ready) VMAT_CUDA(cudaEventCreateWithFlags(&s.x_ready, cudaEventDisableTiming));
+            if (!s.done) VMAT_CUDA(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
+            if (!s.out_ready) VMAT_CUDA(cudaEventCreateWithFlags(&s.out_ready, cudaEventDisableTiming));
         }
+        h->e2e_slots_ready = true;
     }
     vmat_ddc::E2ESlot &s = h->slot[slot];
     // x of this slot was last read by the evaluation submitted two calls ago: its `done` event has long fired

@@ -5,6 +5,7 @@
 #include <stdio.h>
 #include <limits.h>
 #include <vector>
+#include <atomic>
 #include "../../include/vmat.h"
 #include "smqueue.cuh"
 // items a CTA takes per visit to its SM's queue (smqueue.cuh): one atomic per chunk.  Measured on B200 (config 3, dose
@@ -40,6 +41,26 @@ extern thread_local int g_vmat_launches;
             return VMAT_ERR_CUDA;                                                           \
         }                                                                                   \
     } while (0)
+
+// Resident CTAs per SM of a persistent kernel on the handle's device, asked once per (kernel instance, device) - not
+// once per process: a process may hold handles on GPUs (or MIG slices) of different size.  `table` is the calling
+// template instance's own static array, zero-initialised; a racing first call asks twice and stores the same value.
+constexpr int VMAT_MAX_DEVICES = 64;
+template <typename Kernel>
+static inline int vmat_resident_ctas(Kernel kernel, int threads, int device, std::atomic<int> *table)
+{
+    const bool cached = device >= 0 && device < VMAT_MAX_DEVICES;
+    int o = cached ? table[device].load(std::memory_order_relaxed) : 0;
+    if (o > 0) return o;
+    int cur = device;
+    cudaGetDevice(&cur);
+    if (cur != device) cudaSetDevice(device);                 // the occupancy query answers for the current device
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, kernel, threads, 0) != cudaSuccess) { o = 0; cudaGetLastError(); }
+    if (cur != device) cudaSetDevice(cur);
+    o = o > 0 ? o : 1;
+    if (cached) table[device].store(o, std::memory_order_relaxed);
+    return o;
+}
 
 // ------------------------------------------------------------------ one matrix layout on the device
 // A layout is a PADDED, GROUPED CSR (spmv.cuh): the rows are cut into segments (one warp each), every
@@ -155,6 +176,7 @@ struct vmat_ddc {
         bool in_flight = false;
     } slot[2];
     cudaStream_t e2e_in = nullptr, e2e_out = nullptr;
+    bool e2e_sync_ready = false, e2e_slots_ready = false;    // set last: every buffer / stream / event above exists
 };
 
 // ------------------------------------------------------------------ tuning constants

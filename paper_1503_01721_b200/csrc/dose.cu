@@ -165,13 +165,8 @@ template <bool FUSE, int FMT>
 static int dose_grid(const vmat_ddc *h)
 {
     if (h->queues_dose().nq == 0) return h->n_blocks;
-    static int occ = 0;                                               // per kernel instance
-    if (occ == 0) {
-        int o = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_dose<FUSE, FMT>, DOSE_THREADS, 0);
-        occ = o > 0 ? o : 1;
-    }
-    return min(h->n_blocks, h->n_sm * occ);
+    static std::atomic<int> occ[VMAT_MAX_DEVICES];                   // per kernel instance and device
+    return min(h->n_blocks, h->n_sm * vmat_resident_ctas(k_dose<FUSE, FMT>, DOSE_THREADS, h->device, occ));
 }
 int vmat_dose_grid(const vmat_ddc *h, bool fuse)
 {

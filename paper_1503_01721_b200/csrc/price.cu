@@ -323,13 +323,8 @@ static int price_grid(const vmat_ddc *h)
 {
     const int n_items = (h->n_beamlets + PRICE_WARPS - 1) / PRICE_WARPS;
     if (h->queues_price().nq == 0) return n_items;
-    static int occ = 0;                                               // per kernel instance
-    if (occ == 0) {
-        int o = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_price<SELECT, FMT, SKIP>, PRICE_THREADS, 0);
-        occ = o > 0 ? o : 1;
-    }
-    return min(n_items, h->n_sm * occ);
+    static std::atomic<int> occ[VMAT_MAX_DEVICES];                   // per kernel instance and device
+    return min(n_items, h->n_sm * vmat_resident_ctas(k_price<SELECT, FMT, SKIP>, PRICE_THREADS, h->device, occ));
 }
 int vmat_price_grid(const vmat_ddc *h)                                // of the fused price + selection launch
 {
