@@ -9,7 +9,8 @@ control point) on a fresh fluence vector x, through t
 
 Prints ONE JSON line (rank 0).  Multi-GPU: the path does not need a second GPU (BASELINE.json
 north_star), so N > 1 runs N independent replicas, one process per GPU ("replicas only", weak scaling).
-`--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded angle-block sample.
+`--impl reference` times the CPU oracle (oracle/) on the host cores: the whole matrix when K + W evaluations fit the time
+budget (the all-cores variant for config 3), else an evenly spaced sample of control points (angle blocks).
 """
 from __future__ import annotations
 
@@ -285,7 +286,9 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": 1.0 / t_med, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_med, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": spec.name, "evaluated": what, "sample_nnz": desc["nnz"], "fraction_of_matrix": frac},
+        "config": {"workload": spec.name, "n_voxels": int(A["n_v"]), "n_beamlets": int(A["n_b"]), "nnz": int(desc["nnz"]),
+                   "n_angles": int(desc["control_points"]), "n_leaf_rows": int(len(A["lco"]) - 1),
+                   "evaluated": what, "sample_nnz": desc["nnz"], "fraction_of_matrix": frac},
         "cpu_baseline": {"value": 1.0 / t_med, "unit": UNIT, "cores": n_thr, "kind": "oracle", "variant": ORACLE_KINDS[kind],
                          "sample": f"{what} of {spec.name}, {desc['nnz']} nnz; every step one whole evaluation O1-O5, "
                                    f"median of the {len(timed)} timed steps; measured, not extrapolated"},
@@ -465,7 +468,7 @@ def run_sharded(args):
     start.record()
     for k in range(K):
         best = sh.price_eval(xs[W + k], obj, out)
-        launches += 7                  # dose, objective + partial sum, price+select, angle price, best pair, merge
+        launches += sh.last_launches   # counted by the library: vmat_last_launch_count() after each of its five calls
     stop.record()
     barrier()
     best = sharded.best_to_host(best)                            # the only read of the merged result on the host
@@ -666,13 +669,9 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timing: K evaluations between two events, per-kernel events inside
+    # ---- device-resident timing: K evaluations between two events, nothing else on the stream (this is `value`)
     for k in range(W):
         vm.vmat_price_eval(h, xs[k], obj, out)
-    ev_k = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
-    for evs in ev_k:
-        for e in evs:
-            e.record()                                       # creates the underlying cudaEvent_t handles
     start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     sampler = ClockSampler(local)
@@ -682,18 +681,51 @@ def run_ours(args):
     launches = 0
     start.record()
     for k in range(K):
-        h.set_profile_events(ev_k[k])
         vm.vmat_price_eval(h, xs[W + k], obj, out)
         launches += vm.last_launch_count()
     stop.record()
     barrier()
-    clocks = sampler.stop() if rank == 0 else None
-    h.set_profile_events(None)
     elapsed_ms = start.elapsed_time(stop)
-    t_dose = np.array([e[0].elapsed_time(e[1]) for e in ev_k])
-    t_price = np.array([e[2].elapsed_time(e[3]) for e in ev_k])
     best_last = int(out.best_angle.item())
     F_last = float(out.F.item())
+
+    # ---- the same K evaluations once more with four events per step around the two streaming kernels (the roofline's
+    # per-launch durations; kept out of the loop above, where the event records cost 1-3 % on the small configs)
+    def kernel_pass(n, x_of):
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(n)]
+        for evs in ev:
+            for e in evs:
+                e.record()                                   # creates the underlying cudaEvent_t handles
+        for k in range(n):
+            h.set_profile_events(ev[k])
+            vm.vmat_price_eval(h, x_of(k), obj, out)
+        h.set_profile_events(None)
+        torch.cuda.synchronize()
+        return (np.array([e[0].elapsed_time(e[1]) for e in ev]), np.array([e[2].elapsed_time(e[3]) for e in ev]))
+
+    t_dose, t_price = kernel_pass(K, lambda k: xs[W + k])
+    clocks = sampler.stop() if rank == 0 else None
+
+    # ---- sustained leg ("200 consecutive evaluations"): evaluations back to back for at least
+    # --sustained-seconds of device time, so that the GPU reaches the state it runs this path in for a whole plan (on
+    # B200 the power cap, not the full clock of a 0.1-s burst); then, without a pause, a short pass with kernel events
+    sustained = None
+    if args.sustained_seconds > 0:
+        n_sus = min(max(K, int(np.ceil(args.sustained_seconds * 1e3 / max(elapsed_ms / K, 1e-3)))), 100000)
+        s_sampler = ClockSampler(local)
+        barrier()
+        if rank == 0:
+            s_sampler.start()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record()
+        for k in range(n_sus):
+            vm.vmat_price_eval(h, xs[k % len(xs)], obj, out)
+        s1.record()
+        n_kp = min(max(K, 20), 50)
+        sd, sp = kernel_pass(n_kp, lambda k: xs[k % len(xs)])
+        s_clocks = s_sampler.stop() if rank == 0 else None
+        sustained = {"steps": n_sus, "ms": s0.elapsed_time(s1), "t_dose": sd, "t_price": sp, "clocks": s_clocks,
+                     "kernel_pass_steps": n_kp}
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     # (vmat_price_eval_host_submit / _wait: two slots, so the copies of one evaluation overlap the kernels of the other;
@@ -764,6 +796,8 @@ def run_ours(args):
 
     # ---- max over ranks
     elapsed_ms, e2e_ms = reduce_max([elapsed_ms, e2e_ms], dist if use_dist else None, dev)
+    if sustained is not None:
+        sustained["ms"] = reduce_max([sustained["ms"]], dist if use_dist else None, dev)[0]
 
     if rank == 0:
         peak, peak_src = measured_peaks()
@@ -816,6 +850,9 @@ def run_ours(args):
             "e2e": {"value": aggregate(world, K, e2e_ms)["value"], "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / K,
                     "api": "vmat_price_eval_host_submit / _wait (two slots: copies overlap the other slot's kernels)",
+                    "copied_in": "x (pinned host, 4 n_beamlets bytes)",
+                    "copied_back": "F, L, R, row_price, angle_price, best_angle (what the consumer of the path reads); "
+                                   "d, g and p stay on the device",
                     "result_check": e2e_check,
                     "synchronous_call": {"value": world * K / (e2e_sync_ms * 1e-3), "ms_per_step": e2e_sync_ms / K,
                                          "api": "vmat_price_eval_host"}},
@@ -828,6 +865,20 @@ def run_ours(args):
             "kernels": [k_dose, k_price],
             "result_check": {"F_last": F_last, "best_angle_last": best_last},
         }
+        if sustained is not None:
+            s_ms = sustained["ms"] / sustained["steps"]
+            sd, sp = float(sustained["t_dose"].mean()), float(sustained["t_price"].mean())
+            line["sustained"] = {
+                "evals_per_s": world * sustained["steps"] / (sustained["ms"] * 1e-3), "ms_per_step": s_ms,
+                "seconds": sustained["ms"] * 1e-3, "steps": sustained["steps"],
+                "hbm_gbs": B_eval / (s_ms * 1e-3) / 1e9, "hbm_frac_of_measured": B_eval / (s_ms * 1e-3) / 1e9 / peak,
+                "kernels": [{"name": k_dose["name"], "ms": sd, "gbs": B_dose / (sd * 1e-3) / 1e9,
+                             "frac": B_dose / (sd * 1e-3) / 1e9 / peak},
+                            {"name": k_price["name"], "ms": sp, "gbs": B_price / (sp * 1e-3) / 1e9,
+                             "frac": B_price / (sp * 1e-3) / 1e9 / peak}],
+                "kernel_pass": f"{sustained['kernel_pass_steps']} evaluations with kernel events, enqueued right behind the "
+                               "sustained loop (same thermal / power state)",
+                "x": "the K + W seeded draws, cycled", "clocks": sustained["clocks"]}
         if mp_line is not None:
             mp_line["frac_of_measured"] = mp_line["gbs"] / peak
             line["master_problem"] = mp_line
@@ -862,6 +913,9 @@ def main():
                          "point over the ranks (NEXT-4)")
     ap.add_argument("--schedule", default="auto", choices=["auto", "sm-affine", "static"],
                     help="work distribution of the dose and price kernels (vmat_ddc_set_schedule)")
+    ap.add_argument("--sustained-seconds", type=float, default=3.0,
+                    help="after the K timed steps, run evaluations back to back for this long (device time) and report "
+                         "them as `sustained` (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-mp", action="store_true", help="skip the master-problem measurement")
     ap.add_argument("--mp-apertures", type=int, default=128)

@@ -27,7 +27,7 @@ from typing import List, Optional, Sequence
 
 import torch
 
-from . import (DDC, Objective, PriceEvalOut, vmat_best_pair, vmat_ddc_create, vmat_dose, vmat_merge_best,
+from . import (DDC, Objective, PriceEvalOut, last_launch_count, vmat_best_pair, vmat_ddc_create, vmat_dose, vmat_merge_best,
                vmat_objective_grad, vmat_price_select)
 
 
@@ -109,6 +109,7 @@ class ShardedDDC:
         self.n_angles_total, self.n_beamlets_total = n_angles_total, n_beamlets_total
         self.n_voxels = handle.n_voxels
         self._pair = None
+        self.last_launches = 0
 
     @classmethod
     def create(cls, n_voxels: int, n_beamlets: int, coo_voxel: torch.Tensor, coo_beamlet: torch.Tensor,
@@ -138,14 +139,20 @@ class ShardedDDC:
         point in global numbering or -1} after the second exchange; no host synchronisation (`best_to_host` reads it)."""
         dist = self._dist()
         vmat_dose(self.h, x_local, out.d)
+        n = last_launch_count()
         if dist is not None:
             dist.all_reduce(out.d, op=dist.ReduceOp.SUM, group=self.group)          # d = sum_m D_m x_m
         vmat_objective_grad(self.h, out.d, obj, out.g, out.F)
+        n += last_launch_count()
         vmat_price_select(self.h, out.g, out, angle_mask_local)
+        n += last_launch_count()
         if self._pair is None:
             self._pair = torch.empty(2, dtype=torch.float64, device=out.d.device)
         vmat_best_pair(self.h, out, self.block.angle_lo, self._pair)
-        return merge_best(self._pair, self.group)
+        n += last_launch_count()
+        best = merge_best(self._pair, self.group)
+        self.last_launches = n + last_launch_count()         # libvmat kernels of this evaluation (vmat_last_launch_count)
+        return best
 
     def close(self):
         self.h.close()

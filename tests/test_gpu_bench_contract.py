@@ -43,9 +43,17 @@ def test_json_line_of_both_arms():
     for section in ("master_problem", "plan_optimisation", "constrained_selection", "plan_optimisation_constrained"):
         assert section in ours, section
     assert ours["plan_optimisation"]["F_end"] < 0.01 * ours["plan_optimisation"]["F_start"]
+    sus = ours["sustained"]                                          # the steady-state leg behind the K timed steps
+    assert sus["steps"] >= 20 and sus["evals_per_s"] > 0 and sus["seconds"] > 0
+    assert abs(sus["evals_per_s"] * sus["ms_per_step"] * 1e-3 - 1.0) < 1e-6
+    assert len(sus["kernels"]) == 2 and all(k["ms"] > 0 and k["gbs"] > 0 for k in sus["kernels"])
+    assert {"sm_mhz", "sm_max_mhz", "reasons"} <= set(sus["clocks"])
+    assert "copied_back" in e2e
 
     ref = _run(["--impl", "reference", "--config", "0", "--steps", "3", "--warmup", "1"])
     assert ref["impl"] == "reference" and ref["metric"] == ours["metric"] and ref["unit"] == ours["unit"]
     assert ref["config"]["workload"] == ours["config"]["workload"] and ref["higher_is_better"] is True
     assert ref["e2e"] == {"value": ref["value"], "unit": ref["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert ref["cpu_baseline"]["kind"] == "oracle" and ref["cpu_baseline"]["value"] == ref["value"]
+    for key in ("n_voxels", "n_beamlets", "nnz", "n_angles", "n_leaf_rows"):        # the whole matrix: the GPU arm's sizes
+        assert ref["config"][key] == ours["config"][key], key

@@ -109,6 +109,26 @@ def test_merge_rule_on_the_device(vm):
         assert best.tolist() == want
 
 
+def test_merge_rule_on_random_candidate_lists(vm):
+    """vmat_merge_best against the A5 rule written out on the host (the aperture with the lowest
+    price; ties -> smallest control point; none below 0 -> {0, -1}) on seeded candidate lists of 1..64 ranks, prices
+    drawn from a few values so that ties across ranks are the rule, with ranks that report no candidate mixed in."""
+    rng = np.random.default_rng(20260306)
+    for case in range(300):
+        n = int(rng.integers(1, 65))
+        prices = rng.choice([-3.5, -1.25, -1.0, -0.5, -2.0 ** -40, 0.0], size=n)
+        cps = rng.permutation(4 * n)[:n].astype(np.float64)
+        none = (prices >= 0.0) | (rng.random(n) < 0.15)
+        prices[none], cps[none] = 0.0, -1.0
+        want = [0.0, -1.0]
+        for pr, k in zip(prices.tolist(), cps.tolist()):                 # the rule, one candidate at a time
+            if k >= 0 and pr < 0.0 and (pr < want[0] or (pr == want[0] and k < want[1])):
+                want = [pr, k]
+        best = torch.empty(2, dtype=torch.float64, device=DEV)
+        vm.vmat_merge_best(torch.from_numpy(np.stack([prices, cps], 1)).to(DEV).contiguous(), best)
+        assert best.tolist() == want, case
+
+
 def test_collective_path_on_one_gpu_with_nccl(tmp_path):
     """ShardedDDC.price_eval through a REAL torch.distributed process group of world size 1 with the nccl backend: the
     all-reduce of the dose and the all-gather of the candidates run (not the no-process-group bypass), and the result
