@@ -788,9 +788,11 @@ def run_ours(args):
         try:
             s_ = ClockSampler(local)
             s_.start()
-            gbs_ro = vm.vmat_hbm_read_probe(4 << 30, 40)
+            from paper_1503_01721_b200 import probe
+            gbs_ro, _ = probe.hbm_read_probe(4 << 30, 40)
             read_probe = {"gbs": gbs_ro, "bytes": 4 << 30, "passes": 40, "clocks": s_.stop(),
-                          "kernel": "vmat_hbm_read_probe: 256-bit L1::no_allocate loads, four per thread, nothing else"}
+                          "kernel": "vmat_hbm_read_probe (libvmat_probe.so, a bench aid outside the product library): "
+                                    "256-bit L1::no_allocate loads, four per thread, nothing else"}
         except Exception as e:
             read_probe = {"failed": f"{type(e).__name__}: {e}"[:200]}
 

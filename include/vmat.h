@@ -285,8 +285,9 @@ int vmat_leaf_windows(const vmat_ddc *h, const uint8_t *angle_mask, const int32_
  * its gradient entry zeroed; y is clipped into the box after every update; first step = exact line minimiser
  * of the current quadratic piece; iteration 1, 3, .. use Eq. (7), 2, 4, .. Eq. (8), the previous delta is kept
  * when <s,t> <= 0; z is recomputed as DA y every iteration.
- * The handle owns a dense voxel-major copy of the aperture dose vectors (float [n_voxels][max_apertures],
- * max_apertures <= 384; rows of voxels no aperture reaches are never read) and the FP64 iteration state; y persists between solves (warm start, as in the
+ * The handle owns a dense copy of the aperture dose vectors in blocks of 32 apertures, voxel-major inside a block
+ * (float [ceil(max_apertures / 32)][n_voxels rounded up to 16][32], max_apertures <= 384: one voxel's 32 coefficients
+ * of a block are one 128-byte line; rows of voxels no aperture reaches are never read) and the FP64 iteration state; y persists between solves (warm start, as in the
  * column-generation loop L56).  All sums are FP64 in a fixed order: results are deterministic. */
 typedef struct vmat_mp vmat_mp;
 int vmat_mp_create(vmat_mp **out, int32_t n_voxels, int32_t max_apertures, void *stream);
@@ -385,12 +386,6 @@ int vmat_ddc_set_profile_events(vmat_ddc *h, void *const *ev /* host [4] or NULL
  * themselves after every completed launch; this repairs them after an aborted or overlapping one) and waits for that:
  * synchronises the legacy default stream. */
 int vmat_ddc_set_schedule(vmat_ddc *h, int32_t sm_affine);
-
-/* Measurement aid (bench.py: roofline.read_only_stream): GB/s of a kernel that does nothing but read `bytes` of a
- * scratch buffer, `reps` times back to back, with the 256-bit streaming loads of the dose and price kernels - what a
- * READ-ONLY stream reaches on this device at the clock it runs at (MEASURED_PEAKS.json's hbm_gbs is a copy: read +
- * write).  Allocates and frees its buffer; synchronous.  gbs host [1] out. */
-int vmat_hbm_read_probe(int64_t bytes, int32_t reps, double *gbs, void *stream);
 
 /* Thread-local, static storage; never NULL. */
 const char *vmat_last_error(void);

@@ -19,7 +19,7 @@ from typing import Optional
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("VMAT_LIB", os.path.join(_HERE, "libvmat.so"))     # VMAT_LIB: load another build of libvmat
+LIB_PATH = os.path.join(_HERE, "libvmat.so")
 _lib = None
 
 VMAT_OK = 0
@@ -34,7 +34,7 @@ EXPORTS = [
     "vmat_mp_solve", "vmat_mp_history", "vmat_column_generation",
     "vmat_ddc_set_leaf_geometry", "vmat_select_apertures_constrained", "vmat_leaf_windows",
     "vmat_column_generation_ex", "vmat_price_select", "vmat_mp_reached_voxels", "vmat_mp_pass_geometry", "vmat_check_structure_ids", "vmat_best_pair", "vmat_merge_best",
-    "vmat_price_eval_host_submit", "vmat_price_eval_host_wait", "vmat_ddc_set_schedule", "vmat_hbm_read_probe",
+    "vmat_price_eval_host_submit", "vmat_price_eval_host_wait", "vmat_ddc_set_schedule",
     "vmat_objective_grad_static",
 ]
 
@@ -54,11 +54,17 @@ class _Info(ctypes.Structure):
         "sm_affine_dose", "sm_affine_price")]
 
 
-def load_library():
-    """Load libvmat.so (built in-tree by `python -m paper_1503_01721_b200.build`).  Raises if absent."""
-    global _lib
+def load_library(path: Optional[str] = None):
+    """Load libvmat.so (built in-tree by `python -m paper_1503_01721_b200.build`).  Raises if absent.
+    path: another build of the library (e.g. one made with tuning -D flags); only honoured by the first call of the
+    process, a later call with a different path raises."""
+    global _lib, LIB_PATH
     if _lib is not None:
+        if path is not None and os.path.abspath(path) != os.path.abspath(LIB_PATH):
+            raise RuntimeError(f"libvmat is already loaded from {LIB_PATH}")
         return _lib
+    if path is not None:
+        LIB_PATH = path
     if not os.path.exists(LIB_PATH):
         raise RuntimeError(f"{LIB_PATH} not found: build it with `python -m paper_1503_01721_b200.build` "
                            "(there is no CPU fallback)")
@@ -82,7 +88,6 @@ def load_library():
     lib.vmat_price_eval_host_wait.argtypes = [vp, i32]
     lib.vmat_ddc_set_profile_events.argtypes = [vp, vp]
     lib.vmat_ddc_set_schedule.argtypes = [vp, i32]
-    lib.vmat_hbm_read_probe.argtypes = [ctypes.c_int64, i32, vp, vp]
     f64 = ctypes.c_double
     lib.vmat_mp_create.argtypes = [ctypes.POINTER(vp), i32, i32, vp]
     lib.vmat_mp_destroy.argtypes = [vp]
@@ -573,14 +578,6 @@ def mp_pass_geometry(m: int, device="cuda:0") -> dict:
         return mp.pass_geometry(m)
     finally:
         mp.close()
-
-
-def vmat_hbm_read_probe(n_bytes: int, reps: int = 20) -> float:
-    """GB/s of a read-only stream over a scratch buffer of n_bytes (vmat_hbm_read_probe); needs a CUDA device."""
-    load_library()
-    gbs = ctypes.c_double(0.0)
-    _check(load_library().vmat_hbm_read_probe(int(n_bytes), int(reps), ctypes.byref(gbs), _stream()))
-    return float(gbs.value)
 
 
 def last_launch_count() -> int:

@@ -1,4 +1,5 @@
-"""Build libvmat.so in-tree with nvcc for sm_100a (B200).  `python -m paper_1503_01721_b200.build`."""
+"""Build libvmat.so (the product) and libvmat_probe.so (a measurement aid of bench.py, csrc/probe/) in-tree with nvcc
+for sm_100a (B200).  `python -m paper_1503_01721_b200.build`."""
 from __future__ import annotations
 
 import glob
@@ -9,6 +10,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvmat.so")
+PROBE_LIB = os.path.join(HERE, "libvmat_probe.so")
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
@@ -20,19 +22,24 @@ def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")))
 
 
+def probe_sources():
+    return sorted(glob.glob(os.path.join(CSRC, "probe", "*.cu")))
+
+
 def needs_build() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(PROBE_LIB):
         return True
-    t = os.path.getmtime(LIB)
-    deps = sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + \
-        [os.path.join(os.path.dirname(HERE), "include", "vmat.h")]
+    t = min(os.path.getmtime(LIB), os.path.getmtime(PROBE_LIB))
+    inc = os.path.join(os.path.dirname(HERE), "include")
+    deps = sources() + probe_sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + \
+        [os.path.join(inc, "vmat.h"), os.path.join(inc, "vmat_probe.h")]
     return any(os.path.getmtime(p) > t for p in deps)
 
 
 def build(force: bool = False, verbose: bool = False, defines=()) -> str:
-    """defines: extra -D... flags (the tuning constants of csrc/common.cuh, e.g. -DVMAT_PRICE_MINB=5, and the
-    measurement switch -DVMAT_DIAG_NOGATHER of csrc/spmv.cuh); a build with any of them replaces libvmat.so until the
-    next plain build."""
+    """defines: extra -D... flags (the tuning constants of csrc/common.cuh, e.g. -DVMAT_PRICE_MINB=5, and
+    -DVMAT_CHECKED: device-side asserts on every stream access and gathered index of the layout-walking kernels, see
+    MatView in csrc/common.cuh); a build with any of them replaces libvmat.so until the next plain build."""
     if not force and not defines and not needs_build():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
@@ -40,6 +47,9 @@ def build(force: bool = False, verbose: bool = False, defines=()) -> str:
     cmd = [nvcc] + NVCC_FLAGS + list(defines) + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + sources()
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
+    tmp = PROBE_LIB + f".tmp{os.getpid()}"
+    subprocess.check_call([nvcc] + NVCC_FLAGS + ["-o", tmp] + probe_sources())
+    os.replace(tmp, PROBE_LIB)
     return LIB
 
 

@@ -90,6 +90,7 @@ k_aperture_scatter(const int64_t *__restrict__ pptr, MatView A, int j_lo, int j_
     const int64_t s = pptr[j], e = pptr[j + 1];
     const int nt = (int)((e - s) >> 8);
     auto add = [&](float v, int vox) {
+        VMAT_ASSERT_INDEX(A, vox);
         if (v != 0.f) atomicAdd(acc + vox, (unsigned long long)__double2ll_rn((double)v * scale));
     };
     TileCursor<FMT> tc(A, s, lane);
@@ -182,56 +183,6 @@ int vmat_check_structure_ids(const uint8_t *voxel_struct, int32_t n_voxels, int3
     return VMAT_OK;
 }
 int vmat_last_launch_count(void) { return g_vmat_launches; }
-
-// ---------------------------------------------------------------- measurement aid: what a read-only stream reaches
-// The streaming kernels only READ the matrix, while the copy benchmark behind MEASURED_PEAKS.json reads and writes;
-// this kernel reads a buffer with the same 256-bit L1::no_allocate / L2::evict_first loads, four per thread, and
-// nothing else: the ceiling of the access pattern on this device at the clock it runs at.
-__global__ void __launch_bounds__(256) k_read_probe(const char *__restrict__ buf, size_t n32, uint32_t *__restrict__ sink)
-{
-    const size_t i = (size_t)blockIdx.x * 1024 + threadIdx.x;
-    if (i + 768 < n32) {
-        Vec8 r[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) r[u] = ld_stream_256(buf + (i + (size_t)u * 256) * 32);
-        uint32_t acc = 0;
-#pragma unroll
-        for (int u = 0; u < 4; ++u)
-#pragma unroll
-            for (int k = 0; k < 8; ++k) acc ^= r[u].w[k];
-        if (acc == 0x9e3779b9u) sink[0] = acc;                     // never true for a zeroed buffer: keeps the loads
-    }
-}
-
-int vmat_hbm_read_probe(int64_t bytes, int32_t reps, double *gbs, void *stream)
-{
-    REQUIRE(gbs != nullptr && reps >= 1 && bytes >= (int64_t)1 << 20, "gbs is NULL, reps < 1 or bytes < 1 MiB");
-    cudaStream_t st = (cudaStream_t)stream;
-    char *buf = nullptr;
-    uint32_t *sink = nullptr;
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    bytes &= ~(int64_t)32767;
-    VMAT_CUDA(cudaMalloc((void **)&buf, (size_t)bytes + 4));
-    sink = (uint32_t *)(buf + bytes);
-    auto cleanup = [&]() { if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); cudaFree(buf); };
-    cudaError_t e = cudaMemsetAsync(buf, 0, (size_t)bytes + 4, st);
-    if (e == cudaSuccess) e = cudaEventCreate(&e0);
-    if (e == cudaSuccess) e = cudaEventCreate(&e1);
-    const size_t n32 = (size_t)bytes / 32;
-    const unsigned grid = (unsigned)((n32 + 1023) / 1024);
-    g_vmat_launches = 0;
-    if (e == cudaSuccess) { k_read_probe<<<grid, 256, 0, st>>>(buf, n32, sink); ++g_vmat_launches; e = cudaEventRecord(e0, st); }   // warm-up
-    for (int r = 0; r < reps && e == cudaSuccess; ++r) { k_read_probe<<<grid, 256, 0, st>>>(buf, n32, sink); ++g_vmat_launches; }
-    if (e == cudaSuccess) e = cudaEventRecord(e1, st);
-    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
-    if (e == cudaSuccess) e = cudaGetLastError();
-    float ms = 0.f;
-    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
-    cleanup();
-    VMAT_CUDA(e);
-    *gbs = (double)bytes * reps / ((double)ms * 1e-3) / 1e9;
-    return VMAT_OK;
-}
 
 int vmat_ddc_destroy(vmat_ddc *h)
 {
@@ -416,6 +367,8 @@ int vmat_ddc_create_ex(vmat_ddc **out, int32_t n_voxels, int32_t n_beamlets, int
         }
     }
     if (rc == VMAT_OK) rc = vmat_build_layouts(h, coo_voxel, coo_beamlet, coo_val, index_bits, st);
+    h->D.n_sec = n_beamlets;
+    h->Dt.n_sec = n_voxels;
     if (rc == VMAT_OK) rc = build_sm_queues(h, st);
     if (rc == VMAT_OK) rc = vmat_ddc_set_schedule(h, -1);
     if (rc == VMAT_OK) rc = upload(&h->angle_col_offset, angle_col_offset, (int64_t)n_angles + 1, &h->bytes_device);

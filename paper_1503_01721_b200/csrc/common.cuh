@@ -79,6 +79,7 @@ struct PackedLayout {
     float *val = nullptr;     // [P (+pad)]
     void *sec = nullptr;      // narrow: uint16_t off[P (+pad)];  wide: int32_t idx[P (+pad)]
     int32_t *base = nullptr;  // narrow: [P/32 (+pad)];           wide: unused (NULL)
+    int32_t n_sec = 0;        // size of the secondary dimension (length of the vector the product gathers from)
     int64_t bytes() const     // device bytes of the streams a product reads (values + indices + padded row starts)
     {
         return index_bits == 16 ? 6 * P + 4 * (P / 32) + 8 * ((int64_t)n_rows + 1)
@@ -87,12 +88,33 @@ struct PackedLayout {
 };
 
 // Device view handed to the kernels.
+//
+// Checked build (`python -m paper_1503_01721_b200.build --force -DVMAT_CHECKED`; compute-sanitizer is not available on
+// the B200 pool this was developed on): the view also carries the layout's extent, and every stream access and every
+// gathered index of the kernels that walk a layout (k_dose, k_price, k_aperture_scatter) is asserted against it -
+// pads, tails after the last full tile and early-closed groups included.  A violation traps the kernel and the next
+// CUDA call returns cudaErrorAssert, which fails whatever test is running.  The normal build compiles none of it.
 struct MatView {
     const float *val;
     const void *sec;
     const int32_t *base;
+#ifdef VMAT_CHECKED
+    int64_t P;               // stored entries
+    int32_t n_sec;           // valid secondary indices are [0, n_sec)
+#endif
 };
+#ifdef VMAT_CHECKED
+#include <assert.h>
+static inline MatView view_of(const PackedLayout &A) { return MatView{A.val, A.sec, A.base, A.P, A.n_sec}; }
+#define VMAT_ASSERT_STREAM(A, first, n) assert((int64_t)(first) >= 0 && (int64_t)(first) + (int64_t)(n) <= (A).P)
+#define VMAT_ASSERT_INDEX(A, c) assert((unsigned)(c) < (unsigned)(A).n_sec)
+#define VMAT_ASSERT(cond) assert(cond)
+#else
 static inline MatView view_of(const PackedLayout &A) { return MatView{A.val, A.sec, A.base}; }
+#define VMAT_ASSERT_STREAM(A, first, n) ((void)0)
+#define VMAT_ASSERT_INDEX(A, c) ((void)0)
+#define VMAT_ASSERT(cond) ((void)0)
+#endif
 // kernel variant for a layout (spmv.cuh: FMT_WIDE 0, FMT_NARROW 1, FMT_NARROW_1BASE 2)
 static inline int fmt_of(const PackedLayout &A)
 {

@@ -81,6 +81,7 @@ k_dose(const int64_t *__restrict__ pptr, const MatView A, const int32_t *__restr
             } else {
                 // ---- several short rows: products into this warp's slice at their padded position k - s ...
                 float *wp = prod[warp];
+                VMAT_ASSERT(e - s <= DOSE_SEG_NNZ);                  // the run of short rows fits this warp's slice
                 const int nt = (int)((e - s) >> 8);
                 TileCursor<FMT> tc(A, s, lane);
 #pragma unroll 1
@@ -91,7 +92,10 @@ k_dose(const int64_t *__restrict__ pptr, const MatView A, const int32_t *__restr
                     tile_indices<FMT>(A, tc, tr, lane, c);
                     float *dst = wp + ti * TILE + lane;
 #pragma unroll
-                    for (int t = 0; t < 8; ++t) dst[32 * t] = __uint_as_float(tr.v.w[t]) * ld_gather(x + c[t]);
+                    for (int t = 0; t < 8; ++t) {
+                        VMAT_ASSERT_INDEX(A, c[t]);
+                        dst[32 * t] = __uint_as_float(tr.v.w[t]) * ld_gather(x + c[t]);
+                    }
                 }
                 const int64_t k0 = s + (int64_t)nt * TILE;
                 float *dst = wp + nt * TILE + lane;
@@ -108,6 +112,7 @@ k_dose(const int64_t *__restrict__ pptr, const MatView A, const int32_t *__restr
                     float acc = 0.f;
                     if (r < r1) {
                         const int b = (int)(pptr[r] - s), f = (int)(pptr[r + 1] - s);
+                        VMAT_ASSERT(0 <= b && b <= f && f <= (int)(e - s));
                         for (int k = b + gl; k < f; k += G) acc += wp[k];
                     }
                     for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);

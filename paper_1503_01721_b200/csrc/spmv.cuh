@@ -78,6 +78,7 @@ struct TileRegs {
 template <int FMT>
 __device__ __forceinline__ void tile_load(const MatView &A, const TileCursor<FMT> &tc, int lane, TileRegs<FMT> &r)
 {
+    VMAT_ASSERT_STREAM(A, (int64_t)tc.u * 8, 8);
     r.v = ld_stream_256(tc.v(A));
     if (FMT != FMT_WIDE) {
         const Vec4 o = ld_stream_128(tc.i(A));
@@ -121,10 +122,8 @@ __device__ __forceinline__ float tile_dot(const MatView &A, const TileCursor<FMT
 {
     int c[8];
     tile_indices<FMT>(A, tc, r, lane, c);
-#ifdef VMAT_DIAG_NOGATHER                      /* measurement only: every gather hits the same 128 bytes */
 #pragma unroll
-    for (int t = 0; t < 8; ++t) c[t] &= 31;
-#endif
+    for (int t = 0; t < 8; ++t) VMAT_ASSERT_INDEX(A, c[t]);
     float acc = 0.f;
 #pragma unroll
     for (int t = 0; t < 8; ++t) acc = fmaf(__uint_as_float(r.v.w[t]), ld_gather(vec + c[t]), acc);
@@ -135,9 +134,11 @@ __device__ __forceinline__ float tile_dot(const MatView &A, const TileCursor<FMT
 template <int FMT>
 __device__ __forceinline__ void group_entry(const MatView &A, int64_t kg, int lane, float &v, int &c)
 {
+    VMAT_ASSERT_STREAM(A, kg + lane, 1);
     v = ld_stream_f(A.val + kg + lane);
     if (FMT != FMT_WIDE) c = base_index(ld_stream_i(A.base + (kg >> 5))) + ld_stream_u16((const uint16_t *)A.sec + kg + lane);
     else        c = ld_stream_i((const int32_t *)A.sec + kg + lane);
+    VMAT_ASSERT_INDEX(A, c);
 }
 
 // The ngt (0..7) plain-order groups after the last full tile, starting at padded position k0:

@@ -37,6 +37,16 @@ def test_library_exports_every_declared_symbol(lib_path):
     assert lib.vmat_last_error() is not None
 
 
+def test_probe_library_is_separate(lib_path):
+    """The measurement aid of bench.py lives in its own library: libvmat exports nothing of it."""
+    from paper_1503_01721_b200 import build
+    assert os.path.exists(build.PROBE_LIB)
+    probe, lib = ctypes.CDLL(build.PROBE_LIB), ctypes.CDLL(lib_path)
+    assert hasattr(probe, "vmat_hbm_read_probe") and hasattr(probe, "vmat_probe_last_error")
+    assert not hasattr(lib, "vmat_hbm_read_probe")
+    assert probe.vmat_hbm_read_probe(ctypes.c_int64(10), 1, None, None, None) == -1     # rejected before any CUDA call
+
+
 def test_binding_lists_the_same_symbols(lib_path):
     import paper_1503_01721_b200 as vm
     assert sorted(vm.EXPORTS) == _declared_symbols()
