@@ -95,7 +95,7 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-NCU_CAPTURES = ["r2_ncu_full_cfg3_sm_affine.csv", "r2_ncu_full_cfg3.csv", "r1_ncu_full_cfg3_v6.csv",
+NCU_CAPTURES = ["r3_ncu_full_cfg2.csv", "r2_ncu_full_cfg3_sm_affine.csv", "r2_ncu_full_cfg3.csv", "r1_ncu_full_cfg3_v6.csv",
                 "r1_ncu_full_cfg3_v4.csv"]                                           # newest first
 
 
